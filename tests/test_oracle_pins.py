@@ -1,0 +1,402 @@
+"""Pins for the CPU oracle (no GPU).  Each test fixes the oracle to something other than itself:
+closed forms, scipy quadrature, brute force, invariances the mathematics demands.
+Citations: PAPER.md line numbers; readings R# are in DESIGN.md section 3."""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate, special
+
+import oracle as O
+
+C = 299792.458
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _gold():
+    rows = []
+    for line in open(os.path.join(GOLD, "survey_checks.txt")):
+        line = line.split("--")[0].strip()
+        if line and not line.startswith("#"):
+            p = line.split()
+            rows.append((p[0], [float(x) for x in p[1:]]))
+    return rows
+
+
+# ---------------------------------------------------------------- cosmology, Eq. 1
+@pytest.mark.parametrize("z", [1e-4, 0.01, 0.3, 1.0, 2.0, 7.5])
+def test_dL_closed_form_matter_only(z):
+    # Om = 1: d_L = 2c(1+z)(1-(1+z)^-1/2)/H0   (north_star closed form)
+    ref = 2 * C * (1 + z) * (1 - (1 + z) ** -0.5) / 70.0
+    assert O.dL(z, 70.0, 1.0) == pytest.approx(ref, rel=2e-15)
+
+
+@pytest.mark.parametrize("z", [1e-4, 0.01, 0.3, 1.0, 2.0, 7.5])
+def test_dL_closed_form_lambda_only(z):
+    # Om = 0 (Omega_Lambda = 1): d_L = c z (1+z)/H0
+    assert O.dL(z, 55.0, 0.0) == pytest.approx(C * z * (1 + z) / 55.0, rel=2e-15)
+
+
+@pytest.mark.parametrize("H0,Om,z", [(70, 0.3, 0.1), (70, 0.3, 1.0), (70, 0.3, 2.0), (67.4, 0.315, 1.0),
+                                     (20, 0.1, 1.5), (140, 0.5, 1.5), (200, 0.25, 0.02)])
+def test_dL_against_scipy_quad(H0, Om, z):
+    val, _ = integrate.quad(lambda x: 1.0 / math.sqrt(Om * (1 + x) ** 3 + 1 - Om), 0, z, epsabs=0, epsrel=1e-13)
+    assert O.dL(z, H0, Om) == pytest.approx((1 + z) * C / H0 * val, rel=1e-12)
+
+
+def test_golden_survey_values(theta0):
+    for kind, a in _gold():
+        if kind == "dL":
+            assert O.dL(a[0], a[1], a[2]) == pytest.approx(a[3], rel=1e-12)
+        elif kind == "u":
+            assert O.u_of_z(a[0], a[1]) == pytest.approx(a[2], rel=1e-12)
+        elif kind == "ddLdz":
+            z, H0, Om = a[:3]
+            h = 1e-5
+            fd = (O.dL(z + h, H0, Om) - O.dL(z - h, H0, Om)) / (2 * h)
+            assert fd == pytest.approx(a[3], rel=1e-8)
+        elif kind == "lnp":
+            m1, m2 = a[0], a[1]
+            assert math.log(O.p1(m1, theta0) * O.p2(m2, m1, theta0)) == pytest.approx(a[2], abs=2e-12)
+        elif kind == "npl":
+            assert O.norm_pl(theta0) == pytest.approx(a[0], rel=1e-11)
+        elif kind == "ng":
+            assert O.norm_g(theta0) == pytest.approx(a[0], rel=1e-11)
+        elif kind == "psi":
+            th = theta0.copy()
+            th[9:12] = a[1:4]
+            assert O.psi(a[0], th) == pytest.approx(a[4], rel=1e-12)
+
+
+@pytest.mark.parametrize("Om", [0.05, 0.3, 0.5, 1.0])
+def test_z_of_dL_round_trip_exact(Om):
+    for z in [1e-6, 0.003, 0.2, 0.9, 1.7, 4.0]:
+        for H0 in (20.0, 70.0, 200.0):
+            assert O.z_of_dL(O.dL(z, H0, Om), H0, Om) == pytest.approx(z, rel=1e-12, abs=1e-15)
+
+
+@pytest.mark.parametrize("Om,bound", [(0.3, 5e-11), (0.1, 2e-10), (0.5, 5e-11)])
+def test_hermite_table_nodes_and_error(Om, bound):
+    # reading R9: nodes are exact inverses; cubic Hermite error bounds measured in SURVEY 8c item 9
+    zt, dt, um = O.build_table(Om, 2.0, 1025)
+    assert zt[0] == 0.0 and zt[-1] == 2.0
+    assert np.all(np.diff(zt) > 0) and np.all(dt > 0)
+    du = um / 1024
+    for m in (1, 7, 300, 777, 1023):
+        assert O.u_of_z(zt[m], Om) == pytest.approx(m * du, rel=1e-13)
+        assert O.z_table(m * du, zt, dt, um) == pytest.approx(zt[m], abs=4e-15)  # exact at nodes
+        # slope: dz/du by central difference of the exact inverse
+        h = 1e-6
+        fd = (O.z_of_u(m * du + h, Om) - O.z_of_u(m * du - h, Om)) / (2 * h)
+        assert dt[m] / du == pytest.approx(fd, rel=1e-8)
+    rng = np.random.default_rng(1)
+    err = max(abs(O.z_table(u, zt, dt, um) - O.z_of_u(u, Om)) for u in rng.uniform(0, um, 1500))
+    assert err < bound
+    assert O.z_table(um, zt, dt, um) is None and O.z_table(1.5 * um, zt, dt, um) is None  # u >= umax dead (R11)
+
+
+# ---------------------------------------------------------------- population (readings R2-R4)
+@pytest.mark.parametrize("th_mod", [{}, {2: 1.5, 6: 25.0, 7: 2.0, 8: 0.1}, {2: 5.0, 6: 45.0, 7: 8.0, 8: 0.0},
+                                    {4: 4.6, 5: 86.3, 2: 2.9, 6: 30.7, 7: 6.3, 8: 0.4}])
+def test_p1_normalised(theta0, th_mod):
+    th = theta0.copy()
+    for k, v in th_mod.items():
+        th[k] = v
+    val, _ = integrate.quad(lambda m: O.p1(m, th), th[4], th[5], points=[th[6]], epsabs=0, epsrel=1e-12, limit=400)
+    assert val == pytest.approx(1.0, abs=1e-10)
+    assert O.p1(th[4], th) == 0.0 and O.p1(th[5], th) > 0.0 and O.p1(th[5] * (1 + 1e-15) + 1e-9, th) == 0.0  # R15
+
+
+@pytest.mark.parametrize("beta", [1.1, 0.0, -0.5, 4.0, -1.0])
+def test_p2_normalised(theta0, beta):
+    th = theta0.copy()
+    th[3] = beta
+    for m1 in (5.5, 30.0, 100.0):
+        val, _ = integrate.quad(lambda m: O.p2(m, m1, th), th[4], m1, epsabs=0, epsrel=1e-12)
+        assert val == pytest.approx(1.0, abs=1e-10)
+    assert O.p2(th[4], 30.0, th) > 0 and O.p2(30.0, 30.0, th) > 0 and O.p2(30.0001, 30.0, th) == 0.0  # R15
+
+
+def test_p1_lambda0_pure_power_law(theta0):
+    th = theta0.copy()
+    th[8] = 0.0
+    a, lo, hi = th[2], th[4], th[5]
+    for m in (5.1, 20.0, 99.0):
+        ref = (1 - a) / (hi ** (1 - a) - lo ** (1 - a)) * m ** (-a)
+        assert O.p1(m, th) == pytest.approx(ref, rel=1e-14)
+
+
+def test_p1_peak_term(theta0):
+    # lambda = 1: pure truncated Gaussian, compare against scipy's erf-normalised density
+    th = theta0.copy()
+    th[8] = 1.0
+    mu, s, lo, hi = th[6], th[7], th[4], th[5]
+    Z = 0.5 * (special.erf((hi - mu) / (s * math.sqrt(2))) - special.erf((lo - mu) / (s * math.sqrt(2))))
+    for m in (20.0, 35.0, 50.0):
+        ref = math.exp(-0.5 * ((m - mu) / s) ** 2) / (s * math.sqrt(2 * math.pi)) / Z
+        assert O.p1(m, th) == pytest.approx(ref, rel=1e-13)
+
+
+def test_rate(theta0):
+    assert O.psi(0.0, theta0) == pytest.approx(1.0, rel=1e-15)
+    # low-z slope gamma, high-z slope -kappa (Madau-Dickinson)
+    g, k, zp = theta0[9:12]
+    assert math.log(O.psi(1e-3, theta0)) / math.log1p(1e-3) == pytest.approx(g, abs=2e-2)
+    z1, z2 = 400.0, 800.0
+    slope = (math.log(O.psi(z2, theta0)) - math.log(O.psi(z1, theta0))) / (math.log1p(z2) - math.log1p(z1))
+    assert slope == pytest.approx(-k, abs=1e-3)
+
+
+def test_theta_domain(theta0):
+    assert O.theta_valid(theta0)
+    for idx, bad in [(0, 0.0), (0, -1.0), (1, 0.0), (1, 1.2), (7, 0.0), (4, 100.0), (4, -1.0), (8, -0.1), (8, 1.1),
+                     (2, float("nan"))]:
+        th = theta0.copy()
+        th[idx] = bad
+        assert not O.theta_valid(th)
+
+
+# ---------------------------------------------------------------- LOS interpolation (reading R10)
+def test_los_lerp():
+    rng = np.random.default_rng(3)
+    nz, zmax = 64, 1.5
+    zb = np.linspace(0, zmax, nz)
+    tab = np.stack([2.0 + 3.0 * zb, rng.uniform(0.1, 1, nz)])
+    for b in (0, 1, 17, 62):
+        assert O.los_lerp(tab, zmax, 1, zb[b]) == pytest.approx(tab[1, b], rel=1e-13)
+    for z in rng.uniform(0, zmax, 50):
+        assert O.los_lerp(tab, zmax, 0, z) == pytest.approx(2.0 + 3.0 * z, rel=1e-14)       # exact for linear
+        assert O.los_lerp(tab, zmax, 1, z) == pytest.approx(np.interp(z, zb, tab[1]), rel=1e-12)
+    t32 = tab.astype(np.float32)
+    for z in rng.uniform(0, zmax, 50):
+        assert O.los_lerp(t32, zmax, 1, z) == pytest.approx(O.los_lerp(tab, zmax, 1, z), rel=2.0 ** -23)
+    a = O.los_allsky(tab, zmax)
+    np.testing.assert_allclose(a, tab.mean(0), rtol=1e-15)
+
+
+# ---------------------------------------------------------------- LSE / N_eff (Eq. 8)
+def test_lse_properties():
+    rng = np.random.default_rng(5)
+    lw = rng.normal(-30, 3, 257)
+    l, n = O.lse(lw)
+    w = np.exp(lw)
+    assert l == pytest.approx(math.log(w.sum()), rel=1e-14)
+    assert n == pytest.approx(w.sum() ** 2 / (w ** 2).sum(), rel=1e-13)
+    l2, n2 = O.lse(rng.permutation(lw))
+    assert l2 == pytest.approx(l, rel=1e-15) and n2 == pytest.approx(n, rel=1e-13)
+    l3, n3 = O.lse(lw + 7.25)
+    assert l3 == pytest.approx(l + 7.25, rel=1e-15) and n3 == pytest.approx(n, rel=1e-13)
+    l4, n4 = O.lse(np.concatenate([lw, lw]))
+    assert l4 == pytest.approx(l + math.log(2), rel=1e-15) and n4 == pytest.approx(2 * n, rel=1e-13)
+    l5, n5 = O.lse(np.full(100, -3.0))
+    assert l5 == pytest.approx(-3.0 + math.log(100)) and n5 == pytest.approx(100.0)
+    l6, n6 = O.lse(np.array([0.0, -800.0, -900.0]))
+    assert l6 == pytest.approx(0.0, abs=1e-300) and n6 == pytest.approx(1.0)
+    l7, n7 = O.lse(np.full(4, -np.inf))
+    assert l7 == -np.inf and n7 == 0.0
+    l8, _ = O.lse(np.array([-np.inf, -2.0]))
+    assert l8 == pytest.approx(-2.0)
+    # far outside the range of a double in linear space
+    l9, _ = O.lse(np.array([-5000.0, -5000.0]))
+    assert l9 == pytest.approx(-5000.0 + math.log(2))
+
+
+# ---------------------------------------------------------------- whole weight: invariances
+def _toy_event(n=300, seed=11, zmax=1.5, nz=128, rows=4):
+    rng = np.random.default_rng(seed)
+    dl = 1500.0 * np.exp(0.25 * rng.standard_normal(n))
+    m1z = 45.0 * (1 + 0.08 * rng.standard_normal(n))
+    m2z = 33.0 * (1 + 0.08 * rng.standard_normal(n))
+    m1z, m2z = np.maximum(m1z, m2z), np.minimum(m1z, m2z)
+    row = np.sort(rng.integers(0, rows, n)).astype(np.int32)
+    tab = rng.uniform(0.2, 2.0, (rows, nz))
+    ev = dict(ev_sample_off=np.array([0, n // 3, n], dtype=np.int64), dL=dl, m1z=m1z, m2z=m2z, sample_row=row,
+              log_pe_prior=None)
+    return ev, tab, zmax
+
+
+@pytest.mark.parametrize("mode", [O.TABLE, O.EXACT])
+def test_H0_scaling_invariance(theta0, mode):
+    # Om fixed: (H0 -> s H0, dL -> dL/s) leaves z unchanged, adds 3 ln s to every live log w under the dL^2 prior
+    ev, tab, zmax = _toy_event()
+    s = 1.37
+    th2 = theta0.copy()
+    th2[0] *= s
+    ev2 = dict(ev, dL=ev["dL"] / s)
+    L1, n1, k1 = O.event_loglik(theta0, ev, tab, zmax, mode=mode)
+    L2, n2, k2 = O.event_loglik(th2, ev2, tab, zmax, mode=mode)
+    np.testing.assert_allclose(L2, L1 + 3 * math.log(s), rtol=0, atol=2e-12)
+    np.testing.assert_allclose(n2, n1, rtol=1e-11)
+    assert np.array_equal(k1, k2)
+    # with an explicit prior passed unchanged the shift is 1 ln s
+    lpe = 2 * np.log(ev["dL"])
+    L3, _, _ = O.event_loglik(th2, dict(ev2, log_pe_prior=lpe), tab, zmax, mode=mode)
+    np.testing.assert_allclose(L3, L1 + 1 * math.log(s), rtol=0, atol=2e-12)
+
+
+def test_padding_and_permutation_invariance(theta0):
+    # "padded indices do not contribute anything": zero-weight samples change log L_i by -log((S+p)/S)
+    ev, tab, zmax = _toy_event()
+    L1, n1, k1 = O.event_loglik(theta0, ev, tab, zmax)
+    n = ev["dL"].size
+    pad = 57
+    ev2 = dict(ev_sample_off=np.array([0, n // 3, n + pad], dtype=np.int64),
+               dL=np.concatenate([ev["dL"], np.full(pad, 1e7)]),          # beyond the z table: dead (R11)
+               m1z=np.concatenate([ev["m1z"], np.full(pad, 40.0)]), m2z=np.concatenate([ev["m2z"], np.full(pad, 30.0)]),
+               sample_row=np.concatenate([ev["sample_row"], np.zeros(pad, np.int32)]), log_pe_prior=None)
+    L2, n2, k2 = O.event_loglik(theta0, ev2, tab, zmax)
+    S1 = n - n // 3
+    assert L2[0, 0] == pytest.approx(L1[0, 0], abs=1e-13)
+    assert L2[0, 1] == pytest.approx(L1[0, 1] - math.log((S1 + pad) / S1), abs=1e-12)
+    assert n2[0, 1] == pytest.approx(n1[0, 1], rel=1e-12) and k2[0, 1] == k1[0, 1]
+    # permutation of the samples inside an event
+    rng = np.random.default_rng(0)
+    p = np.concatenate([rng.permutation(n // 3), n // 3 + rng.permutation(S1)])
+    ev3 = dict(ev, dL=ev["dL"][p], m1z=ev["m1z"][p], m2z=ev["m2z"][p], sample_row=ev["sample_row"][p])
+    L3, n3, k3 = O.event_loglik(theta0, ev3, tab, zmax)
+    np.testing.assert_allclose(L3, L1, rtol=0, atol=1e-12)
+    assert np.array_equal(k3, k1)
+
+
+def test_dead_samples_and_bad_theta(theta0):
+    ev, tab, zmax = _toy_event()
+    ev = dict(ev)
+    n = ev["dL"].size
+    a = n // 3
+    # every way a sample can be dead: none may give NaN or touch memory out of range
+    ev["dL"] = ev["dL"].copy(); ev["m1z"] = ev["m1z"].copy(); ev["m2z"] = ev["m2z"].copy()
+    ev["sample_row"] = ev["sample_row"].copy()
+    ev["dL"][0] = np.nan; ev["dL"][1] = -5.0; ev["m1z"][2] = np.inf; ev["m2z"][3] = 0.0
+    ev["sample_row"][4] = -1; ev["sample_row"][5] = 99; ev["m1z"][6] = 1.0; ev["m1z"][7] = 1e4; ev["dL"][8] = 1e9
+    L, ne, k = O.event_loglik(theta0, ev, tab, zmax)
+    assert np.all(np.isfinite(L)) and k[0, 0] <= a - 9
+    # all dead => -inf, N_eff 0, and the total is -inf, never NaN
+    ev["m1z"][:a] = 1.0
+    L, ne, k = O.event_loglik(theta0, ev, tab, zmax)
+    assert L[0, 0] == -np.inf and ne[0, 0] == 0.0 and k[0, 0] == 0 and np.isfinite(L[0, 1])
+    tot = O.total_from_parts(L, np.array([-3.0]))
+    assert tot[0] == -np.inf
+    bad = theta0.copy(); bad[7] = -1.0
+    L, ne, k = O.event_loglik(np.stack([theta0, bad]), ev, tab, zmax)
+    assert np.all(np.isnan(L[1])) and not np.any(np.isnan(L[0]))
+    assert np.isnan(O.total_from_parts(L, np.array([-3.0, -3.0]))[1])
+
+
+def test_table_vs_exact_mode(theta0):
+    ev, tab, zmax = _toy_event(n=600)
+    for H0 in (40.0, 70.0, 110.0):
+        th = theta0.copy(); th[0] = H0
+        Lt, _, kt = O.event_loglik(th, ev, tab, zmax, mode=O.TABLE)
+        Le, _, ke = O.event_loglik(th, ev, tab, zmax, mode=O.EXACT)
+        np.testing.assert_allclose(Lt, Le, rtol=0, atol=3e-10)     # Hermite M=1025 (<= 3e-11 measured)
+        assert np.array_equal(kt, ke)
+
+
+def test_total_composition():
+    # Eq. 3: log L = sum_i log L_i - N_det log xi
+    L = np.array([[-1.0, -2.0, -3.5], [0.5, 0.25, -0.125]])
+    xi = np.array([-4.0, 2.0])
+    np.testing.assert_allclose(O.total_from_parts(L, xi), [-6.5 + 12.0, 0.625 - 6.0], rtol=1e-15)
+
+
+# ---------------------------------------------------------------- whole estimator: Monte-Carlo toy vs quadrature
+def test_mc_estimator_converges_to_source_frame_quadrature(theta0):
+    """north_star's 1-event toy.  Samples ~ g(dL) g1(m1z) g2(m2z) (posterior under the dL^2 prior).  The estimator
+    (1/S) sum w must converge to I = int dz R(z) p_los(z) g_d(dL(z))/dL(z)^2 int dm1 p1 g1(m1(1+z)) int dm2 p2 g2(m2(1+z)),
+    written in SOURCE-frame coordinates: it contains no Jacobian, so it checks J's form and direction (Eq. 7, R6)."""
+    rng = np.random.default_rng(2024)
+    S = 400_000
+    mu_d, s_d = math.log(2000.0), 0.2
+    dl = np.exp(mu_d + s_d * rng.standard_normal(S))
+    m1z = 45.0 + 2.25 * rng.standard_normal(S)
+    m2z = 36.0 + 1.8 * rng.standard_normal(S)
+    zmax, nz = 1.5, 512
+    zb = np.linspace(0, zmax, nz)
+    row = 0.4 + 0.3 * np.sin(5 * zb) + 2.0 * np.exp(-0.5 * ((zb - 0.38) / 0.02) ** 2)   # a galaxy spike on a smooth floor
+    tab = row[None, :].copy()
+    ev = dict(ev_sample_off=np.array([0, S], dtype=np.int64), dL=dl, m1z=m1z, m2z=m2z,
+              sample_row=np.zeros(S, np.int32), log_pe_prior=None)
+    L, neff, nlive = O.event_loglik(theta0, ev, tab, zmax, mode=O.EXACT)
+    mc = math.exp(L[0, 0])
+    stderr_rel = math.sqrt(1.0 / neff[0, 0] - 1.0 / S)
+
+    H0, Om = theta0[0], theta0[1]
+    norm = lambda x, m, s: np.exp(-0.5 * ((x - m) / s) ** 2) / (s * math.sqrt(2 * math.pi))
+    xg, wg = np.polynomial.legendre.leggauss(48)
+
+    def gl(f, a, b):
+        return 0.5 * (b - a) * sum(w * f(0.5 * (b - a) * x + 0.5 * (a + b)) for x, w in zip(xg, wg))
+
+    def mass_int(z):
+        x = 1 + z
+        lo1, hi1 = max(theta0[4], (45 - 7 * 2.25) / x), min(theta0[5], (45 + 7 * 2.25) / x)
+
+        def inner(m1):
+            lo2, hi2 = max(theta0[4], (36 - 7 * 1.8) / x), min(m1, (36 + 7 * 1.8) / x)
+            if hi2 <= lo2:
+                return 0.0
+            return O.p1(m1, theta0) * norm(m1 * x, 45.0, 2.25) * gl(lambda m2: O.p2(m2, m1, theta0) * norm(m2 * x, 36.0, 1.8), lo2, hi2)
+        return gl(inner, lo1, hi1) if hi1 > lo1 else 0.0
+
+    def zint(z):
+        d = O.dL(z, H0, Om)
+        gd = math.exp(-0.5 * ((math.log(d) - mu_d) / s_d) ** 2) / (d * s_d * math.sqrt(2 * math.pi))
+        return O.psi(z, theta0) / (1 + z) * np.interp(z, zb, row) * gd / d ** 2 * mass_int(z)
+
+    # d_L ~ 2000 Mpc e^{+-6*0.2} maps to z in about [0.12, 1.0]; split at the spike for accuracy
+    I = sum(gl(zint, a, b) for a, b in [(0.10, 0.30), (0.30, 0.36), (0.36, 0.40), (0.40, 0.46), (0.46, 0.7), (0.7, 1.2)])
+    zscore = (mc - I) / (I * stderr_rel)
+    assert abs(zscore) < 4.0, (mc, I, stderr_rel)
+    assert stderr_rel < 5e-3
+
+
+# ---------------------------------------------------------------- selection closed form
+def test_selection_constant_weights(theta0):
+    """Injections drawn exactly from the model at theta_0 (density ∝ p_pop R pbar in source coordinates, transformed to
+    detector coordinates) have equal weights Z0 => xi = Z0 n_found/n_draw, N_eff = n_found (Eq. 4)."""
+    rng = np.random.default_rng(9)
+    zmax, nz = 1.5, 256
+    zb = np.linspace(0, zmax, nz)
+    allsky = 0.3 + zb ** 2 * np.exp(-2 * zb)
+    # z from pz ∝ psi/(1+z) * pbar on [0, zmax), tabulated inverse CDF on a fine grid
+    zf = np.linspace(0, zmax * (1 - 1e-9), 20001)
+    dens = np.array([O.psi(z, theta0) for z in zf]) / (1 + zf) * np.interp(zf, zb, allsky)
+    cdf = np.concatenate([[0], np.cumsum(0.5 * (dens[1:] + dens[:-1]) * np.diff(zf))])
+    Z0 = cdf[-1]
+    n = 3000
+    z = np.interp(rng.uniform(0, 1, n), cdf / Z0, zf)
+    # masses: anything inside the support; the proposal density is the model's own, so it cancels
+    m1 = rng.uniform(6, 90, n)
+    m2 = theta0[4] + (m1 - theta0[4]) * rng.uniform(0, 1, n)
+    H0, Om = theta0[0], theta0[1]
+    dl = np.array([O.dL(zz, H0, Om) for zz in z])
+    h = 1e-6
+    ddl = np.array([(O.dL(zz + h, H0, Om) - O.dL(zz - h, H0, Om)) / (2 * h) for zz in z])   # Jacobian by finite difference
+    pz = np.interp(z, zf, dens)   # un-normalised: weights come out equal to exactly 1
+    lp = np.log(pz) + np.log([O.p1(a, theta0) * O.p2(b, a, theta0) for a, b in zip(m1, m2)]) - 2 * np.log1p(z) - np.log(ddl)
+    inj = dict(dL=dl, m1z=m1 * (1 + z), m2z=m2 * (1 + z), log_pdraw=lp, n_draw=7.0 * n)
+    logxi, neff = O.selection_logxi(theta0, inj, allsky, zmax, mode=O.EXACT)
+    assert logxi[0] == pytest.approx(math.log(n / (7.0 * n)), abs=2e-6)     # finite-difference Jacobian + grid interp
+    assert neff[0] == pytest.approx(n, rel=1e-8)
+
+
+# ---------------------------------------------------------------- A0 packing (integer, bit-exact)
+def test_pack_events_against_lexsort():
+    rng = np.random.default_rng(4)
+    n, ne = 5000, 13
+    eid = rng.integers(0, ne, n).astype(np.int32)
+    eid[eid == 7] = 6                              # an empty event
+    row = rng.integers(0, 40, n).astype(np.int32)
+    out = O.pack_events(eid, row, ne)
+    perm = np.lexsort((np.arange(n), row, eid))     # stable by construction
+    assert np.array_equal(out["perm"], perm)
+    assert np.array_equal(out["ev_sample_off"], np.concatenate([[0], np.cumsum(np.bincount(eid, minlength=ne))]))
+    pairs = np.unique(np.stack([eid, row], 1), axis=0)
+    assert out["n_pixrefs"] == len(pairs)
+    assert np.array_equal(out["ev_pix_rows"], pairs[:, 1])
+    assert np.array_equal(out["ev_pix_off"], np.concatenate([[0], np.cumsum(np.bincount(pairs[:, 0], minlength=ne))]))
+    se, sr = eid[perm], row[perm]
+    starts = np.flatnonzero(np.concatenate([[True], (se[1:] != se[:-1]) | (sr[1:] != sr[:-1])]))
+    assert np.array_equal(out["pix_sample_off"], np.concatenate([starts, [n]]))
+    assert out["ev_sample_off"][7] == out["ev_sample_off"][8]
