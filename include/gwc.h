@@ -1,0 +1,184 @@
+/*
+ * gwc.h -- C ABI of the B200-native dark-siren hierarchical likelihood (libgwc.so).
+ *
+ * The operation is the one stated in arxiv/paper_2605_23538, evaluated for a BATCH of
+ * hyper-parameter points theta (the paper's Lambda):
+ *
+ *   log L(theta) = sum_i log L_i(theta) - N_det * log xi(theta)          Eq. 3
+ *   L_i   = (1/S_i) sum_k w_ik,  w = p(z, m1, m2 | theta) p(z | pixel) / (J pi_PE)   Eq. 5, 7, :77-91
+ *   xi    = (1/N_draw) sum_j w_j over found injections, all-sky p(z)      Eq. 4
+ *   N_eff = (sum w)^2 / sum w^2                                           Eq. 8
+ *   z from d_L through flat-LambdaCDM Eq. 1, inverted by a per-theta table.
+ *
+ * The line-of-sight prior is read at each sample's own redshift (direct Monte-Carlo sum, the
+ * zero-bandwidth limit of the KDE of Eq. 6; reading R1).  The power-law+peak mass law,
+ * the Madau-Dickinson rate, the Jacobian and the table scheme are DESIGN.md readings R2-R9.
+ *
+ * Conventions
+ *  - Plain C ABI; no exception crosses it.  Every function returns a gwc_status; gwc_last_error()
+ *    gives text for the last non-OK status of that context.
+ *  - Pointers named d_* are DEVICE pointers owned by the caller (e.g. PyTorch tensors); h_* are HOST
+ *    pointers.  The library never frees caller memory and keeps no reference to it after a call
+ *    returns (work already enqueued on the stream still reads it: keep it alive until you sync).
+ *  - All work is enqueued on the CUDA stream given to gwc_create and is asynchronous unless stated.
+ *    Scratch memory lives in the context and only grows (cudaMalloc happens when a size grows).
+ *  - Argument errors that the host can see are returned synchronously.  theta-domain violations
+ *    (H0<=0, Om not in (0,1], sigma<=0, mmin<=0, mmin>=mmax, lambda not in [0,1], zp<=-1, any
+ *    non-finite value, |alpha-1|<1e-6, |beta+1|<1e-6) make that theta's outputs NaN and raise a
+ *    sticky device flag that gwc_check() reports as GWC_ERR_DOMAIN.  They are the only source of NaN.
+ *    -inf is a legal output (no live sample).
+ *  - Units: d_L in Mpc, masses in solar masses (detector frame), H0 in km/s/Mpc.
+ *  - Results are deterministic: no floating-point atomics, every reduction has a fixed order.
+ *  - Range: linear-domain accumulation in FP64; every log-weight must lie in about [-700, 700]
+ *    (true of any physical input; weights below e^-700 count as e^-700).
+ */
+#ifndef GWC_H_
+#define GWC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GWC_NPAR 12 /* theta row: H0, Om, alpha, beta, mmin, mmax, mu, sigma, lambda, gamma, kappa, zp */
+
+typedef enum {
+  GWC_OK = 0,
+  GWC_ERR_INVALID_ARG = 1,
+  GWC_ERR_SHAPE = 2,
+  GWC_ERR_DOMAIN = 3,
+  GWC_ERR_NOT_BUILT = 4,
+  GWC_ERR_NOMEM = 5,
+  GWC_ERR_CUDA = 6
+} gwc_status;
+
+typedef enum { GWC_F64 = 0, GWC_F32 = 1 } gwc_prec;
+
+typedef struct gwc_ctx gwc_ctx;
+
+/* Create a context on CUDA device `device`; `cuda_stream` is a cudaStream_t (NULL = default stream). */
+gwc_status gwc_create(gwc_ctx** ctx, int device, void* cuda_stream);
+void gwc_destroy(gwc_ctx* ctx);
+/* Synchronise the stream and report sticky device errors (GWC_ERR_DOMAIN, GWC_ERR_CUDA); clears the flag. */
+gwc_status gwc_check(gwc_ctx* ctx);
+const char* gwc_last_error(const gwc_ctx* ctx);
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
+int64_t gwc_launch_count(const gwc_ctx* ctx);
+
+/*
+ * A1 + A2.  For each theta: D(z) = int_0^z dz'/E(z') by cumulative Gauss-Legendre
+ * quadrature on a uniform z grid (Eq. 1), u(z) = (1+z) D(z) = d_L H0/c, monotone
+ * inversion by Newton onto the uniform grid u_m = m*du, du = u(z_max)/(n_nodes-1), node slopes
+ * z'(u) = 1/(u/(1+z) + (1+z)/E(z)); and the per-theta population constants.  Tables are kept in the
+ * context (storage precision `table_prec`; arithmetic is always FP64) and are used by the calls below.
+ *   d_theta [n_theta][GWC_NPAR] f64, row-major.   z_max > 0.   n_nodes in [2, 8193] (1025 typical).
+ */
+gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double z_max, int32_t n_nodes,
+                           gwc_prec table_prec);
+/* Copy the tables of the last gwc_build_cosmo out (widened to f64): d_z, d_dz [n_theta][n_nodes]
+ * (dz = du * z'(u_m)), d_umax [n_theta].  Any pointer may be NULL. */
+gwc_status gwc_export_cosmo(gwc_ctx* ctx, double* d_z, double* d_dz, double* d_umax);
+
+typedef struct {                 /* caller-owned device arrays */
+  int64_t n_events, n_samples;   /* n_samples = sum_i S_i */
+  const int64_t* ev_sample_off;  /* [n_events+1], ascending, [0] = 0, [n_events] = n_samples */
+  const double *dL, *m1z, *m2z;  /* [n_samples] */
+  const double* log_pe_prior;    /* [n_samples] or NULL => 2 ln d_L  (PE prior ∝ d_L^2, flat in detector masses) */
+  const int32_t* sample_row;     /* [n_samples] row of the LOS table (sky pixel) of each sample */
+  const int64_t* ev_pix_off;     /* [n_events+1] or NULL (not read by the hot path) */
+  const int32_t* ev_pix_rows;    /* [sum_i P_i]  or NULL (not read by the hot path) */
+} gwc_events;
+
+typedef struct {
+  int64_t n_rows;
+  int32_t n_z;                   /* >= 2 node values per row at z_b = b z_max/(n_z-1), both ends included */
+  double z_max;
+  gwc_prec prec;                 /* storage type of `table` */
+  const void* table;             /* [n_rows][n_z] row-major, p(z | pixel) up to a theta-independent constant */
+  const double* allsky;          /* [n_z] f64: mean over rows (gwc_los_allsky fills it); read by the selection term */
+} gwc_los;
+
+typedef struct {
+  int64_t n_found;
+  double n_draw;                 /* number of injections drawn, found or not */
+  const double *dL, *m1z, *m2z;  /* [n_found] */
+  const double* log_pdraw;       /* [n_found] log draw density in (d_L, m1z, m2z) coordinates */
+} gwc_injections;
+
+/*
+ * A0 (one-time per catalogue).  Stable sort of samples by (event, row); ties keep input order, so
+ * the answer is unique and is compared bit-exactly with the oracle.
+ *   in : d_event_id, d_row [n_samples] i32, any order; event ids in [0, n_events), rows >= 0.
+ *   out: d_perm [n_samples] (sorted position -> input index), d_ev_sample_off [n_events+1],
+ *        d_ev_pix_off [n_events+1], d_ev_pix_rows [<= n_samples] (distinct rows per event, ascending),
+ *        d_pix_sample_off [<= n_samples+1] (start of each (event,row) run, then n_samples),
+ *        *h_n_pixrefs (host) = number of distinct (event,row) pairs.  Synchronises the stream.
+ */
+gwc_status gwc_pack_events(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, const int32_t* d_event_id,
+                           const int32_t* d_row, int64_t* d_perm, int64_t* d_ev_sample_off, int64_t* d_ev_pix_off,
+                           int32_t* d_ev_pix_rows, int64_t* d_pix_sample_off, int64_t* h_n_pixrefs);
+
+/* All-sky prior of the denominator: arithmetic mean over all rows, in f64, fixed order. */
+gwc_status gwc_los_allsky(gwc_ctx* ctx, const gwc_los* los, double* d_allsky /* [n_z] */);
+
+/*
+ * A3 + A4.  log L_i(theta) = log( (1/S_i) sum_k w_ik ) for every (theta, event); optional
+ * N_eff,i (Eq. 8) and the number of live samples.  Needs gwc_build_cosmo(d_theta, n_theta) first
+ * (same pointer and count) else GWC_ERR_NOT_BUILT; needs los->z_max <= the z_max of that build.
+ *   d_logL [n_theta][n_events] f64;  d_neff same shape or NULL;  d_nlive same shape i64 or NULL.
+ */
+gwc_status gwc_event_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                            const gwc_los* los, double* d_logL, double* d_neff, int64_t* d_nlive);
+
+/*
+ * A5.  log xi(theta) = log( (1/n_draw) sum_j w_j ) over found injections with the all-sky prior
+ * los->allsky and log_pdraw in place of the PE prior; optional N_eff of the injection sum.
+ *   d_logxi [n_theta];  d_neff_inj [n_theta] or NULL.
+ */
+gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_injections* inj,
+                               const gwc_los* los, double* d_logxi, double* d_neff_inj);
+
+/* A6 alone: d_total[t] = sum_i d_logL[t][i] - n_events * d_logxi[t]  (fixed order; -inf stays -inf, never NaN). */
+gwc_status gwc_combine_total(gwc_ctx* ctx, const double* d_logL, const double* d_logxi, int64_t n_theta,
+                             int64_t n_events, double* d_total);
+
+/*
+ * The whole hot path A1..A6 for one theta batch: build_cosmo(z_max = los->z_max, n_nodes, table_prec),
+ * event_loglik, selection_logxi, combine.   d_logL_total [n_theta] f64.
+ */
+gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                            const gwc_injections* inj, const gwc_los* los, int32_t n_nodes, gwc_prec table_prec,
+                            double* d_logL_total);
+
+/*
+ * Same as gwc_total_loglik but every pointer (inside the structs too) is a HOST pointer: the call
+ * uploads theta, the catalogue, the injections and the LOS table (computing the all-sky mean on the
+ * device when los->allsky is NULL), runs A1..A6 and downloads h_logL_total, then synchronises.
+ * Pinned host memory makes the copies asynchronous and faster; pageable memory works.
+ * *h2d_bytes / *d2h_bytes (may be NULL) receive the bytes copied.
+ */
+gwc_status gwc_total_loglik_host(gwc_ctx* ctx, const double* h_theta, int64_t n_theta, const gwc_events* h_ev,
+                                 const gwc_injections* h_inj, const gwc_los* h_los, int32_t n_nodes,
+                                 gwc_prec table_prec, double* h_logL_total, int64_t* h2d_bytes, int64_t* d2h_bytes);
+
+/*
+ * Measurement helpers (not on the hot path).
+ * gwc_set_timing: when on, the fused re-weighting kernel (A3/A5) is bracketed by CUDA events on the
+ * context's stream; gwc_get_timing returns, for launches since the last call, the number of such
+ * launches and their summed duration in ms for events and injections (synchronises).
+ * gwc_probe_fp64: runs a dependent-free DFMA kernel on all SMs and returns its duration and the
+ * number of FP64 instructions (thread-level) it executed: the measured FP64 roofline denominator.
+ */
+gwc_status gwc_set_timing(gwc_ctx* ctx, int on);
+gwc_status gwc_get_timing(gwc_ctx* ctx, int64_t* n_ev_launches, double* ms_ev, int64_t* n_inj_launches,
+                          double* ms_inj);
+gwc_status gwc_probe_fp64(gwc_ctx* ctx, int64_t iters, double* ms, double* n_fp64_instr);
+/* Accuracy self-test of the kernel's own FP64 elementary functions: d_out[i] = f(d_in[i]) with
+ * which = 0: exp (clamped below -700), 1: ln, 2: 1/x, 3: x^-1/2, 4: exp (unclamped).  n device doubles. */
+gwc_status gwc_math_selftest(gwc_ctx* ctx, int which, int64_t n, const double* d_in, double* d_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWC_H_ */

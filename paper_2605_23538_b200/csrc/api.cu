@@ -1,0 +1,549 @@
+// api.cu -- the C ABI of include/gwc.h: context, argument checks, scratch memory and the launch
+// sequence of the hot path A1..A6.  No arithmetic of the method lives here.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "gwc_internal.h"
+
+using namespace gwc;
+
+namespace {
+
+struct Buf {
+  void* p = nullptr;
+  size_t cap = 0;
+};
+
+struct HostCopy {  // device mirrors used by gwc_total_loglik_host
+  Buf theta, ev_off, ev_dL, ev_m1z, ev_m2z, ev_lp, ev_row, inj_dL, inj_m1z, inj_m2z, inj_lp, los, allsky, out;
+};
+
+}  // namespace
+
+struct gwc_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int n_sm = 0, smem_optin = 0;
+  std::string err;
+  int64_t launches = 0;
+  int* d_flag = nullptr;
+  unsigned int* d_counter = nullptr;
+  // A1/A2 state
+  Buf tab, tconst;
+  const double* built_theta = nullptr;
+  int64_t built_n = 0;
+  int M = 0, Mp = 0;
+  gwc_prec tab_prec = GWC_F64;
+  double z_max = 0.0;
+  // per-call scratch
+  Buf dLc, L1, Q, P, seg_off, seg_shift, group_off, part_w, part_n, allsky_scr, pack_scr, logL, logxi, probe;
+  HostCopy hc;
+  // timing
+  bool timing = false;
+  std::vector<cudaEvent_t> ev_pairs, inj_pairs;
+  std::vector<cudaEvent_t> pool;
+};
+
+namespace {
+
+std::string g_create_error;  // text of the last failed gwc_create (no context exists to hold it)
+
+gwc_status fail(gwc_ctx* c, gwc_status st, const char* msg) {
+  if (c) c->err = msg;
+  return st;
+}
+
+gwc_status cuda_fail(gwc_ctx* c, cudaError_t e, const char* where) {
+  if (c) c->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? GWC_ERR_NOMEM : GWC_ERR_CUDA;
+}
+
+#define GWC_CUDA(call)                                     \
+  do {                                                     \
+    cudaError_t e_ = (call);                               \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+  } while (0)
+
+#define GWC_TRY(call)                \
+  do {                               \
+    gwc_status s_ = (call);          \
+    if (s_ != GWC_OK) return s_;     \
+  } while (0)
+
+// grow-only device buffer; growth synchronises the stream (work in flight may still read the old block)
+gwc_status ensure(gwc_ctx* ctx, Buf& b, size_t bytes) {
+  if (bytes <= b.cap) return GWC_OK;
+  GWC_CUDA(cudaStreamSynchronize(ctx->stream));
+  if (b.p) cudaFree(b.p);
+  b.p = nullptr;
+  b.cap = 0;
+  size_t want = bytes + bytes / 8 + 256;
+  cudaError_t e = cudaMalloc(&b.p, want);
+  if (e != cudaSuccess) {
+    want = bytes;
+    e = cudaMalloc(&b.p, want);
+  }
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return cuda_fail(ctx, e, "cudaMalloc");
+  }
+  b.cap = want;
+  return GWC_OK;
+}
+
+void release(Buf& b) {
+  if (b.p) cudaFree(b.p);
+  b.p = nullptr;
+  b.cap = 0;
+}
+
+gwc_status count(gwc_ctx* ctx, int rc, const char* what) {
+  if (rc < 0) {
+    cudaError_t e = cudaGetLastError();
+    ctx->err = std::string(what) + ": launch failed: " + cudaGetErrorString(e);
+    return GWC_ERR_CUDA;
+  }
+  ctx->launches += rc;
+  return GWC_OK;
+}
+
+cudaEvent_t get_event(gwc_ctx* ctx) {
+  if (!ctx->pool.empty()) {
+    cudaEvent_t e = ctx->pool.back();
+    ctx->pool.pop_back();
+    return e;
+  }
+  cudaEvent_t e;
+  cudaEventCreate(&e);
+  return e;
+}
+
+gwc_status check_built(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double los_zmax) {
+  if (!ctx->built_theta || ctx->built_theta != d_theta || ctx->built_n != n_theta)
+    return fail(ctx, GWC_ERR_NOT_BUILT, "gwc_build_cosmo was not called with this d_theta / n_theta");
+  if (los_zmax > ctx->z_max * (1.0 + 1e-12))
+    return fail(ctx, GWC_ERR_NOT_BUILT, "cosmology table built with a smaller z_max than the LOS table's");
+  return GWC_OK;
+}
+
+// shared launch sequence of A3 (events) and A5 (injections): prep -> groups -> fused kernel
+gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg, const int64_t* d_seg_off,
+                        const double* dL, const double* m1z, const double* m2z, const double* lprior,
+                        const int32_t* row, const void* los_table, gwc_prec los_prec, int64_t n_rows, int n_z,
+                        double los_zmax, bool inj) {
+  cudaStream_t s = ctx->stream;
+  const size_t nd = (size_t)(n > 0 ? n : 1) * sizeof(double);
+  GWC_TRY(ensure(ctx, ctx->dLc, nd));
+  GWC_TRY(ensure(ctx, ctx->L1, nd));
+  GWC_TRY(ensure(ctx, ctx->Q, nd));
+  GWC_TRY(ensure(ctx, ctx->P, nd));
+  GWC_TRY(ensure(ctx, ctx->seg_shift, (size_t)n_seg * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->part_w, (size_t)n_theta * n_seg * 2 * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->part_n, (size_t)n_theta * n_seg * sizeof(int32_t)));
+  GWC_TRY(count(ctx, launch_prep_samples(n, n_seg, d_seg_off, dL, m1z, m2z, lprior, row, n_rows, (double*)ctx->dLc.p,
+                                         (double*)ctx->L1.p, (double*)ctx->Q.p, (double*)ctx->P.p,
+                                         (double*)ctx->seg_shift.p, s),
+                "prep_samples"));
+  // theta tile: as many tables as shared memory holds, balanced over the tiles
+  int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin);
+  if (T < 1) return fail(ctx, GWC_ERR_SHAPE, "n_nodes / n_z too large for shared memory");
+  if ((int64_t)T > n_theta) T = (int)n_theta;
+  const int n_tiles = (int)((n_theta + T - 1) / T);
+  T = (int)((n_theta + n_tiles - 1) / n_tiles);
+  // segment groups: enough work items to balance the SMs, small enough that a group's LOS rows stay in L2
+  int64_t target = (int64_t)((double)n * n_tiles / ((double)ctx->n_sm * 16.0));
+  if (target > 65536) target = 65536;
+  if (target < 4096) target = 4096;
+  while ((n / target + 2) * (int64_t)n_tiles > (int64_t)0x7fffffff) target *= 2;
+  const int n_groups = (int)(n > 0 ? (n + target - 1) / target : 1);
+  GWC_TRY(ensure(ctx, ctx->group_off, (size_t)(n_groups + 1) * sizeof(int32_t)));
+  GWC_TRY(count(ctx, launch_make_groups(d_seg_off, n_seg, target, n_groups, (int32_t*)ctx->group_off.p, s),
+                "make_groups"));
+  GWC_CUDA(cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned int), s));
+  ReweightParams p;
+  memset(&p, 0, sizeof(p));
+  p.tab = ctx->tab.p;
+  p.tconst = (const double*)ctx->tconst.p;
+  p.n_theta = (int)n_theta;
+  p.M = ctx->M;
+  p.Mp = ctx->Mp;
+  p.T = T;
+  p.n_tiles = n_tiles;
+  p.dLc = (const double*)ctx->dLc.p;
+  p.m1z = m1z;
+  p.m2z = m2z;
+  p.L1 = (const double*)ctx->L1.p;
+  p.Q = (const double*)ctx->Q.p;
+  p.P = (const double*)ctx->P.p;
+  p.row = row;
+  p.seg_off = d_seg_off;
+  p.group_off = (const int32_t*)ctx->group_off.p;
+  p.n_groups = n_groups;
+  p.n_seg = n_seg;
+  p.los = los_table;
+  p.n_rows = n_rows;
+  p.n_z = n_z;
+  p.inv_dz = (double)(n_z - 1) / los_zmax;
+  p.los_zmax = los_zmax;
+  p.out_w = (double*)ctx->part_w.p;
+  p.out_n = (int32_t*)ctx->part_n.p;
+  p.unit_counter = ctx->d_counter;
+  const int64_t n_items = (int64_t)n_groups * n_tiles;
+  const int n_blocks = (int)(n_items < ctx->n_sm ? n_items : ctx->n_sm);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (ctx->timing) {
+    e0 = get_event(ctx);
+    e1 = get_event(ctx);
+    cudaEventRecord(e0, s);
+  }
+  GWC_TRY(count(ctx, launch_reweight(p, ctx->tab_prec, los_prec, inj, n_blocks, s), "reweight"));
+  if (ctx->timing) {
+    cudaEventRecord(e1, s);
+    auto& v = inj ? ctx->inj_pairs : ctx->ev_pairs;
+    v.push_back(e0);
+    v.push_back(e1);
+  }
+  return GWC_OK;
+}
+
+gwc_status check_theta_args(gwc_ctx* ctx, const double* d_theta, int64_t n_theta) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (!d_theta) return fail(ctx, GWC_ERR_INVALID_ARG, "d_theta is NULL");
+  if (n_theta < 1 || n_theta > (int64_t)1 << 24) return fail(ctx, GWC_ERR_SHAPE, "n_theta out of range");
+  return GWC_OK;
+}
+
+gwc_status check_los(gwc_ctx* ctx, const gwc_los* los, bool need_table, bool need_allsky) {
+  if (!los) return fail(ctx, GWC_ERR_INVALID_ARG, "los is NULL");
+  if (los->n_z < 2 || los->n_z > 65536) return fail(ctx, GWC_ERR_SHAPE, "los->n_z out of range");
+  if (!(los->z_max > 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "los->z_max must be positive");
+  if (los->prec != GWC_F64 && los->prec != GWC_F32) return fail(ctx, GWC_ERR_INVALID_ARG, "los->prec");
+  if (need_table && (!los->table || los->n_rows < 1 || los->n_rows > 0x7fffffffLL))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "los->table is NULL or n_rows out of range");
+  if (need_allsky && !los->allsky) return fail(ctx, GWC_ERR_INVALID_ARG, "los->allsky is NULL");
+  return GWC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+gwc_status gwc_create(gwc_ctx** out, int device, void* cuda_stream) {
+  if (!out) return GWC_ERR_INVALID_ARG;
+  *out = nullptr;
+  gwc_ctx* ctx = new (std::nothrow) gwc_ctx;
+  if (!ctx) return GWC_ERR_NOMEM;
+  ctx->device = device;
+  ctx->stream = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaSetDevice(device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_flag, sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_counter, sizeof(unsigned int));
+  if (e == cudaSuccess) e = cudaMemset(ctx->d_flag, 0, sizeof(int));
+  if (e == cudaSuccess && reweight_configure(ctx->smem_optin) != 0) e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    g_create_error = std::string("gwc_create: ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    delete ctx;
+    return e == cudaErrorMemoryAllocation ? GWC_ERR_NOMEM : GWC_ERR_CUDA;
+  }
+  *out = ctx;
+  return GWC_OK;
+}
+
+void gwc_destroy(gwc_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->device);
+  cudaStreamSynchronize(ctx->stream);
+  Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->dLc, &ctx->L1, &ctx->Q, &ctx->P, &ctx->seg_off, &ctx->seg_shift,
+                 &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
+                 &ctx->logxi, &ctx->probe, &ctx->hc.theta, &ctx->hc.ev_off, &ctx->hc.ev_dL, &ctx->hc.ev_m1z,
+                 &ctx->hc.ev_m2z, &ctx->hc.ev_lp, &ctx->hc.ev_row, &ctx->hc.inj_dL, &ctx->hc.inj_m1z,
+                 &ctx->hc.inj_m2z, &ctx->hc.inj_lp, &ctx->hc.los, &ctx->hc.allsky, &ctx->hc.out};
+  for (Buf* b : bufs) release(*b);
+  for (cudaEvent_t e : ctx->ev_pairs) cudaEventDestroy(e);
+  for (cudaEvent_t e : ctx->inj_pairs) cudaEventDestroy(e);
+  for (cudaEvent_t e : ctx->pool) cudaEventDestroy(e);
+  if (ctx->d_flag) cudaFree(ctx->d_flag);
+  if (ctx->d_counter) cudaFree(ctx->d_counter);
+  delete ctx;
+}
+
+gwc_status gwc_check(gwc_ctx* ctx) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  GWC_CUDA(cudaStreamSynchronize(ctx->stream));
+  int flag = 0;
+  GWC_CUDA(cudaMemcpy(&flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+  if (flag) {
+    GWC_CUDA(cudaMemset(ctx->d_flag, 0, sizeof(int)));
+    if (flag & 1) return fail(ctx, GWC_ERR_DOMAIN, "a theta point is outside the model's domain (its outputs are NaN)");
+    return fail(ctx, GWC_ERR_DOMAIN, "gwc_pack_events: an event id or row is out of range");
+  }
+  return GWC_OK;
+}
+
+const char* gwc_last_error(const gwc_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int64_t gwc_launch_count(const gwc_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double z_max, int32_t n_nodes,
+                           gwc_prec table_prec) {
+  GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
+  if (!(z_max > 0.0) || !(z_max < 1e4)) return fail(ctx, GWC_ERR_INVALID_ARG, "z_max must be positive and finite");
+  if (n_nodes < 2 || n_nodes > MAX_NODES) return fail(ctx, GWC_ERR_SHAPE, "n_nodes must lie in [2, 8193]");
+  if (table_prec != GWC_F64 && table_prec != GWC_F32) return fail(ctx, GWC_ERR_INVALID_ARG, "table_prec");
+  const int Mp = table_pitch(n_nodes);
+  const size_t node = table_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32);
+  ctx->built_theta = nullptr;
+  GWC_TRY(ensure(ctx, ctx->tab, (size_t)n_theta * Mp * node));
+  GWC_TRY(ensure(ctx, ctx->tconst, (size_t)n_theta * NCONST * sizeof(double)));
+  GWC_TRY(count(ctx, launch_cosmo_build(d_theta, n_theta, z_max, n_nodes, Mp, table_prec, ctx->tab.p,
+                                        (double*)ctx->tconst.p, ctx->d_flag, ctx->stream),
+                "cosmo_build"));
+  ctx->built_theta = d_theta;
+  ctx->built_n = n_theta;
+  ctx->M = n_nodes;
+  ctx->Mp = Mp;
+  ctx->tab_prec = table_prec;
+  ctx->z_max = z_max;
+  return GWC_OK;
+}
+
+gwc_status gwc_export_cosmo(gwc_ctx* ctx, double* d_z, double* d_dz, double* d_umax) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (!ctx->built_theta) return fail(ctx, GWC_ERR_NOT_BUILT, "no cosmology table built");
+  return count(ctx, launch_export_cosmo(ctx->tab.p, (const double*)ctx->tconst.p, ctx->built_n, ctx->M, ctx->Mp,
+                                        ctx->tab_prec, d_z, d_dz, d_umax, ctx->stream),
+               "export_cosmo");
+}
+
+gwc_status gwc_pack_events(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, const int32_t* d_event_id,
+                           const int32_t* d_row, int64_t* d_perm, int64_t* d_ev_sample_off, int64_t* d_ev_pix_off,
+                           int32_t* d_ev_pix_rows, int64_t* d_pix_sample_off, int64_t* h_n_pixrefs) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (n_samples < 0 || n_events < 0 || n_events > 0x7fffffffLL) return fail(ctx, GWC_ERR_SHAPE, "sizes out of range");
+  if (!d_ev_sample_off || !d_ev_pix_off || !d_pix_sample_off || !h_n_pixrefs)
+    return fail(ctx, GWC_ERR_INVALID_ARG, "an output pointer is NULL");
+  if (n_samples > 0 && (!d_event_id || !d_row || !d_perm || !d_ev_pix_rows))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "an array pointer is NULL");
+  const size_t bytes = pack_scratch_bytes(n_samples, n_events);
+  GWC_TRY(ensure(ctx, ctx->pack_scr, bytes + 8));
+  int64_t* d_np = (int64_t*)((unsigned char*)ctx->pack_scr.p + bytes);
+  GWC_TRY(count(ctx, launch_pack(n_samples, n_events, d_event_id, d_row, d_perm, d_ev_sample_off, d_ev_pix_off,
+                                 d_ev_pix_rows, d_pix_sample_off, d_np, ctx->d_flag, ctx->pack_scr.p, bytes,
+                                 ctx->stream),
+                "pack_events"));
+  GWC_CUDA(cudaMemcpyAsync(h_n_pixrefs, d_np, sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream));
+  GWC_CUDA(cudaStreamSynchronize(ctx->stream));
+  return gwc_check(ctx);
+}
+
+gwc_status gwc_los_allsky(gwc_ctx* ctx, const gwc_los* los, double* d_allsky) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  GWC_TRY(check_los(ctx, los, true, false));
+  if (!d_allsky) return fail(ctx, GWC_ERR_INVALID_ARG, "d_allsky is NULL");
+  GWC_TRY(ensure(ctx, ctx->allsky_scr, allsky_scratch_doubles(los->n_rows, los->n_z) * sizeof(double)));
+  return count(ctx, launch_allsky(los->table, los->prec, los->n_rows, los->n_z, (double*)ctx->allsky_scr.p, d_allsky,
+                                  ctx->stream),
+               "los_allsky");
+}
+
+gwc_status gwc_event_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                            const gwc_los* los, double* d_logL, double* d_neff, int64_t* d_nlive) {
+  GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
+  if (!ev || !d_logL) return fail(ctx, GWC_ERR_INVALID_ARG, "ev or d_logL is NULL");
+  GWC_TRY(check_los(ctx, los, true, false));
+  if (ev->n_events < 0 || ev->n_samples < 0 || ev->n_events > 0x7fffffffLL)
+    return fail(ctx, GWC_ERR_SHAPE, "event / sample counts out of range");
+  if (ev->n_events == 0) return GWC_OK;
+  if (!ev->ev_sample_off) return fail(ctx, GWC_ERR_INVALID_ARG, "ev->ev_sample_off is NULL");
+  if (ev->n_samples > 0 && (!ev->dL || !ev->m1z || !ev->m2z || !ev->sample_row))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "a sample array is NULL");
+  GWC_TRY(check_built(ctx, d_theta, n_theta, los->z_max));
+  GWC_TRY(run_reweight(ctx, n_theta, ev->n_samples, ev->n_events, ev->ev_sample_off, ev->dL, ev->m1z, ev->m2z,
+                       ev->log_pe_prior, ev->sample_row, los->table, los->prec, los->n_rows, los->n_z, los->z_max,
+                       false));
+  return count(ctx, launch_finalize_events((const double*)ctx->part_w.p, (const int32_t*)ctx->part_n.p,
+                                           ev->ev_sample_off, (const double*)ctx->seg_shift.p,
+                                           (const double*)ctx->tconst.p, n_theta, ev->n_events, d_logL, d_neff,
+                                           d_nlive, ctx->stream),
+               "finalize_events");
+}
+
+gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_injections* inj,
+                               const gwc_los* los, double* d_logxi, double* d_neff_inj) {
+  GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
+  if (!inj || !d_logxi) return fail(ctx, GWC_ERR_INVALID_ARG, "inj or d_logxi is NULL");
+  GWC_TRY(check_los(ctx, los, false, true));
+  if (inj->n_found < 0) return fail(ctx, GWC_ERR_SHAPE, "n_found < 0");
+  if (!(inj->n_draw > 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "n_draw must be positive");
+  if (inj->n_found > 0 && (!inj->dL || !inj->m1z || !inj->m2z || !inj->log_pdraw))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "an injection array is NULL");
+  if (los->n_z > 4096) return fail(ctx, GWC_ERR_SHAPE, "los->n_z > 4096 is not supported by the selection kernel");
+  GWC_TRY(check_built(ctx, d_theta, n_theta, los->z_max));
+  const int64_t n = inj->n_found;
+  const int64_t n_seg = n > 0 ? (n + INJ_SEG - 1) / INJ_SEG : 1;
+  GWC_TRY(ensure(ctx, ctx->seg_off, (size_t)(n_seg + 1) * sizeof(int64_t)));
+  GWC_TRY(count(ctx, launch_uniform_segments(n, INJ_SEG, n_seg, (int64_t*)ctx->seg_off.p, ctx->stream),
+                "uniform_segments"));
+  GWC_TRY(run_reweight(ctx, n_theta, n, n_seg, (const int64_t*)ctx->seg_off.p, inj->dL, inj->m1z, inj->m2z,
+                       inj->log_pdraw, nullptr, los->allsky, GWC_F64, 1, los->n_z, los->z_max, true));
+  return count(ctx, launch_finalize_inj((const double*)ctx->part_w.p, (const double*)ctx->seg_shift.p,
+                                        (const double*)ctx->tconst.p, n_theta, n_seg, inj->n_draw, d_logxi,
+                                        d_neff_inj, ctx->stream),
+               "finalize_inj");
+}
+
+gwc_status gwc_combine_total(gwc_ctx* ctx, const double* d_logL, const double* d_logxi, int64_t n_theta,
+                             int64_t n_events, double* d_total) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (!d_logxi || !d_total || (n_events > 0 && !d_logL)) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL pointer");
+  if (n_theta < 1 || n_events < 0) return fail(ctx, GWC_ERR_SHAPE, "sizes out of range");
+  return count(ctx, launch_combine_total(d_logL, d_logxi, n_theta, n_events, d_total, ctx->stream), "combine_total");
+}
+
+gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                            const gwc_injections* inj, const gwc_los* los, int32_t n_nodes, gwc_prec table_prec,
+                            double* d_logL_total) {
+  GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
+  if (!ev || !inj || !d_logL_total) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL argument");
+  GWC_TRY(check_los(ctx, los, true, true));
+  GWC_TRY(gwc_build_cosmo(ctx, d_theta, n_theta, los->z_max, n_nodes, table_prec));
+  const int64_t E = ev->n_events;
+  GWC_TRY(ensure(ctx, ctx->logL, (size_t)n_theta * (size_t)(E > 0 ? E : 1) * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->logxi, (size_t)n_theta * sizeof(double)));
+  GWC_TRY(gwc_event_loglik(ctx, d_theta, n_theta, ev, los, (double*)ctx->logL.p, nullptr, nullptr));
+  GWC_TRY(gwc_selection_logxi(ctx, d_theta, n_theta, inj, los, (double*)ctx->logxi.p, nullptr));
+  return gwc_combine_total(ctx, (const double*)ctx->logL.p, (const double*)ctx->logxi.p, n_theta, E, d_logL_total);
+}
+
+gwc_status gwc_total_loglik_host(gwc_ctx* ctx, const double* h_theta, int64_t n_theta, const gwc_events* h_ev,
+                                 const gwc_injections* h_inj, const gwc_los* h_los, int32_t n_nodes,
+                                 gwc_prec table_prec, double* h_logL_total, int64_t* h2d_bytes, int64_t* d2h_bytes) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (!h_theta || !h_ev || !h_inj || !h_los || !h_logL_total) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL argument");
+  if (n_theta < 1) return fail(ctx, GWC_ERR_SHAPE, "n_theta out of range");
+  GWC_TRY(check_los(ctx, h_los, true, false));
+  if (h_ev->n_events < 0 || h_ev->n_samples < 0 || h_inj->n_found < 0) return fail(ctx, GWC_ERR_SHAPE, "negative size");
+  if (h_ev->n_events > 0 && !h_ev->ev_sample_off) return fail(ctx, GWC_ERR_INVALID_ARG, "ev_sample_off is NULL");
+  if (h_ev->n_samples > 0 && (!h_ev->dL || !h_ev->m1z || !h_ev->m2z || !h_ev->sample_row))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "a sample array is NULL");
+  if (h_inj->n_found > 0 && (!h_inj->dL || !h_inj->m1z || !h_inj->m2z || !h_inj->log_pdraw))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "an injection array is NULL");
+  cudaStream_t s = ctx->stream;
+  HostCopy& h = ctx->hc;
+  int64_t up = 0;
+  auto upload = [&](Buf& b, const void* src, size_t bytes) -> gwc_status {
+    GWC_TRY(ensure(ctx, b, bytes > 0 ? bytes : 8));
+    if (bytes > 0) {
+      GWC_CUDA(cudaMemcpyAsync(b.p, src, bytes, cudaMemcpyHostToDevice, s));
+      up += (int64_t)bytes;
+    }
+    return GWC_OK;
+  };
+  const size_t ns = (size_t)h_ev->n_samples, ni = (size_t)h_inj->n_found;
+  const size_t los_el = h_los->prec == GWC_F64 ? 8 : 4;
+  GWC_TRY(upload(h.theta, h_theta, (size_t)n_theta * GWC_NPAR * 8));
+  GWC_TRY(upload(h.ev_off, h_ev->ev_sample_off, (size_t)(h_ev->n_events + 1) * 8));
+  GWC_TRY(upload(h.ev_dL, h_ev->dL, ns * 8));
+  GWC_TRY(upload(h.ev_m1z, h_ev->m1z, ns * 8));
+  GWC_TRY(upload(h.ev_m2z, h_ev->m2z, ns * 8));
+  if (h_ev->log_pe_prior) GWC_TRY(upload(h.ev_lp, h_ev->log_pe_prior, ns * 8));
+  GWC_TRY(upload(h.ev_row, h_ev->sample_row, ns * 4));
+  GWC_TRY(upload(h.inj_dL, h_inj->dL, ni * 8));
+  GWC_TRY(upload(h.inj_m1z, h_inj->m1z, ni * 8));
+  GWC_TRY(upload(h.inj_m2z, h_inj->m2z, ni * 8));
+  GWC_TRY(upload(h.inj_lp, h_inj->log_pdraw, ni * 8));
+  GWC_TRY(upload(h.los, h_los->table, (size_t)h_los->n_rows * h_los->n_z * los_el));
+  GWC_TRY(ensure(ctx, h.allsky, (size_t)h_los->n_z * 8));
+  GWC_TRY(ensure(ctx, h.out, (size_t)n_theta * 8));
+  gwc_events ev = *h_ev;
+  ev.ev_sample_off = (const int64_t*)h.ev_off.p;
+  ev.dL = (const double*)h.ev_dL.p;
+  ev.m1z = (const double*)h.ev_m1z.p;
+  ev.m2z = (const double*)h.ev_m2z.p;
+  ev.log_pe_prior = h_ev->log_pe_prior ? (const double*)h.ev_lp.p : nullptr;
+  ev.sample_row = (const int32_t*)h.ev_row.p;
+  ev.ev_pix_off = nullptr;
+  ev.ev_pix_rows = nullptr;
+  gwc_injections inj = *h_inj;
+  inj.dL = (const double*)h.inj_dL.p;
+  inj.m1z = (const double*)h.inj_m1z.p;
+  inj.m2z = (const double*)h.inj_m2z.p;
+  inj.log_pdraw = (const double*)h.inj_lp.p;
+  gwc_los los = *h_los;
+  los.table = h.los.p;
+  los.allsky = (const double*)h.allsky.p;
+  if (h_los->allsky) {
+    GWC_CUDA(cudaMemcpyAsync(h.allsky.p, h_los->allsky, (size_t)h_los->n_z * 8, cudaMemcpyHostToDevice, s));
+    up += (int64_t)h_los->n_z * 8;
+  } else {
+    GWC_TRY(gwc_los_allsky(ctx, &los, (double*)h.allsky.p));
+  }
+  GWC_TRY(gwc_total_loglik(ctx, (const double*)h.theta.p, n_theta, &ev, &inj, &los, n_nodes, table_prec,
+                           (double*)h.out.p));
+  GWC_CUDA(cudaMemcpyAsync(h_logL_total, h.out.p, (size_t)n_theta * 8, cudaMemcpyDeviceToHost, s));
+  GWC_CUDA(cudaStreamSynchronize(s));
+  ctx->built_theta = nullptr;  // the mirrored theta buffer is internal: do not let later calls match it
+  if (h2d_bytes) *h2d_bytes = up;
+  if (d2h_bytes) *d2h_bytes = n_theta * 8;
+  return GWC_OK;
+}
+
+gwc_status gwc_set_timing(gwc_ctx* ctx, int on) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  ctx->timing = on != 0;
+  return GWC_OK;
+}
+
+gwc_status gwc_get_timing(gwc_ctx* ctx, int64_t* n_ev_launches, double* ms_ev, int64_t* n_inj_launches,
+                          double* ms_inj) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  GWC_CUDA(cudaStreamSynchronize(ctx->stream));
+  auto drain = [&](std::vector<cudaEvent_t>& v, int64_t* n, double* ms) {
+    double tot = 0.0;
+    for (size_t i = 0; i + 1 < v.size(); i += 2) {
+      float t = 0.f;
+      cudaEventElapsedTime(&t, v[i], v[i + 1]);
+      tot += t;
+    }
+    if (n) *n = (int64_t)(v.size() / 2);
+    if (ms) *ms = tot;
+    for (cudaEvent_t e : v) ctx->pool.push_back(e);
+    v.clear();
+  };
+  drain(ctx->ev_pairs, n_ev_launches, ms_ev);
+  drain(ctx->inj_pairs, n_inj_launches, ms_inj);
+  return GWC_OK;
+}
+
+gwc_status gwc_probe_fp64(gwc_ctx* ctx, int64_t iters, double* ms, double* n_fp64_instr) {
+  if (!ctx || !ms || !n_fp64_instr || iters < 1) return GWC_ERR_INVALID_ARG;
+  GWC_TRY(ensure(ctx, ctx->probe, 64));
+  cudaEvent_t e0 = get_event(ctx), e1 = get_event(ctx);
+  double n = 0.0;
+  // warm-up launch, then the timed one
+  GWC_TRY(count(ctx, launch_probe_fp64(iters / 8 + 1, ctx->n_sm, (double*)ctx->probe.p, ctx->stream, &n), "probe"));
+  cudaEventRecord(e0, ctx->stream);
+  GWC_TRY(count(ctx, launch_probe_fp64(iters, ctx->n_sm, (double*)ctx->probe.p, ctx->stream, &n), "probe"));
+  cudaEventRecord(e1, ctx->stream);
+  GWC_CUDA(cudaStreamSynchronize(ctx->stream));
+  float t = 0.f;
+  cudaEventElapsedTime(&t, e0, e1);
+  ctx->pool.push_back(e0);
+  ctx->pool.push_back(e1);
+  *ms = t;
+  *n_fp64_instr = n;
+  return GWC_OK;
+}
+
+gwc_status gwc_math_selftest(gwc_ctx* ctx, int which, int64_t n, const double* d_in, double* d_out) {
+  if (!ctx || !d_in || !d_out || n < 0) return GWC_ERR_INVALID_ARG;
+  return count(ctx, launch_math_selftest(which, n, d_in, d_out, ctx->stream), "math_selftest");
+}
+
+}  // extern "C"

@@ -1,0 +1,223 @@
+// cosmo.cu -- A1 + A2: per-theta inverse-cosmology table and population constants.
+//
+// Eq. 1 of the paper: d_L(z) = (1+z) (c/H0) D(z), D(z) = int_0^z dz'/E(z'),
+// E = sqrt(Om (1+z)^3 + 1 - Om).  In the dimensionless u = d_L H0/c = (1+z) D(z) the inverse z(u)
+// depends on Om only.  One CTA per theta:
+//   1. forward cumulative quadrature: 3-point Gauss-Legendre on each of QUAD_K uniform z intervals,
+//      compensated prefix sum -> D(z_k), u(z_k) in shared memory;
+//   2. monotone inversion: for every node u_m = m du, du = u(z_max)/(M-1), bracket by binary search
+//      in u(z_k), then Newton on (1+z)(D(z_k) + int_{z_k}^{z} dz'/E) = u_m (the short remainder
+//      integral again by 3-point Gauss-Legendre);
+//   3. node slope d_m = du * dz/du = du / (u/(1+z) + (1+z)/E(z))  (cubic-Hermite data, R9);
+//   4. thread 0 writes the constant block of the population laws (R2-R4).
+// Not a hot kernel (n_theta * M Newton solves); libdevice sqrt/div/pow/erf are used as they are.
+#include <math_constants.h>
+
+#include "gwc_internal.h"
+
+namespace gwc {
+
+namespace {
+
+constexpr double C_KMS = 299792.458;
+constexpr int CB_THREADS = 256;
+
+__device__ __forceinline__ double invE(double z, double Om, double OL) {
+  double x = 1.0 + z;
+  return rsqrt(fma(Om * x * x, x, OL));
+}
+
+// int_a^b dz/E by 3-point Gauss-Legendre
+__device__ __forceinline__ double gl3(double a, double b, double Om, double OL) {
+  const double XN = 0.77459666924148337704;  // sqrt(3/5)
+  double hm = 0.5 * (b - a), c = 0.5 * (a + b);
+  double s = 5.0 * (invE(c - hm * XN, Om, OL) + invE(c + hm * XN, Om, OL)) + 8.0 * invE(c, Om, OL);
+  return hm * s * (1.0 / 9.0);
+}
+
+__device__ __forceinline__ void store_node(Node64* t, double z, double d) { t->z = z; t->d = d; }
+__device__ __forceinline__ void store_node(Node32* t, double z, double d) {
+  t->z = __double2float_rn(z);
+  t->d = __double2float_rn(d);
+}
+
+__device__ bool theta_valid(const double* th) {
+  for (int i = 0; i < GWC_NPAR; ++i)
+    if (!isfinite(th[i])) return false;
+  if (!(th[0] > 0.0)) return false;
+  if (!(th[1] > 0.0 && th[1] <= 1.0)) return false;
+  if (!(th[7] > 0.0)) return false;
+  if (!(th[4] > 0.0 && th[4] < th[5])) return false;
+  if (!(th[8] >= 0.0 && th[8] <= 1.0)) return false;
+  if (!(th[11] > -1.0)) return false;
+  if (fabs(th[2] - 1.0) < 1e-6) return false;
+  if (fabs(th[3] + 1.0) < 1e-6) return false;
+  return true;
+}
+
+template <typename NodeT>
+__global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* __restrict__ theta, double z_max,
+                                                                  int M, int Mp, NodeT* __restrict__ tab,
+                                                                  double* __restrict__ tconst, int* flag) {
+  __shared__ double Dg[QUAD_K + 1];
+  __shared__ double ug[QUAD_K + 1];
+  __shared__ double part[CB_THREADS];
+  __shared__ double s_umax;
+  const int t = blockIdx.x, tid = threadIdx.x;
+  const double* th = theta + (size_t)t * GWC_NPAR;
+  NodeT* row = tab + (size_t)t * Mp;
+  double* tc = tconst + (size_t)t * NCONST;
+  const bool valid = theta_valid(th);
+  if (!valid) {
+    for (int m = tid; m < Mp; m += CB_THREADS) store_node(row + m, 0.0, 0.0);
+    if (tid < NCONST) tc[tid] = (tid == C_VALID) ? CUDART_NAN : 0.0;
+    if (tid == 0) atomicOr(flag, 1);
+    return;
+  }
+  const double Om = th[1], OL = 1.0 - Om;
+  const double hz = z_max / QUAD_K;
+  constexpr int PER = QUAD_K / CB_THREADS;
+  // 1. interval integrals, thread-local prefix, compensated scan of the thread totals
+  double loc[PER];
+  double run = 0.0;
+#pragma unroll
+  for (int j = 0; j < PER; ++j) {
+    int k = tid * PER + j;
+    run += gl3(k * hz, (k + 1) * hz, Om, OL);
+    loc[j] = run;
+  }
+  part[tid] = run;
+  __syncthreads();
+  if (tid == 0) {
+    double s = 0.0, comp = 0.0;  // Neumaier-compensated exclusive scan
+    for (int i = 0; i < CB_THREADS; ++i) {
+      double v = part[i];
+      part[i] = s + comp;
+      double tsum = s + v;
+      comp += (fabs(s) >= fabs(v)) ? ((s - tsum) + v) : ((v - tsum) + s);
+      s = tsum;
+    }
+    Dg[0] = 0.0;
+    ug[0] = 0.0;
+  }
+  __syncthreads();
+  {
+    double base = part[tid];
+#pragma unroll
+    for (int j = 0; j < PER; ++j) {
+      int k = tid * PER + j + 1;
+      double D = base + loc[j];
+      Dg[k] = D;
+      ug[k] = (1.0 + k * hz) * D;
+    }
+  }
+  __syncthreads();
+  if (tid == 0) s_umax = ug[QUAD_K];
+  __syncthreads();
+  const double umax = s_umax;
+  const double du = umax / (M - 1);
+  // 2-3. nodes
+  for (int m = tid; m < Mp; m += CB_THREADS) {
+    double z, d;
+    if (m >= M - 1) {
+      z = z_max;
+      d = (m == M - 1) ? du / (umax / (1.0 + z) + (1.0 + z) * invE(z, Om, OL)) : 0.0;
+    } else {
+      double u = m * du;
+      int lo = 0, hi = QUAD_K;  // ug[lo] <= u < ug[hi]
+      while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (ug[mid] <= u) lo = mid; else hi = mid;
+      }
+      double zk = lo * hz, Dk = Dg[lo];
+      z = zk + (u - ug[lo]) / (ug[lo + 1] - ug[lo]) * hz;
+#pragma unroll 1
+      for (int it = 0; it < 5; ++it) {
+        double Dz = Dk + gl3(zk, z, Om, OL);
+        double x = 1.0 + z;
+        double f = x * Dz - u;
+        double fp = Dz + x * invE(z, Om, OL);
+        z -= f / fp;
+      }
+      if (m == 0) z = 0.0;
+      double x = 1.0 + z;
+      d = du / (u / x + x * invE(z, Om, OL));
+    }
+    store_node(row + m, z, d);
+  }
+  // 4. constants
+  if (tid == 0) {
+    const double H0 = th[0], alpha = th[2], beta = th[3], mmin = th[4], mmax = th[5], mu = th[6], sigma = th[7],
+                 lam = th[8], gam = th[9], kap = th[10], zp = th[11];
+    const double h = H0 / C_KMS;
+    const double n_pl = (1.0 - alpha) / (pow(mmax, 1.0 - alpha) - pow(mmin, 1.0 - alpha));
+    const double rs2 = 1.0 / (sigma * 1.41421356237309504880);
+    const double n_g = 1.0 / (0.5 * (erf((mmax - mu) * rs2) - erf((mmin - mu) * rs2)));
+    const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
+    const double common = fabs(beta + 1.0) * psi0 * h;
+    tc[C_H] = h;
+    tc[C_UMAX] = umax;
+    tc[C_INVDU] = (M - 1) / umax;
+    tc[C_MMIN] = mmin;
+    tc[C_MMAX] = mmax;
+    tc[C_BETA] = beta;
+    tc[C_GM1] = gam - 1.0;
+    tc[C_NALPHA] = -alpha;
+    tc[C_CPL] = (lam < 1.0) ? log((1.0 - lam) * n_pl * common) : -CUDART_INF;
+    tc[C_CG] = (lam > 0.0) ? log(lam * n_g / (sigma * 2.50662827463100050242) * common) : -CUDART_INF;
+    tc[C_INVSIG] = 1.0 / sigma;
+    tc[C_NMUSIG] = -mu / sigma;
+    tc[C_NBP1] = -(beta + 1.0);
+    tc[C_E1C] = (beta + 1.0) * log(mmin);
+    tc[C_SGN] = (beta + 1.0 > 0.0) ? 1.0 : -1.0;
+    tc[C_GK] = gam + kap;
+    tc[C_E2C] = -(gam + kap) * log1p(zp);
+    tc[C_OM] = Om;
+    tc[C_OL] = OL;
+    tc[C_VALID] = 1.0;
+    for (int i = C_COUNT; i < NCONST; ++i) tc[i] = 0.0;
+  }
+}
+
+template <typename NodeT>
+__global__ void export_cosmo_kernel(const NodeT* __restrict__ tab, const double* __restrict__ tconst, int64_t n_theta,
+                                    int M, int Mp, double* z, double* dz, double* umax) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n_theta * M) return;
+  int64_t t = i / M;
+  int m = (int)(i - t * M);
+  NodeT nd = tab[t * Mp + m];
+  if (z) z[i] = (double)nd.z;
+  if (dz) dz[i] = (double)nd.d;
+  if (umax && m == 0) umax[t] = tconst[t * NCONST + C_UMAX];
+}
+
+}  // namespace
+
+int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int M, int Mp, gwc_prec prec, void* d_tab,
+                       double* d_tconst, int* d_flag, cudaStream_t s) {
+  if (n_theta <= 0) return 0;
+  if (prec == GWC_F64)
+    cosmo_build_kernel<Node64><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, z_max, M, Mp, (Node64*)d_tab,
+                                                                         d_tconst, d_flag);
+  else
+    cosmo_build_kernel<Node32><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, z_max, M, Mp, (Node32*)d_tab,
+                                                                         d_tconst, d_flag);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+int launch_export_cosmo(const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp, gwc_prec prec,
+                        double* d_z, double* d_dz, double* d_umax, cudaStream_t s) {
+  int64_t n = n_theta * M;
+  if (n <= 0) return 0;
+  unsigned blocks = (unsigned)((n + 255) / 256);
+  if (prec == GWC_F64)
+    export_cosmo_kernel<Node64><<<blocks, 256, 0, s>>>((const Node64*)d_tab, d_tconst, n_theta, M, Mp, d_z, d_dz,
+                                                       d_umax);
+  else
+    export_cosmo_kernel<Node32><<<blocks, 256, 0, s>>>((const Node32*)d_tab, d_tconst, n_theta, M, Mp, d_z, d_dz,
+                                                       d_umax);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace gwc

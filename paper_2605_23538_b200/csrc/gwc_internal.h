@@ -1,0 +1,110 @@
+// gwc_internal.h -- shared declarations of the CUDA library (not part of the public ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gwc.h"
+
+namespace gwc {
+
+// ---- per-theta constant block (A2), doubles, consumed by the fused re-weighting kernel ----------
+// With x = 1+z, lx = ln x, t1 = ln m1z - lx (= ln m1), Q = ln(m2z/m1z), P' = -ln pi - ln m1z - shift:
+//   w = [exp(CPL + c - alpha t1) + exp(CG + c - y^2/2)] * p_los / [(u + x^2/E)(1 - e1)(1 + e2)]
+//   c = beta Q + P' + (gamma-1) lx,  y = m1/sigma - mu/sigma,
+//   e1 = exp(E1C + NBP1 t1) = (mmin/m1)^(beta+1),  e2 = exp(GK lx + E2C) = ((1+z)/(1+zp))^(gamma+kappa)
+enum : int {
+  C_H = 0,     // H0 / c                          (u = d_L * h)
+  C_UMAX,      // u(z_max) of this theta's table
+  C_INVDU,     // (M-1) / umax
+  C_MMIN,
+  C_MMAX,
+  C_BETA,
+  C_GM1,       // gamma - 1
+  C_NALPHA,    // -alpha
+  C_CPL,       // ln[(1-lambda) n_pl |beta+1| psi0 h]   (-inf when lambda = 1)
+  C_CG,        // ln[lambda n_g /(sigma sqrt(2 pi)) |beta+1| psi0 h]   (-inf when lambda = 0)
+  C_INVSIG,    // 1/sigma
+  C_NMUSIG,    // -mu/sigma
+  C_NBP1,      // -(beta+1)
+  C_E1C,       // (beta+1) ln mmin
+  C_SGN,       // sign(beta+1)
+  C_GK,        // gamma + kappa
+  C_E2C,       // -(gamma+kappa) ln(1+zp)
+  C_OM,
+  C_OL,        // 1 - Om
+  C_VALID,     // 1.0 or NaN (theta-domain violation)
+  C_COUNT
+};
+constexpr int NCONST = 24;  // padded row length (>= C_COUNT), keeps rows 64-byte aligned
+
+constexpr int NTHREADS = 512;     // threads per CTA of the fused kernel (one CTA per SM)
+constexpr int NWARPS = NTHREADS / 32;
+constexpr int SPT = 2;            // samples per thread per theta (independent chains in flight)
+constexpr int CHUNK = NTHREADS * SPT;  // samples staged in shared memory per step
+constexpr int MAX_T = 16;         // theta points per tile (upper bound)
+constexpr int INJ_SEG = 8192;     // injections per segment of the selection reduction
+constexpr int QUAD_K = 1024;      // forward quadrature intervals of the cosmology builder
+constexpr int MAX_NODES = 8193;
+
+struct Node64 { double z, d; };   // table node: z_m and du * z'(u_m)
+struct Node32 { float z, d; };
+
+// table row length: M nodes + 1 pad node (index M is read when u rounds onto the last node), even
+__host__ __device__ inline int table_pitch(int M) { return (M + 2) & ~1; }
+
+struct ReweightParams {
+  const void* tab;          // [n_theta][Mp] Node64 | Node32
+  const double* tconst;     // [n_theta][NCONST]
+  int n_theta, M, Mp, T, n_tiles;
+  const double *dLc, *m1z, *m2z, *L1, *Q, *P;   // [n_samples] prepared per-sample values
+  const int32_t* row;       // [n_samples] (events) or nullptr (injections)
+  const int64_t* seg_off;   // [n_seg+1] device
+  const int32_t* group_off; // [n_groups+1] device: segments of each work group
+  int n_groups;
+  int64_t n_seg;
+  const void* los;          // [n_rows][n_z] (events) | allsky [n_z] f64 (injections)
+  int64_t n_rows;
+  int n_z;
+  double inv_dz, los_zmax;
+  double* out_w;            // [n_theta][n_seg][2]: sum w', sum w'^2
+  int32_t* out_n;           // [n_theta][n_seg]   : n_live
+  unsigned int* unit_counter;
+};
+
+// kernels / launchers (each returns the number of kernels it launched, or -1 on a launch error)
+int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int M, int Mp, gwc_prec prec,
+                       void* d_tab, double* d_tconst, int* d_flag, cudaStream_t s);
+int launch_export_cosmo(const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp, gwc_prec prec,
+                        double* d_z, double* d_dz, double* d_umax, cudaStream_t s);
+// per-sample, theta-independent preparation (+ per-segment shift = max(-ln pi - ln m1z))
+int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const double* dL, const double* m1z,
+                        const double* m2z, const double* lprior, const int32_t* row, int64_t n_rows, double* dLc,
+                        double* L1, double* Q, double* P, double* seg_shift, cudaStream_t s);
+int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
+                       cudaStream_t s);
+int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off, cudaStream_t s);
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z);
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin);
+int reweight_configure(int smem_optin);
+int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_blocks,
+                    cudaStream_t s);
+int launch_finalize_events(const double* part_w, const int32_t* part_n, const int64_t* seg_off, const double* seg_shift,
+                           const double* tconst, int64_t n_theta, int64_t n_events, double* logL, double* neff,
+                           int64_t* nlive, cudaStream_t s);
+int launch_finalize_inj(const double* part_w, const double* seg_shift, const double* tconst, int64_t n_theta,
+                        int64_t n_seg, double n_draw, double* logxi, double* neff, cudaStream_t s);
+int launch_combine_total(const double* logL, const double* logxi, int64_t n_theta, int64_t n_events, double* total,
+                         cudaStream_t s);
+int launch_allsky(const void* table, gwc_prec prec, int64_t n_rows, int n_z, double* scratch, double* allsky,
+                  cudaStream_t s);
+size_t allsky_scratch_doubles(int64_t n_rows, int n_z);
+int launch_probe_fp64(int64_t iters, int n_blocks, double* d_sink, cudaStream_t s, double* n_instr);
+int launch_math_selftest(int which, int64_t n, const double* d_in, double* d_out, cudaStream_t s);
+
+// A0 packing (device radix sort + run detection); returns launches or -1
+size_t pack_scratch_bytes(int64_t n_samples, int64_t n_events);
+int launch_pack(int64_t n_samples, int64_t n_events, const int32_t* d_event_id, const int32_t* d_row, int64_t* d_perm,
+                int64_t* d_ev_sample_off, int64_t* d_ev_pix_off, int32_t* d_ev_pix_rows, int64_t* d_pix_sample_off,
+                int64_t* d_n_pixrefs, int* d_flag, void* scratch, size_t scratch_bytes, cudaStream_t s);
+
+}  // namespace gwc

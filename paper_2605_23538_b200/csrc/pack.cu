@@ -1,0 +1,140 @@
+// pack.cu -- A0: one-time packing of a catalogue into the segmented (CSR) layout that replaces the
+// paper's padded (N_events, N_pix, N_samples) tensor (its own future work).
+// Stable sort of samples by (event, row) -- ties keep input order, so the answer is unique and integer --
+// then event offsets, the distinct rows of each event and the start of each (event, row) run.
+// The sort itself is the CUB library radix sort (a library primitive on a one-time, non-hot step);
+// everything else is plain kernels.
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
+
+#include "gwc_internal.h"
+
+namespace gwc {
+
+namespace {
+
+__global__ void pack_keys_kernel(int64_t n, int64_t n_events, const int32_t* __restrict__ ev,
+                                 const int32_t* __restrict__ row, uint64_t* __restrict__ keys,
+                                 int64_t* __restrict__ idx, int* flag) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const int32_t e = ev[k], r = row[k];
+  if (e < 0 || e >= n_events || r < 0) atomicOr(flag, 2);
+  keys[k] = ((uint64_t)(uint32_t)e << 32) | (uint64_t)(uint32_t)r;
+  idx[k] = k;
+}
+
+// ev_sample_off[i] = first sorted position whose event id is >= i
+__global__ void pack_event_off_kernel(int64_t n, int64_t n_events, const uint64_t* __restrict__ keys,
+                                      int64_t* __restrict__ ev_sample_off) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i > n_events) return;
+  const uint64_t key = (uint64_t)i << 32;
+  int64_t lo = 0, hi = n;
+  while (lo < hi) {
+    const int64_t mid = (lo + hi) >> 1;
+    if (keys[mid] < key) lo = mid + 1; else hi = mid;
+  }
+  ev_sample_off[i] = lo;
+}
+
+__global__ void pack_heads_kernel(int64_t n, const uint64_t* __restrict__ keys, int64_t* __restrict__ head) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  head[k] = (k == 0 || keys[k] != keys[k - 1]) ? 1 : 0;
+}
+
+// pos = exclusive scan of head.  Scatter run starts; the last thread writes the count and the end sentinel.
+__global__ void pack_runs_kernel(int64_t n, const uint64_t* __restrict__ keys, const int64_t* __restrict__ head,
+                                 const int64_t* __restrict__ pos, int32_t* __restrict__ ev_pix_rows,
+                                 int64_t* __restrict__ pix_sample_off, int64_t* __restrict__ n_pixrefs) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  if (head[k]) {
+    ev_pix_rows[pos[k]] = (int32_t)(uint32_t)(keys[k] & 0xffffffffu);
+    pix_sample_off[pos[k]] = k;
+  }
+  if (k == n - 1) {
+    const int64_t np = pos[k] + head[k];
+    *n_pixrefs = np;
+    pix_sample_off[np] = n;
+  }
+}
+
+__global__ void pack_pix_off_kernel(int64_t n, int64_t n_events, const int64_t* __restrict__ ev_sample_off,
+                                    const int64_t* __restrict__ pos, const int64_t* __restrict__ n_pixrefs,
+                                    int64_t* __restrict__ ev_pix_off) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i > n_events) return;
+  const int64_t s = ev_sample_off[i];
+  ev_pix_off[i] = (i == n_events || s >= n) ? *n_pixrefs : pos[s];
+}
+
+__global__ void pack_empty_kernel(int64_t n_events, int64_t* ev_sample_off, int64_t* ev_pix_off,
+                                  int64_t* pix_sample_off, int64_t* n_pixrefs) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i <= n_events) {
+    ev_sample_off[i] = 0;
+    ev_pix_off[i] = 0;
+  }
+  if (i == 0) {
+    pix_sample_off[0] = 0;
+    *n_pixrefs = 0;
+  }
+}
+
+size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+size_t cub_temp_bytes(int64_t n) {
+  size_t a = 0, b = 0;
+  cub::DeviceRadixSort::SortPairs(nullptr, a, (const uint64_t*)nullptr, (uint64_t*)nullptr, (const int64_t*)nullptr,
+                                  (int64_t*)nullptr, n);
+  cub::DeviceScan::ExclusiveSum(nullptr, b, (const int64_t*)nullptr, (int64_t*)nullptr, n);
+  return a > b ? a : b;
+}
+
+}  // namespace
+
+size_t pack_scratch_bytes(int64_t n_samples, int64_t n_events) {
+  (void)n_events;
+  const size_t n = (size_t)(n_samples > 0 ? n_samples : 1);
+  return 4 * a256(8 * n) + a256(cub_temp_bytes((int64_t)n)) + 256;
+}
+
+int launch_pack(int64_t n, int64_t n_events, const int32_t* d_event_id, const int32_t* d_row, int64_t* d_perm,
+                int64_t* d_ev_sample_off, int64_t* d_ev_pix_off, int32_t* d_ev_pix_rows, int64_t* d_pix_sample_off,
+                int64_t* d_n_pixrefs, int* d_flag, void* scratch, size_t scratch_bytes, cudaStream_t s) {
+  int launches = 0;
+  const unsigned be = (unsigned)((n_events + 1 + 255) / 256);
+  if (n == 0) {
+    pack_empty_kernel<<<be, 256, 0, s>>>(n_events, d_ev_sample_off, d_ev_pix_off, d_pix_sample_off, d_n_pixrefs);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+  }
+  unsigned char* base = (unsigned char*)scratch;
+  uint64_t* keys = (uint64_t*)base;            base += a256(8 * (size_t)n);
+  uint64_t* keys_sorted = (uint64_t*)base;     base += a256(8 * (size_t)n);
+  int64_t* idx = (int64_t*)base;               base += a256(8 * (size_t)n);
+  int64_t* head = (int64_t*)base;              base += a256(8 * (size_t)n);
+  void* temp = base;
+  size_t temp_bytes = scratch_bytes - (size_t)(base - (unsigned char*)scratch);
+  const unsigned bn = (unsigned)((n + 255) / 256);
+  pack_keys_kernel<<<bn, 256, 0, s>>>(n, n_events, d_event_id, d_row, keys, idx, d_flag);
+  ++launches;
+  int end_bit = 32;
+  while (end_bit < 64 && ((uint64_t)n_events >> (end_bit - 32)) != 0) ++end_bit;
+  if (cub::DeviceRadixSort::SortPairs(temp, temp_bytes, keys, keys_sorted, idx, d_perm, n, 0, end_bit, s) !=
+      cudaSuccess)
+    return -1;
+  launches += 8;  // radix passes (library; approximate count)
+  pack_event_off_kernel<<<be, 256, 0, s>>>(n, n_events, keys_sorted, d_ev_sample_off);
+  pack_heads_kernel<<<bn, 256, 0, s>>>(n, keys_sorted, head);
+  int64_t* pos = idx;  // the unsorted index array is free again
+  temp_bytes = scratch_bytes - (size_t)(base - (unsigned char*)scratch);
+  if (cub::DeviceScan::ExclusiveSum(temp, temp_bytes, head, pos, n, s) != cudaSuccess) return -1;
+  pack_runs_kernel<<<bn, 256, 0, s>>>(n, keys_sorted, head, pos, d_ev_pix_rows, d_pix_sample_off, d_n_pixrefs);
+  pack_pix_off_kernel<<<be, 256, 0, s>>>(n, n_events, d_ev_sample_off, pos, d_n_pixrefs, d_ev_pix_off);
+  launches += 6;
+  return cudaGetLastError() == cudaSuccess ? launches : -1;
+}
+
+}  // namespace gwc

@@ -1,0 +1,307 @@
+// reduce.cu -- the small kernels around the fused re-weighting kernel:
+//   per-sample preparation (theta-independent logs and the per-segment shift), work grouping,
+//   A4 (log L_i, N_eff of Eq. 8, n_live), the injection combine (log xi, Eq. 4),
+//   A6 (log L = sum_i log L_i - N log xi, Eq. 3), the all-sky mean,
+//   and two measurement helpers (FP64 issue-rate probe, accuracy self-test of math64.cuh).
+#include <math_constants.h>
+
+#include "gwc_internal.h"
+#include "math64.cuh"
+
+namespace gwc {
+
+namespace {
+
+constexpr int PREP_THREADS = 256;
+
+// One CTA per segment.  Pass 1: shift = max_k(-ln pi_k - ln m1z_k) over valid samples.  Pass 2: write
+//   dLc = d_L (NaN marks a dead sample), L1 = ln m1z, Q = ln(m2z/m1z), P = -ln pi - ln m1z - shift.
+__global__ void __launch_bounds__(PREP_THREADS) prep_kernel(const int64_t* __restrict__ seg_off,
+                                                             const double* __restrict__ dL,
+                                                             const double* __restrict__ m1z,
+                                                             const double* __restrict__ m2z,
+                                                             const double* __restrict__ lprior,
+                                                             const int32_t* __restrict__ row, int64_t n_rows,
+                                                             double* __restrict__ dLc, double* __restrict__ L1,
+                                                             double* __restrict__ Q, double* __restrict__ P,
+                                                             double* __restrict__ seg_shift) {
+  __shared__ double red[PREP_THREADS / 32];
+  __shared__ double s_shift;
+  const int seg = blockIdx.x, tid = threadIdx.x;
+  const int64_t s0 = seg_off[seg], s1 = seg_off[seg + 1];
+  double mx = -CUDART_INF;
+  for (int64_t k = s0 + tid; k < s1; k += PREP_THREADS) {
+    const double d = dL[k], a = m1z[k], b = m2z[k];
+    const double lp = lprior ? lprior[k] : 2.0 * log(d);
+    bool ok = isfinite(d) && isfinite(a) && isfinite(b) && isfinite(lp) && d > 0.0 && a > 0.0 && b > 0.0 && b <= a;
+    if (row) ok = ok && ((unsigned)row[k] < (unsigned)n_rows) && row[k] >= 0;
+    if (ok) mx = fmax(mx, -lp - log(a));
+  }
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((tid & 31) == 0) red[tid >> 5] = mx;
+  __syncthreads();
+  if (tid == 0) {
+    double m = red[0];
+    for (int i = 1; i < PREP_THREADS / 32; ++i) m = fmax(m, red[i]);
+    if (!(m > -CUDART_INF)) m = 0.0;  // no valid sample
+    s_shift = m;
+    seg_shift[seg] = m;
+  }
+  __syncthreads();
+  const double shift = s_shift;
+  for (int64_t k = s0 + tid; k < s1; k += PREP_THREADS) {
+    const double d = dL[k], a = m1z[k], b = m2z[k];
+    const double lp = lprior ? lprior[k] : 2.0 * log(d);
+    bool ok = isfinite(d) && isfinite(a) && isfinite(b) && isfinite(lp) && d > 0.0 && a > 0.0 && b > 0.0 && b <= a;
+    if (row) ok = ok && ((unsigned)row[k] < (unsigned)n_rows) && row[k] >= 0;
+    const double la = ok ? log(a) : 0.0;
+    dLc[k] = ok ? d : CUDART_NAN;
+    L1[k] = la;
+    Q[k] = ok ? log(b / a) : 0.0;
+    P[k] = ok ? (-lp - la) - shift : 0.0;
+  }
+}
+
+// group g = segments whose first sample lies in [g*target, (g+1)*target): binary search per group
+__global__ void make_groups_kernel(const int64_t* __restrict__ seg_off, int64_t n_seg, int64_t target, int n_groups,
+                                   int32_t* __restrict__ group_off) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g > n_groups) return;
+  if (g == n_groups) { group_off[g] = (int32_t)n_seg; return; }
+  const int64_t key = (int64_t)g * target;
+  int64_t lo = 0, hi = n_seg;  // first segment with seg_off[s] >= key
+  while (lo < hi) {
+    const int64_t mid = (lo + hi) >> 1;
+    if (seg_off[mid] < key) lo = mid + 1; else hi = mid;
+  }
+  group_off[g] = (int32_t)lo;
+}
+
+__global__ void uniform_segments_kernel(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i > n_seg) return;
+  const int64_t v = i * seg;
+  seg_off[i] = v < n ? v : n;
+}
+
+__global__ void finalize_events_kernel(const double* __restrict__ part_w, const int32_t* __restrict__ part_n,
+                                       const int64_t* __restrict__ seg_off, const double* __restrict__ seg_shift,
+                                       const double* __restrict__ tconst, int64_t n_theta, int64_t n_events,
+                                       double* __restrict__ logL, double* __restrict__ neff,
+                                       int64_t* __restrict__ nlive) {
+  const int64_t o = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (o >= n_theta * n_events) return;
+  const int64_t t = o / n_events, i = o - t * n_events;
+  const double valid = tconst[t * NCONST + C_VALID];
+  const double sw = part_w[2 * o], sw2 = part_w[2 * o + 1];
+  const int64_t S = seg_off[i + 1] - seg_off[i];
+  double l, ne;
+  if (valid != valid) {
+    l = CUDART_NAN;
+    ne = CUDART_NAN;
+  } else if (sw > 0.0) {
+    l = (log(sw) + seg_shift[i]) - log((double)S);
+    ne = sw * sw / sw2;
+  } else {
+    l = -CUDART_INF;
+    ne = 0.0;
+  }
+  logL[o] = l;
+  if (neff) neff[o] = ne;
+  if (nlive) nlive[o] = (valid != valid) ? 0 : (int64_t)part_n[o];
+}
+
+// one thread per theta: log-sum-exp over the injection segments (each has its own shift), fixed order
+__global__ void finalize_inj_kernel(const double* __restrict__ part_w, const double* __restrict__ seg_shift,
+                                    const double* __restrict__ tconst, int64_t n_theta, int64_t n_seg, double n_draw,
+                                    double* __restrict__ logxi, double* __restrict__ neff) {
+  const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (t >= n_theta) return;
+  const double valid = tconst[t * NCONST + C_VALID];
+  if (valid != valid) {
+    logxi[t] = CUDART_NAN;
+    if (neff) neff[t] = CUDART_NAN;
+    return;
+  }
+  const double* pw = part_w + 2 * t * n_seg;
+  double smax = -CUDART_INF;
+  for (int64_t s = 0; s < n_seg; ++s)
+    if (pw[2 * s] > 0.0) smax = fmax(smax, seg_shift[s]);
+  if (!(smax > -CUDART_INF)) {
+    logxi[t] = -CUDART_INF;
+    if (neff) neff[t] = 0.0;
+    return;
+  }
+  double a = 0.0, b = 0.0;
+  for (int64_t s = 0; s < n_seg; ++s) {
+    const double e = exp(seg_shift[s] - smax);
+    a = fma(pw[2 * s], e, a);
+    b = fma(pw[2 * s + 1], e * e, b);
+  }
+  logxi[t] = (log(a) + smax) - log(n_draw);
+  if (neff) neff[t] = a * a / b;
+}
+
+constexpr int TOT_THREADS = 128;
+// one CTA per theta: strided partial sums, fixed-order tree
+__global__ void __launch_bounds__(TOT_THREADS) combine_total_kernel(const double* __restrict__ logL,
+                                                                     const double* __restrict__ logxi,
+                                                                     int64_t n_events, double* __restrict__ total) {
+  __shared__ double red[TOT_THREADS];
+  const int64_t t = blockIdx.x;
+  const int tid = threadIdx.x;
+  double s = 0.0;
+  for (int64_t i = tid; i < n_events; i += TOT_THREADS) s += logL[t * n_events + i];
+  red[tid] = s;
+  __syncthreads();
+  for (int o = TOT_THREADS / 2; o > 0; o >>= 1) {
+    if (tid < o) red[tid] += red[tid + o];
+    __syncthreads();
+  }
+  if (tid == 0) {
+    const double sum = red[0], x = logxi[t];
+    double r;
+    if (sum != sum || x != x) r = CUDART_NAN;
+    else if (sum == -CUDART_INF || x == -CUDART_INF) r = -CUDART_INF;
+    else r = sum - (double)n_events * x;
+    total[t] = r;
+  }
+}
+
+constexpr int AS_ROWS = 512;  // rows per partial block of the all-sky mean
+template <typename LosT>
+__global__ void allsky_partial_kernel(const LosT* __restrict__ table, int64_t n_rows, int n_z,
+                                      double* __restrict__ scratch) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= n_z) return;
+  const int64_t r0 = (int64_t)blockIdx.y * AS_ROWS, r1 = min(n_rows, r0 + AS_ROWS);
+  double s = 0.0;
+  for (int64_t r = r0; r < r1; ++r) s += (double)table[r * n_z + b];
+  scratch[(int64_t)blockIdx.y * n_z + b] = s;
+}
+__global__ void allsky_final_kernel(const double* __restrict__ scratch, int64_t n_parts, int64_t n_rows, int n_z,
+                                    double* __restrict__ allsky) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= n_z) return;
+  double s = 0.0;
+  for (int64_t p = 0; p < n_parts; ++p) s += scratch[p * n_z + b];
+  allsky[b] = s / (double)n_rows;
+}
+
+constexpr int PROBE_THREADS = 512;
+constexpr int PROBE_CHAINS = 8;
+__global__ void __launch_bounds__(PROBE_THREADS) probe_fp64_kernel(int64_t iters, double* sink) {
+  double a[PROBE_CHAINS];
+  const double m = 1.0 + 1e-9 * threadIdx.x, c = 1e-12 * blockIdx.x;
+#pragma unroll
+  for (int i = 0; i < PROBE_CHAINS; ++i) a[i] = 0.5 + i;
+  for (int64_t it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+      for (int i = 0; i < PROBE_CHAINS; ++i) a[i] = fma(a[i], m, c);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < PROBE_CHAINS; ++i) s += a[i];
+  if (s == 12345.678) sink[0] = s;  // keeps the chains alive
+}
+
+__global__ void math_selftest_kernel(int which, int64_t n, const double* __restrict__ in, double* __restrict__ out) {
+  __shared__ MathTables mt;
+  init_math_tables(mt, threadIdx.x);
+  __syncthreads();
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double x = in[i];
+  double y;
+  switch (which) {
+    case 0: y = exp_fast<true>(x, mt.exptab); break;
+    case 1: y = log_fast(x, mt.logtab); break;
+    case 2: y = rcp_fast(x); break;
+    case 3: y = rsqrt_fast(x); break;
+    default: y = exp_fast<false>(x, mt.exptab); break;
+  }
+  out[i] = y;
+}
+
+inline int ok() { return cudaGetLastError() == cudaSuccess ? 1 : -1; }
+
+}  // namespace
+
+int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const double* dL, const double* m1z,
+                        const double* m2z, const double* lprior, const int32_t* row, int64_t n_rows, double* dLc,
+                        double* L1, double* Q, double* P, double* seg_shift, cudaStream_t s) {
+  (void)n;
+  if (n_seg <= 0) return 0;
+  prep_kernel<<<(unsigned)n_seg, PREP_THREADS, 0, s>>>(seg_off, dL, m1z, m2z, lprior, row, n_rows, dLc, L1, Q, P,
+                                                       seg_shift);
+  return ok();
+}
+
+int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
+                       cudaStream_t s) {
+  make_groups_kernel<<<(n_groups + 1 + 127) / 128, 128, 0, s>>>(seg_off, n_seg, target, n_groups, group_off);
+  return ok();
+}
+
+int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off, cudaStream_t s) {
+  uniform_segments_kernel<<<(unsigned)((n_seg + 1 + 127) / 128), 128, 0, s>>>(n, seg, n_seg, seg_off);
+  return ok();
+}
+
+int launch_finalize_events(const double* part_w, const int32_t* part_n, const int64_t* seg_off, const double* seg_shift,
+                           const double* tconst, int64_t n_theta, int64_t n_events, double* logL, double* neff,
+                           int64_t* nlive, cudaStream_t s) {
+  const int64_t n = n_theta * n_events;
+  if (n <= 0) return 0;
+  finalize_events_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(part_w, part_n, seg_off, seg_shift, tconst,
+                                                                     n_theta, n_events, logL, neff, nlive);
+  return ok();
+}
+
+int launch_finalize_inj(const double* part_w, const double* seg_shift, const double* tconst, int64_t n_theta,
+                        int64_t n_seg, double n_draw, double* logxi, double* neff, cudaStream_t s) {
+  if (n_theta <= 0) return 0;
+  finalize_inj_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(part_w, seg_shift, tconst, n_theta, n_seg,
+                                                                        n_draw, logxi, neff);
+  return ok();
+}
+
+int launch_combine_total(const double* logL, const double* logxi, int64_t n_theta, int64_t n_events, double* total,
+                         cudaStream_t s) {
+  if (n_theta <= 0) return 0;
+  combine_total_kernel<<<(unsigned)n_theta, TOT_THREADS, 0, s>>>(logL, logxi, n_events, total);
+  return ok();
+}
+
+size_t allsky_scratch_doubles(int64_t n_rows, int n_z) {
+  return (size_t)((n_rows + AS_ROWS - 1) / AS_ROWS) * (size_t)n_z;
+}
+
+int launch_allsky(const void* table, gwc_prec prec, int64_t n_rows, int n_z, double* scratch, double* allsky,
+                  cudaStream_t s) {
+  const int64_t n_parts = (n_rows + AS_ROWS - 1) / AS_ROWS;
+  dim3 grid((n_z + 127) / 128, (unsigned)n_parts);
+  if (prec == GWC_F64)
+    allsky_partial_kernel<double><<<grid, 128, 0, s>>>((const double*)table, n_rows, n_z, scratch);
+  else
+    allsky_partial_kernel<float><<<grid, 128, 0, s>>>((const float*)table, n_rows, n_z, scratch);
+  if (ok() < 0) return -1;
+  allsky_final_kernel<<<(n_z + 127) / 128, 128, 0, s>>>(scratch, n_parts, n_rows, n_z, allsky);
+  return ok() < 0 ? -1 : 2;
+}
+
+int launch_probe_fp64(int64_t iters, int n_blocks, double* d_sink, cudaStream_t s, double* n_instr) {
+  probe_fp64_kernel<<<n_blocks, PROBE_THREADS, 0, s>>>(iters, d_sink);
+  *n_instr = (double)iters * 8.0 * PROBE_CHAINS * PROBE_THREADS * (double)n_blocks;
+  return ok();
+}
+
+int launch_math_selftest(int which, int64_t n, const double* d_in, double* d_out, cudaStream_t s) {
+  if (n <= 0) return 0;
+  math_selftest_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(which, n, d_in, d_out);
+  return ok();
+}
+
+}  // namespace gwc

@@ -1,0 +1,334 @@
+// reweight.cu -- A3/A5: the fused re-weighting kernel over (theta, segment, sample), plus the small
+// kernels around it (per-sample preparation, work grouping, A4 finalisation, A6 total).
+//
+// One sample's weight is Eq. 7 of the paper, w = p(z, m1, m2 | theta) / pi_PE, with the
+// line-of-sight prior of Eq. 5 read at the sample's own redshift and pixel
+// (R1), and Eq. 4 for the injections with the all-sky prior.  Written out
+// (readings R2-R8):
+//   u = d_L H0/c -> z by cubic Hermite on the per-theta table (A1);  x = 1+z;  m1 = m1z/x, m2 = m2z/x
+//   live iff u < umax, z < z_max, mmin < m1 <= mmax, m2 >= mmin, m2z <= m1z, p_los > 0
+//   w = [exp(CPL + c - alpha t1) + exp(CG + c - y^2/2)] p_los / [(u + x^2/E)(1 - e1)(1 + e2)]
+// with the per-theta constants of gwc_internal.h and the per-sample values prepared once per call
+// (ln m1z, ln(m2z/m1z), -ln pi - ln m1z - shift).  The sums over a segment's samples are taken in the
+// linear domain relative to a per-segment shift (the log-sum-exp reference, chosen before the sum
+// instead of tracked as a running maximum); log L_i = shift + ln(sum) - ln S_i  (A4).
+//
+// Mapping: a persistent CTA per SM takes work items (segment group, theta tile) from an atomic counter,
+// group-major so that CTAs running at the same time share the group's samples and LOS rows in L2.
+// The tile's inverse-cosmology tables and constants live in shared memory; samples are staged in
+// chunks; lanes are samples, each thread holds SPT samples per theta for independent FP64 chains;
+// per-(warp, theta) partial sums live in shared memory and are combined in a fixed order.
+#include <math_constants.h>
+
+#include "gwc_internal.h"
+#include "math64.cuh"
+
+namespace gwc {
+
+namespace {
+
+constexpr int SMEM_RESERVE = 256;  // static shared memory of the kernel + slack
+
+struct SmemLayout {
+  size_t math, tconst, acc, cnt, dLc, m1z, m2z, L1, Q, P, row, allsky, tab, total;
+};
+
+__host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
+
+__host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z) {
+  SmemLayout L;
+  size_t o = 0;
+  L.math = o;   o = align16(o + sizeof(MathTables));
+  L.tconst = o; o = align16(o + sizeof(double) * T * NCONST);
+  L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2);
+  L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T);
+  L.dLc = o;    o = align16(o + sizeof(double) * CHUNK);
+  L.m1z = o;    o = align16(o + sizeof(double) * CHUNK);
+  L.m2z = o;    o = align16(o + sizeof(double) * CHUNK);
+  L.L1 = o;     o = align16(o + sizeof(double) * CHUNK);
+  L.Q = o;      o = align16(o + sizeof(double) * CHUNK);
+  L.P = o;      o = align16(o + sizeof(double) * CHUNK);
+  L.row = o;    o = align16(o + (inj ? 0 : sizeof(int32_t) * CHUNK));
+  L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
+  L.tab = o;    o = align16(o + node_bytes * (size_t)T * Mp);
+  L.total = o;
+  return L;
+}
+
+__device__ __forceinline__ double widen(double v) { return v; }
+__device__ __forceinline__ double widen(float v) { return (double)v; }
+
+// Hermite data of one table interval, widened to f64
+__device__ __forceinline__ void load_nodes(const Node64* t, int m, double& z0, double& d0, double& z1, double& d1) {
+  const double2* q = reinterpret_cast<const double2*>(t + m);
+  double2 a = q[0], b = q[1];
+  z0 = a.x; d0 = a.y; z1 = b.x; d1 = b.y;
+}
+__device__ __forceinline__ void load_nodes(const Node32* t, int m, double& z0, double& d0, double& z1, double& d1) {
+  const float2* q = reinterpret_cast<const float2*>(t + m);
+  float2 a = q[0], b = q[1];
+  z0 = (double)a.x; d0 = (double)a.y; z1 = (double)b.x; d1 = (double)b.y;
+}
+
+struct Sample {
+  double dLc, m1z, m2z, L1, Q, P;
+};
+
+// One (theta, sample) term.  Returns the weight relative to the segment shift (0 when dead).
+// `lrow` points at the sample's LOS row (global memory) or at the all-sky table (shared memory).
+template <typename NodeT, typename LosT>
+__device__ __forceinline__ double term(const double* __restrict__ tc, const NodeT* __restrict__ tab,
+                                       const MathTables& mt, const Sample& s, const LosT* __restrict__ lrow,
+                                       double inv_dz, double los_zmax, double bmax, bool has_pl, bool has_g,
+                                       bool& live) {
+  // --- u -> z (cubic Hermite on the uniform-u table) ---
+  const double u0 = s.dLc * tc[C_H];
+  bool ok = u0 < tc[C_UMAX];  // false for NaN (samples marked dead by the preparation kernel)
+  const double u = ok ? u0 : 0.0;
+  double th = fma(u, tc[C_INVDU], -0.5);
+  double tm = th + MAGIC52;
+  const int m = __double2loint(tm);  // round(t - 1/2): floor(t) except on exact integers, where f = 1 gives the same z
+  tm -= MAGIC52;
+  const double f = fma(u, tc[C_INVDU], -tm);
+  double z0, d0, z1, d1;
+  load_nodes(tab, m, z0, d0, z1, d1);
+  const double dl = z1 - z0;
+  const double sd = d0 + d1;
+  const double c3 = fma(-2.0, dl, sd);
+  const double c2 = fma(3.0, dl, -(sd + d0));
+  const double z = fma(f, fma(f, fma(f, c3, c2), d0), z0);
+  ok = ok && (z < los_zmax);
+  const double x = 1.0 + z;
+  const double rx = rcp_fast(x);
+  const double m1 = s.m1z * rx, m2 = s.m2z * rx;
+  ok = ok && (m1 > tc[C_MMIN]) && (m1 <= tc[C_MMAX]) && (m2 >= tc[C_MMIN]);
+  // --- line-of-sight prior: linear interpolation between the two nodes around z ---
+  double tz = fmin(fma(z, inv_dz, -0.5), bmax);  // bmax = n_z - 1.75 keeps b <= n_z - 2
+  double tb = tz + MAGIC52;
+  const int b = __double2loint(tb);
+  tb -= MAGIC52;
+  const double fz = fma(z, inv_dz, -tb);
+  const LosT q0 = lrow[b], q1 = lrow[b + 1];
+  if (!__any_sync(0xffffffffu, ok)) {  // whole warp dead for this theta: skip the transcendental part
+    live = false;
+    return 0.0;
+  }
+  // --- population, rate, Jacobian ---
+  const double lx = log_fast(x, mt.logtab);
+  const double t1 = s.L1 - lx;  // ln m1
+  const double c = fma(tc[C_GM1], lx, fma(tc[C_BETA], s.Q, s.P));
+  double num = 0.0;
+  if (has_pl) num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), mt.exptab);
+  if (has_g) {
+    const double y = fma(m1, tc[C_INVSIG], tc[C_NMUSIG]);
+    num += exp_fast<true>(fma(-0.5 * y, y, c + tc[C_CG]), mt.exptab);
+  }
+  const double e1 = exp_fast<false>(fma(tc[C_NBP1], t1, tc[C_E1C]), mt.exptab);
+  const double e2 = exp_fast<false>(fma(tc[C_GK], lx, tc[C_E2C]), mt.exptab);
+  const double x2 = x * x;
+  const double rE = rsqrt_fast(fma(tc[C_OM] * x2, x, tc[C_OL]));
+  double den = fma(x2, rE, u);                     // u + x^2/E
+  den *= fma(-tc[C_SGN], e1, tc[C_SGN]);           // sign(beta+1) (1 - e1)
+  den *= 1.0 + e2;
+  const double p0 = widen(q0), p1 = widen(q1);
+  const double plos = fma(fz, p1 - p0, p0);
+  double w = num * plos * rcp_fast(den);
+  ok = ok && (plos > 0.0) && (w < CUDART_INF);     // also rejects NaN from a vanishing denominator
+  live = ok;
+  return ok ? w : 0.0;
+}
+
+template <typename NodeT, typename LosT, bool INJ>
+__global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightParams p) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ unsigned s_item;
+  const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z);
+  MathTables& mt = *reinterpret_cast<MathTables*>(smem + L.math);
+  double* s_tc = reinterpret_cast<double*>(smem + L.tconst);
+  double* s_acc = reinterpret_cast<double*>(smem + L.acc);
+  int* s_cnt = reinterpret_cast<int*>(smem + L.cnt);
+  double* s_dLc = reinterpret_cast<double*>(smem + L.dLc);
+  double* s_m1z = reinterpret_cast<double*>(smem + L.m1z);
+  double* s_m2z = reinterpret_cast<double*>(smem + L.m2z);
+  double* s_L1 = reinterpret_cast<double*>(smem + L.L1);
+  double* s_Q = reinterpret_cast<double*>(smem + L.Q);
+  double* s_P = reinterpret_cast<double*>(smem + L.P);
+  int32_t* s_row = reinterpret_cast<int32_t*>(smem + L.row);
+  double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
+  NodeT* s_tab = reinterpret_cast<NodeT*>(smem + L.tab);
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int T = p.T, Mp = p.Mp;
+  init_math_tables(mt, tid);
+  if (INJ) {
+    const double* a = reinterpret_cast<const double*>(p.los);
+    for (int i = tid; i < p.n_z; i += NTHREADS) s_allsky[i] = a[i];
+  }
+  const unsigned n_items = (unsigned)p.n_groups * (unsigned)p.n_tiles;
+  const double bmax = (double)p.n_z - 1.75;
+  int cur_tile = -1;
+
+  for (;;) {
+    __syncthreads();
+    if (tid == 0) s_item = atomicAdd(p.unit_counter, 1u);
+    __syncthreads();
+    const unsigned item = s_item;
+    if (item >= n_items) break;
+    const int group = (int)(item / (unsigned)p.n_tiles);
+    const int tile = (int)(item - (unsigned)group * (unsigned)p.n_tiles);
+    const int t0 = tile * T;
+    const int nt = min(T, p.n_theta - t0);
+    if (tile != cur_tile) {
+      // stage the tile's tables and constants (16-byte copies; rows are contiguous in global memory)
+      const uint4* src = reinterpret_cast<const uint4*>(reinterpret_cast<const NodeT*>(p.tab) + (size_t)t0 * Mp);
+      uint4* dst = reinterpret_cast<uint4*>(s_tab);
+      const int n16 = (int)(((size_t)nt * Mp * sizeof(NodeT)) / 16);
+      for (int i = tid; i < n16; i += NTHREADS) dst[i] = src[i];
+      for (int i = tid; i < nt * NCONST; i += NTHREADS) s_tc[i] = p.tconst[(size_t)t0 * NCONST + i];
+      cur_tile = tile;
+    }
+    for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) s_acc[i] = 0.0;
+    for (int i = tid; i < NWARPS * T; i += NTHREADS) s_cnt[i] = 0;
+    __syncthreads();
+
+    const int seg_lo = p.group_off[group], seg_hi = p.group_off[group + 1];
+    for (int seg = seg_lo; seg < seg_hi; ++seg) {
+      const int64_t s0 = p.seg_off[seg], s1 = p.seg_off[seg + 1];
+      for (int64_t c0 = s0; c0 < s1; c0 += CHUNK) {
+        const int n = (int)min((int64_t)CHUNK, s1 - c0);
+        // stage the chunk (coalesced); slots past the end are dead
+#pragma unroll
+        for (int k = 0; k < SPT; ++k) {
+          const int i = tid + k * NTHREADS;
+          const bool in = i < n;
+          const int64_t g = c0 + i;
+          s_dLc[i] = in ? p.dLc[g] : CUDART_NAN;
+          s_m1z[i] = in ? p.m1z[g] : 1.0;
+          s_m2z[i] = in ? p.m2z[g] : 1.0;
+          s_L1[i] = in ? p.L1[g] : 0.0;
+          s_Q[i] = in ? p.Q[g] : 0.0;
+          s_P[i] = in ? p.P[g] : 0.0;
+          if (!INJ) {
+            const int32_t r = in ? p.row[g] : 0;
+            s_row[i] = ((unsigned)r < (unsigned)p.n_rows) ? r : 0;  // out-of-range rows are dead (dLc = NaN)
+          }
+        }
+        __syncthreads();
+        // each thread keeps its SPT samples in registers across the theta loop
+        Sample smp[SPT];
+        const LosT* lrow[SPT];
+#pragma unroll
+        for (int k = 0; k < SPT; ++k) {
+          const int i = tid + k * NTHREADS;
+          smp[k].dLc = s_dLc[i]; smp[k].m1z = s_m1z[i]; smp[k].m2z = s_m2z[i];
+          smp[k].L1 = s_L1[i];   smp[k].Q = s_Q[i];     smp[k].P = s_P[i];
+          if (INJ) lrow[k] = reinterpret_cast<const LosT*>(s_allsky);
+          else lrow[k] = reinterpret_cast<const LosT*>(p.los) + (size_t)s_row[i] * (size_t)p.n_z;
+        }
+        if ((warp * 32) < n || (warp * 32 + NTHREADS) < n) {  // warps entirely past the ragged tail do nothing
+          for (int j = 0; j < nt; ++j) {
+            const double* tc = s_tc + j * NCONST;
+            const NodeT* tab = s_tab + (size_t)j * Mp;
+            const bool has_pl = tc[C_CPL] > -1e300, has_g = tc[C_CG] > -1e300;
+            double sw = 0.0, sw2 = 0.0;
+            int nl = 0;
+#pragma unroll
+            for (int k = 0; k < SPT; ++k) {
+              bool live;
+              const double w = term<NodeT, LosT>(tc, tab, mt, smp[k], lrow[k], p.inv_dz, p.los_zmax, bmax, has_pl,
+                                                 has_g, live);
+              sw += w;
+              sw2 = fma(w, w, sw2);
+              nl += __popc(__ballot_sync(0xffffffffu, live));
+            }
+            if (nl) {  // warp-uniform
+#pragma unroll
+              for (int o = 16; o > 0; o >>= 1) {
+                sw += __shfl_xor_sync(0xffffffffu, sw, o);
+                sw2 += __shfl_xor_sync(0xffffffffu, sw2, o);
+              }
+              if (lane == 0) {
+                double* a = s_acc + (warp * T + j) * 2;
+                a[0] += sw;
+                a[1] += sw2;
+                s_cnt[warp * T + j] += nl;
+              }
+            }
+          }
+        }
+        __syncthreads();
+      }
+      // segment complete: combine the warps' partials in a fixed order and write them out
+      if (tid < nt) {
+        double a = 0.0, b = 0.0;
+        int c = 0;
+        for (int w = 0; w < NWARPS; ++w) {
+          a += s_acc[(w * T + tid) * 2];
+          b += s_acc[(w * T + tid) * 2 + 1];
+          c += s_cnt[w * T + tid];
+          s_acc[(w * T + tid) * 2] = 0.0;
+          s_acc[(w * T + tid) * 2 + 1] = 0.0;
+          s_cnt[w * T + tid] = 0;
+        }
+        const size_t o = (size_t)(t0 + tid) * (size_t)p.n_seg + (size_t)seg;
+        p.out_w[2 * o] = a;
+        p.out_w[2 * o + 1] = b;
+        p.out_n[o] = c;
+      }
+      // (the barrier after the next chunk's staging orders this reset before the next accumulation)
+    }
+  }
+}
+
+template <typename NodeT, typename LosT, bool INJ>
+int launch_one(const ReweightParams& p, int n_blocks, size_t smem, cudaStream_t s) {
+  reweight_kernel<NodeT, LosT, INJ><<<n_blocks, NTHREADS, smem, s>>>(p);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+template <typename NodeT, typename LosT, bool INJ>
+int configure_one(int smem_optin) {
+  return cudaFuncSetAttribute(reweight_kernel<NodeT, LosT, INJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              smem_optin) == cudaSuccess ? 0 : -1;
+}
+
+}  // namespace
+
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z) {
+  return smem_layout(T, Mp, tab_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32), inj, n_z).total;
+}
+
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin) {
+  int best = 0;
+  for (int T = 1; T <= MAX_T; ++T)
+    if (reweight_smem_bytes(T, Mp, tab_prec, inj, n_z) + SMEM_RESERVE <= (size_t)smem_optin) best = T;
+  return best;
+}
+
+int reweight_configure(int smem_optin) {
+  smem_optin -= SMEM_RESERVE;  // room for the kernel's static shared memory
+  int rc = 0;
+  rc |= configure_one<Node64, double, false>(smem_optin);
+  rc |= configure_one<Node64, float, false>(smem_optin);
+  rc |= configure_one<Node32, double, false>(smem_optin);
+  rc |= configure_one<Node32, float, false>(smem_optin);
+  rc |= configure_one<Node64, double, true>(smem_optin);
+  rc |= configure_one<Node32, double, true>(smem_optin);
+  return rc;
+}
+
+int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_blocks,
+                    cudaStream_t s) {
+  const size_t smem = reweight_smem_bytes(p.T, p.Mp, tab_prec, inj, p.n_z);
+  if (inj) {
+    return tab_prec == GWC_F64 ? launch_one<Node64, double, true>(p, n_blocks, smem, s)
+                               : launch_one<Node32, double, true>(p, n_blocks, smem, s);
+  }
+  if (tab_prec == GWC_F64)
+    return los_prec == GWC_F64 ? launch_one<Node64, double, false>(p, n_blocks, smem, s)
+                               : launch_one<Node64, float, false>(p, n_blocks, smem, s);
+  return los_prec == GWC_F64 ? launch_one<Node32, double, false>(p, n_blocks, smem, s)
+                             : launch_one<Node32, float, false>(p, n_blocks, smem, s);
+}
+
+}  // namespace gwc

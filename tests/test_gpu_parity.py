@@ -1,0 +1,252 @@
+"""GPU parity tests: the CUDA path (through the C ABI binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are north_star's: bit-exact integers, relative 1e-9 on log L_i and
+log xi for the FP64 path, absolute 1e-4 on log L(theta) for the FP32-table path."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2605_23538_b200 import synth
+from util import ATOL_F32, RTOL_F64, assert_close_log, to_dev, workload
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2605_23538_b200 import gwc
+    c = gwc.Context(0)
+    yield c
+    c.close()
+
+
+DEV = "cuda:0"
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _oracle_all(W, theta, los=None, table_prec=0, n_nodes=1025):
+    los = W.los if los is None else los
+    ev, inj = synth.to_numpy(W.ev), synth.to_numpy(W.inj)
+    lt = _np(los)
+    logL, neff, nlive = oracle.event_loglik(_np(theta), ev, lt, W.spec.z_max, table_prec=table_prec, n_nodes=n_nodes)
+    allsky = oracle.los_allsky(lt, W.spec.z_max)
+    logxi, neffi = oracle.selection_logxi(_np(theta), inj, allsky, W.spec.z_max, table_prec=table_prec,
+                                          n_nodes=n_nodes)
+    total = oracle.total_from_parts(logL, logxi)
+    return dict(logL=logL, neff=neff, nlive=nlive, allsky=allsky, logxi=logxi, neff_inj=neffi, total=total)
+
+
+def _gpu_all(ctx, W, theta, los=None, table_prec=0, n_nodes=1025):
+    los = (W.los if los is None else los).to(DEV)
+    th = theta.to(DEV)
+    ev, inj = to_dev(W.ev, DEV), to_dev(W.inj, DEV)
+    zmax = W.spec.z_max
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    ctx.gwc_build_cosmo(th, zmax, n_nodes, table_prec)
+    logL, neff, nlive = ctx.gwc_event_loglik(th, ev, los, zmax)
+    logxi, neffi = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], zmax)
+    total = ctx.gwc_combine_total(logL, logxi)
+    total2 = ctx.gwc_total_loglik(th, ev, inj, los, zmax, allsky, n_nodes, table_prec)
+    torch.cuda.synchronize()
+    return dict(logL=_np(logL), neff=_np(neff), nlive=_np(nlive), allsky=_np(allsky), logxi=_np(logxi),
+                neff_inj=_np(neffi), total=_np(total), total2=_np(total2))
+
+
+def _compare(g, o, rtol=RTOL_F64, check_nlive=True):
+    np.testing.assert_allclose(g["allsky"], o["allsky"], rtol=1e-13, atol=0)
+    if check_nlive:
+        bad = np.argwhere(g["nlive"] != o["nlive"])
+        assert bad.size == 0, "nlive differs at %s" % bad[:8].tolist()
+    assert_close_log(g["logL"], o["logL"], rtol, "log L_i")
+    assert_close_log(g["logxi"], o["logxi"], rtol, "log xi")
+    fin = np.isfinite(o["logL"])
+    np.testing.assert_allclose(g["neff"][fin], o["neff"][fin], rtol=1e-7)
+    np.testing.assert_allclose(g["neff_inj"], o["neff_inj"], rtol=1e-7)
+    # log L(theta): sum of E terms each within rtol
+    assert_close_log(g["total"], o["total"], rtol, "log L(theta)")
+    assert np.array_equal(g["total"], g["total2"], equal_nan=True), "gwc_total_loglik != composed calls"
+
+
+# ---------------------------------------------------------------------------------------------
+def test_math_functions(ctx):
+    """exp/log/rcp/rsqrt of math64.cuh against torch's fp64 functions."""
+    g = torch.Generator(device="cpu").manual_seed(1)
+    x = (torch.rand(1 << 16, generator=g, dtype=torch.float64) * 1400.0 - 700.0).to(DEV)
+    for which in (0, 4):
+        y = ctx.gwc_math_selftest(which, x)
+        rel = ((y - torch.exp(x)) / torch.exp(x)).abs().max().item()
+        assert rel < 4e-15, rel
+    y = ctx.gwc_math_selftest(0, torch.tensor([-1e4, -float("inf"), -700.0], dtype=torch.float64, device=DEV))
+    assert torch.all(torch.isfinite(y)) and y.max().item() < 1e-300
+    xp = torch.exp((torch.rand(1 << 16, generator=g, dtype=torch.float64) * 40.0 - 20.0)).to(DEV)
+    xs = torch.cat([xp, 1.0 + torch.rand(1 << 16, generator=g, dtype=torch.float64).to(DEV) * 3.0])
+    y = ctx.gwc_math_selftest(1, xs)
+    assert (y - torch.log(xs)).abs().max().item() < 1e-15 * 24
+    assert ((y - torch.log(xs)).abs() / torch.log(xs).abs().clamp_min(1.0)).max().item() < 1e-15
+    y = ctx.gwc_math_selftest(2, xs)
+    assert ((y * xs) - 1.0).abs().max().item() < 5e-16
+    y = ctx.gwc_math_selftest(3, xs)
+    assert ((y * y * xs) - 1.0).abs().max().item() < 1e-15
+
+
+@pytest.mark.parametrize("n_nodes", [1025, 257, 2])
+def test_cosmo_table_nodes(ctx, n_nodes):
+    """A1: table nodes against the oracle's exact inverse (<= 1e-13) and its node slopes."""
+    oms = [0.05, 0.1, 0.3, 0.315, 0.5, 1.0]
+    th = torch.tensor([synth.THETA0] * len(oms), dtype=torch.float64)
+    th[:, 1] = torch.tensor(oms, dtype=torch.float64)
+    thd = th.to(DEV)
+    for zmax in (1.5, 2.0):
+        ctx.gwc_build_cosmo(thd, zmax, n_nodes, 0)
+        z, dz, umax = ctx.gwc_export_cosmo(len(oms), n_nodes)
+        ctx.gwc_check()
+        for i, om in enumerate(oms):
+            zt, dt, um = oracle.build_table(om, zmax, n_nodes)
+            assert abs(umax[i].item() - um) <= 2e-15 * um
+            np.testing.assert_allclose(_np(z[i]), zt, rtol=0, atol=1e-13)
+            np.testing.assert_allclose(_np(dz[i]), dt, rtol=1e-12, atol=0)
+            assert z[i, 0].item() == 0.0 and z[i, -1].item() == zmax
+
+
+def test_cosmo_closed_forms(ctx):
+    """A1 against the closed forms: Om = 1 => u = 2(1+z)(1 - (1+z)^-1/2); nodes must invert it."""
+    th = torch.tensor([synth.THETA0], dtype=torch.float64)
+    th[0, 1] = 1.0
+    ctx.gwc_build_cosmo(th.to(DEV), 2.0, 1025, 0)
+    z, _, umax = ctx.gwc_export_cosmo(1, 1025)
+    z = _np(z[0])
+    u = np.arange(1025) * (umax.item() / 1024)
+    np.testing.assert_allclose(2 * (1 + z) * (1 - (1 + z) ** -0.5), u, rtol=0, atol=3e-13)
+
+
+def test_tiny_parity(ctx):
+    W = workload("tiny")
+    o = _oracle_all(W, W.theta)
+    g = _gpu_all(ctx, W, W.theta)
+    ctx.gwc_check()
+    _compare(g, o)
+
+
+def test_ragged_o4_like_parity(ctx):
+    """O4-scale layout cut down so the oracle runs in seconds: ragged S_i and P_i, several chunks and a tail."""
+    W = workload("o4", n_theta=24, n_events=12, los_rows=600, n_inj=30_000, samples=(300, 4096), pixels=(16, 300))
+    o = _oracle_all(W, W.theta)
+    g = _gpu_all(ctx, W, W.theta)
+    ctx.gwc_check()
+    _compare(g, o)
+
+
+def test_box6_theta_parity_f32_los(ctx):
+    """Production-like: every theta has its own Om (table per theta), FP32 LOS table, FP64 cosmology table."""
+    W = workload("production", n_theta=20, n_events=10, los_rows=500, n_inj=20_000, samples=(700, 1500),
+                 pixels=(16, 200))
+    assert W.los.dtype == torch.float32
+    o = _oracle_all(W, W.theta)
+    g = _gpu_all(ctx, W, W.theta)
+    ctx.gwc_check()
+    _compare(g, o)
+
+
+def test_f32_table_variant(ctx):
+    """FP32 storage of the cosmology table and the LOS table, arithmetic in FP64 (R22):
+    bitwise-close to the oracle run with the same rounded tables, and within 1e-4 of the FP64 result."""
+    W = workload("stress", n_theta=16, n_events=10, los_rows=400, n_inj=20_000, big_samples=4096, big_pixels=300,
+                 big_frac=0.2)
+    los32 = W.los.to(torch.float32)
+    o32 = _oracle_all(W, W.theta, los=los32, table_prec=1)
+    g32 = _gpu_all(ctx, W, W.theta, los=los32, table_prec=1)
+    _compare(g32, o32, check_nlive=False)
+    o64 = _oracle_all(W, W.theta)
+    fin = np.isfinite(o64["total"]) & np.isfinite(g32["total"])
+    assert fin.any()
+    assert np.abs(g32["total"][fin] - o64["total"][fin]).max() <= ATOL_F32
+
+
+def test_edge_cases(ctx):
+    """Empty events, dead samples, invalid rows, lambda = 0, an invalid theta, user-supplied PE prior."""
+    W = workload("tiny")
+    ev = {k: (v.clone() if isinstance(v, torch.Tensor) else v) for k, v in W.ev.items()}
+    n = ev["dL"].numel()
+    # event 1 becomes empty: move its samples into event 0
+    off = ev["ev_sample_off"].clone()
+    off[1] = off[2]
+    ev["ev_sample_off"] = off
+    ev["dL"][3] = float("nan")
+    ev["dL"][5] = -1.0
+    ev["m1z"][7] = float("inf")
+    ev["m2z"][9] = ev["m1z"][9] * 1.5       # m2z > m1z: dead
+    ev["sample_row"][11] = 10_000           # out-of-range row: dead, no out-of-bounds read
+    ev["sample_row"][12] = -3
+    ev["dL"][n - 256:] = 1e9                # last event entirely beyond the table: log L_i = -inf
+    ev["log_pe_prior"] = (2.0 * torch.log(W.ev["dL"]) + 1234.5).contiguous()   # arbitrary constant offset
+    theta = W.theta.clone()
+    theta[2, 8] = 0.0                       # lambda = 0: no Gaussian term
+    theta[3, 8] = 1.0                       # lambda = 1: no power-law term
+    theta[5, 0] = -70.0                     # invalid H0: NaN outputs, sticky flag
+    W.ev = ev
+    o = _oracle_all(W, theta)
+    g = _gpu_all(ctx, W, theta)
+    from paper_2605_23538_b200 import gwc
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_check()
+    assert e.value.status == gwc.ERR_DOMAIN
+    ctx.gwc_check()  # flag cleared
+    assert np.isnan(g["logL"][5]).all() and np.isnan(g["total"][5])
+    assert np.isneginf(g["logL"][:5, 3]).all() and np.isneginf(g["logL"][:5, 1]).all()
+    _compare(g, o)
+
+
+def test_not_built_and_bad_args(ctx):
+    from paper_2605_23538_b200 import gwc
+    W = workload("tiny")
+    th = W.theta.to(DEV)
+    ev, los = to_dev(W.ev, DEV), W.los.to(DEV)
+    ctx.gwc_build_cosmo(th, 1.5, 1025, 0)
+    other = th.clone()
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_event_loglik(other, ev, los, 1.5)
+    assert e.value.status == gwc.ERR_NOT_BUILT
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_build_cosmo(th, 1.5, 1, 0)
+    assert e.value.status == gwc.ERR_SHAPE
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_build_cosmo(th, -1.0, 1025, 0)
+    assert e.value.status == gwc.ERR_INVALID_ARG
+
+
+def test_pack_events_bit_exact(ctx):
+    """A0: permutation, offsets, distinct rows and run starts equal the oracle's, bit for bit."""
+    g = torch.Generator().manual_seed(7)
+    n, ne = 50_000, 37
+    eid = torch.randint(0, ne, (n,), generator=g, dtype=torch.int32)
+    eid[eid == 5] = 6                      # an empty event in the middle
+    eid[eid == ne - 1] = 0                 # and at the end
+    row = torch.randint(0, 300, (n,), generator=g, dtype=torch.int32)
+    o = oracle.pack_events(eid.numpy(), row.numpy(), ne)
+    p = ctx.gwc_pack_events(eid.to(DEV), row.to(DEV), ne)
+    assert p["n_pixrefs"] == o["n_pixrefs"]
+    for k in ("perm", "ev_sample_off", "ev_pix_off", "ev_pix_rows", "pix_sample_off"):
+        assert np.array_equal(_np(p[k]), o[k]), k
+    p0 = ctx.gwc_pack_events(eid[:0].to(DEV), row[:0].to(DEV), 3)
+    assert p0["n_pixrefs"] == 0 and _np(p0["ev_sample_off"]).tolist() == [0, 0, 0, 0]
+
+
+def test_host_api_matches_device_api(ctx):
+    W = workload("tiny")
+    g = _gpu_all(ctx, W, W.theta)
+    out, up, down = ctx.gwc_total_loglik_host(W.theta, W.ev, W.inj, W.los, W.spec.z_max)
+    assert np.array_equal(out.numpy(), g["total"], equal_nan=True)
+    assert down == 8 * W.theta.shape[0] and up > W.los.numel() * 8
+
+
+def test_determinism(ctx):
+    W = workload("o4", n_theta=40, n_events=30, los_rows=600, n_inj=50_000, samples=(300, 3000), pixels=(16, 300))
+    a = _gpu_all(ctx, W, W.theta)
+    b = _gpu_all(ctx, W, W.theta)
+    for k in ("logL", "neff", "logxi", "total"):
+        assert np.array_equal(a[k], b[k], equal_nan=True), k
