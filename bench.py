@@ -1,0 +1,354 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (A1..A6, gwc_total_loglik) on synthetic catalogues.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload o5|production|o4|stress|tiny]
+                    [--impl gwc|reference] [--theta-scale F]
+
+A step = one pass of the whole hot path over one theta batch of the workload: cosmology tables, event
+re-weighting, selection term, total.  `value` = (theta x sample) terms per second with inputs resident in
+HBM (events + injections); `e2e` = the same through gwc_total_loglik_host with HOST buffers (uploads and
+the download inside the timed region).  N > 1: one process per GPU (torchrun), the theta batch is sharded
+by giving every rank its own full-size batch (weak scaling, replicated catalogue, no data-path collective).
+`--impl reference` times the CPU oracle on a bounded sample of the same workload (rank 0 only).
+Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2605_23538_b200 import synth  # noqa: E402
+
+METRIC = "(theta*event*sample) terms/s, whole hot path (events + injections)"
+UNIT = "terms/s"
+# Algorithmic FP64-pipe instructions per term of THIS formulation (counted from SASS)
+FP64_INSTR_LIVE = 125.0
+FP64_INSTR_DEAD = 32.0
+# B200 FP64 issue peak derived from the unit counts: 148 SMs x 64 FP64 lanes x 1.965 GHz
+FP64_PEAK_INSTR = 148 * 64 * 1.965e9
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(prefix="gwc_clocks_", suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            pass
+        try:
+            rows = [r.strip().split(", ") for r in open(self.path) if r.strip()]
+            os.unlink(self.path)
+        except Exception:
+            return out
+        sm, reasons, mx, pw = [], set(), None, []
+        for r in rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1]))
+                mx = float(r[2])
+                pw.append(float(r[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.strip().lower() == "active":
+                    reasons.add(name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=mx, reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw) if pw else None)
+        return out
+
+
+def _bench_spec(name: str, theta_scale: float):
+    spec = synth.CONFIGS[name]
+    if theta_scale != 1.0:
+        spec = synth.scaled(spec, n_theta=max(1, int(round(spec.n_theta * theta_scale))))
+    return spec
+
+
+def _pin(t):
+    return t.pin_memory() if isinstance(t, torch.Tensor) else t
+
+
+# ---------------------------------------------------------------------------------------------
+def run_gwc(args):
+    from paper_2605_23538_b200 import gwc
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    dist = world > 1
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the gwc path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if dist:
+        import torch.distributed as td
+        td.init_process_group("nccl", device_id=dev)
+    spec = _bench_spec(args.workload, args.theta_scale)
+    t_gen = time.time()
+    W = synth.make_workload(spec, seed=args.seed, device=dev, keep_f64_los=False)
+    # every rank owns a full-size theta batch of its own (weak scaling over theta)
+    theta = synth.make_theta(spec, args.seed + 7919 * rank, dev)
+    torch.cuda.synchronize()
+    t_gen = time.time() - t_gen
+    ctx = gwc.Context(local)
+    zmax = spec.z_max
+    prec = gwc.F32 if args.table_prec == "f32" else gwc.F64
+    allsky = ctx.gwc_los_allsky(W.los, zmax)
+    out = torch.empty(theta.shape[0], dtype=torch.float64, device=dev)
+    n_samples, n_inj, n_theta = W.n_samples, int(W.inj["dL"].numel()), int(theta.shape[0])
+    terms_ev, terms_inj = float(n_theta) * n_samples, float(n_theta) * n_inj
+    terms = terms_ev + terms_inj
+
+    def step():
+        ctx.gwc_total_loglik(theta, W.ev, W.inj, W.los, zmax, allsky, args.n_nodes, prec, out=out)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            td.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    # live fraction (untimed): needed for the algorithmic instruction count
+    ctx.gwc_build_cosmo(theta, zmax, args.n_nodes, prec)
+    _, _, nlive = ctx.gwc_event_loglik(theta, W.ev, W.los, zmax, want_neff=False, want_nlive=True)
+    live_frac_ev = float(nlive.sum().item()) / max(terms_ev, 1.0)
+    del nlive
+    barrier()
+    ctx.gwc_set_timing(True)
+    ctx.gwc_get_timing()
+    launches0 = ctx.gwc_launch_count()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else {}
+    launches = ctx.gwc_launch_count() - launches0
+    tm = ctx.gwc_get_timing()
+    ctx.gwc_set_timing(False)
+    ctx.gwc_check()
+    if dist:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        td.all_reduce(t, op=td.ReduceOp.MAX)
+        ms = float(t.item())
+    value = terms * world * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the host API (pinned host buffers, copies inside the timed region) ----
+    h_theta = _pin(theta.cpu())
+    h_ev = {k: _pin(v.cpu()) if isinstance(v, torch.Tensor) else v for k, v in W.ev.items()}
+    h_inj = {k: _pin(v.cpu()) if isinstance(v, torch.Tensor) else v for k, v in W.inj.items()}
+    h_los = _pin(W.los.cpu())
+    h_out = _pin(torch.empty(n_theta, dtype=torch.float64))
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    up = down = 0
+    _, up, down = ctx.gwc_total_loglik_host(h_theta, h_ev, h_inj, h_los, zmax, None, args.n_nodes, prec, out=h_out)
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(e2e_steps):
+        ctx.gwc_total_loglik_host(h_theta, h_ev, h_inj, h_los, zmax, None, args.n_nodes, prec, out=h_out)
+    e1.record()
+    barrier()
+    ms_e2e = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3 if not dist else 0.0)
+    if dist:
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+        td.all_reduce(t, op=td.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e_value = terms * world * e2e_steps / (ms_e2e * 1e-3)
+    same = bool(torch.equal(h_out, out.cpu()) or torch.allclose(h_out, out.cpu(), rtol=0, atol=0, equal_nan=True))
+
+    if rank != 0:
+        if dist:
+            td.destroy_process_group()
+        return
+    # ---- roofline of the dominant kernel (event re-weighting), timed live with CUDA events on its stream ----
+    ms_ev_kernel = tm["ms_ev"] / max(tm["n_ev"], 1)
+    ms_inj_kernel = tm["ms_inj"] / max(tm["n_inj"], 1)
+    instr = terms_ev * (live_frac_ev * FP64_INSTR_LIVE + (1.0 - live_frac_ev) * FP64_INSTR_DEAD)
+    achieved = instr * 2.0 / (ms_ev_kernel * 1e-3) / 1e12          # FP64 issue slots x 2 flop
+    peak = FP64_PEAK_INSTR * 2.0 / 1e12
+    probe_ms, probe_n = ctx.gwc_probe_fp64(1 << 13)
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "reweight_kernel<events>", "kernel_ms": ms_ev_kernel,
+                "kernel_share_of_step": ms_ev_kernel / (ms / args.steps),
+                "inj_kernel_ms": ms_inj_kernel,
+                "fp64_instr_per_live_term": FP64_INSTR_LIVE, "fp64_instr_per_dead_term": FP64_INSTR_DEAD,
+                "live_fraction_events": live_frac_ev,
+                "peak_source": "derived: 148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md section 7)",
+                "peak_measured_dfma_probe": probe_n * 2.0 / (probe_ms * 1e-3) / 1e12}
+    cpu = cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": spec.name, "n_theta": n_theta, "n_events": spec.n_events, "n_samples": n_samples,
+                   "n_injections": n_inj, "los_rows": spec.los_rows, "n_z": spec.n_z, "los_dtype": spec.los_dtype,
+                   "cosmo_table": "%s x %d nodes" % (args.table_prec, args.n_nodes), "seed": args.seed,
+                   "parallelism": "theta-sharded x%d, catalogue replicated" % world,
+                   "l2": "inputs larger than L2 (samples %.0f MB + LOS table %.0f MB per pass)"
+                         % (n_samples * 28 / 1e6, W.los.numel() * W.los.element_size() / 1e6),
+                   "generation_s": round(t_gen, 1)},
+        "evals_per_s": n_theta * world * args.steps / (ms * 1e-3),
+        "event_terms_per_s_kernel": terms_ev / (ms_ev_kernel * 1e-3),
+        "inj_terms_per_s_kernel": terms_inj / (ms_inj_kernel * 1e-3) if ms_inj_kernel > 0 else None,
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": up, "d2h_bytes_per_step": down,
+                "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps, "matches_device_path": same},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if dist:
+        td.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------------------------
+def cpu_baseline(spec, seed, W=None, theta=None, budget_s=15.0):
+    """The oracle as it stands, on the host cores, on a bounded sample of the workload:
+    the first theta points x the first events (all their samples) + the same theta x a slice of injections."""
+    import oracle
+    if W is None:
+        small = synth.scaled(spec, n_events=min(spec.n_events, 64), n_inj=min(spec.n_inj, 50_000),
+                             los_rows=min(spec.los_rows, 4096))
+        W = synth.make_workload(small, seed=seed, device="cpu", keep_f64_los=False)
+        theta = synth.make_theta(small, seed, "cpu")
+    cores = oracle.num_threads()
+    n_ev = min(int(W.ev["ev_sample_off"].numel()) - 1, 32)
+    off = W.ev["ev_sample_off"][: n_ev + 1].cpu()
+    ns = int(off[-1])
+    rows = W.ev["sample_row"][:ns].cpu().to(torch.int64)
+    r_lo, r_hi = int(rows.min()), int(rows.max()) + 1
+    # only the touched block of LOS rows goes to the host (row ids shifted to match)
+    los = W.los[r_lo:r_hi].cpu().numpy()
+    ev = {"ev_sample_off": off.numpy(), "dL": W.ev["dL"][:ns].cpu().numpy(), "m1z": W.ev["m1z"][:ns].cpu().numpy(),
+          "m2z": W.ev["m2z"][:ns].cpu().numpy(), "sample_row": (rows - r_lo).to(torch.int32).numpy(),
+          "log_pe_prior": None}
+    n_inj = min(int(W.inj["dL"].numel()), 4 * ns)
+    inj = {k: (v[:n_inj].cpu().numpy() if isinstance(v, torch.Tensor) else v) for k, v in W.inj.items()}
+    allsky = W.los.mean(0, dtype=torch.float64).cpu().numpy()   # plain torch, not the CUDA path
+    th = theta.cpu().numpy()
+    # calibrate on `cores` theta points, then size the timed run to the budget
+    n0 = min(cores, th.shape[0])
+    t0 = time.perf_counter()
+    oracle.event_loglik(th[:n0], ev, los, spec.z_max)
+    oracle.selection_logxi(th[:n0], inj, allsky, spec.z_max)
+    t_cal = max(time.perf_counter() - t0, 1e-3)
+    n_th = int(max(n0, min(th.shape[0], (budget_s / t_cal) * n0)))
+    n_th = max(cores, (n_th // cores) * cores) if th.shape[0] >= cores else th.shape[0]
+    n_th = min(n_th, th.shape[0])
+    t0 = time.perf_counter()
+    oracle.event_loglik(th[:n_th], ev, los, spec.z_max)
+    oracle.selection_logxi(th[:n_th], inj, allsky, spec.z_max)
+    dt = time.perf_counter() - t0
+    terms = float(n_th) * (ns + n_inj)
+    return {"value": terms / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%d theta x (first %d events = %d samples + first %d injections), TABLE mode, %.1f s"
+                      % (n_th, n_ev, ns, n_inj, dt),
+            "seconds": dt}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on a bounded sample, same metric/unit (rank 0 only)."""
+    if _env_int("RANK", 0) != 0:
+        return
+    spec = _bench_spec(args.workload, args.theta_scale)
+    small = synth.scaled(spec, n_events=min(spec.n_events, 32), n_inj=min(spec.n_inj, 100_000),
+                         los_rows=min(spec.los_rows, 4096), n_theta=min(spec.n_theta, 256))
+    W = synth.make_workload(small, seed=args.seed, device="cpu", keep_f64_los=False)
+    theta = synth.make_theta(small, args.seed, "cpu")
+    per_step = max(2.0, min(20.0, 120.0 / max(args.steps + args.warmup, 1)))
+    res = None
+    for _ in range(args.warmup):
+        res = cpu_baseline(small, args.seed, W=W, theta=theta, budget_s=per_step)
+    vals, secs = [], 0.0
+    for _ in range(args.steps):
+        res = cpu_baseline(small, args.seed, W=W, theta=theta, budget_s=per_step)
+        vals.append(res["value"])
+        secs += res["seconds"]
+    value = float(np.mean(vals))
+    res["value"] = value
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": _env_int("WORLD_SIZE", 1),
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / max(args.steps, 1) * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": spec.name, "sample": res["sample"], "seed": args.seed},
+            "cpu_baseline": res,
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="o5", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--impl", default="gwc", choices=["gwc", "reference"])
+    ap.add_argument("--theta-scale", type=float, default=1.0, help="scale the theta batch (profiling runs only)")
+    ap.add_argument("--table-prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--n-nodes", type=int, default=1025)
+    ap.add_argument("--seed", type=int, default=synth.DEFAULT_SEED)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle timing budget (0 = skip)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "gwc" and args.theta_scale == 1.0:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gwc(args)
+
+
+if __name__ == "__main__":
+    main()
