@@ -74,21 +74,29 @@ struct Sample {
   double dLc, m1z, m2z, L1, Q, P;
 };
 
-// One (theta, sample) term.  Returns the weight relative to the segment shift (0 when dead).
+// What the first half of a term hands to the second half.
+struct Mid {
+  double u, z, x, m1, fz, q0, q1;
+  bool ok;
+};
+
+__device__ __forceinline__ bool lt(double a, double b) { return a < b; }
+
+// First half of one (theta, sample) term: u -> z by cubic Hermite on the per-theta table, source-frame masses,
+// support tests, and the two line-of-sight nodes around z (loads issued here, consumed at the end of the term).
 // `lrow` points at the sample's LOS row (global memory) or at the all-sky table (shared memory).
+// No branch and no warp-synchronous operation: the SPT terms of a thread are interleaved by the scheduler.
 template <typename NodeT, typename LosT>
-__device__ __forceinline__ double term(const double* __restrict__ tc, const NodeT* __restrict__ tab,
-                                       const MathTables& mt, const Sample& s, const LosT* __restrict__ lrow,
-                                       double inv_dz, double los_zmax, double bmax, bool has_pl, bool has_g,
-                                       bool& live) {
-  // --- u -> z (cubic Hermite on the uniform-u table) ---
+__device__ __forceinline__ void term_head(const double* __restrict__ tc, const NodeT* __restrict__ tab, const Sample& s,
+                                          const LosT* __restrict__ lrow, double inv_dz, double los_zmax, int bmax,
+                                          Mid& o) {
   const double u0 = s.dLc * tc[C_H];
   bool ok = u0 < tc[C_UMAX];  // false for NaN (samples marked dead by the preparation kernel)
   const double u = ok ? u0 : 0.0;
-  double th = fma(u, tc[C_INVDU], -0.5);
-  double tm = th + MAGIC52;
+  const double th = fma(u, tc[C_INVDU], -0.5);
+  double tm = th + KM[K_MAGIC];
   const int m = __double2loint(tm);  // round(t - 1/2): floor(t) except on exact integers, where f = 1 gives the same z
-  tm -= MAGIC52;
+  tm -= KM[K_MAGIC];
   const double f = fma(u, tc[C_INVDU], -tm);
   double z0, d0, z1, d1;
   load_nodes(tab, m, z0, d0, z1, d1);
@@ -97,45 +105,61 @@ __device__ __forceinline__ double term(const double* __restrict__ tc, const Node
   const double c3 = fma(-2.0, dl, sd);
   const double c2 = fma(3.0, dl, -(sd + d0));
   const double z = fma(f, fma(f, fma(f, c3, c2), d0), z0);
-  ok = ok && (z < los_zmax);
   const double x = 1.0 + z;
   const double rx = rcp_fast(x);
   const double m1 = s.m1z * rx, m2 = s.m2z * rx;
-  ok = ok && (m1 > tc[C_MMIN]) && (m1 <= tc[C_MMAX]) && (m2 >= tc[C_MMIN]);
-  // --- line-of-sight prior: linear interpolation between the two nodes around z ---
-  double tz = fmin(fma(z, inv_dz, -0.5), bmax);  // bmax = n_z - 1.75 keeps b <= n_z - 2
-  double tb = tz + MAGIC52;
-  const int b = __double2loint(tb);
-  tb -= MAGIC52;
-  const double fz = fma(z, inv_dz, -tb);
-  const LosT q0 = lrow[b], q1 = lrow[b + 1];
-  if (!__any_sync(0xffffffffu, ok)) {  // whole warp dead for this theta: skip the transcendental part
-    live = false;
-    return 0.0;
-  }
-  // --- population, rate, Jacobian ---
+  ok = ok & lt(z, los_zmax) & (m1 > tc[C_MMIN]) & (m1 <= tc[C_MMAX]) & (m2 >= tc[C_MMIN]);
+  // line-of-sight prior: the two nodes around z (index clamped for dead samples beyond the table)
+  double tb = fma(z, inv_dz, -0.5) + KM[K_MAGIC];
+  const int b = min(__double2loint(tb), bmax);
+  tb -= KM[K_MAGIC];
+  o.fz = fma(z, inv_dz, -tb);
+  o.q0 = widen(lrow[b]);
+  o.q1 = widen(lrow[b + 1]);
+  o.u = u; o.z = z; o.x = x; o.m1 = m1; o.ok = ok;
+}
+
+// Second half: population, rate, Jacobian and the LOS interpolation.  Returns the weight relative to the
+// segment shift (0 when dead).
+__device__ __forceinline__ double term_tail(const double* __restrict__ tc, const MathTables& mt, const Sample& s,
+                                            const Mid& h, bool& live) {
+  const double x = h.x;
   const double lx = log_fast(x, mt.logtab);
   const double t1 = s.L1 - lx;  // ln m1
   const double c = fma(tc[C_GM1], lx, fma(tc[C_BETA], s.Q, s.P));
-  double num = 0.0;
-  if (has_pl) num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), mt.exptab);
-  if (has_g) {
-    const double y = fma(m1, tc[C_INVSIG], tc[C_NMUSIG]);
-    num += exp_fast<true>(fma(-0.5 * y, y, c + tc[C_CG]), mt.exptab);
-  }
+  // lambda = 1 / lambda = 0: CPL / CG is -inf, the clamped exponential returns e^-700 (~1e-304, nothing)
+  const double y = fma(h.m1, tc[C_INVSIG], tc[C_NMUSIG]);
+  const double num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), mt.exptab) +
+                     exp_fast<true>(fma(-0.5 * y, y, c + tc[C_CG]), mt.exptab);
   const double e1 = exp_fast<false>(fma(tc[C_NBP1], t1, tc[C_E1C]), mt.exptab);
   const double e2 = exp_fast<false>(fma(tc[C_GK], lx, tc[C_E2C]), mt.exptab);
   const double x2 = x * x;
   const double rE = rsqrt_fast(fma(tc[C_OM] * x2, x, tc[C_OL]));
-  double den = fma(x2, rE, u);                     // u + x^2/E
+  double den = fma(x2, rE, h.u);                   // u + x^2/E
   den *= fma(-tc[C_SGN], e1, tc[C_SGN]);           // sign(beta+1) (1 - e1)
   den *= 1.0 + e2;
-  const double p0 = widen(q0), p1 = widen(q1);
-  const double plos = fma(fz, p1 - p0, p0);
-  double w = num * plos * rcp_fast(den);
-  ok = ok && (plos > 0.0) && (w < CUDART_INF);     // also rejects NaN from a vanishing denominator
+  const double plos = fma(h.fz, h.q1 - h.q0, h.q0);
+  const double w = num * plos * rcp_fast(den);
+  const bool ok = h.ok & (plos > 0.0) & lt(w, CUDART_INF);  // also rejects NaN from a vanishing denominator
   live = ok;
   return ok ? w : 0.0;
+}
+
+// Sums of four per-lane values over the warp in a fixed order: (a0, a1) belong to theta j, (b0, b1) to theta j+1.
+// Returns the total of a0 on lane 0, a1 on lane 8, b0 on lane 16, b1 on lane 24 (6 shuffles instead of 20).
+__device__ __forceinline__ double warp_sum4(double a0, double a1, double b0, double b1, int lane) {
+  const unsigned FULL = 0xffffffffu;
+  const bool up = (lane & 16) != 0;
+  double k0 = up ? b0 : a0, k1 = up ? b1 : a1;
+  k0 += __shfl_xor_sync(FULL, up ? a0 : b0, 16);
+  k1 += __shfl_xor_sync(FULL, up ? a1 : b1, 16);
+  const bool up8 = (lane & 8) != 0;
+  double k = up8 ? k1 : k0;
+  k += __shfl_xor_sync(FULL, up8 ? k0 : k1, 8);
+  k += __shfl_xor_sync(FULL, k, 4);
+  k += __shfl_xor_sync(FULL, k, 2);
+  k += __shfl_xor_sync(FULL, k, 1);
+  return k;
 }
 
 template <typename NodeT, typename LosT, bool INJ>
@@ -165,7 +189,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     for (int i = tid; i < p.n_z; i += NTHREADS) s_allsky[i] = a[i];
   }
   const unsigned n_items = (unsigned)p.n_groups * (unsigned)p.n_tiles;
-  const double bmax = (double)p.n_z - 1.75;
+  const int bmax = p.n_z - 2;
+  const double inv_dz = p.inv_dz, los_zmax = p.los_zmax;
   int cur_tile = -1;
 
   for (;;) {
@@ -217,6 +242,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         // each thread keeps its SPT samples in registers across the theta loop
         Sample smp[SPT];
         const LosT* lrow[SPT];
+        double dmin = CUDART_INF;  // smallest d_L of the warp's samples: a whole-warp range test per theta
 #pragma unroll
         for (int k = 0; k < SPT; ++k) {
           const int i = tid + k * NTHREADS;
@@ -224,34 +250,46 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           smp[k].L1 = s_L1[i];   smp[k].Q = s_Q[i];     smp[k].P = s_P[i];
           if (INJ) lrow[k] = reinterpret_cast<const LosT*>(s_allsky);
           else lrow[k] = reinterpret_cast<const LosT*>(p.los) + (size_t)s_row[i] * (size_t)p.n_z;
+          dmin = fmin(dmin, smp[k].dLc);  // fmin drops the NaN of dead samples
         }
-        if ((warp * 32) < n || (warp * 32 + NTHREADS) < n) {  // warps entirely past the ragged tail do nothing
-          for (int j = 0; j < nt; ++j) {
-            const double* tc = s_tc + j * NCONST;
-            const NodeT* tab = s_tab + (size_t)j * Mp;
-            const bool has_pl = tc[C_CPL] > -1e300, has_g = tc[C_CG] > -1e300;
-            double sw = 0.0, sw2 = 0.0;
-            int nl = 0;
 #pragma unroll
-            for (int k = 0; k < SPT; ++k) {
-              bool live;
-              const double w = term<NodeT, LosT>(tc, tab, mt, smp[k], lrow[k], p.inv_dz, p.los_zmax, bmax, has_pl,
-                                                 has_g, live);
-              sw += w;
-              sw2 = fma(w, w, sw2);
-              nl += __popc(__ballot_sync(0xffffffffu, live));
-            }
-            if (nl) {  // warp-uniform
+        for (int o = 16; o > 0; o >>= 1) dmin = fmin(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
+        if (dmin < CUDART_INF) {  // warps entirely past the ragged tail (or entirely dead) do nothing
+          for (int j = 0; j < nt; j += 2) {
+            double acc[2][2];
+            int cnt = 0;
 #pragma unroll
-              for (int o = 16; o > 0; o >>= 1) {
-                sw += __shfl_xor_sync(0xffffffffu, sw, o);
-                sw2 += __shfl_xor_sync(0xffffffffu, sw2, o);
+            for (int h = 0; h < 2; ++h) {
+              acc[h][0] = 0.0;
+              acc[h][1] = 0.0;
+              const int jj = min(j + h, nt - 1);
+              const double* tc = s_tc + jj * NCONST;
+              // the whole warp beyond this theta's table (or no second theta in the pair): nothing to add
+              if ((j + h < nt) & (dmin * tc[C_H] < tc[C_UMAX])) {
+                const NodeT* tab = s_tab + (size_t)jj * Mp;
+                Mid mid[SPT];
+#pragma unroll
+                for (int k = 0; k < SPT; ++k)
+                  term_head<NodeT, LosT>(tc, tab, smp[k], lrow[k], inv_dz, los_zmax, bmax, mid[k]);
+#pragma unroll
+                for (int k = 0; k < SPT; ++k) {
+                  bool live;
+                  const double w = term_tail(tc, mt, smp[k], mid[k], live);
+                  acc[h][0] += w;
+                  acc[h][1] = fma(w, w, acc[h][1]);
+                  cnt += (live ? 1 : 0) << (16 * h);
+                }
               }
-              if (lane == 0) {
-                double* a = s_acc + (warp * T + j) * 2;
-                a[0] += sw;
-                a[1] += sw2;
-                s_cnt[warp * T + j] += nl;
+            }
+            cnt = __reduce_add_sync(0xffffffffu, cnt);
+            if (cnt) {  // warp-uniform
+              const double k = warp_sum4(acc[0][0], acc[0][1], acc[1][0], acc[1][1], lane);
+              if ((lane & 7) == 0) {
+                const int h = lane >> 4;
+                if (j + h < nt) {
+                  s_acc[(warp * T + j + h) * 2 + ((lane >> 3) & 1)] += k;
+                  if ((lane & 8) == 0) s_cnt[warp * T + j + h] += (cnt >> (16 * h)) & 0xffff;
+                }
               }
             }
           }
