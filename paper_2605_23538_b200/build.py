@@ -37,6 +37,7 @@ def _stale(target: str, deps) -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ_DIR, exist_ok=True)
     nvcc = _nvcc()
+    extra = os.environ.get("GWC_NVCC_FLAGS", "").split()   # e.g. -DGWC_NTHREADS=768 (tuning experiments)
     jobs = []
     for src in SOURCES:
         s = os.path.join(CSRC, src)
@@ -46,7 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(job):
         s, o = job
-        cmd = [nvcc] + NVCC_FLAGS + ["-I", INCLUDE, "-c", s, "-o", o]
+        cmd = [nvcc] + NVCC_FLAGS + extra + ["-I", INCLUDE, "-c", s, "-o", o]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (s, r.stdout, r.stderr))

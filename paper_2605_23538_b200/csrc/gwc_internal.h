@@ -37,9 +37,15 @@ enum : int {
 };
 constexpr int NCONST = 24;  // padded row length (>= C_COUNT), keeps rows 64-byte aligned
 
-constexpr int NTHREADS = 512;     // threads per CTA of the fused kernel (one CTA per SM)
+#ifndef GWC_NTHREADS
+#define GWC_NTHREADS 512
+#endif
+#ifndef GWC_SPT
+#define GWC_SPT 2
+#endif
+constexpr int NTHREADS = GWC_NTHREADS;  // threads per CTA of the fused kernel (one CTA per SM)
 constexpr int NWARPS = NTHREADS / 32;
-constexpr int SPT = 2;            // samples per thread per theta (independent chains in flight)
+constexpr int SPT = GWC_SPT;      // samples per thread per theta (independent chains in flight)
 constexpr int CHUNK = NTHREADS * SPT;  // samples staged in shared memory per step
 constexpr int MAX_T = 16;         // theta points per tile (upper bound)
 constexpr int INJ_SEG = 8192;     // injections per segment of the selection reduction

@@ -20,6 +20,8 @@
 // per-(warp, theta) partial sums live in shared memory and are combined in a fixed order.
 #include <math_constants.h>
 
+#include <type_traits>
+
 #include "gwc_internal.h"
 #include "math64.cuh"
 
@@ -30,11 +32,13 @@ namespace {
 constexpr int SMEM_RESERVE = 256;  // static shared memory of the kernel + slack
 
 struct SmemLayout {
-  size_t math, tconst, acc, cnt, dLc, m1z, m2z, L1, Q, P, row, allsky, tab, total;
+  size_t math, tconst, acc, cnt, A, m2z, C, P, row, allsky, tab, total;
 };
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
+// Per-chunk sample staging: A = (d_L, m1z) and m2z feed the first half of a term, C = (ln m1z, ln(m2z/m1z))
+// and P the second half; pairs are read with one 128-bit shared load.
 __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z) {
   SmemLayout L;
   size_t o = 0;
@@ -42,11 +46,9 @@ __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_byt
   L.tconst = o; o = align16(o + sizeof(double) * T * NCONST);
   L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2);
   L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T);
-  L.dLc = o;    o = align16(o + sizeof(double) * CHUNK);
-  L.m1z = o;    o = align16(o + sizeof(double) * CHUNK);
+  L.A = o;      o = align16(o + sizeof(double2) * CHUNK);
   L.m2z = o;    o = align16(o + sizeof(double) * CHUNK);
-  L.L1 = o;     o = align16(o + sizeof(double) * CHUNK);
-  L.Q = o;      o = align16(o + sizeof(double) * CHUNK);
+  L.C = o;      o = align16(o + sizeof(double2) * CHUNK);
   L.P = o;      o = align16(o + sizeof(double) * CHUNK);
   L.row = o;    o = align16(o + (inj ? 0 : sizeof(int32_t) * CHUNK));
   L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
@@ -70,27 +72,41 @@ __device__ __forceinline__ void load_nodes(const Node32* t, int m, double& z0, d
   z0 = (double)a.x; d0 = (double)a.y; z1 = (double)b.x; d1 = (double)b.y;
 }
 
-struct Sample {
-  double dLc, m1z, m2z, L1, Q, P;
-};
-
-// What the first half of a term hands to the second half.
+// What the first half of a term hands to the second half (carried across one step of the theta pipeline).
+template <typename LosT>
 struct Mid {
-  double u, z, x, m1, fz, q0, q1;
+  double u, z, m1, fz;
+  LosT q0, q1;
   bool ok;
 };
 
 __device__ __forceinline__ bool lt(double a, double b) { return a < b; }
 
+// LOS node loads.  From global memory they are volatile asm: the load stays in the pipeline stage that computes
+// its address (the compiler would otherwise sink it next to its use, one stage later, and expose the L2 latency).
+template <bool GLOBAL>
+__device__ __forceinline__ float los_load(const float* p) {
+  if (!GLOBAL) return *p;
+  float v;
+  asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+  return v;
+}
+template <bool GLOBAL>
+__device__ __forceinline__ double los_load(const double* p) {
+  if (!GLOBAL) return *p;
+  double v;
+  asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+
 // First half of one (theta, sample) term: u -> z by cubic Hermite on the per-theta table, source-frame masses,
-// support tests, and the two line-of-sight nodes around z (loads issued here, consumed at the end of the term).
-// `lrow` points at the sample's LOS row (global memory) or at the all-sky table (shared memory).
-// No branch and no warp-synchronous operation: the SPT terms of a thread are interleaved by the scheduler.
-template <typename NodeT, typename LosT>
-__device__ __forceinline__ void term_head(const double* __restrict__ tc, const NodeT* __restrict__ tab, const Sample& s,
-                                          const LosT* __restrict__ lrow, double inv_dz, double los_zmax, int bmax,
-                                          Mid& o) {
-  const double u0 = s.dLc * tc[C_H];
+// support tests, and the loads of the two line-of-sight nodes around z.  `lrow` points at the sample's LOS row
+// (global memory) or at the all-sky table (shared memory).  No branch, no warp-synchronous operation.
+template <typename NodeT, typename LosT, bool GLOBAL>
+__device__ __forceinline__ void term_head(const double* __restrict__ tc, const NodeT* __restrict__ tab, double2 A,
+                                          double m2z, const LosT* __restrict__ lrow, double inv_dz, double los_zmax,
+                                          int bmax, Mid<LosT>& o) {
+  const double u0 = A.x * tc[C_H];
   bool ok = u0 < tc[C_UMAX];  // false for NaN (samples marked dead by the preparation kernel)
   const double u = ok ? u0 : 0.0;
   const double th = fma(u, tc[C_INVDU], -0.5);
@@ -105,28 +121,28 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
   const double c3 = fma(-2.0, dl, sd);
   const double c2 = fma(3.0, dl, -(sd + d0));
   const double z = fma(f, fma(f, fma(f, c3, c2), d0), z0);
-  const double x = 1.0 + z;
-  const double rx = rcp_fast(x);
-  const double m1 = s.m1z * rx, m2 = s.m2z * rx;
+  const double rx = rcp_fast(1.0 + z);
+  const double m1 = A.y * rx, m2 = m2z * rx;
   ok = ok & lt(z, los_zmax) & (m1 > tc[C_MMIN]) & (m1 <= tc[C_MMAX]) & (m2 >= tc[C_MMIN]);
   // line-of-sight prior: the two nodes around z (index clamped for dead samples beyond the table)
   double tb = fma(z, inv_dz, -0.5) + KM[K_MAGIC];
   const int b = min(__double2loint(tb), bmax);
   tb -= KM[K_MAGIC];
   o.fz = fma(z, inv_dz, -tb);
-  o.q0 = widen(lrow[b]);
-  o.q1 = widen(lrow[b + 1]);
-  o.u = u; o.z = z; o.x = x; o.m1 = m1; o.ok = ok;
+  o.q0 = los_load<GLOBAL>(lrow + b);
+  o.q1 = los_load<GLOBAL>(lrow + b + 1);
+  o.u = u; o.z = z; o.m1 = m1; o.ok = ok;
 }
 
-// Second half: population, rate, Jacobian and the LOS interpolation.  Returns the weight relative to the
-// segment shift (0 when dead).
-__device__ __forceinline__ double term_tail(const double* __restrict__ tc, const MathTables& mt, const Sample& s,
-                                            const Mid& h, bool& live) {
-  const double x = h.x;
+// Second half: population, rate, Jacobian and the LOS interpolation.  C = (ln m1z, ln(m2z/m1z)),
+// P = -ln pi - ln m1z - shift.  Returns the weight relative to the segment shift (0 when dead).
+template <typename LosT>
+__device__ __forceinline__ double term_tail(const double* __restrict__ tc, const MathTables& mt, double2 C, double P,
+                                            const Mid<LosT>& h, bool& live) {
+  const double x = 1.0 + h.z;
   const double lx = log_fast(x, mt.logtab);
-  const double t1 = s.L1 - lx;  // ln m1
-  const double c = fma(tc[C_GM1], lx, fma(tc[C_BETA], s.Q, s.P));
+  const double t1 = C.x - lx;  // ln m1
+  const double c = fma(tc[C_GM1], lx, fma(tc[C_BETA], C.y, P));
   // lambda = 1 / lambda = 0: CPL / CG is -inf, the clamped exponential returns e^-700 (~1e-304, nothing)
   const double y = fma(h.m1, tc[C_INVSIG], tc[C_NMUSIG]);
   const double num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), mt.exptab) +
@@ -138,14 +154,15 @@ __device__ __forceinline__ double term_tail(const double* __restrict__ tc, const
   double den = fma(x2, rE, h.u);                   // u + x^2/E
   den *= fma(-tc[C_SGN], e1, tc[C_SGN]);           // sign(beta+1) (1 - e1)
   den *= 1.0 + e2;
-  const double plos = fma(h.fz, h.q1 - h.q0, h.q0);
+  const double q0 = widen(h.q0), q1 = widen(h.q1);
+  const double plos = fma(h.fz, q1 - q0, q0);
   const double w = num * plos * rcp_fast(den);
   const bool ok = h.ok & (plos > 0.0) & lt(w, CUDART_INF);  // also rejects NaN from a vanishing denominator
   live = ok;
   return ok ? w : 0.0;
 }
 
-// Sums of four per-lane values over the warp in a fixed order: (a0, a1) belong to theta j, (b0, b1) to theta j+1.
+// Sums of four per-lane values over the warp in a fixed order: (a0, a1) belong to one theta, (b0, b1) to another.
 // Returns the total of a0 on lane 0, a1 on lane 8, b0 on lane 16, b1 on lane 24 (6 shuffles instead of 20).
 __device__ __forceinline__ double warp_sum4(double a0, double a1, double b0, double b1, int lane) {
   const unsigned FULL = 0xffffffffu;
@@ -162,20 +179,27 @@ __device__ __forceinline__ double warp_sum4(double a0, double a1, double b0, dou
   return k;
 }
 
+// index of the lowest set bit, which is then cleared (-1 when empty)
+__device__ __forceinline__ int pop_lowest(unsigned& mask) {
+  if (!mask) return -1;
+  const int j = __ffs(mask) - 1;
+  mask &= mask - 1;
+  return j;
+}
+
 template <typename NodeT, typename LosT, bool INJ>
 __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
+  typedef typename std::conditional<INJ, double, LosT>::type RowT;  // the all-sky table is f64
   const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z);
   MathTables& mt = *reinterpret_cast<MathTables*>(smem + L.math);
   double* s_tc = reinterpret_cast<double*>(smem + L.tconst);
   double* s_acc = reinterpret_cast<double*>(smem + L.acc);
   int* s_cnt = reinterpret_cast<int*>(smem + L.cnt);
-  double* s_dLc = reinterpret_cast<double*>(smem + L.dLc);
-  double* s_m1z = reinterpret_cast<double*>(smem + L.m1z);
+  double2* s_A = reinterpret_cast<double2*>(smem + L.A);
   double* s_m2z = reinterpret_cast<double*>(smem + L.m2z);
-  double* s_L1 = reinterpret_cast<double*>(smem + L.L1);
-  double* s_Q = reinterpret_cast<double*>(smem + L.Q);
+  double2* s_C = reinterpret_cast<double2*>(smem + L.C);
   double* s_P = reinterpret_cast<double*>(smem + L.P);
   int32_t* s_row = reinterpret_cast<int32_t*>(smem + L.row);
   double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
@@ -227,11 +251,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           const int i = tid + k * NTHREADS;
           const bool in = i < n;
           const int64_t g = c0 + i;
-          s_dLc[i] = in ? p.dLc[g] : CUDART_NAN;
-          s_m1z[i] = in ? p.m1z[g] : 1.0;
+          s_A[i] = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
           s_m2z[i] = in ? p.m2z[g] : 1.0;
-          s_L1[i] = in ? p.L1[g] : 0.0;
-          s_Q[i] = in ? p.Q[g] : 0.0;
+          s_C[i] = make_double2(in ? p.L1[g] : 0.0, in ? p.Q[g] : 0.0);
           s_P[i] = in ? p.P[g] : 0.0;
           if (!INJ) {
             const int32_t r = in ? p.row[g] : 0;
@@ -239,59 +261,97 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           }
         }
         __syncthreads();
-        // each thread keeps its SPT samples in registers across the theta loop
-        Sample smp[SPT];
-        const LosT* lrow[SPT];
+        // Samples stay in shared memory (read where used: registers go to the interleaved chains instead);
+        // a thread keeps only the address of each of its samples' LOS rows.
+        const RowT* lrow[SPT];
         double dmin = CUDART_INF;  // smallest d_L of the warp's samples: a whole-warp range test per theta
 #pragma unroll
         for (int k = 0; k < SPT; ++k) {
           const int i = tid + k * NTHREADS;
-          smp[k].dLc = s_dLc[i]; smp[k].m1z = s_m1z[i]; smp[k].m2z = s_m2z[i];
-          smp[k].L1 = s_L1[i];   smp[k].Q = s_Q[i];     smp[k].P = s_P[i];
-          if (INJ) lrow[k] = reinterpret_cast<const LosT*>(s_allsky);
-          else lrow[k] = reinterpret_cast<const LosT*>(p.los) + (size_t)s_row[i] * (size_t)p.n_z;
-          dmin = fmin(dmin, smp[k].dLc);  // fmin drops the NaN of dead samples
+          if (INJ) lrow[k] = reinterpret_cast<const RowT*>(s_allsky);
+          else lrow[k] = reinterpret_cast<const RowT*>(p.los) + (size_t)s_row[i] * (size_t)p.n_z;
+          dmin = fmin(dmin, s_A[i].x);  // fmin drops the NaN of dead samples
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) dmin = fmin(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
-        if (dmin < CUDART_INF) {  // warps entirely past the ragged tail (or entirely dead) do nothing
-          for (int j = 0; j < nt; j += 2) {
-            double acc[2][2];
+        // theta points of the tile for which at least one sample of this warp lies inside the table
+        // (none for warps entirely past the ragged tail)
+        unsigned todo = __ballot_sync(0xffffffffu, lane < nt && dmin * s_tc[min(lane, nt - 1) * NCONST + C_H] <
+                                                                    s_tc[min(lane, nt - 1) * NCONST + C_UMAX]);
+        // Software pipeline over the theta points: the first half of the next point (table look-up, LOS loads)
+        // is issued together with the second half of the current one, so its latencies hide behind FP64 work.
+        int ja = pop_lowest(todo);
+        if (ja >= 0) {
+          Mid<RowT> cur[SPT], nxt[SPT];
+#pragma unroll
+          for (int k = 0; k < SPT; ++k) {
+            const int i = tid + k * NTHREADS;
+            term_head<NodeT, RowT, !INJ>(s_tc + ja * NCONST, s_tab + (size_t)ja * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz,
+                                   los_zmax, bmax, cur[k]);
+          }
+          for (;;) {
+            const int jb = pop_lowest(todo);
+            const int jh = jb >= 0 ? jb : ja;  // (a redundant look-up when the list ends on an odd count)
+            double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
             int cnt = 0;
+            {
+              const double* tch = s_tc + jh * NCONST;
+              const double* tct = s_tc + ja * NCONST;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              acc[h][0] = 0.0;
-              acc[h][1] = 0.0;
-              const int jj = min(j + h, nt - 1);
-              const double* tc = s_tc + jj * NCONST;
-              // the whole warp beyond this theta's table (or no second theta in the pair): nothing to add
-              if ((j + h < nt) & (dmin * tc[C_H] < tc[C_UMAX])) {
-                const NodeT* tab = s_tab + (size_t)jj * Mp;
-                Mid mid[SPT];
+              for (int k = 0; k < SPT; ++k) {
+                const int i = tid + k * NTHREADS;
+                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz, los_zmax, bmax,
+                                       nxt[k]);
+              }
 #pragma unroll
-                for (int k = 0; k < SPT; ++k)
-                  term_head<NodeT, LosT>(tc, tab, smp[k], lrow[k], inv_dz, los_zmax, bmax, mid[k]);
+              for (int k = 0; k < SPT; ++k) {
+                const int i = tid + k * NTHREADS;
+                bool live;
+                const double w = term_tail<RowT>(tct, mt, s_C[i], s_P[i], cur[k], live);
+                a0 += w;
+                a1 = fma(w, w, a1);
+                cnt += live ? 1 : 0;
+              }
+            }
+            const int jc = pop_lowest(todo);
+            {
+              // (when the list ends on an odd count this second step runs on a repeated point and is discarded:
+              // a branch here would let the compiler sink the loads of the first step behind it)
+              const bool second = jb >= 0;
+              const int jh2 = jc >= 0 ? jc : jh;
+              const double* tch = s_tc + jh2 * NCONST;
+              const double* tct = s_tc + jh * NCONST;
 #pragma unroll
-                for (int k = 0; k < SPT; ++k) {
-                  bool live;
-                  const double w = term_tail(tc, mt, smp[k], mid[k], live);
-                  acc[h][0] += w;
-                  acc[h][1] = fma(w, w, acc[h][1]);
-                  cnt += (live ? 1 : 0) << (16 * h);
-                }
+              for (int k = 0; k < SPT; ++k) {
+                const int i = tid + k * NTHREADS;
+                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh2 * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz,
+                                             los_zmax, bmax, cur[k]);
+              }
+#pragma unroll
+              for (int k = 0; k < SPT; ++k) {
+                const int i = tid + k * NTHREADS;
+                bool live;
+                double w = term_tail<RowT>(tct, mt, s_C[i], s_P[i], nxt[k], live);
+                live = live & second;
+                w = live ? w : 0.0;
+                b0 += w;
+                b1 = fma(w, w, b1);
+                cnt += live ? 0x10000 : 0;
               }
             }
             cnt = __reduce_add_sync(0xffffffffu, cnt);
             if (cnt) {  // warp-uniform
-              const double k = warp_sum4(acc[0][0], acc[0][1], acc[1][0], acc[1][1], lane);
+              const double k = warp_sum4(a0, a1, b0, b1, lane);
               if ((lane & 7) == 0) {
-                const int h = lane >> 4;
-                if (j + h < nt) {
-                  s_acc[(warp * T + j + h) * 2 + ((lane >> 3) & 1)] += k;
-                  if ((lane & 8) == 0) s_cnt[warp * T + j + h] += (cnt >> (16 * h)) & 0xffff;
+                const int j = (lane & 16) ? jb : ja;
+                if (j >= 0) {
+                  s_acc[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
+                  if ((lane & 8) == 0) s_cnt[warp * T + j] += (lane & 16) ? (cnt >> 16) : (cnt & 0xffff);
                 }
               }
             }
+            if (jc < 0) break;
+            ja = jc;
           }
         }
         __syncthreads();
