@@ -228,6 +228,7 @@ def run_gwc(args):
                 "peak_source": "derived: 148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md section 7)",
                 "peak_measured_dfma_probe": probe_n * 2.0 / (probe_ms * 1e-3) / 1e12}
     cpu = cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
+    stress = stress_report(ctx, W, theta, zmax, allsky, args.n_nodes) if spec.name == "stress" else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -249,9 +250,39 @@ def run_gwc(args):
         "roofline": roofline,
         "cpu_baseline": cpu,
     }
+    if stress is not None:
+        line["stress_report"] = stress
     print(json.dumps(line))
     if dist:
         td.destroy_process_group()
+
+
+def stress_report(ctx, W, theta, zmax, allsky, n_nodes):
+    """Config 5: FP64 tables and FP32 tables (cosmology + LOS) side by side on the whole theta batch (untimed):
+    max |delta log L(theta)|, the theta points where a sample flipped across a support edge, and N_eff per event."""
+    from paper_2605_23538_b200 import gwc
+    los64 = W.los if W.los.dtype == torch.float64 else W.los.to(torch.float64)
+    los32 = los64.to(torch.float32)
+    res = {}
+    for name, los, prec in (("f64", los64, gwc.F64), ("f32", los32, gwc.F32)):
+        ctx.gwc_build_cosmo(theta, zmax, n_nodes, prec)
+        logL, neff, nlive = ctx.gwc_event_loglik(theta, W.ev, los, zmax)
+        tot = ctx.gwc_total_loglik(theta, W.ev, W.inj, los, zmax, allsky, n_nodes, prec)
+        res[name] = (logL, neff, nlive, tot)
+    ctx.gwc_check()
+    t64, t32 = res["f64"][3], res["f32"][3]
+    both = torch.isfinite(t64) & torch.isfinite(t32)
+    same = (res["f64"][2] == res["f32"][2]).all(dim=1)
+    d = (t64 - t32).abs()
+    neff = res["f64"][1]
+    fin = torch.isfinite(res["f64"][0])
+    q = torch.quantile(neff[fin][:: max(1, int(fin.sum()) // 1_000_000)], torch.tensor([0.0, 0.05, 0.5, 0.95, 1.0],
+                                                                                      dtype=neff.dtype, device=neff.device))
+    mx = lambda m: float(d[m].max().item()) if bool(m.any()) else None
+    return {"n_theta_finite_both": int(both.sum()), "max_abs_dlogL_no_flip": mx(both & same),
+            "n_theta_with_flip": int((~same).sum()), "max_abs_dlogL_with_flip": mx(both & ~same),
+            "neff_per_event_quantiles_0_5_50_95_100": [float(x) for x in q],
+            "frac_event_terms_minus_inf": float((~fin).float().mean().item())}
 
 
 # ---------------------------------------------------------------------------------------------

@@ -1,0 +1,152 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same workload
+generator, same seed, same theta batch, same C-ABI calls).  The oracle cannot run 1e11 terms, so the
+comparison is on sampled outputs it can compute one by one:
+  * all events x a seeded subset of 8 theta points  -> log L_i, N_eff, nlive, log xi and log L(theta) in full
+  * all theta x a seeded subset of 16 events (the largest and the smallest included) -> log L_i, nlive
+o4 is compared in full.  Tolerances are north_star's (tests/util.py)."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2605_23538_b200 import synth
+from util import ATOL_F32, RTOL_F64, assert_close_log
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2605_23538_b200 import gwc
+    c = gwc.Context(0)
+    yield c
+    c.close()
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _sub_events(ev_np, ids):
+    """Host event dict restricted to the events `ids` (rows stay global)."""
+    off = ev_np["ev_sample_off"]
+    parts = [np.arange(off[i], off[i + 1]) for i in ids]
+    idx = np.concatenate(parts) if parts else np.zeros(0, np.int64)
+    new_off = np.zeros(len(ids) + 1, np.int64)
+    new_off[1:] = np.cumsum([p.size for p in parts])
+    return {"ev_sample_off": new_off, "dL": ev_np["dL"][idx], "m1z": ev_np["m1z"][idx], "m2z": ev_np["m2z"][idx],
+            "sample_row": ev_np["sample_row"][idx], "log_pe_prior": None}
+
+
+def _pick(n, k, seed, must=()):
+    rng = np.random.default_rng(seed)
+    ids = list(dict.fromkeys(list(must) + rng.permutation(n).tolist()))[:min(k, n)]
+    return np.array(sorted(ids), dtype=np.int64)
+
+
+def _run_gpu(ctx, W, theta, los, table_prec):
+    zmax = W.spec.z_max
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    ctx.gwc_build_cosmo(theta, zmax, 1025, table_prec)
+    logL, neff, nlive = ctx.gwc_event_loglik(theta, W.ev, los, zmax)
+    logxi, neffi = ctx.gwc_selection_logxi(theta, W.inj, allsky, los.shape[1], zmax)
+    total = ctx.gwc_total_loglik(theta, W.ev, W.inj, los, zmax, allsky, 1025, table_prec)
+    ctx.gwc_check()
+    torch.cuda.synchronize()
+    return dict(logL=logL, neff=neff, nlive=nlive, logxi=logxi, neff_inj=neffi, total=total, allsky=allsky)
+
+
+def _check_sampled(W, theta, los, g, table_prec, n_th=8, n_ev=16, rtol=RTOL_F64, check_nlive=True):
+    zmax = W.spec.z_max
+    ev_np, inj_np, los_np, th_np = synth.to_numpy(W.ev), synth.to_numpy(W.inj), _np(los), _np(theta)
+    E = ev_np["ev_sample_off"].size - 1
+    S = np.diff(ev_np["ev_sample_off"])
+    allsky = oracle.los_allsky(los_np, zmax)
+    np.testing.assert_allclose(_np(g["allsky"]), allsky, rtol=1e-13, atol=0)
+    kw = dict(table_prec=table_prec, n_nodes=1025)
+    # (a) all events x a theta subset: everything, including log L(theta)
+    tsel = _pick(th_np.shape[0], n_th, 11)
+    oL, oN, oC = oracle.event_loglik(th_np[tsel], ev_np, los_np, zmax, **kw)
+    oX, oXn = oracle.selection_logxi(th_np[tsel], inj_np, allsky, zmax, **kw)
+    oT = oracle.total_from_parts(oL, oX)
+    gL, gC = _np(g["logL"][tsel]), _np(g["nlive"][tsel])
+    if check_nlive:
+        assert np.array_equal(gC, oC), "nlive differs at %s" % np.argwhere(gC != oC)[:8].tolist()
+    worst = assert_close_log(gL, oL, rtol, "log L_i (theta subset)")
+    assert_close_log(_np(g["logxi"][tsel]), oX, rtol, "log xi")
+    assert_close_log(_np(g["total"][tsel]), oT, rtol, "log L(theta)")
+    fin = np.isfinite(oL)
+    neff_rtol = 1e-7 if rtol <= RTOL_F64 else 1e-3
+    np.testing.assert_allclose(_np(g["neff"][tsel])[fin], oN[fin], rtol=neff_rtol)
+    np.testing.assert_allclose(_np(g["neff_inj"][tsel]), oXn, rtol=neff_rtol)
+    # (b) all theta x an event subset (largest and smallest segments included)
+    esel = _pick(E, n_ev, 13, must=(int(np.argmax(S)), int(np.argmin(S))))
+    sub = _sub_events(ev_np, esel)
+    oL2, _, oC2 = oracle.event_loglik(th_np, sub, los_np, zmax, **kw)
+    gL2, gC2 = _np(g["logL"][:, esel]), _np(g["nlive"][:, esel])
+    if check_nlive:
+        assert np.array_equal(gC2, oC2), "nlive differs (event subset)"
+    worst = max(worst, assert_close_log(gL2, oL2, rtol, "log L_i (event subset)"))
+    return dict(tsel=tsel, total=oT, worst=worst)
+
+
+def _device_workload(name):
+    spec = synth.CONFIGS[name]
+    W = synth.make_workload(spec, seed=synth.DEFAULT_SEED, device=DEV, keep_f64_los=False)
+    theta = synth.make_theta(spec, synth.DEFAULT_SEED, DEV)     # rank 0's batch in bench.py
+    return W, theta
+
+
+def test_o4_full(ctx):
+    """O4-scale in full: every (theta, event) and every theta of the selection term."""
+    W, theta = _device_workload("o4")
+    g = _run_gpu(ctx, W, theta, W.los, 0)
+    n_th = theta.shape[0]
+    r = _check_sampled(W, theta, W.los, g, 0, n_th=n_th, n_ev=8)
+    assert r["tsel"].size == n_th
+
+
+@pytest.mark.parametrize("name", ["production", "o5"])
+def test_full_size_sampled(ctx, name):
+    W, theta = _device_workload(name)
+    assert W.los.dtype == torch.float32
+    g = _run_gpu(ctx, W, theta, W.los, 0)
+    _check_sampled(W, theta, W.los, g, 0)
+
+
+def test_stress_f64_and_f32_tables(ctx):
+    """Config 5: FP64 tables against the oracle at 1e-9; FP32 tables (LOS + cosmology) against the FP64 oracle at
+    1e-4 absolute on log L(theta), and at 1e-9 against the oracle run on the same rounded tables."""
+    W, theta = _device_workload("stress")
+    assert W.los.dtype == torch.float64
+    g64 = _run_gpu(ctx, W, theta, W.los, 0)
+    r64 = _check_sampled(W, theta, W.los, g64, 0)
+    los32 = W.los.to(torch.float32)
+    g32 = _run_gpu(ctx, W, theta, los32, 1)
+    # same rounded tables on both sides; a node whose f64 value sits on an f32 rounding boundary may round apart
+    # (|dz| <= 6e-8 on that interval), so this comparison is looser and nlive is not required to be identical
+    _check_sampled(W, theta, los32, g32, 1, n_ev=4, rtol=1e-6, check_nlive=False)
+    # A sample whose z (or m1 = m1z/(1+z)) lies within the f32 rounding of the z table (|dz| <= 6e-8 z) of a support
+    # edge is live with one table and dead with the other (R20/R22).  Such a flip changes log L_i by about
+    # w_k / sum w, far more than rounding does, so theta points with a flip are found through nlive, counted,
+    # printed and required to be rare; every other theta must meet north_star's 1e-4.
+    same = (g32["nlive"] == g64["nlive"]).all(dim=1).cpu().numpy()
+    a, b = _np(g32["total"]), _np(g64["total"])
+    both = np.isfinite(a) & np.isfinite(b)
+    d = np.abs(a - b)
+    n_flip = int((~same).sum())
+    print("stress f32 tables vs f64 tables, %d theta: max |dlogL(theta)| = %.3e without a flip (%d theta), "
+          "%.3e with one (%d theta)" % (both.sum(), d[both & same].max(), (both & same).sum(),
+                                        d[both & ~same].max() if (both & ~same).any() else 0.0, n_flip))
+    assert (both & same).sum() >= 0.9 * both.sum()
+    assert d[both & same].max() <= ATOL_F32
+    assert n_flip <= 0.1 * same.size
+    # against the FP64 oracle on the theta subset (flip-free points)
+    tsel = r64["tsel"]
+    t32, t64 = a[tsel], r64["total"]
+    fin = np.isfinite(t64) & np.isfinite(t32) & same[tsel]
+    assert fin.any()
+    assert np.abs(t32[fin] - t64[fin]).max() <= ATOL_F32
