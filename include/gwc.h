@@ -72,6 +72,9 @@ int64_t gwc_launch_count(const gwc_ctx* ctx);
  * inversion by Newton onto the uniform grid u_m = m*du, du = u(z_max)/(n_nodes-1), node slopes
  * z'(u) = 1/(u/(1+z) + (1+z)/E(z)); and the per-theta population constants.  Tables are kept in the
  * context (storage precision `table_prec`; arithmetic is always FP64) and are used by the calls below.
+ * table_prec = GWC_F32 selects 32-bit storage (8 bytes per node instead of 16): z_m as an unsigned 32-bit
+ * fixed-point fraction of z_max (absolute step z_max/(2^32-1)), the slope as a binary32 in the same units
+ * (R22).
  *   d_theta [n_theta][GWC_NPAR] f64, row-major.   z_max > 0.   n_nodes in [2, 8193] (1025 typical).
  */
 gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double z_max, int32_t n_nodes,

@@ -400,14 +400,24 @@ static int prep_cosmo(const double* th, int mode, double z_max, int M, orc_cosmo
   return 0;
 }
 
-/* optional FP32 storage of the cosmology table (reading R22): round to nearest, widen back */
-static void round_table_f32(double* buf, int M) {
-  for (int i = 0; i < 2 * M; ++i) buf[i] = (double)(float)buf[i];
+/* optional 32-bit storage of the cosmology table (reading R22): with q = z_max / (2^32 - 1),
+ * a node z_m is stored as the unsigned 32-bit integer nearest to z_m / q, its slope du z'_m as the binary32
+ * nearest to (du z'_m) / q; what the look-up reads back is integer * q and (double)float * q. */
+static void round_table_32(double* buf, int M, double z_max) {
+  const double qmax = 4294967295.0;
+  const double q = z_max / qmax;
+  for (int i = 0; i < M; ++i) {
+    double k = nearbyint(buf[i] / q);
+    if (k > qmax) k = qmax;
+    if (k < 0.0) k = 0.0;
+    buf[i] = k * q;
+  }
+  for (int i = M; i < 2 * M; ++i) buf[i] = (double)(float)(buf[i] / q) * q;
 }
 
 /*
  * log L_i(theta) = LSE_k log w_ik - ln S_i, N_eff,i, nlive_i  for every (theta, event).
- * Outputs [n_theta][n_events] row-major.  table_prec: 0 = f64 cosmology table, 1 = f32-rounded.
+ * Outputs [n_theta][n_events] row-major.  table_prec: 0 = f64 cosmology table, 1 = 32-bit storage (R22).
  */
 int orc_event_loglik(const double* theta, int64_t n_theta, const orc_events* ev, const orc_los* L, int mode,
                      double z_max, int M, int table_prec, double* logL, double* neff, int64_t* nlive) {
@@ -434,7 +444,7 @@ int orc_event_loglik(const double* theta, int64_t n_theta, const orc_events* ev,
     orc_cosmo_tab ct;
     double* buf = NULL;
     if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lw); continue; }
-    if (mode == 0 && table_prec == 1) round_table_f32(buf, M);
+    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
     for (int64_t i = 0; i < ev->n_events; ++i) {
       int64_t a = ev->ev_sample_off[i], b = ev->ev_sample_off[i + 1];
       int64_t cnt = 0;
@@ -485,7 +495,7 @@ int orc_selection_logxi(const double* theta, int64_t n_theta, const orc_injectio
     orc_cosmo_tab ct;
     double* buf = NULL;
     if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lw); continue; }
-    if (mode == 0 && table_prec == 1) round_table_f32(buf, M);
+    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
     for (int64_t k = 0; k < inj->n_found; ++k) {
       int live;
       lw[k] = orc_log_weight(th, mode, &ct, inj->dL[k], inj->m1z[k], inj->m2z[k], inj->log_pdraw[k], &A, 0, &live);

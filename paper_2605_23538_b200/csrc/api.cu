@@ -188,6 +188,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.n_z = n_z;
   p.inv_dz = (double)(n_z - 1) / los_zmax;
   p.los_zmax = los_zmax;
+  p.tab_zq = ctx->z_max / NODE32_QMAX;
   p.out_w = (double*)ctx->part_w.p;
   p.out_n = (int32_t*)ctx->part_n.p;
   p.unit_counter = ctx->d_counter;
@@ -317,7 +318,7 @@ gwc_status gwc_export_cosmo(gwc_ctx* ctx, double* d_z, double* d_dz, double* d_u
   if (!ctx) return GWC_ERR_INVALID_ARG;
   if (!ctx->built_theta) return fail(ctx, GWC_ERR_NOT_BUILT, "no cosmology table built");
   return count(ctx, launch_export_cosmo(ctx->tab.p, (const double*)ctx->tconst.p, ctx->built_n, ctx->M, ctx->Mp,
-                                        ctx->tab_prec, d_z, d_dz, d_umax, ctx->stream),
+                                        ctx->tab_prec, ctx->z_max, d_z, d_dz, d_umax, ctx->stream),
                "export_cosmo");
 }
 

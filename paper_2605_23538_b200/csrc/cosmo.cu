@@ -35,10 +35,12 @@ __device__ __forceinline__ double gl3(double a, double b, double Om, double OL) 
   return hm * s * (1.0 / 9.0);
 }
 
-__device__ __forceinline__ void store_node(Node64* t, double z, double d) { t->z = z; t->d = d; }
-__device__ __forceinline__ void store_node(Node32* t, double z, double d) {
-  t->z = __double2float_rn(z);
-  t->d = __double2float_rn(d);
+__device__ __forceinline__ void store_node(Node64* t, double z, double d, double) { t->z = z; t->d = d; }
+// 32-bit storage (R22): z_m as a fixed-point fraction of z_max (absolute step z_max / (2^32 - 1), 256x
+// finer than an f32 near z_max), the slope in the same units as an f32.
+__device__ __forceinline__ void store_node(Node32* t, double z, double d, double inv_q) {
+  t->zq = __double2uint_rn(fmin(z * inv_q, NODE32_QMAX));
+  t->d = __double2float_rn(d * inv_q);
 }
 
 __device__ bool theta_valid(const double* th) {
@@ -69,7 +71,7 @@ __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* _
   double* tc = tconst + (size_t)t * NCONST;
   const bool valid = theta_valid(th);
   if (!valid) {
-    for (int m = tid; m < Mp; m += CB_THREADS) store_node(row + m, 0.0, 0.0);
+    for (int m = tid; m < Mp; m += CB_THREADS) store_node(row + m, 0.0, 0.0, 0.0);
     if (tid < NCONST) tc[tid] = (tid == C_VALID) ? CUDART_NAN : 0.0;
     if (tid == 0) atomicOr(flag, 1);
     return;
@@ -143,7 +145,7 @@ __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* _
       double x = 1.0 + z;
       d = du / (u / x + x * invE(z, Om, OL));
     }
-    store_node(row + m, z, d);
+    store_node(row + m, z, d, NODE32_QMAX / z_max);
   }
   // 4. constants
   if (tid == 0) {
@@ -179,16 +181,21 @@ __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* _
   }
 }
 
+__device__ __forceinline__ double node_z(const Node64& n, double) { return n.z; }
+__device__ __forceinline__ double node_d(const Node64& n, double) { return n.d; }
+__device__ __forceinline__ double node_z(const Node32& n, double z_max) { return (double)n.zq * (z_max / NODE32_QMAX); }
+__device__ __forceinline__ double node_d(const Node32& n, double z_max) { return (double)n.d * (z_max / NODE32_QMAX); }
+
 template <typename NodeT>
 __global__ void export_cosmo_kernel(const NodeT* __restrict__ tab, const double* __restrict__ tconst, int64_t n_theta,
-                                    int M, int Mp, double* z, double* dz, double* umax) {
+                                    int M, int Mp, double z_max, double* z, double* dz, double* umax) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n_theta * M) return;
   int64_t t = i / M;
   int m = (int)(i - t * M);
   NodeT nd = tab[t * Mp + m];
-  if (z) z[i] = (double)nd.z;
-  if (dz) dz[i] = (double)nd.d;
+  if (z) z[i] = node_z(nd, z_max);
+  if (dz) dz[i] = node_d(nd, z_max);
   if (umax && m == 0) umax[t] = tconst[t * NCONST + C_UMAX];
 }
 
@@ -207,15 +214,15 @@ int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int
 }
 
 int launch_export_cosmo(const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp, gwc_prec prec,
-                        double* d_z, double* d_dz, double* d_umax, cudaStream_t s) {
+                        double z_max, double* d_z, double* d_dz, double* d_umax, cudaStream_t s) {
   int64_t n = n_theta * M;
   if (n <= 0) return 0;
   unsigned blocks = (unsigned)((n + 255) / 256);
   if (prec == GWC_F64)
-    export_cosmo_kernel<Node64><<<blocks, 256, 0, s>>>((const Node64*)d_tab, d_tconst, n_theta, M, Mp, d_z, d_dz,
+    export_cosmo_kernel<Node64><<<blocks, 256, 0, s>>>((const Node64*)d_tab, d_tconst, n_theta, M, Mp, z_max, d_z, d_dz,
                                                        d_umax);
   else
-    export_cosmo_kernel<Node32><<<blocks, 256, 0, s>>>((const Node32*)d_tab, d_tconst, n_theta, M, Mp, d_z, d_dz,
+    export_cosmo_kernel<Node32><<<blocks, 256, 0, s>>>((const Node32*)d_tab, d_tconst, n_theta, M, Mp, z_max, d_z, d_dz,
                                                        d_umax);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }

@@ -53,7 +53,8 @@ constexpr int QUAD_K = 1024;      // forward quadrature intervals of the cosmolo
 constexpr int MAX_NODES = 8193;
 
 struct Node64 { double z, d; };   // table node: z_m and du * z'(u_m)
-struct Node32 { float z, d; };
+struct Node32 { uint32_t zq; float d; };  // 32-bit storage: z_m = zq * z_max / (2^32 - 1), d in the same units
+constexpr double NODE32_QMAX = 4294967295.0;
 
 // table row length: M nodes + 1 pad node (index M is read when u rounds onto the last node), even
 __host__ __device__ inline int table_pitch(int M) { return (M + 2) & ~1; }
@@ -72,6 +73,7 @@ struct ReweightParams {
   int64_t n_rows;
   int n_z;
   double inv_dz, los_zmax;
+  double tab_zq;            // Node32 tables: z_max of the cosmology table / (2^32 - 1)
   double* out_w;            // [n_theta][n_seg][2]: sum w', sum w'^2
   int32_t* out_n;           // [n_theta][n_seg]   : n_live
   unsigned int* unit_counter;
@@ -81,7 +83,7 @@ struct ReweightParams {
 int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int M, int Mp, gwc_prec prec,
                        void* d_tab, double* d_tconst, int* d_flag, cudaStream_t s);
 int launch_export_cosmo(const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp, gwc_prec prec,
-                        double* d_z, double* d_dz, double* d_umax, cudaStream_t s);
+                        double z_max, double* d_z, double* d_dz, double* d_umax, cudaStream_t s);
 // per-sample, theta-independent preparation (+ per-segment shift = max(-ln pi - ln m1z))
 int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const double* dL, const double* m1z,
                         const double* m2z, const double* lprior, const int32_t* row, int64_t n_rows, double* dLc,

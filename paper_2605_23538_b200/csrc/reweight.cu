@@ -66,11 +66,14 @@ __device__ __forceinline__ void load_nodes(const Node64* t, int m, double& z0, d
   double2 a = q[0], b = q[1];
   z0 = a.x; d0 = a.y; z1 = b.x; d1 = b.y;
 }
+// (32-bit nodes: values in units of z_max / (2^32 - 1); the conversions run on the XU pipe, node_scale() follows)
 __device__ __forceinline__ void load_nodes(const Node32* t, int m, double& z0, double& d0, double& z1, double& d1) {
-  const float2* q = reinterpret_cast<const float2*>(t + m);
-  float2 a = q[0], b = q[1];
-  z0 = (double)a.x; d0 = (double)a.y; z1 = (double)b.x; d1 = (double)b.y;
+  const uint2* q = reinterpret_cast<const uint2*>(t + m);
+  const uint2 a = q[0], b = q[1];
+  z0 = (double)a.x; d0 = (double)__uint_as_float(a.y); z1 = (double)b.x; d1 = (double)__uint_as_float(b.y);
 }
+__device__ __forceinline__ double node_scale(const Node64*, double z, double) { return z; }
+__device__ __forceinline__ double node_scale(const Node32*, double z, double zq) { return z * zq; }
 
 // What the first half of a term hands to the second half (carried across one step of the theta pipeline).
 template <typename LosT>
@@ -105,7 +108,7 @@ __device__ __forceinline__ double los_load(const double* p) {
 template <typename NodeT, typename LosT, bool GLOBAL>
 __device__ __forceinline__ void term_head(const double* __restrict__ tc, const NodeT* __restrict__ tab, double2 A,
                                           double m2z, const LosT* __restrict__ lrow, double inv_dz, double los_zmax,
-                                          int bmax, Mid<LosT>& o) {
+                                          double zq, int bmax, Mid<LosT>& o) {
   const double u0 = A.x * tc[C_H];
   bool ok = u0 < tc[C_UMAX];  // false for NaN (samples marked dead by the preparation kernel)
   const double u = ok ? u0 : 0.0;
@@ -120,7 +123,7 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
   const double sd = d0 + d1;
   const double c3 = fma(-2.0, dl, sd);
   const double c2 = fma(3.0, dl, -(sd + d0));
-  const double z = fma(f, fma(f, fma(f, c3, c2), d0), z0);
+  const double z = node_scale(tab, fma(f, fma(f, fma(f, c3, c2), d0), z0), zq);
   const double rx = rcp_fast(1.0 + z);
   const double m1 = A.y * rx, m2 = m2z * rx;
   ok = ok & lt(z, los_zmax) & (m1 > tc[C_MMIN]) & (m1 <= tc[C_MMAX]) & (m2 >= tc[C_MMIN]);
@@ -214,7 +217,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   }
   const unsigned n_items = (unsigned)p.n_groups * (unsigned)p.n_tiles;
   const int bmax = p.n_z - 2;
-  const double inv_dz = p.inv_dz, los_zmax = p.los_zmax;
+  const double inv_dz = p.inv_dz, los_zmax = p.los_zmax, zq = p.tab_zq;
   int cur_tile = -1;
 
   for (;;) {
@@ -287,7 +290,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           for (int k = 0; k < SPT; ++k) {
             const int i = tid + k * NTHREADS;
             term_head<NodeT, RowT, !INJ>(s_tc + ja * NCONST, s_tab + (size_t)ja * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz,
-                                   los_zmax, bmax, cur[k]);
+                                   los_zmax, zq, bmax, cur[k]);
           }
           for (;;) {
             const int jb = pop_lowest(todo);
@@ -300,8 +303,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
                 const int i = tid + k * NTHREADS;
-                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz, los_zmax, bmax,
-                                       nxt[k]);
+                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz, los_zmax, zq,
+                                       bmax, nxt[k]);
               }
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
@@ -325,7 +328,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               for (int k = 0; k < SPT; ++k) {
                 const int i = tid + k * NTHREADS;
                 term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh2 * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz,
-                                             los_zmax, bmax, cur[k]);
+                                             los_zmax, zq, bmax, cur[k]);
               }
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
