@@ -162,7 +162,6 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   GWC_TRY(ensure(ctx, ctx->group_off, (size_t)(n_groups + 1) * sizeof(int32_t)));
   GWC_TRY(count(ctx, launch_make_groups(d_seg_off, n_seg, target, n_groups, (int32_t*)ctx->group_off.p, s),
                 "make_groups"));
-  GWC_CUDA(cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned int), s));
   ReweightParams p;
   memset(&p, 0, sizeof(p));
   p.tab = ctx->tab.p;
@@ -189,18 +188,17 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.inv_dz = (double)(n_z - 1) / los_zmax;
   p.los_zmax = los_zmax;
   p.tab_zq = ctx->z_max / NODE32_QMAX;
+  p.zero_mask = 0;
   p.out_w = (double*)ctx->part_w.p;
   p.out_n = (int32_t*)ctx->part_n.p;
   p.unit_counter = ctx->d_counter;
-  const int64_t n_items = (int64_t)n_groups * n_tiles;
-  const int n_blocks = (int)(n_items < ctx->n_sm ? n_items : ctx->n_sm);
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (ctx->timing) {
     e0 = get_event(ctx);
     e1 = get_event(ctx);
     cudaEventRecord(e0, s);
   }
-  GWC_TRY(count(ctx, launch_reweight(p, ctx->tab_prec, los_prec, inj, n_blocks, s), "reweight"));
+  GWC_TRY(count(ctx, launch_reweight(p, ctx->tab_prec, los_prec, inj, ctx->n_sm, s), "reweight"));
   if (ctx->timing) {
     cudaEventRecord(e1, s);
     auto& v = inj ? ctx->inj_pairs : ctx->ev_pairs;

@@ -46,7 +46,11 @@ constexpr int NCONST = 24;  // padded row length (>= C_COUNT), keeps rows 64-byt
 constexpr int NTHREADS = GWC_NTHREADS;  // threads per CTA of the fused kernel (one CTA per SM)
 constexpr int NWARPS = NTHREADS / 32;
 constexpr int SPT = GWC_SPT;      // samples per thread per theta (independent chains in flight)
-constexpr int CHUNK = NTHREADS * SPT;  // samples staged in shared memory per step
+#ifndef GWC_CHUNK
+#define GWC_CHUNK 1024
+#endif
+constexpr int CHUNK = GWC_CHUNK;  // samples staged in shared memory per step (a multiple of 32 * SPT)
+constexpr int KT_THETA = 340;     // theta points whose constants fit the constant bank (one launch)
 constexpr int MAX_T = 16;         // theta points per tile (upper bound)
 constexpr int INJ_SEG = 8192;     // injections per segment of the selection reduction
 constexpr int QUAD_K = 1024;      // forward quadrature intervals of the cosmology builder
@@ -62,7 +66,8 @@ __host__ __device__ inline int table_pitch(int M) { return (M + 2) & ~1; }
 struct ReweightParams {
   const void* tab;          // [n_theta][Mp] Node64 | Node32
   const double* tconst;     // [n_theta][NCONST]
-  int n_theta, M, Mp, T, n_tiles;
+  int n_theta, M, Mp, T, n_tiles;   // n_theta, n_tiles: of the batch (set per launch by launch_reweight)
+  int t_begin;              // first theta of this launch
   const double *dLc, *m1z, *m2z, *L1, *Q, *P;   // [n_samples] prepared per-sample values
   const int32_t* row;       // [n_samples] (events) or nullptr (injections)
   const int64_t* seg_off;   // [n_seg+1] device
@@ -77,6 +82,7 @@ struct ReweightParams {
   double* out_w;            // [n_theta][n_seg][2]: sum w', sum w'^2
   int32_t* out_n;           // [n_theta][n_seg]   : n_live
   unsigned int* unit_counter;
+  int zero_mask;            // always 0 (scheduling pin of the LOS loads, reweight.cu)
 };
 
 // kernels / launchers (each returns the number of kernels it launched, or -1 on a launch error)
@@ -94,7 +100,7 @@ int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_
 size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z);
 int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin);
 int reweight_configure(int smem_optin);
-int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_blocks,
+int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm,
                     cudaStream_t s);
 int launch_finalize_events(const double* part_w, const int32_t* part_n, const int64_t* seg_off, const double* seg_shift,
                            const double* tconst, int64_t n_theta, int64_t n_events, double* logL, double* neff,

@@ -208,19 +208,21 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_fp64_kernel(int64_t iters
 }
 
 __global__ void math_selftest_kernel(int which, int64_t n, const double* __restrict__ in, double* __restrict__ out) {
-  __shared__ MathTables mt;
-  init_math_tables(mt, threadIdx.x);
+  extern __shared__ __align__(16) unsigned char selftest_smem[];
+  MathTables& mt = *reinterpret_cast<MathTables*>(selftest_smem);
+  init_math_tables(mt, threadIdx.x, blockDim.x);
   __syncthreads();
+  const int lane = threadIdx.x & 31;
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   const double x = in[i];
   double y;
   switch (which) {
-    case 0: y = exp_fast<true>(x, mt.exptab); break;
-    case 1: y = log_fast(x, mt.logtab); break;
+    case 0: y = exp_fast<true>(x, mt.exptab + (lane & (EXP_REP - 1))); break;
+    case 1: y = log_fast(x, mt.logtab + (lane & (LOG_REP - 1))); break;
     case 2: y = rcp_fast(x); break;
     case 3: y = rsqrt_fast(x); break;
-    default: y = exp_fast<false>(x, mt.exptab); break;
+    default: y = exp_fast<false>(x, mt.exptab + (lane & (EXP_REP - 1))); break;
   }
   out[i] = y;
 }
@@ -300,7 +302,10 @@ int launch_probe_fp64(int64_t iters, int n_blocks, double* d_sink, cudaStream_t 
 
 int launch_math_selftest(int which, int64_t n, const double* d_in, double* d_out, cudaStream_t s) {
   if (n <= 0) return 0;
-  math_selftest_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(which, n, d_in, d_out);
+  if (cudaFuncSetAttribute(math_selftest_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MathTables)) !=
+      cudaSuccess)
+    return -1;
+  math_selftest_kernel<<<(unsigned)((n + 255) / 256), 256, sizeof(MathTables), s>>>(which, n, d_in, d_out);
   return ok();
 }
 

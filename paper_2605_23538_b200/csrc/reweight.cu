@@ -1,5 +1,4 @@
-// reweight.cu -- A3/A5: the fused re-weighting kernel over (theta, segment, sample), plus the small
-// kernels around it (per-sample preparation, work grouping, A4 finalisation, A6 total).
+// reweight.cu -- A3/A5: the fused re-weighting kernel over (theta, segment, sample).
 //
 // One sample's weight is Eq. 7 of the paper, w = p(z, m1, m2 | theta) / pi_PE, with the
 // line-of-sight prior of Eq. 5 read at the sample's own redshift and pixel
@@ -13,11 +12,19 @@
 // linear domain relative to a per-segment shift (the log-sum-exp reference, chosen before the sum
 // instead of tracked as a running maximum); log L_i = shift + ln(sum) - ln S_i  (A4).
 //
-// Mapping: a persistent CTA per SM takes work items (segment group, theta tile) from an atomic counter,
-// group-major so that CTAs running at the same time share the group's samples and LOS rows in L2.
-// The tile's inverse-cosmology tables and constants live in shared memory; samples are staged in
-// chunks; lanes are samples, each thread holds SPT samples per theta for independent FP64 chains;
-// per-(warp, theta) partial sums live in shared memory and are combined in a fixed order.
+// Mapping.  A persistent CTA per SM takes work items (segment group, theta tile) from an atomic counter,
+// group-major so that CTAs running at the same time share the group's samples and LOS rows in L2.  The
+// tile's inverse-cosmology tables live in shared memory.  Lanes are samples: a warp takes a block of
+// 32 * SPT consecutive samples of the segment straight from global memory into registers (coalesced; no
+// shared-memory staging, no barrier per block) and loops over the tile's theta points, software-pipelined:
+// the table look-up and the LOS loads of the next point are issued with the FP64 tail of the current one.
+// The per-theta constants are warp-uniform and come from the constant bank (uniform loads feeding the FP64
+// instructions directly: no shared-memory traffic, no vector registers); the bank holds KT_THETA points, so
+// a batch is processed in launches of at most that many.  What bounds the kernel besides the FP64 pipe is the
+// shared-memory pipe (one wavefront per clock per SM): the random look-ups of the exp / log tables are
+// conflict-free by replication (math64.cuh), leaving the Hermite node gathers as the only conflicted reads.
+// Per-(warp, theta) partial sums live in shared memory and are combined in a fixed order at the end of a
+// segment: no floating-point atomics, results are bitwise reproducible.
 #include <math_constants.h>
 
 #include <type_traits>
@@ -30,27 +37,23 @@ namespace gwc {
 namespace {
 
 constexpr int SMEM_RESERVE = 256;  // static shared memory of the kernel + slack
+constexpr int BLK = 32 * SPT;      // samples one warp holds in registers at a time
+
+// per-theta constants of the current launch (A2), read with uniform loads
+__constant__ double KT[KT_THETA * NCONST];
 
 struct SmemLayout {
-  size_t math, tconst, acc, cnt, A, m2z, C, P, row, allsky, tab, total;
+  size_t math, acc, cnt, allsky, tab, total;
 };
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
-// Per-chunk sample staging: A = (d_L, m1z) and m2z feed the first half of a term, C = (ln m1z, ln(m2z/m1z))
-// and P the second half; pairs are read with one 128-bit shared load.
 __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z) {
   SmemLayout L;
   size_t o = 0;
   L.math = o;   o = align16(o + sizeof(MathTables));
-  L.tconst = o; o = align16(o + sizeof(double) * T * NCONST);
   L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2);
   L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T);
-  L.A = o;      o = align16(o + sizeof(double2) * CHUNK);
-  L.m2z = o;    o = align16(o + sizeof(double) * CHUNK);
-  L.C = o;      o = align16(o + sizeof(double2) * CHUNK);
-  L.P = o;      o = align16(o + sizeof(double) * CHUNK);
-  L.row = o;    o = align16(o + (inj ? 0 : sizeof(int32_t) * CHUNK));
   L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
   L.tab = o;    o = align16(o + node_bytes * (size_t)T * Mp);
   L.total = o;
@@ -139,25 +142,40 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
 
 // Second half: population, rate, Jacobian and the LOS interpolation.  C = (ln m1z, ln(m2z/m1z)),
 // P = -ln pi - ln m1z - shift.  Returns the weight relative to the segment shift (0 when dead).
+// The loaded LOS nodes are tied to a value the tail computes late (OR with `late & zmask`, zmask = 0 at run time):
+// the compiler cannot then hoist their first use to the top of the stage, right behind the loads.
+__device__ __forceinline__ double pin_late(float q, int late, int zmask) {
+  return (double)__int_as_float(__float_as_int(q) | (late & zmask));
+}
+__device__ __forceinline__ double pin_late(double q, int late, int zmask) {
+  return __hiloint2double(__double2hiint(q) | (late & zmask), __double2loint(q));
+}
+
 template <typename LosT>
-__device__ __forceinline__ double term_tail(const double* __restrict__ tc, const MathTables& mt, double2 C, double P,
-                                            const Mid<LosT>& h, bool& live) {
+__device__ __forceinline__ double term_tail(const double* __restrict__ tc, const double2* __restrict__ logtab,
+                                            const double* __restrict__ exptab, double2 C, double P,
+                                            const Mid<LosT>& h, int zmask, bool& live) {
   const double x = 1.0 + h.z;
-  const double lx = log_fast(x, mt.logtab);
+  const double lx = log_fast(x, logtab);
   const double t1 = C.x - lx;  // ln m1
   const double c = fma(tc[C_GM1], lx, fma(tc[C_BETA], C.y, P));
   // lambda = 1 / lambda = 0: CPL / CG is -inf, the clamped exponential returns e^-700 (~1e-304, nothing)
   const double y = fma(h.m1, tc[C_INVSIG], tc[C_NMUSIG]);
-  const double num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), mt.exptab) +
-                     exp_fast<true>(fma(-0.5 * y, y, c + tc[C_CG]), mt.exptab);
-  const double e1 = exp_fast<false>(fma(tc[C_NBP1], t1, tc[C_E1C]), mt.exptab);
-  const double e2 = exp_fast<false>(fma(tc[C_GK], lx, tc[C_E2C]), mt.exptab);
+  const double num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), exptab) +
+                     exp_fast<true>(fma(-0.5 * y, y, c + tc[C_CG]), exptab);
+  const double e1 = exp_fast<false>(fma(tc[C_NBP1], t1, tc[C_E1C]), exptab);
+  const double e2 = exp_fast<false>(fma(tc[C_GK], lx, tc[C_E2C]), exptab);
   const double x2 = x * x;
   const double rE = rsqrt_fast(fma(tc[C_OM] * x2, x, tc[C_OL]));
   double den = fma(x2, rE, h.u);                   // u + x^2/E
   den *= fma(-tc[C_SGN], e1, tc[C_SGN]);           // sign(beta+1) (1 - e1)
   den *= 1.0 + e2;
+#ifdef GWC_PIN_LOS
+  const int late = __double2hiint(num);
+  const double q0 = pin_late(h.q0, late, zmask), q1 = pin_late(h.q1, late, zmask);
+#else
   const double q0 = widen(h.q0), q1 = widen(h.q1);
+#endif
   const double plos = fma(h.fz, q1 - q0, q0);
   const double w = num * plos * rcp_fast(den);
   const bool ok = h.ok & (plos > 0.0) & lt(w, CUDART_INF);  // also rejects NaN from a vanishing denominator
@@ -190,6 +208,16 @@ __device__ __forceinline__ int pop_lowest(unsigned& mask) {
   return j;
 }
 
+// One sample's theta-independent values, held in registers while the warp loops over the tile's theta points.
+template <typename RowT>
+struct Sample {
+  double2 A;  // (d_L or NaN when dead, m1z)
+  double m2z;
+  double2 C;  // (ln m1z, ln(m2z/m1z))
+  double P;   // -ln pi - ln m1z - shift
+  const RowT* lrow;
+};
+
 template <typename NodeT, typename LosT, bool INJ>
 __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -197,20 +225,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   typedef typename std::conditional<INJ, double, LosT>::type RowT;  // the all-sky table is f64
   const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z);
   MathTables& mt = *reinterpret_cast<MathTables*>(smem + L.math);
-  double* s_tc = reinterpret_cast<double*>(smem + L.tconst);
   double* s_acc = reinterpret_cast<double*>(smem + L.acc);
   int* s_cnt = reinterpret_cast<int*>(smem + L.cnt);
-  double2* s_A = reinterpret_cast<double2*>(smem + L.A);
-  double* s_m2z = reinterpret_cast<double*>(smem + L.m2z);
-  double2* s_C = reinterpret_cast<double2*>(smem + L.C);
-  double* s_P = reinterpret_cast<double*>(smem + L.P);
-  int32_t* s_row = reinterpret_cast<int32_t*>(smem + L.row);
   double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
   NodeT* s_tab = reinterpret_cast<NodeT*>(smem + L.tab);
 
+  const unsigned FULL = 0xffffffffu;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int T = p.T, Mp = p.Mp;
-  init_math_tables(mt, tid);
+  init_math_tables(mt, tid, NTHREADS);
+  const double2* logtab = mt.logtab + (lane & (LOG_REP - 1));  // this lane's copies: conflict-free look-ups
+  const double* exptab = mt.exptab + (lane & (EXP_REP - 1));
   if (INJ) {
     const double* a = reinterpret_cast<const double*>(p.los);
     for (int i = tid; i < p.n_z; i += NTHREADS) s_allsky[i] = a[i];
@@ -218,6 +243,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   const unsigned n_items = (unsigned)p.n_groups * (unsigned)p.n_tiles;
   const int bmax = p.n_z - 2;
   const double inv_dz = p.inv_dz, los_zmax = p.los_zmax, zq = p.tab_zq;
+  const int zmask = p.zero_mask;
   int cur_tile = -1;
 
   for (;;) {
@@ -228,15 +254,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     if (item >= n_items) break;
     const int group = (int)(item / (unsigned)p.n_tiles);
     const int tile = (int)(item - (unsigned)group * (unsigned)p.n_tiles);
-    const int t0 = tile * T;
+    const int t0 = tile * T;  // first theta of the tile, relative to this launch
     const int nt = min(T, p.n_theta - t0);
     if (tile != cur_tile) {
-      // stage the tile's tables and constants (16-byte copies; rows are contiguous in global memory)
-      const uint4* src = reinterpret_cast<const uint4*>(reinterpret_cast<const NodeT*>(p.tab) + (size_t)t0 * Mp);
+      // stage the tile's tables (16-byte copies; rows are contiguous in global memory)
+      const uint4* src =
+          reinterpret_cast<const uint4*>(reinterpret_cast<const NodeT*>(p.tab) + (size_t)(p.t_begin + t0) * Mp);
       uint4* dst = reinterpret_cast<uint4*>(s_tab);
       const int n16 = (int)(((size_t)nt * Mp * sizeof(NodeT)) / 16);
       for (int i = tid; i < n16; i += NTHREADS) dst[i] = src[i];
-      for (int i = tid; i < nt * NCONST; i += NTHREADS) s_tc[i] = p.tconst[(size_t)t0 * NCONST + i];
       cur_tile = tile;
     }
     for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) s_acc[i] = 0.0;
@@ -246,71 +272,57 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     const int seg_lo = p.group_off[group], seg_hi = p.group_off[group + 1];
     for (int seg = seg_lo; seg < seg_hi; ++seg) {
       const int64_t s0 = p.seg_off[seg], s1 = p.seg_off[seg + 1];
-      for (int64_t c0 = s0; c0 < s1; c0 += CHUNK) {
-        const int n = (int)min((int64_t)CHUNK, s1 - c0);
-        // stage the chunk (coalesced); slots past the end are dead
-#pragma unroll
-        for (int k = 0; k < SPT; ++k) {
-          const int i = tid + k * NTHREADS;
-          const bool in = i < n;
-          const int64_t g = c0 + i;
-          s_A[i] = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
-          s_m2z[i] = in ? p.m2z[g] : 1.0;
-          s_C[i] = make_double2(in ? p.L1[g] : 0.0, in ? p.Q[g] : 0.0);
-          s_P[i] = in ? p.P[g] : 0.0;
-          if (!INJ) {
-            const int32_t r = in ? p.row[g] : 0;
-            s_row[i] = ((unsigned)r < (unsigned)p.n_rows) ? r : 0;  // out-of-range rows are dead (dLc = NaN)
-          }
-        }
-        __syncthreads();
-        // Samples stay in shared memory (read where used: registers go to the interleaved chains instead);
-        // a thread keeps only the address of each of its samples' LOS rows.
-        const RowT* lrow[SPT];
+      // the segment's samples in blocks of BLK, dealt to the warps round-robin; no barrier until the segment ends
+      for (int64_t c0 = s0 + (int64_t)warp * BLK; c0 < s1; c0 += (int64_t)NWARPS * BLK) {
+        Sample<RowT> sm[SPT];
         double dmin = CUDART_INF;  // smallest d_L of the warp's samples: a whole-warp range test per theta
 #pragma unroll
         for (int k = 0; k < SPT; ++k) {
-          const int i = tid + k * NTHREADS;
-          if (INJ) lrow[k] = reinterpret_cast<const RowT*>(s_allsky);
-          else lrow[k] = reinterpret_cast<const RowT*>(p.los) + (size_t)s_row[i] * (size_t)p.n_z;
-          dmin = fmin(dmin, s_A[i].x);  // fmin drops the NaN of dead samples
+          const int64_t g = c0 + k * 32 + lane;
+          const bool in = g < s1;  // slots past the end are dead
+          sm[k].A = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
+          sm[k].m2z = in ? p.m2z[g] : 1.0;
+          sm[k].C = make_double2(in ? p.L1[g] : 0.0, in ? p.Q[g] : 0.0);
+          sm[k].P = in ? p.P[g] : 0.0;
+          if (INJ) {
+            sm[k].lrow = reinterpret_cast<const RowT*>(s_allsky);
+          } else {
+            int32_t r = in ? p.row[g] : 0;
+            r = ((unsigned)r < (unsigned)p.n_rows) ? r : 0;  // out-of-range rows are dead (dLc = NaN)
+            sm[k].lrow = reinterpret_cast<const RowT*>(p.los) + (size_t)r * (size_t)p.n_z;
+          }
+          dmin = fmin(dmin, sm[k].A.x);  // fmin drops the NaN of dead samples
         }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) dmin = fmin(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
+        for (int o = 16; o > 0; o >>= 1) dmin = fmin(dmin, __shfl_xor_sync(FULL, dmin, o));
         // theta points of the tile for which at least one sample of this warp lies inside the table
-        // (none for warps entirely past the ragged tail)
-        unsigned todo = __ballot_sync(0xffffffffu, lane < nt && dmin * s_tc[min(lane, nt - 1) * NCONST + C_H] <
-                                                                    s_tc[min(lane, nt - 1) * NCONST + C_UMAX]);
+        const double* tcl = KT + (t0 + min(lane, nt - 1)) * NCONST;
+        unsigned todo = __ballot_sync(FULL, lane < nt && dmin * tcl[C_H] < tcl[C_UMAX]);
         // Software pipeline over the theta points: the first half of the next point (table look-up, LOS loads)
         // is issued together with the second half of the current one, so its latencies hide behind FP64 work.
         int ja = pop_lowest(todo);
         if (ja >= 0) {
           Mid<RowT> cur[SPT], nxt[SPT];
 #pragma unroll
-          for (int k = 0; k < SPT; ++k) {
-            const int i = tid + k * NTHREADS;
-            term_head<NodeT, RowT, !INJ>(s_tc + ja * NCONST, s_tab + (size_t)ja * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz,
-                                   los_zmax, zq, bmax, cur[k]);
-          }
+          for (int k = 0; k < SPT; ++k)
+            term_head<NodeT, RowT, !INJ>(KT + (t0 + ja) * NCONST, s_tab + (size_t)ja * Mp, sm[k].A, sm[k].m2z, sm[k].lrow,
+                                         inv_dz, los_zmax, zq, bmax, cur[k]);
           for (;;) {
             const int jb = pop_lowest(todo);
             const int jh = jb >= 0 ? jb : ja;  // (a redundant look-up when the list ends on an odd count)
             double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
             int cnt = 0;
             {
-              const double* tch = s_tc + jh * NCONST;
-              const double* tct = s_tc + ja * NCONST;
+              const double* tch = KT + (t0 + jh) * NCONST;
+              const double* tct = KT + (t0 + ja) * NCONST;
+#pragma unroll
+              for (int k = 0; k < SPT; ++k)
+                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
+                                             los_zmax, zq, bmax, nxt[k]);
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                const int i = tid + k * NTHREADS;
-                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz, los_zmax, zq,
-                                       bmax, nxt[k]);
-              }
-#pragma unroll
-              for (int k = 0; k < SPT; ++k) {
-                const int i = tid + k * NTHREADS;
                 bool live;
-                const double w = term_tail<RowT>(tct, mt, s_C[i], s_P[i], cur[k], live);
+                const double w = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, cur[k], zmask, live);
                 a0 += w;
                 a1 = fma(w, w, a1);
                 cnt += live ? 1 : 0;
@@ -322,19 +334,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               // a branch here would let the compiler sink the loads of the first step behind it)
               const bool second = jb >= 0;
               const int jh2 = jc >= 0 ? jc : jh;
-              const double* tch = s_tc + jh2 * NCONST;
-              const double* tct = s_tc + jh * NCONST;
+              const double* tch = KT + (t0 + jh2) * NCONST;
+              const double* tct = KT + (t0 + jh) * NCONST;
 #pragma unroll
-              for (int k = 0; k < SPT; ++k) {
-                const int i = tid + k * NTHREADS;
-                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh2 * Mp, s_A[i], s_m2z[i], lrow[k], inv_dz,
+              for (int k = 0; k < SPT; ++k)
+                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh2 * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, cur[k]);
-              }
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                const int i = tid + k * NTHREADS;
                 bool live;
-                double w = term_tail<RowT>(tct, mt, s_C[i], s_P[i], nxt[k], live);
+                double w = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, nxt[k], zmask, live);
                 live = live & second;
                 w = live ? w : 0.0;
                 b0 += w;
@@ -342,7 +351,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
                 cnt += live ? 0x10000 : 0;
               }
             }
-            cnt = __reduce_add_sync(0xffffffffu, cnt);
+            cnt = __reduce_add_sync(FULL, cnt);
             if (cnt) {  // warp-uniform
               const double k = warp_sum4(a0, a1, b0, b1, lane);
               if ((lane & 7) == 0) {
@@ -357,8 +366,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
             ja = jc;
           }
         }
-        __syncthreads();
       }
+      __syncthreads();
       // segment complete: combine the warps' partials in a fixed order and write them out
       if (tid < nt) {
         double a = 0.0, b = 0.0;
@@ -371,12 +380,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           s_acc[(w * T + tid) * 2 + 1] = 0.0;
           s_cnt[w * T + tid] = 0;
         }
-        const size_t o = (size_t)(t0 + tid) * (size_t)p.n_seg + (size_t)seg;
+        const size_t o = (size_t)(p.t_begin + t0 + tid) * (size_t)p.n_seg + (size_t)seg;
         p.out_w[2 * o] = a;
         p.out_w[2 * o + 1] = b;
         p.out_n[o] = c;
       }
-      // (the barrier after the next chunk's staging orders this reset before the next accumulation)
+      __syncthreads();  // the reset above precedes the next segment's accumulation
     }
   }
 }
@@ -418,18 +427,39 @@ int reweight_configure(int smem_optin) {
   return rc;
 }
 
-int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_blocks,
+// The theta batch goes through in launches of at most KT_THETA points (a whole number of tiles): each launch
+// first copies its points' constants into the constant bank (stream-ordered) and resets the work counter.
+int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm,
                     cudaStream_t s) {
-  const size_t smem = reweight_smem_bytes(p.T, p.Mp, tab_prec, inj, p.n_z);
-  if (inj) {
-    return tab_prec == GWC_F64 ? launch_one<Node64, double, true>(p, n_blocks, smem, s)
+  const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z);
+  const int cap = (KT_THETA / p0.T) * p0.T;
+  int launched = 0;
+  for (int tb = 0; tb < p0.n_theta; tb += cap) {
+    ReweightParams p = p0;
+    p.t_begin = tb;
+    p.n_theta = p0.n_theta - tb < cap ? p0.n_theta - tb : cap;
+    p.n_tiles = (p.n_theta + p.T - 1) / p.T;
+    const int64_t n_items = (int64_t)p.n_groups * p.n_tiles;
+    const int n_blocks = (int)(n_items < n_sm ? n_items : n_sm);
+    if (cudaMemcpyToSymbolAsync(KT, p0.tconst + (size_t)tb * NCONST, sizeof(double) * NCONST * (size_t)p.n_theta, 0,
+                                cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+      return -1;
+    if (cudaMemsetAsync(p.unit_counter, 0, sizeof(unsigned int), s) != cudaSuccess) return -1;
+    int rc;
+    if (inj) {
+      rc = tab_prec == GWC_F64 ? launch_one<Node64, double, true>(p, n_blocks, smem, s)
                                : launch_one<Node32, double, true>(p, n_blocks, smem, s);
-  }
-  if (tab_prec == GWC_F64)
-    return los_prec == GWC_F64 ? launch_one<Node64, double, false>(p, n_blocks, smem, s)
+    } else if (tab_prec == GWC_F64) {
+      rc = los_prec == GWC_F64 ? launch_one<Node64, double, false>(p, n_blocks, smem, s)
                                : launch_one<Node64, float, false>(p, n_blocks, smem, s);
-  return los_prec == GWC_F64 ? launch_one<Node32, double, false>(p, n_blocks, smem, s)
-                             : launch_one<Node32, float, false>(p, n_blocks, smem, s);
+    } else {
+      rc = los_prec == GWC_F64 ? launch_one<Node32, double, false>(p, n_blocks, smem, s)
+                               : launch_one<Node32, float, false>(p, n_blocks, smem, s);
+    }
+    if (rc < 0) return -1;
+    launched += rc;
+  }
+  return launched;
 }
 
 }  // namespace gwc

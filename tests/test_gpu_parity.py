@@ -74,20 +74,21 @@ def _compare(g, o, rtol=RTOL_F64, check_nlive=True):
 
 # ---------------------------------------------------------------------------------------------
 def test_math_functions(ctx):
-    """exp/log/rcp/rsqrt of math64.cuh against torch's fp64 functions."""
+    """exp/log/rcp/rsqrt of math64.cuh against torch's fp64 functions.  exp and log are built to ~2e-13 (cubic /
+    quartic on a 256- / 128-entry table: DESIGN.md section 6), 5000x inside north_star's 1e-9; rcp and rsqrt are
+    correctly rounded to an ulp or two."""
     g = torch.Generator(device="cpu").manual_seed(1)
     x = (torch.rand(1 << 16, generator=g, dtype=torch.float64) * 1400.0 - 700.0).to(DEV)
     for which in (0, 4):
         y = ctx.gwc_math_selftest(which, x)
         rel = ((y - torch.exp(x)) / torch.exp(x)).abs().max().item()
-        assert rel < 4e-15, rel
+        assert rel < 3e-13, rel
     y = ctx.gwc_math_selftest(0, torch.tensor([-1e4, -float("inf"), -700.0], dtype=torch.float64, device=DEV))
     assert torch.all(torch.isfinite(y)) and y.max().item() < 1e-300
     xp = torch.exp((torch.rand(1 << 16, generator=g, dtype=torch.float64) * 40.0 - 20.0)).to(DEV)
     xs = torch.cat([xp, 1.0 + torch.rand(1 << 16, generator=g, dtype=torch.float64).to(DEV) * 3.0])
     y = ctx.gwc_math_selftest(1, xs)
-    assert (y - torch.log(xs)).abs().max().item() < 1e-15 * 24
-    assert ((y - torch.log(xs)).abs() / torch.log(xs).abs().clamp_min(1.0)).max().item() < 1e-15
+    assert (y - torch.log(xs)).abs().max().item() < 3e-13
     y = ctx.gwc_math_selftest(2, xs)
     assert ((y * xs) - 1.0).abs().max().item() < 5e-16
     y = ctx.gwc_math_selftest(3, xs)
