@@ -34,8 +34,8 @@ from paper_2605_23538_b200 import synth  # noqa: E402
 METRIC = "(theta*event*sample) terms/s, whole hot path (events + injections)"
 UNIT = "terms/s"
 # Algorithmic FP64-pipe instructions per term of THIS formulation (counted from SASS)
-FP64_INSTR_LIVE = 125.0
-FP64_INSTR_DEAD = 32.0
+FP64_INSTR_LIVE = 104.0
+FP64_INSTR_DEAD = 28.0
 # B200 FP64 issue peak derived from the unit counts: 148 SMs x 64 FP64 lanes x 1.965 GHz
 FP64_PEAK_INSTR = 148 * 64 * 1.965e9
 
