@@ -51,7 +51,10 @@ constexpr int SPT = GWC_SPT;      // samples per thread per theta (independent c
 #endif
 constexpr int CHUNK = GWC_CHUNK;  // samples staged in shared memory per step (a multiple of 32 * SPT)
 constexpr int KT_THETA = 340;     // theta points whose constants fit the constant bank (one launch)
-constexpr int MAX_T = 16;         // theta points per tile (upper bound)
+#ifndef GWC_MAX_T
+#define GWC_MAX_T 16
+#endif
+constexpr int MAX_T = GWC_MAX_T;  // theta points per tile (upper bound)
 constexpr int INJ_SEG = 8192;     // injections per segment of the selection reduction
 constexpr int QUAD_K = 1024;      // forward quadrature intervals of the cosmology builder
 constexpr int MAX_NODES = 8193;
