@@ -219,8 +219,12 @@ def run_gwc(args):
     achieved = instr * 2.0 / (ms_ev_kernel * 1e-3) / 1e12          # FP64 issue slots x 2 flop
     peak = FP64_PEAK_INSTR * 2.0 / 1e12
     probe_ms, probe_n = ctx.gwc_probe_fp64(1 << 13)
+    # DRAM bytes of the event kernel from the ncu --set full capture (profiles/r01c): 7.26e9 per 340-theta launch
+    # of the O5 catalogue; kernel_ms covers the ceil(n_theta / 340) launches of one step, so the traffic does too
+    traffic = 7.26e9 * n_theta / 340.0 if spec.name == "o5" else None
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "reweight_kernel<events>", "kernel_ms": ms_ev_kernel,
+                "traffic": traffic, "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01c "
+                "(bytes per step's event-kernel launches; HBM does not bind)" if traffic else None, "kernel": "reweight_kernel<events>", "kernel_ms": ms_ev_kernel,
                 "kernel_share_of_step": ms_ev_kernel / (ms / args.steps),
                 "inj_kernel_ms": ms_inj_kernel,
                 "fp64_instr_per_live_term": FP64_INSTR_LIVE, "fp64_instr_per_dead_term": FP64_INSTR_DEAD,

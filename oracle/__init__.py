@@ -64,6 +64,7 @@ def lib():
             "orc_los_lerp": (d, [vp, i64, d]), "orc_los_allsky": (None, [vp, vp]),
             "orc_lse": (None, [vp, i64, vp, vp]),
             "orc_event_loglik": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, vp, vp, vp]),
+            "orc_event_loglik_pixcut": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, d, vp, vp, vp, vp]),
             "orc_selection_logxi": (C.c_int, [vp, i64, vp, vp, i32, d, C.c_int, d, C.c_int, C.c_int, vp, vp]),
             "orc_total_from_parts": (None, [vp, vp, i64, i64, vp]),
             "orc_pack_events": (i64, [i64, i64, vp, vp, vp, vp, vp, vp, vp]),
@@ -168,6 +169,30 @@ def event_loglik(theta, ev, los_table, los_z_max, *, mode=TABLE, z_max=None, n_n
                                 _p(logL), _p(neff), _p(nlive))
     assert rc == 0
     return logL, neff, nlive
+
+
+def event_loglik_pixcut(theta, ev, los_table, los_z_max, neff_min, *, mode=TABLE, z_max=None, n_nodes=1025,
+                        table_prec=0):
+    """Event term with the per-pixel N_eff cut of Eq. 8 (R25).  Same inputs as
+    event_loglik plus the threshold; returns logL, neff (f64), nlive, npass (int64), all [n_theta, n_events]."""
+    th = _theta(theta)
+    off = np.ascontiguousarray(ev["ev_sample_off"], dtype=np.int64)
+    dl, m1, m2 = _f64(ev["dL"]), _f64(ev["m1z"]), _f64(ev["m2z"])
+    row = np.ascontiguousarray(ev["sample_row"], dtype=np.int32)
+    lpe = ev.get("log_pe_prior")
+    lpe = None if lpe is None else _f64(lpe)
+    ne = off.size - 1
+    es = _Events(ne, dl.size, off.ctypes.data, dl.ctypes.data, m1.ctypes.data, m2.ctypes.data,
+                 None if lpe is None else lpe.ctypes.data, row.ctypes.data)
+    ls, keep = _los_struct(los_table, los_z_max)
+    nt = th.shape[0]
+    logL, neff = np.empty((nt, ne)), np.empty((nt, ne))
+    nlive, npass = np.empty((nt, ne), dtype=np.int64), np.empty((nt, ne), dtype=np.int64)
+    zm = float(los_z_max if z_max is None else z_max)
+    rc = lib().orc_event_loglik_pixcut(_p(th), nt, C.addressof(es), C.addressof(ls), mode, zm, n_nodes, table_prec,
+                                       float(neff_min), _p(logL), _p(neff), _p(nlive), _p(npass))
+    assert rc == 0
+    return logL, neff, nlive, npass
 
 
 def selection_logxi(theta, inj, allsky, los_z_max, *, mode=TABLE, z_max=None, n_nodes=1025, table_prec=0):

@@ -468,6 +468,90 @@ int orc_event_loglik(const double* theta, int64_t n_theta, const orc_events* ev,
 }
 
 /*
+ * NEXT row 2: the per-pixel effective-sample cut of Eq. 8 (fiducial threshold 2,
+ * PAPER.md:194).  A pixel of event i is a maximal run of consecutive samples with the same sample_row (the A0
+ * packing makes every (event, row) one run).  With the weights of Eq. 7 taken relative to the run's largest,
+ *   W_j = sum_k w_k,  Q_j = sum_k w_k^2,  N_eff,j = W_j^2 / Q_j,
+ * pixel j contributes iff it has a live sample and W_j^2 >= neff_min * Q_j (decided in this linear form, so that
+ * a pixel of n equal weights has N_eff = n exactly); "If a pixel does not pass this threshold ... it does not
+ * contribute to the total likelihood".  Then  log L_i = LSE over the samples of the passing pixels - ln S_i
+ * (S_i still counts every sample of the event: DESIGN.md R25), N_eff,i and nlive_i over the same samples, and
+ * npass_i = number of passing pixels.
+ */
+int orc_event_loglik_pixcut(const double* theta, int64_t n_theta, const orc_events* ev, const orc_los* L, int mode,
+                            double z_max, int M, int table_prec, double neff_min, double* logL, double* neff,
+                            int64_t* nlive, int64_t* npass) {
+  int err = 0;
+  int64_t smax = 0;
+  for (int64_t i = 0; i < ev->n_events; ++i) {
+    int64_t s = ev->ev_sample_off[i + 1] - ev->ev_sample_off[i];
+    if (s > smax) smax = s;
+  }
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t t = 0; t < n_theta; ++t) {
+    const double* th = theta + t * ORC_NPAR;
+    double* lw = (double*)malloc(sizeof(double) * (size_t)(smax > 0 ? smax : 1));
+    double* keep = (double*)malloc(sizeof(double) * (size_t)(smax > 0 ? smax : 1));
+    int* lv = (int*)malloc(sizeof(int) * (size_t)(smax > 0 ? smax : 1));
+    if (!orc_theta_valid(th) || !lw || !keep || !lv) {
+      for (int64_t i = 0; i < ev->n_events; ++i) {
+        logL[t * ev->n_events + i] = NAN;
+        if (neff) neff[t * ev->n_events + i] = NAN;
+        if (nlive) nlive[t * ev->n_events + i] = 0;
+        if (npass) npass[t * ev->n_events + i] = 0;
+      }
+      if (!lw || !keep || !lv) err = 1;
+      free(lw); free(keep); free(lv);
+      continue;
+    }
+    orc_cosmo_tab ct;
+    double* buf = NULL;
+    if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lw); free(keep); free(lv); continue; }
+    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
+    for (int64_t i = 0; i < ev->n_events; ++i) {
+      int64_t a = ev->ev_sample_off[i], b = ev->ev_sample_off[i + 1];
+      for (int64_t k = a; k < b; ++k) {
+        double lpi = ev->log_pe_prior ? ev->log_pe_prior[k] : 2.0 * log(ev->dL[k]);
+        lw[k - a] = orc_log_weight(th, mode, &ct, ev->dL[k], ev->m1z[k], ev->m2z[k], lpi, L,
+                                   (int64_t)ev->sample_row[k], &lv[k - a]);
+      }
+      int64_t nkeep = 0, cnt = 0, np = 0;
+      int64_t r0 = a;
+      while (r0 < b) {                       /* one pixel: samples r0 .. r1-1 */
+        int64_t r1 = r0 + 1;
+        while (r1 < b && ev->sample_row[r1] == ev->sample_row[r0]) ++r1;
+        double m = -INFINITY;
+        for (int64_t k = r0; k < r1; ++k) if (lw[k - a] > m) m = lw[k - a];
+        if (m > -INFINITY) {
+          long double W = 0.0L, Q = 0.0L;
+          for (int64_t k = r0; k < r1; ++k) {
+            if (lw[k - a] == -INFINITY) continue;
+            double e = exp(lw[k - a] - m);
+            W += e;
+            Q += (long double)e * e;
+          }
+          double Wd = (double)W, Qd = (double)Q;
+          if (Wd * Wd >= neff_min * Qd) {
+            ++np;
+            for (int64_t k = r0; k < r1; ++k) { keep[nkeep++] = lw[k - a]; cnt += lv[k - a]; }
+          }
+        }
+        r0 = r1;
+      }
+      double l1, l2;
+      lse2(keep, nkeep, &l1, &l2);
+      logL[t * ev->n_events + i] = (b > a) ? l1 - log((double)(b - a)) : -INFINITY;
+      if (neff) neff[t * ev->n_events + i] = (l1 == -INFINITY) ? 0.0 : exp(2.0 * l1 - l2);
+      if (nlive) nlive[t * ev->n_events + i] = cnt;
+      if (npass) npass[t * ev->n_events + i] = np;
+    }
+    free(buf);
+    free(lw); free(keep); free(lv);
+  }
+  return err;
+}
+
+/*
  * log xi(theta) = LSE_j log w_j - ln n_draw over found injections, with the all-sky
  * prior (a 1-row f64 table) in place of the pixel row and log_pdraw in place of the PE prior.
  */

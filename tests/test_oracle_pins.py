@@ -400,3 +400,115 @@ def test_pack_events_against_lexsort():
     starts = np.flatnonzero(np.concatenate([[True], (se[1:] != se[:-1]) | (sr[1:] != sr[:-1])]))
     assert np.array_equal(out["pix_sample_off"], np.concatenate([starts, [n]]))
     assert out["ev_sample_off"][7] == out["ev_sample_off"][8]
+
+
+# ---- NEXT row 2: the per-pixel N_eff cut of Eq. 8 (PAPER.md:93-95) ----------------------------------------------
+def _runs(row, a, b):
+    """[start, end) of the maximal runs of equal row inside samples a..b."""
+    out, r0 = [], a
+    while r0 < b:
+        r1 = r0 + 1
+        while r1 < b and row[r1] == row[r0]:
+            r1 += 1
+        out.append((r0, r1))
+        r0 = r1
+    return out
+
+
+def test_pixcut_threshold_zero_is_the_uncut_estimator(theta0):
+    # every pixel with a live sample passes N_eff >= 0, so the cut path must reproduce the pinned uncut one
+    ev, tab, zmax = _toy_event()
+    th = np.stack([theta0, theta0 * np.array([1.4] + [1.0] * 11)])
+    L0, n0, k0 = O.event_loglik(th, ev, tab, zmax)
+    L1, n1, k1, p1 = O.event_loglik_pixcut(th, ev, tab, zmax, 0.0)
+    np.testing.assert_allclose(L1, L0, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(n1, n0, rtol=1e-12)
+    assert np.array_equal(k1, k0)
+    # and an unreachable threshold leaves nothing
+    L2, n2, k2, p2 = O.event_loglik_pixcut(th, ev, tab, zmax, 1e9)
+    assert np.all(np.isneginf(L2)) and np.all(n2 == 0) and np.all(k2 == 0) and np.all(p2 == 0)
+
+
+def test_pixcut_equals_recombination_of_single_pixel_events(theta0):
+    # Eq. 8 by another route: make every pixel its own event, take its N_eff and log L from the (pinned) uncut
+    # path, keep the pixels with N_eff >= threshold and recombine:  L_i = (1/S_i) sum_pass S_j L_j.
+    ev, tab, zmax = _toy_event(n=400, seed=5, rows=9)
+    th = np.stack([theta0, theta0 * np.array([0.8] + [1.0] * 11), theta0 * np.array([1.5] + [1.0] * 11)])
+    off = ev["ev_sample_off"]
+    row = ev["sample_row"]
+    for thr in (1.5, 2.0, 4.0, 12.5):
+        L, N, K, P = O.event_loglik_pixcut(th, ev, tab, zmax, thr)
+        for i in range(off.size - 1):
+            runs = _runs(row, off[i], off[i + 1])
+            sub_off = np.array([0] + [r1 - off[i] for _, r1 in runs], dtype=np.int64)
+            sl = slice(off[i], off[i + 1])
+            sub = dict(ev_sample_off=sub_off, dL=ev["dL"][sl], m1z=ev["m1z"][sl], m2z=ev["m2z"][sl],
+                       sample_row=row[sl], log_pe_prior=None)
+            Lj, Nj, Kj = O.event_loglik(th, sub, tab, zmax)
+            Sj = np.diff(sub_off).astype(float)
+            for t in range(th.shape[0]):
+                ok = np.isfinite(Lj[t]) & (Nj[t] >= thr * (1 + 1e-12))
+                edge = np.isfinite(Lj[t]) & (np.abs(Nj[t] - thr) <= thr * 1e-12)
+                assert not edge.any()                      # no pixel sits on the threshold in this toy
+                assert P[t, i] == ok.sum() and K[t, i] == Kj[t][ok].sum()
+                if ok.any():
+                    want = np.log(np.sum(Sj[ok] * np.exp(Lj[t][ok] - Lj[t][ok].max()))) + Lj[t][ok].max() \
+                        - np.log(off[i + 1] - off[i])
+                    assert L[t, i] == pytest.approx(want, abs=1e-12)
+                else:
+                    assert np.isneginf(L[t, i])
+    # the cut can only remove weight
+    Lc = O.event_loglik_pixcut(th, ev, tab, zmax, 2.0)[0]
+    Lu = O.event_loglik(th, ev, tab, zmax)[0]
+    assert np.all(Lc <= Lu + 1e-13)
+
+
+def test_pixcut_equal_weights_count_the_samples(theta0):
+    # a pixel of n identical samples has N_eff = n exactly (the decision is taken as W^2 >= n_min Q):
+    # pixels of 1, 2, 3 and 5 copies of one sample -> thresholds 2, 3, 3.5 keep {2,3,5}, {3,5}, {5}
+    ev, tab, zmax = _toy_event(n=30, seed=2, rows=4)
+    reps = [1, 2, 3, 5]
+    n = sum(reps)
+    one = lambda key: np.full(n, ev[key][0])
+    e1 = dict(ev_sample_off=np.array([0, n], dtype=np.int64), dL=one("dL"), m1z=one("m1z"), m2z=one("m2z"),
+              sample_row=np.repeat(np.arange(4, dtype=np.int32), reps), log_pe_prior=None)
+    tab1 = np.tile(tab[:1], (4, 1))                         # the same LOS row everywhere: identical weights
+    L0, _, k0 = O.event_loglik(theta0, e1, tab1, zmax)
+    assert k0[0, 0] == n
+    lw = L0[0, 0]                                          # = log w of the one sample (mean of n equal weights)
+    for thr, kept in ((2.0, [2, 3, 5]), (3.0, [3, 5]), (3.5, [5]), (1.0, reps), (5.0, [5]), (5.0001, [])):
+        L, N, K, P = O.event_loglik_pixcut(theta0, e1, tab1, zmax, thr)
+        assert P[0, 0] == len(kept) and K[0, 0] == sum(kept)
+        if kept:
+            assert L[0, 0] == pytest.approx(lw + math.log(sum(kept) / n), abs=1e-13)
+            assert N[0, 0] == pytest.approx(sum(kept), rel=1e-12)
+        else:
+            assert np.isneginf(L[0, 0]) and N[0, 0] == 0
+
+
+def test_pixcut_invariant_under_pixel_order_and_dead_padding(theta0):
+    ev, tab, zmax = _toy_event(n=240, seed=8, rows=6)
+    off = ev["ev_sample_off"]
+    base = O.event_loglik_pixcut(theta0, ev, tab, zmax, 2.0)
+    # reverse the order of the pixels inside each event (samples inside a pixel keep their order)
+    idx = []
+    for i in range(off.size - 1):
+        for r0, r1 in reversed(_runs(ev["sample_row"], off[i], off[i + 1])):
+            idx.extend(range(r0, r1))
+    idx = np.array(idx)
+    ev2 = dict(ev, dL=ev["dL"][idx], m1z=ev["m1z"][idx], m2z=ev["m2z"][idx], sample_row=ev["sample_row"][idx])
+    got = O.event_loglik_pixcut(theta0, ev2, tab, zmax, 2.0)
+    np.testing.assert_allclose(got[0], base[0], rtol=0, atol=1e-12)
+    assert np.array_equal(got[2], base[2]) and np.array_equal(got[3], base[3])
+    # dead samples appended to the last pixel of the last event change S_i only
+    pad = 11
+    n = ev["dL"].size
+    ev3 = dict(ev_sample_off=np.array([off[0], off[1], n + pad], dtype=np.int64),
+               dL=np.concatenate([ev["dL"], np.full(pad, 1e7)]), m1z=np.concatenate([ev["m1z"], np.full(pad, 40.0)]),
+               m2z=np.concatenate([ev["m2z"], np.full(pad, 30.0)]),
+               sample_row=np.concatenate([ev["sample_row"], np.full(pad, ev["sample_row"][-1], np.int32)]),
+               log_pe_prior=None)
+    got3 = O.event_loglik_pixcut(theta0, ev3, tab, zmax, 2.0)
+    S1 = n - off[1]
+    assert got3[0][0, 1] == pytest.approx(base[0][0, 1] - math.log((S1 + pad) / S1), abs=1e-12)
+    assert np.array_equal(got3[3], base[3]) and np.array_equal(got3[2], base[2])
