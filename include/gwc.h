@@ -135,6 +135,22 @@ gwc_status gwc_event_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
                             const gwc_los* los, double* d_logL, double* d_neff, int64_t* d_nlive);
 
 /*
+ * A3 + A4 with the per-pixel effective-sample cut of Eq. 8 (fiducial threshold 2,
+ * PAPER.md:194; R25).  A pixel of an event is a maximal run of consecutive samples with the same
+ * sample_row (gwc_pack_events orders the samples so that every (event, row) is one run).  With W_j = sum_k w_k
+ * and Q_j = sum_k w_k^2 over the samples of pixel j, the pixel contributes iff it has a live sample and
+ * W_j^2 >= neff_min * Q_j (N_eff,j >= neff_min, decided in FP64 in this form); then
+ *   log L_i = log( (1/S_i) sum over passing pixels of W_j ),   S_i = all samples of the event,
+ * N_eff,i and the live count over the samples of the passing pixels, and the number of passing pixels.
+ * neff_min = 0 gives gwc_event_loglik's results.  Same preconditions and errors as gwc_event_loglik;
+ * neff_min < 0 or NaN -> GWC_ERR_INVALID_ARG.
+ *   d_logL [n_theta][n_events] f64;  d_neff f64, d_nlive i64, d_npass i64: same shape or NULL.
+ */
+gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                                   const gwc_los* los, double neff_min, double* d_logL, double* d_neff,
+                                   int64_t* d_nlive, int64_t* d_npass);
+
+/*
  * A5.  log xi(theta) = log( (1/n_draw) sum_j w_j ) over found injections with the all-sky prior
  * los->allsky and log_pdraw in place of the PE prior; optional N_eff of the injection sum.
  *   d_logxi [n_theta];  d_neff_inj [n_theta] or NULL.

@@ -39,7 +39,7 @@ struct gwc_ctx {
   gwc_prec tab_prec = GWC_F64;
   double z_max = 0.0;
   // per-call scratch
-  Buf dLc, L1, Q, P, seg_off, seg_shift, group_off, part_w, part_n, allsky_scr, pack_scr, logL, logxi, probe;
+  Buf dLc, L1, Q, P, seg_off, seg_shift, group_off, part_w, part_n, part_np, allsky_scr, pack_scr, logL, logxi, probe;
   HostCopy hc;
   // timing
   bool timing = false;
@@ -133,7 +133,7 @@ gwc_status check_built(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, dou
 gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg, const int64_t* d_seg_off,
                         const double* dL, const double* m1z, const double* m2z, const double* lprior,
                         const int32_t* row, const void* los_table, gwc_prec los_prec, int64_t n_rows, int n_z,
-                        double los_zmax, bool inj) {
+                        double los_zmax, bool inj, bool pixcut = false, double neff_min = 0.0) {
   cudaStream_t s = ctx->stream;
   const size_t nd = (size_t)(n > 0 ? n : 1) * sizeof(double);
   GWC_TRY(ensure(ctx, ctx->dLc, nd));
@@ -143,6 +143,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   GWC_TRY(ensure(ctx, ctx->seg_shift, (size_t)n_seg * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->part_w, (size_t)n_theta * n_seg * 2 * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->part_n, (size_t)n_theta * n_seg * sizeof(int32_t)));
+  if (pixcut) GWC_TRY(ensure(ctx, ctx->part_np, (size_t)n_theta * n_seg * sizeof(int32_t)));
   GWC_TRY(count(ctx, launch_prep_samples(n, n_seg, d_seg_off, dL, m1z, m2z, lprior, row, n_rows, (double*)ctx->dLc.p,
                                          (double*)ctx->L1.p, (double*)ctx->Q.p, (double*)ctx->P.p,
                                          (double*)ctx->seg_shift.p, s),
@@ -191,6 +192,9 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.zero_mask = 0;
   p.out_w = (double*)ctx->part_w.p;
   p.out_n = (int32_t*)ctx->part_n.p;
+  p.out_np = pixcut ? (int32_t*)ctx->part_np.p : nullptr;
+  p.pixcut = pixcut ? 1 : 0;
+  p.neff_min = neff_min;
   p.unit_counter = ctx->d_counter;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (ctx->timing) {
@@ -259,7 +263,7 @@ void gwc_destroy(gwc_ctx* ctx) {
   cudaSetDevice(ctx->device);
   cudaStreamSynchronize(ctx->stream);
   Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->dLc, &ctx->L1, &ctx->Q, &ctx->P, &ctx->seg_off, &ctx->seg_shift,
-                 &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
+                 &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
                  &ctx->logxi, &ctx->probe, &ctx->hc.theta, &ctx->hc.ev_off, &ctx->hc.ev_dL, &ctx->hc.ev_m1z,
                  &ctx->hc.ev_m2z, &ctx->hc.ev_lp, &ctx->hc.ev_row, &ctx->hc.inj_dL, &ctx->hc.inj_m1z,
                  &ctx->hc.inj_m2z, &ctx->hc.inj_lp, &ctx->hc.los, &ctx->hc.allsky, &ctx->hc.out};
@@ -371,6 +375,35 @@ gwc_status gwc_event_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
                                            (const double*)ctx->tconst.p, n_theta, ev->n_events, d_logL, d_neff,
                                            d_nlive, ctx->stream),
                "finalize_events");
+}
+
+gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                                   const gwc_los* los, double neff_min, double* d_logL, double* d_neff,
+                                   int64_t* d_nlive, int64_t* d_npass) {
+  GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
+  if (!ev || !d_logL) return fail(ctx, GWC_ERR_INVALID_ARG, "ev or d_logL is NULL");
+  if (!(neff_min >= 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "neff_min must be >= 0");
+  GWC_TRY(check_los(ctx, los, true, false));
+  if (ev->n_events < 0 || ev->n_samples < 0 || ev->n_events > 0x7fffffffLL)
+    return fail(ctx, GWC_ERR_SHAPE, "event / sample counts out of range");
+  if (ev->n_events == 0) return GWC_OK;
+  if (!ev->ev_sample_off) return fail(ctx, GWC_ERR_INVALID_ARG, "ev->ev_sample_off is NULL");
+  if (ev->n_samples > 0 && (!ev->dL || !ev->m1z || !ev->m2z || !ev->sample_row))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "a sample array is NULL");
+  GWC_TRY(check_built(ctx, d_theta, n_theta, los->z_max));
+  GWC_TRY(run_reweight(ctx, n_theta, ev->n_samples, ev->n_events, ev->ev_sample_off, ev->dL, ev->m1z, ev->m2z,
+                       ev->log_pe_prior, ev->sample_row, los->table, los->prec, los->n_rows, los->n_z, los->z_max,
+                       false, true, neff_min));
+  GWC_TRY(count(ctx, launch_finalize_events((const double*)ctx->part_w.p, (const int32_t*)ctx->part_n.p,
+                                            ev->ev_sample_off, (const double*)ctx->seg_shift.p,
+                                            (const double*)ctx->tconst.p, n_theta, ev->n_events, d_logL, d_neff,
+                                            d_nlive, ctx->stream),
+                "finalize_events"));
+  if (d_npass)
+    GWC_TRY(count(ctx, launch_widen_i32((const int32_t*)ctx->part_np.p, (const double*)ctx->tconst.p, n_theta,
+                                        ev->n_events, d_npass, ctx->stream),
+                  "widen_npass"));
+  return GWC_OK;
 }
 
 gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_injections* inj,

@@ -84,6 +84,9 @@ struct ReweightParams {
   double tab_zq;            // Node32 tables: z_max of the cosmology table / (2^32 - 1)
   double* out_w;            // [n_theta][n_seg][2]: sum w', sum w'^2
   int32_t* out_n;           // [n_theta][n_seg]   : n_live
+  int32_t* out_np;          // [n_theta][n_seg]   : passing pixels (pixel-cut mode)
+  int pixcut;               // 1: per-pixel effective-sample cut (Eq. 8), threshold neff_min
+  double neff_min;
   unsigned int* unit_counter;
   int zero_mask;            // always 0 (scheduling pin of the LOS loads, reweight.cu)
 };
@@ -110,6 +113,8 @@ int launch_finalize_events(const double* part_w, const int32_t* part_n, const in
                            int64_t* nlive, cudaStream_t s);
 int launch_finalize_inj(const double* part_w, const double* seg_shift, const double* tconst, int64_t n_theta,
                         int64_t n_seg, double n_draw, double* logxi, double* neff, cudaStream_t s);
+int launch_widen_i32(const int32_t* in, const double* tconst, int64_t n_theta, int64_t n, int64_t* out,
+                     cudaStream_t s);
 int launch_combine_total(const double* logL, const double* logxi, int64_t n_theta, int64_t n_events, double* total,
                          cudaStream_t s);
 int launch_allsky(const void* table, gwc_prec prec, int64_t n_rows, int n_z, double* scratch, double* allsky,

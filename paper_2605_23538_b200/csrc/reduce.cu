@@ -227,6 +227,15 @@ __global__ void math_selftest_kernel(int which, int64_t n, const double* __restr
   out[i] = y;
 }
 
+// int32 counts [n_theta][n] -> int64 (0 for a theta outside the domain)
+__global__ void widen_i32_kernel(const int32_t* __restrict__ in, const double* __restrict__ tconst, int64_t n_theta,
+                                 int64_t n, int64_t* __restrict__ out) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n_theta * n) return;
+  const int64_t t = i / n;
+  out[i] = tconst[t * NCONST + C_VALID] == 1.0 ? (int64_t)in[i] : 0;
+}
+
 inline int ok() { return cudaGetLastError() == cudaSuccess ? 1 : -1; }
 
 }  // namespace
@@ -267,6 +276,14 @@ int launch_finalize_inj(const double* part_w, const double* seg_shift, const dou
   if (n_theta <= 0) return 0;
   finalize_inj_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(part_w, seg_shift, tconst, n_theta, n_seg,
                                                                         n_draw, logxi, neff);
+  return ok();
+}
+
+int launch_widen_i32(const int32_t* in, const double* tconst, int64_t n_theta, int64_t n, int64_t* out,
+                     cudaStream_t s) {
+  const int64_t m = n_theta * n;
+  if (m <= 0) return 0;
+  widen_i32_kernel<<<(unsigned)((m + 255) / 256), 256, 0, s>>>(in, tconst, n_theta, n, out);
   return ok();
 }
 

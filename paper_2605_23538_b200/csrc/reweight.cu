@@ -43,7 +43,7 @@ constexpr int BLK = 32 * SPT;      // samples one warp holds in registers at a t
 __constant__ double KT[KT_THETA * NCONST];
 
 struct SmemLayout {
-  size_t math, acc, cnt, allsky, tab, total;
+  size_t math, acc, cnt, np, carry, carryn, allsky, tab, total;
 };
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
@@ -54,6 +54,9 @@ __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_byt
   L.math = o;   o = align16(o + sizeof(MathTables));
   L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2);
   L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T);
+  L.np = o;     o = align16(o + sizeof(int) * NWARPS * T);            // pixel-cut mode: passing pixels
+  L.carry = o;  o = align16(o + sizeof(double) * NWARPS * T * 2);     // pixel-cut mode: run left open by a block
+  L.carryn = o; o = align16(o + sizeof(int) * NWARPS * T);
   L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
   L.tab = o;    o = align16(o + node_bytes * (size_t)T * Mp);
   L.total = o;
@@ -208,6 +211,94 @@ __device__ __forceinline__ int pop_lowest(unsigned& mask) {
   return j;
 }
 
+// ---- per-pixel effective-sample cut (Eq. 8; R25) -------------------------------------
+// A pixel is a maximal run of consecutive samples of the segment with the same sample_row.  The warp's block
+// holds positions pos = k * 32 + lane; PixShape is the run structure of the block (the same for every theta).
+struct PixShape {
+  int d[SPT];        // lanes back to the head of this position's run inside row k (>= 64: the run began earlier)
+  bool tail[SPT];    // last sample of its run
+  int maxd[SPT];     // largest reach of the row (d, or the lane index where the run began earlier): scan steps needed
+  bool last_open;    // the block's last position is inside a run that continues in the next block
+};
+
+// Segmented inclusive scan of (W, Q, n) over the 32 lanes of one row; lanes add from `o` lanes back while that
+// lane is still inside their run.
+__device__ __forceinline__ void seg_scan(double& W, double& Q, int& n, int d, int maxd) {
+  const unsigned FULL = 0xffffffffu;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    if (o > maxd) break;  // warp-uniform
+    const double tW = __shfl_up_sync(FULL, W, o), tQ = __shfl_up_sync(FULL, Q, o);
+    const int tn = __shfl_up_sync(FULL, n, o);
+    const bool take = d >= 64 ? (int)(threadIdx.x & 31) >= o : d >= o;
+    W += take ? tW : 0.0;
+    Q += take ? tQ : 0.0;
+    n += take ? tn : 0;
+  }
+}
+
+// From the per-sample weights of one theta to what the passing pixels add to this lane's sums.
+//   in : w[k], live[k]; carry = (W, Q, n) of the run left open by the previous block (slot of this warp and theta)
+//   out: cW, cQ, cn (weights, squared weights, live samples of the passing pixels that end on this lane), cp = how many
+__device__ __forceinline__ void pix_reduce(const PixShape& ps, const double* w, const bool* live, double neff_min,
+                                           double* carryWQ, int* carryN, int lane, double& cW, double& cQ, int& cn,
+                                           int& cp) {
+  const unsigned FULL = 0xffffffffu;
+  double W[SPT], Q[SPT];
+  int n[SPT];
+#pragma unroll
+  for (int k = 0; k < SPT; ++k) {
+    W[k] = w[k];
+    Q[k] = w[k] * w[k];
+    n[k] = live[k] ? 1 : 0;
+    seg_scan(W[k], Q[k], n[k], ps.d[k], ps.maxd[k]);
+  }
+  // runs that began before the row: add what the previous row (or the previous block) accumulated for them
+  double inW = carryWQ[0], inQ = carryWQ[1];
+  int inN = *carryN;
+#pragma unroll
+  for (int k = 0; k < SPT; ++k) {
+    const bool open_left = ps.d[k] >= 64;
+    W[k] += open_left ? inW : 0.0;
+    Q[k] += open_left ? inQ : 0.0;
+    n[k] += open_left ? inN : 0;
+    inW = __shfl_sync(FULL, W[k], 31);
+    inQ = __shfl_sync(FULL, Q[k], 31);
+    inN = __shfl_sync(FULL, n[k], 31);
+  }
+  __syncwarp();
+  if (lane == 0) {  // what the next block inherits
+    carryWQ[0] = ps.last_open ? inW : 0.0;
+    carryWQ[1] = ps.last_open ? inQ : 0.0;
+    *carryN = ps.last_open ? inN : 0;
+  }
+  __syncwarp();
+  cW = 0.0;
+  cQ = 0.0;
+  cn = 0;
+  cp = 0;
+#pragma unroll
+  for (int k = 0; k < SPT; ++k) {
+    const bool pass = ps.tail[k] && W[k] > 0.0 && W[k] * W[k] >= neff_min * Q[k];
+    cW += pass ? W[k] : 0.0;
+    cQ += pass ? Q[k] : 0.0;
+    cn += pass ? n[k] : 0;
+    cp += pass ? 1 : 0;
+  }
+}
+
+// First sample at or after x that starts a pixel (s1 when there is none); s0 starts one by definition.
+__device__ __forceinline__ int64_t first_head(const int32_t* __restrict__ row, int64_t s0, int64_t s1, int64_t x,
+                                              int lane) {
+  if (x <= s0) return s0;
+  for (; x < s1; x += 32) {
+    const int64_t g = x + lane;
+    const unsigned m = __ballot_sync(0xffffffffu, g < s1 && row[g] != row[g - 1]);
+    if (m) return x + (__ffs(m) - 1);
+  }
+  return s1;
+}
+
 // One sample's theta-independent values, held in registers while the warp loops over the tile's theta points.
 template <typename RowT>
 struct Sample {
@@ -218,7 +309,7 @@ struct Sample {
   const RowT* lrow;
 };
 
-template <typename NodeT, typename LosT, bool INJ>
+template <typename NodeT, typename LosT, bool INJ, bool PIX>
 __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
@@ -227,6 +318,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   MathTables& mt = *reinterpret_cast<MathTables*>(smem + L.math);
   double* s_acc = reinterpret_cast<double*>(smem + L.acc);
   int* s_cnt = reinterpret_cast<int*>(smem + L.cnt);
+  int* s_np = reinterpret_cast<int*>(smem + L.np);
+  double* s_carry = reinterpret_cast<double*>(smem + L.carry);
+  int* s_carryn = reinterpret_cast<int*>(smem + L.carryn);
   double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
   NodeT* s_tab = reinterpret_cast<NodeT*>(smem + L.tab);
 
@@ -267,19 +361,47 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     }
     for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) s_acc[i] = 0.0;
     for (int i = tid; i < NWARPS * T; i += NTHREADS) s_cnt[i] = 0;
+    if (PIX) {
+      for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) s_carry[i] = 0.0;
+      for (int i = tid; i < NWARPS * T; i += NTHREADS) {
+        s_np[i] = 0;
+        s_carryn[i] = 0;
+      }
+    }
     __syncthreads();
 
     const int seg_lo = p.group_off[group], seg_hi = p.group_off[group + 1];
     for (int seg = seg_lo; seg < seg_hi; ++seg) {
       const int64_t s0 = p.seg_off[seg], s1 = p.seg_off[seg + 1];
-      // the segment's samples in blocks of BLK, dealt to the warps round-robin; no barrier until the segment ends
-      for (int64_t c0 = s0 + (int64_t)warp * BLK; c0 < s1; c0 += (int64_t)NWARPS * BLK) {
+      // The segment's samples in blocks of BLK, dealt to the warps round-robin; no barrier until the segment ends.
+      // Pixel-cut mode: each warp takes one contiguous range instead, cut where a pixel starts, so that every
+      // pixel lies inside one warp and the run a block leaves open is continued by the same warp's next block.
+      int64_t w_lo = s0 + (int64_t)warp * BLK, w_hi = s1, w_step = (int64_t)NWARPS * BLK;
+      if (PIX) {
+        const int64_t len = s1 - s0;
+        w_lo = first_head(p.row, s0, s1, s0 + len * warp / NWARPS, lane);
+        w_hi = warp + 1 == NWARPS ? s1 : first_head(p.row, s0, s1, s0 + len * (warp + 1) / NWARPS, lane);
+        w_step = BLK;
+      }
+      for (int64_t c0 = w_lo; c0 < w_hi; c0 += w_step) {
         Sample<RowT> sm[SPT];
+        PixShape ps;
         double dmin = CUDART_INF;  // smallest d_L of the warp's samples: a whole-warp range test per theta
 #pragma unroll
         for (int k = 0; k < SPT; ++k) {
           const int64_t g = c0 + k * 32 + lane;
-          const bool in = g < s1;  // slots past the end are dead
+          const bool in = g < w_hi;  // slots past the end are dead
+          if (PIX) {
+            // run structure of the row: heads, distance to the head, tails
+            const int32_t r = in ? p.row[g] : 0;
+            const bool head = in && (g == w_lo || p.row[g - 1] != r);
+            const bool tail = in && (g + 1 >= w_hi || p.row[g + 1] != r);
+            const unsigned hm = __ballot_sync(FULL, head) & (0xffffffffu >> (31 - lane));
+            ps.d[k] = hm ? lane - (31 - __clz(hm)) : 64;
+            ps.tail[k] = tail;
+            ps.maxd[k] = __reduce_max_sync(FULL, in ? (hm ? ps.d[k] : lane) : 0);
+            if (k == SPT - 1) ps.last_open = __shfl_sync(FULL, (int)(in && !tail), 31) != 0;
+          }
           sm[k].A = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
           sm[k].m2z = in ? p.m2z[g] : 1.0;
           sm[k].C = make_double2(in ? p.L1[g] : 0.0, in ? p.Q[g] : 0.0);
@@ -298,6 +420,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         // theta points of the tile for which at least one sample of this warp lies inside the table
         const double* tcl = KT + (t0 + min(lane, nt - 1)) * NCONST;
         unsigned todo = __ballot_sync(FULL, lane < nt && dmin * tcl[C_H] < tcl[C_UMAX]);
+        if (PIX) todo = 0xffffffffu >> (32 - nt);  // every theta sees every block: open runs are carried through
         // Software pipeline over the theta points: the first half of the next point (table look-up, LOS loads)
         // is issued together with the second half of the current one, so its latencies hide behind FP64 work.
         int ja = pop_lowest(todo);
@@ -311,7 +434,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
             const int jb = pop_lowest(todo);
             const int jh = jb >= 0 ? jb : ja;  // (a redundant look-up when the list ends on an odd count)
             double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
-            int cnt = 0;
+            int cnt = 0, cntb = 0, npa = 0, npb = 0;  // (cntb, npa, npb: pixel-cut mode)
             {
               const double* tch = KT + (t0 + jh) * NCONST;
               const double* tct = KT + (t0 + ja) * NCONST;
@@ -319,14 +442,20 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               for (int k = 0; k < SPT; ++k)
                 term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, nxt[k]);
+              double wv[SPT];
+              bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                bool live;
-                const double w = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, cur[k], zmask, live);
-                a0 += w;
-                a1 = fma(w, w, a1);
-                cnt += live ? 1 : 0;
+                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, cur[k], zmask, lv[k]);
+                if (!PIX) {
+                  a0 += wv[k];
+                  a1 = fma(wv[k], wv[k], a1);
+                  cnt += lv[k] ? 1 : 0;
+                }
               }
+              if (PIX)
+                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + ja) * 2, s_carryn + warp * T + ja, lane, a0, a1,
+                           cnt, npa);
             }
             const int jc = pop_lowest(todo);
             {
@@ -340,16 +469,43 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               for (int k = 0; k < SPT; ++k)
                 term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh2 * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, cur[k]);
+              double wv[SPT];
+              bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                bool live;
-                double w = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, nxt[k], zmask, live);
-                live = live & second;
-                w = live ? w : 0.0;
-                b0 += w;
-                b1 = fma(w, w, b1);
-                cnt += live ? 0x10000 : 0;
+                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, nxt[k], zmask, lv[k]);
+                lv[k] = lv[k] & second;
+                wv[k] = lv[k] ? wv[k] : 0.0;
+                if (!PIX) {
+                  b0 += wv[k];
+                  b1 = fma(wv[k], wv[k], b1);
+                  cnt += lv[k] ? 0x10000 : 0;
+                }
               }
+              if (PIX && second)  // warp-uniform
+                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + jh) * 2, s_carryn + warp * T + jh, lane, b0, b1,
+                           cntb, npb);
+            }
+            if (PIX) {
+              // pixel-cut mode: the live counts of whole pixels do not fit the 16-bit packing; four reductions
+              cnt = __reduce_add_sync(FULL, cnt);
+              cntb = __reduce_add_sync(FULL, cntb);
+              npa = __reduce_add_sync(FULL, npa);
+              npb = __reduce_add_sync(FULL, npb);
+              const double k = warp_sum4(a0, a1, b0, b1, lane);
+              if ((lane & 7) == 0) {
+                const int j = (lane & 16) ? jb : ja;
+                if (j >= 0) {
+                  s_acc[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
+                  if ((lane & 8) == 0) {
+                    s_cnt[warp * T + j] += (lane & 16) ? cntb : cnt;
+                    s_np[warp * T + j] += (lane & 16) ? npb : npa;
+                  }
+                }
+              }
+              if (jc < 0) break;
+              ja = jc;
+              continue;
             }
             cnt = __reduce_add_sync(FULL, cnt);
             if (cnt) {  // warp-uniform
@@ -371,7 +527,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       // segment complete: combine the warps' partials in a fixed order and write them out
       if (tid < nt) {
         double a = 0.0, b = 0.0;
-        int c = 0;
+        int c = 0, np = 0;
         for (int w = 0; w < NWARPS; ++w) {
           a += s_acc[(w * T + tid) * 2];
           b += s_acc[(w * T + tid) * 2 + 1];
@@ -379,26 +535,31 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           s_acc[(w * T + tid) * 2] = 0.0;
           s_acc[(w * T + tid) * 2 + 1] = 0.0;
           s_cnt[w * T + tid] = 0;
+          if (PIX) {
+            np += s_np[w * T + tid];
+            s_np[w * T + tid] = 0;
+          }
         }
         const size_t o = (size_t)(p.t_begin + t0 + tid) * (size_t)p.n_seg + (size_t)seg;
         p.out_w[2 * o] = a;
         p.out_w[2 * o + 1] = b;
         p.out_n[o] = c;
+        if (PIX) p.out_np[o] = np;
       }
       __syncthreads();  // the reset above precedes the next segment's accumulation
     }
   }
 }
 
-template <typename NodeT, typename LosT, bool INJ>
+template <typename NodeT, typename LosT, bool INJ, bool PIX = false>
 int launch_one(const ReweightParams& p, int n_blocks, size_t smem, cudaStream_t s) {
-  reweight_kernel<NodeT, LosT, INJ><<<n_blocks, NTHREADS, smem, s>>>(p);
+  reweight_kernel<NodeT, LosT, INJ, PIX><<<n_blocks, NTHREADS, smem, s>>>(p);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-template <typename NodeT, typename LosT, bool INJ>
+template <typename NodeT, typename LosT, bool INJ, bool PIX = false>
 int configure_one(int smem_optin) {
-  return cudaFuncSetAttribute(reweight_kernel<NodeT, LosT, INJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  return cudaFuncSetAttribute(reweight_kernel<NodeT, LosT, INJ, PIX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               smem_optin) == cudaSuccess ? 0 : -1;
 }
 
@@ -422,6 +583,10 @@ int reweight_configure(int smem_optin) {
   rc |= configure_one<Node64, float, false>(smem_optin);
   rc |= configure_one<Node32, double, false>(smem_optin);
   rc |= configure_one<Node32, float, false>(smem_optin);
+  rc |= configure_one<Node64, double, false, true>(smem_optin);
+  rc |= configure_one<Node64, float, false, true>(smem_optin);
+  rc |= configure_one<Node32, double, false, true>(smem_optin);
+  rc |= configure_one<Node32, float, false, true>(smem_optin);
   rc |= configure_one<Node64, double, true>(smem_optin);
   rc |= configure_one<Node32, double, true>(smem_optin);
   return rc;
@@ -449,6 +614,13 @@ int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_pr
     if (inj) {
       rc = tab_prec == GWC_F64 ? launch_one<Node64, double, true>(p, n_blocks, smem, s)
                                : launch_one<Node32, double, true>(p, n_blocks, smem, s);
+    } else if (p.pixcut) {
+      if (tab_prec == GWC_F64)
+        rc = los_prec == GWC_F64 ? launch_one<Node64, double, false, true>(p, n_blocks, smem, s)
+                                 : launch_one<Node64, float, false, true>(p, n_blocks, smem, s);
+      else
+        rc = los_prec == GWC_F64 ? launch_one<Node32, double, false, true>(p, n_blocks, smem, s)
+                                 : launch_one<Node32, float, false, true>(p, n_blocks, smem, s);
     } else if (tab_prec == GWC_F64) {
       rc = los_prec == GWC_F64 ? launch_one<Node64, double, false>(p, n_blocks, smem, s)
                                : launch_one<Node64, float, false>(p, n_blocks, smem, s);

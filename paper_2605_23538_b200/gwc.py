@@ -23,7 +23,7 @@ _STATUS = ["GWC_OK", "GWC_ERR_INVALID_ARG", "GWC_ERR_SHAPE", "GWC_ERR_DOMAIN", "
            "GWC_ERR_CUDA"]
 
 EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_launch_count", "gwc_build_cosmo",
-           "gwc_export_cosmo", "gwc_pack_events", "gwc_los_allsky", "gwc_event_loglik", "gwc_selection_logxi",
+           "gwc_export_cosmo", "gwc_pack_events", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_selection_logxi",
            "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_host", "gwc_set_timing", "gwc_get_timing",
            "gwc_probe_fp64", "gwc_math_selftest"]
 
@@ -74,6 +74,7 @@ def load():
         "gwc_pack_events": (ci, [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]),
         "gwc_los_allsky": (ci, [vp, C.POINTER(Los), vp]),
         "gwc_event_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), vp, vp, vp]),
+        "gwc_event_loglik_pixcut": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), dbl, vp, vp, vp, vp]),
         "gwc_selection_logxi": (ci, [vp, vp, i64, C.POINTER(Injections), C.POINTER(Los), vp, vp]),
         "gwc_combine_total": (ci, [vp, vp, vp, i64, i64, vp]),
         "gwc_total_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci, vp]),
@@ -214,6 +215,19 @@ class Context:
         self._ck(self._lib.gwc_event_loglik(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(los),
                                             logL.data_ptr(), _ptr(neff), _ptr(nlive)))
         return logL, neff, nlive
+
+    def gwc_event_loglik_pixcut(self, theta, ev, table, z_max, neff_min):
+        """Event term with the per-pixel N_eff cut of Eq. 8: returns logL, neff, nlive, npass."""
+        nt, ne = theta.shape[0], ev["ev_sample_off"].numel() - 1
+        logL = torch.empty((nt, ne), dtype=torch.float64, device=self.device)
+        neff = torch.empty_like(logL)
+        nlive = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
+        npass = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
+        es, los = make_events(ev), make_los(table, z_max)
+        self._ck(self._lib.gwc_event_loglik_pixcut(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(los),
+                                                   float(neff_min), logL.data_ptr(), neff.data_ptr(),
+                                                   nlive.data_ptr(), npass.data_ptr()))
+        return logL, neff, nlive, npass
 
     def gwc_selection_logxi(self, theta, inj, allsky, n_z, z_max, want_neff=True):
         nt = theta.shape[0]

@@ -251,3 +251,86 @@ def test_determinism(ctx):
     b = _gpu_all(ctx, W, W.theta)
     for k in ("logL", "neff", "logxi", "total"):
         assert np.array_equal(a[k], b[k], equal_nan=True), k
+
+
+# ---- NEXT row 2: the per-pixel N_eff cut of Eq. 8 (R25) -------------------------------
+def _pixcut_both(ctx, W, theta, thr, los=None):
+    los = W.los if los is None else los
+    zmax = W.spec.z_max
+    th = theta.to(DEV)
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    g = ctx.gwc_event_loglik_pixcut(th, to_dev(W.ev, DEV), los.to(DEV), zmax, thr)
+    ctx.gwc_check()
+    o = oracle.event_loglik_pixcut(_np(theta), synth.to_numpy(W.ev), _np(los), zmax, thr)
+    return [_np(x) for x in g], o
+
+
+def _pixcut_compare(g, o, what):
+    gL, gN, gK, gP = g
+    oL, oN, oK, oP = o
+    bad = np.argwhere(gP != oP)
+    assert bad.size == 0, "%s: npass differs at %s" % (what, bad[:8].tolist())
+    bad = np.argwhere(gK != oK)
+    assert bad.size == 0, "%s: nlive differs at %s" % (what, bad[:8].tolist())
+    assert_close_log(gL, oL, RTOL_F64, what + " log L_i")
+    fin = np.isfinite(oL)
+    np.testing.assert_allclose(gN[fin], oN[fin], rtol=1e-7)
+
+
+@pytest.mark.parametrize("thr", [0.0, 2.0, 5.0])
+def test_pixcut_tiny(ctx, thr):
+    W = workload("tiny")
+    g, o = _pixcut_both(ctx, W, W.theta, thr)
+    _pixcut_compare(g, o, "tiny thr=%g" % thr)
+    if thr == 0.0:      # threshold 0 = the uncut path, bit for bit the same sums
+        th = W.theta.to(DEV)
+        logL, neff, nlive = ctx.gwc_event_loglik(th, to_dev(W.ev, DEV), W.los.to(DEV), W.spec.z_max)
+        np.testing.assert_allclose(g[0], _np(logL), rtol=1e-13, atol=0)
+        assert np.array_equal(g[2], _np(nlive))
+
+
+@pytest.mark.parametrize("thr", [2.0, 3.5])
+def test_pixcut_ragged_catalogue(ctx, thr):
+    """O4-like catalogue: ragged events, pixels of 1 to hundreds of samples, pixels that span blocks and warps."""
+    W = workload("o4", n_theta=24, n_events=12, los_rows=600, n_inj=1000)
+    g, o = _pixcut_both(ctx, W, W.theta, thr)
+    _pixcut_compare(g, o, "o4-like thr=%g" % thr)
+    assert (o[3] > 0).any() and (o[3] < o[3].max()).any()
+    # the cut bites: some events lose pixels relative to threshold 0
+    o0 = oracle.event_loglik_pixcut(_np(W.theta), synth.to_numpy(W.ev), _np(W.los), W.spec.z_max, 0.0)
+    assert (o[3] < o0[3]).any()
+
+
+def test_pixcut_long_and_short_pixels(ctx):
+    """Stress layout: events of 32768 samples over thousands of pixels next to events of 512 over 16; plus a
+    hand-made event whose single pixel spans many blocks and one with every sample its own pixel."""
+    W = workload("stress", n_theta=8, n_events=8, los_rows=300, n_inj=1000, big_samples=6000, big_pixels=250,
+                 big_frac=0.25)
+    off = W.ev["ev_sample_off"]
+    row = W.ev["sample_row"].clone()
+    a, b = int(off[0]), int(off[1])
+    row[a:b] = 7                                   # event 0: one pixel over the whole event
+    a, b = int(off[1]), int(off[2])
+    row[a:b] = (torch.arange(b - a) // 2 % 290).to(row.dtype)   # event 1: every pixel has two samples
+    a, b = int(off[2]), int(off[3])
+    row[a:b] = (torch.arange(b - a) % 290).to(row.dtype)        # event 2: every sample its own pixel
+    W.ev["sample_row"] = row
+    for thr in (2.0, 1.0):
+        g, o = _pixcut_both(ctx, W, W.theta, thr)
+        _pixcut_compare(g, o, "stress-like thr=%g" % thr)
+
+
+def test_pixcut_determinism_and_args(ctx):
+    from paper_2605_23538_b200 import gwc
+    W = workload("o4", n_theta=8, n_events=6, los_rows=200, n_inj=500)
+    th = W.theta.to(DEV)
+    ev, los = to_dev(W.ev, DEV), W.los.to(DEV)
+    ctx.gwc_build_cosmo(th, W.spec.z_max, 1025, 0)
+    a = ctx.gwc_event_loglik_pixcut(th, ev, los, W.spec.z_max, 2.0)
+    b = ctx.gwc_event_loglik_pixcut(th, ev, los, W.spec.z_max, 2.0)
+    for x, y in zip(a, b):
+        assert torch.equal(x, y)
+    with pytest.raises(gwc.GwcError):
+        ctx.gwc_event_loglik_pixcut(th, ev, los, W.spec.z_max, -1.0)
+    with pytest.raises(gwc.GwcError):
+        ctx.gwc_event_loglik_pixcut(th, ev, los, W.spec.z_max, float("nan"))
