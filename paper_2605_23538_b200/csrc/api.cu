@@ -149,7 +149,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
                                          (double*)ctx->seg_shift.p, s),
                 "prep_samples"));
   // theta tile: as many tables as shared memory holds, balanced over the tiles
-  int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin);
+  int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut);
   if (T < 1) return fail(ctx, GWC_ERR_SHAPE, "n_nodes / n_z too large for shared memory");
   if ((int64_t)T > n_theta) T = (int)n_theta;
   const int n_tiles = (int)((n_theta + T - 1) / T);

@@ -103,8 +103,8 @@ int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const 
 int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
                        cudaStream_t s);
 int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off, cudaStream_t s);
-size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z);
-int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin);
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix);
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix);
 int reweight_configure(int smem_optin);
 int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm,
                     cudaStream_t s);

@@ -43,20 +43,23 @@ constexpr int BLK = 32 * SPT;      // samples one warp holds in registers at a t
 __constant__ double KT[KT_THETA * NCONST];
 
 struct SmemLayout {
-  size_t math, acc, cnt, np, carry, carryn, allsky, tab, total;
+  size_t math, acc, cnt, np, carry, carryn, lead, leadn, allsky, tab, total;
 };
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
-__host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z) {
+__host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z, bool pix) {
   SmemLayout L;
   size_t o = 0;
   L.math = o;   o = align16(o + sizeof(MathTables));
   L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2);
   L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T);
-  L.np = o;     o = align16(o + sizeof(int) * NWARPS * T);            // pixel-cut mode: passing pixels
-  L.carry = o;  o = align16(o + sizeof(double) * NWARPS * T * 2);     // pixel-cut mode: run left open by a block
-  L.carryn = o; o = align16(o + sizeof(int) * NWARPS * T);
+  // pixel-cut mode only: passing pixels; the run a block leaves open (W, Q, n); the run open at the range start
+  L.np = o;     o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
+  L.carry = o;  o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 : 0));
+  L.carryn = o; o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
+  L.lead = o;   o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 : 0));
+  L.leadn = o;  o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
   L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
   L.tab = o;    o = align16(o + node_bytes * (size_t)T * Mp);
   L.total = o;
@@ -217,6 +220,7 @@ __device__ __forceinline__ int pop_lowest(unsigned& mask) {
 struct PixShape {
   int d[SPT];        // lanes back to the head of this position's run inside row k (>= 64: the run began earlier)
   bool tail[SPT];    // last sample of its run
+  bool lead[SPT];    // inside the run that was already open where this warp's range begins
   int maxd[SPT];     // largest reach of the row (d, or the lane index where the run began earlier): scan steps needed
   bool last_open;    // the block's last position is inside a run that continues in the next block
 };
@@ -239,10 +243,11 @@ __device__ __forceinline__ void seg_scan(double& W, double& Q, int& n, int d, in
 
 // From the per-sample weights of one theta to what the passing pixels add to this lane's sums.
 //   in : w[k], live[k]; carry = (W, Q, n) of the run left open by the previous block (slot of this warp and theta)
+//        leadWQ / leadN: where the run that was open at the start of the warp's range is put when it ends here
 //   out: cW, cQ, cn (weights, squared weights, live samples of the passing pixels that end on this lane), cp = how many
 __device__ __forceinline__ void pix_reduce(const PixShape& ps, const double* w, const bool* live, double neff_min,
-                                           double* carryWQ, int* carryN, int lane, double& cW, double& cQ, int& cn,
-                                           int& cp) {
+                                           double* carryWQ, int* carryN, double* leadWQ, int* leadN, int lane,
+                                           double& cW, double& cQ, int& cn, int& cp) {
   const unsigned FULL = 0xffffffffu;
   double W[SPT], Q[SPT];
   int n[SPT];
@@ -279,24 +284,17 @@ __device__ __forceinline__ void pix_reduce(const PixShape& ps, const double* w, 
   cp = 0;
 #pragma unroll
   for (int k = 0; k < SPT; ++k) {
-    const bool pass = ps.tail[k] && W[k] > 0.0 && W[k] * W[k] >= neff_min * Q[k];
+    if (ps.tail[k] && ps.lead[k]) {  // began in an earlier warp's range: the segment-end stitch decides (one lane at most)
+      leadWQ[0] = W[k];
+      leadWQ[1] = Q[k];
+      *leadN = n[k];
+    }
+    const bool pass = ps.tail[k] && !ps.lead[k] && W[k] > 0.0 && W[k] * W[k] >= neff_min * Q[k];
     cW += pass ? W[k] : 0.0;
     cQ += pass ? Q[k] : 0.0;
     cn += pass ? n[k] : 0;
     cp += pass ? 1 : 0;
   }
-}
-
-// First sample at or after x that starts a pixel (s1 when there is none); s0 starts one by definition.
-__device__ __forceinline__ int64_t first_head(const int32_t* __restrict__ row, int64_t s0, int64_t s1, int64_t x,
-                                              int lane) {
-  if (x <= s0) return s0;
-  for (; x < s1; x += 32) {
-    const int64_t g = x + lane;
-    const unsigned m = __ballot_sync(0xffffffffu, g < s1 && row[g] != row[g - 1]);
-    if (m) return x + (__ffs(m) - 1);
-  }
-  return s1;
 }
 
 // One sample's theta-independent values, held in registers while the warp loops over the tile's theta points.
@@ -314,13 +312,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
   typedef typename std::conditional<INJ, double, LosT>::type RowT;  // the all-sky table is f64
-  const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z);
+  const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z, PIX);
   MathTables& mt = *reinterpret_cast<MathTables*>(smem + L.math);
   double* s_acc = reinterpret_cast<double*>(smem + L.acc);
   int* s_cnt = reinterpret_cast<int*>(smem + L.cnt);
   int* s_np = reinterpret_cast<int*>(smem + L.np);
   double* s_carry = reinterpret_cast<double*>(smem + L.carry);
   int* s_carryn = reinterpret_cast<int*>(smem + L.carryn);
+  double* s_lead = reinterpret_cast<double*>(smem + L.lead);
+  int* s_leadn = reinterpret_cast<int*>(smem + L.leadn);
+  __shared__ int s_hashead[NWARPS];  // pixel-cut mode: the warp's range of the current segment contains a pixel start
   double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
   NodeT* s_tab = reinterpret_cast<NodeT*>(smem + L.tab);
 
@@ -362,10 +363,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) s_acc[i] = 0.0;
     for (int i = tid; i < NWARPS * T; i += NTHREADS) s_cnt[i] = 0;
     if (PIX) {
-      for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) s_carry[i] = 0.0;
+      for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) {
+        s_carry[i] = 0.0;
+        s_lead[i] = 0.0;
+      }
       for (int i = tid; i < NWARPS * T; i += NTHREADS) {
         s_np[i] = 0;
         s_carryn[i] = 0;
+        s_leadn[i] = 0;
       }
     }
     __syncthreads();
@@ -374,13 +379,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     for (int seg = seg_lo; seg < seg_hi; ++seg) {
       const int64_t s0 = p.seg_off[seg], s1 = p.seg_off[seg + 1];
       // The segment's samples in blocks of BLK, dealt to the warps round-robin; no barrier until the segment ends.
-      // Pixel-cut mode: each warp takes one contiguous range instead, cut where a pixel starts, so that every
-      // pixel lies inside one warp and the run a block leaves open is continued by the same warp's next block.
+      // Pixel-cut mode: each warp takes one contiguous range of whole blocks instead, so that the run a block
+      // leaves open is continued by the same warp's next block; the pixels that cross from one warp's range
+      // into the next are put together when the segment ends (lead / trail sums below).
       int64_t w_lo = s0 + (int64_t)warp * BLK, w_hi = s1, w_step = (int64_t)NWARPS * BLK;
+      bool lead_open = true;  // no pixel start seen yet in this warp's range
       if (PIX) {
-        const int64_t len = s1 - s0;
-        w_lo = first_head(p.row, s0, s1, s0 + len * warp / NWARPS, lane);
-        w_hi = warp + 1 == NWARPS ? s1 : first_head(p.row, s0, s1, s0 + len * (warp + 1) / NWARPS, lane);
+        const int64_t nb = (s1 - s0 + BLK - 1) / BLK;
+        w_lo = s0 + nb * warp / NWARPS * BLK;
+        w_hi = min(s1, s0 + nb * (warp + 1) / NWARPS * BLK);
         w_step = BLK;
       }
       for (int64_t c0 = w_lo; c0 < w_hi; c0 += w_step) {
@@ -394,13 +401,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           if (PIX) {
             // run structure of the row: heads, distance to the head, tails
             const int32_t r = in ? p.row[g] : 0;
-            const bool head = in && (g == w_lo || p.row[g - 1] != r);
-            const bool tail = in && (g + 1 >= w_hi || p.row[g + 1] != r);
-            const unsigned hm = __ballot_sync(FULL, head) & (0xffffffffu >> (31 - lane));
+            const bool head = in && (g == s0 || p.row[g - 1] != r);
+            const bool tail = in && (g + 1 >= s1 || p.row[g + 1] != r);
+            const unsigned hall = __ballot_sync(FULL, head);
+            const unsigned hm = hall & (0xffffffffu >> (31 - lane));
             ps.d[k] = hm ? lane - (31 - __clz(hm)) : 64;
             ps.tail[k] = tail;
+            ps.lead[k] = lead_open && hm == 0;
             ps.maxd[k] = __reduce_max_sync(FULL, in ? (hm ? ps.d[k] : lane) : 0);
+            // (ranges end on block boundaries or on the segment's last sample, which is a tail)
             if (k == SPT - 1) ps.last_open = __shfl_sync(FULL, (int)(in && !tail), 31) != 0;
+            lead_open = lead_open && hall == 0;
           }
           sm[k].A = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
           sm[k].m2z = in ? p.m2z[g] : 1.0;
@@ -454,8 +465,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
                 }
               }
               if (PIX)
-                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + ja) * 2, s_carryn + warp * T + ja, lane, a0, a1,
-                           cnt, npa);
+                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + ja) * 2, s_carryn + warp * T + ja,
+                           s_lead + (warp * T + ja) * 2, s_leadn + warp * T + ja, lane, a0, a1, cnt, npa);
             }
             const int jc = pop_lowest(todo);
             {
@@ -483,8 +494,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
                 }
               }
               if (PIX && second)  // warp-uniform
-                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + jh) * 2, s_carryn + warp * T + jh, lane, b0, b1,
-                           cntb, npb);
+                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + jh) * 2, s_carryn + warp * T + jh,
+                           s_lead + (warp * T + jh) * 2, s_leadn + warp * T + jh, lane, b0, b1, cntb, npb);
             }
             if (PIX) {
               // pixel-cut mode: the live counts of whole pixels do not fit the 16-bit packing; four reductions
@@ -523,6 +534,21 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           }
         }
       }
+      if (PIX) {
+        // What this warp's range leaves for the stitch: the run open at its start (lead), whether a pixel starts
+        // inside it, and the run open at its end (trail = the carry slot).  No pixel start at all: the whole range
+        // is one open run and belongs to the lead.
+        __syncwarp();
+        if (lead_open && lane < nt) {
+          s_lead[(warp * T + lane) * 2] += s_carry[(warp * T + lane) * 2];
+          s_lead[(warp * T + lane) * 2 + 1] += s_carry[(warp * T + lane) * 2 + 1];
+          s_leadn[warp * T + lane] += s_carryn[warp * T + lane];
+          s_carry[(warp * T + lane) * 2] = 0.0;
+          s_carry[(warp * T + lane) * 2 + 1] = 0.0;
+          s_carryn[warp * T + lane] = 0;
+        }
+        if (lane == 0) s_hashead[warp] = lead_open ? 0 : 1;
+      }
       __syncthreads();
       // segment complete: combine the warps' partials in a fixed order and write them out
       if (tid < nt) {
@@ -538,6 +564,39 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           if (PIX) {
             np += s_np[w * T + tid];
             s_np[w * T + tid] = 0;
+          }
+        }
+        if (PIX) {
+          // pixels that cross warp ranges: walk the ranges in order, close the open run wherever a pixel starts
+          double oW = 0.0, oQ = 0.0;
+          int oN = 0;
+          for (int w = 0; w <= NWARPS; ++w) {
+            if (w < NWARPS) {
+              oW += s_lead[(w * T + tid) * 2];
+              oQ += s_lead[(w * T + tid) * 2 + 1];
+              oN += s_leadn[w * T + tid];
+            }
+            if (w == NWARPS || s_hashead[w]) {
+              if (oW > 0.0 && oW * oW >= p.neff_min * oQ) {
+                a += oW;
+                b += oQ;
+                c += oN;
+                np += 1;
+              }
+              if (w < NWARPS) {
+                oW = s_carry[(w * T + tid) * 2];
+                oQ = s_carry[(w * T + tid) * 2 + 1];
+                oN = s_carryn[w * T + tid];
+              }
+            }
+            if (w < NWARPS) {
+              s_lead[(w * T + tid) * 2] = 0.0;
+              s_lead[(w * T + tid) * 2 + 1] = 0.0;
+              s_leadn[w * T + tid] = 0;
+              s_carry[(w * T + tid) * 2] = 0.0;
+              s_carry[(w * T + tid) * 2 + 1] = 0.0;
+              s_carryn[w * T + tid] = 0;
+            }
           }
         }
         const size_t o = (size_t)(p.t_begin + t0 + tid) * (size_t)p.n_seg + (size_t)seg;
@@ -565,14 +624,14 @@ int configure_one(int smem_optin) {
 
 }  // namespace
 
-size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z) {
-  return smem_layout(T, Mp, tab_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32), inj, n_z).total;
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix) {
+  return smem_layout(T, Mp, tab_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32), inj, n_z, pix).total;
 }
 
-int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin) {
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix) {
   int best = 0;
   for (int T = 1; T <= MAX_T; ++T)
-    if (reweight_smem_bytes(T, Mp, tab_prec, inj, n_z) + SMEM_RESERVE <= (size_t)smem_optin) best = T;
+    if (reweight_smem_bytes(T, Mp, tab_prec, inj, n_z, pix) + SMEM_RESERVE <= (size_t)smem_optin) best = T;
   return best;
 }
 
@@ -596,7 +655,7 @@ int reweight_configure(int smem_optin) {
 // first copies its points' constants into the constant bank (stream-ordered) and resets the work counter.
 int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm,
                     cudaStream_t s) {
-  const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z);
+  const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z, p0.pixcut != 0);
   const int cap = (KT_THETA / p0.T) * p0.T;
   int launched = 0;
   for (int tb = 0; tb < p0.n_theta; tb += cap) {

@@ -150,3 +150,33 @@ def test_stress_f64_and_f32_tables(ctx):
     fin = np.isfinite(t64) & np.isfinite(t32) & same[tsel]
     assert fin.any()
     assert np.abs(t32[fin] - t64[fin]).max() <= ATOL_F32
+
+
+def test_production_pixcut_sampled(ctx):
+    """NEXT row 2 at full size: the per-pixel N_eff cut (threshold 2, the paper's fiducial) on the
+    production batch, all events x a seeded subset of theta against the oracle.  A pixel of two samples has
+    N_eff = 2 - (w1 - w2)^2 / (w1^2 + w2^2) <= 2: with weights equal to ~1e-8 the decision N_eff >= 2 hangs on
+    the last bit of the sums (R25), so (theta, event) pairs whose pixel count differs from the
+    oracle's are counted, printed and required to be rare; all others must meet the 1e-9 bar."""
+    W, theta = _device_workload("production")
+    zmax = W.spec.z_max
+    ctx.gwc_build_cosmo(theta, zmax, 1025, 0)
+    gL, gN, gK, gP = [_np(x) for x in ctx.gwc_event_loglik_pixcut(theta, W.ev, W.los, zmax, 2.0)]
+    ctx.gwc_check()
+    tsel = _pick(theta.shape[0], 8, 11)
+    oL, oN, oK, oP = oracle.event_loglik_pixcut(_np(theta)[tsel], synth.to_numpy(W.ev), _np(W.los), zmax, 2.0)
+    same = gP[tsel] == oP
+    n_flip = int((~same).sum())
+    print("production pixcut: %d (theta, event) pairs, %d with a different pixel count (max |dnpass| %d); "
+          "mean passing pixels %.1f of %.1f" % (same.size, n_flip, int(np.abs(gP[tsel] - oP).max()), oP.mean(),
+                                                oracle.event_loglik_pixcut(_np(theta)[tsel[:1]], synth.to_numpy(W.ev),
+                                                                           _np(W.los), zmax, 0.0)[3].mean()))
+    assert n_flip <= 1e-3 * same.size
+    assert np.abs(gP[tsel] - oP).max() <= 1
+    assert np.array_equal(gK[tsel][same], oK[same])
+    g, o = gL[tsel], oL
+    assert np.array_equal(np.isneginf(g[same]), np.isneginf(o[same]))
+    fin = same & np.isfinite(o)
+    err = np.abs(g[fin] - o[fin]) / np.maximum(np.abs(o[fin]), 1.0)
+    assert err.max() <= RTOL_F64, err.max()
+    np.testing.assert_allclose(gN[tsel][fin], oN[fin], rtol=1e-7)
