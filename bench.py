@@ -231,6 +231,24 @@ def run_gwc(args):
                 "live_fraction_events": live_frac_ev,
                 "peak_source": "derived: 148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md section 7)",
                 "peak_measured_dfma_probe": probe_n * 2.0 / (probe_ms * 1e-3) / 1e12}
+    # ---- NEXT row 2, reported beside the headline: the event term with the per-pixel N_eff cut (Eq. 8) ----
+    pix = None
+    if args.pixcut >= 0:
+        ctx.gwc_build_cosmo(theta, zmax, args.n_nodes, prec)
+        ctx.gwc_event_loglik_pixcut(theta, W.ev, W.los, zmax, args.pixcut)
+        torch.cuda.synchronize()
+        ctx.gwc_set_timing(True)
+        ctx.gwc_get_timing()
+        npass = None
+        for _ in range(2):
+            _, _, _, npass = ctx.gwc_event_loglik_pixcut(theta, W.ev, W.los, zmax, args.pixcut)
+        torch.cuda.synchronize()
+        tp = ctx.gwc_get_timing()
+        ctx.gwc_set_timing(False)
+        ms_pix = tp["ms_ev"] / max(tp["n_ev"], 1)
+        pix = {"neff_min": args.pixcut, "event_kernel_ms": ms_pix, "event_terms_per_s": terms_ev / (ms_pix * 1e-3),
+               "slowdown_vs_uncut": ms_pix / ms_ev_kernel, "mean_passing_pixels_per_event": float(npass.double().mean())}
+        del npass
     cpu = cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
     stress = stress_report(ctx, W, theta, zmax, allsky, args.n_nodes) if spec.name == "stress" else None
     line = {
@@ -256,6 +274,8 @@ def run_gwc(args):
     }
     if stress is not None:
         line["stress_report"] = stress
+    if pix is not None:
+        line["pixcut"] = pix
     print(json.dumps(line))
     if dist:
         td.destroy_process_group()
@@ -376,6 +396,8 @@ def main():
     ap.add_argument("--seed", type=int, default=synth.DEFAULT_SEED)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle timing budget (0 = skip)")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--pixcut", type=float, default=2.0,
+                    help="also time the event term with the per-pixel N_eff cut at this threshold (< 0: skip)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "gwc" and args.theta_scale == 1.0:
         args.warmup = 3
