@@ -334,3 +334,37 @@ def test_pixcut_determinism_and_args(ctx):
         ctx.gwc_event_loglik_pixcut(th, ev, los, W.spec.z_max, -1.0)
     with pytest.raises(gwc.GwcError):
         ctx.gwc_event_loglik_pixcut(th, ev, los, W.spec.z_max, float("nan"))
+
+
+def test_pixcut_edge_cases_and_32bit_tables(ctx):
+    """Pixel cut with empty events, dead / invalid samples (which still delimit pixels by their raw row value),
+    a user PE prior, f32 LOS rows and the 32-bit cosmology table."""
+    W = workload("o4", n_theta=12, n_events=6, los_rows=120, n_inj=500)
+    ev = {k: (v.clone() if isinstance(v, torch.Tensor) else v) for k, v in W.ev.items()}
+    off = ev["ev_sample_off"].clone()
+    off[2] = off[3]                               # event 2 becomes empty, its samples join event 1
+    ev["ev_sample_off"] = off
+    ev["dL"][5] = float("nan")
+    ev["dL"][17] = -2.0
+    ev["sample_row"][40:44] = 10_000              # invalid rows: dead, but a pixel of their own
+    ev["sample_row"][60] = -7
+    ev["m2z"][80] = ev["m1z"][80] * 2.0
+    g = torch.Generator().manual_seed(3)
+    ev["log_pe_prior"] = 2.0 * torch.log(ev["dL"].abs().clamp_min(1.0)) + 0.3 * torch.rand(ev["dL"].numel(), generator=g,
+                                                                                         dtype=torch.float64)
+    zmax = W.spec.z_max
+    th = W.theta.to(DEV)
+    for los, prec in ((W.los, 0), (W.los.to(torch.float32), 0), (W.los.to(torch.float32), 1)):
+        ctx.gwc_build_cosmo(th, zmax, 1025, prec)
+        gq = [_np(x) for x in ctx.gwc_event_loglik_pixcut(th, to_dev(ev, DEV), los.to(DEV), zmax, 2.0)]
+        ctx.gwc_check()
+        o = oracle.event_loglik_pixcut(_np(W.theta), synth.to_numpy(ev), _np(los), zmax, 2.0, table_prec=prec)
+        if prec == 0:
+            _pixcut_compare(gq, o, "edge cases (%s LOS)" % los.dtype)
+        else:   # 32-bit nodes: a node on a rounding boundary may round apart on the two sides (as test_f32_table_variant)
+            same = gq[3] == o[3]
+            assert same.mean() > 0.99
+            fin = same & np.isfinite(o[0])
+            assert np.array_equal(np.isneginf(gq[0][same]), np.isneginf(o[0][same]))
+            assert (np.abs(gq[0][fin] - o[0][fin]) / np.maximum(np.abs(o[0][fin]), 1.0)).max() <= 1e-6
+    assert np.all(np.isneginf(gq[0][:, 2])) and np.all(gq[3][:, 2] == 0)
