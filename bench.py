@@ -228,6 +228,9 @@ def run_gwc(args):
                 "kernel_share_of_step": ms_ev_kernel / (ms / args.steps),
                 "inj_kernel_ms": ms_inj_kernel,
                 "fp64_instr_per_live_term": FP64_INSTR_LIVE, "fp64_instr_per_dead_term": FP64_INSTR_DEAD,
+                # the same time against the budget BASELINE.md froze before any code (180 live / 30 dead): context only
+                "frac_at_survey_budget_180_30": terms_ev * (live_frac_ev * 180.0 + (1.0 - live_frac_ev) * 30.0)
+                / (ms_ev_kernel * 1e-3) / FP64_PEAK_INSTR,
                 "live_fraction_events": live_frac_ev,
                 "peak_source": "derived: 148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md section 7)",
                 "peak_measured_dfma_probe": probe_n * 2.0 / (probe_ms * 1e-3) / 1e12}
