@@ -65,6 +65,8 @@ def lib():
             "orc_lse": (None, [vp, i64, vp, vp]),
             "orc_event_loglik": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, vp, vp, vp]),
             "orc_event_loglik_pixcut": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, d, vp, vp, vp, vp]),
+            "orc_event_loglik_kde": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, C.c_int, d, vp, vp]),
+            "orc_kde_samples": (C.c_int, [vp, vp, i64, d, C.c_int, d, C.c_int, vp, vp]),
             "orc_selection_logxi": (C.c_int, [vp, i64, vp, vp, i32, d, C.c_int, d, C.c_int, C.c_int, vp, vp]),
             "orc_total_from_parts": (None, [vp, vp, i64, i64, vp]),
             "orc_pack_events": (i64, [i64, i64, vp, vp, vp, vp, vp, vp, vp]),
@@ -193,6 +195,46 @@ def event_loglik_pixcut(theta, ev, los_table, los_z_max, neff_min, *, mode=TABLE
                                        float(neff_min), _p(logL), _p(neff), _p(nlive), _p(npass))
     assert rc == 0
     return logL, neff, nlive, npass
+
+
+def _events_struct(ev):
+    off = np.ascontiguousarray(ev["ev_sample_off"], dtype=np.int64)
+    dl, m1, m2 = _f64(ev["dL"]), _f64(ev["m1z"]), _f64(ev["m2z"])
+    row = np.ascontiguousarray(ev["sample_row"], dtype=np.int32)
+    lpe = ev.get("log_pe_prior")
+    lpe = None if lpe is None else _f64(lpe)
+    es = _Events(off.size - 1, dl.size, off.ctypes.data, dl.ctypes.data, m1.ctypes.data, m2.ctypes.data,
+                 None if lpe is None else lpe.ctypes.data, row.ctypes.data)
+    return es, (off, dl, m1, m2, row, lpe)
+
+
+def event_loglik_kde(theta, ev, los_table, los_z_max, *, n_grid=256, neff_min=0.0, mode=TABLE, z_max=None,
+                     n_nodes=1025, table_prec=0):
+    """Event term with the paper's KDE numerator (Eq. 5-7, D1; R26-R30).  Returns logL (f64) and npass
+    (int64), both [n_theta, n_events]."""
+    th = _theta(theta)
+    es, keep_ev = _events_struct(ev)
+    ls, keep = _los_struct(los_table, los_z_max)
+    nt, ne = th.shape[0], es.n_events
+    logL, npass = np.empty((nt, ne)), np.empty((nt, ne), dtype=np.int64)
+    zm = float(los_z_max if z_max is None else z_max)
+    rc = lib().orc_event_loglik_kde(_p(th), nt, C.addressof(es), C.addressof(ls), mode, zm, n_nodes, table_prec,
+                                    int(n_grid), float(neff_min), _p(logL), _p(npass))
+    assert rc == 0
+    return logL, npass
+
+
+def kde_samples(theta1, ev, n_rows, los_z_max, *, mode=TABLE, z_max=None, n_nodes=1025):
+    """Per-sample (z_k, log v_k) of ONE theta: the inputs of the KDE (v = Eq. 7's weight without the z prior)."""
+    th = _theta(theta1)
+    assert th.shape[0] == 1
+    es, keep_ev = _events_struct(ev)
+    n = es.n_samples
+    z, lv = np.empty(n), np.empty(n)
+    zm = float(los_z_max if z_max is None else z_max)
+    rc = lib().orc_kde_samples(_p(th), C.addressof(es), int(n_rows), float(los_z_max), mode, zm, n_nodes, _p(z), _p(lv))
+    assert rc == 0
+    return z, lv
 
 
 def selection_logxi(theta, inj, allsky, los_z_max, *, mode=TABLE, z_max=None, n_nodes=1025, table_prec=0):

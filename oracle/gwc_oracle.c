@@ -551,6 +551,166 @@ int orc_event_loglik_pixcut(const double* theta, int64_t n_theta, const orc_even
   return err;
 }
 
+/* ------------------------------------------------------------------------------------------------ */
+/* NEXT row 1: the paper's own numerator, a kernel density estimate in z per sky pixel   */
+/* (Eq. 5-7; bandwidth Eq. D1; 256-node grid).             */
+/* Readings R26-R30 of DESIGN.md.  For pixel j of event i (a run of equal sample_row, R25):            */
+/*   v_k  = p(m1, m2 | theta) / (J pi_PE)      the weight of Eq. 7 without the redshift prior          */
+/*   h_j  = 1.06 sigma_j n_j^(-1/5)            sigma_j = v-weighted standard deviation of the z_k,      */
+/*                                             n_j = live samples of the pixel                          */
+/*   f_j(z) = sum_k v_k N(z; z_k, h_j)          Eq. 6, Gaussian kernel                                   */
+/*   I_j  = trapezoid over the G-node uniform grid on [0, z_max] of f_j(z) p_los(z | row_j) R(z; theta) */
+/*   L_i  = (1/S_i) sum_j I_j over the pixels with n_j >= 2, sigma_j > 0 and N_eff,j >= neff_min.      */
+/* ------------------------------------------------------------------------------------------------ */
+/* log v_k and z_k of one sample; -INFINITY when dead (same support rules as orc_log_weight, minus p_los > 0) */
+static double kde_sample(const double* th, int mode, const orc_cosmo_tab* ct, double dL, double m1z, double m2z,
+                         double lpi, double los_z_max, int64_t row, int64_t n_rows, double* z_out) {
+  *z_out = 0.0;
+  if (!(isfinite(dL) && isfinite(m1z) && isfinite(m2z) && isfinite(lpi))) return -INFINITY;
+  if (!(dL > 0.0 && m1z > 0.0 && m2z > 0.0)) return -INFINITY;
+  if (row < 0 || row >= n_rows) return -INFINITY;
+  double H0 = th[P_H0], Om = th[P_OM];
+  double u = dL * H0 / C_KMS;
+  double z;
+  if (mode == 0) {
+    if (orc_z_table(u, ct->ztab, ct->dztab, ct->M, ct->umax, &z)) return -INFINITY;
+  } else {
+    if (!(u < ct->umax)) return -INFINITY;
+    z = orc_z_of_u(u, Om);
+  }
+  if (!(z < los_z_max)) return -INFINITY;
+  double x = 1.0 + z;
+  double m1 = m1z / x, m2 = m2z / x;
+  if (!(m1 > th[P_MMIN] && m1 <= th[P_MMAX] && m2 >= th[P_MMIN] && m2z <= m1z)) return -INFINITY;
+  double p1 = p1_c(m1, th, &ct->pop);
+  double p2 = orc_p2(m2 <= m1 ? m2 : m1, m1, th);
+  if (!(p1 > 0.0) || !(p2 > 0.0)) return -INFINITY;
+  double J = x * x * (C_KMS / H0) * (u / x + x / orc_E(z, Om));
+  *z_out = z;
+  return log(p1) + log(p2) - log(J) - lpi;
+}
+
+/* per-sample (z_k, log v_k) of one theta, for the pins (numpy recomputes bandwidths and closed forms from them) */
+int orc_kde_samples(const double* th, const orc_events* ev, int64_t n_rows, double los_z_max, int mode, double z_max,
+                    int M, double* z_out, double* lv_out) {
+  if (!orc_theta_valid(th)) return 1;
+  orc_cosmo_tab ct;
+  double* buf = NULL;
+  if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) return 1;
+  for (int64_t k = 0; k < ev->n_samples; ++k) {
+    double lpi = ev->log_pe_prior ? ev->log_pe_prior[k] : 2.0 * log(ev->dL[k]);
+    lv_out[k] = kde_sample(th, mode, &ct, ev->dL[k], ev->m1z[k], ev->m2z[k], lpi, los_z_max,
+                           (int64_t)ev->sample_row[k], n_rows, &z_out[k]);
+  }
+  free(buf);
+  return 0;
+}
+
+/*
+ * log L_i(theta) with the KDE numerator, for every (theta, event); npass = pixels that contributed.
+ * n_grid = G (>= 2).  Outputs [n_theta][n_events].
+ */
+int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events* ev, const orc_los* L, int mode,
+                         double z_max, int M, int table_prec, int n_grid, double neff_min, double* logL,
+                         int64_t* npass) {
+  int err = 0;
+  int64_t smax = 0;
+  for (int64_t i = 0; i < ev->n_events; ++i) {
+    int64_t s = ev->ev_sample_off[i + 1] - ev->ev_sample_off[i];
+    if (s > smax) smax = s;
+  }
+  const double dzg = L->z_max / (n_grid - 1);
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t t = 0; t < n_theta; ++t) {
+    const double* th = theta + t * ORC_NPAR;
+    size_t nb = (size_t)(smax > 0 ? smax : 1);
+    double* lv = (double*)malloc(sizeof(double) * nb);
+    double* zz = (double*)malloc(sizeof(double) * nb);
+    double* lI = (double*)malloc(sizeof(double) * nb);   /* log I_j of the passing pixels of one event */
+    double* Rg = (double*)malloc(sizeof(double) * (size_t)n_grid);
+    if (!orc_theta_valid(th) || !lv || !zz || !lI || !Rg) {
+      for (int64_t i = 0; i < ev->n_events; ++i) {
+        logL[t * ev->n_events + i] = NAN;
+        if (npass) npass[t * ev->n_events + i] = 0;
+      }
+      if (!lv || !zz || !lI || !Rg) err = 1;
+      free(lv); free(zz); free(lI); free(Rg);
+      continue;
+    }
+    orc_cosmo_tab ct;
+    double* buf = NULL;
+    if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lv); free(zz); free(lI); free(Rg); continue; }
+    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
+    for (int g = 0; g < n_grid; ++g) {            /* rate term on the grid: R(z) = psi(z) / (1+z), reading R4 */
+      double zg = g * dzg;
+      Rg[g] = psi_c(zg, th, &ct.pop) / (1.0 + zg);
+    }
+    for (int64_t i = 0; i < ev->n_events; ++i) {
+      int64_t a = ev->ev_sample_off[i], b = ev->ev_sample_off[i + 1];
+      for (int64_t k = a; k < b; ++k) {
+        double lpi = ev->log_pe_prior ? ev->log_pe_prior[k] : 2.0 * log(ev->dL[k]);
+        lv[k - a] = kde_sample(th, mode, &ct, ev->dL[k], ev->m1z[k], ev->m2z[k], lpi, L->z_max,
+                               (int64_t)ev->sample_row[k], L->n_rows, &zz[k - a]);
+      }
+      int64_t np = 0;
+      int64_t r0 = a;
+      while (r0 < b) {                            /* one pixel: samples r0 .. r1-1 */
+        int64_t r1 = r0 + 1;
+        while (r1 < b && ev->sample_row[r1] == ev->sample_row[r0]) ++r1;
+        int64_t row = ev->sample_row[r0];
+        int64_t n = 0;
+        double m = -INFINITY;
+        for (int64_t k = r0; k < r1; ++k)
+          if (lv[k - a] > -INFINITY) { ++n; if (lv[k - a] > m) m = lv[k - a]; }
+        if (n >= 2) {
+          long double V = 0.0L, Vz = 0.0L, Q = 0.0L;
+          for (int64_t k = r0; k < r1; ++k) {
+            if (lv[k - a] == -INFINITY) continue;
+            double e = exp(lv[k - a] - m);
+            V += e; Vz += (long double)e * zz[k - a]; Q += (long double)e * e;
+          }
+          double mu = (double)(Vz / V);
+          long double S2 = 0.0L;
+          for (int64_t k = r0; k < r1; ++k) {
+            if (lv[k - a] == -INFINITY) continue;
+            double e = exp(lv[k - a] - m), d = zz[k - a] - mu;
+            S2 += (long double)e * d * d;
+          }
+          double var = (double)(S2 / V);
+          double Vd = (double)V, Qd = (double)Q;
+          if (var > 0.0 && Vd * Vd >= neff_min * Qd) {
+            double h = 1.06 * sqrt(var) * pow((double)n, -0.2);            /* Eq. D1 */
+            double norm = 1.0 / (h * sqrt(2.0 * M_PI));
+            long double I = 0.0L;
+            for (int g = 0; g < n_grid; ++g) {
+              double zg = g * dzg;
+              double f = 0.0;                                                /* Eq. 6 at z_g, relative to e^m */
+              for (int64_t k = r0; k < r1; ++k) {
+                if (lv[k - a] == -INFINITY) continue;
+                double q = (zg - zz[k - a]) / h;
+                f += exp(lv[k - a] - m) * norm * exp(-0.5 * q * q);
+              }
+              double zl = zg < L->z_max ? zg : L->z_max;                     /* last node: the table's last value */
+              double prior = orc_los_lerp(L, row, zl) * Rg[g];
+              double c = (g == 0 || g == n_grid - 1) ? 0.5 * dzg : dzg;      /* trapezoid */
+              I += (long double)c * f * prior;
+            }
+            if (I > 0.0L) { lI[np++] = m + (double)logl(I); }
+          }
+        }
+        r0 = r1;
+      }
+      double l1, l2;
+      lse2(lI, np, &l1, &l2);
+      logL[t * ev->n_events + i] = (b > a) ? l1 - log((double)(b - a)) : -INFINITY;
+      if (npass) npass[t * ev->n_events + i] = np;
+    }
+    free(buf);
+    free(lv); free(zz); free(lI); free(Rg);
+  }
+  return err;
+}
+
 /*
  * log xi(theta) = LSE_j log w_j - ln n_draw over found injections, with the all-sky
  * prior (a 1-row f64 table) in place of the pixel row and log_pdraw in place of the PE prior.

@@ -512,3 +512,142 @@ def test_pixcut_invariant_under_pixel_order_and_dead_padding(theta0):
     S1 = n - off[1]
     assert got3[0][0, 1] == pytest.approx(base[0][0, 1] - math.log((S1 + pad) / S1), abs=1e-12)
     assert np.array_equal(got3[3], base[3]) and np.array_equal(got3[2], base[2])
+
+
+# ---- NEXT row 1: the paper's KDE numerator (Eq. 5-7, D1; R26-R30) -------------------------------------
+def _kde_event(n=300, seed=21, rows=4, dl0=2600.0, pix_min=2):
+    """One-or-two-event toy whose every pixel has >= pix_min samples well inside the z grid."""
+    rng = np.random.default_rng(seed)
+    dl = dl0 * np.exp(0.12 * rng.standard_normal(n))
+    m1z = 50.0 * (1 + 0.06 * rng.standard_normal(n))
+    m2z = 38.0 * (1 + 0.06 * rng.standard_normal(n))
+    m1z, m2z = np.maximum(m1z, m2z), np.minimum(m1z, m2z)
+    half = n // 2
+    row = np.concatenate([np.sort(rng.integers(0, rows, half)), np.sort(rng.integers(0, rows, n - half))]).astype(np.int32)
+    return dict(ev_sample_off=np.array([0, half, n], dtype=np.int64), dL=dl, m1z=m1z, m2z=m2z, sample_row=row,
+                log_pe_prior=None)
+
+
+def _theta_unit_rate(theta0):
+    th = theta0.copy()
+    th[9], th[10] = 1.0, -1.0       # gamma = 1, kappa = -1: psi(z)/(1+z) = 1 identically (psi0 = 2, denominator 2)
+    return th
+
+
+def test_kde_unit_rate_is_one(theta0):
+    th = _theta_unit_rate(theta0)
+    for z in (0.0, 0.3, 1.2):
+        assert O.lib().orc_psi(z, O._p(O._theta(th))) / (1 + z) == pytest.approx(1.0, abs=1e-15)
+
+
+def test_kde_linear_prior_equals_direct_sum(theta0):
+    # int N(z; z_k, h) (a + b z) dz = a + b z_k: with a LOS row linear in z and a unit rate the KDE numerator is the
+    # direct Monte-Carlo sum, whatever the bandwidth (kernels resolved by the grid, h >= 2 dz, and inside it).
+    ev = _kde_event()
+    zmax, nz = 1.5, 64
+    zb = np.linspace(0, zmax, nz)
+    tab = np.stack([0.7 + 0.0 * zb, 0.2 + 1.3 * zb, 2.0 - 0.9 * zb, 0.05 + 0.4 * zb])
+    th = _theta_unit_rate(theta0)
+    Ld, _, kd = O.event_loglik(th, ev, tab, zmax)
+    Lk, npk = O.event_loglik_kde(th, ev, tab, zmax, n_grid=256)
+    assert np.all(kd > 0) and np.all(npk == 4)
+    np.testing.assert_allclose(Lk, Ld, rtol=0, atol=2e-7)     # Gaussian tails beyond the grid: < 1e-7
+    # the grid resolution does not matter while h >= 2 dz
+    Lk2, _ = O.event_loglik_kde(th, ev, tab, zmax, n_grid=200)
+    np.testing.assert_allclose(Lk2, Lk, rtol=0, atol=1e-9)
+
+
+def _pixel_runs(ev):
+    off, row = ev["ev_sample_off"], ev["sample_row"]
+    return [[(r0, r1) for r0, r1 in _runs(row, off[i], off[i + 1])] for i in range(off.size - 1)]
+
+
+def _scott(z, v):
+    """Eq. D1 with the v-weighted standard deviation of the pixel's redshifts and n = its live samples."""
+    mu = np.sum(v * z) / np.sum(v)
+    sig = math.sqrt(np.sum(v * (z - mu) ** 2) / np.sum(v))
+    return 1.06 * sig * z.size ** (-0.2)
+
+
+def test_kde_bandwidth_through_quadratic_prior(theta0):
+    # int N(z; z_k, h) z^2 dz = z_k^2 + h^2: a LOS row equal to z^2 exposes the bandwidth of every pixel.
+    ev = _kde_event(n=260, seed=4, rows=5)
+    zmax, nz = 1.5, 4096                                   # fine LOS nodes: the lerp of z^2 is exact to 3e-8
+    zb = np.linspace(0, zmax, nz)
+    tab = np.tile(zb ** 2, (5, 1))
+    th = _theta_unit_rate(theta0)
+    z, lv = O.kde_samples(th, ev, 5, zmax)
+    assert np.all(np.isfinite(lv))
+    Lk, _ = O.event_loglik_kde(th, ev, tab, zmax, n_grid=256)
+    off = ev["ev_sample_off"]
+    for i, runs in enumerate(_pixel_runs(ev)):
+        tot, tot_h0 = 0.0, 0.0
+        for r0, r1 in runs:
+            v = np.exp(lv[r0:r1])
+            h = _scott(z[r0:r1], v)
+            assert h > 2 * zmax / 255
+            tot += np.sum(v * (z[r0:r1] ** 2 + h * h))
+            tot_h0 += np.sum(v * z[r0:r1] ** 2)
+        want = math.log(tot / (off[i + 1] - off[i]))
+        assert Lk[0, i] == pytest.approx(want, abs=2e-6)
+        # the h^2 term is what is being pinned: without it the value is off by far more than the tolerance
+        assert abs(math.log(tot_h0 / (off[i + 1] - off[i])) - want) > 1e-3
+
+
+def test_kde_against_continuous_quadrature(theta0):
+    # generic theta (the rate term varies over the grid), one pixel, smooth prior: the 256-node trapezoid of
+    # f(z) p_los(z) R(z) against scipy's adaptive quadrature of the same continuous integrand
+    ev = _kde_event(n=40, seed=9, rows=1)
+    ev = dict(ev, ev_sample_off=np.array([0, 40], dtype=np.int64))
+    zmax, nz = 1.5, 16
+    zb = np.linspace(0, zmax, nz)
+    tab = (0.3 + 2.0 * zb)[None, :]                        # linear: its lerp is the function itself
+    th = theta0.copy()
+    z, lv = O.kde_samples(th, ev, 1, zmax)
+    v = np.exp(lv)
+    h = _scott(z, v)
+    th_arr = O._theta(th)
+    R = lambda x: O.lib().orc_psi(float(x), O._p(th_arr)) / (1 + x)
+    f = lambda x: np.sum(v * np.exp(-0.5 * ((x - z) / h) ** 2)) / (h * math.sqrt(2 * math.pi)) * (0.3 + 2.0 * x) * R(x)
+    I, _ = integrate.quad(f, 0, zmax, points=[z.min(), z.mean(), z.max()], epsabs=0, epsrel=1e-11, limit=400)
+    Lk, npk = O.event_loglik_kde(th, ev, tab, zmax, n_grid=256)
+    assert npk[0, 0] == 1
+    assert Lk[0, 0] == pytest.approx(math.log(I / 40), abs=1e-6)
+    # and it is not the direct sum: the prior's curvature times h^2 shows
+    Ld, _, _ = O.event_loglik(th, ev, tab, zmax)
+    assert abs(Ld[0, 0] - Lk[0, 0]) > 1e-5
+
+
+def test_kde_pixel_rules_and_invariances(theta0):
+    ev = _kde_event(n=120, seed=12, rows=3)
+    zmax, nz = 1.5, 64
+    tab = np.random.default_rng(1).uniform(0.2, 2.0, (5, nz))
+    base, npb = O.event_loglik_kde(theta0, ev, tab, zmax)
+    # a pixel of one sample has no bandwidth: appended to an event it changes S_i only
+    n = ev["dL"].size
+    off = ev["ev_sample_off"]
+    ev2 = dict(ev_sample_off=np.array([off[0], off[1], n + 1], dtype=np.int64), dL=np.append(ev["dL"], ev["dL"][-1]),
+               m1z=np.append(ev["m1z"], ev["m1z"][-1]), m2z=np.append(ev["m2z"], ev["m2z"][-1]),
+               sample_row=np.append(ev["sample_row"], np.int32(4)), log_pe_prior=None)
+    got, npg = O.event_loglik_kde(theta0, ev2, tab, zmax)
+    S1 = n - off[1]
+    assert got[0, 1] == pytest.approx(base[0, 1] - math.log((S1 + 1) / S1), abs=1e-12) and npg[0, 1] == npb[0, 1]
+    # two identical samples: sigma = 0, no bandwidth either
+    ev3 = dict(ev2, ev_sample_off=np.array([off[0], off[1], n + 2], dtype=np.int64), dL=np.append(ev2["dL"], ev["dL"][-1]),
+               m1z=np.append(ev2["m1z"], ev["m1z"][-1]), m2z=np.append(ev2["m2z"], ev["m2z"][-1]),
+               sample_row=np.append(ev2["sample_row"], np.int32(4)))
+    got3, np3 = O.event_loglik_kde(theta0, ev3, tab, zmax)
+    assert got3[0, 1] == pytest.approx(base[0, 1] - math.log((S1 + 2) / S1), abs=1e-12) and np3[0, 1] == npb[0, 1]
+    # the N_eff cut of Eq. 8 on the KDE weights: unreachable threshold leaves nothing, threshold 0 everything
+    assert np.all(np.isneginf(O.event_loglik_kde(theta0, ev, tab, zmax, neff_min=1e9)[0]))
+    # permutation of the samples inside each pixel
+    rng = np.random.default_rng(3)
+    idx = np.concatenate([r0 + rng.permutation(r1 - r0) for runs in _pixel_runs(ev) for r0, r1 in runs])
+    evp = dict(ev, dL=ev["dL"][idx], m1z=ev["m1z"][idx], m2z=ev["m2z"][idx])
+    gotp, _ = O.event_loglik_kde(theta0, evp, tab, zmax)
+    np.testing.assert_allclose(gotp, base, rtol=0, atol=1e-12)
+    # H0 scaling (Om fixed): z unchanged, every v_k gains 3 ln s, bandwidths unchanged
+    s = 1.3
+    th2 = theta0.copy(); th2[0] *= s
+    gots, _ = O.event_loglik_kde(th2, dict(ev, dL=ev["dL"] / s), tab, zmax)
+    np.testing.assert_allclose(gots, base + 3 * math.log(s), rtol=0, atol=1e-11)
