@@ -151,6 +151,23 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
                                    int64_t* d_nlive, int64_t* d_npass);
 
 /*
+ * The event term with the paper's own numerator: a Gaussian kernel density estimate in redshift per sky pixel
+ * (Eq. 5-7; Scott bandwidth Eq. D1; n_grid = 256 fiducial, PAPER.md:213;
+ * DESIGN.md R26-R30).  Pixels as in gwc_event_loglik_pixcut.  For pixel j:
+ *   v_k = p(m1, m2 | theta) / (J pi_PE)  (Eq. 7 without the redshift prior),  n_j = its live samples,
+ *   h_j = 1.06 sigma_j n_j^(-1/5) with sigma_j the v-weighted standard deviation of the z_k,
+ *   I_j = trapezoid over the n_grid-node uniform grid on [0, los->z_max] of
+ *         [sum_k v_k N(z; z_k, h_j)] p_los(z | row_j) psi(z) / (1+z),
+ *   log L_i = log( (1/S_i) sum_j I_j )  over the pixels with n_j >= 2, sigma_j > 0 and N_eff,j >= neff_min.
+ * All arithmetic FP64.  Needs gwc_build_cosmo(d_theta, n_theta) first.  n_grid in [2, 256] else GWC_ERR_SHAPE;
+ * neff_min < 0 or NaN -> GWC_ERR_INVALID_ARG.
+ *   d_logL [n_theta][n_events] f64;  d_npass same shape i64 or NULL (pixels that contributed).
+ */
+gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                                const gwc_los* los, int32_t n_grid, double neff_min, double* d_logL,
+                                int64_t* d_npass);
+
+/*
  * A5.  log xi(theta) = log( (1/n_draw) sum_j w_j ) over found injections with the all-sky prior
  * los->allsky and log_pdraw in place of the PE prior; optional N_eff of the injection sum.
  *   d_logxi [n_theta];  d_neff_inj [n_theta] or NULL.

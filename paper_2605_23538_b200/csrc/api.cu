@@ -406,6 +406,54 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
   return GWC_OK;
 }
 
+gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                                const gwc_los* los, int32_t n_grid, double neff_min, double* d_logL,
+                                int64_t* d_npass) {
+  GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
+  if (!ev || !d_logL) return fail(ctx, GWC_ERR_INVALID_ARG, "ev or d_logL is NULL");
+  if (!(neff_min >= 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "neff_min must be >= 0");
+  if (n_grid < 2 || n_grid > 256) return fail(ctx, GWC_ERR_SHAPE, "n_grid must be in [2, 256]");
+  GWC_TRY(check_los(ctx, los, true, false));
+  if (ev->n_events < 0 || ev->n_samples < 0 || ev->n_events > 0x7fffffffLL)
+    return fail(ctx, GWC_ERR_SHAPE, "event / sample counts out of range");
+  if (ev->n_events == 0) return GWC_OK;
+  if (!ev->ev_sample_off) return fail(ctx, GWC_ERR_INVALID_ARG, "ev->ev_sample_off is NULL");
+  if (ev->n_samples > 0 && (!ev->dL || !ev->m1z || !ev->m2z || !ev->sample_row))
+    return fail(ctx, GWC_ERR_INVALID_ARG, "a sample array is NULL");
+  GWC_TRY(check_built(ctx, d_theta, n_theta, los->z_max));
+  // the per-event reference of the linear-domain sums (and nothing else) comes from the sample preparation
+  cudaStream_t s = ctx->stream;
+  const int64_t n = ev->n_samples, n_seg = ev->n_events;
+  const size_t nd = (size_t)(n > 0 ? n : 1) * sizeof(double);
+  GWC_TRY(ensure(ctx, ctx->dLc, nd));
+  GWC_TRY(ensure(ctx, ctx->L1, nd));
+  GWC_TRY(ensure(ctx, ctx->Q, nd));
+  GWC_TRY(ensure(ctx, ctx->P, nd));
+  GWC_TRY(ensure(ctx, ctx->seg_shift, (size_t)n_seg * sizeof(double)));
+  GWC_TRY(count(ctx, launch_prep_samples(n, n_seg, ev->ev_sample_off, ev->dL, ev->m1z, ev->m2z, ev->log_pe_prior,
+                                         ev->sample_row, los->n_rows, (double*)ctx->dLc.p, (double*)ctx->L1.p,
+                                         (double*)ctx->Q.p, (double*)ctx->P.p, (double*)ctx->seg_shift.p, s),
+                "prep_samples"));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (ctx->timing) {
+    e0 = get_event(ctx);
+    e1 = get_event(ctx);
+    cudaEventRecord(e0, s);
+  }
+  GWC_TRY(count(ctx, launch_kde(d_theta, ctx->tab.p, (const double*)ctx->tconst.p, n_theta, ctx->M, ctx->Mp,
+                                ctx->tab_prec, ctx->z_max / NODE32_QMAX, ev->n_events, ev->ev_sample_off, ev->dL,
+                                ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->seg_shift.p,
+                                los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, d_logL,
+                                d_npass, ctx->n_sm, s),
+                "kde"));
+  if (ctx->timing) {
+    cudaEventRecord(e1, s);
+    ctx->ev_pairs.push_back(e0);
+    ctx->ev_pairs.push_back(e1);
+  }
+  return GWC_OK;
+}
+
 gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_injections* inj,
                                const gwc_los* los, double* d_logxi, double* d_neff_inj) {
   GWC_TRY(check_theta_args(ctx, d_theta, n_theta));

@@ -120,6 +120,11 @@ int launch_combine_total(const double* logL, const double* logxi, int64_t n_thet
 int launch_allsky(const void* table, gwc_prec prec, int64_t n_rows, int n_z, double* scratch, double* allsky,
                   cudaStream_t s);
 size_t allsky_scratch_doubles(int64_t n_rows, int n_z);
+int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp,
+               gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
+               const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
+               const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
+               double* logL, int64_t* npass, int n_sm, cudaStream_t s);
 int launch_probe_fp64(int64_t iters, int n_blocks, double* d_sink, cudaStream_t s, double* n_instr);
 int launch_math_selftest(int which, int64_t n, const double* d_in, double* d_out, cudaStream_t s);
 

@@ -1,0 +1,323 @@
+// kde.cu -- NEXT row 1: the paper's own numerator, a kernel density estimate in redshift per sky
+// pixel (Eq. 5-7; bandwidth Eq. D1; 256-node grid).
+//
+// For pixel j of event i (a maximal run of equal sample_row, R25) and one theta (readings R26-R30):
+//   v_k  = p(m1, m2 | theta) / (J pi_PE)        Eq. 7's weight without the redshift prior
+//   h_j  = 1.06 sigma_j n_j^(-1/5)              sigma_j: v-weighted standard deviation of the z_k, n_j: live samples
+//   f_j(z) = sum_k v_k N(z; z_k, h_j)            Eq. 6
+//   I_j  = trapezoid over the G-node grid on [0, z_max] of f_j(z) p_los(z | row_j) psi(z)/(1+z)
+//   L_i  = (1/S_i) sum_j I_j   over the pixels with n_j >= 2, sigma_j > 0, N_eff,j >= neff_min (Eq. 8)
+//
+// Mapping.  One warp per (theta, event), event-major so that the warps of a CTA share the event's samples in L1.
+// The warp walks the event pixel by pixel.  Per pixel it makes three passes over the pixel's samples, lanes =
+// samples: moments (sum v, sum v z, sum v^2, n), centred second moment, and the KDE itself, for which the lanes
+// turn into grid nodes (node g = lane + 32 i, i < 8): the (z_k, v_k) of 32 samples at a time are handed round by
+// shuffles and every lane adds v_k N(z_g; z_k, h) into its 8 node sums.  The prior p_los R c_g at the lane's nodes is
+// then applied once per pixel.  Everything is FP64; the Gaussian uses math64.cuh's 7-instruction exp (the hot
+// instruction: G exponentials per (theta, sample)), the per-sample weight plain libdevice functions.  All sums run in
+// a fixed order (samples in order inside a lane, butterfly across lanes, pixels in order): bitwise reproducible.
+#include <math_constants.h>
+
+#include "gwc_internal.h"
+#include "math64.cuh"
+
+namespace gwc {
+
+namespace {
+
+constexpr int KDE_THREADS = 256;
+constexpr int KDE_WARPS = KDE_THREADS / 32;
+constexpr int KDE_NPL = 8;            // grid nodes per lane: G <= 256
+constexpr double C_KMS_KDE = 299792.458;
+
+struct KdeParams {
+  const double* theta;      // [n_theta][12]
+  const void* tab;          // [n_theta][Mp] Node64 | Node32
+  const double* tconst;     // [n_theta][NCONST] (umax, 1/du, validity)
+  int64_t n_theta, n_events;
+  int M, Mp;
+  double tab_zq;
+  const int64_t* ev_off;    // [n_events+1]
+  const double *dL, *m1z, *m2z, *lprior;   // lprior may be NULL (2 ln d_L)
+  const int32_t* row;
+  const double* seg_shift;  // [n_events] reference of the linear-domain sums (prep_kernel)
+  const void* los;          // [n_rows][n_z]
+  int64_t n_rows;
+  int n_z;
+  double los_zmax;
+  int n_grid;
+  double neff_min;
+  double* logL;             // [n_theta][n_events]
+  int64_t* npass;           // [n_theta][n_events] or NULL
+};
+
+__device__ __forceinline__ double wsum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// per-theta values a warp keeps while it walks an event
+struct ThetaK {
+  double h0c, umax, invdu, mmin, mmax, alpha, beta, mu, sigma;
+  double a_pl, a_g;      // (1 - lambda) n_pl  and  lambda n_g / (sigma sqrt(2 pi))
+  double bp1, mminb;     // beta + 1, mmin^(beta+1)
+  double Om, OL, cH;     // c / H0
+};
+
+__device__ __forceinline__ void node_pair(const Node64* t, int m, double& z0, double& d0, double& z1, double& d1,
+                                          double) {
+  z0 = t[m].z; d0 = t[m].d; z1 = t[m + 1].z; d1 = t[m + 1].d;
+}
+__device__ __forceinline__ void node_pair(const Node32* t, int m, double& z0, double& d0, double& z1, double& d1,
+                                          double zq) {
+  z0 = (double)t[m].zq * zq; d0 = (double)t[m].d * zq; z1 = (double)t[m + 1].zq * zq; d1 = (double)t[m + 1].d * zq;
+}
+
+// z_k and ln v_k of one sample (-inf when dead): DESIGN.md section 3 without p_los and the rate term
+template <typename NodeT>
+__device__ __forceinline__ double sample_lv(const ThetaK& K, const NodeT* tab, int M, double zq, double dL, double m1z,
+                                            double m2z, double lpi, int32_t row, int64_t n_rows, double los_zmax,
+                                            double& z_out) {
+  z_out = 0.0;
+  const double NEG = -CUDART_INF;
+  if (!(isfinite(dL) && isfinite(m1z) && isfinite(m2z) && isfinite(lpi))) return NEG;
+  if (!(dL > 0.0 && m1z > 0.0 && m2z > 0.0)) return NEG;
+  if (row < 0 || (int64_t)row >= n_rows) return NEG;
+  const double u = dL * K.h0c;
+  if (!(u < K.umax)) return NEG;
+  const double t = u * K.invdu;
+  int m = (int)floor(t);
+  m = m > M - 2 ? M - 2 : m;
+  const double f = t - (double)m;
+  double z0, d0, z1, d1;
+  node_pair(tab, m, z0, d0, z1, d1, zq);
+  const double dl = z1 - z0, sd = d0 + d1;
+  const double c3 = fma(-2.0, dl, sd), c2 = fma(3.0, dl, -(sd + d0));
+  const double z = fma(f, fma(f, fma(f, c3, c2), d0), z0);
+  if (!(z < los_zmax)) return NEG;
+  const double x = 1.0 + z;
+  const double m1 = m1z / x, m2 = m2z / x;
+  if (!(m1 > K.mmin && m1 <= K.mmax && m2 >= K.mmin && m2z <= m1z)) return NEG;
+  const double y = (m1 - K.mu) / K.sigma;
+  const double p1 = K.a_pl * pow(m1, -K.alpha) + K.a_g * exp(-0.5 * y * y);
+  const double p2 = K.bp1 * pow(m2 <= m1 ? m2 : m1, K.beta) / (pow(m1, K.bp1) - K.mminb);
+  if (!(p1 > 0.0) || !(p2 > 0.0)) return NEG;
+  const double E = sqrt(fma(K.Om * x * x, x, K.OL));
+  const double J = x * x * K.cH * (u / x + x / E);
+  z_out = z;
+  return log(p1) + log(p2) - log(J) - lpi;
+}
+
+template <typename NodeT, typename LosT>
+__global__ void __launch_bounds__(KDE_THREADS) kde_kernel(const KdeParams p) {
+  extern __shared__ __align__(16) unsigned char kde_smem[];
+  MathTables& mt = *reinterpret_cast<MathTables*>(kde_smem);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  init_math_tables(mt, tid, KDE_THREADS);
+  __syncthreads();
+  const double* exptab = mt.exptab + (lane & (EXP_REP - 1));
+  const unsigned FULL = 0xffffffffu;
+  const int G = p.n_grid;
+  const double dzg = p.los_zmax / (G - 1);
+  const double dzl = p.los_zmax / (p.n_z - 1);
+  const int64_t n_units = p.n_theta * p.n_events;
+
+  for (int64_t unit = (int64_t)blockIdx.x * KDE_WARPS + warp; unit < n_units; unit += (int64_t)gridDim.x * KDE_WARPS) {
+    const int64_t ev = unit / p.n_theta, t = unit - ev * p.n_theta;   // event-major
+    const int64_t s0 = p.ev_off[ev], s1 = p.ev_off[ev + 1];
+    const size_t o = (size_t)t * (size_t)p.n_events + (size_t)ev;
+    const double* th = p.theta + t * GWC_NPAR;
+    if (!(p.tconst[t * NCONST + C_VALID] == 1.0)) {   // theta outside the domain: NaN (sticky flag set by build_cosmo)
+      if (lane == 0) {
+        p.logL[o] = CUDART_NAN;
+        if (p.npass) p.npass[o] = 0;
+      }
+      continue;
+    }
+    // ---- per-theta values (every lane computes them: no divergence, no broadcast) ----
+    ThetaK K;
+    {
+      const double H0 = th[0], alpha = th[2], beta = th[3], mmin = th[4], mmax = th[5], mu = th[6], sigma = th[7],
+                   lam = th[8];
+      K.h0c = H0 / C_KMS_KDE;
+      K.cH = C_KMS_KDE / H0;
+      K.umax = p.tconst[t * NCONST + C_UMAX];
+      K.invdu = p.tconst[t * NCONST + C_INVDU];
+      K.mmin = mmin; K.mmax = mmax; K.alpha = alpha; K.beta = beta; K.mu = mu; K.sigma = sigma;
+      const double n_pl = (1.0 - alpha) / (pow(mmax, 1.0 - alpha) - pow(mmin, 1.0 - alpha));
+      const double rs2 = 1.0 / (sigma * 1.41421356237309504880);
+      const double n_g = 1.0 / (0.5 * (erf((mmax - mu) * rs2) - erf((mmin - mu) * rs2)));
+      K.a_pl = (1.0 - lam) * n_pl;
+      K.a_g = lam * n_g / (sigma * 2.50662827463100050242);
+      K.bp1 = beta + 1.0;
+      K.mminb = pow(mmin, beta + 1.0);
+      K.Om = th[1];
+      K.OL = 1.0 - th[1];
+    }
+    // rate term times the trapezoid weight at this lane's grid nodes: c_g psi(z_g) / (1 + z_g)   (reading R4)
+    double rg[KDE_NPL];
+    {
+      const double gam = th[9], kap = th[10], zp = th[11];
+      const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
+#pragma unroll
+      for (int i = 0; i < KDE_NPL; ++i) {
+        const int g = lane + 32 * i;
+        const double x = 1.0 + g * dzg;
+        const double psi = psi0 * pow(x, gam) / (1.0 + pow(x / (1.0 + zp), gam + kap));
+        const double c = (g == 0 || g == G - 1) ? 0.5 * dzg : dzg;
+        rg[i] = g < G ? c * psi / x : 0.0;
+      }
+    }
+    const NodeT* tab = reinterpret_cast<const NodeT*>(p.tab) + (size_t)t * p.Mp;
+    const double shift = p.seg_shift[ev];
+    double esum = 0.0;   // sum over the passing pixels of I_j, relative to e^shift
+    int np = 0;
+
+    int64_t r0 = s0;
+    while (r0 < s1) {
+      // ---- the pixel: samples r0 .. r1-1 with the row of r0 ----
+      const int32_t prow = p.row[r0];
+      int64_t r1 = r0 + 1;
+      for (;;) {
+        const int64_t g = r1 + lane;
+        const unsigned stop = __ballot_sync(FULL, g >= s1 || p.row[g < s1 ? g : s1 - 1] != prow);
+        if (stop) { r1 += __ffs(stop) - 1; break; }
+        r1 += 32;
+      }
+      // ---- pass 1: sum v, sum v z, sum v^2, live count ----
+      double V = 0.0, Vz = 0.0, Q = 0.0;
+      int n = 0;
+      for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+        const int64_t k = c0 + lane;
+        double z = 0.0, v = 0.0;
+        if (k < r1) {
+          const double d = p.dL[k];
+          const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
+          const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
+          v = lv > -CUDART_INF ? exp(lv - shift) : 0.0;
+          n += lv > -CUDART_INF ? 1 : 0;
+        }
+        V += v;
+        Vz = fma(v, z, Vz);
+        Q = fma(v, v, Q);
+      }
+      V = wsum(V); Vz = wsum(Vz); Q = wsum(Q);
+      n = __reduce_add_sync(FULL, n);
+      bool pass = n >= 2 && V > 0.0 && V * V >= p.neff_min * Q;   // warp-uniform
+      double h = 0.0;
+      if (pass) {
+        // ---- pass 2: centred second moment ----
+        const double mu = Vz / V;
+        double S2 = 0.0;
+        for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+          const int64_t k = c0 + lane;
+          if (k < r1) {
+            double z;
+            const double d = p.dL[k];
+            const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
+            const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
+            const double v = lv > -CUDART_INF ? exp(lv - shift) : 0.0;
+            S2 = fma(v * (z - mu), z - mu, S2);
+          }
+        }
+        S2 = wsum(S2);
+        const double var = S2 / V;
+        pass = var > 0.0;
+        h = 1.06 * sqrt(var) * pow((double)n, -0.2);   // Eq. D1
+      }
+      if (pass) {
+        // ---- pass 3: the KDE on the grid; lanes are grid nodes, samples handed round 32 at a time ----
+        const double invh = 1.0 / h;
+        const double norm = invh * 0.39894228040143267794;   // 1 / (h sqrt(2 pi))
+        const double sinvh = invh * 0.70710678118654752440;  // so that the exponent is -(q')^2
+        double acc[KDE_NPL];
+#pragma unroll
+        for (int i = 0; i < KDE_NPL; ++i) acc[i] = 0.0;
+        for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+          const int64_t k = c0 + lane;
+          double zs = 0.0, a = 0.0;   // z_k / (h sqrt 2), v_k / (h sqrt(2 pi))
+          if (k < r1) {
+            double z;
+            const double d = p.dL[k];
+            const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
+            const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
+            a = lv > -CUDART_INF ? exp(lv - shift) * norm : 0.0;
+            zs = z * sinvh;
+          }
+          const int cnt = (int)min((int64_t)32, r1 - c0);
+          for (int j = 0; j < cnt; ++j) {
+            const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
+#pragma unroll
+            for (int i = 0; i < KDE_NPL; ++i) {
+              const double q = fma((double)(lane + 32 * i), dzg * sinvh, -zj);
+              acc[i] = fma(aj, exp_fast<true>(-q * q, exptab), acc[i]);
+            }
+          }
+        }
+        // ---- prior at the lane's nodes: p_los(z_g | row) by the table's linear interpolation, times c_g R(z_g) ----
+        const LosT* lrow = reinterpret_cast<const LosT*>(p.los) + (size_t)prow * (size_t)p.n_z;
+        double part = 0.0;
+#pragma unroll
+        for (int i = 0; i < KDE_NPL; ++i) {
+          const int g = lane + 32 * i;
+          if (g < G) {
+            const double zg = fmin(g * dzg, p.los_zmax);
+            const double tz = zg / dzl;
+            int b = (int)floor(tz);
+            b = b > p.n_z - 2 ? p.n_z - 2 : b;
+            const double fz = tz - (double)b;
+            const double q0 = (double)lrow[b], q1 = (double)lrow[b + 1];
+            part = fma(acc[i], (q0 + fz * (q1 - q0)) * rg[i], part);
+          }
+        }
+        const double I = wsum(part);
+        if (I > 0.0) {
+          esum += I;
+          ++np;
+        }
+      }
+      r0 = r1;
+    }
+    if (lane == 0) {
+      p.logL[o] = (s1 > s0 && esum > 0.0) ? shift + log(esum) - log((double)(s1 - s0)) : -CUDART_INF;
+      if (p.npass) p.npass[o] = np;
+    }
+  }
+}
+
+}  // namespace
+
+int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp,
+               gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
+               const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
+               const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
+               double* logL, int64_t* npass, int n_sm, cudaStream_t s) {
+  if (n_theta <= 0 || n_events <= 0) return 0;
+  KdeParams p;
+  p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.n_theta = n_theta; p.n_events = n_events;
+  p.M = M; p.Mp = Mp; p.tab_zq = tab_zq; p.ev_off = ev_off; p.dL = dL; p.m1z = m1z; p.m2z = m2z; p.lprior = lprior;
+  p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
+  p.n_grid = n_grid; p.neff_min = neff_min; p.logL = logL; p.npass = npass;
+  const size_t smem = sizeof(MathTables);
+  const int64_t units = n_theta * n_events;
+  int64_t blocks = (units + KDE_WARPS - 1) / KDE_WARPS;
+  const int64_t cap = (int64_t)n_sm * 8;   // up to 8 CTAs of 256 threads per SM, the rest by the grid-stride loop
+  if (blocks > cap) blocks = cap;
+#define GWC_KDE_LAUNCH(NodeT, LosT)                                                                              \
+  do {                                                                                                           \
+    if (cudaFuncSetAttribute(kde_kernel<NodeT, LosT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != \
+        cudaSuccess)                                                                                             \
+      return -1;                                                                                                 \
+    kde_kernel<NodeT, LosT><<<(unsigned)blocks, KDE_THREADS, smem, s>>>(p);                                      \
+  } while (0)
+  if (tab_prec == GWC_F64) {
+    if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node64, double); else GWC_KDE_LAUNCH(Node64, float);
+  } else {
+    if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node32, double); else GWC_KDE_LAUNCH(Node32, float);
+  }
+#undef GWC_KDE_LAUNCH
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace gwc

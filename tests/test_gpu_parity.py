@@ -368,3 +368,80 @@ def test_pixcut_edge_cases_and_32bit_tables(ctx):
             assert np.array_equal(np.isneginf(gq[0][same]), np.isneginf(o[0][same]))
             assert (np.abs(gq[0][fin] - o[0][fin]) / np.maximum(np.abs(o[0][fin]), 1.0)).max() <= 1e-6
     assert np.all(np.isneginf(gq[0][:, 2])) and np.all(gq[3][:, 2] == 0)
+
+
+# ---- NEXT row 1: the paper's KDE numerator (Eq. 5-7, D1; R26-R30) -------------------------------------
+def _kde_both(ctx, W, theta, ev=None, los=None, n_grid=256, neff_min=0.0, prec=0):
+    ev = W.ev if ev is None else ev
+    los = W.los if los is None else los
+    zmax = W.spec.z_max
+    th = theta.to(DEV)
+    ctx.gwc_build_cosmo(th, zmax, 1025, prec)
+    gL, gP = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), los.to(DEV), zmax, n_grid, neff_min)
+    ctx.gwc_check()
+    oL, oP = oracle.event_loglik_kde(_np(theta), synth.to_numpy(ev), _np(los), zmax, n_grid=n_grid, neff_min=neff_min,
+                                     table_prec=prec)
+    return (_np(gL), _np(gP)), (oL, oP)
+
+
+def _kde_compare(g, o, what, rtol=RTOL_F64):
+    bad = np.argwhere(g[1] != o[1])
+    assert bad.size == 0, "%s: npass differs at %s" % (what, bad[:8].tolist())
+    return assert_close_log(g[0], o[0], rtol, what + " log L_i (KDE)")
+
+
+@pytest.mark.parametrize("n_grid,neff_min", [(256, 0.0), (256, 2.0), (100, 0.0), (33, 3.0)])
+def test_kde_tiny(ctx, n_grid, neff_min):
+    W = workload("tiny")
+    g, o = _kde_both(ctx, W, W.theta, n_grid=n_grid, neff_min=neff_min)
+    worst = _kde_compare(g, o, "tiny G=%d nmin=%g" % (n_grid, neff_min))
+    assert np.isfinite(o[0]).any() and (o[1] > 0).any()
+    print("KDE tiny G=%d: max rel err %.2e" % (n_grid, worst))
+
+
+def test_kde_ragged_catalogue(ctx):
+    """O4-like: ragged events, pixels of 1 sample (no bandwidth) to hundreds, f32 and f64 LOS rows."""
+    W = workload("o4", n_theta=16, n_events=10, los_rows=500, n_inj=500)
+    for los in (W.los, W.los.to(torch.float32)):
+        g, o = _kde_both(ctx, W, W.theta, los=los, neff_min=2.0)
+        _kde_compare(g, o, "o4-like %s" % los.dtype)
+    assert (o[1] > 1).any()
+
+
+def test_kde_edge_cases(ctx):
+    from paper_2605_23538_b200 import gwc
+    W = workload("o4", n_theta=10, n_events=6, los_rows=120, n_inj=500)
+    ev = {k: (v.clone() if isinstance(v, torch.Tensor) else v) for k, v in W.ev.items()}
+    off = ev["ev_sample_off"].clone()
+    off[2] = off[3]                               # an empty event
+    ev["ev_sample_off"] = off
+    ev["dL"][5] = float("nan")
+    ev["dL"][17] = -2.0
+    ev["sample_row"][40:44] = 10_000              # invalid rows: a pixel of dead samples
+    ev["m2z"][80] = ev["m1z"][80] * 2.0
+    a, b = int(off[4]), int(off[5])
+    ev["dL"][a:b] = 1e9                           # an event entirely beyond the table
+    ev["dL"][int(off[0]) + 100:int(off[0]) + 103] = ev["dL"][int(off[0]) + 100]   # (nearly) repeated samples
+    theta = W.theta.clone()
+    theta[3, 8] = 0.0                             # lambda = 0
+    theta[4, 7] = -1.0                            # invalid sigma: NaN row + GWC_ERR_DOMAIN
+    zmax = W.spec.z_max
+    th = theta.to(DEV)
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    gL, gP = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), W.los.to(DEV), zmax, 256, 0.0)
+    with pytest.raises(gwc.GwcError):
+        ctx.gwc_check()
+    oL, oP = oracle.event_loglik_kde(_np(theta), synth.to_numpy(ev), _np(W.los), zmax)
+    _kde_compare((_np(gL), _np(gP)), (oL, oP), "edge cases")
+    assert np.all(np.isnan(oL[4])) and np.all(np.isneginf(oL[[0, 1, 2, 3, 5]][:, 2])) and np.all(np.isneginf(oL[0, 4]))
+    for bad in (1, 257):
+        with pytest.raises(gwc.GwcError):
+            ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), W.los.to(DEV), zmax, bad, 0.0)
+    # determinism
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    g2 = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), W.los.to(DEV), zmax, 256, 0.0)
+    try:
+        ctx.gwc_check()
+    except gwc.GwcError:
+        pass
+    assert torch.equal(torch.nan_to_num(g2[0], nan=7.0), torch.nan_to_num(gL, nan=7.0)) and torch.equal(g2[1], gP)
