@@ -39,7 +39,7 @@ struct gwc_ctx {
   gwc_prec tab_prec = GWC_F64;
   double z_max = 0.0;
   // per-call scratch
-  Buf dLc, L1, Q, P, seg_off, seg_shift, group_off, part_w, part_n, part_np, allsky_scr, pack_scr, logL, logxi, probe;
+  Buf dLc, L1, Q, P, seg_off, seg_shift, group_off, part_w, part_n, part_np, kde_scr, kde_len, allsky_scr, pack_scr, logL, logxi, probe;
   HostCopy hc;
   // timing
   bool timing = false;
@@ -263,7 +263,7 @@ void gwc_destroy(gwc_ctx* ctx) {
   cudaSetDevice(ctx->device);
   cudaStreamSynchronize(ctx->stream);
   Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->dLc, &ctx->L1, &ctx->Q, &ctx->P, &ctx->seg_off, &ctx->seg_shift,
-                 &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
+                 &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->kde_scr, &ctx->kde_len, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
                  &ctx->logxi, &ctx->probe, &ctx->hc.theta, &ctx->hc.ev_off, &ctx->hc.ev_dL, &ctx->hc.ev_m1z,
                  &ctx->hc.ev_m2z, &ctx->hc.ev_lp, &ctx->hc.ev_row, &ctx->hc.inj_dL, &ctx->hc.inj_m1z,
                  &ctx->hc.inj_m2z, &ctx->hc.inj_lp, &ctx->hc.los, &ctx->hc.allsky, &ctx->hc.out};
@@ -440,11 +440,20 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
     e1 = get_event(ctx);
     cudaEventRecord(e0, s);
   }
+  // scratch of the kernel: one slice of (z, v) pairs per resident warp, as long as the longest event
+  GWC_TRY(ensure(ctx, ctx->kde_len, sizeof(int64_t)));
+  GWC_TRY(count(ctx, launch_max_segment(ev->ev_sample_off, ev->n_events, (int64_t*)ctx->kde_len.p, s), "max_segment"));
+  int64_t max_len = 0;
+  GWC_CUDA(cudaMemcpyAsync(&max_len, ctx->kde_len.p, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+  GWC_CUDA(cudaStreamSynchronize(s));
+  if (max_len < 0 || max_len > ev->n_samples) return fail(ctx, GWC_ERR_SHAPE, "ev_sample_off is not ascending");
+  const int n_blocks = kde_grid_blocks(n_theta, ev->n_events, ctx->n_sm);
+  GWC_TRY(ensure(ctx, ctx->kde_scr, kde_scratch_bytes(n_blocks, max_len)));
   GWC_TRY(count(ctx, launch_kde(d_theta, ctx->tab.p, (const double*)ctx->tconst.p, n_theta, ctx->M, ctx->Mp,
                                 ctx->tab_prec, ctx->z_max / NODE32_QMAX, ev->n_events, ev->ev_sample_off, ev->dL,
                                 ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->seg_shift.p,
                                 los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, d_logL,
-                                d_npass, ctx->n_sm, s),
+                                d_npass, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, s),
                 "kde"));
   if (ctx->timing) {
     cudaEventRecord(e1, s);

@@ -9,9 +9,10 @@
 //   L_i  = (1/S_i) sum_j I_j   over the pixels with n_j >= 2, sigma_j > 0, N_eff,j >= neff_min (Eq. 8)
 //
 // Mapping.  One warp per (theta, event), event-major so that the warps of a CTA share the event's samples in L1.
-// The warp walks the event pixel by pixel.  Per pixel it makes three passes over the pixel's samples, lanes =
-// samples: moments (sum v, sum v z, sum v^2, n), centred second moment, and the KDE itself, for which the lanes
-// turn into grid nodes (node g = lane + 32 i, i < 8): the (z_k, v_k) of 32 samples at a time are handed round by
+// The warp first computes (z_k, v_k) of the whole event, 32 samples at a time with every lane busy, into its slice
+// of a scratch buffer (L1/L2-resident), then walks the event pixel by pixel.  Per pixel it makes three passes over
+// the stored pairs, lanes = samples: moments (sum v, sum v z, sum v^2, n), centred second moment, and the KDE itself,
+// for which the lanes turn into grid nodes (node g = lane + 32 i, i < 8): the (z_k, v_k) of 32 samples at a time are handed round by
 // shuffles and every lane adds v_k N(z_g; z_k, h) into its 8 node sums.  The prior p_los R c_g at the lane's nodes is
 // then applied once per pixel.  Everything is FP64; the Gaussian uses math64.cuh's 7-instruction exp (the hot
 // instruction: G exponentials per (theta, sample)), the per-sample weight plain libdevice functions.  All sums run in
@@ -47,6 +48,8 @@ struct KdeParams {
   double los_zmax;
   int n_grid;
   double neff_min;
+  double2* scr;             // [resident warps][scr_stride]: (z_k, v_k) of the event a warp is working on (v < 0: dead)
+  int64_t scr_stride;       // >= the longest event
   double* logL;             // [n_theta][n_events]
   int64_t* npass;           // [n_theta][n_events] or NULL
 };
@@ -110,7 +113,7 @@ __device__ __forceinline__ double sample_lv(const ThetaK& K, const NodeT* tab, i
 }
 
 template <typename NodeT, typename LosT>
-__global__ void __launch_bounds__(KDE_THREADS) kde_kernel(const KdeParams p) {
+__global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) {
   extern __shared__ __align__(16) unsigned char kde_smem[];
   MathTables& mt = *reinterpret_cast<MathTables*>(kde_smem);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -171,6 +174,19 @@ __global__ void __launch_bounds__(KDE_THREADS) kde_kernel(const KdeParams p) {
     }
     const NodeT* tab = reinterpret_cast<const NodeT*>(p.tab) + (size_t)t * p.Mp;
     const double shift = p.seg_shift[ev];
+    // ---- (z_k, v_k) of every sample of the event, relative to e^shift ----
+    double2* scr = p.scr + ((size_t)blockIdx.x * KDE_WARPS + warp) * (size_t)p.scr_stride - s0;   // indexed by sample
+    for (int64_t c0 = s0; c0 < s1; c0 += 32) {
+      const int64_t k = c0 + lane;
+      if (k < s1) {
+        double z;
+        const double d = p.dL[k];
+        const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
+        const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
+        scr[k] = make_double2(z, lv > -CUDART_INF ? exp(lv - shift) : -1.0);
+      }
+    }
+    __syncwarp();
     double esum = 0.0;   // sum over the passing pixels of I_j, relative to e^shift
     int np = 0;
 
@@ -192,11 +208,10 @@ __global__ void __launch_bounds__(KDE_THREADS) kde_kernel(const KdeParams p) {
         const int64_t k = c0 + lane;
         double z = 0.0, v = 0.0;
         if (k < r1) {
-          const double d = p.dL[k];
-          const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
-          const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
-          v = lv > -CUDART_INF ? exp(lv - shift) : 0.0;
-          n += lv > -CUDART_INF ? 1 : 0;
+          const double2 zv = scr[k];
+          z = zv.x;
+          v = zv.y >= 0.0 ? zv.y : 0.0;
+          n += zv.y >= 0.0 ? 1 : 0;
         }
         V += v;
         Vz = fma(v, z, Vz);
@@ -213,12 +228,9 @@ __global__ void __launch_bounds__(KDE_THREADS) kde_kernel(const KdeParams p) {
         for (int64_t c0 = r0; c0 < r1; c0 += 32) {
           const int64_t k = c0 + lane;
           if (k < r1) {
-            double z;
-            const double d = p.dL[k];
-            const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
-            const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
-            const double v = lv > -CUDART_INF ? exp(lv - shift) : 0.0;
-            S2 = fma(v * (z - mu), z - mu, S2);
+            const double2 zv = scr[k];
+            const double v = zv.y >= 0.0 ? zv.y : 0.0;
+            S2 = fma(v * (zv.x - mu), zv.x - mu, S2);
           }
         }
         S2 = wsum(S2);
@@ -238,12 +250,9 @@ __global__ void __launch_bounds__(KDE_THREADS) kde_kernel(const KdeParams p) {
           const int64_t k = c0 + lane;
           double zs = 0.0, a = 0.0;   // z_k / (h sqrt 2), v_k / (h sqrt(2 pi))
           if (k < r1) {
-            double z;
-            const double d = p.dL[k];
-            const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
-            const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
-            a = lv > -CUDART_INF ? exp(lv - shift) * norm : 0.0;
-            zs = z * sinvh;
+            const double2 zv = scr[k];
+            a = zv.y >= 0.0 ? zv.y * norm : 0.0;
+            zs = zv.x * sinvh;
           }
           const int cnt = (int)min((int64_t)32, r1 - c0);
           for (int j = 0; j < cnt; ++j) {
@@ -283,6 +292,7 @@ __global__ void __launch_bounds__(KDE_THREADS) kde_kernel(const KdeParams p) {
       p.logL[o] = (s1 > s0 && esum > 0.0) ? shift + log(esum) - log((double)(s1 - s0)) : -CUDART_INF;
       if (p.npass) p.npass[o] = np;
     }
+    __syncwarp();   // the scratch slice is rewritten by the next unit
   }
 }
 
@@ -292,18 +302,16 @@ int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
-               double* logL, int64_t* npass, int n_sm, cudaStream_t s) {
+               double* logL, int64_t* npass, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
   if (n_theta <= 0 || n_events <= 0) return 0;
   KdeParams p;
   p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.n_theta = n_theta; p.n_events = n_events;
   p.M = M; p.Mp = Mp; p.tab_zq = tab_zq; p.ev_off = ev_off; p.dL = dL; p.m1z = m1z; p.m2z = m2z; p.lprior = lprior;
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
   p.n_grid = n_grid; p.neff_min = neff_min; p.logL = logL; p.npass = npass;
+  p.scr = (double2*)scratch; p.scr_stride = scr_stride;
   const size_t smem = sizeof(MathTables);
-  const int64_t units = n_theta * n_events;
-  int64_t blocks = (units + KDE_WARPS - 1) / KDE_WARPS;
-  const int64_t cap = (int64_t)n_sm * 8;   // up to 8 CTAs of 256 threads per SM, the rest by the grid-stride loop
-  if (blocks > cap) blocks = cap;
+  const int64_t blocks = n_blocks;
 #define GWC_KDE_LAUNCH(NodeT, LosT)                                                                              \
   do {                                                                                                           \
     if (cudaFuncSetAttribute(kde_kernel<NodeT, LosT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != \
@@ -318,6 +326,18 @@ int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst,
   }
 #undef GWC_KDE_LAUNCH
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+// grid of the KDE kernel (persistent, two CTAs of 8 warps per SM) and the scratch it needs: one slice of
+// `max_event_len` (z, v) pairs per resident warp
+int kde_grid_blocks(int64_t n_theta, int64_t n_events, int n_sm) {
+  const int64_t units = n_theta * n_events;
+  int64_t blocks = (units + KDE_WARPS - 1) / KDE_WARPS;
+  if (blocks > (int64_t)n_sm * 2) blocks = (int64_t)n_sm * 2;
+  return (int)(blocks < 1 ? 1 : blocks);
+}
+size_t kde_scratch_bytes(int n_blocks, int64_t max_event_len) {
+  return (size_t)n_blocks * KDE_WARPS * (size_t)(max_event_len > 0 ? max_event_len : 1) * sizeof(double2);
 }
 
 }  // namespace gwc

@@ -84,6 +84,16 @@ __global__ void uniform_segments_kernel(int64_t n, int64_t seg, int64_t n_seg, i
   seg_off[i] = v < n ? v : n;
 }
 
+// longest segment (single block; d_out must hold 0 before the launch)
+__global__ void max_segment_kernel(const int64_t* __restrict__ seg_off, int64_t n_seg, int64_t* __restrict__ d_out) {
+  long long m = 0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_seg; i += (int64_t)gridDim.x * blockDim.x) {
+    const long long l = seg_off[i + 1] - seg_off[i];
+    m = l > m ? l : m;
+  }
+  atomicMax(reinterpret_cast<long long*>(d_out), m);
+}
+
 __global__ void finalize_events_kernel(const double* __restrict__ part_w, const int32_t* __restrict__ part_n,
                                        const int64_t* __restrict__ seg_off, const double* __restrict__ seg_shift,
                                        const double* __restrict__ tconst, int64_t n_theta, int64_t n_events,
@@ -253,6 +263,15 @@ int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const 
 int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
                        cudaStream_t s) {
   make_groups_kernel<<<(n_groups + 1 + 127) / 128, 128, 0, s>>>(seg_off, n_seg, target, n_groups, group_off);
+  return ok();
+}
+
+int launch_max_segment(const int64_t* seg_off, int64_t n_seg, int64_t* d_out, cudaStream_t s) {
+  if (cudaMemsetAsync(d_out, 0, sizeof(int64_t), s) != cudaSuccess) return -1;
+  if (n_seg <= 0) return 0;
+  int64_t blocks = (n_seg + 255) / 256;
+  if (blocks > 1024) blocks = 1024;
+  max_segment_kernel<<<(unsigned)blocks, 256, 0, s>>>(seg_off, n_seg, d_out);
   return ok();
 }
 
