@@ -252,6 +252,30 @@ def run_gwc(args):
         pix = {"neff_min": args.pixcut, "event_kernel_ms": ms_pix, "event_terms_per_s": terms_ev / (ms_pix * 1e-3),
                "slowdown_vs_uncut": ms_pix / ms_ev_kernel, "mean_passing_pixels_per_event": float(npass.double().mean())}
         del npass
+    # ---- NEXT row 1, reported beside the headline: the event term with the paper's KDE numerator (Eq. 5-7) on a
+    # bounded slice of the theta batch (it needs 256 Gaussian evaluations per (theta, sample) instead of one term) ----
+    kde = None
+    if args.kde_theta > 0:
+        th_k = theta[:min(args.kde_theta, n_theta)].contiguous()
+        ctx.gwc_build_cosmo(th_k, zmax, args.n_nodes, prec)
+        ctx.gwc_event_loglik_kde(th_k, W.ev, W.los, zmax, 256, 2.0)
+        torch.cuda.synchronize()
+        ctx.gwc_set_timing(True)
+        ctx.gwc_get_timing()
+        nused = None
+        for _ in range(2):
+            _, _, nused = ctx.gwc_event_loglik_kde(th_k, W.ev, W.los, zmax, 256, 2.0)
+        torch.cuda.synchronize()
+        tk = ctx.gwc_get_timing()
+        ctx.gwc_set_timing(False)
+        ms_kde = tk["ms_ev"] / max(tk["n_ev"], 1)
+        evals = float(nused.sum().item()) * 256.0
+        # 10 FP64 instructions per Gaussian evaluation (offset, square, 7-instruction exp, accumulate): DESIGN.md 11
+        kde = {"n_theta": int(th_k.shape[0]), "n_grid": 256, "neff_min": 2.0, "kernel_ms": ms_kde,
+               "event_terms_per_s": th_k.shape[0] * n_samples / (ms_kde * 1e-3),
+               "gaussian_evals_per_s": evals / (ms_kde * 1e-3),
+               "roofline_frac_fp64": evals * 10.0 / (ms_kde * 1e-3) / FP64_PEAK_INSTR}
+        del nused
     cpu = cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
     stress = stress_report(ctx, W, theta, zmax, allsky, args.n_nodes) if spec.name == "stress" else None
     line = {
@@ -279,6 +303,8 @@ def run_gwc(args):
         line["stress_report"] = stress
     if pix is not None:
         line["pixcut"] = pix
+    if kde is not None:
+        line["kde"] = kde
     print(json.dumps(line))
     if dist:
         td.destroy_process_group()
@@ -399,6 +425,8 @@ def main():
     ap.add_argument("--seed", type=int, default=synth.DEFAULT_SEED)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle timing budget (0 = skip)")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--kde-theta", type=int, default=16,
+                    help="also time the KDE-numerator event term on this many theta points (0: skip)")
     ap.add_argument("--pixcut", type=float, default=2.0,
                     help="also time the event term with the per-pixel N_eff cut at this threshold (< 0: skip)")
     args = ap.parse_args()

@@ -161,11 +161,13 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
  *   log L_i = log( (1/S_i) sum_j I_j )  over the pixels with n_j >= 2, sigma_j > 0 and N_eff,j >= neff_min.
  * All arithmetic FP64.  Needs gwc_build_cosmo(d_theta, n_theta) first.  n_grid in [2, 256] else GWC_ERR_SHAPE;
  * neff_min < 0 or NaN -> GWC_ERR_INVALID_ARG.
- *   d_logL [n_theta][n_events] f64;  d_npass same shape i64 or NULL (pixels that contributed).
+ *   d_logL [n_theta][n_events] f64;  d_npass, d_nused same shape i64 or NULL (pixels that contributed, and their
+ *   live samples: n_grid * d_nused Gaussian evaluations were needed).
+ * Synchronises the stream once (the longest event sizes a scratch buffer).
  */
 gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                                 const gwc_los* los, int32_t n_grid, double neff_min, double* d_logL,
-                                int64_t* d_npass);
+                                int64_t* d_npass, int64_t* d_nused);
 
 /*
  * A5.  log xi(theta) = log( (1/n_draw) sum_j w_j ) over found injections with the all-sky prior

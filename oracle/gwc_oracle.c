@@ -612,7 +612,7 @@ int orc_kde_samples(const double* th, const orc_events* ev, int64_t n_rows, doub
  */
 int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events* ev, const orc_los* L, int mode,
                          double z_max, int M, int table_prec, int n_grid, double neff_min, double* logL,
-                         int64_t* npass) {
+                         int64_t* npass, int64_t* nused) {
   int err = 0;
   int64_t smax = 0;
   for (int64_t i = 0; i < ev->n_events; ++i) {
@@ -632,6 +632,7 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
       for (int64_t i = 0; i < ev->n_events; ++i) {
         logL[t * ev->n_events + i] = NAN;
         if (npass) npass[t * ev->n_events + i] = 0;
+        if (nused) nused[t * ev->n_events + i] = 0;
       }
       if (!lv || !zz || !lI || !Rg) err = 1;
       free(lv); free(zz); free(lI); free(Rg);
@@ -652,7 +653,7 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
         lv[k - a] = kde_sample(th, mode, &ct, ev->dL[k], ev->m1z[k], ev->m2z[k], lpi, L->z_max,
                                (int64_t)ev->sample_row[k], L->n_rows, &zz[k - a]);
       }
-      int64_t np = 0;
+      int64_t np = 0, nu = 0;
       int64_t r0 = a;
       while (r0 < b) {                            /* one pixel: samples r0 .. r1-1 */
         int64_t r1 = r0 + 1;
@@ -695,7 +696,7 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
               double c = (g == 0 || g == n_grid - 1) ? 0.5 * dzg : dzg;      /* trapezoid */
               I += (long double)c * f * prior;
             }
-            if (I > 0.0L) { lI[np++] = m + (double)logl(I); }
+            if (I > 0.0L) { lI[np++] = m + (double)logl(I); nu += n; }
           }
         }
         r0 = r1;
@@ -704,6 +705,7 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
       lse2(lI, np, &l1, &l2);
       logL[t * ev->n_events + i] = (b > a) ? l1 - log((double)(b - a)) : -INFINITY;
       if (npass) npass[t * ev->n_events + i] = np;
+      if (nused) nused[t * ev->n_events + i] = nu;
     }
     free(buf);
     free(lv); free(zz); free(lI); free(Rg);

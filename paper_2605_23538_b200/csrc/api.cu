@@ -408,7 +408,7 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
 
 gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                                 const gwc_los* los, int32_t n_grid, double neff_min, double* d_logL,
-                                int64_t* d_npass) {
+                                int64_t* d_npass, int64_t* d_nused) {
   GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
   if (!ev || !d_logL) return fail(ctx, GWC_ERR_INVALID_ARG, "ev or d_logL is NULL");
   if (!(neff_min >= 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "neff_min must be >= 0");
@@ -453,7 +453,7 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
                                 ctx->tab_prec, ctx->z_max / NODE32_QMAX, ev->n_events, ev->ev_sample_off, ev->dL,
                                 ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->seg_shift.p,
                                 los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, d_logL,
-                                d_npass, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, s),
+                                d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, s),
                 "kde"));
   if (ctx->timing) {
     cudaEventRecord(e1, s);

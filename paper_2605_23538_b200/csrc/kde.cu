@@ -52,6 +52,7 @@ struct KdeParams {
   int64_t scr_stride;       // >= the longest event
   double* logL;             // [n_theta][n_events]
   int64_t* npass;           // [n_theta][n_events] or NULL
+  int64_t* nused;           // [n_theta][n_events] or NULL: live samples of the contributing pixels
 };
 
 __device__ __forceinline__ double wsum(double v) {
@@ -135,6 +136,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       if (lane == 0) {
         p.logL[o] = CUDART_NAN;
         if (p.npass) p.npass[o] = 0;
+        if (p.nused) p.nused[o] = 0;
       }
       continue;
     }
@@ -189,6 +191,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
     __syncwarp();
     double esum = 0.0;   // sum over the passing pixels of I_j, relative to e^shift
     int np = 0;
+    int64_t nu = 0;
 
     int64_t r0 = s0;
     while (r0 < s1) {
@@ -284,6 +287,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         if (I > 0.0) {
           esum += I;
           ++np;
+          nu += n;
         }
       }
       r0 = r1;
@@ -291,6 +295,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
     if (lane == 0) {
       p.logL[o] = (s1 > s0 && esum > 0.0) ? shift + log(esum) - log((double)(s1 - s0)) : -CUDART_INF;
       if (p.npass) p.npass[o] = np;
+      if (p.nused) p.nused[o] = nu;
     }
     __syncwarp();   // the scratch slice is rewritten by the next unit
   }
@@ -302,13 +307,13 @@ int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
-               double* logL, int64_t* npass, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
+               double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
   if (n_theta <= 0 || n_events <= 0) return 0;
   KdeParams p;
   p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.n_theta = n_theta; p.n_events = n_events;
   p.M = M; p.Mp = Mp; p.tab_zq = tab_zq; p.ev_off = ev_off; p.dL = dL; p.m1z = m1z; p.m2z = m2z; p.lprior = lprior;
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
-  p.n_grid = n_grid; p.neff_min = neff_min; p.logL = logL; p.npass = npass;
+  p.n_grid = n_grid; p.neff_min = neff_min; p.logL = logL; p.npass = npass; p.nused = nused;
   p.scr = (double2*)scratch; p.scr_stride = scr_stride;
   const size_t smem = sizeof(MathTables);
   const int64_t blocks = n_blocks;

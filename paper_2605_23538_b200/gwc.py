@@ -76,7 +76,7 @@ def load():
         "gwc_los_allsky": (ci, [vp, C.POINTER(Los), vp]),
         "gwc_event_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), vp, vp, vp]),
         "gwc_event_loglik_pixcut": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), dbl, vp, vp, vp, vp]),
-        "gwc_event_loglik_kde": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), i32, dbl, vp, vp]),
+        "gwc_event_loglik_kde": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), i32, dbl, vp, vp, vp]),
         "gwc_selection_logxi": (ci, [vp, vp, i64, C.POINTER(Injections), C.POINTER(Los), vp, vp]),
         "gwc_combine_total": (ci, [vp, vp, vp, i64, i64, vp]),
         "gwc_total_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci, vp]),
@@ -232,14 +232,16 @@ class Context:
         return logL, neff, nlive, npass
 
     def gwc_event_loglik_kde(self, theta, ev, table, z_max, n_grid=256, neff_min=0.0):
-        """Event term with the paper's KDE numerator (Eq. 5-7, D1): returns logL, npass."""
+        """Event term with the paper's KDE numerator (Eq. 5-7, D1): returns logL, npass, nused."""
         nt, ne = theta.shape[0], ev["ev_sample_off"].numel() - 1
         logL = torch.empty((nt, ne), dtype=torch.float64, device=self.device)
         npass = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
+        nused = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
         es, los = make_events(ev), make_los(table, z_max)
         self._ck(self._lib.gwc_event_loglik_kde(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(los),
-                                                int(n_grid), float(neff_min), logL.data_ptr(), npass.data_ptr()))
-        return logL, npass
+                                                int(n_grid), float(neff_min), logL.data_ptr(), npass.data_ptr(),
+                                                nused.data_ptr()))
+        return logL, npass, nused
 
     def gwc_selection_logxi(self, theta, inj, allsky, n_z, z_max, want_neff=True):
         nt = theta.shape[0]

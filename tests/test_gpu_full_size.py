@@ -180,3 +180,27 @@ def test_production_pixcut_sampled(ctx):
     err = np.abs(g[fin] - o[fin]) / np.maximum(np.abs(o[fin]), 1.0)
     assert err.max() <= RTOL_F64, err.max()
     np.testing.assert_allclose(gN[tsel][fin], oN[fin], rtol=1e-7)
+
+
+def test_o4_kde_theta_subset(ctx):
+    """NEXT row 1 at catalogue size: the KDE numerator on the whole O4-scale catalogue (200 events, 4.4e5 samples,
+    16..512 pixels per event) for a seeded subset of 6 theta (the oracle needs 256 Gaussians per (theta, sample))."""
+    W, theta = _device_workload("o4")
+    tsel = _pick(theta.shape[0], 6, 17)
+    th = theta[torch.as_tensor(tsel, device=theta.device)].contiguous()
+    zmax = W.spec.z_max
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    gL, gP, gU = [_np(x) for x in ctx.gwc_event_loglik_kde(th, W.ev, W.los, zmax, 256, 2.0)]
+    ctx.gwc_check()
+    oL, oP, oU = oracle.event_loglik_kde(_np(th), synth.to_numpy(W.ev), _np(W.los), zmax, n_grid=256, neff_min=2.0,
+                                         want_nused=True)
+    same = gP == oP
+    print("o4 KDE: %d (theta, event) pairs, %d with a different pixel count; mean contributing pixels %.1f, "
+          "samples used %.0f of %.0f" % (same.size, int((~same).sum()), oP.mean(), oU.mean(),
+                                         W.ev["dL"].numel() / oP.shape[1]))
+    assert (~same).sum() <= 1e-3 * same.size
+    assert np.array_equal(gU[same], oU[same])
+    assert np.array_equal(np.isneginf(gL[same]), np.isneginf(oL[same]))
+    fin = same & np.isfinite(oL)
+    err = np.abs(gL[fin] - oL[fin]) / np.maximum(np.abs(oL[fin]), 1.0)
+    assert err.max() <= RTOL_F64, err.max()

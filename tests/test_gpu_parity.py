@@ -377,10 +377,11 @@ def _kde_both(ctx, W, theta, ev=None, los=None, n_grid=256, neff_min=0.0, prec=0
     zmax = W.spec.z_max
     th = theta.to(DEV)
     ctx.gwc_build_cosmo(th, zmax, 1025, prec)
-    gL, gP = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), los.to(DEV), zmax, n_grid, neff_min)
+    gL, gP, gU = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), los.to(DEV), zmax, n_grid, neff_min)
     ctx.gwc_check()
-    oL, oP = oracle.event_loglik_kde(_np(theta), synth.to_numpy(ev), _np(los), zmax, n_grid=n_grid, neff_min=neff_min,
-                                     table_prec=prec)
+    oL, oP, oU = oracle.event_loglik_kde(_np(theta), synth.to_numpy(ev), _np(los), zmax, n_grid=n_grid,
+                                         neff_min=neff_min, table_prec=prec, want_nused=True)
+    assert np.array_equal(_np(gU), oU), "nused differs"
     return (_np(gL), _np(gP)), (oL, oP)
 
 
@@ -428,7 +429,7 @@ def test_kde_edge_cases(ctx):
     zmax = W.spec.z_max
     th = theta.to(DEV)
     ctx.gwc_build_cosmo(th, zmax, 1025, 0)
-    gL, gP = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), W.los.to(DEV), zmax, 256, 0.0)
+    gL, gP, _ = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), W.los.to(DEV), zmax, 256, 0.0)
     with pytest.raises(gwc.GwcError):
         ctx.gwc_check()
     oL, oP = oracle.event_loglik_kde(_np(theta), synth.to_numpy(ev), _np(W.los), zmax)
