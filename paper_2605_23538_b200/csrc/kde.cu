@@ -80,7 +80,7 @@ __device__ __forceinline__ void node_pair(const Node32* t, int m, double& z0, do
 
 // z_k and ln v_k of one sample (-inf when dead): DESIGN.md section 3 without p_los and the rate term
 template <typename NodeT>
-__device__ __forceinline__ double sample_lv(const ThetaK& K, const NodeT* tab, int M, double zq, double dL, double m1z,
+__device__ __noinline__ double sample_lv(const ThetaK& K, const NodeT* tab, int M, double zq, double dL, double m1z,
                                             double m2z, double lpi, int32_t row, int64_t n_rows, double los_zmax,
                                             double& z_out) {
   z_out = 0.0;
@@ -117,6 +117,8 @@ template <typename NodeT, typename LosT>
 __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) {
   extern __shared__ __align__(16) unsigned char kde_smem[];
   MathTables& mt = *reinterpret_cast<MathTables*>(kde_smem);
+  // rate term at the grid nodes, one row per warp (kept out of the registers of the KDE loop)
+  double* s_rg = reinterpret_cast<double*>(kde_smem + sizeof(MathTables)) + (threadIdx.x >> 5) * (32 * KDE_NPL);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   init_math_tables(mt, tid, KDE_THREADS);
   __syncthreads();
@@ -161,7 +163,6 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       K.OL = 1.0 - th[1];
     }
     // rate term times the trapezoid weight at this lane's grid nodes: c_g psi(z_g) / (1 + z_g)   (reading R4)
-    double rg[KDE_NPL];
     {
       const double gam = th[9], kap = th[10], zp = th[11];
       const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
@@ -171,9 +172,10 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         const double x = 1.0 + g * dzg;
         const double psi = psi0 * pow(x, gam) / (1.0 + pow(x / (1.0 + zp), gam + kap));
         const double c = (g == 0 || g == G - 1) ? 0.5 * dzg : dzg;
-        rg[i] = g < G ? c * psi / x : 0.0;
+        s_rg[g] = g < G ? c * psi / x : 0.0;
       }
     }
+    __syncwarp();
     const NodeT* tab = reinterpret_cast<const NodeT*>(p.tab) + (size_t)t * p.Mp;
     const double shift = p.seg_shift[ev];
     // ---- (z_k, v_k) of every sample of the event, relative to e^shift ----
@@ -280,7 +282,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
             b = b > p.n_z - 2 ? p.n_z - 2 : b;
             const double fz = tz - (double)b;
             const double q0 = (double)lrow[b], q1 = (double)lrow[b + 1];
-            part = fma(acc[i], (q0 + fz * (q1 - q0)) * rg[i], part);
+            part = fma(acc[i], (q0 + fz * (q1 - q0)) * s_rg[g], part);
           }
         }
         const double I = wsum(part);
@@ -315,7 +317,7 @@ int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst,
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
   p.n_grid = n_grid; p.neff_min = neff_min; p.logL = logL; p.npass = npass; p.nused = nused;
   p.scr = (double2*)scratch; p.scr_stride = scr_stride;
-  const size_t smem = sizeof(MathTables);
+  const size_t smem = sizeof(MathTables) + sizeof(double) * KDE_WARPS * 32 * KDE_NPL;
   const int64_t blocks = n_blocks;
 #define GWC_KDE_LAUNCH(NodeT, LosT)                                                                              \
   do {                                                                                                           \
