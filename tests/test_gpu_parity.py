@@ -284,6 +284,7 @@ def test_pixcut_tiny(ctx, thr):
     _pixcut_compare(g, o, "tiny thr=%g" % thr)
     if thr == 0.0:      # threshold 0 = the uncut path, bit for bit the same sums
         th = W.theta.to(DEV)
+        ctx.gwc_build_cosmo(th, W.spec.z_max, 1025, 0)
         logL, neff, nlive = ctx.gwc_event_loglik(th, to_dev(W.ev, DEV), W.los.to(DEV), W.spec.z_max)
         np.testing.assert_allclose(g[0], _np(logL), rtol=1e-13, atol=0)
         assert np.array_equal(g[2], _np(nlive))
