@@ -46,3 +46,56 @@ def max_over_ranks(value: float, device, group: Optional[dist.ProcessGroup] = No
     t = torch.tensor([value], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
     return float(t.item())
+
+
+# ---- event / injection sharding (SURVEY.md 8e-2): for catalogues that outgrow one GPU or very small theta batches --
+# Each rank owns a contiguous block of events (balanced by samples) and a contiguous block of the found injections,
+# evaluates every theta on them with the ordinary calls (gwc_event_loglik, gwc_selection_logxi with the GLOBAL
+# n_draw), and the ranks exchange two small arrays: an all-reduce of sum_i log L_i  [n_theta]  and an all-gather of
+# (log xi_r, N_eff,r)  [world][n_theta][2], combined in rank order so that every rank gets the same bits.
+def event_range(ev_sample_off: torch.Tensor, rank: int, world: int) -> Tuple[int, int]:
+    """[lo, hi) of the events owned by `rank`: contiguous blocks cut where the cumulative sample count crosses
+    k * n_samples / world (every event belongs to exactly one rank; a rank may own none)."""
+    if world < 1 or not (0 <= rank < world):
+        raise ValueError("bad rank/world")
+    off = ev_sample_off.detach().cpu().to(torch.int64)
+    n_events = off.numel() - 1
+    total = int(off[-1] - off[0])
+    if n_events <= 0:
+        return 0, 0
+    mid = (off[:-1] + off[1:]).to(torch.float64) * 0.5 - float(off[0])     # event centres in sample units
+    owner = torch.clamp((mid * world / max(total, 1)).floor().to(torch.int64), 0, world - 1) if total > 0 else \
+        torch.div(torch.arange(n_events) * world, n_events, rounding_mode="floor")
+    lo = int((owner < rank).sum())
+    return lo, lo + int((owner == rank).sum())
+
+
+def combine_event_sharded(sum_logL_local: torch.Tensor, logxi_local: torch.Tensor, neff_inj_local: torch.Tensor,
+                          n_events_total: int, group: Optional[dist.ProcessGroup] = None):
+    """log L(theta) = sum over ALL events of log L_i - n_events_total * log xi from per-rank pieces.
+    sum_logL_local [n_theta]: sum of log L_i over this rank's events (0 for a rank without events).
+    logxi_local, neff_inj_local [n_theta]: selection term over this rank's injections, computed with the global
+    n_draw, so that xi = sum_r xi_r; N_eff = (sum_r S1_r)^2 / sum_r S2_r with S1_r = xi_r, S2_r = xi_r^2 / N_eff,r.
+    Returns (total, logxi, neff_inj), identical on every rank (fixed rank order)."""
+    world = dist.get_world_size(group)
+    s = sum_logL_local.clone()
+    parts = [torch.empty_like(s) for _ in range(world)]
+    dist.all_gather(parts, s, group=group)                   # gathered, then summed in rank order: same bits everywhere
+    sum_logL = torch.stack(parts, 0).sum(0) if world > 1 else s
+    pair = torch.stack([logxi_local, neff_inj_local], -1).contiguous()
+    pairs = [torch.empty_like(pair) for _ in range(world)]
+    dist.all_gather(pairs, pair, group=group)
+    lx = torch.stack([p[..., 0] for p in pairs], 0)          # [world][n_theta]
+    ne = torch.stack([p[..., 1] for p in pairs], 0)
+    m = lx.max(0).values
+    m_safe = torch.where(torch.isfinite(m), m, torch.zeros_like(m))
+    s1 = torch.exp(lx - m_safe)                              # xi_r relative to e^m  (0 for -inf)
+    s2 = torch.where(ne > 0, s1 * s1 / ne.clamp_min(1e-300), torch.zeros_like(s1))
+    S1, S2 = s1.sum(0), s2.sum(0)
+    logxi = torch.where(S1 > 0, m_safe + torch.log(S1.clamp_min(1e-300)), torch.full_like(m, float("-inf")))
+    neff = torch.where(S2 > 0, S1 * S1 / S2.clamp_min(1e-300), torch.zeros_like(S1))
+    total = sum_logL - float(n_events_total) * logxi
+    total = torch.where(torch.isneginf(sum_logL) | torch.isneginf(logxi), torch.full_like(total, float("-inf")), total)
+    nan = torch.isnan(sum_logL) | torch.isnan(lx).any(0)
+    total = torch.where(nan, torch.full_like(total, float("nan")), total)
+    return total, logxi, neff

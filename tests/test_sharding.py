@@ -70,3 +70,71 @@ def test_world2_gloo_theta_sharding_matches_single_process(tmp_path, n_theta):
     for r in range(world):
         got = np.load(os.path.join(str(tmp_path), "rank%d.npy" % r))
         assert np.array_equal(got, ref, equal_nan=True)
+
+
+def test_event_range_partitions_exactly():
+    rng = np.random.default_rng(0)
+    for n_events in (1, 2, 5, 40):
+        sizes = rng.integers(1, 5000, n_events)
+        off = torch.from_numpy(np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64))
+        for world in (1, 2, 3, 8):
+            edges = [shard.event_range(off, r, world) for r in range(world)]
+            assert edges[0][0] == 0 and edges[-1][1] == n_events
+            assert all(edges[r][1] == edges[r + 1][0] for r in range(world - 1))
+            if n_events >= 8 * world:
+                per = [int(off[b] - off[a]) for a, b in edges]
+                assert max(per) <= 2 * int(off[-1]) // world + 5000
+
+
+def _worker_events(rank, world, port, n_theta, out_dir):
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import oracle
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        oracle.set_num_threads(1)
+        spec = synth.scaled(synth.CONFIGS["tiny"], n_theta=n_theta)
+        W = synth.make_workload(spec, device="cpu")
+        ev, inj = synth.to_numpy(W.ev), synth.to_numpy(W.inj)
+        th = W.theta.numpy()
+        lo, hi = shard.event_range(W.ev["ev_sample_off"], rank, world)
+        off = ev["ev_sample_off"]
+        sl = slice(off[lo], off[hi])
+        sub = dict(ev_sample_off=(off[lo:hi + 1] - off[lo]).astype(np.int64), dL=ev["dL"][sl], m1z=ev["m1z"][sl],
+                   m2z=ev["m2z"][sl], sample_row=ev["sample_row"][sl], log_pe_prior=None)
+        los = W.los.numpy()
+        if hi > lo:
+            logL, _, _ = oracle.event_loglik(th, sub, los, spec.z_max)
+            s = np.where(np.isneginf(logL).any(1), -np.inf, logL.sum(1))
+        else:
+            s = np.zeros(th.shape[0])
+        nf = inj["dL"].size
+        a, b = shard.theta_range(nf, rank, world)             # the same balanced split serves the injections
+        sub_inj = dict(dL=inj["dL"][a:b], m1z=inj["m1z"][a:b], m2z=inj["m2z"][a:b], log_pdraw=inj["log_pdraw"][a:b],
+                       n_draw=inj["n_draw"])                  # global n_draw
+        allsky = oracle.los_allsky(los, spec.z_max)
+        lx, ne = oracle.selection_logxi(th, sub_inj, allsky, spec.z_max)
+        total, logxi, neff = shard.combine_event_sharded(torch.from_numpy(s), torch.from_numpy(lx),
+                                                         torch.from_numpy(ne), off.size - 1)
+        np.save(os.path.join(out_dir, "ev_rank%d.npy" % rank), np.stack([total.numpy(), logxi.numpy(), neff.numpy()]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world2_gloo_event_sharding_matches_single_process(tmp_path):
+    import oracle
+    world, n_theta = 2, 6
+    mp.spawn(_worker_events, args=(world, _free_port(), n_theta, str(tmp_path)), nprocs=world, join=True)
+    spec = synth.scaled(synth.CONFIGS["tiny"], n_theta=n_theta)
+    W = synth.make_workload(spec, device="cpu")
+    ev, inj, los = synth.to_numpy(W.ev), synth.to_numpy(W.inj), W.los.numpy()
+    ref = oracle.total_loglik(W.theta.numpy(), ev, inj, los, spec.z_max)
+    lx, ne = oracle.selection_logxi(W.theta.numpy(), inj, oracle.los_allsky(los, spec.z_max), spec.z_max)
+    got = [np.load(os.path.join(str(tmp_path), "ev_rank%d.npy" % r)) for r in range(world)]
+    assert np.array_equal(got[0], got[1], equal_nan=True)      # every rank holds the same bits
+    fin = np.isfinite(ref)
+    assert np.array_equal(np.isneginf(got[0][0]), np.isneginf(ref))
+    np.testing.assert_allclose(got[0][0][fin], ref[fin], rtol=1e-12)
+    np.testing.assert_allclose(got[0][1], lx, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(got[0][2], ne, rtol=1e-10)
