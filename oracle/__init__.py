@@ -70,6 +70,7 @@ def lib():
             "orc_selection_logxi": (C.c_int, [vp, i64, vp, vp, i32, d, C.c_int, d, C.c_int, C.c_int, vp, vp]),
             "orc_total_from_parts": (None, [vp, vp, i64, i64, vp]),
             "orc_pack_events": (i64, [i64, i64, vp, vp, vp, vp, vp, vp, vp]),
+            "orc_cap_pixels": (i64, [i64, i64, i64, vp, vp, vp, i64, C.c_uint64, vp]),
             "orc_num_threads": (C.c_int, []), "orc_set_num_threads": (None, [C.c_int]),
         }
         for name, (res, args) in sig.items():
@@ -292,3 +293,17 @@ def num_threads():
 
 def set_num_threads(n):
     lib().orc_set_num_threads(int(n))
+
+
+def cap_pixels(perm, ev_sample_off, pix_sample_off, cap, seed):
+    """Per-pixel sample cap on a packed catalogue (R31).  Returns perm_kept,
+    ev_sample_off', pix_sample_off' (new arrays)."""
+    perm = np.ascontiguousarray(perm, dtype=np.int64)
+    evo = np.array(ev_sample_off, dtype=np.int64, copy=True)
+    pxo = np.array(pix_sample_off, dtype=np.int64, copy=True)
+    out = np.empty(max(perm.size, 1), dtype=np.int64)
+    nk = lib().orc_cap_pixels(perm.size, evo.size - 1, pxo.size - 1, _p(perm), _p(evo), _p(pxo), int(cap),
+                              int(seed) & 0xFFFFFFFFFFFFFFFF, _p(out))
+    assert nk >= 0
+    return out[:nk].copy(), evo, pxo
+

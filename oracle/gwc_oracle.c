@@ -828,3 +828,60 @@ int64_t orc_pack_events(int64_t n_samples, int64_t n_events, const int32_t* even
   free(keys);
   return np;
 }
+
+/*
+ * NEXT row 3b: the per-pixel sample cap, "the option to randomly downsample the GW posterior
+ * samples in a given pixel" (fiducial 2500).  Reading R31: applied to a packed
+ * catalogue; a pixel ((event, row) run) of n > cap samples keeps the cap samples with the smallest
+ * (hash32(seed, original sample index), packed position); smaller pixels keep everything; kept samples keep their
+ * packed order.  hash32 = the upper half of splitmix64's output function applied to seed + (index+1) * golden.
+ * perm_in [n_samples], ev_sample_off [n_events+1] and pix_sample_off [n_pix+1] are those of orc_pack_events;
+ * the two offset arrays are rewritten for the kept samples, perm_out receives the kept entries of perm_in.
+ * Returns the number of kept samples.
+ */
+static uint32_t cap_hash32(uint64_t seed, uint64_t index) {
+  uint64_t z = seed + (index + 1ULL) * 0x9E3779B97F4A7C15ULL;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  z = z ^ (z >> 31);
+  return (uint32_t)(z >> 32);
+}
+
+typedef struct { uint32_t h; int64_t pos; } cap_key;
+static int cap_cmp(const void* a, const void* b) {
+  const cap_key* x = (const cap_key*)a;
+  const cap_key* y = (const cap_key*)b;
+  if (x->h != y->h) return x->h < y->h ? -1 : 1;
+  return x->pos < y->pos ? -1 : (x->pos > y->pos ? 1 : 0);
+}
+
+int64_t orc_cap_pixels(int64_t n_samples, int64_t n_events, int64_t n_pix, const int64_t* perm_in,
+                       int64_t* ev_sample_off, int64_t* pix_sample_off, int64_t cap, uint64_t seed,
+                       int64_t* perm_out) {
+  if (cap < 1) return -1;
+  char* keep = (char*)calloc((size_t)(n_samples > 0 ? n_samples : 1), 1);
+  cap_key* keys = (cap_key*)malloc(sizeof(cap_key) * (size_t)(n_samples > 0 ? n_samples : 1));
+  int64_t* newpos = (int64_t*)malloc(sizeof(int64_t) * (size_t)(n_samples + 1));
+  if (!keep || !keys || !newpos) { free(keep); free(keys); free(newpos); return -1; }
+  for (int64_t j = 0; j < n_pix; ++j) {
+    int64_t a = pix_sample_off[j], b = pix_sample_off[j + 1];
+    if (b - a <= cap) {
+      for (int64_t k = a; k < b; ++k) keep[k] = 1;
+      continue;
+    }
+    for (int64_t k = a; k < b; ++k) { keys[k - a].h = cap_hash32(seed, (uint64_t)perm_in[k]); keys[k - a].pos = k; }
+    qsort(keys, (size_t)(b - a), sizeof(cap_key), cap_cmp);
+    for (int64_t r = 0; r < cap; ++r) keep[keys[r].pos] = 1;
+  }
+  int64_t nk = 0;
+  for (int64_t k = 0; k < n_samples; ++k) {
+    newpos[k] = nk;
+    if (keep[k]) perm_out[nk++] = perm_in[k];
+  }
+  newpos[n_samples] = nk;
+  for (int64_t i = 0; i <= n_events; ++i) ev_sample_off[i] = newpos[ev_sample_off[i]];
+  for (int64_t j = 0; j <= n_pix; ++j) pix_sample_off[j] = newpos[pix_sample_off[j]];
+  free(keep); free(keys); free(newpos);
+  return nk;
+}
+

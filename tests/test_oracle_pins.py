@@ -651,3 +651,80 @@ def test_kde_pixel_rules_and_invariances(theta0):
     th2 = theta0.copy(); th2[0] *= s
     gots, _ = O.event_loglik_kde(th2, dict(ev, dL=ev["dL"] / s), tab, zmax)
     np.testing.assert_allclose(gots, base + 3 * math.log(s), rtol=0, atol=1e-11)
+
+
+# ---- NEXT row 3b: the per-pixel sample cap (R31) -----------------------------------
+def _cap_catalogue(seed=0, n=6000, n_events=5, rows=12):
+    rng = np.random.default_rng(seed)
+    ev = rng.integers(0, n_events, n).astype(np.int32)
+    row = np.minimum(rng.geometric(0.35, n) - 1, rows - 1).astype(np.int32)   # a few crowded pixels, a long tail
+    return ev, row, O.pack_events(ev, row, n_events)
+
+
+def test_cap_pixels_properties():
+    ev, row, P = _cap_catalogue()
+    sizes = np.diff(P["pix_sample_off"])
+    assert sizes.max() > 200 and sizes.min() < 5
+    for cap in (1, 7, 100, 10 ** 6):
+        perm, evo, pxo = O.cap_pixels(P["perm"], P["ev_sample_off"], P["pix_sample_off"], cap, 1234)
+        assert np.array_equal(np.diff(pxo), np.minimum(sizes, cap))          # every pixel keeps min(n, cap)
+        assert perm.size == pxo[-1] == evo[-1] and evo[0] == 0
+        # the kept samples are a subsequence of the packed order (order preserved, no duplicates)
+        pos = {v: i for i, v in enumerate(P["perm"])}
+        where = np.array([pos[v] for v in perm])
+        assert np.all(np.diff(where) > 0)
+        # and they stay inside their own pixel and event
+        for j in range(sizes.size):
+            a, b = P["pix_sample_off"][j], P["pix_sample_off"][j + 1]
+            assert set(perm[pxo[j]:pxo[j + 1]]) <= set(P["perm"][a:b])
+        assert np.array_equal(np.diff(evo), np.bincount(ev[perm], minlength=5))
+        if cap >= sizes.max():
+            assert np.array_equal(perm, P["perm"])
+    # seeded: same seed same choice, another seed another choice
+    a = O.cap_pixels(P["perm"], P["ev_sample_off"], P["pix_sample_off"], 7, 99)[0]
+    b = O.cap_pixels(P["perm"], P["ev_sample_off"], P["pix_sample_off"], 7, 99)[0]
+    c = O.cap_pixels(P["perm"], P["ev_sample_off"], P["pix_sample_off"], 7, 100)[0]
+    assert np.array_equal(a, b) and not np.array_equal(a, c)
+    # the choice depends on the original sample index only, not on where packing put the sample:
+    # relabelling the events (another packed order) keeps the same original samples
+    P2 = O.pack_events((4 - ev).astype(np.int32), row, 5)
+    d = O.cap_pixels(P2["perm"], P2["ev_sample_off"], P2["pix_sample_off"], 7, 99)[0]
+    assert set(a) == set(d)
+
+
+def test_cap_pixels_is_uniform_without_replacement():
+    # one pixel of 40 samples, cap 10, 4000 seeds: every sample is kept with probability 1/4 (binomial, 5 sigma)
+    n, cap, trials = 40, 10, 4000
+    perm = np.arange(n, dtype=np.int64)
+    evo, pxo = np.array([0, n]), np.array([0, n])
+    counts = np.zeros(n)
+    for s in range(trials):
+        kept = O.cap_pixels(perm, evo, pxo, cap, s)[0]
+        assert kept.size == cap and np.unique(kept).size == cap
+        counts[kept] += 1
+    sigma = math.sqrt(trials * 0.25 * 0.75)
+    assert np.abs(counts - trials * 0.25).max() < 5 * sigma
+
+
+def test_cap_pixels_against_numpy_lexsort():
+    # the same rule written with numpy: inside a crowded pixel keep the cap smallest (hash32, packed position)
+    ev, row, P = _cap_catalogue(seed=3)
+    seed, cap = 20260915, 25
+    def h32(idx):
+        M = (1 << 64) - 1
+        z = (seed + (int(idx) + 1) * 0x9E3779B97F4A7C15) & M
+        z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & M
+        z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & M
+        return (z ^ (z >> 31)) >> 32
+    keep = np.zeros(P["perm"].size, bool)
+    pso = P["pix_sample_off"]
+    for j in range(pso.size - 1):
+        a, b = pso[j], pso[j + 1]
+        if b - a <= cap:
+            keep[a:b] = True
+        else:
+            h = np.array([h32(v) for v in P["perm"][a:b]], dtype=np.uint64)
+            order = np.lexsort((np.arange(a, b), h))
+            keep[a + order[:cap]] = True
+    got = O.cap_pixels(P["perm"], P["ev_sample_off"], pso, cap, seed)[0]
+    assert np.array_equal(got, P["perm"][keep])
