@@ -122,6 +122,23 @@ gwc_status gwc_pack_events(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, co
                            const int32_t* d_row, int64_t* d_perm, int64_t* d_ev_sample_off, int64_t* d_ev_pix_off,
                            int32_t* d_ev_pix_rows, int64_t* d_pix_sample_off, int64_t* h_n_pixrefs);
 
+/*
+ * The per-pixel sample cap, "the option to randomly downsample the GW posterior samples in a given pixel"
+ * (fiducial cap 2500; R31), applied to the output of gwc_pack_events (one-time,
+ * integer work, compared bit for bit with the oracle).  A pixel ((event, row) run) with more than `cap` samples keeps
+ * the `cap` samples with the smallest (hash32(seed, original sample index), packed position), hash32 = upper half of
+ * splitmix64's output function of seed + (index + 1) * 0x9E3779B97F4A7C15; smaller pixels keep everything; kept
+ * samples keep their packed order.  The choice depends on the original indices only, not on the packing.
+ *   in : d_perm [n_samples] (gwc_pack_events' permutation), n_pixrefs
+ *   in/out: d_ev_sample_off [n_events+1], d_pix_sample_off [n_pixrefs+1]: rewritten for the kept samples
+ *   out: d_perm_out [n_samples] (first *h_n_kept entries valid; must not alias d_perm), h_n_kept (host)
+ * ev_pix_off / ev_pix_rows are unchanged (every pixel keeps at least one sample).  cap < 1 -> GWC_ERR_INVALID_ARG.
+ * Synchronises the stream.
+ */
+gwc_status gwc_cap_pixels(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, int64_t n_pixrefs,
+                          const int64_t* d_perm, int64_t* d_ev_sample_off, int64_t* d_pix_sample_off, int64_t cap,
+                          uint64_t seed, int64_t* d_perm_out, int64_t* h_n_kept);
+
 /* All-sky prior of the denominator: arithmetic mean over all rows, in f64, fixed order. */
 gwc_status gwc_los_allsky(gwc_ctx* ctx, const gwc_los* los, double* d_allsky /* [n_z] */);
 

@@ -345,6 +345,26 @@ gwc_status gwc_pack_events(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, co
   return gwc_check(ctx);
 }
 
+gwc_status gwc_cap_pixels(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, int64_t n_pixrefs,
+                          const int64_t* d_perm, int64_t* d_ev_sample_off, int64_t* d_pix_sample_off, int64_t cap,
+                          uint64_t seed, int64_t* d_perm_out, int64_t* h_n_kept) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (n_samples < 0 || n_events < 0 || n_pixrefs < 0 || n_pixrefs > n_samples || n_pixrefs > 0x7fffffffLL)
+    return fail(ctx, GWC_ERR_SHAPE, "sizes out of range");
+  if (cap < 1) return fail(ctx, GWC_ERR_INVALID_ARG, "cap must be >= 1");
+  if (!d_ev_sample_off || !d_pix_sample_off || !h_n_kept) return fail(ctx, GWC_ERR_INVALID_ARG, "a pointer is NULL");
+  if (n_samples > 0 && (!d_perm || !d_perm_out)) return fail(ctx, GWC_ERR_INVALID_ARG, "a permutation pointer is NULL");
+  const size_t bytes = cap_scratch_bytes(n_samples);
+  GWC_TRY(ensure(ctx, ctx->pack_scr, bytes + 8));
+  int64_t* d_nk = (int64_t*)((unsigned char*)ctx->pack_scr.p + bytes);
+  GWC_TRY(count(ctx, launch_cap_pixels(n_samples, n_events, n_pixrefs, d_perm, d_ev_sample_off, d_pix_sample_off, cap,
+                                       seed, d_perm_out, d_nk, ctx->pack_scr.p, bytes, ctx->stream),
+                "cap_pixels"));
+  GWC_CUDA(cudaMemcpyAsync(h_n_kept, d_nk, sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream));
+  GWC_CUDA(cudaStreamSynchronize(ctx->stream));
+  return gwc_check(ctx);
+}
+
 gwc_status gwc_los_allsky(gwc_ctx* ctx, const gwc_los* los, double* d_allsky) {
   if (!ctx) return GWC_ERR_INVALID_ARG;
   GWC_TRY(check_los(ctx, los, true, false));

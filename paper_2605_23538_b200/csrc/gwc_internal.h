@@ -137,4 +137,9 @@ int launch_pack(int64_t n_samples, int64_t n_events, const int32_t* d_event_id, 
                 int64_t* d_ev_sample_off, int64_t* d_ev_pix_off, int32_t* d_ev_pix_rows, int64_t* d_pix_sample_off,
                 int64_t* d_n_pixrefs, int* d_flag, void* scratch, size_t scratch_bytes, cudaStream_t s);
 
+size_t cap_scratch_bytes(int64_t n_samples);
+int launch_cap_pixels(int64_t n, int64_t n_events, int64_t n_pix, const int64_t* d_perm_in, int64_t* d_ev_sample_off,
+                      int64_t* d_pix_sample_off, int64_t cap, uint64_t seed, int64_t* d_perm_out, int64_t* d_n_kept,
+                      void* scratch, size_t scratch_bytes, cudaStream_t s);
+
 }  // namespace gwc

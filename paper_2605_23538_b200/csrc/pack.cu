@@ -83,6 +83,59 @@ __global__ void pack_empty_kernel(int64_t n_events, int64_t* ev_sample_off, int6
   }
 }
 
+// ---- per-pixel sample cap (R31) ---------------------------------------------------
+// upper half of splitmix64's output function applied to seed + (index + 1) * golden ratio
+__device__ __forceinline__ uint32_t cap_hash32(uint64_t seed, uint64_t index) {
+  uint64_t z = seed + (index + 1ULL) * 0x9E3779B97F4A7C15ULL;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  z = z ^ (z >> 31);
+  return (uint32_t)(z >> 32);
+}
+
+// key of packed position k = (its pixel, hash of its original sample index); value = k
+__global__ void cap_keys_kernel(int64_t n, int64_t n_pix, const int64_t* __restrict__ perm,
+                                const int64_t* __restrict__ pix_sample_off, uint64_t seed, uint64_t* __restrict__ keys,
+                                int64_t* __restrict__ vals) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  int64_t lo = 0, hi = n_pix;  // largest j with pix_sample_off[j] <= k
+  while (hi - lo > 1) {
+    const int64_t mid = (lo + hi) >> 1;
+    if (pix_sample_off[mid] <= k) lo = mid; else hi = mid;
+  }
+  keys[k] = ((uint64_t)lo << 32) | (uint64_t)cap_hash32(seed, (uint64_t)perm[k]);
+  vals[k] = k;
+}
+
+// after the stable sort the samples of a pixel are in (hash, packed position) order: the first `cap` are kept
+__global__ void cap_flags_kernel(int64_t n, const uint64_t* __restrict__ keys_sorted,
+                                 const int64_t* __restrict__ vals_sorted, const int64_t* __restrict__ pix_sample_off,
+                                 int64_t cap, int64_t* __restrict__ keep) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t j = (int64_t)(keys_sorted[i] >> 32);
+  keep[vals_sorted[i]] = (i - pix_sample_off[j] < cap) ? 1 : 0;
+}
+
+__global__ void cap_compact_kernel(int64_t n, const int64_t* __restrict__ perm_in, const int64_t* __restrict__ keep,
+                                   const int64_t* __restrict__ newpos, int64_t* __restrict__ perm_out,
+                                   int64_t* __restrict__ n_kept) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  if (keep[k]) perm_out[newpos[k]] = perm_in[k];
+  if (k == n - 1) *n_kept = newpos[k] + keep[k];
+}
+
+// offsets of the kept samples, in place (each thread reads its own old value)
+__global__ void cap_offsets_kernel(int64_t n, int64_t m, int64_t* __restrict__ off, const int64_t* __restrict__ newpos,
+                                   const int64_t* __restrict__ n_kept) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i > m) return;
+  const int64_t o = off[i];
+  off[i] = o >= n ? *n_kept : newpos[o];
+}
+
 size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 size_t cub_temp_bytes(int64_t n) {
@@ -135,6 +188,45 @@ int launch_pack(int64_t n, int64_t n_events, const int32_t* d_event_id, const in
   pack_pix_off_kernel<<<be, 256, 0, s>>>(n, n_events, d_ev_sample_off, pos, d_n_pixrefs, d_ev_pix_off);
   launches += 6;
   return cudaGetLastError() == cudaSuccess ? launches : -1;
+}
+
+size_t cap_scratch_bytes(int64_t n_samples) {
+  const size_t n = (size_t)(n_samples > 0 ? n_samples : 1);
+  return 6 * a256(8 * n) + a256(cub_temp_bytes((int64_t)n)) + 256;
+}
+
+// Per-pixel sample cap on a packed catalogue: rewrites the two offset arrays for the kept samples, writes the kept
+// entries of perm_in to perm_out (packed order preserved) and their number to d_n_kept.
+int launch_cap_pixels(int64_t n, int64_t n_events, int64_t n_pix, const int64_t* d_perm_in, int64_t* d_ev_sample_off,
+                      int64_t* d_pix_sample_off, int64_t cap, uint64_t seed, int64_t* d_perm_out, int64_t* d_n_kept,
+                      void* scratch, size_t scratch_bytes, cudaStream_t s) {
+  if (n == 0) {
+    if (cudaMemsetAsync(d_n_kept, 0, sizeof(int64_t), s) != cudaSuccess) return -1;
+    return 0;
+  }
+  unsigned char* base = (unsigned char*)scratch;
+  uint64_t* keys = (uint64_t*)base;            base += a256(8 * (size_t)n);
+  uint64_t* keys_sorted = (uint64_t*)base;     base += a256(8 * (size_t)n);
+  int64_t* vals = (int64_t*)base;              base += a256(8 * (size_t)n);
+  int64_t* vals_sorted = (int64_t*)base;       base += a256(8 * (size_t)n);
+  int64_t* keep = (int64_t*)base;              base += a256(8 * (size_t)n);
+  int64_t* newpos = (int64_t*)base;            base += a256(8 * (size_t)n);
+  void* temp = base;
+  size_t temp_bytes = scratch_bytes - (size_t)(base - (unsigned char*)scratch);
+  const unsigned bn = (unsigned)((n + 255) / 256);
+  cap_keys_kernel<<<bn, 256, 0, s>>>(n, n_pix, d_perm_in, d_pix_sample_off, seed, keys, vals);
+  int end_bit = 33;
+  while (end_bit < 64 && ((uint64_t)n_pix >> (end_bit - 32)) != 0) ++end_bit;
+  if (cub::DeviceRadixSort::SortPairs(temp, temp_bytes, keys, keys_sorted, vals, vals_sorted, n, 0, end_bit, s) !=
+      cudaSuccess)
+    return -1;
+  cap_flags_kernel<<<bn, 256, 0, s>>>(n, keys_sorted, vals_sorted, d_pix_sample_off, cap, keep);
+  temp_bytes = scratch_bytes - (size_t)(base - (unsigned char*)scratch);
+  if (cub::DeviceScan::ExclusiveSum(temp, temp_bytes, keep, newpos, n, s) != cudaSuccess) return -1;
+  cap_compact_kernel<<<bn, 256, 0, s>>>(n, d_perm_in, keep, newpos, d_perm_out, d_n_kept);
+  cap_offsets_kernel<<<(unsigned)((n_events + 1 + 255) / 256), 256, 0, s>>>(n, n_events, d_ev_sample_off, newpos, d_n_kept);
+  cap_offsets_kernel<<<(unsigned)((n_pix + 1 + 255) / 256), 256, 0, s>>>(n, n_pix, d_pix_sample_off, newpos, d_n_kept);
+  return cudaGetLastError() == cudaSuccess ? 14 : -1;  // 5 kernels + the library's radix and scan passes (approximate)
 }
 
 }  // namespace gwc

@@ -23,7 +23,7 @@ _STATUS = ["GWC_OK", "GWC_ERR_INVALID_ARG", "GWC_ERR_SHAPE", "GWC_ERR_DOMAIN", "
            "GWC_ERR_CUDA"]
 
 EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_launch_count", "gwc_build_cosmo",
-           "gwc_export_cosmo", "gwc_pack_events", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",
+           "gwc_export_cosmo", "gwc_pack_events", "gwc_cap_pixels", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",
            "gwc_selection_logxi",
            "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_host", "gwc_set_timing", "gwc_get_timing",
            "gwc_probe_fp64", "gwc_math_selftest"]
@@ -73,6 +73,7 @@ def load():
         "gwc_build_cosmo": (ci, [vp, vp, i64, dbl, i32, ci]),
         "gwc_export_cosmo": (ci, [vp, vp, vp, vp]),
         "gwc_pack_events": (ci, [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]),
+        "gwc_cap_pixels": (ci, [vp, i64, i64, i64, vp, vp, vp, i64, C.c_uint64, vp, C.POINTER(i64)]),
         "gwc_los_allsky": (ci, [vp, C.POINTER(Los), vp]),
         "gwc_event_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), vp, vp, vp]),
         "gwc_event_loglik_pixcut": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), dbl, vp, vp, vp, vp]),
@@ -201,6 +202,19 @@ class Context:
         k = int(npx.value)
         return dict(perm=perm[:n], ev_sample_off=eso, ev_pix_off=epo, ev_pix_rows=epr[:k], pix_sample_off=pso[:k + 1],
                     n_pixrefs=k)
+
+    def gwc_cap_pixels(self, packed: dict, cap: int, seed: int):
+        """Per-pixel sample cap on the output of gwc_pack_events: returns perm_kept,
+        ev_sample_off', pix_sample_off' (new tensors; `packed` is left untouched)."""
+        perm = packed["perm"].contiguous()
+        eso, pso = packed["ev_sample_off"].clone(), packed["pix_sample_off"].clone()
+        n = perm.numel()
+        out = torch.empty(max(n, 1), dtype=torch.int64, device=self.device)
+        nk = C.c_int64(0)
+        self._ck(self._lib.gwc_cap_pixels(self._h, n, eso.numel() - 1, pso.numel() - 1, perm.data_ptr(), eso.data_ptr(),
+                                          pso.data_ptr(), int(cap), int(seed) & 0xFFFFFFFFFFFFFFFF, out.data_ptr(),
+                                          C.byref(nk)))
+        return out[:int(nk.value)], eso, pso
 
     def gwc_los_allsky(self, table: torch.Tensor, z_max: float) -> torch.Tensor:
         out = torch.empty(table.shape[1], dtype=torch.float64, device=self.device)

@@ -447,3 +447,48 @@ def test_kde_edge_cases(ctx):
     except gwc.GwcError:
         pass
     assert torch.equal(torch.nan_to_num(g2[0], nan=7.0), torch.nan_to_num(gL, nan=7.0)) and torch.equal(g2[1], gP)
+
+
+# ---- NEXT row 3b: the per-pixel sample cap (R31) -----------------------------------
+def test_cap_pixels_bit_exact(ctx):
+    """The kept permutation and both offset arrays equal the oracle's, bit for bit, for crowded and sparse pixels,
+    several caps and seeds, an empty event and an empty catalogue; the capped catalogue then goes through the hot
+    path like any other."""
+    from paper_2605_23538_b200 import gwc
+    g = torch.Generator().manual_seed(11)
+    n, ne = 200_000, 23
+    eid = torch.randint(0, ne, (n,), generator=g, dtype=torch.int32)
+    eid[eid == 4] = 5                                                       # an empty event
+    geo = torch.empty(n).geometric_(0.02, generator=g).to(torch.int32) - 1  # a few crowded pixels, a long tail
+    row = torch.clamp(geo, max=900)
+    o = oracle.pack_events(eid.numpy(), row.numpy(), ne)
+    p = ctx.gwc_pack_events(eid.to(DEV), row.to(DEV), ne)
+    sizes = np.diff(o["pix_sample_off"])
+    assert sizes.max() > 300 and (sizes == 1).any()
+    for cap, seed in ((1, 0), (16, 20260915), (250, 7), (10 ** 9, 3), (16, 2 ** 63 + 5)):
+        gp, ge, gx = ctx.gwc_cap_pixels(p, cap, seed)
+        op, oe, ox = oracle.cap_pixels(o["perm"], o["ev_sample_off"], o["pix_sample_off"], cap, seed)
+        assert np.array_equal(_np(gp), op), (cap, seed)
+        assert np.array_equal(_np(ge), oe) and np.array_equal(_np(gx), ox)
+    assert np.array_equal(_np(p["perm"]), o["perm"])                        # the packed input was left untouched
+    p0 = ctx.gwc_pack_events(eid[:0].to(DEV), row[:0].to(DEV), 3)
+    k0, e0, x0 = ctx.gwc_cap_pixels(p0, 5, 1)
+    assert k0.numel() == 0 and _np(e0).tolist() == [0, 0, 0, 0]
+    with pytest.raises(gwc.GwcError):
+        ctx.gwc_cap_pixels(p, 0, 1)
+    # a capped catalogue through the hot path: pack + cap the tiny workload's samples, compare with the oracle
+    W = workload("tiny")
+    off = W.ev["ev_sample_off"]
+    ev_id = torch.repeat_interleave(torch.arange(off.numel() - 1, dtype=torch.int32), off[1:] - off[:-1])
+    pk = ctx.gwc_pack_events(ev_id.to(DEV), W.ev["sample_row"].to(DEV), off.numel() - 1)
+    keep, eso, _ = ctx.gwc_cap_pixels(pk, 20, 5)
+    kc = keep.cpu()
+    evc = dict(ev_sample_off=eso.cpu(), dL=W.ev["dL"][kc], m1z=W.ev["m1z"][kc], m2z=W.ev["m2z"][kc],
+               sample_row=W.ev["sample_row"][kc], log_pe_prior=None)
+    assert kc.numel() < W.ev["dL"].numel()
+    th = W.theta.to(DEV)
+    ctx.gwc_build_cosmo(th, W.spec.z_max, 1025, 0)
+    logL, _, nlive = ctx.gwc_event_loglik(th, to_dev(evc, DEV), W.los.to(DEV), W.spec.z_max)
+    oL, _, oK = oracle.event_loglik(_np(W.theta), synth.to_numpy(evc), _np(W.los), W.spec.z_max)
+    assert np.array_equal(_np(nlive), oK)
+    assert_close_log(_np(logL), oL, RTOL_F64, "capped catalogue log L_i")
