@@ -492,3 +492,36 @@ def test_cap_pixels_bit_exact(ctx):
     oL, _, oK = oracle.event_loglik(_np(W.theta), synth.to_numpy(evc), _np(W.los), W.spec.z_max)
     assert np.array_equal(_np(nlive), oK)
     assert_close_log(_np(logL), oL, RTOL_F64, "capped catalogue log L_i")
+
+
+def test_theta_batch_across_constant_bank_launches(ctx):
+    """The fused kernel takes its per-theta constants from the constant bank, 340 points per launch: a batch of 345
+    (one full launch + a 5-point one, tiles of 10 cut at 340) must match the oracle point by point."""
+    W = workload("tiny", n_theta=345)
+    o = _oracle_all(W, W.theta)
+    g = _gpu_all(ctx, W, W.theta)
+    ctx.gwc_check()
+    _compare(g, o)
+    # the same points evaluated in another grouping give the same bits (no dependence on the launch split)
+    th = W.theta.to(DEV)
+    ev, los = to_dev(W.ev, DEV), W.los.to(DEV)
+    sub = th[337:345].contiguous()
+    ctx.gwc_build_cosmo(sub, W.spec.z_max, 1025, 0)
+    logL_sub, _, _ = ctx.gwc_event_loglik(sub, ev, los, W.spec.z_max)
+    assert np.array_equal(_np(logL_sub), g["logL"][337:345], equal_nan=True)
+
+
+def test_kde_32bit_tables(ctx):
+    """KDE numerator with f32 LOS rows and the 32-bit cosmology table (R22): against the oracle on the same rounded
+    tables (a node on a rounding boundary may round apart: 1e-6), and within 1e-4 per event of the FP64 result."""
+    W = workload("o4", n_theta=8, n_events=6, los_rows=200, n_inj=500)
+    los32 = W.los.to(torch.float32)
+    g32, o32 = _kde_both(ctx, W, W.theta, los=los32, neff_min=2.0, prec=1)
+    same = g32[1] == o32[1]
+    assert same.mean() > 0.99
+    fin = same & np.isfinite(o32[0])
+    assert (np.abs(g32[0][fin] - o32[0][fin]) / np.maximum(np.abs(o32[0][fin]), 1.0)).max() <= 1e-6
+    g64, _ = _kde_both(ctx, W, W.theta, neff_min=2.0, prec=0)
+    both = (g32[1] == g64[1]) & np.isfinite(g64[0]) & np.isfinite(g32[0])
+    assert both.mean() > 0.9
+    assert np.abs(g32[0][both] - g64[0][both]).max() <= ATOL_F32
