@@ -194,6 +194,8 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.out_n = (int32_t*)ctx->part_n.p;
   p.out_np = pixcut ? (int32_t*)ctx->part_np.p : nullptr;
   p.pixcut = pixcut ? 1 : 0;
+  // events shorter on average than 2048 samples leave warps of a 16-warp CTA without a block: let them share it
+  p.teams = (!inj && !pixcut && n_seg > 0 && n / n_seg < 2048) ? 1 : 0;
   p.neff_min = neff_min;
   p.unit_counter = ctx->d_counter;
   cudaEvent_t e0 = nullptr, e1 = nullptr;

@@ -307,7 +307,8 @@ struct Sample {
   const RowT* lrow;
 };
 
-template <typename NodeT, typename LosT, bool INJ, bool PIX>
+// TEAMS: short segments share the CTA (chosen by the host for catalogues of short events; see launch_reweight)
+template <typename NodeT, typename LosT, bool INJ, bool PIX, bool TEAMS>
 __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
@@ -376,13 +377,33 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     __syncthreads();
 
     const int seg_lo = p.group_off[group], seg_hi = p.group_off[group + 1];
-    for (int seg = seg_lo; seg < seg_hi; ++seg) {
+    for (int seg0 = seg_lo; seg0 < seg_hi;) {
+      // Short segments share the CTA: when the next 2 (4) segments each fit one block per warp of a half (quarter) of
+      // the CTA, the halves (quarters) take one segment each, so that no warp idles through a segment with fewer
+      // blocks than the CTA has warps.
+      int sh = 0;  // log2 of the number of segments taken at once
+      if (TEAMS && seg0 + 2 <= seg_hi) {
+        const int64_t o0 = p.seg_off[seg0], o1 = p.seg_off[seg0 + 1], o2 = p.seg_off[seg0 + 2];
+        if (o1 - o0 <= (NWARPS / 2) * BLK && o2 - o1 <= (NWARPS / 2) * BLK) {
+          sh = 1;
+          if (seg0 + 4 <= seg_hi) {
+            const int64_t o3 = p.seg_off[seg0 + 3], o4 = p.seg_off[seg0 + 4];
+            if (o1 - o0 <= (NWARPS / 4) * BLK && o2 - o1 <= (NWARPS / 4) * BLK && o3 - o2 <= (NWARPS / 4) * BLK &&
+                o4 - o3 <= (NWARPS / 4) * BLK)
+              sh = 2;
+          }
+        }
+      }
+      const int nteam = 1 << sh;
+      const int tsz = NWARPS >> sh;            // warps per team
+      const int seg = seg0 + (warp / (NWARPS / 4) >> (2 - sh));   // this warp's segment
+      const int wt = warp & (tsz - 1);         // this warp inside its team
       const int64_t s0 = p.seg_off[seg], s1 = p.seg_off[seg + 1];
       // The segment's samples in blocks of BLK, dealt to the warps round-robin; no barrier until the segment ends.
       // Pixel-cut mode: each warp takes one contiguous range of whole blocks instead, so that the run a block
       // leaves open is continued by the same warp's next block; the pixels that cross from one warp's range
       // into the next are put together when the segment ends (lead / trail sums below).
-      int64_t w_lo = s0 + (int64_t)warp * BLK, w_hi = s1, w_step = (int64_t)NWARPS * BLK;
+      int64_t w_lo = s0 + (int64_t)wt * BLK, w_hi = s1, w_step = (int64_t)tsz * BLK;
       bool lead_open = true;  // no pixel start seen yet in this warp's range
       if (PIX) {
         const int64_t nb = (s1 - s0 + BLK - 1) / BLK;
@@ -551,19 +572,20 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       }
       __syncthreads();
       // segment complete: combine the warps' partials in a fixed order and write them out
-      if (tid < nt) {
+      if ((tid & 31) < nt && (tid >> 5) < nteam) {
+        const int team = tid >> 5, j = tid & 31;  // one thread per (segment of this round, theta)
         double a = 0.0, b = 0.0;
         int c = 0, np = 0;
-        for (int w = 0; w < NWARPS; ++w) {
-          a += s_acc[(w * T + tid) * 2];
-          b += s_acc[(w * T + tid) * 2 + 1];
-          c += s_cnt[w * T + tid];
-          s_acc[(w * T + tid) * 2] = 0.0;
-          s_acc[(w * T + tid) * 2 + 1] = 0.0;
-          s_cnt[w * T + tid] = 0;
+        for (int w = team * tsz; w < (team + 1) * tsz; ++w) {
+          a += s_acc[(w * T + j) * 2];
+          b += s_acc[(w * T + j) * 2 + 1];
+          c += s_cnt[w * T + j];
+          s_acc[(w * T + j) * 2] = 0.0;
+          s_acc[(w * T + j) * 2 + 1] = 0.0;
+          s_cnt[w * T + j] = 0;
           if (PIX) {
-            np += s_np[w * T + tid];
-            s_np[w * T + tid] = 0;
+            np += s_np[w * T + j];
+            s_np[w * T + j] = 0;
           }
         }
         if (PIX) {
@@ -572,9 +594,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           int oN = 0;
           for (int w = 0; w <= NWARPS; ++w) {
             if (w < NWARPS) {
-              oW += s_lead[(w * T + tid) * 2];
-              oQ += s_lead[(w * T + tid) * 2 + 1];
-              oN += s_leadn[w * T + tid];
+              oW += s_lead[(w * T + j) * 2];
+              oQ += s_lead[(w * T + j) * 2 + 1];
+              oN += s_leadn[w * T + j];
             }
             if (w == NWARPS || s_hashead[w]) {
               if (oW > 0.0 && oW * oW >= p.neff_min * oQ) {
@@ -584,41 +606,42 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
                 np += 1;
               }
               if (w < NWARPS) {
-                oW = s_carry[(w * T + tid) * 2];
-                oQ = s_carry[(w * T + tid) * 2 + 1];
-                oN = s_carryn[w * T + tid];
+                oW = s_carry[(w * T + j) * 2];
+                oQ = s_carry[(w * T + j) * 2 + 1];
+                oN = s_carryn[w * T + j];
               }
             }
             if (w < NWARPS) {
-              s_lead[(w * T + tid) * 2] = 0.0;
-              s_lead[(w * T + tid) * 2 + 1] = 0.0;
-              s_leadn[w * T + tid] = 0;
-              s_carry[(w * T + tid) * 2] = 0.0;
-              s_carry[(w * T + tid) * 2 + 1] = 0.0;
-              s_carryn[w * T + tid] = 0;
+              s_lead[(w * T + j) * 2] = 0.0;
+              s_lead[(w * T + j) * 2 + 1] = 0.0;
+              s_leadn[w * T + j] = 0;
+              s_carry[(w * T + j) * 2] = 0.0;
+              s_carry[(w * T + j) * 2 + 1] = 0.0;
+              s_carryn[w * T + j] = 0;
             }
           }
         }
-        const size_t o = (size_t)(p.t_begin + t0 + tid) * (size_t)p.n_seg + (size_t)seg;
+        const size_t o = (size_t)(p.t_begin + t0 + j) * (size_t)p.n_seg + (size_t)(seg0 + team);
         p.out_w[2 * o] = a;
         p.out_w[2 * o + 1] = b;
         p.out_n[o] = c;
         if (PIX) p.out_np[o] = np;
       }
       __syncthreads();  // the reset above precedes the next segment's accumulation
+      seg0 += nteam;
     }
   }
 }
 
-template <typename NodeT, typename LosT, bool INJ, bool PIX = false>
+template <typename NodeT, typename LosT, bool INJ, bool PIX = false, bool TEAMS = false>
 int launch_one(const ReweightParams& p, int n_blocks, size_t smem, cudaStream_t s) {
-  reweight_kernel<NodeT, LosT, INJ, PIX><<<n_blocks, NTHREADS, smem, s>>>(p);
+  reweight_kernel<NodeT, LosT, INJ, PIX, TEAMS><<<n_blocks, NTHREADS, smem, s>>>(p);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-template <typename NodeT, typename LosT, bool INJ, bool PIX = false>
+template <typename NodeT, typename LosT, bool INJ, bool PIX = false, bool TEAMS = false>
 int configure_one(int smem_optin) {
-  return cudaFuncSetAttribute(reweight_kernel<NodeT, LosT, INJ, PIX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  return cudaFuncSetAttribute(reweight_kernel<NodeT, LosT, INJ, PIX, TEAMS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               smem_optin) == cudaSuccess ? 0 : -1;
 }
 
@@ -646,6 +669,10 @@ int reweight_configure(int smem_optin) {
   rc |= configure_one<Node64, float, false, true>(smem_optin);
   rc |= configure_one<Node32, double, false, true>(smem_optin);
   rc |= configure_one<Node32, float, false, true>(smem_optin);
+  rc |= configure_one<Node64, double, false, false, true>(smem_optin);
+  rc |= configure_one<Node64, float, false, false, true>(smem_optin);
+  rc |= configure_one<Node32, double, false, false, true>(smem_optin);
+  rc |= configure_one<Node32, float, false, false, true>(smem_optin);
   rc |= configure_one<Node64, double, true>(smem_optin);
   rc |= configure_one<Node32, double, true>(smem_optin);
   return rc;
@@ -680,6 +707,13 @@ int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_pr
       else
         rc = los_prec == GWC_F64 ? launch_one<Node32, double, false, true>(p, n_blocks, smem, s)
                                  : launch_one<Node32, float, false, true>(p, n_blocks, smem, s);
+    } else if (p.teams) {
+      if (tab_prec == GWC_F64)
+        rc = los_prec == GWC_F64 ? launch_one<Node64, double, false, false, true>(p, n_blocks, smem, s)
+                                 : launch_one<Node64, float, false, false, true>(p, n_blocks, smem, s);
+      else
+        rc = los_prec == GWC_F64 ? launch_one<Node32, double, false, false, true>(p, n_blocks, smem, s)
+                                 : launch_one<Node32, float, false, false, true>(p, n_blocks, smem, s);
     } else if (tab_prec == GWC_F64) {
       rc = los_prec == GWC_F64 ? launch_one<Node64, double, false>(p, n_blocks, smem, s)
                                : launch_one<Node64, float, false>(p, n_blocks, smem, s);
