@@ -52,8 +52,9 @@ __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_byt
   SmemLayout L;
   size_t o = 0;
   L.math = o;   o = align16(o + sizeof(MathTables));
-  L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2);
-  L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T);
+  // (two sets of sums unless pixel-cut mode: a warp may start the next segment while the slowest finish this one)
+  L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2 * (pix ? 1 : 2));
+  L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T * (pix ? 1 : 2));
   // pixel-cut mode only: passing pixels; the run a block leaves open (W, Q, n); the run open at the range start
   L.np = o;     o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
   L.carry = o;  o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 : 0));
@@ -310,6 +311,11 @@ struct Sample {
 // TEAMS: short segments share the CTA (chosen by the host for catalogues of short events; see launch_reweight)
 template <typename NodeT, typename LosT, bool INJ, bool PIX, bool TEAMS>
 __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightParams p) {
+  // ASYNC: no barrier between segments.  The sums of consecutive segments go to alternating buffers; the last warp to
+  // finish a segment combines it (fixed warp order) while the others are already on the next one, and the blocks are
+  // dealt round-robin across segment boundaries, so the warps' loads even out over the group.
+  constexpr bool ASYNC = !PIX && !TEAMS;
+  constexpr int NBUF = PIX ? 1 : 2;
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
   typedef typename std::conditional<INJ, double, LosT>::type RowT;  // the all-sky table is f64
@@ -322,6 +328,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   int* s_carryn = reinterpret_cast<int*>(smem + L.carryn);
   double* s_lead = reinterpret_cast<double*>(smem + L.lead);
   int* s_leadn = reinterpret_cast<int*>(smem + L.leadn);
+  __shared__ int s_arrive[2], s_done;  // ASYNC: warps that finished a segment (per buffer), segments combined so far
   __shared__ int s_hashead[NWARPS];  // pixel-cut mode: the warp's range of the current segment contains a pixel start
   double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
   NodeT* s_tab = reinterpret_cast<NodeT*>(smem + L.tab);
@@ -361,8 +368,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       for (int i = tid; i < n16; i += NTHREADS) dst[i] = src[i];
       cur_tile = tile;
     }
-    for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) s_acc[i] = 0.0;
-    for (int i = tid; i < NWARPS * T; i += NTHREADS) s_cnt[i] = 0;
+    for (int i = tid; i < NWARPS * T * 2 * NBUF; i += NTHREADS) s_acc[i] = 0.0;
+    for (int i = tid; i < NWARPS * T * NBUF; i += NTHREADS) s_cnt[i] = 0;
+    if (tid == 0) {
+      s_arrive[0] = 0;
+      s_arrive[1] = 0;
+      s_done = 0;
+    }
+    int rot = 0;  // ASYNC: the warp that takes the first block of the current segment
     if (PIX) {
       for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) {
         s_carry[i] = 0.0;
@@ -399,11 +412,22 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       const int seg = seg0 + (warp / (NWARPS / 4) >> (2 - sh));   // this warp's segment
       const int wt = warp & (tsz - 1);         // this warp inside its team
       const int64_t s0 = p.seg_off[seg], s1 = p.seg_off[seg + 1];
+      const int sidx = seg0 - seg_lo;
+      const int buf = ASYNC ? (sidx & 1) : 0;
+      double* acc_b = s_acc + buf * (NWARPS * T * 2);
+      int* cnt_b = s_cnt + buf * (NWARPS * T);
+      if (ASYNC && sidx >= 2) {
+        // this buffer last held segment sidx-2: wait until it has been combined and cleared
+        while (*(volatile int*)&s_done < sidx - 1) {
+        }
+        __threadfence_block();  // the cleared buffer is seen after the release
+      }
       // The segment's samples in blocks of BLK, dealt to the warps round-robin; no barrier until the segment ends.
       // Pixel-cut mode: each warp takes one contiguous range of whole blocks instead, so that the run a block
       // leaves open is continued by the same warp's next block; the pixels that cross from one warp's range
       // into the next are put together when the segment ends (lead / trail sums below).
-      int64_t w_lo = s0 + (int64_t)wt * BLK, w_hi = s1, w_step = (int64_t)tsz * BLK;
+      int64_t w_lo = s0 + (int64_t)(ASYNC ? ((warp - rot) & (NWARPS - 1)) : wt) * BLK, w_hi = s1, w_step = (int64_t)tsz * BLK;
+      if (ASYNC) rot = (rot + (int)((s1 - s0 + BLK - 1) / BLK)) & (NWARPS - 1);
       bool lead_open = true;  // no pixel start seen yet in this warp's range
       if (PIX) {
         const int64_t nb = (s1 - s0 + BLK - 1) / BLK;
@@ -528,9 +552,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               if ((lane & 7) == 0) {
                 const int j = (lane & 16) ? jb : ja;
                 if (j >= 0) {
-                  s_acc[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
+                  acc_b[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
                   if ((lane & 8) == 0) {
-                    s_cnt[warp * T + j] += (lane & 16) ? cntb : cnt;
+                    cnt_b[warp * T + j] += (lane & 16) ? cntb : cnt;
                     s_np[warp * T + j] += (lane & 16) ? npb : npa;
                   }
                 }
@@ -545,8 +569,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               if ((lane & 7) == 0) {
                 const int j = (lane & 16) ? jb : ja;
                 if (j >= 0) {
-                  s_acc[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
-                  if ((lane & 8) == 0) s_cnt[warp * T + j] += (lane & 16) ? (cnt >> 16) : (cnt & 0xffff);
+                  acc_b[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
+                  if ((lane & 8) == 0) cnt_b[warp * T + j] += (lane & 16) ? (cnt >> 16) : (cnt & 0xffff);
                 }
               }
             }
@@ -570,9 +594,45 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         }
         if (lane == 0) s_hashead[warp] = lead_open ? 0 : 1;
       }
+      if (ASYNC) {
+        __syncwarp();
+        int last = 0;
+        if (lane == 0) {
+          __threadfence_block();  // this warp's sums before its arrival
+          last = atomicAdd(&s_arrive[buf], 1) == NWARPS - 1;
+        }
+        last = __shfl_sync(FULL, last, 0);
+        if (last) {  // every warp has arrived: this one combines the segment, in warp order, and clears the buffer
+          __threadfence_block();
+          if (lane < nt) {
+            double a = 0.0, b = 0.0;
+            int c = 0;
+            for (int w = 0; w < NWARPS; ++w) {
+              a += *(volatile double*)&acc_b[(w * T + lane) * 2];
+              b += *(volatile double*)&acc_b[(w * T + lane) * 2 + 1];
+              c += *(volatile int*)&cnt_b[w * T + lane];
+              acc_b[(w * T + lane) * 2] = 0.0;
+              acc_b[(w * T + lane) * 2 + 1] = 0.0;
+              cnt_b[w * T + lane] = 0;
+            }
+            const size_t o = (size_t)(p.t_begin + t0 + lane) * (size_t)p.n_seg + (size_t)seg;
+            p.out_w[2 * o] = a;
+            p.out_w[2 * o + 1] = b;
+            p.out_n[o] = c;
+          }
+          __syncwarp();
+          if (lane == 0) {
+            s_arrive[buf] = 0;
+            __threadfence_block();  // the cleared buffer before the release
+            atomicAdd(&s_done, 1);
+          }
+        }
+        seg0 += 1;
+        continue;
+      }
       __syncthreads();
       // segment complete: combine the warps' partials in a fixed order and write them out
-      if ((tid & 31) < nt && (tid >> 5) < nteam) {
+      if ((tid & 31) < nt && (tid >> 5) < nteam) {  // (acc_b = s_acc here: one buffer)
         const int team = tid >> 5, j = tid & 31;  // one thread per (segment of this round, theta)
         double a = 0.0, b = 0.0;
         int c = 0, np = 0;
