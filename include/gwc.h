@@ -207,6 +207,16 @@ gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
                             double* d_logL_total);
 
 /*
+ * The paper's likelihood in one call: Eq. 5 with the KDE numerator (gwc_event_loglik_kde: n_grid, neff_min), the
+ * per-pixel cut of Eq. 8 and the selection term of Eq. 4:  build_cosmo(z_max = los->z_max, n_nodes, table_prec),
+ * the KDE event term, gwc_selection_logxi, gwc_combine_total.  Same arguments, errors and NaN / -inf rules as
+ * gwc_total_loglik; synchronises the stream once (gwc_event_loglik_kde).
+ */
+gwc_status gwc_total_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                                const gwc_injections* inj, const gwc_los* los, int32_t n_nodes, gwc_prec table_prec,
+                                int32_t n_grid, double neff_min, double* d_logL_total /* [n_theta] */);
+
+/*
  * Same as gwc_total_loglik but every pointer (inside the structs too) is a HOST pointer: the call
  * uploads theta, the catalogue, the injections and the LOS table (computing the all-sky mean on the
  * device when los->allsky is NULL), runs A1..A6 and downloads h_logL_total, then synchronises.

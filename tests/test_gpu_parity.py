@@ -525,3 +525,21 @@ def test_kde_32bit_tables(ctx):
     both = (g32[1] == g64[1]) & np.isfinite(g64[0]) & np.isfinite(g32[0])
     assert both.mean() > 0.9
     assert np.abs(g32[0][both] - g64[0][both]).max() <= ATOL_F32
+
+
+def test_total_loglik_kde_composition(ctx):
+    """gwc_total_loglik_kde = KDE event term + selection term + A6, against the oracle's pieces."""
+    W = workload("tiny")
+    zmax = W.spec.z_max
+    th, ev, inj, los = W.theta.to(DEV), to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    tot = _np(ctx.gwc_total_loglik_kde(th, ev, inj, los, zmax, allsky, 256, 2.0))
+    ctx.gwc_check()
+    oL, _ = oracle.event_loglik_kde(_np(W.theta), synth.to_numpy(W.ev), _np(W.los), zmax, n_grid=256, neff_min=2.0)
+    oX, _ = oracle.selection_logxi(_np(W.theta), synth.to_numpy(W.inj), oracle.los_allsky(_np(W.los), zmax), zmax)
+    assert_close_log(tot, oracle.total_from_parts(oL, oX), RTOL_F64, "log L(theta), KDE numerator")
+    # composed calls give the same bits
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    gL, _, _ = ctx.gwc_event_loglik_kde(th, ev, los, zmax, 256, 2.0)
+    gX, _ = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], zmax)
+    assert np.array_equal(_np(ctx.gwc_combine_total(gL, gX)), tot, equal_nan=True)
