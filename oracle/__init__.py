@@ -65,7 +65,7 @@ def lib():
             "orc_lse": (None, [vp, i64, vp, vp]),
             "orc_event_loglik": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, vp, vp, vp]),
             "orc_event_loglik_pixcut": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, d, vp, vp, vp, vp]),
-            "orc_event_loglik_kde": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, C.c_int, d, vp, vp, vp]),
+            "orc_event_loglik_kde": (C.c_int, [vp, i64, vp, vp, C.c_int, d, C.c_int, C.c_int, C.c_int, d, C.c_int, vp, vp, vp]),
             "orc_kde_samples": (C.c_int, [vp, vp, i64, d, C.c_int, d, C.c_int, vp, vp]),
             "orc_selection_logxi": (C.c_int, [vp, i64, vp, vp, i32, d, C.c_int, d, C.c_int, C.c_int, vp, vp]),
             "orc_total_from_parts": (None, [vp, vp, i64, i64, vp]),
@@ -210,7 +210,7 @@ def _events_struct(ev):
 
 
 def event_loglik_kde(theta, ev, los_table, los_z_max, *, n_grid=256, neff_min=0.0, mode=TABLE, z_max=None,
-                     n_nodes=1025, table_prec=0, want_nused=False):
+                     n_nodes=1025, table_prec=0, want_nused=False, bandwidth="scott"):
     """Event term with the paper's KDE numerator (Eq. 5-7, D1; R26-R30).  Returns logL (f64) and npass
     (int64), both [n_theta, n_events]."""
     th = _theta(theta)
@@ -221,7 +221,8 @@ def event_loglik_kde(theta, ev, los_table, los_z_max, *, n_grid=256, neff_min=0.
     nused = np.empty((nt, ne), dtype=np.int64)
     zm = float(los_z_max if z_max is None else z_max)
     rc = lib().orc_event_loglik_kde(_p(th), nt, C.addressof(es), C.addressof(ls), mode, zm, n_nodes, table_prec,
-                                    int(n_grid), float(neff_min), _p(logL), _p(npass), _p(nused))
+                                    int(n_grid), float(neff_min), {"scott": 0, "silverman": 1}[bandwidth], _p(logL),
+                                    _p(npass), _p(nused))
     assert rc == 0
     if want_nused:
         return logL, npass, nused

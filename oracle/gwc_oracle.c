@@ -610,8 +610,25 @@ int orc_kde_samples(const double* th, const orc_events* ev, int64_t n_rows, doub
  * log L_i(theta) with the KDE numerator, for every (theta, event); npass = pixels that contributed.
  * n_grid = G (>= 2).  Outputs [n_theta][n_events].
  */
+static int dbl_cmp(const void* a, const void* b) {
+  double x = *(const double*)a, y = *(const double*)b;
+  return x < y ? -1 : (x > y ? 1 : 0);
+}
+
+/* q-quantile of sorted x[0..n-1] by linear interpolation between the order statistics at q (n-1) (the "linear"
+ * definition: numpy's default) */
+static double quantile_sorted(const double* x, int64_t n, double q) {
+  double pos = q * (double)(n - 1);
+  int64_t lo = (int64_t)floor(pos);
+  if (lo >= n - 1) return x[n - 1];
+  double f = pos - (double)lo;
+  return x[lo] + f * (x[lo + 1] - x[lo]);
+}
+
+/* bw_rule: 0 = Scott, Eq. D1; 1 = Silverman, Eq. D2:
+ * h = 0.9 min(sigma, IQR / 1.34) n^(-1/5) with the IQR of the pixel's live z_k (plain quantiles, reading R32). */
 int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events* ev, const orc_los* L, int mode,
-                         double z_max, int M, int table_prec, int n_grid, double neff_min, double* logL,
+                         double z_max, int M, int table_prec, int n_grid, double neff_min, int bw_rule, double* logL,
                          int64_t* npass, int64_t* nused) {
   int err = 0;
   int64_t smax = 0;
@@ -681,6 +698,17 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
           double Vd = (double)V, Qd = (double)Q;
           if (var > 0.0 && Vd * Vd >= neff_min * Qd) {
             double h = 1.06 * sqrt(var) * pow((double)n, -0.2);            /* Eq. D1 */
+            if (bw_rule == 1) {                                              /* Eq. D2 */
+              int64_t c = 0;
+              for (int64_t k = r0; k < r1; ++k)
+                if (lv[k - a] > -INFINITY) lI[np + c++] = zz[k - a];          /* (free tail of lI as a work area) */
+              qsort(lI + np, (size_t)c, sizeof(double), dbl_cmp);
+              double iqr = quantile_sorted(lI + np, c, 0.75) - quantile_sorted(lI + np, c, 0.25);
+              double spread = sqrt(var);
+              if (iqr / 1.34 < spread) spread = iqr / 1.34;
+              h = 0.9 * spread * pow((double)n, -0.2);
+              if (!(h > 0.0)) { r0 = r1; continue; }                          /* IQR = 0: no bandwidth, no contribution */
+            }
             double norm = 1.0 / (h * sqrt(2.0 * M_PI));
             long double I = 0.0L;
             for (int g = 0; g < n_grid; ++g) {

@@ -728,3 +728,37 @@ def test_cap_pixels_against_numpy_lexsort():
             keep[a + order[:cap]] = True
     got = O.cap_pixels(P["perm"], P["ev_sample_off"], pso, cap, seed)[0]
     assert np.array_equal(got, P["perm"][keep])
+
+
+def test_kde_silverman_bandwidth_through_quadratic_prior(theta0):
+    # Eq. D2: h = 0.9 min(sigma, IQR / 1.34) n^(-1/5); the z^2 prior exposes it as for Scott's rule.  numpy's
+    # percentile (linear interpolation) is the independent IQR; both branches of the min occur in the toy.
+    ev = _kde_event(n=260, seed=4, rows=5)
+    rng = np.random.default_rng(5)
+    far = rng.choice(260, 12, replace=False)              # outliers: sigma inflates, the IQR does not
+    ev["dL"][far] *= 1.6
+    zmax, nz = 1.5, 4096
+    zb = np.linspace(0, zmax, nz)
+    tab = np.tile(zb ** 2, (5, 1))
+    th = _theta_unit_rate(theta0)
+    z, lv = O.kde_samples(th, ev, 5, zmax)
+    assert np.all(np.isfinite(lv))
+    Lk, _ = O.event_loglik_kde(th, ev, tab, zmax, n_grid=256, bandwidth="silverman")
+    Ls, _ = O.event_loglik_kde(th, ev, tab, zmax, n_grid=256, bandwidth="scott")
+    off = ev["ev_sample_off"]
+    used_iqr = used_sigma = 0
+    for i, runs in enumerate(_pixel_runs(ev)):
+        tot = 0.0
+        for r0, r1 in runs:
+            v, zz = np.exp(lv[r0:r1]), z[r0:r1]
+            mu = np.sum(v * zz) / np.sum(v)
+            sig = math.sqrt(np.sum(v * (zz - mu) ** 2) / np.sum(v))
+            q1, q3 = np.percentile(zz, [25, 75])
+            used_iqr += (q3 - q1) / 1.34 < sig
+            used_sigma += (q3 - q1) / 1.34 >= sig
+            h = 0.9 * min(sig, (q3 - q1) / 1.34) * zz.size ** (-0.2)
+            tot += np.sum(v * (zz ** 2 + h * h))
+        want = math.log(tot / (off[i + 1] - off[i]))
+        assert Lk[0, i] == pytest.approx(want, abs=2e-6)
+        assert abs(Ls[0, i] - Lk[0, i]) > 1e-4            # and it is not Scott's bandwidth
+    assert used_iqr > 0 and used_sigma > 0
