@@ -54,6 +54,8 @@ typedef enum {
 } gwc_status;
 
 typedef enum { GWC_F64 = 0, GWC_F32 = 1 } gwc_prec;
+/* bandwidth rule of the KDE numerator: Scott, Eq. D1 (the paper's default) | Silverman, Eq. D2 (:300) */
+typedef enum { GWC_BW_SCOTT = 0, GWC_BW_SILVERMAN = 1 } gwc_bw_rule;
 
 typedef struct gwc_ctx gwc_ctx;
 
@@ -172,7 +174,9 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
  * (Eq. 5-7; Scott bandwidth Eq. D1; n_grid = 256 fiducial, PAPER.md:213;
  * DESIGN.md R26-R30).  Pixels as in gwc_event_loglik_pixcut.  For pixel j:
  *   v_k = p(m1, m2 | theta) / (J pi_PE)  (Eq. 7 without the redshift prior),  n_j = its live samples,
- *   h_j = 1.06 sigma_j n_j^(-1/5) with sigma_j the v-weighted standard deviation of the z_k,
+ *   h_j = 1.06 sigma_j n_j^(-1/5) with sigma_j the v-weighted standard deviation of the z_k (bw_rule = GWC_BW_SCOTT),
+ *         or 0.9 min(sigma_j, IQR_j / 1.34) n_j^(-1/5) with the interquartile range of the live z_k, plain quantiles
+ *         by linear interpolation (GWC_BW_SILVERMAN; R32),
  *   I_j = trapezoid over the n_grid-node uniform grid on [0, los->z_max] of
  *         [sum_k v_k N(z; z_k, h_j)] p_los(z | row_j) psi(z) / (1+z),
  *   log L_i = log( (1/S_i) sum_j I_j )  over the pixels with n_j >= 2, sigma_j > 0 and N_eff,j >= neff_min.
@@ -183,7 +187,7 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
  * Synchronises the stream once (the longest event sizes a scratch buffer).
  */
 gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
-                                const gwc_los* los, int32_t n_grid, double neff_min, double* d_logL,
+                                const gwc_los* los, int32_t n_grid, double neff_min, int32_t bw_rule, double* d_logL,
                                 int64_t* d_npass, int64_t* d_nused);
 
 /*
@@ -214,7 +218,7 @@ gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
  */
 gwc_status gwc_total_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                                 const gwc_injections* inj, const gwc_los* los, int32_t n_nodes, gwc_prec table_prec,
-                                int32_t n_grid, double neff_min, double* d_logL_total /* [n_theta] */);
+                                int32_t n_grid, double neff_min, int32_t bw_rule, double* d_logL_total /* [n_theta] */);
 
 /*
  * Same as gwc_total_loglik but every pointer (inside the structs too) is a HOST pointer: the call

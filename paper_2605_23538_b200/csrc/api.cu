@@ -429,12 +429,13 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
 }
 
 gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
-                                const gwc_los* los, int32_t n_grid, double neff_min, double* d_logL,
+                                const gwc_los* los, int32_t n_grid, double neff_min, int32_t bw_rule, double* d_logL,
                                 int64_t* d_npass, int64_t* d_nused) {
   GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
   if (!ev || !d_logL) return fail(ctx, GWC_ERR_INVALID_ARG, "ev or d_logL is NULL");
   if (!(neff_min >= 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "neff_min must be >= 0");
   if (n_grid < 2 || n_grid > 256) return fail(ctx, GWC_ERR_SHAPE, "n_grid must be in [2, 256]");
+  if (bw_rule != GWC_BW_SCOTT && bw_rule != GWC_BW_SILVERMAN) return fail(ctx, GWC_ERR_INVALID_ARG, "unknown bw_rule");
   GWC_TRY(check_los(ctx, los, true, false));
   if (ev->n_events < 0 || ev->n_samples < 0 || ev->n_events > 0x7fffffffLL)
     return fail(ctx, GWC_ERR_SHAPE, "event / sample counts out of range");
@@ -474,7 +475,8 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   GWC_TRY(count(ctx, launch_kde(d_theta, ctx->tab.p, (const double*)ctx->tconst.p, n_theta, ctx->M, ctx->Mp,
                                 ctx->tab_prec, ctx->z_max / NODE32_QMAX, ev->n_events, ev->ev_sample_off, ev->dL,
                                 ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->seg_shift.p,
-                                los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, d_logL,
+                                los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, bw_rule,
+                                d_logL,
                                 d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, s),
                 "kde"));
   if (ctx->timing) {
@@ -534,7 +536,7 @@ gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
 
 gwc_status gwc_total_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                                 const gwc_injections* inj, const gwc_los* los, int32_t n_nodes, gwc_prec table_prec,
-                                int32_t n_grid, double neff_min, double* d_logL_total) {
+                                int32_t n_grid, double neff_min, int32_t bw_rule, double* d_logL_total) {
   GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
   if (!ev || !inj || !d_logL_total) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL argument");
   GWC_TRY(check_los(ctx, los, true, true));
@@ -542,8 +544,8 @@ gwc_status gwc_total_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   const int64_t E = ev->n_events;
   GWC_TRY(ensure(ctx, ctx->logL, (size_t)n_theta * (size_t)(E > 0 ? E : 1) * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->logxi, (size_t)n_theta * sizeof(double)));
-  GWC_TRY(gwc_event_loglik_kde(ctx, d_theta, n_theta, ev, los, n_grid, neff_min, (double*)ctx->logL.p, nullptr,
-                               nullptr));
+  GWC_TRY(gwc_event_loglik_kde(ctx, d_theta, n_theta, ev, los, n_grid, neff_min, bw_rule, (double*)ctx->logL.p,
+                               nullptr, nullptr));
   GWC_TRY(gwc_selection_logxi(ctx, d_theta, n_theta, inj, los, (double*)ctx->logxi.p, nullptr));
   return gwc_combine_total(ctx, (const double*)ctx->logL.p, (const double*)ctx->logxi.p, n_theta, E, d_logL_total);
 }

@@ -125,7 +125,7 @@ int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
-               double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s);
+               int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s);
 int kde_grid_blocks(int64_t n_theta, int64_t n_events, int n_sm);
 size_t kde_scratch_bytes(int n_blocks, int64_t max_event_len);
 int launch_max_segment(const int64_t* seg_off, int64_t n_seg, int64_t* d_out, cudaStream_t s);

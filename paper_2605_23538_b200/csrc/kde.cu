@@ -48,6 +48,7 @@ struct KdeParams {
   double los_zmax;
   int n_grid;
   double neff_min;
+  int bw_rule;              // 0 = Scott (Eq. D1), 1 = Silverman (Eq. D2)
   double2* scr;             // [resident warps][scr_stride]: (z_k, v_k) of the event a warp is working on (v < 0: dead)
   int64_t scr_stride;       // >= the longest event
   double* logL;             // [n_theta][n_events]
@@ -111,6 +112,58 @@ __device__ __noinline__ double sample_lv(const ThetaK& K, const NodeT* tab, int 
   const double J = x * x * K.cH * (u / x + x / E);
   z_out = z;
   return log(p1) + log(p2) - log(J) - lpi;
+}
+
+// ---- order statistics of a pixel's live redshifts (Silverman's rule, Eq. D2) --------------------------------------
+// k-th smallest (0-based) of the live z of scr[r0..r1): bisection on the bit pattern (positive doubles order like
+// their bits), one counting pass per bit; exact, every lane returns the same value.
+__device__ double kth_live_z(const double2* scr, int64_t r0, int64_t r1, int64_t k, int lane) {
+  unsigned long long prefix = 0;
+  for (int bit = 62; bit >= 0; --bit) {
+    const unsigned long long cand = prefix | (1ull << bit);
+    int cnt = 0;
+    for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+      const int64_t i = c0 + lane;
+      if (i < r1) {
+        const double2 zv = scr[i];
+        cnt += (zv.y >= 0.0 && (unsigned long long)__double_as_longlong(zv.x) < cand) ? 1 : 0;
+      }
+    }
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if ((int64_t)cnt <= k) prefix = cand;
+  }
+  return __longlong_as_double((long long)prefix);
+}
+
+// the order statistic after x = the k-th one: x again when it is repeated, else the smallest live z above it
+__device__ double next_live_z(const double2* scr, int64_t r0, int64_t r1, int64_t k, double x, int lane) {
+  int le = 0;
+  double up = CUDART_INF;
+  for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+    const int64_t i = c0 + lane;
+    if (i < r1) {
+      const double2 zv = scr[i];
+      if (zv.y >= 0.0) {
+        le += zv.x <= x ? 1 : 0;
+        up = zv.x > x ? fmin(up, zv.x) : up;
+      }
+    }
+  }
+  le = __reduce_add_sync(0xffffffffu, le);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) up = fmin(up, __shfl_xor_sync(0xffffffffu, up, o));
+  return (int64_t)le >= k + 2 ? x : up;
+}
+
+// q-quantile of the n live z by linear interpolation between the order statistics at q (n - 1)
+__device__ double live_quantile(const double2* scr, int64_t r0, int64_t r1, int64_t n, double q, int lane) {
+  const double pos = q * (double)(n - 1);
+  const int64_t lo = (int64_t)floor(pos);
+  if (lo >= n - 1) return kth_live_z(scr, r0, r1, n - 1, lane);
+  const double f = pos - (double)lo;
+  const double x0 = kth_live_z(scr, r0, r1, lo, lane);
+  const double x1 = next_live_z(scr, r0, r1, lo, x0, lane);
+  return x0 + f * (x1 - x0);
 }
 
 template <typename NodeT, typename LosT>
@@ -242,6 +295,13 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         const double var = S2 / V;
         pass = var > 0.0;
         h = 1.06 * sqrt(var) * pow((double)n, -0.2);   // Eq. D1
+        if (pass && p.bw_rule == 1) {                  // Eq. D2
+          const double iqr = live_quantile(scr, r0, r1, n, 0.75, lane) - live_quantile(scr, r0, r1, n, 0.25, lane);
+          double spread = sqrt(var);
+          spread = iqr / 1.34 < spread ? iqr / 1.34 : spread;
+          h = 0.9 * spread * pow((double)n, -0.2);
+          pass = h > 0.0;
+        }
       }
       if (pass) {
         // ---- pass 3: the KDE on the grid; lanes are grid nodes, samples handed round 32 at a time ----
@@ -309,13 +369,13 @@ int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
-               double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
+               int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
   if (n_theta <= 0 || n_events <= 0) return 0;
   KdeParams p;
   p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.n_theta = n_theta; p.n_events = n_events;
   p.M = M; p.Mp = Mp; p.tab_zq = tab_zq; p.ev_off = ev_off; p.dL = dL; p.m1z = m1z; p.m2z = m2z; p.lprior = lprior;
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
-  p.n_grid = n_grid; p.neff_min = neff_min; p.logL = logL; p.npass = npass; p.nused = nused;
+  p.n_grid = n_grid; p.neff_min = neff_min; p.bw_rule = bw_rule; p.logL = logL; p.npass = npass; p.nused = nused;
   p.scr = (double2*)scratch; p.scr_stride = scr_stride;
   const size_t smem = sizeof(MathTables) + sizeof(double) * KDE_WARPS * 32 * KDE_NPL;
   const int64_t blocks = n_blocks;

@@ -29,6 +29,9 @@ EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_laun
            "gwc_probe_fp64", "gwc_math_selftest"]
 
 
+BW_RULES = {"scott": 0, "silverman": 1}
+
+
 class GwcError(RuntimeError):
     def __init__(self, status: int, text: str):
         super().__init__("%s: %s" % (_STATUS[status] if 0 <= status < len(_STATUS) else status, text))
@@ -77,12 +80,12 @@ def load():
         "gwc_los_allsky": (ci, [vp, C.POINTER(Los), vp]),
         "gwc_event_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), vp, vp, vp]),
         "gwc_event_loglik_pixcut": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), dbl, vp, vp, vp, vp]),
-        "gwc_event_loglik_kde": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), i32, dbl, vp, vp, vp]),
+        "gwc_event_loglik_kde": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Los), i32, dbl, i32, vp, vp, vp]),
         "gwc_selection_logxi": (ci, [vp, vp, i64, C.POINTER(Injections), C.POINTER(Los), vp, vp]),
         "gwc_combine_total": (ci, [vp, vp, vp, i64, i64, vp]),
         "gwc_total_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci, vp]),
         "gwc_total_loglik_kde": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci, i32,
-                                      dbl, vp]),
+                                      dbl, i32, vp]),
         "gwc_total_loglik_host": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci,
                                        vp, C.POINTER(i64), C.POINTER(i64)]),
         "gwc_set_timing": (ci, [vp, ci]),
@@ -247,7 +250,7 @@ class Context:
                                                    nlive.data_ptr(), npass.data_ptr()))
         return logL, neff, nlive, npass
 
-    def gwc_event_loglik_kde(self, theta, ev, table, z_max, n_grid=256, neff_min=0.0):
+    def gwc_event_loglik_kde(self, theta, ev, table, z_max, n_grid=256, neff_min=0.0, bandwidth="scott"):
         """Event term with the paper's KDE numerator (Eq. 5-7, D1): returns logL, npass, nused."""
         nt, ne = theta.shape[0], ev["ev_sample_off"].numel() - 1
         logL = torch.empty((nt, ne), dtype=torch.float64, device=self.device)
@@ -255,8 +258,8 @@ class Context:
         nused = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
         es, los = make_events(ev), make_los(table, z_max)
         self._ck(self._lib.gwc_event_loglik_kde(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(los),
-                                                int(n_grid), float(neff_min), logL.data_ptr(), npass.data_ptr(),
-                                                nused.data_ptr()))
+                                                int(n_grid), float(neff_min), BW_RULES[bandwidth], logL.data_ptr(),
+                                                npass.data_ptr(), nused.data_ptr()))
         return logL, npass, nused
 
     def gwc_selection_logxi(self, theta, inj, allsky, n_z, z_max, want_neff=True):
@@ -286,14 +289,14 @@ class Context:
         return out
 
     def gwc_total_loglik_kde(self, theta, ev, inj, table, z_max, allsky, n_grid=256, neff_min=2.0, n_nodes=1025,
-                             table_prec=F64):
+                             table_prec=F64, bandwidth="scott"):
         """The paper's likelihood in one call: KDE numerator + per-pixel N_eff cut + selection term."""
         nt = theta.shape[0]
         out = torch.empty(nt, dtype=torch.float64, device=self.device)
         es, js, los = make_events(ev), make_injections(inj), make_los(table, z_max, allsky)
         self._ck(self._lib.gwc_total_loglik_kde(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(js),
                                                 C.byref(los), n_nodes, table_prec, int(n_grid), float(neff_min),
-                                                out.data_ptr()))
+                                                BW_RULES[bandwidth], out.data_ptr()))
         return out
 
     def gwc_total_loglik_host(self, theta, ev, inj, table, z_max, allsky=None, n_nodes=1025, table_prec=F64, out=None):

@@ -372,16 +372,16 @@ def test_pixcut_edge_cases_and_32bit_tables(ctx):
 
 
 # ---- NEXT row 1: the paper's KDE numerator (Eq. 5-7, D1; R26-R30) -------------------------------------
-def _kde_both(ctx, W, theta, ev=None, los=None, n_grid=256, neff_min=0.0, prec=0):
+def _kde_both(ctx, W, theta, ev=None, los=None, n_grid=256, neff_min=0.0, prec=0, bandwidth="scott"):
     ev = W.ev if ev is None else ev
     los = W.los if los is None else los
     zmax = W.spec.z_max
     th = theta.to(DEV)
     ctx.gwc_build_cosmo(th, zmax, 1025, prec)
-    gL, gP, gU = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), los.to(DEV), zmax, n_grid, neff_min)
+    gL, gP, gU = ctx.gwc_event_loglik_kde(th, to_dev(ev, DEV), los.to(DEV), zmax, n_grid, neff_min, bandwidth)
     ctx.gwc_check()
     oL, oP, oU = oracle.event_loglik_kde(_np(theta), synth.to_numpy(ev), _np(los), zmax, n_grid=n_grid,
-                                         neff_min=neff_min, table_prec=prec, want_nused=True)
+                                         neff_min=neff_min, table_prec=prec, want_nused=True, bandwidth=bandwidth)
     assert np.array_equal(_np(gU), oU), "nused differs"
     return (_np(gL), _np(gP)), (oL, oP)
 
@@ -543,3 +543,22 @@ def test_total_loglik_kde_composition(ctx):
     gL, _, _ = ctx.gwc_event_loglik_kde(th, ev, los, zmax, 256, 2.0)
     gX, _ = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], zmax)
     assert np.array_equal(_np(ctx.gwc_combine_total(gL, gX)), tot, equal_nan=True)
+
+
+def test_kde_silverman_bandwidth(ctx):
+    """Eq. D2 on the GPU: the interquartile range by exact selection (bisection on the bit pattern of the live
+    redshifts) against the oracle's sort, on pixels of 2 samples to hundreds; and it differs from Scott's rule."""
+    from paper_2605_23538_b200 import gwc
+    W = workload("o4", n_theta=12, n_events=8, los_rows=400, n_inj=500)
+    g, o = _kde_both(ctx, W, W.theta, neff_min=0.0, bandwidth="silverman")
+    _kde_compare(g, o, "silverman")
+    gs, _ = _kde_both(ctx, W, W.theta, neff_min=0.0, bandwidth="scott")
+    fin = np.isfinite(g[0]) & np.isfinite(gs[0])
+    assert fin.any() and np.abs(g[0][fin] - gs[0][fin]).max() > 1e-3
+    Wt = workload("tiny")
+    g, o = _kde_both(ctx, Wt, Wt.theta, neff_min=2.0, bandwidth="silverman")
+    _kde_compare(g, o, "silverman tiny")
+    th = Wt.theta.to(DEV)
+    ctx.gwc_build_cosmo(th, Wt.spec.z_max, 1025, 0)
+    with pytest.raises(KeyError):
+        ctx.gwc_event_loglik_kde(th, to_dev(Wt.ev, DEV), Wt.los.to(DEV), Wt.spec.z_max, 256, 0.0, "biweight")
