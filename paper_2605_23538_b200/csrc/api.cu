@@ -189,7 +189,6 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.inv_dz = (double)(n_z - 1) / los_zmax;
   p.los_zmax = los_zmax;
   p.tab_zq = ctx->z_max / NODE32_QMAX;
-  p.zero_mask = 0;
   p.out_w = (double*)ctx->part_w.p;
   p.out_n = (int32_t*)ctx->part_n.p;
   p.out_np = pixcut ? (int32_t*)ctx->part_np.p : nullptr;

@@ -46,10 +46,6 @@ constexpr int NCONST = 24;  // padded row length (>= C_COUNT), keeps rows 64-byt
 constexpr int NTHREADS = GWC_NTHREADS;  // threads per CTA of the fused kernel (one CTA per SM)
 constexpr int NWARPS = NTHREADS / 32;
 constexpr int SPT = GWC_SPT;      // samples per thread per theta (independent chains in flight)
-#ifndef GWC_CHUNK
-#define GWC_CHUNK 1024
-#endif
-constexpr int CHUNK = GWC_CHUNK;  // samples staged in shared memory per step (a multiple of 32 * SPT)
 constexpr int KT_THETA = 340;     // theta points whose constants fit the constant bank (one launch)
 #ifndef GWC_MAX_T
 #define GWC_MAX_T 16
@@ -89,7 +85,6 @@ struct ReweightParams {
   int pixcut;               // 1: per-pixel effective-sample cut (Eq. 8), threshold neff_min
   double neff_min;
   unsigned int* unit_counter;
-  int zero_mask;            // always 0 (scheduling pin of the LOS loads, reweight.cu)
 };
 
 // kernels / launchers (each returns the number of kernels it launched, or -1 on a launch error)

@@ -149,19 +149,10 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
 
 // Second half: population, rate, Jacobian and the LOS interpolation.  C = (ln m1z, ln(m2z/m1z)),
 // P = -ln pi - ln m1z - shift.  Returns the weight relative to the segment shift (0 when dead).
-// The loaded LOS nodes are tied to a value the tail computes late (OR with `late & zmask`, zmask = 0 at run time):
-// the compiler cannot then hoist their first use to the top of the stage, right behind the loads.
-__device__ __forceinline__ double pin_late(float q, int late, int zmask) {
-  return (double)__int_as_float(__float_as_int(q) | (late & zmask));
-}
-__device__ __forceinline__ double pin_late(double q, int late, int zmask) {
-  return __hiloint2double(__double2hiint(q) | (late & zmask), __double2loint(q));
-}
-
 template <typename LosT>
 __device__ __forceinline__ double term_tail(const double* __restrict__ tc, const double2* __restrict__ logtab,
                                             const double* __restrict__ exptab, double2 C, double P,
-                                            const Mid<LosT>& h, int zmask, bool& live) {
+                                            const Mid<LosT>& h, bool& live) {
   const double x = 1.0 + h.z;
   const double lx = log_fast(x, logtab);
   const double t1 = C.x - lx;  // ln m1
@@ -177,12 +168,7 @@ __device__ __forceinline__ double term_tail(const double* __restrict__ tc, const
   double den = fma(x2, rE, h.u);                   // u + x^2/E
   den *= fma(-tc[C_SGN], e1, tc[C_SGN]);           // sign(beta+1) (1 - e1)
   den *= 1.0 + e2;
-#ifdef GWC_PIN_LOS
-  const int late = __double2hiint(num);
-  const double q0 = pin_late(h.q0, late, zmask), q1 = pin_late(h.q1, late, zmask);
-#else
   const double q0 = widen(h.q0), q1 = widen(h.q1);
-#endif
   const double plos = fma(h.fz, q1 - q0, q0);
   const double w = num * plos * rcp_fast(den);
   const bool ok = h.ok & (plos > 0.0) & lt(w, CUDART_INF);  // also rejects NaN from a vanishing denominator
@@ -346,7 +332,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   const unsigned n_items = (unsigned)p.n_groups * (unsigned)p.n_tiles;
   const int bmax = p.n_z - 2;
   const double inv_dz = p.inv_dz, los_zmax = p.los_zmax, zq = p.tab_zq;
-  const int zmask = p.zero_mask;
   int cur_tile = -1;
 
   for (;;) {
@@ -502,7 +487,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, cur[k], zmask, lv[k]);
+                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, cur[k], lv[k]);
                 if (!PIX) {
                   a0 += wv[k];
                   a1 = fma(wv[k], wv[k], a1);
@@ -529,7 +514,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, nxt[k], zmask, lv[k]);
+                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, nxt[k], lv[k]);
                 lv[k] = lv[k] & second;
                 wv[k] = lv[k] ? wv[k] : 0.0;
                 if (!PIX) {
