@@ -79,18 +79,19 @@ __device__ __forceinline__ void node_pair(const Node32* t, int m, double& z0, do
   z0 = (double)t[m].zq * zq; d0 = (double)t[m].d * zq; z1 = (double)t[m + 1].zq * zq; d1 = (double)t[m + 1].d * zq;
 }
 
-// z_k and ln v_k of one sample (-inf when dead): DESIGN.md section 3 without p_los and the rate term
+// z_k and v_k of one sample relative to e^shift (v < 0: dead): DESIGN.md section 3 without p_los and the rate term.
+// `scale` = exp(-l_pi - shift) (for the default prior exp(-shift) / d_L^2, no logarithm at all).  Powers and the
+// Gaussian go through math64.cuh's exp / ln (2e-13), like the fused kernel.
 template <typename NodeT>
-__device__ __noinline__ double sample_lv(const ThetaK& K, const NodeT* tab, int M, double zq, double dL, double m1z,
-                                            double m2z, double lpi, int32_t row, int64_t n_rows, double los_zmax,
-                                            double& z_out) {
+__device__ __forceinline__ double sample_v(const ThetaK& K, const NodeT* tab, int M, double zq, double dL, double m1z,
+                                           double m2z, double scale, int32_t row, int64_t n_rows, double los_zmax,
+                                           const double2* logtab, const double* exptab, double& z_out) {
   z_out = 0.0;
-  const double NEG = -CUDART_INF;
-  if (!(isfinite(dL) && isfinite(m1z) && isfinite(m2z) && isfinite(lpi))) return NEG;
-  if (!(dL > 0.0 && m1z > 0.0 && m2z > 0.0)) return NEG;
-  if (row < 0 || (int64_t)row >= n_rows) return NEG;
+  if (!(isfinite(dL) && isfinite(m1z) && isfinite(m2z) && isfinite(scale))) return -1.0;
+  if (!(dL > 0.0 && m1z > 0.0 && m2z > 0.0)) return -1.0;
+  if (row < 0 || (int64_t)row >= n_rows) return -1.0;
   const double u = dL * K.h0c;
-  if (!(u < K.umax)) return NEG;
+  if (!(u < K.umax)) return -1.0;
   const double t = u * K.invdu;
   int m = (int)floor(t);
   m = m > M - 2 ? M - 2 : m;
@@ -100,18 +101,21 @@ __device__ __noinline__ double sample_lv(const ThetaK& K, const NodeT* tab, int 
   const double dl = z1 - z0, sd = d0 + d1;
   const double c3 = fma(-2.0, dl, sd), c2 = fma(3.0, dl, -(sd + d0));
   const double z = fma(f, fma(f, fma(f, c3, c2), d0), z0);
-  if (!(z < los_zmax)) return NEG;
+  if (!(z < los_zmax)) return -1.0;
   const double x = 1.0 + z;
-  const double m1 = m1z / x, m2 = m2z / x;
-  if (!(m1 > K.mmin && m1 <= K.mmax && m2 >= K.mmin && m2z <= m1z)) return NEG;
+  const double rx = rcp_fast(x);
+  const double m1 = m1z * rx, m2 = m2z * rx;
+  if (!(m1 > K.mmin && m1 <= K.mmax && m2 >= K.mmin && m2z <= m1z)) return -1.0;
+  const double lm1 = log_fast(m1, logtab), lm2 = log_fast(m2 <= m1 ? m2 : m1, logtab);
   const double y = (m1 - K.mu) / K.sigma;
-  const double p1 = K.a_pl * pow(m1, -K.alpha) + K.a_g * exp(-0.5 * y * y);
-  const double p2 = K.bp1 * pow(m2 <= m1 ? m2 : m1, K.beta) / (pow(m1, K.bp1) - K.mminb);
-  if (!(p1 > 0.0) || !(p2 > 0.0)) return NEG;
-  const double E = sqrt(fma(K.Om * x * x, x, K.OL));
-  const double J = x * x * K.cH * (u / x + x / E);
+  const double p1 = K.a_pl * exp_fast<true>(-K.alpha * lm1, exptab) + K.a_g * exp_fast<true>(-0.5 * y * y, exptab);
+  const double p2 = K.bp1 * exp_fast<true>(K.beta * lm2, exptab) / (exp_fast<true>(K.bp1 * lm1, exptab) - K.mminb);
+  if (!(p1 > 0.0) || !(p2 > 0.0)) return -1.0;
+  const double rE = rsqrt_fast(fma(K.Om * x * x, x, K.OL));
+  const double J = x * x * K.cH * (u * rx + x * rE);
   z_out = z;
-  return log(p1) + log(p2) - log(J) - lpi;
+  const double v = p1 * p2 * scale / J;
+  return v >= 0.0 ? v : -1.0;   // (NaN from a degenerate theta: dead)
 }
 
 // ---- order statistics of a pixel's live redshifts (Silverman's rule, Eq. D2) --------------------------------------
@@ -176,6 +180,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
   init_math_tables(mt, tid, KDE_THREADS);
   __syncthreads();
   const double* exptab = mt.exptab + (lane & (EXP_REP - 1));
+  const double2* logtab = mt.logtab + (lane & (LOG_REP - 1));
   const unsigned FULL = 0xffffffffu;
   const int G = p.n_grid;
   const double dzg = p.los_zmax / (G - 1);
@@ -231,6 +236,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
     __syncwarp();
     const NodeT* tab = reinterpret_cast<const NodeT*>(p.tab) + (size_t)t * p.Mp;
     const double shift = p.seg_shift[ev];
+    const double eshift = exp(-shift);
     // ---- (z_k, v_k) of every sample of the event, relative to e^shift ----
     double2* scr = p.scr + ((size_t)blockIdx.x * KDE_WARPS + warp) * (size_t)p.scr_stride - s0;   // indexed by sample
     for (int64_t c0 = s0; c0 < s1; c0 += 32) {
@@ -238,9 +244,12 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       if (k < s1) {
         double z;
         const double d = p.dL[k];
-        const double lpi = p.lprior ? p.lprior[k] : 2.0 * log(d);
-        const double lv = sample_lv(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], lpi, p.row[k], p.n_rows, p.los_zmax, z);
-        scr[k] = make_double2(z, lv > -CUDART_INF ? exp(lv - shift) : -1.0);
+        const double lp = p.lprior ? p.lprior[k] : 0.0;
+        const double scale = !p.lprior ? eshift / (d * d)
+                                       : (isfinite(lp) ? exp_fast<true>(-lp - shift, exptab) : CUDART_NAN);
+        const double v = sample_v(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], scale, p.row[k], p.n_rows, p.los_zmax,
+                                  logtab, exptab, z);
+        scr[k] = make_double2(z, v);
       }
     }
     __syncwarp();
