@@ -377,10 +377,21 @@ def cpu_baseline(spec, seed, W=None, theta=None, budget_s=15.0):
     oracle.selection_logxi(th[:n_th], inj, allsky, spec.z_max)
     dt = time.perf_counter() - t0
     terms = float(n_th) * (ns + n_inj)
+    # the same oracle on ONE thread (terms/s/core), on as many theta points as ~2 s allow
+    n1 = int(max(1, min(n0, round(2.0 / t_cal * n0 / max(cores, 1)))))
+    oracle.set_num_threads(1)
+    try:
+        t0 = time.perf_counter()
+        oracle.event_loglik(th[:n1], ev, los, spec.z_max)
+        oracle.selection_logxi(th[:n1], inj, allsky, spec.z_max)
+        dt1 = time.perf_counter() - t0
+    finally:
+        oracle.set_num_threads(cores)
     return {"value": terms / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "%d theta x (first %d events = %d samples + first %d injections), TABLE mode, %.1f s"
                       % (n_th, n_ev, ns, n_inj, dt),
-            "seconds": dt}
+            "seconds": dt, "value_one_core": float(n1) * (ns + n_inj) / dt1,
+            "sample_one_core": "%d theta on 1 thread, %.1f s" % (n1, dt1)}
 
 
 def run_reference(args):
