@@ -232,6 +232,15 @@ gwc_status gwc_total_loglik_host(gwc_ctx* ctx, const double* h_theta, int64_t n_
                                  gwc_prec table_prec, double* h_logL_total, int64_t* h2d_bytes, int64_t* d2h_bytes);
 
 /*
+ * Small-batch (latency) mode: the sampler's pattern is one theta point per call on a catalogue that never changes
+ * (PAPER.md:129, :166).  With caching on, the theta-independent preparation of the events and of the injections
+ * (per-sample logarithms and the per-segment reference of the sums) is kept in the context and reused by every later
+ * call that presents the same device pointers and sizes.  THE CALLER PROMISES that the contents of those arrays have
+ * not changed in between; turning the cache off (or on again) forgets everything.  Off by default.
+ */
+gwc_status gwc_cache_catalogue(gwc_ctx* ctx, int on);
+
+/*
  * Measurement helpers (not on the hot path).
  * gwc_set_timing: when on, the fused re-weighting kernel (A3/A5) is bracketed by CUDA events on the
  * context's stream; gwc_get_timing returns, for launches since the last call, the number of such

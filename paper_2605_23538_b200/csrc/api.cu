@@ -23,6 +23,15 @@ struct HostCopy {  // device mirrors used by gwc_total_loglik_host
 
 }  // namespace
 
+// Per-sample prepared values (d_L or NaN, ln m1z, ln(m2z/m1z), -l_pi - ln m1z - shift) and the per-segment shift of
+// one sample set, with the identity of the arrays they were computed from.
+struct PrepSet {
+  Buf dLc, L1, Q, P, seg_shift;
+  const void *k_dL = nullptr, *k_m1z = nullptr, *k_m2z = nullptr, *k_lp = nullptr, *k_row = nullptr, *k_off = nullptr;
+  int64_t k_n = -1, k_nseg = -1, k_nrows = -1;
+  bool valid = false;
+};
+
 struct gwc_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
@@ -39,8 +48,11 @@ struct gwc_ctx {
   gwc_prec tab_prec = GWC_F64;
   double z_max = 0.0;
   // per-call scratch
-  Buf dLc, L1, Q, P, seg_off, seg_shift, group_off, part_w, part_n, part_np, kde_scr, kde_len, allsky_scr, pack_scr, logL, logxi, probe;
+  Buf seg_off, group_off, part_w, part_n, part_np, kde_scr, kde_len, allsky_scr, pack_scr, logL, logxi, probe;
   HostCopy hc;
+  // theta-independent preparation of the events [0] and the injections [1] (kept between calls when caching is on)
+  PrepSet prep[2];
+  bool cache_prep = false;
   // timing
   bool timing = false;
   std::vector<cudaEvent_t> ev_pairs, inj_pairs;
@@ -129,25 +141,41 @@ gwc_status check_built(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, dou
   return GWC_OK;
 }
 
+// theta-independent preparation of a sample set; skipped when caching is on and the same arrays come again
+gwc_status prepare_samples(gwc_ctx* ctx, PrepSet& ps, int64_t n, int64_t n_seg, const int64_t* d_seg_off,
+                           const double* dL, const double* m1z, const double* m2z, const double* lprior,
+                           const int32_t* row, int64_t n_rows) {
+  if (ctx->cache_prep && ps.valid && ps.k_dL == dL && ps.k_m1z == m1z && ps.k_m2z == m2z && ps.k_lp == lprior &&
+      ps.k_row == row && ps.k_off == d_seg_off && ps.k_n == n && ps.k_nseg == n_seg && ps.k_nrows == n_rows)
+    return GWC_OK;
+  ps.valid = false;
+  const size_t nd = (size_t)(n > 0 ? n : 1) * sizeof(double);
+  GWC_TRY(ensure(ctx, ps.dLc, nd));
+  GWC_TRY(ensure(ctx, ps.L1, nd));
+  GWC_TRY(ensure(ctx, ps.Q, nd));
+  GWC_TRY(ensure(ctx, ps.P, nd));
+  GWC_TRY(ensure(ctx, ps.seg_shift, (size_t)(n_seg > 0 ? n_seg : 1) * sizeof(double)));
+  GWC_TRY(count(ctx, launch_prep_samples(n, n_seg, d_seg_off, dL, m1z, m2z, lprior, row, n_rows, (double*)ps.dLc.p,
+                                         (double*)ps.L1.p, (double*)ps.Q.p, (double*)ps.P.p, (double*)ps.seg_shift.p,
+                                         ctx->stream),
+                "prep_samples"));
+  ps.k_dL = dL; ps.k_m1z = m1z; ps.k_m2z = m2z; ps.k_lp = lprior; ps.k_row = row; ps.k_off = d_seg_off;
+  ps.k_n = n; ps.k_nseg = n_seg; ps.k_nrows = n_rows;
+  ps.valid = true;
+  return GWC_OK;
+}
+
 // shared launch sequence of A3 (events) and A5 (injections): prep -> groups -> fused kernel
 gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg, const int64_t* d_seg_off,
                         const double* dL, const double* m1z, const double* m2z, const double* lprior,
                         const int32_t* row, const void* los_table, gwc_prec los_prec, int64_t n_rows, int n_z,
                         double los_zmax, bool inj, bool pixcut = false, double neff_min = 0.0) {
   cudaStream_t s = ctx->stream;
-  const size_t nd = (size_t)(n > 0 ? n : 1) * sizeof(double);
-  GWC_TRY(ensure(ctx, ctx->dLc, nd));
-  GWC_TRY(ensure(ctx, ctx->L1, nd));
-  GWC_TRY(ensure(ctx, ctx->Q, nd));
-  GWC_TRY(ensure(ctx, ctx->P, nd));
-  GWC_TRY(ensure(ctx, ctx->seg_shift, (size_t)n_seg * sizeof(double)));
+  PrepSet& ps = ctx->prep[inj ? 1 : 0];
+  GWC_TRY(prepare_samples(ctx, ps, n, n_seg, d_seg_off, dL, m1z, m2z, lprior, row, n_rows));
   GWC_TRY(ensure(ctx, ctx->part_w, (size_t)n_theta * n_seg * 2 * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->part_n, (size_t)n_theta * n_seg * sizeof(int32_t)));
   if (pixcut) GWC_TRY(ensure(ctx, ctx->part_np, (size_t)n_theta * n_seg * sizeof(int32_t)));
-  GWC_TRY(count(ctx, launch_prep_samples(n, n_seg, d_seg_off, dL, m1z, m2z, lprior, row, n_rows, (double*)ctx->dLc.p,
-                                         (double*)ctx->L1.p, (double*)ctx->Q.p, (double*)ctx->P.p,
-                                         (double*)ctx->seg_shift.p, s),
-                "prep_samples"));
   // theta tile: as many tables as shared memory holds, balanced over the tiles
   int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut);
   if (T < 1) return fail(ctx, GWC_ERR_SHAPE, "n_nodes / n_z too large for shared memory");
@@ -172,12 +200,12 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.Mp = ctx->Mp;
   p.T = T;
   p.n_tiles = n_tiles;
-  p.dLc = (const double*)ctx->dLc.p;
+  p.dLc = (const double*)ps.dLc.p;
   p.m1z = m1z;
   p.m2z = m2z;
-  p.L1 = (const double*)ctx->L1.p;
-  p.Q = (const double*)ctx->Q.p;
-  p.P = (const double*)ctx->P.p;
+  p.L1 = (const double*)ps.L1.p;
+  p.Q = (const double*)ps.Q.p;
+  p.P = (const double*)ps.P.p;
   p.row = row;
   p.seg_off = d_seg_off;
   p.group_off = (const int32_t*)ctx->group_off.p;
@@ -194,7 +222,9 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.out_np = pixcut ? (int32_t*)ctx->part_np.p : nullptr;
   p.pixcut = pixcut ? 1 : 0;
   // events shorter on average than 2048 samples leave warps of a 16-warp CTA without a block: let them share it
-  p.teams = (!inj && !pixcut && n_seg > 0 && n / n_seg < 2048) ? 1 : 0;
+  // batches of a few theta points (the sampler's one-point-per-call pattern): no discarded pipeline step
+  p.odd = (!pixcut && n_theta <= 9 && (n_theta & 1)) ? 1 : 0;
+  p.teams = (!inj && !pixcut && !p.odd && n_seg > 0 && n / n_seg < 2048) ? 1 : 0;
   p.neff_min = neff_min;
   p.unit_counter = ctx->d_counter;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -263,7 +293,9 @@ void gwc_destroy(gwc_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
   cudaStreamSynchronize(ctx->stream);
-  Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->dLc, &ctx->L1, &ctx->Q, &ctx->P, &ctx->seg_off, &ctx->seg_shift,
+  Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->seg_off, &ctx->prep[0].dLc, &ctx->prep[0].L1, &ctx->prep[0].Q,
+                 &ctx->prep[0].P, &ctx->prep[0].seg_shift, &ctx->prep[1].dLc, &ctx->prep[1].L1, &ctx->prep[1].Q,
+                 &ctx->prep[1].P, &ctx->prep[1].seg_shift,
                  &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->kde_scr, &ctx->kde_len, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
                  &ctx->logxi, &ctx->probe, &ctx->hc.theta, &ctx->hc.ev_off, &ctx->hc.ev_dL, &ctx->hc.ev_m1z,
                  &ctx->hc.ev_m2z, &ctx->hc.ev_lp, &ctx->hc.ev_row, &ctx->hc.inj_dL, &ctx->hc.inj_m1z,
@@ -392,7 +424,7 @@ gwc_status gwc_event_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
                        ev->log_pe_prior, ev->sample_row, los->table, los->prec, los->n_rows, los->n_z, los->z_max,
                        false));
   return count(ctx, launch_finalize_events((const double*)ctx->part_w.p, (const int32_t*)ctx->part_n.p,
-                                           ev->ev_sample_off, (const double*)ctx->seg_shift.p,
+                                           ev->ev_sample_off, (const double*)ctx->prep[0].seg_shift.p,
                                            (const double*)ctx->tconst.p, n_theta, ev->n_events, d_logL, d_neff,
                                            d_nlive, ctx->stream),
                "finalize_events");
@@ -416,7 +448,7 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
                        ev->log_pe_prior, ev->sample_row, los->table, los->prec, los->n_rows, los->n_z, los->z_max,
                        false, true, neff_min));
   GWC_TRY(count(ctx, launch_finalize_events((const double*)ctx->part_w.p, (const int32_t*)ctx->part_n.p,
-                                            ev->ev_sample_off, (const double*)ctx->seg_shift.p,
+                                            ev->ev_sample_off, (const double*)ctx->prep[0].seg_shift.p,
                                             (const double*)ctx->tconst.p, n_theta, ev->n_events, d_logL, d_neff,
                                             d_nlive, ctx->stream),
                 "finalize_events"));
@@ -446,16 +478,8 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   // the per-event reference of the linear-domain sums (and nothing else) comes from the sample preparation
   cudaStream_t s = ctx->stream;
   const int64_t n = ev->n_samples, n_seg = ev->n_events;
-  const size_t nd = (size_t)(n > 0 ? n : 1) * sizeof(double);
-  GWC_TRY(ensure(ctx, ctx->dLc, nd));
-  GWC_TRY(ensure(ctx, ctx->L1, nd));
-  GWC_TRY(ensure(ctx, ctx->Q, nd));
-  GWC_TRY(ensure(ctx, ctx->P, nd));
-  GWC_TRY(ensure(ctx, ctx->seg_shift, (size_t)n_seg * sizeof(double)));
-  GWC_TRY(count(ctx, launch_prep_samples(n, n_seg, ev->ev_sample_off, ev->dL, ev->m1z, ev->m2z, ev->log_pe_prior,
-                                         ev->sample_row, los->n_rows, (double*)ctx->dLc.p, (double*)ctx->L1.p,
-                                         (double*)ctx->Q.p, (double*)ctx->P.p, (double*)ctx->seg_shift.p, s),
-                "prep_samples"));
+  GWC_TRY(prepare_samples(ctx, ctx->prep[0], n, n_seg, ev->ev_sample_off, ev->dL, ev->m1z, ev->m2z, ev->log_pe_prior,
+                          ev->sample_row, los->n_rows));
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (ctx->timing) {
     e0 = get_event(ctx);
@@ -473,7 +497,7 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   GWC_TRY(ensure(ctx, ctx->kde_scr, kde_scratch_bytes(n_blocks, max_len)));
   GWC_TRY(count(ctx, launch_kde(d_theta, ctx->tab.p, (const double*)ctx->tconst.p, n_theta, ctx->M, ctx->Mp,
                                 ctx->tab_prec, ctx->z_max / NODE32_QMAX, ev->n_events, ev->ev_sample_off, ev->dL,
-                                ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->seg_shift.p,
+                                ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->prep[0].seg_shift.p,
                                 los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, bw_rule,
                                 d_logL,
                                 d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, s),
@@ -504,7 +528,7 @@ gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_th
                 "uniform_segments"));
   GWC_TRY(run_reweight(ctx, n_theta, n, n_seg, (const int64_t*)ctx->seg_off.p, inj->dL, inj->m1z, inj->m2z,
                        inj->log_pdraw, nullptr, los->allsky, GWC_F64, 1, los->n_z, los->z_max, true));
-  return count(ctx, launch_finalize_inj((const double*)ctx->part_w.p, (const double*)ctx->seg_shift.p,
+  return count(ctx, launch_finalize_inj((const double*)ctx->part_w.p, (const double*)ctx->prep[1].seg_shift.p,
                                         (const double*)ctx->tconst.p, n_theta, n_seg, inj->n_draw, d_logxi,
                                         d_neff_inj, ctx->stream),
                "finalize_inj");
@@ -619,6 +643,14 @@ gwc_status gwc_total_loglik_host(gwc_ctx* ctx, const double* h_theta, int64_t n_
   ctx->built_theta = nullptr;  // the mirrored theta buffer is internal: do not let later calls match it
   if (h2d_bytes) *h2d_bytes = up;
   if (d2h_bytes) *d2h_bytes = n_theta * 8;
+  return GWC_OK;
+}
+
+gwc_status gwc_cache_catalogue(gwc_ctx* ctx, int on) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  ctx->cache_prep = on != 0;
+  ctx->prep[0].valid = false;
+  ctx->prep[1].valid = false;
   return GWC_OK;
 }
 

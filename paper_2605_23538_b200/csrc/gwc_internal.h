@@ -81,6 +81,7 @@ struct ReweightParams {
   double* out_w;            // [n_theta][n_seg][2]: sum w', sum w'^2
   int32_t* out_n;           // [n_theta][n_seg]   : n_live
   int32_t* out_np;          // [n_theta][n_seg]   : passing pixels (pixel-cut mode)
+  int odd;                  // 1: kernel variant with a tail-only path for odd theta counts (batches of a few points)
   int teams;                // 1: kernel variant in which short segments share the CTA (catalogues of short events)
   int pixcut;               // 1: per-pixel effective-sample cut (Eq. 8), threshold neff_min
   double neff_min;

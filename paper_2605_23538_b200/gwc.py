@@ -25,7 +25,7 @@ _STATUS = ["GWC_OK", "GWC_ERR_INVALID_ARG", "GWC_ERR_SHAPE", "GWC_ERR_DOMAIN", "
 EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_launch_count", "gwc_build_cosmo",
            "gwc_export_cosmo", "gwc_pack_events", "gwc_cap_pixels", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",
            "gwc_selection_logxi",
-           "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_set_timing", "gwc_get_timing",
+           "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_cache_catalogue", "gwc_set_timing", "gwc_get_timing",
            "gwc_probe_fp64", "gwc_math_selftest"]
 
 
@@ -88,6 +88,7 @@ def load():
                                       dbl, i32, vp]),
         "gwc_total_loglik_host": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci,
                                        vp, C.POINTER(i64), C.POINTER(i64)]),
+        "gwc_cache_catalogue": (ci, [vp, ci]),
         "gwc_set_timing": (ci, [vp, ci]),
         "gwc_get_timing": (ci, [vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64), C.POINTER(dbl)]),
         "gwc_probe_fp64": (ci, [vp, i64, C.POINTER(dbl), C.POINTER(dbl)]),
@@ -311,6 +312,10 @@ class Context:
                                                  C.byref(js), C.byref(los), n_nodes, table_prec,
                                                  _ptr(out, torch.float64, False), C.byref(up), C.byref(down)))
         return out, int(up.value), int(down.value)
+
+    def gwc_cache_catalogue(self, on: bool):
+        """Keep the theta-independent preparation between calls (the caller promises unchanged arrays)."""
+        self._ck(self._lib.gwc_cache_catalogue(self._h, int(on)))
 
     def gwc_set_timing(self, on: bool):
         self._ck(self._lib.gwc_set_timing(self._h, int(on)))

@@ -562,3 +562,42 @@ def test_kde_silverman_bandwidth(ctx):
     ctx.gwc_build_cosmo(th, Wt.spec.z_max, 1025, 0)
     with pytest.raises(KeyError):
         ctx.gwc_event_loglik_kde(th, to_dev(Wt.ev, DEV), Wt.los.to(DEV), Wt.spec.z_max, 256, 0.0, "biweight")
+
+
+def test_catalogue_cache_and_small_batches(ctx):
+    """Latency mode: with the catalogue cache on, repeated small-batch calls (1, 2, 3, 5 theta: odd counts take the
+    tail-only kernel variant) give the bits of the uncached calls; changing an array and presenting another pointer
+    recomputes; turning the cache off forgets."""
+    W = workload("tiny", n_theta=9)
+    zmax = W.spec.z_max
+    ev, inj, los = to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    o = _oracle_all(W, W.theta)
+    ref = {}
+    for nt in (1, 2, 3, 5, 9):
+        th = W.theta[:nt].to(DEV)
+        ref[nt] = _np(ctx.gwc_total_loglik(th, ev, inj, los, zmax, allsky))
+        assert_close_log(ref[nt], o["total"][:nt], RTOL_F64, "log L(theta), %d theta" % nt)
+    ctx.gwc_cache_catalogue(True)
+    try:
+        n0 = ctx.gwc_launch_count()
+        ctx.gwc_total_loglik(W.theta[:1].to(DEV), ev, inj, los, zmax, allsky)
+        first = ctx.gwc_launch_count() - n0
+        for nt in (1, 2, 3, 5, 9, 1):
+            th = W.theta[:nt].to(DEV)
+            n0 = ctx.gwc_launch_count()
+            got = _np(ctx.gwc_total_loglik(th, ev, inj, los, zmax, allsky))
+            assert np.array_equal(got, ref[nt], equal_nan=True)
+            if nt == 1:
+                assert ctx.gwc_launch_count() - n0 == first - 2       # the two preparation kernels are skipped
+        # another array (new pointer, new contents): recomputed
+        ev2 = dict(ev, dL=(ev["dL"] * 1.01))
+        th = W.theta[:3].to(DEV)
+        got2 = _np(ctx.gwc_total_loglik(th, ev2, inj, los, zmax, allsky))
+        ev2_cpu = dict(W.ev, dL=W.ev["dL"] * 1.01)
+        o2 = oracle.total_loglik(_np(W.theta[:3]), synth.to_numpy(ev2_cpu), synth.to_numpy(W.inj), _np(W.los), zmax)
+        assert_close_log(got2, o2, RTOL_F64, "after a new d_L array")
+    finally:
+        ctx.gwc_cache_catalogue(False)
+    got = _np(ctx.gwc_total_loglik(W.theta[:5].to(DEV), ev, inj, los, zmax, allsky))
+    assert np.array_equal(got, ref[5], equal_nan=True)
