@@ -276,6 +276,27 @@ def run_gwc(args):
                "gaussian_evals_per_s": evals / (ms_kde * 1e-3),
                "roofline_frac_fp64": evals * 10.0 / (ms_kde * 1e-3) / FP64_PEAK_INSTR}
         del nused
+    # ---- NEXT row 4, reported beside the headline: one theta per call (the sampler's pattern), catalogue cache on ----
+    lat = None
+    if args.latency_calls > 0:
+        th1 = theta[:1].contiguous()
+        ctx.gwc_cache_catalogue(True)
+        try:
+            for _ in range(3):
+                ctx.gwc_total_loglik(th1, W.ev, W.inj, W.los, zmax, allsky, args.n_nodes, prec)
+            torch.cuda.synchronize()
+            l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0 = time.perf_counter()
+            l0.record()
+            for _ in range(args.latency_calls):
+                ctx.gwc_total_loglik(th1, W.ev, W.inj, W.los, zmax, allsky, args.n_nodes, prec)
+            l1.record()
+            torch.cuda.synchronize()
+            wall = (time.perf_counter() - t0) / args.latency_calls * 1e3
+            lat = {"n_theta": 1, "calls": args.latency_calls, "device_ms_per_call": l0.elapsed_time(l1) / args.latency_calls,
+                   "wall_ms_per_call": wall, "catalogue_cache": True}
+        finally:
+            ctx.gwc_cache_catalogue(False)
     cpu = cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
     stress = stress_report(ctx, W, theta, zmax, allsky, args.n_nodes) if spec.name == "stress" else None
     line = {
@@ -305,6 +326,8 @@ def run_gwc(args):
         line["pixcut"] = pix
     if kde is not None:
         line["kde"] = kde
+    if lat is not None:
+        line["latency"] = lat
     print(json.dumps(line))
     if dist:
         td.destroy_process_group()
@@ -436,6 +459,8 @@ def main():
     ap.add_argument("--seed", type=int, default=synth.DEFAULT_SEED)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle timing budget (0 = skip)")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--latency-calls", type=int, default=50,
+                    help="also time this many one-theta calls with the catalogue cache on (0: skip)")
     ap.add_argument("--kde-theta", type=int, default=16,
                     help="also time the KDE-numerator event term on this many theta points (0: skip)")
     ap.add_argument("--pixcut", type=float, default=2.0,
