@@ -214,17 +214,15 @@ struct PixShape {
 
 // Segmented inclusive scan of (W, Q, n) over the 32 lanes of one row; lanes add from `o` lanes back while that
 // lane is still inside their run.
-__device__ __forceinline__ void seg_scan(double& W, double& Q, int& n, int d, int maxd) {
+__device__ __forceinline__ void seg_scan(double& W, double& Q, int d, int maxd) {
   const unsigned FULL = 0xffffffffu;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
     if (o > maxd) break;  // warp-uniform
     const double tW = __shfl_up_sync(FULL, W, o), tQ = __shfl_up_sync(FULL, Q, o);
-    const int tn = __shfl_up_sync(FULL, n, o);
     const bool take = d >= 64 ? (int)(threadIdx.x & 31) >= o : d >= o;
     W += take ? tW : 0.0;
     Q += take ? tQ : 0.0;
-    n += take ? tn : 0;
   }
 }
 
@@ -242,8 +240,11 @@ __device__ __forceinline__ void pix_reduce(const PixShape& ps, const double* w, 
   for (int k = 0; k < SPT; ++k) {
     W[k] = w[k];
     Q[k] = w[k] * w[k];
-    n[k] = live[k] ? 1 : 0;
-    seg_scan(W[k], Q[k], n[k], ps.d[k], ps.maxd[k]);
+    seg_scan(W[k], Q[k], ps.d[k], ps.maxd[k]);
+    // live samples of the run inside this row: no scan needed, a ballot and a population count over the run's lanes
+    const unsigned lm = __ballot_sync(FULL, live[k]);
+    const int first = ps.d[k] >= 64 ? 0 : lane - ps.d[k];
+    n[k] = __popc(lm & (0xffffffffu >> (31 - lane)) & (0xffffffffu << first));
   }
   // runs that began before the row: add what the previous row (or the previous block) accumulated for them
   double inW = carryWQ[0], inQ = carryWQ[1];
