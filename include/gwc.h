@@ -29,8 +29,27 @@
  *    -inf is a legal output (no live sample).
  *  - Units: d_L in Mpc, masses in solar masses (detector frame), H0 in km/s/Mpc.
  *  - Results are deterministic: no floating-point atomics, every reduction has a fixed order.
- *  - Range: linear-domain accumulation in FP64; every log-weight must lie in about [-700, 700]
- *    (true of any physical input; weights below e^-700 count as e^-700).
+ *  - Range (R23): the sums of an event (of a block of 8192 injections) are taken in the linear domain in
+ *    FP64, relative to a reference fixed before theta is known: max over its valid samples of
+ *    (-log_pe_prior - ln m1z).  The result is exact to the stated tolerances as long as the largest live weight
+ *    of the event lies within 300 nats of that reference -- true of any physical input, whose spread inside one
+ *    event is a few nats.  When a log_pe_prior / log_pdraw of enormous spread breaks this (every live weight more
+ *    than 300 nats below the reference), the outputs of that (theta, event) are NaN and gwc_check() returns
+ *    GWC_ERR_RANGE; nothing is clamped silently.  (Single weights more than 700 nats below the reference count as
+ *    e^-700 of it, far below the rounding of the sum.  gwc_event_loglik_pixcut decides per pixel: a pixel whose
+ *    own weights all lie more than 300 nats below its event's reference may be counted wrongly in d_npass /
+ *    d_nlive while contributing nothing to log L_i.)
+ *  - theta and the tables: gwc_build_cosmo keeps, next to the tables, a copy of the theta rows it was given.  The
+ *    calls that need the tables take the same d_theta pointer and count (else GWC_ERR_NOT_BUILT at once) and
+ *    compare the rows on the device with that copy: a row that was changed in place since the build (or a new
+ *    array that landed at the same address) gets NaN outputs and gwc_check() returns GWC_ERR_NOT_BUILT.  Any
+ *    change to theta needs a new gwc_build_cosmo.  A later build (other n_nodes / table_prec / z_max) replaces
+ *    the earlier one: the dependent calls always use the latest.
+ *  - Streams: every context enqueues on its own stream, and several contexts may be used from several host
+ *    threads.  The fused re-weighting kernels of ALL contexts on one device run one after the other (they share
+ *    the device's constant bank for the per-theta constants; each launch waits for the previous one through an
+ *    event, whichever stream it was on).  Each of them fills the GPU, so nothing is lost.  A single context
+ *    must not be used from two threads at the same time.
  */
 #ifndef GWC_H_
 #define GWC_H_
@@ -50,8 +69,11 @@ typedef enum {
   GWC_ERR_DOMAIN = 3,
   GWC_ERR_NOT_BUILT = 4,
   GWC_ERR_NOMEM = 5,
-  GWC_ERR_CUDA = 6
+  GWC_ERR_CUDA = 6,
+  GWC_ERR_RANGE = 7
 } gwc_status;
+
+#define GWC_MAX_NZ_SELECTION 4096 /* largest los->n_z of the selection term (the all-sky table sits in shared memory) */
 
 typedef enum { GWC_F64 = 0, GWC_F32 = 1 } gwc_prec;
 /* bandwidth rule of the KDE numerator: Scott, Eq. D1 (the paper's default) | Silverman, Eq. D2 (:300) */
@@ -62,7 +84,9 @@ typedef struct gwc_ctx gwc_ctx;
 /* Create a context on CUDA device `device`; `cuda_stream` is a cudaStream_t (NULL = default stream). */
 gwc_status gwc_create(gwc_ctx** ctx, int device, void* cuda_stream);
 void gwc_destroy(gwc_ctx* ctx);
-/* Synchronise the stream and report sticky device errors (GWC_ERR_DOMAIN, GWC_ERR_CUDA); clears the flag. */
+/* Synchronise the stream and report sticky device errors, then clear them: GWC_ERR_NOT_BUILT (theta changed since
+ * the build), GWC_ERR_DOMAIN (a theta point outside the model's domain), GWC_ERR_RANGE (see "Range" above), in
+ * that order of precedence; GWC_ERR_CUDA. */
 gwc_status gwc_check(gwc_ctx* ctx);
 const char* gwc_last_error(const gwc_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
@@ -119,6 +143,8 @@ typedef struct {
  *        d_ev_pix_off [n_events+1], d_ev_pix_rows [<= n_samples] (distinct rows per event, ascending),
  *        d_pix_sample_off [<= n_samples+1] (start of each (event,row) run, then n_samples),
  *        *h_n_pixrefs (host) = number of distinct (event,row) pairs.  Synchronises the stream.
+ * An event id outside [0, n_events) or a negative row -> GWC_ERR_DOMAIN (reported by this call itself; the sticky
+ * flags that gwc_check reports are neither read nor cleared).
  */
 gwc_status gwc_pack_events(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, const int32_t* d_event_id,
                            const int32_t* d_row, int64_t* d_perm, int64_t* d_ev_sample_off, int64_t* d_ev_pix_off,
@@ -194,6 +220,7 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
  * A5.  log xi(theta) = log( (1/n_draw) sum_j w_j ) over found injections with the all-sky prior
  * los->allsky and log_pdraw in place of the PE prior; optional N_eff of the injection sum.
  *   d_logxi [n_theta];  d_neff_inj [n_theta] or NULL.
+ * los->n_z <= GWC_MAX_NZ_SELECTION (4096) else GWC_ERR_SHAPE (here and, before any work, in gwc_total_loglik*).
  */
 gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_injections* inj,
                                const gwc_los* los, double* d_logxi, double* d_neff_inj);

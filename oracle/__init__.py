@@ -59,6 +59,7 @@ def lib():
             "orc_z_of_u": (d, [d, d]), "orc_z_of_dL": (d, [d, d, d]),
             "orc_build_table": (None, [d, d, C.c_int, vp, vp, vp]),
             "orc_z_table": (C.c_int, [d, vp, vp, C.c_int, d, vp]),
+            "orc_round_table_32": (None, [vp, C.c_int, d]),
             "orc_theta_valid": (C.c_int, [vp]), "orc_norm_pl": (d, [vp]), "orc_norm_g": (d, [vp]),
             "orc_p1": (d, [d, vp]), "orc_p2": (d, [d, d, vp]), "orc_psi": (d, [d, vp]),
             "orc_los_lerp": (d, [vp, i64, d]), "orc_los_allsky": (None, [vp, vp]),
@@ -117,6 +118,14 @@ def build_table(Om, z_max, M=1025):
     zt, dt, um = np.empty(M), np.empty(M), np.empty(1)
     lib().orc_build_table(Om, z_max, M, _p(zt), _p(dt), _p(um))
     return zt, dt, float(um[0])
+
+
+def round_table_32(zt, dt, z_max):
+    """The 32-bit storage of a cosmology table (R22): returns the values a look-up reads back."""
+    M = len(zt)
+    buf = np.concatenate([_f64(zt), _f64(dt)])
+    lib().orc_round_table_32(_p(buf), M, float(z_max))
+    return buf[:M].copy(), buf[M:].copy()
 
 
 def z_table(u, zt, dt, umax):

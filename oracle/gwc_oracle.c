@@ -402,8 +402,11 @@ static int prep_cosmo(const double* th, int mode, double z_max, int M, orc_cosmo
 
 /* optional 32-bit storage of the cosmology table (reading R22): with q = z_max / (2^32 - 1),
  * a node z_m is stored as the unsigned 32-bit integer nearest to z_m / q, its slope du z'_m as the binary32
- * nearest to (du z'_m) / q; what the look-up reads back is integer * q and (double)float * q. */
-static void round_table_32(double* buf, int M, double z_max) {
+ * nearest to (du z'_m) / q; what the look-up reads back is integer * q and (double)float * q.
+ * buf = [z_0 .. z_{M-1}, d_0 .. d_{M-1}] is rewritten in place.  Pinned by tests/test_oracle_pins.py
+ * (test_round_table_32_*): the quantisation bounds q/2 and 2^-24, the stored values being representable, and the
+ * bound both imply on log L_i. */
+void orc_round_table_32(double* buf, int M, double z_max) {
   const double qmax = 4294967295.0;
   const double q = z_max / qmax;
   for (int i = 0; i < M; ++i) {
@@ -444,7 +447,7 @@ int orc_event_loglik(const double* theta, int64_t n_theta, const orc_events* ev,
     orc_cosmo_tab ct;
     double* buf = NULL;
     if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lw); continue; }
-    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
+    if (mode == 0 && table_prec == 1) orc_round_table_32(buf, M, z_max);
     for (int64_t i = 0; i < ev->n_events; ++i) {
       int64_t a = ev->ev_sample_off[i], b = ev->ev_sample_off[i + 1];
       int64_t cnt = 0;
@@ -507,7 +510,7 @@ int orc_event_loglik_pixcut(const double* theta, int64_t n_theta, const orc_even
     orc_cosmo_tab ct;
     double* buf = NULL;
     if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lw); free(keep); free(lv); continue; }
-    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
+    if (mode == 0 && table_prec == 1) orc_round_table_32(buf, M, z_max);
     for (int64_t i = 0; i < ev->n_events; ++i) {
       int64_t a = ev->ev_sample_off[i], b = ev->ev_sample_off[i + 1];
       for (int64_t k = a; k < b; ++k) {
@@ -658,7 +661,7 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
     orc_cosmo_tab ct;
     double* buf = NULL;
     if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lv); free(zz); free(lI); free(Rg); continue; }
-    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
+    if (mode == 0 && table_prec == 1) orc_round_table_32(buf, M, z_max);
     for (int g = 0; g < n_grid; ++g) {            /* rate term on the grid: R(z) = psi(z) / (1+z), reading R4 */
       double zg = g * dzg;
       Rg[g] = psi_c(zg, th, &ct.pop) / (1.0 + zg);
@@ -769,7 +772,7 @@ int orc_selection_logxi(const double* theta, int64_t n_theta, const orc_injectio
     orc_cosmo_tab ct;
     double* buf = NULL;
     if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lw); continue; }
-    if (mode == 0 && table_prec == 1) round_table_32(buf, M, z_max);
+    if (mode == 0 && table_prec == 1) orc_round_table_32(buf, M, z_max);
     for (int64_t k = 0; k < inj->n_found; ++k) {
       int live;
       lw[k] = orc_log_weight(th, mode, &ct, inj->dL[k], inj->m1z[k], inj->m2z[k], inj->log_pdraw[k], &A, 0, &live);

@@ -42,8 +42,10 @@ struct gwc_ctx {
   unsigned int* d_counter = nullptr;
   // A1/A2 state
   Buf tab, tconst;
+  Buf theta_snap, tvalid;   // the theta rows the tables were built from; per-theta validity (1.0 | NaN)
   const double* built_theta = nullptr;
   int64_t built_n = 0;
+  bool fresh_build = false;   // inside gwc_total_loglik*: the build was enqueued by this very call, no verification
   int M = 0, Mp = 0;
   gwc_prec tab_prec = GWC_F64;
   double z_max = 0.0;
@@ -133,12 +135,19 @@ cudaEvent_t get_event(gwc_ctx* ctx) {
   return e;
 }
 
+// The tables in the context belong to the theta rows gwc_build_cosmo saw.  Host side: same pointer and count.
+// Device side: the caller's rows are compared bit for bit with the copy taken at build time (an in-place update, or
+// another tensor that the allocator put at the same address, is caught here): a row that differs gets NaN outputs and
+// raises the sticky FLAG_STALE, which gwc_check reports as GWC_ERR_NOT_BUILT.
 gwc_status check_built(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double los_zmax) {
   if (!ctx->built_theta || ctx->built_theta != d_theta || ctx->built_n != n_theta)
     return fail(ctx, GWC_ERR_NOT_BUILT, "gwc_build_cosmo was not called with this d_theta / n_theta");
   if (los_zmax > ctx->z_max * (1.0 + 1e-12))
     return fail(ctx, GWC_ERR_NOT_BUILT, "cosmology table built with a smaller z_max than the LOS table's");
-  return GWC_OK;
+  if (ctx->fresh_build) return GWC_OK;
+  return count(ctx, launch_verify_theta(d_theta, (const double*)ctx->theta_snap.p, (const double*)ctx->tconst.p,
+                                        n_theta, (double*)ctx->tvalid.p, ctx->d_flag, ctx->stream),
+               "verify_theta");
 }
 
 // theta-independent preparation of a sample set; skipped when caching is on and the same arrays come again
@@ -233,7 +242,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
     e1 = get_event(ctx);
     cudaEventRecord(e0, s);
   }
-  GWC_TRY(count(ctx, launch_reweight(p, ctx->tab_prec, los_prec, inj, ctx->n_sm, s), "reweight"));
+  GWC_TRY(count(ctx, launch_reweight(p, ctx->tab_prec, los_prec, inj, ctx->n_sm, ctx->device, s), "reweight"));
   if (ctx->timing) {
     cudaEventRecord(e1, s);
     auto& v = inj ? ctx->inj_pairs : ctx->ev_pairs;
@@ -242,6 +251,13 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   }
   return GWC_OK;
 }
+
+// scope guard of gwc_total_loglik*: between the build and the dependent calls of one entry point
+struct FreshBuild {
+  gwc_ctx* c;
+  explicit FreshBuild(gwc_ctx* ctx) : c(ctx) { c->fresh_build = true; }
+  ~FreshBuild() { c->fresh_build = false; }
+};
 
 gwc_status check_theta_args(gwc_ctx* ctx, const double* d_theta, int64_t n_theta) {
   if (!ctx) return GWC_ERR_INVALID_ARG;
@@ -275,9 +291,9 @@ gwc_status gwc_create(gwc_ctx** out, int device, void* cuda_stream) {
   cudaError_t e = cudaSetDevice(device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
-  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_flag, sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_flag, 2 * sizeof(int));   // [0] sticky flags, [1] A0 packing
   if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_counter, sizeof(unsigned int));
-  if (e == cudaSuccess) e = cudaMemset(ctx->d_flag, 0, sizeof(int));
+  if (e == cudaSuccess) e = cudaMemset(ctx->d_flag, 0, 2 * sizeof(int));
   if (e == cudaSuccess && reweight_configure(ctx->smem_optin) != 0) e = cudaGetLastError();
   if (e != cudaSuccess) {
     g_create_error = std::string("gwc_create: ") + cudaGetErrorString(e);
@@ -293,7 +309,7 @@ void gwc_destroy(gwc_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
   cudaStreamSynchronize(ctx->stream);
-  Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->seg_off, &ctx->prep[0].dLc, &ctx->prep[0].L1, &ctx->prep[0].Q,
+  Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->theta_snap, &ctx->tvalid, &ctx->seg_off, &ctx->prep[0].dLc, &ctx->prep[0].L1, &ctx->prep[0].Q,
                  &ctx->prep[0].P, &ctx->prep[0].seg_shift, &ctx->prep[1].dLc, &ctx->prep[1].L1, &ctx->prep[1].Q,
                  &ctx->prep[1].P, &ctx->prep[1].seg_shift,
                  &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->kde_scr, &ctx->kde_len, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
@@ -316,8 +332,15 @@ gwc_status gwc_check(gwc_ctx* ctx) {
   GWC_CUDA(cudaMemcpy(&flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
   if (flag) {
     GWC_CUDA(cudaMemset(ctx->d_flag, 0, sizeof(int)));
-    if (flag & 1) return fail(ctx, GWC_ERR_DOMAIN, "a theta point is outside the model's domain (its outputs are NaN)");
-    return fail(ctx, GWC_ERR_DOMAIN, "gwc_pack_events: an event id or row is out of range");
+    if (flag & FLAG_STALE)
+      return fail(ctx, GWC_ERR_NOT_BUILT,
+                  "d_theta changed after gwc_build_cosmo: the outputs of the changed points are NaN (rebuild first)");
+    if (flag & FLAG_DOMAIN)
+      return fail(ctx, GWC_ERR_DOMAIN, "a theta point is outside the model's domain (its outputs are NaN)");
+    if (flag & FLAG_RANGE)
+      return fail(ctx, GWC_ERR_RANGE,
+                  "the live weights of a segment all lie more than 300 nats below its reference (its outputs are NaN): "
+                  "log_pe_prior / log_pdraw has too wide a spread inside one event");
   }
   return GWC_OK;
 }
@@ -337,8 +360,11 @@ gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta,
   ctx->built_theta = nullptr;
   GWC_TRY(ensure(ctx, ctx->tab, (size_t)n_theta * Mp * node));
   GWC_TRY(ensure(ctx, ctx->tconst, (size_t)n_theta * NCONST * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->theta_snap, (size_t)n_theta * GWC_NPAR * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->tvalid, (size_t)n_theta * sizeof(double)));
   GWC_TRY(count(ctx, launch_cosmo_build(d_theta, n_theta, z_max, n_nodes, Mp, table_prec, ctx->tab.p,
-                                        (double*)ctx->tconst.p, ctx->d_flag, ctx->stream),
+                                        (double*)ctx->tconst.p, (double*)ctx->theta_snap.p, (double*)ctx->tvalid.p,
+                                        ctx->d_flag, ctx->stream),
                 "cosmo_build"));
   ctx->built_theta = d_theta;
   ctx->built_n = n_theta;
@@ -369,13 +395,19 @@ gwc_status gwc_pack_events(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, co
   const size_t bytes = pack_scratch_bytes(n_samples, n_events);
   GWC_TRY(ensure(ctx, ctx->pack_scr, bytes + 8));
   int64_t* d_np = (int64_t*)((unsigned char*)ctx->pack_scr.p + bytes);
+  // the packing has a flag word of its own (d_flag[1]): a theta-domain flag left by an earlier call is neither
+  // reported here nor consumed
+  GWC_CUDA(cudaMemsetAsync(ctx->d_flag + 1, 0, sizeof(int), ctx->stream));
   GWC_TRY(count(ctx, launch_pack(n_samples, n_events, d_event_id, d_row, d_perm, d_ev_sample_off, d_ev_pix_off,
-                                 d_ev_pix_rows, d_pix_sample_off, d_np, ctx->d_flag, ctx->pack_scr.p, bytes,
+                                 d_ev_pix_rows, d_pix_sample_off, d_np, ctx->d_flag + 1, ctx->pack_scr.p, bytes,
                                  ctx->stream),
                 "pack_events"));
+  int bad = 0;
   GWC_CUDA(cudaMemcpyAsync(h_n_pixrefs, d_np, sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream));
+  GWC_CUDA(cudaMemcpyAsync(&bad, ctx->d_flag + 1, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
   GWC_CUDA(cudaStreamSynchronize(ctx->stream));
-  return gwc_check(ctx);
+  if (bad) return fail(ctx, GWC_ERR_DOMAIN, "gwc_pack_events: an event id or row is out of range");
+  return GWC_OK;
 }
 
 gwc_status gwc_cap_pixels(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, int64_t n_pixrefs,
@@ -395,7 +427,7 @@ gwc_status gwc_cap_pixels(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, int
                 "cap_pixels"));
   GWC_CUDA(cudaMemcpyAsync(h_n_kept, d_nk, sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream));
   GWC_CUDA(cudaStreamSynchronize(ctx->stream));
-  return gwc_check(ctx);
+  return GWC_OK;
 }
 
 gwc_status gwc_los_allsky(gwc_ctx* ctx, const gwc_los* los, double* d_allsky) {
@@ -425,8 +457,8 @@ gwc_status gwc_event_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
                        false));
   return count(ctx, launch_finalize_events((const double*)ctx->part_w.p, (const int32_t*)ctx->part_n.p,
                                            ev->ev_sample_off, (const double*)ctx->prep[0].seg_shift.p,
-                                           (const double*)ctx->tconst.p, n_theta, ev->n_events, d_logL, d_neff,
-                                           d_nlive, ctx->stream),
+                                           (const double*)ctx->tvalid.p, n_theta, ev->n_events, d_logL, d_neff,
+                                           d_nlive, ctx->d_flag, ctx->stream),
                "finalize_events");
 }
 
@@ -449,11 +481,11 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
                        false, true, neff_min));
   GWC_TRY(count(ctx, launch_finalize_events((const double*)ctx->part_w.p, (const int32_t*)ctx->part_n.p,
                                             ev->ev_sample_off, (const double*)ctx->prep[0].seg_shift.p,
-                                            (const double*)ctx->tconst.p, n_theta, ev->n_events, d_logL, d_neff,
-                                            d_nlive, ctx->stream),
+                                            (const double*)ctx->tvalid.p, n_theta, ev->n_events, d_logL, d_neff,
+                                            d_nlive, ctx->d_flag, ctx->stream),
                 "finalize_events"));
   if (d_npass)
-    GWC_TRY(count(ctx, launch_widen_i32((const int32_t*)ctx->part_np.p, (const double*)ctx->tconst.p, n_theta,
+    GWC_TRY(count(ctx, launch_widen_i32((const int32_t*)ctx->part_np.p, (const double*)ctx->tvalid.p, n_theta,
                                         ev->n_events, d_npass, ctx->stream),
                   "widen_npass"));
   return GWC_OK;
@@ -480,12 +512,6 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   const int64_t n = ev->n_samples, n_seg = ev->n_events;
   GWC_TRY(prepare_samples(ctx, ctx->prep[0], n, n_seg, ev->ev_sample_off, ev->dL, ev->m1z, ev->m2z, ev->log_pe_prior,
                           ev->sample_row, los->n_rows));
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  if (ctx->timing) {
-    e0 = get_event(ctx);
-    e1 = get_event(ctx);
-    cudaEventRecord(e0, s);
-  }
   // scratch of the kernel: one slice of (z, v) pairs per resident warp, as long as the longest event
   GWC_TRY(ensure(ctx, ctx->kde_len, sizeof(int64_t)));
   GWC_TRY(count(ctx, launch_max_segment(ev->ev_sample_off, ev->n_events, (int64_t*)ctx->kde_len.p, s), "max_segment"));
@@ -495,19 +521,26 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   if (max_len < 0 || max_len > ev->n_samples) return fail(ctx, GWC_ERR_SHAPE, "ev_sample_off is not ascending");
   const int n_blocks = kde_grid_blocks(n_theta, ev->n_events, ctx->n_sm);
   GWC_TRY(ensure(ctx, ctx->kde_scr, kde_scratch_bytes(n_blocks, max_len)));
-  GWC_TRY(count(ctx, launch_kde(d_theta, ctx->tab.p, (const double*)ctx->tconst.p, n_theta, ctx->M, ctx->Mp,
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (ctx->timing) {   // (taken after the last step that can fail before the launch: nothing leaks on an error return)
+    e0 = get_event(ctx);
+    e1 = get_event(ctx);
+    cudaEventRecord(e0, s);
+  }
+  // the population parameters come from the copy of theta the tables were built from, never from a changed array
+  const gwc_status st_kde = count(ctx, launch_kde((const double*)ctx->theta_snap.p, ctx->tab.p, (const double*)ctx->tconst.p, (const double*)ctx->tvalid.p, n_theta, ctx->M, ctx->Mp,
                                 ctx->tab_prec, ctx->z_max / NODE32_QMAX, ev->n_events, ev->ev_sample_off, ev->dL,
                                 ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->prep[0].seg_shift.p,
                                 los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, bw_rule,
                                 d_logL,
                                 d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, s),
-                "kde"));
+                "kde");
   if (ctx->timing) {
     cudaEventRecord(e1, s);
     ctx->ev_pairs.push_back(e0);
     ctx->ev_pairs.push_back(e1);
   }
-  return GWC_OK;
+  return st_kde;
 }
 
 gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_injections* inj,
@@ -519,7 +552,8 @@ gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_th
   if (!(inj->n_draw > 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "n_draw must be positive");
   if (inj->n_found > 0 && (!inj->dL || !inj->m1z || !inj->m2z || !inj->log_pdraw))
     return fail(ctx, GWC_ERR_INVALID_ARG, "an injection array is NULL");
-  if (los->n_z > 4096) return fail(ctx, GWC_ERR_SHAPE, "los->n_z > 4096 is not supported by the selection kernel");
+  if (los->n_z > GWC_MAX_NZ_SELECTION)
+    return fail(ctx, GWC_ERR_SHAPE, "los->n_z > 4096 is not supported by the selection term (all-sky table in shared memory)");
   GWC_TRY(check_built(ctx, d_theta, n_theta, los->z_max));
   const int64_t n = inj->n_found;
   const int64_t n_seg = n > 0 ? (n + INJ_SEG - 1) / INJ_SEG : 1;
@@ -528,9 +562,9 @@ gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_th
                 "uniform_segments"));
   GWC_TRY(run_reweight(ctx, n_theta, n, n_seg, (const int64_t*)ctx->seg_off.p, inj->dL, inj->m1z, inj->m2z,
                        inj->log_pdraw, nullptr, los->allsky, GWC_F64, 1, los->n_z, los->z_max, true));
-  return count(ctx, launch_finalize_inj((const double*)ctx->part_w.p, (const double*)ctx->prep[1].seg_shift.p,
-                                        (const double*)ctx->tconst.p, n_theta, n_seg, inj->n_draw, d_logxi,
-                                        d_neff_inj, ctx->stream),
+  return count(ctx, launch_finalize_inj((const double*)ctx->part_w.p, (const int32_t*)ctx->part_n.p,
+                                        (const double*)ctx->prep[1].seg_shift.p, (const double*)ctx->tvalid.p, n_theta,
+                                        n_seg, inj->n_draw, d_logxi, d_neff_inj, ctx->d_flag, ctx->stream),
                "finalize_inj");
 }
 
@@ -548,10 +582,13 @@ gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
   GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
   if (!ev || !inj || !d_logL_total) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL argument");
   GWC_TRY(check_los(ctx, los, true, true));
+  if (los->n_z > GWC_MAX_NZ_SELECTION)   // before any work: the selection term at the end would refuse it
+    return fail(ctx, GWC_ERR_SHAPE, "los->n_z > 4096 is not supported by the selection term");
   GWC_TRY(gwc_build_cosmo(ctx, d_theta, n_theta, los->z_max, n_nodes, table_prec));
   const int64_t E = ev->n_events;
   GWC_TRY(ensure(ctx, ctx->logL, (size_t)n_theta * (size_t)(E > 0 ? E : 1) * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->logxi, (size_t)n_theta * sizeof(double)));
+  FreshBuild fresh(ctx);   // the tables were enqueued by this call on this stream: no verification launches
   GWC_TRY(gwc_event_loglik(ctx, d_theta, n_theta, ev, los, (double*)ctx->logL.p, nullptr, nullptr));
   GWC_TRY(gwc_selection_logxi(ctx, d_theta, n_theta, inj, los, (double*)ctx->logxi.p, nullptr));
   return gwc_combine_total(ctx, (const double*)ctx->logL.p, (const double*)ctx->logxi.p, n_theta, E, d_logL_total);
@@ -563,10 +600,13 @@ gwc_status gwc_total_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
   if (!ev || !inj || !d_logL_total) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL argument");
   GWC_TRY(check_los(ctx, los, true, true));
+  if (los->n_z > GWC_MAX_NZ_SELECTION)
+    return fail(ctx, GWC_ERR_SHAPE, "los->n_z > 4096 is not supported by the selection term");
   GWC_TRY(gwc_build_cosmo(ctx, d_theta, n_theta, los->z_max, n_nodes, table_prec));
   const int64_t E = ev->n_events;
   GWC_TRY(ensure(ctx, ctx->logL, (size_t)n_theta * (size_t)(E > 0 ? E : 1) * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->logxi, (size_t)n_theta * sizeof(double)));
+  FreshBuild fresh(ctx);
   GWC_TRY(gwc_event_loglik_kde(ctx, d_theta, n_theta, ev, los, n_grid, neff_min, bw_rule, (double*)ctx->logL.p,
                                nullptr, nullptr));
   GWC_TRY(gwc_selection_logxi(ctx, d_theta, n_theta, inj, los, (double*)ctx->logxi.p, nullptr));
@@ -636,11 +676,18 @@ gwc_status gwc_total_loglik_host(gwc_ctx* ctx, const double* h_theta, int64_t n_
   } else {
     GWC_TRY(gwc_los_allsky(ctx, &los, (double*)h.allsky.p));
   }
-  GWC_TRY(gwc_total_loglik(ctx, (const double*)h.theta.p, n_theta, &ev, &inj, &los, n_nodes, table_prec,
-                           (double*)h.out.p));
+  // the mirrors keep their addresses from one call to the next while their contents change: the cached preparation
+  // (gwc_cache_catalogue) must not match them
+  ctx->prep[0].valid = false;
+  ctx->prep[1].valid = false;
+  const gwc_status st_run = gwc_total_loglik(ctx, (const double*)h.theta.p, n_theta, &ev, &inj, &los, n_nodes,
+                                             table_prec, (double*)h.out.p);
+  ctx->prep[0].valid = false;
+  ctx->prep[1].valid = false;
+  ctx->built_theta = nullptr;  // the mirrored theta buffer is internal: do not let later calls match it
+  GWC_TRY(st_run);
   GWC_CUDA(cudaMemcpyAsync(h_logL_total, h.out.p, (size_t)n_theta * 8, cudaMemcpyDeviceToHost, s));
   GWC_CUDA(cudaStreamSynchronize(s));
-  ctx->built_theta = nullptr;  // the mirrored theta buffer is internal: do not let later calls match it
   if (h2d_bytes) *h2d_bytes = up;
   if (d2h_bytes) *d2h_bytes = n_theta * 8;
   return GWC_OK;

@@ -60,7 +60,9 @@ __device__ bool theta_valid(const double* th) {
 template <typename NodeT>
 __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* __restrict__ theta, double z_max,
                                                                   int M, int Mp, NodeT* __restrict__ tab,
-                                                                  double* __restrict__ tconst, int* flag) {
+                                                                  double* __restrict__ tconst,
+                                                                  double* __restrict__ theta_snap,
+                                                                  double* __restrict__ tvalid, int* flag) {
   __shared__ double Dg[QUAD_K + 1];
   __shared__ double ug[QUAD_K + 1];
   __shared__ double part[CB_THREADS];
@@ -70,10 +72,13 @@ __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* _
   NodeT* row = tab + (size_t)t * Mp;
   double* tc = tconst + (size_t)t * NCONST;
   const bool valid = theta_valid(th);
+  // the copy of theta the tables belong to (the dependent calls compare the caller's array with it)
+  if (tid < GWC_NPAR) theta_snap[(size_t)t * GWC_NPAR + tid] = th[tid];
+  if (tid == 0) tvalid[t] = valid ? 1.0 : CUDART_NAN;
   if (!valid) {
     for (int m = tid; m < Mp; m += CB_THREADS) store_node(row + m, 0.0, 0.0, 0.0);
     if (tid < NCONST) tc[tid] = (tid == C_VALID) ? CUDART_NAN : 0.0;
-    if (tid == 0) atomicOr(flag, 1);
+    if (tid == 0) atomicOr(flag, FLAG_DOMAIN);
     return;
   }
   const double Om = th[1], OL = 1.0 - Om;
@@ -202,14 +207,37 @@ __global__ void export_cosmo_kernel(const NodeT* __restrict__ tab, const double*
 }  // namespace
 
 int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int M, int Mp, gwc_prec prec, void* d_tab,
-                       double* d_tconst, int* d_flag, cudaStream_t s) {
+                       double* d_tconst, double* d_theta_snap, double* d_tvalid, int* d_flag, cudaStream_t s) {
   if (n_theta <= 0) return 0;
   if (prec == GWC_F64)
     cosmo_build_kernel<Node64><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, z_max, M, Mp, (Node64*)d_tab,
-                                                                         d_tconst, d_flag);
+                                                                         d_tconst, d_theta_snap, d_tvalid, d_flag);
   else
     cosmo_build_kernel<Node32><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, z_max, M, Mp, (Node32*)d_tab,
-                                                                         d_tconst, d_flag);
+                                                                         d_tconst, d_theta_snap, d_tvalid, d_flag);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+namespace {
+// one thread per theta: bitwise comparison of the caller's row with the copy the tables were built from
+__global__ void verify_theta_kernel(const double* __restrict__ theta, const double* __restrict__ snap,
+                                    const double* __restrict__ tconst, int64_t n_theta, double* __restrict__ tvalid,
+                                    int* flag) {
+  const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (t >= n_theta) return;
+  bool same = true;
+  for (int i = 0; i < GWC_NPAR; ++i)
+    same = same && __double_as_longlong(theta[t * GWC_NPAR + i]) == __double_as_longlong(snap[t * GWC_NPAR + i]);
+  tvalid[t] = same ? tconst[t * NCONST + C_VALID] : CUDART_NAN;
+  if (!same) atomicOr(flag, FLAG_STALE);
+}
+}  // namespace
+
+int launch_verify_theta(const double* d_theta, const double* d_theta_snap, const double* d_tconst, int64_t n_theta,
+                        double* d_tvalid, int* d_flag, cudaStream_t s) {
+  if (n_theta <= 0) return 0;
+  verify_theta_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(d_theta, d_theta_snap, d_tconst, n_theta,
+                                                                        d_tvalid, d_flag);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -89,8 +89,22 @@ struct ReweightParams {
 };
 
 // kernels / launchers (each returns the number of kernels it launched, or -1 on a launch error)
+// sticky device flag word (gwc_ctx::d_flag[0]); d_flag[1] belongs to the A0 packing alone
+enum : int {
+  FLAG_DOMAIN = 1,   // a theta point outside the model's domain (gwc_build_cosmo)
+  FLAG_STALE = 4,    // d_theta differs from the copy taken by gwc_build_cosmo
+  FLAG_RANGE = 8     // every live weight of a segment lies below e^-300 of the segment's reference
+};
+// smallest linear-domain segment sum (relative to the segment's reference) that is still trusted: below it the
+// clamped exponentials (e^-700) and the squares of the weights lose their meaning (R23)
+constexpr double RANGE_MIN_SUM = 5.148200222412013e-131;   // e^-300
+
 int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int M, int Mp, gwc_prec prec,
-                       void* d_tab, double* d_tconst, int* d_flag, cudaStream_t s);
+                       void* d_tab, double* d_tconst, double* d_theta_snap, double* d_tvalid, int* d_flag,
+                       cudaStream_t s);
+// compares d_theta with the copy gwc_build_cosmo took: tvalid[t] = tconst[t][C_VALID] or NaN (+ FLAG_STALE)
+int launch_verify_theta(const double* d_theta, const double* d_theta_snap, const double* d_tconst, int64_t n_theta,
+                        double* d_tvalid, int* d_flag, cudaStream_t s);
 int launch_export_cosmo(const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp, gwc_prec prec,
                         double z_max, double* d_z, double* d_dz, double* d_umax, cudaStream_t s);
 // per-sample, theta-independent preparation (+ per-segment shift = max(-ln pi - ln m1z))
@@ -103,21 +117,23 @@ int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_
 size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix);
 int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix);
 int reweight_configure(int smem_optin);
-int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm,
+int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm, int device,
                     cudaStream_t s);
+// tvalid [n_theta]: 1.0, or NaN for a theta outside the domain / changed since the build
 int launch_finalize_events(const double* part_w, const int32_t* part_n, const int64_t* seg_off, const double* seg_shift,
-                           const double* tconst, int64_t n_theta, int64_t n_events, double* logL, double* neff,
-                           int64_t* nlive, cudaStream_t s);
-int launch_finalize_inj(const double* part_w, const double* seg_shift, const double* tconst, int64_t n_theta,
-                        int64_t n_seg, double n_draw, double* logxi, double* neff, cudaStream_t s);
-int launch_widen_i32(const int32_t* in, const double* tconst, int64_t n_theta, int64_t n, int64_t* out,
+                           const double* tvalid, int64_t n_theta, int64_t n_events, double* logL,
+                           double* neff, int64_t* nlive, int* d_flag, cudaStream_t s);
+int launch_finalize_inj(const double* part_w, const int32_t* part_n, const double* seg_shift, const double* tvalid,
+                        int64_t n_theta, int64_t n_seg, double n_draw, double* logxi, double* neff, int* d_flag,
+                        cudaStream_t s);
+int launch_widen_i32(const int32_t* in, const double* tvalid, int64_t n_theta, int64_t n, int64_t* out,
                      cudaStream_t s);
 int launch_combine_total(const double* logL, const double* logxi, int64_t n_theta, int64_t n_events, double* total,
                          cudaStream_t s);
 int launch_allsky(const void* table, gwc_prec prec, int64_t n_rows, int n_z, double* scratch, double* allsky,
                   cudaStream_t s);
 size_t allsky_scratch_doubles(int64_t n_rows, int n_z);
-int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp,
+int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, const double* d_tvalid, int64_t n_theta, int M, int Mp,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,

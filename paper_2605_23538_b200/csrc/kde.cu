@@ -32,9 +32,10 @@ constexpr int KDE_NPL = 8;            // grid nodes per lane: G <= 256
 constexpr double C_KMS_KDE = 299792.458;
 
 struct KdeParams {
-  const double* theta;      // [n_theta][12]
+  const double* theta;      // [n_theta][12]: the copy gwc_build_cosmo took (the tables belong to it)
   const void* tab;          // [n_theta][Mp] Node64 | Node32
-  const double* tconst;     // [n_theta][NCONST] (umax, 1/du, validity)
+  const double* tconst;     // [n_theta][NCONST] (umax, 1/du)
+  const double* tvalid;     // [n_theta] 1.0, or NaN: outside the domain / changed since the build
   int64_t n_theta, n_events;
   int M, Mp;
   double tab_zq;
@@ -192,7 +193,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
     const int64_t s0 = p.ev_off[ev], s1 = p.ev_off[ev + 1];
     const size_t o = (size_t)t * (size_t)p.n_events + (size_t)ev;
     const double* th = p.theta + t * GWC_NPAR;
-    if (!(p.tconst[t * NCONST + C_VALID] == 1.0)) {   // theta outside the domain: NaN (sticky flag set by build_cosmo)
+    if (!(p.tvalid[t] == 1.0)) {   // theta outside the domain or changed since the build: NaN (sticky flag set)
       if (lane == 0) {
         p.logL[o] = CUDART_NAN;
         if (p.npass) p.npass[o] = 0;
@@ -374,14 +375,14 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
 
 }  // namespace
 
-int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp,
+int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, const double* d_tvalid, int64_t n_theta, int M, int Mp,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
                int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
   if (n_theta <= 0 || n_events <= 0) return 0;
   KdeParams p;
-  p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.n_theta = n_theta; p.n_events = n_events;
+  p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.tvalid = d_tvalid; p.n_theta = n_theta; p.n_events = n_events;
   p.M = M; p.Mp = Mp; p.tab_zq = tab_zq; p.ev_off = ev_off; p.dL = dL; p.m1z = m1z; p.m2z = m2z; p.lprior = lprior;
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
   p.n_grid = n_grid; p.neff_min = neff_min; p.bw_rule = bw_rule; p.logL = logL; p.npass = npass; p.nused = nused;

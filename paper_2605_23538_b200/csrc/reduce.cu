@@ -96,19 +96,26 @@ __global__ void max_segment_kernel(const int64_t* __restrict__ seg_off, int64_t 
 
 __global__ void finalize_events_kernel(const double* __restrict__ part_w, const int32_t* __restrict__ part_n,
                                        const int64_t* __restrict__ seg_off, const double* __restrict__ seg_shift,
-                                       const double* __restrict__ tconst, int64_t n_theta, int64_t n_events,
+                                       const double* __restrict__ tvalid, int64_t n_theta, int64_t n_events,
                                        double* __restrict__ logL, double* __restrict__ neff,
-                                       int64_t* __restrict__ nlive) {
+                                       int64_t* __restrict__ nlive, int* __restrict__ flag) {
   const int64_t o = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (o >= n_theta * n_events) return;
   const int64_t t = o / n_events, i = o - t * n_events;
-  const double valid = tconst[t * NCONST + C_VALID];
+  const double valid = tvalid[t];
   const double sw = part_w[2 * o], sw2 = part_w[2 * o + 1];
+  const int32_t n = part_n[o];
   const int64_t S = seg_off[i + 1] - seg_off[i];
   double l, ne;
   if (valid != valid) {
     l = CUDART_NAN;
     ne = CUDART_NAN;
+  } else if (n > 0 && !(sw >= RANGE_MIN_SUM)) {
+    // every live weight lies more than 300 nats below the segment's reference (a log_pe_prior of enormous spread):
+    // the linear-domain sums have left their range (gwc.h, "Range"; R23)
+    l = CUDART_NAN;
+    ne = CUDART_NAN;
+    atomicOr(flag, FLAG_RANGE);
   } else if (sw > 0.0) {
     l = (log(sw) + seg_shift[i]) - log((double)S);
     ne = sw * sw / sw2;
@@ -118,25 +125,36 @@ __global__ void finalize_events_kernel(const double* __restrict__ part_w, const 
   }
   logL[o] = l;
   if (neff) neff[o] = ne;
-  if (nlive) nlive[o] = (valid != valid) ? 0 : (int64_t)part_n[o];
+  if (nlive) nlive[o] = (valid != valid) ? 0 : (int64_t)n;
 }
 
 // one thread per theta: log-sum-exp over the injection segments (each has its own shift), fixed order
-__global__ void finalize_inj_kernel(const double* __restrict__ part_w, const double* __restrict__ seg_shift,
-                                    const double* __restrict__ tconst, int64_t n_theta, int64_t n_seg, double n_draw,
-                                    double* __restrict__ logxi, double* __restrict__ neff) {
+__global__ void finalize_inj_kernel(const double* __restrict__ part_w, const int32_t* __restrict__ part_n,
+                                    const double* __restrict__ seg_shift, const double* __restrict__ tvalid,
+                                    int64_t n_theta, int64_t n_seg, double n_draw, double* __restrict__ logxi,
+                                    double* __restrict__ neff, int* __restrict__ flag) {
   const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (t >= n_theta) return;
-  const double valid = tconst[t * NCONST + C_VALID];
+  const double valid = tvalid[t];
   if (valid != valid) {
     logxi[t] = CUDART_NAN;
     if (neff) neff[t] = CUDART_NAN;
     return;
   }
   const double* pw = part_w + 2 * t * n_seg;
+  const int32_t* pn = part_n + t * n_seg;
   double smax = -CUDART_INF;
-  for (int64_t s = 0; s < n_seg; ++s)
+  bool range = false;
+  for (int64_t s = 0; s < n_seg; ++s) {
     if (pw[2 * s] > 0.0) smax = fmax(smax, seg_shift[s]);
+    range = range || (pn[s] > 0 && !(pw[2 * s] >= RANGE_MIN_SUM));
+  }
+  if (range) {  // a segment whose live weights all lie below e^-300 of its reference (see finalize_events_kernel)
+    logxi[t] = CUDART_NAN;
+    if (neff) neff[t] = CUDART_NAN;
+    atomicOr(flag, FLAG_RANGE);
+    return;
+  }
   if (!(smax > -CUDART_INF)) {
     logxi[t] = -CUDART_INF;
     if (neff) neff[t] = 0.0;
@@ -238,12 +256,12 @@ __global__ void math_selftest_kernel(int which, int64_t n, const double* __restr
 }
 
 // int32 counts [n_theta][n] -> int64 (0 for a theta outside the domain)
-__global__ void widen_i32_kernel(const int32_t* __restrict__ in, const double* __restrict__ tconst, int64_t n_theta,
+__global__ void widen_i32_kernel(const int32_t* __restrict__ in, const double* __restrict__ tvalid, int64_t n_theta,
                                  int64_t n, int64_t* __restrict__ out) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n_theta * n) return;
   const int64_t t = i / n;
-  out[i] = tconst[t * NCONST + C_VALID] == 1.0 ? (int64_t)in[i] : 0;
+  out[i] = tvalid[t] == 1.0 ? (int64_t)in[i] : 0;
 }
 
 inline int ok() { return cudaGetLastError() == cudaSuccess ? 1 : -1; }
@@ -281,28 +299,29 @@ int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_
 }
 
 int launch_finalize_events(const double* part_w, const int32_t* part_n, const int64_t* seg_off, const double* seg_shift,
-                           const double* tconst, int64_t n_theta, int64_t n_events, double* logL, double* neff,
-                           int64_t* nlive, cudaStream_t s) {
+                           const double* tvalid, int64_t n_theta, int64_t n_events, double* logL,
+                           double* neff, int64_t* nlive, int* d_flag, cudaStream_t s) {
   const int64_t n = n_theta * n_events;
   if (n <= 0) return 0;
-  finalize_events_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(part_w, part_n, seg_off, seg_shift, tconst,
-                                                                     n_theta, n_events, logL, neff, nlive);
+  finalize_events_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(part_w, part_n, seg_off, seg_shift, tvalid,
+                                                                     n_theta, n_events, logL, neff, nlive, d_flag);
   return ok();
 }
 
-int launch_finalize_inj(const double* part_w, const double* seg_shift, const double* tconst, int64_t n_theta,
-                        int64_t n_seg, double n_draw, double* logxi, double* neff, cudaStream_t s) {
+int launch_finalize_inj(const double* part_w, const int32_t* part_n, const double* seg_shift, const double* tvalid,
+                        int64_t n_theta, int64_t n_seg, double n_draw, double* logxi, double* neff, int* d_flag,
+                        cudaStream_t s) {
   if (n_theta <= 0) return 0;
-  finalize_inj_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(part_w, seg_shift, tconst, n_theta, n_seg,
-                                                                        n_draw, logxi, neff);
+  finalize_inj_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(part_w, part_n, seg_shift, tvalid, n_theta,
+                                                                        n_seg, n_draw, logxi, neff, d_flag);
   return ok();
 }
 
-int launch_widen_i32(const int32_t* in, const double* tconst, int64_t n_theta, int64_t n, int64_t* out,
+int launch_widen_i32(const int32_t* in, const double* tvalid, int64_t n_theta, int64_t n, int64_t* out,
                      cudaStream_t s) {
   const int64_t m = n_theta * n;
   if (m <= 0) return 0;
-  widen_i32_kernel<<<(unsigned)((m + 255) / 256), 256, 0, s>>>(in, tconst, n_theta, n, out);
+  widen_i32_kernel<<<(unsigned)((m + 255) / 256), 256, 0, s>>>(in, tvalid, n_theta, n, out);
   return ok();
 }
 

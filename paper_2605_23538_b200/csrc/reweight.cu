@@ -27,6 +27,7 @@
 // segment: no floating-point atomics, results are bitwise reproducible.
 #include <math_constants.h>
 
+#include <mutex>
 #include <type_traits>
 
 #include "gwc_internal.h"
@@ -41,6 +42,19 @@ constexpr int BLK = 32 * SPT;      // samples one warp holds in registers at a t
 
 // per-theta constants of the current launch (A2), read with uniform loads
 __constant__ double KT[KT_THETA * NCONST];
+
+// The constant bank is one per device, shared by every context (and stream) of the process.  Launches that use it are
+// therefore chained across streams: a launch waits (cudaStreamWaitEvent) for the event recorded behind the previous
+// launch whenever that one went to another stream, so no copy into the bank can overtake a kernel still reading it.
+// Kernels of this size fill the GPU, so nothing is lost by running them one after the other (gwc.h, "Streams").
+constexpr int MAX_DEVICES = 64;
+struct BankGuard {
+  std::mutex mu;
+  cudaEvent_t last = nullptr;     // recorded behind the last kernel that read the bank
+  cudaStream_t last_stream = nullptr;
+  bool used = false;
+};
+BankGuard g_bank[MAX_DEVICES];
 
 struct SmemLayout {
   size_t math, acc, cnt, np, carry, carryn, lead, leadn, allsky, tab, total;
@@ -757,11 +771,15 @@ int reweight_configure(int smem_optin) {
 
 // The theta batch goes through in launches of at most KT_THETA points (a whole number of tiles): each launch
 // first copies its points' constants into the constant bank (stream-ordered) and resets the work counter.
-int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm,
+int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm, int device,
                     cudaStream_t s) {
   const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z, p0.pixcut != 0);
   const int cap = (KT_THETA / p0.T) * p0.T;
   int launched = 0;
+  if (device < 0 || device >= MAX_DEVICES) return -1;
+  BankGuard& bank = g_bank[device];
+  std::lock_guard<std::mutex> lock(bank.mu);   // the enqueue order below is the order of the event chain
+  if (!bank.last && cudaEventCreateWithFlags(&bank.last, cudaEventDisableTiming) != cudaSuccess) return -1;
   for (int tb = 0; tb < p0.n_theta; tb += cap) {
     ReweightParams p = p0;
     p.t_begin = tb;
@@ -769,6 +787,7 @@ int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_pr
     p.n_tiles = (p.n_theta + p.T - 1) / p.T;
     const int64_t n_items = (int64_t)p.n_groups * p.n_tiles;
     const int n_blocks = (int)(n_items < n_sm ? n_items : n_sm);
+    if (bank.used && bank.last_stream != s && cudaStreamWaitEvent(s, bank.last, 0) != cudaSuccess) return -1;
     if (cudaMemcpyToSymbolAsync(KT, p0.tconst + (size_t)tb * NCONST, sizeof(double) * NCONST * (size_t)p.n_theta, 0,
                                 cudaMemcpyDeviceToDevice, s) != cudaSuccess)
       return -1;
@@ -810,6 +829,9 @@ int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_pr
     }
     if (rc < 0) return -1;
     launched += rc;
+    if (cudaEventRecord(bank.last, s) != cudaSuccess) return -1;
+    bank.used = true;
+    bank.last_stream = s;
   }
   return launched;
 }

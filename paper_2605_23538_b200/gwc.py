@@ -18,9 +18,9 @@ LIB_PATH = os.path.join(_HERE, "libgwc.so")
 
 NPAR = 12
 F64, F32 = 0, 1
-OK, ERR_INVALID_ARG, ERR_SHAPE, ERR_DOMAIN, ERR_NOT_BUILT, ERR_NOMEM, ERR_CUDA = range(7)
+OK, ERR_INVALID_ARG, ERR_SHAPE, ERR_DOMAIN, ERR_NOT_BUILT, ERR_NOMEM, ERR_CUDA, ERR_RANGE = range(8)
 _STATUS = ["GWC_OK", "GWC_ERR_INVALID_ARG", "GWC_ERR_SHAPE", "GWC_ERR_DOMAIN", "GWC_ERR_NOT_BUILT", "GWC_ERR_NOMEM",
-           "GWC_ERR_CUDA"]
+           "GWC_ERR_CUDA", "GWC_ERR_RANGE"]
 
 EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_launch_count", "gwc_build_cosmo",
            "gwc_export_cosmo", "gwc_pack_events", "gwc_cap_pixels", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",

@@ -1,0 +1,320 @@
+"""GPU tests of the paths around the hot loop that round 1 left untested:
+other node counts of the cosmology table, a LOS table that ends below the cosmology table, a user PE prior of wide
+spread (the range rule of gwc.h), two contexts on two streams of one device, theta changed in place after the build,
+the catalogue cache across host calls, the flag word of the packing, the n_z limit of the selection term."""
+from __future__ import annotations
+
+import threading
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2605_23538_b200 import synth
+from util import RTOL_F64, assert_close_log, to_dev, workload
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2605_23538_b200 import gwc
+    c = gwc.Context(0)
+    yield c
+    c.close()
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _mini():
+    """Ragged O4-like mini catalogue with a box-6 theta batch (every theta its own Om)."""
+    W = workload("production", n_theta=23, n_events=9, los_rows=400, n_inj=20_000, samples=(300, 3000),
+                 pixels=(16, 200))
+    return W
+
+
+@pytest.mark.parametrize("n_nodes", [257, 2049, 4097])
+@pytest.mark.parametrize("table_prec", [0, 1])
+def test_hot_path_other_node_counts(ctx, n_nodes, table_prec):
+    """The whole hot path with M != 1025: the theta tile T, the table pitch and the shared-memory layout all change
+    with M (M = 2049 -> T = 5, M = 4097 -> T = 2 for f64 nodes)."""
+    W = _mini()
+    zmax = W.spec.z_max
+    th, ev, inj, los = W.theta.to(DEV), to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    ctx.gwc_build_cosmo(th, zmax, n_nodes, table_prec)
+    logL, neff, nlive = ctx.gwc_event_loglik(th, ev, los, zmax)
+    logxi, neffi = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], zmax)
+    total = ctx.gwc_total_loglik(th, ev, inj, los, zmax, allsky, n_nodes, table_prec)
+    gLp, _, gKp, gPp = ctx.gwc_event_loglik_pixcut(th, ev, los, zmax, 2.0)
+    ctx.gwc_check()
+    kw = dict(n_nodes=n_nodes, table_prec=table_prec)
+    ev_np, inj_np, los_np, th_np = synth.to_numpy(W.ev), synth.to_numpy(W.inj), _np(W.los), _np(W.theta)
+    oL, oN, oK = oracle.event_loglik(th_np, ev_np, los_np, zmax, **kw)
+    oX, oXn = oracle.selection_logxi(th_np, inj_np, oracle.los_allsky(los_np, zmax), zmax, **kw)
+    assert np.array_equal(_np(nlive), oK)
+    assert_close_log(_np(logL), oL, RTOL_F64, "log L_i, M=%d" % n_nodes)
+    assert_close_log(_np(logxi), oX, RTOL_F64, "log xi, M=%d" % n_nodes)
+    assert_close_log(_np(total), oracle.total_from_parts(oL, oX), RTOL_F64, "log L(theta), M=%d" % n_nodes)
+    fin = np.isfinite(oL)
+    np.testing.assert_allclose(_np(neff)[fin], oN[fin], rtol=1e-7)
+    oLp, _, oKp, oPp = oracle.event_loglik_pixcut(th_np, ev_np, los_np, zmax, 2.0, **kw)
+    assert np.array_equal(_np(gPp), oPp) and np.array_equal(_np(gKp), oKp)
+    assert_close_log(_np(gLp), oLp, RTOL_F64, "pixcut log L_i, M=%d" % n_nodes)
+
+
+def test_los_zmax_below_cosmo_zmax(ctx):
+    """gwc.h allows los->z_max <= the z_max of the build: samples with z >= los z_max are dead although the
+    cosmology table still covers them (R11)."""
+    W = workload("tiny")
+    los_zmax = W.spec.z_max            # 1.5
+    cosmo_zmax = 2.25
+    th, ev, inj, los = W.theta.to(DEV), to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    # push a good part of the samples beyond the LOS table but inside the cosmology table
+    ev["dL"] = (ev["dL"] * 2.2).contiguous()
+    ev_np = synth.to_numpy(W.ev)
+    ev_np["dL"] = ev_np["dL"] * 2.2
+    allsky = ctx.gwc_los_allsky(los, los_zmax)
+    ctx.gwc_build_cosmo(th, cosmo_zmax, 1025, 0)
+    logL, neff, nlive = ctx.gwc_event_loglik(th, ev, los, los_zmax)
+    logxi, _ = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], los_zmax)
+    ctx.gwc_check()
+    oL, oN, oK = oracle.event_loglik(_np(W.theta), ev_np, _np(W.los), los_zmax, z_max=cosmo_zmax)
+    oX, _ = oracle.selection_logxi(_np(W.theta), synth.to_numpy(W.inj), oracle.los_allsky(_np(W.los), los_zmax),
+                                   los_zmax, z_max=cosmo_zmax)
+    oK_same_zmax = oracle.event_loglik(_np(W.theta), ev_np, _np(W.los), los_zmax)[2]
+    assert (oK < W.ev["dL"].numel() // 4).any() and (oK > 0).any()
+    assert np.array_equal(_np(nlive), oK)
+    assert_close_log(_np(logL), oL, RTOL_F64, "log L_i, LOS z_max < cosmology z_max")
+    assert_close_log(_np(logxi), oX, RTOL_F64, "log xi, LOS z_max < cosmology z_max")
+    assert np.array_equal(oK, oK_same_zmax)     # same dead set as a table that ends where the LOS table ends
+    from paper_2605_23538_b200 import gwc
+    ctx.gwc_build_cosmo(th, 1.0, 1025, 0)       # a build that ends below the LOS table is refused
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_event_loglik(th, ev, los, los_zmax)
+    assert e.value.status == gwc.ERR_NOT_BUILT
+
+
+def test_wide_log_pe_prior_range_rule(ctx):
+    """R23 / gwc.h "Range": the sums are relative to max_k(-l_pi - ln m1z) over the VALID samples, whatever theta makes
+    of them.  (a) The sample that sets the reference is dead for every theta and the live ones lie 250 nats below:
+    still 1e-9.  (b) They lie 1000 nats below: the outputs of that event are NaN and gwc_check says GWC_ERR_RANGE --
+    nothing is clamped silently.  The oracle's two-pass log-sum-exp handles both."""
+    from paper_2605_23538_b200 import gwc
+    W = workload("tiny")
+    zmax = W.spec.z_max
+    th, inj, los = W.theta.to(DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    off = W.ev["ev_sample_off"]
+    a, b = int(off[1]), int(off[2])
+    for drop, expect_range in ((250.0, False), (1000.0, True)):
+        ev_cpu = {k: (v.clone() if isinstance(v, torch.Tensor) else v) for k, v in W.ev.items()}
+        lp = 2.0 * torch.log(ev_cpu["dL"])
+        lp[a:b] += drop                    # event 1: every sample's prior raised ...
+        lp[a] -= drop                      # ... except one, which sets the reference ...
+        ev_cpu["m1z"][a] = 1e5             # ... and is dead for every theta (m1 > mmax), though valid
+        ev_cpu["m2z"][a] = 9e4
+        ev_cpu["log_pe_prior"] = lp.contiguous()
+        ev = to_dev(ev_cpu, DEV)
+        ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+        logL, neff, nlive = ctx.gwc_event_loglik(th, ev, los, zmax)
+        gLp, _, gKp, gPp = ctx.gwc_event_loglik_pixcut(th, ev, los, zmax, 0.0)
+        oL, oN, oK = oracle.event_loglik(_np(W.theta), synth.to_numpy(ev_cpu), _np(W.los), zmax)
+        assert (oK[:, 1] > 0).all() and np.isfinite(oL[:, 1]).all()
+        assert np.array_equal(_np(nlive), oK)
+        if not expect_range:
+            ctx.gwc_check()
+            assert_close_log(_np(logL), oL, RTOL_F64, "log L_i, prior spread %g" % drop)
+            np.testing.assert_allclose(_np(neff), oN, rtol=1e-7)
+            assert_close_log(_np(gLp), oL, RTOL_F64, "pixcut(0) log L_i, prior spread %g" % drop)
+        else:
+            with pytest.raises(gwc.GwcError) as e:
+                ctx.gwc_check()
+            assert e.value.status == gwc.ERR_RANGE
+            ctx.gwc_check()                                        # cleared
+            g = _np(logL)
+            assert np.isnan(g[:, 1]).all() and np.isnan(_np(neff)[:, 1]).all()
+            keep = [0, 2, 3]
+            assert_close_log(g[:, keep], oL[:, keep], RTOL_F64, "the other events")
+    # the same rule for the selection term: one 8192-block of injections far below its reference
+    inj_cpu = {k: (v.clone() if isinstance(v, torch.Tensor) else v) for k, v in W.inj.items()}
+    lp = inj_cpu["log_pdraw"].clone()
+    lp[:] += 1000.0
+    lp[0] -= 1000.0
+    inj_cpu["m1z"][0] = 1e5
+    inj_cpu["m2z"][0] = 9e4
+    inj_cpu["log_pdraw"] = lp
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    logxi, _ = ctx.gwc_selection_logxi(th, to_dev(inj_cpu, DEV), allsky, los.shape[1], zmax)
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_check()
+    assert e.value.status == gwc.ERR_RANGE and torch.isnan(logxi).all()
+
+
+def test_two_contexts_two_streams(ctx):
+    """Two contexts on two streams of one device, driven from two host threads at once (the per-theta
+    constants of all contexts share the device's constant bank).  Results must equal the serial ones bit for bit."""
+    from paper_2605_23538_b200 import gwc
+    Wa = workload("o4", n_theta=700, n_events=40, los_rows=2000, n_inj=60_000)
+    Wb = workload("production", n_theta=700, n_events=30, los_rows=2000, n_inj=50_000, seed=5)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    ca, cb = gwc.Context(0, stream=sa), gwc.Context(0, stream=sb)
+    try:
+        def prep(W):
+            return (W.theta.to(DEV), to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV))
+        A, B = prep(Wa), prep(Wb)
+        torch.cuda.synchronize()
+        ska, skb = ctx.gwc_los_allsky(A[3], Wa.spec.z_max), ctx.gwc_los_allsky(B[3], Wb.spec.z_max)
+        ra = ctx.gwc_total_loglik(A[0], A[1], A[2], A[3], Wa.spec.z_max, ska).clone()
+        rb = ctx.gwc_total_loglik(B[0], B[1], B[2], B[3], Wb.spec.z_max, skb).clone()
+        torch.cuda.synchronize()
+        assert torch.isfinite(ra).any() and torch.isfinite(rb).any()
+        out = {"a": [], "b": []}
+
+        def run(c, stream, X, W, sky, key):
+            with torch.cuda.stream(stream):
+                for _ in range(6):
+                    out[key].append(c.gwc_total_loglik(X[0], X[1], X[2], X[3], W.spec.z_max, sky))
+            stream.synchronize()
+
+        ta = threading.Thread(target=run, args=(ca, sa, A, Wa, ska, "a"))
+        tb = threading.Thread(target=run, args=(cb, sb, B, Wb, skb, "b"))
+        ta.start(); tb.start(); ta.join(); tb.join()
+        torch.cuda.synchronize()
+        ca.gwc_check(); cb.gwc_check()
+        for r in out["a"]:
+            assert torch.equal(torch.nan_to_num(r, nan=1.0), torch.nan_to_num(ra, nan=1.0))
+        for r in out["b"]:
+            assert torch.equal(torch.nan_to_num(r, nan=1.0), torch.nan_to_num(rb, nan=1.0))
+        # and interleaved from one thread, no synchronisation in between
+        rs = []
+        for _ in range(4):
+            rs.append((ca.gwc_total_loglik(A[0], A[1], A[2], A[3], Wa.spec.z_max, ska),
+                       cb.gwc_total_loglik(B[0], B[1], B[2], B[3], Wb.spec.z_max, skb)))
+        torch.cuda.synchronize()
+        for x, y in rs:
+            assert torch.equal(torch.nan_to_num(x, nan=1.0), torch.nan_to_num(ra, nan=1.0))
+            assert torch.equal(torch.nan_to_num(y, nan=1.0), torch.nan_to_num(rb, nan=1.0))
+    finally:
+        ca.close(); cb.close()
+
+
+def test_theta_changed_in_place_after_build(ctx):
+    """pointer identity is not enough.  A theta row updated in place after gwc_build_cosmo must not give
+    the old point's results silently: its outputs are NaN and gwc_check says GWC_ERR_NOT_BUILT; the untouched rows
+    keep their values; the KDE path (which reads the population parameters) behaves the same."""
+    from paper_2605_23538_b200 import gwc
+    W = workload("tiny")
+    zmax = W.spec.z_max
+    th, ev, inj, los = W.theta.to(DEV).clone(), to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    ref, _, _ = ctx.gwc_event_loglik(th, ev, los, zmax)
+    refx, _ = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], zmax)
+    refk, _, _ = ctx.gwc_event_loglik_kde(th, ev, los, zmax, 64, 0.0)
+    ctx.gwc_check()
+    th[3, 0] += 5.0           # H0 of point 3
+    th[7, 6] += 1.0           # mu of point 7 (no table depends on it: only the constants do)
+    for call in ("event", "pixcut", "kde", "selection"):
+        if call == "event":
+            got = ctx.gwc_event_loglik(th, ev, los, zmax)[0]
+            want = ref
+        elif call == "pixcut":
+            got = ctx.gwc_event_loglik_pixcut(th, ev, los, zmax, 0.0)[0]
+            want = ref
+        elif call == "kde":
+            got = ctx.gwc_event_loglik_kde(th, ev, los, zmax, 64, 0.0)[0]
+            want = refk
+        else:
+            got = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], zmax)[0][:, None]
+            want = refx[:, None]
+        with pytest.raises(gwc.GwcError) as e:
+            ctx.gwc_check()
+        assert e.value.status == gwc.ERR_NOT_BUILT, call
+        assert torch.isnan(got[3]).all() and torch.isnan(got[7]).all(), call
+        keep = [i for i in range(th.shape[0]) if i not in (3, 7)]
+        if call == "pixcut":
+            np.testing.assert_allclose(_np(got[keep]), _np(want[keep]), rtol=1e-13)
+        else:
+            assert torch.equal(got[keep], want[keep]), call
+    # a rebuild makes the new values legal
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    new, _, _ = ctx.gwc_event_loglik(th, ev, los, zmax)
+    ctx.gwc_check()
+    o = oracle.event_loglik(_np(th), synth.to_numpy(W.ev), _np(W.los), zmax)[0]
+    assert_close_log(_np(new), o, RTOL_F64, "after the rebuild")
+    assert not torch.equal(new[3], ref[3])
+
+
+def test_host_calls_with_cache_on_and_two_catalogues(ctx):
+    """gwc_total_loglik_host uploads into the same internal mirrors every call; with the catalogue cache
+    on a second catalogue of the same shape must not reuse the first one's preparation."""
+    W = workload("tiny")
+    zmax = W.spec.z_max
+    ev2 = dict(W.ev, dL=(W.ev["dL"] * 1.07).contiguous(), m1z=(W.ev["m1z"] * 0.97).contiguous())
+    inj2 = dict(W.inj, dL=(W.inj["dL"] * 0.95).contiguous())
+    o1 = oracle.total_loglik(_np(W.theta), synth.to_numpy(W.ev), synth.to_numpy(W.inj), _np(W.los), zmax)
+    o2 = oracle.total_loglik(_np(W.theta), synth.to_numpy(ev2), synth.to_numpy(inj2), _np(W.los), zmax)
+    ctx.gwc_cache_catalogue(True)
+    try:
+        a, _, _ = ctx.gwc_total_loglik_host(W.theta, W.ev, W.inj, W.los, zmax)
+        a = a.clone()
+        b, _, _ = ctx.gwc_total_loglik_host(W.theta, ev2, inj2, W.los, zmax)
+        b = b.clone()
+        c, _, _ = ctx.gwc_total_loglik_host(W.theta, W.ev, W.inj, W.los, zmax)
+    finally:
+        ctx.gwc_cache_catalogue(False)
+    assert_close_log(a.numpy(), o1, RTOL_F64, "first catalogue")
+    assert_close_log(b.numpy(), o2, RTOL_F64, "second catalogue, same shapes")
+    assert np.array_equal(a.numpy(), c.numpy(), equal_nan=True)
+    assert not np.array_equal(a.numpy(), b.numpy())
+
+
+def test_pack_has_its_own_flag(ctx):
+    """a theta-domain flag left by gwc_build_cosmo is neither reported nor consumed by gwc_pack_events /
+    gwc_cap_pixels; a bad event id is reported by the packing itself and leaves nothing behind."""
+    from paper_2605_23538_b200 import gwc
+    th = torch.tensor([synth.THETA0, synth.THETA0], dtype=torch.float64)
+    th[1, 0] = -1.0
+    ctx.gwc_build_cosmo(th.to(DEV), 1.5, 257, 0)          # raises the sticky domain flag
+    g = torch.Generator().manual_seed(3)
+    eid = torch.randint(0, 5, (1000,), generator=g, dtype=torch.int32)
+    row = torch.randint(0, 40, (1000,), generator=g, dtype=torch.int32)
+    p = ctx.gwc_pack_events(eid.to(DEV), row.to(DEV), 5)  # valid input: must succeed
+    o = oracle.pack_events(eid.numpy(), row.numpy(), 5)
+    assert np.array_equal(_np(p["perm"]), o["perm"])
+    ctx.gwc_cap_pixels(p, 3, 1)
+    with pytest.raises(gwc.GwcError) as e:                # the domain flag is still there for gwc_check
+        ctx.gwc_check()
+    assert e.value.status == gwc.ERR_DOMAIN
+    bad = eid.clone()
+    bad[17] = 9
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_pack_events(bad.to(DEV), row.to(DEV), 5)
+    assert e.value.status == gwc.ERR_DOMAIN
+    ctx.gwc_check()                                        # nothing left behind
+    ctx.gwc_pack_events(eid.to(DEV), row.to(DEV), 5)       # and the next valid call is fine
+
+
+def test_nz_limit_checked_before_any_work(ctx):
+    from paper_2605_23538_b200 import gwc
+    W = workload("tiny")
+    th, ev, inj = W.theta.to(DEV), to_dev(W.ev, DEV), to_dev(W.inj, DEV)
+    nz = 4097
+    los = torch.rand(8, nz, dtype=torch.float64, device=DEV) + 0.5
+    allsky = ctx.gwc_los_allsky(los, 1.5)
+    n0 = ctx.gwc_launch_count()
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_total_loglik(th, ev, inj, los, 1.5, allsky)
+    assert e.value.status == gwc.ERR_SHAPE and ctx.gwc_launch_count() == n0
+    # the event term alone takes it (the LOS rows stay in global memory)
+    ctx.gwc_build_cosmo(th, 1.5, 1025, 0)
+    logL, _, nlive = ctx.gwc_event_loglik(th, ev, los, 1.5)
+    ctx.gwc_check()
+    oL, _, oK = oracle.event_loglik(_np(W.theta), synth.to_numpy(W.ev), _np(los), 1.5)
+    assert np.array_equal(_np(nlive), oK)
+    assert_close_log(_np(logL), oL, RTOL_F64, "log L_i, n_z = 4097")

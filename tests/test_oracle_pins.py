@@ -762,3 +762,64 @@ def test_kde_silverman_bandwidth_through_quadratic_prior(theta0):
         assert Lk[0, i] == pytest.approx(want, abs=2e-6)
         assert abs(Ls[0, i] - Lk[0, i]) > 1e-4            # and it is not Scott's bandwidth
     assert used_iqr > 0 and used_sigma > 0
+
+
+# ---------------------------------------------------------------- 32-bit table storage (R22)
+@pytest.mark.parametrize("Om,zmax,M", [(0.3, 2.0, 1025), (0.1, 1.5, 257), (1.0, 2.0, 1025)])
+def test_round_table_32_quantisation_bounds(Om, zmax, M):
+    """orc_round_table_32 against what R22 fixes: nodes are the nearest multiple of q = z_max/(2^32-1) (so
+    |z32 - z64| <= q/2, z32/q an integer in [0, 2^32-1]); slopes are the nearest binary32 in units of q (relative
+    error <= 2^-24, the stored number exactly a float)."""
+    zt, dt, um = O.build_table(Om, zmax, M)
+    z32, d32 = O.round_table_32(zt, dt, zmax)
+    q = zmax / 4294967295.0
+    assert np.abs(z32 - zt).max() <= 0.5 * q * (1 + 1e-9)
+    k = z32 / q
+    assert np.abs(k - np.rint(k)).max() <= 1e-5 and k.min() >= 0 and k.max() <= 4294967295.0 + 1e-5
+    assert z32[0] == 0.0 and abs(z32[-1] - zmax) <= 1e-15
+    # independent restatement with numpy's own rounding
+    np.testing.assert_array_equal(np.rint(zt / q), np.rint(k))
+    assert np.abs(d32 / dt - 1.0).max() <= 2.0 ** -24 * (1 + 1e-9)
+    assert np.abs(d32 / dt - 1.0).max() > 2.0 ** -30          # the slopes really were rounded
+    f = d32 / q
+    np.testing.assert_allclose(f.astype(np.float32).astype(np.float64), f, rtol=4e-16, atol=0)
+    np.testing.assert_allclose((dt / q).astype(np.float32).astype(np.float64) * q, d32, rtol=4e-16, atol=0)
+
+
+def test_round_table_32_bound_on_loglik(theta0):
+    """table_prec = 1 against table_prec = 0 on the toy event: the node and slope roundings move z by at most
+    dz = q/2 + 2^-24 max|d_m| 4/27 (Hermite basis functions), hence log L_i by at most dz * max |d ln w / dz|;
+    the LOS term dominates that derivative and is bounded from the table itself."""
+    ev, tab, zmax = _toy_event(n=600)
+    M = 1025
+    zt, dt, um = O.build_table(theta0[1], zmax, M)
+    q = zmax / 4294967295.0
+    dz = 0.5 * q + 2.0 ** -24 * np.abs(dt).max() * (4.0 / 27.0)
+    step = zmax / (tab.shape[1] - 1)
+    g_los = (np.abs(np.diff(tab, axis=1)) / np.minimum(tab[:, 1:], tab[:, :-1])).max() / step
+    bound = dz * (g_los + 60.0)       # 60: generous bound on the population / rate / Jacobian terms' slopes in z
+    for H0 in (50.0, 70.0, 100.0):
+        th = theta0.copy(); th[0] = H0
+        L0, n0, k0 = O.event_loglik(th, ev, tab, zmax, table_prec=0, n_nodes=M)
+        L1, n1, k1 = O.event_loglik(th, ev, tab, zmax, table_prec=1, n_nodes=M)
+        assert np.array_equal(k0, k1)
+        d = np.abs(L1 - L0).max()
+        assert 1e-14 < d <= bound, (d, bound)
+        # the look-up itself, restated: Hermite on the rounded arrays
+        z32, d32 = O.round_table_32(zt, dt, zmax)
+        for u in (0.1 * um, 0.37 * um, 0.9 * um):
+            a, b = O.z_table(u, zt, dt, um), O.z_table(u, z32, d32, um)
+            assert abs(a - b) <= dz * (1 + 1e-9)
+
+
+def test_norm_pl_alpha_one_branch(theta0):
+    """alpha = 1: the log limit of the power-law normalisation, 1 / ln(mmax/mmin), by quadrature and by continuity."""
+    th = theta0.copy(); th[2] = 1.0; th[8] = 0.0
+    assert O.norm_pl(th) == pytest.approx(1.0 / math.log(th[5] / th[4]), rel=1e-15)
+    val, err = integrate.quad(lambda m: O.p1(m, th), th[4], th[5], epsabs=0, epsrel=1e-12, limit=200)
+    assert val == pytest.approx(1.0, abs=1e-10)
+    assert O.p1(20.0, th) == pytest.approx(1.0 / (20.0 * math.log(th[5] / th[4])), rel=1e-14)
+    for eps in (1e-6, -1e-6):
+        th2 = th.copy(); th2[2] = 1.0 + eps
+        assert O.norm_pl(th2) == pytest.approx(O.norm_pl(th), rel=1e-5)
+        assert O.p1(20.0, th2) == pytest.approx(O.p1(20.0, th), rel=1e-5)
