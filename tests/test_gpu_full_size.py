@@ -119,35 +119,35 @@ def test_full_size_sampled(ctx, name):
 
 def test_stress_f64_and_f32_tables(ctx):
     """Config 5: FP64 tables against the oracle at 1e-9; FP32 tables (LOS + cosmology) against the FP64 oracle at
-    1e-4 absolute on log L(theta), and at 1e-9 against the oracle run on the same rounded tables."""
+    1e-4 absolute on log L(theta) for every theta, and at 1e-9 against the oracle run on the same rounded tables."""
     W, theta = _device_workload("stress")
     assert W.los.dtype == torch.float64
     g64 = _run_gpu(ctx, W, theta, W.los, 0)
     r64 = _check_sampled(W, theta, W.los, g64, 0)
     los32 = W.los.to(torch.float32)
     g32 = _run_gpu(ctx, W, theta, los32, 1)
-    # same rounded tables on both sides; a node whose f64 value sits on an f32 rounding boundary may round apart
-    # (|dz| <= 6e-8 on that interval), so this comparison is looser and nlive is not required to be identical
-    _check_sampled(W, theta, los32, g32, 1, n_ev=4, rtol=1e-6, check_nlive=False)
-    # A sample whose z (or m1 = m1z/(1+z)) lies within the f32 rounding of the z table (|dz| <= 6e-8 z) of a support
-    # edge is live with one table and dead with the other (DESIGN.md R20/R22).  Such a flip changes log L_i by about
-    # w_k / sum w, far more than rounding does, so theta points with a flip are found through nlive, counted,
-    # printed and required to be rare; every other theta must meet north_star's 1e-4.
+    # same rounded tables on both sides (R22: the oracle rounds its own exact nodes the same way): the 1e-9 bar and
+    # bit-exact nlive hold here too (observed <= 5e-13)
+    _check_sampled(W, theta, los32, g32, 1, n_ev=4)
+    # north_star's bar for the 32-bit-table path: |delta log L(theta)| <= 1e-4 absolute, every theta, no exception.
+    # A sample that the coarser table moved across a support edge (DESIGN.md R20/R22) would show in nlive: the
+    # fixed-point nodes leave none on this config, and the test demands none.
     same = (g32["nlive"] == g64["nlive"]).all(dim=1).cpu().numpy()
     a, b = _np(g32["total"]), _np(g64["total"])
+    assert np.array_equal(np.isfinite(a), np.isfinite(b)) and np.array_equal(np.isnan(a), np.isnan(b))
     both = np.isfinite(a) & np.isfinite(b)
-    d = np.abs(a - b)
+    d = np.abs(a[both] - b[both])
     n_flip = int((~same).sum())
-    print("stress f32 tables vs f64 tables, %d theta: max |dlogL(theta)| = %.3e without a flip (%d theta), "
-          "%.3e with one (%d theta)" % (both.sum(), d[both & same].max(), (both & same).sum(),
-                                        d[both & ~same].max() if (both & ~same).any() else 0.0, n_flip))
-    assert (both & same).sum() >= 0.9 * both.sum()
-    assert d[both & same].max() <= ATOL_F32
-    assert n_flip <= 0.1 * same.size
-    # against the FP64 oracle on the theta subset (flip-free points)
+    print("stress 32-bit tables vs f64 tables: %d theta finite in both, max |dlogL(theta)| = %.3e, %d theta with a "
+          "sample flipped across a support edge" % (both.sum(), d.max(), n_flip))
+    assert both.sum() >= 0.4 * both.size
+    assert n_flip == 0
+    assert d.max() <= ATOL_F32
+    # against the FP64 oracle on the theta subset
     tsel = r64["tsel"]
     t32, t64 = a[tsel], r64["total"]
-    fin = np.isfinite(t64) & np.isfinite(t32) & same[tsel]
+    assert np.array_equal(np.isfinite(t32), np.isfinite(t64))
+    fin = np.isfinite(t64)
     assert fin.any()
     assert np.abs(t32[fin] - t64[fin]).max() <= ATOL_F32
 
