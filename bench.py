@@ -114,6 +114,63 @@ def _pin(t):
 
 
 # ---------------------------------------------------------------------------------------------
+def run_leg(args):
+    """One leg alone (profiling runs: the command an ncu capture under profiles/ names): `events` = gwc_event_loglik,
+    `pixcut` = gwc_event_loglik_pixcut at --pixcut, `kde` = gwc_event_loglik_kde on --kde-theta points, `inj` =
+    gwc_selection_logxi.  W warm-up calls, K timed ones (kernel time by CUDA events on the library's stream)."""
+    from paper_2605_23538_b200 import gwc
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the gwc path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    spec = _bench_spec(args.workload, args.theta_scale)
+    W = synth.make_workload(spec, seed=args.seed, device=dev, keep_f64_los=False)
+    theta = synth.make_theta(spec, args.seed, dev)
+    ctx = gwc.Context(0)
+    zmax = spec.z_max
+    prec = gwc.F32 if args.table_prec == "f32" else gwc.F64
+    if args.leg == "kde":
+        theta = theta[:min(max(args.kde_theta, 1), theta.shape[0])].contiguous()
+    allsky = ctx.gwc_los_allsky(W.los, zmax)
+    ctx.gwc_build_cosmo(theta, zmax, args.n_nodes, prec)
+    n_theta, n_samples = int(theta.shape[0]), W.n_samples
+    units, extra = float(n_theta) * n_samples, {}
+
+    def call():
+        if args.leg == "events":
+            return ctx.gwc_event_loglik(theta, W.ev, W.los, zmax, want_neff=False, want_nlive=True)[2]
+        if args.leg == "pixcut":
+            return ctx.gwc_event_loglik_pixcut(theta, W.ev, W.los, zmax, max(args.pixcut, 0.0))[3]
+        if args.leg == "kde":
+            return ctx.gwc_event_loglik_kde(theta, W.ev, W.los, zmax, 256, 2.0, args.kde_bandwidth)[2]
+        return ctx.gwc_selection_logxi(theta, W.inj, allsky, W.los.shape[1], zmax)[0]
+
+    for _ in range(max(args.warmup, 1)):
+        r = call()
+    torch.cuda.synchronize()
+    ctx.gwc_set_timing(True)
+    ctx.gwc_get_timing()
+    for _ in range(args.steps):
+        r = call()
+    torch.cuda.synchronize()
+    tm = ctx.gwc_get_timing()
+    ctx.gwc_set_timing(False)
+    ctx.gwc_check()
+    key = "inj" if args.leg == "inj" else "ev"
+    ms = tm["ms_" + key] / max(tm["n_" + key], 1)
+    if args.leg == "inj":
+        units = float(n_theta) * int(W.inj["dL"].numel())
+    elif args.leg == "kde":
+        extra["gaussian_evals_per_s"] = float(r.sum().item()) * 256.0 / (ms * 1e-3)
+    elif args.leg == "events":
+        extra["live_fraction"] = float(r.sum().item()) / units
+    else:
+        extra["mean_passing_pixels_per_event"] = float(r.double().mean())
+    print(json.dumps(dict({"leg": args.leg, "workload": spec.name, "n_theta": n_theta, "kernel_ms": ms,
+                           "terms_per_s": units / (ms * 1e-3)}, **extra)))
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------
 def run_gwc(args):
     from paper_2605_23538_b200 import gwc
     rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -463,6 +520,9 @@ def main():
                     help="also time this many one-theta calls with the catalogue cache on (0: skip)")
     ap.add_argument("--kde-theta", type=int, default=16,
                     help="also time the KDE-numerator event term on this many theta points (0: skip)")
+    ap.add_argument("--leg", default="all", choices=["all", "events", "pixcut", "kde", "inj"],
+                    help="run one leg alone and print its kernel time (profiling runs)")
+    ap.add_argument("--kde-bandwidth", default="scott")
     ap.add_argument("--pixcut", type=float, default=2.0,
                     help="also time the event term with the per-pixel N_eff cut at this threshold (< 0: skip)")
     args = ap.parse_args()
@@ -470,6 +530,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         run_reference(args)
+    elif args.leg != "all":
+        run_leg(args)
     else:
         run_gwc(args)
 

@@ -29,6 +29,7 @@ namespace {
 constexpr int KDE_THREADS = 256;
 constexpr int KDE_WARPS = KDE_THREADS / 32;
 constexpr int KDE_NPL = 8;            // grid nodes per lane: G <= 256
+constexpr double KDE_BETA_MAX = 3.0;  // fast path of the KDE pass: grid step <= 3 h sqrt(2)
 constexpr double C_KMS_KDE = 299792.458;
 
 struct KdeParams {
@@ -227,11 +228,11 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
 #pragma unroll
       for (int i = 0; i < KDE_NPL; ++i) {
-        const int g = lane + 32 * i;
+        const int g = KDE_NPL * lane + i;   // a lane owns 8 consecutive nodes; stored [i][lane]: conflict-free
         const double x = 1.0 + g * dzg;
         const double psi = psi0 * pow(x, gam) / (1.0 + pow(x / (1.0 + zp), gam + kap));
         const double c = (g == 0 || g == G - 1) ? 0.5 * dzg : dzg;
-        s_rg[g] = g < G ? c * psi / x : 0.0;
+        s_rg[i * 32 + lane] = g < G ? c * psi / x : 0.0;
       }
     }
     __syncwarp();
@@ -321,21 +322,68 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         double acc[KDE_NPL];
 #pragma unroll
         for (int i = 0; i < KDE_NPL; ++i) acc[i] = 0.0;
-        for (int64_t c0 = r0; c0 < r1; c0 += 32) {
-          const int64_t k = c0 + lane;
-          double zs = 0.0, a = 0.0;   // z_k / (h sqrt 2), v_k / (h sqrt(2 pi))
-          if (k < r1) {
-            const double2 zv = scr[k];
-            a = zv.y >= 0.0 ? zv.y * norm : 0.0;
-            zs = zv.x * sinvh;
+        const double beta = dzg * sinvh;   // grid step in units of h sqrt(2)
+        if (beta <= KDE_BETA_MAX) {
+          // Fast path (the grid resolves the kernel: h >= dz / 4.2).  A lane owns KDE_NPL CONSECUTIVE nodes
+          // g = 8 lane + s.  With q_c = (8 lane + 4) beta - z_k / (h sqrt 2) the exponent at node s is
+          //   -(q_c + o beta)^2 = -q_c^2 - 2 o beta q_c - o^2 beta^2,   o = s - 4,
+          // so N(z_g; z_k, h) = E P^o C_o with E = exp(-q_c^2), P = exp(-2 beta q_c) and the per-pixel constants
+          // C_o = exp(-o^2 beta^2), which leave the sum over samples: two exponentials and a reciprocal per
+          // (sample, lane) instead of eight exponentials, the other nodes by multiplication (every intermediate is a
+          // Gaussian value <= 1).  q_c is clamped to +-(12.5 + 4 beta): beyond it every node of the lane is below
+          // e^-156 of the sample's own peak, and inside the clamp all arguments stay within the range of exp_fast.
+          const double qL = (double)(KDE_NPL * lane + 4) * beta;
+          const double Qc = 12.5 + 4.0 * beta;
+          const double g2 = -2.0 * beta;
+          for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+            const int64_t k = c0 + lane;
+            double zs = 0.0, a = 0.0;   // z_k / (h sqrt 2), v_k / (h sqrt(2 pi))
+            if (k < r1) {
+              const double2 zv = scr[k];
+              a = zv.y >= 0.0 ? zv.y * norm : 0.0;
+              zs = zv.x * sinvh;
+            }
+            const int cnt = (int)min((int64_t)32, r1 - c0);
+#pragma unroll 2
+            for (int j = 0; j < cnt; ++j) {
+              const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
+              const double qc = fmin(fmax(qL - zj, -Qc), Qc);
+              const double E = exp_fast<false>(-qc * qc, exptab);
+              const double P = exp_fast<false>(g2 * qc, exptab);
+              const double Pi = rcp_fast(P);
+              const double u1 = E * P, u2 = u1 * P, u3 = u2 * P;
+              const double d1 = E * Pi, d2 = d1 * Pi, d3 = d2 * Pi, d4 = d3 * Pi;
+              acc[0] = fma(aj, d4, acc[0]);
+              acc[1] = fma(aj, d3, acc[1]);
+              acc[2] = fma(aj, d2, acc[2]);
+              acc[3] = fma(aj, d1, acc[3]);
+              acc[4] = fma(aj, E, acc[4]);
+              acc[5] = fma(aj, u1, acc[5]);
+              acc[6] = fma(aj, u2, acc[6]);
+              acc[7] = fma(aj, u3, acc[7]);
+            }
           }
-          const int cnt = (int)min((int64_t)32, r1 - c0);
-          for (int j = 0; j < cnt; ++j) {
-            const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
+          const double c1 = exp_fast<false>(-beta * beta, exptab);   // C_o = c1^(o^2)
+          const double c2 = c1 * c1, c4 = c2 * c2, c8 = c4 * c4, c9 = c8 * c1, c16 = c8 * c8;
+          acc[0] *= c16; acc[1] *= c9; acc[2] *= c4; acc[3] *= c1; acc[5] *= c1; acc[6] *= c4; acc[7] *= c9;
+        } else {
+          // narrow kernels (h < dz / 4.2, a degenerate pixel): every Gaussian by its own exponential
+          for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+            const int64_t k = c0 + lane;
+            double zs = 0.0, a = 0.0;
+            if (k < r1) {
+              const double2 zv = scr[k];
+              a = zv.y >= 0.0 ? zv.y * norm : 0.0;
+              zs = zv.x * sinvh;
+            }
+            const int cnt = (int)min((int64_t)32, r1 - c0);
+            for (int j = 0; j < cnt; ++j) {
+              const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
 #pragma unroll
-            for (int i = 0; i < KDE_NPL; ++i) {
-              const double q = fma((double)(lane + 32 * i), dzg * sinvh, -zj);
-              acc[i] = fma(aj, exp_fast<true>(-q * q, exptab), acc[i]);
+              for (int i = 0; i < KDE_NPL; ++i) {
+                const double q = fma((double)(KDE_NPL * lane + i), beta, -zj);
+                acc[i] = fma(aj, exp_fast<true>(-q * q, exptab), acc[i]);
+              }
             }
           }
         }
@@ -344,7 +392,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         double part = 0.0;
 #pragma unroll
         for (int i = 0; i < KDE_NPL; ++i) {
-          const int g = lane + 32 * i;
+          const int g = KDE_NPL * lane + i;
           if (g < G) {
             const double zg = fmin(g * dzg, p.los_zmax);
             const double tz = zg / dzl;
@@ -352,7 +400,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
             b = b > p.n_z - 2 ? p.n_z - 2 : b;
             const double fz = tz - (double)b;
             const double q0 = (double)lrow[b], q1 = (double)lrow[b + 1];
-            part = fma(acc[i], (q0 + fz * (q1 - q0)) * s_rg[g], part);
+            part = fma(acc[i], (q0 + fz * (q1 - q0)) * s_rg[i * 32 + lane], part);
           }
         }
         const double I = wsum(part);
