@@ -172,12 +172,118 @@ __device__ double live_quantile(const double2* scr, int64_t r0, int64_t r1, int6
   return x0 + f * (x1 - x0);
 }
 
+// The KDE of one pixel on the grid times the prior, Eq. 5-6: returns this lane's share of
+// I_j = sum_g c_g R(z_g) p_los(z_g | row) sum_k v_k N(z_g; z_k, h)  (lanes own KDE_NPL consecutive nodes each;
+// the caller adds the lanes' shares of all pixels and reduces once per event).  s_w: per-node prior weights of this
+// theta, [i][lane] pairs (w0, w1) = c_g R(z_g) (1 - f_g, f_g) for the two LOS nodes around z_g, and the index b_g.
+struct NodeW { double w0, w1; };
+template <typename LosT>
+__device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int64_t r0, int64_t r1, double h,
+                                            int32_t prow, const KdeParams& p, double dzg, const NodeW* s_w,
+                                            const int* s_b, const double* exptab, int lane) {
+  const unsigned FULL = 0xffffffffu;
+  // the LOS nodes this lane needs (8 consecutive grid nodes = a few cache lines of the row) are pulled into L1 now:
+  // the latency hides behind the sample loop, and no register is held across it
+  const LosT* lrow = reinterpret_cast<const LosT*>(p.los) + (size_t)prow * (size_t)p.n_z;
+#pragma unroll
+  for (int i = 0; i < KDE_NPL; i += 2) asm volatile("prefetch.global.L1 [%0];" ::"l"(lrow + s_b[i * 32 + lane]));
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(lrow + s_b[(KDE_NPL - 1) * 32 + lane] + 1));
+  const double invh = 1.0 / h;
+  const double norm = invh * 0.39894228040143267794;   // 1 / (h sqrt(2 pi))
+  const double sinvh = invh * 0.70710678118654752440;  // so that the exponent is -(q')^2
+  double acc[KDE_NPL];
+#pragma unroll
+  for (int i = 0; i < KDE_NPL; ++i) acc[i] = 0.0;
+  const double beta = dzg * sinvh;   // grid step in units of h sqrt(2)
+  if (beta <= KDE_BETA_MAX) {
+    // Fast path (the grid resolves the kernel: h >= dz / 4.2).  A lane owns KDE_NPL CONSECUTIVE nodes
+    // g = 8 lane + s.  With q_c = (8 lane + 4) beta - z_k / (h sqrt 2) the exponent at node s is
+    //   -(q_c + o beta)^2 = -q_c^2 - 2 o beta q_c - o^2 beta^2,   o = s - 4,
+    // so N(z_g; z_k, h) = E P^o C_o with E = exp(-q_c^2), P = exp(-2 beta q_c) and the per-pixel constants
+    // C_o = exp(-o^2 beta^2), which leave the sum over samples: two exponentials and a reciprocal per
+    // (sample, lane) instead of eight exponentials, the other nodes by multiplication (every intermediate is a
+    // Gaussian value <= 1).  q_c is clamped to +-(12.5 + 4 beta): beyond it every node of the lane is below
+    // e^-156 of the sample's own peak, and inside the clamp all arguments stay within the range of exp_fast.
+    const double qL = (double)(KDE_NPL * lane + 4) * beta;
+    const int hiQc = __double2hiint(12.5 + 4.0 * beta);   // the clamp compares high words (2^-20 below the limit)
+    const double g2 = -2.0 * beta;
+    for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+      const int64_t k = c0 + lane;
+      double zs = 0.0, a = 0.0;   // z_k / (h sqrt 2), v_k / (h sqrt(2 pi))
+      if (k < r1) {
+        const double2 zv = scr[k];
+        a = zv.y >= 0.0 ? zv.y * norm : 0.0;
+        zs = zv.x * sinvh;
+      }
+      const int cnt = (int)min((int64_t)32, r1 - c0);
+#pragma unroll 2
+      for (int j = 0; j < cnt; ++j) {
+        const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
+        double qc = qL - zj;
+        {
+          const int hi = __double2hiint(qc);
+          const bool far = (hi & 0x7fffffff) >= hiQc;
+          qc = __hiloint2double(far ? ((hi & (int)0x80000000) | hiQc) : hi, far ? 0 : __double2loint(qc));
+        }
+        const double E = exp_fast<false>(-qc * qc, exptab);
+        const double P = exp_fast<false>(g2 * qc, exptab);
+        const double Pi = rcp_fast(P);
+        const double P2 = P * P, Pi2 = Pi * Pi;
+        const double u1 = E * P, u2 = E * P2, u3 = u1 * P2;
+        const double d1 = E * Pi, d2 = E * Pi2, d3 = d1 * Pi2, d4 = d2 * Pi2;
+        acc[0] = fma(aj, d4, acc[0]);
+        acc[1] = fma(aj, d3, acc[1]);
+        acc[2] = fma(aj, d2, acc[2]);
+        acc[3] = fma(aj, d1, acc[3]);
+        acc[4] = fma(aj, E, acc[4]);
+        acc[5] = fma(aj, u1, acc[5]);
+        acc[6] = fma(aj, u2, acc[6]);
+        acc[7] = fma(aj, u3, acc[7]);
+      }
+    }
+    const double c1 = exp_fast<false>(-beta * beta, exptab);   // C_o = c1^(o^2)
+    const double c2 = c1 * c1, c4 = c2 * c2, c8 = c4 * c4, c9 = c8 * c1, c16 = c8 * c8;
+    acc[0] *= c16; acc[1] *= c9; acc[2] *= c4; acc[3] *= c1; acc[5] *= c1; acc[6] *= c4; acc[7] *= c9;
+  } else {
+    // narrow kernels (h < dz / 4.2, a degenerate pixel): every Gaussian by its own exponential
+    for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+      const int64_t k = c0 + lane;
+      double zs = 0.0, a = 0.0;
+      if (k < r1) {
+        const double2 zv = scr[k];
+        a = zv.y >= 0.0 ? zv.y * norm : 0.0;
+        zs = zv.x * sinvh;
+      }
+      const int cnt = (int)min((int64_t)32, r1 - c0);
+      for (int j = 0; j < cnt; ++j) {
+        const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
+#pragma unroll
+        for (int i = 0; i < KDE_NPL; ++i) {
+          const double q = fma((double)(KDE_NPL * lane + i), beta, -zj);
+          acc[i] = fma(aj, exp_fast<true>(-q * q, exptab), acc[i]);
+        }
+      }
+    }
+  }
+  // prior at the lane's nodes: p_los(z_g | row) by the table's linear interpolation, times c_g R(z_g)
+  double part = 0.0;
+#pragma unroll
+  for (int i = 0; i < KDE_NPL; ++i) {
+    const NodeW w = s_w[i * 32 + lane];
+    const int b = s_b[i * 32 + lane];
+    part = fma(acc[i], fma((double)lrow[b + 1], w.w1, (double)lrow[b] * w.w0), part);
+  }
+  return part;
+}
+
 template <typename NodeT, typename LosT>
 __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) {
   extern __shared__ __align__(16) unsigned char kde_smem[];
   MathTables& mt = *reinterpret_cast<MathTables*>(kde_smem);
-  // rate term at the grid nodes, one row per warp (kept out of the registers of the KDE loop)
-  double* s_rg = reinterpret_cast<double*>(kde_smem + sizeof(MathTables)) + (threadIdx.x >> 5) * (32 * KDE_NPL);
+  // prior weights at the grid nodes, one set per warp (they depend on theta), and the LOS bin of every grid node
+  NodeW* s_w = reinterpret_cast<NodeW*>(kde_smem + sizeof(MathTables)) + (threadIdx.x >> 5) * (32 * KDE_NPL);
+  int* s_b = reinterpret_cast<int*>(kde_smem + sizeof(MathTables) + sizeof(NodeW) * KDE_WARPS * 32 * KDE_NPL);
+  double* s_fz = reinterpret_cast<double*>(s_b + 32 * KDE_NPL);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   init_math_tables(mt, tid, KDE_THREADS);
   __syncthreads();
@@ -188,6 +294,16 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
   const double dzg = p.los_zmax / (G - 1);
   const double dzl = p.los_zmax / (p.n_z - 1);
   const int64_t n_units = p.n_theta * p.n_events;
+  if (tid < 32 * KDE_NPL) {   // LOS bin and fraction of grid node g = 8 l + i, stored at [i][l]
+    const int g = tid, l = g / KDE_NPL, i = g % KDE_NPL;
+    const double zg = fmin(g * dzg, p.los_zmax);
+    const double tz = zg / dzl;
+    int b = (int)floor(tz);
+    b = b > p.n_z - 2 ? p.n_z - 2 : b;
+    s_b[i * 32 + l] = b;
+    s_fz[i * 32 + l] = tz - (double)b;
+  }
+  __syncthreads();
 
   for (int64_t unit = (int64_t)blockIdx.x * KDE_WARPS + warp; unit < n_units; unit += (int64_t)gridDim.x * KDE_WARPS) {
     const int64_t ev = unit / p.n_theta, t = unit - ev * p.n_theta;   // event-major
@@ -222,7 +338,8 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       K.Om = th[1];
       K.OL = 1.0 - th[1];
     }
-    // rate term times the trapezoid weight at this lane's grid nodes: c_g psi(z_g) / (1 + z_g)   (reading R4)
+    // prior weights at this lane's grid nodes: c_g psi(z_g) / (1 + z_g) (trapezoid weight, reading R4) split over the
+    // two LOS nodes around z_g (the table's own linear interpolation, R10)
     {
       const double gam = th[9], kap = th[10], zp = th[11];
       const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
@@ -232,7 +349,10 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         const double x = 1.0 + g * dzg;
         const double psi = psi0 * pow(x, gam) / (1.0 + pow(x / (1.0 + zp), gam + kap));
         const double c = (g == 0 || g == G - 1) ? 0.5 * dzg : dzg;
-        s_rg[i * 32 + lane] = g < G ? c * psi / x : 0.0;
+        const double w = g < G ? c * psi / x : 0.0;
+        const double fz = s_fz[i * 32 + lane];
+        s_w[i * 32 + lane].w0 = w * (1.0 - fz);
+        s_w[i * 32 + lane].w1 = w * fz;
       }
     }
     __syncwarp();
@@ -255,163 +375,104 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       }
     }
     __syncwarp();
-    double esum = 0.0;   // sum over the passing pixels of I_j, relative to e^shift
+    double esum = 0.0;   // this lane's share of the sum over the contributing pixels of I_j, relative to e^shift
     int np = 0;
     int64_t nu = 0;
-
-    int64_t r0 = s0;
-    while (r0 < s1) {
-      // ---- the pixel: samples r0 .. r1-1 with the row of r0 ----
-      const int32_t prow = p.row[r0];
-      int64_t r1 = r0 + 1;
-      for (;;) {
-        const int64_t g = r1 + lane;
-        const unsigned stop = __ballot_sync(FULL, g >= s1 || p.row[g < s1 ? g : s1 - 1] != prow);
-        if (stop) { r1 += __ffs(stop) - 1; break; }
-        r1 += 32;
-      }
-      // ---- pass 1: sum v, sum v z, sum v^2, live count ----
-      double V = 0.0, Vz = 0.0, Q = 0.0;
-      int n = 0;
-      for (int64_t c0 = r0; c0 < r1; c0 += 32) {
-        const int64_t k = c0 + lane;
-        double z = 0.0, v = 0.0;
-        if (k < r1) {
-          const double2 zv = scr[k];
-          z = zv.x;
-          v = zv.y >= 0.0 ? zv.y : 0.0;
-          n += zv.y >= 0.0 ? 1 : 0;
-        }
-        V += v;
-        Vz = fma(v, z, Vz);
-        Q = fma(v, v, Q);
-      }
-      V = wsum(V); Vz = wsum(Vz); Q = wsum(Q);
-      n = __reduce_add_sync(FULL, n);
-      bool pass = n >= 2 && V > 0.0 && V * V >= p.neff_min * Q;   // warp-uniform
-      double h = 0.0;
-      if (pass) {
-        // ---- pass 2: centred second moment ----
-        const double mu = Vz / V;
-        double S2 = 0.0;
-        for (int64_t c0 = r0; c0 < r1; c0 += 32) {
-          const int64_t k = c0 + lane;
-          if (k < r1) {
-            const double2 zv = scr[k];
-            const double v = zv.y >= 0.0 ? zv.y : 0.0;
-            S2 = fma(v * (zv.x - mu), zv.x - mu, S2);
-          }
-        }
-        S2 = wsum(S2);
-        const double var = S2 / V;
-        pass = var > 0.0;
-        h = 1.06 * sqrt(var) * pow((double)n, -0.2);   // Eq. D1
-        if (pass && p.bw_rule == 1) {                  // Eq. D2
-          const double iqr = live_quantile(scr, r0, r1, n, 0.75, lane) - live_quantile(scr, r0, r1, n, 0.25, lane);
-          double spread = sqrt(var);
-          spread = iqr / 1.34 < spread ? iqr / 1.34 : spread;
-          h = 0.9 * spread * pow((double)n, -0.2);
-          pass = h > 0.0;
-        }
-      }
-      if (pass) {
-        // ---- pass 3: the KDE on the grid; lanes are grid nodes, samples handed round 32 at a time ----
-        const double invh = 1.0 / h;
-        const double norm = invh * 0.39894228040143267794;   // 1 / (h sqrt(2 pi))
-        const double sinvh = invh * 0.70710678118654752440;  // so that the exponent is -(q')^2
-        double acc[KDE_NPL];
+    // ---- per-pixel statistics, 32 samples at a time whatever the pixel boundaries (lanes = samples): segmented warp
+    // scans of sum v, sum v d, sum v d^2, sum v^2 with d = z - K, K = the pixel's first live redshift (the shifted
+    // one-pass form of the weighted variance: identical samples give exactly 0, and K lies inside the pixel's own
+    // spread, so the subtraction loses a few ulp at most); the run a row leaves open is carried to the next row.
+    // Pixels end at `tail` lanes: those that pass (n >= 2, N_eff, var > 0) go through the KDE one after the other.
+    double cV = 0.0, cVd = 0.0, cVdd = 0.0, cQ = 0.0, cK = 0.0;   // the open run (warp-uniform)
+    int cn = 0, clen = 0;
+    bool cHasK = false;
+    for (int64_t c0 = s0; c0 < s1; c0 += 32) {
+      const int64_t k = c0 + lane;
+      const bool in = k < s1;
+      const int32_t r = in ? p.row[k] : 0;
+      const bool head = in && (k == s0 || p.row[k - 1] != r);
+      const bool tail = in && (k + 1 >= s1 || p.row[k + 1] != r);
+      const double2 zv = in ? scr[k] : make_double2(0.0, -1.0);
+      const bool live = zv.y >= 0.0;
+      const double v = live ? zv.y : 0.0, z = zv.x;
+      const unsigned hall = __ballot_sync(FULL, head), lm = __ballot_sync(FULL, live);
+      const unsigned le = 0xffffffffu >> (31 - lane);
+      const unsigned hm = hall & le;
+      const bool open_left = hm == 0;                       // this lane's run began before the row
+      const int first = open_left ? 0 : 31 - __clz(hm);     // first lane of the run inside the row
+      const unsigned runm = le & (0xffffffffu << first);    // lanes of the run up to this one
+      const unsigned lrun = lm & runm;
+      double K = __shfl_sync(FULL, z, lrun ? __ffs(lrun) - 1 : lane);
+      if (open_left && cHasK) K = cK;
+      const double dz = z - K;
+      double V = v, Vd = v * dz, Vdd = v * dz * dz, Q = v * v;
+      const int reach = lane - first;
+      const int maxd = __reduce_max_sync(FULL, in ? reach : 0);
 #pragma unroll
-        for (int i = 0; i < KDE_NPL; ++i) acc[i] = 0.0;
-        const double beta = dzg * sinvh;   // grid step in units of h sqrt(2)
-        if (beta <= KDE_BETA_MAX) {
-          // Fast path (the grid resolves the kernel: h >= dz / 4.2).  A lane owns KDE_NPL CONSECUTIVE nodes
-          // g = 8 lane + s.  With q_c = (8 lane + 4) beta - z_k / (h sqrt 2) the exponent at node s is
-          //   -(q_c + o beta)^2 = -q_c^2 - 2 o beta q_c - o^2 beta^2,   o = s - 4,
-          // so N(z_g; z_k, h) = E P^o C_o with E = exp(-q_c^2), P = exp(-2 beta q_c) and the per-pixel constants
-          // C_o = exp(-o^2 beta^2), which leave the sum over samples: two exponentials and a reciprocal per
-          // (sample, lane) instead of eight exponentials, the other nodes by multiplication (every intermediate is a
-          // Gaussian value <= 1).  q_c is clamped to +-(12.5 + 4 beta): beyond it every node of the lane is below
-          // e^-156 of the sample's own peak, and inside the clamp all arguments stay within the range of exp_fast.
-          const double qL = (double)(KDE_NPL * lane + 4) * beta;
-          const double Qc = 12.5 + 4.0 * beta;
-          const double g2 = -2.0 * beta;
-          for (int64_t c0 = r0; c0 < r1; c0 += 32) {
-            const int64_t k = c0 + lane;
-            double zs = 0.0, a = 0.0;   // z_k / (h sqrt 2), v_k / (h sqrt(2 pi))
-            if (k < r1) {
-              const double2 zv = scr[k];
-              a = zv.y >= 0.0 ? zv.y * norm : 0.0;
-              zs = zv.x * sinvh;
-            }
-            const int cnt = (int)min((int64_t)32, r1 - c0);
-#pragma unroll 2
-            for (int j = 0; j < cnt; ++j) {
-              const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
-              const double qc = fmin(fmax(qL - zj, -Qc), Qc);
-              const double E = exp_fast<false>(-qc * qc, exptab);
-              const double P = exp_fast<false>(g2 * qc, exptab);
-              const double Pi = rcp_fast(P);
-              const double u1 = E * P, u2 = u1 * P, u3 = u2 * P;
-              const double d1 = E * Pi, d2 = d1 * Pi, d3 = d2 * Pi, d4 = d3 * Pi;
-              acc[0] = fma(aj, d4, acc[0]);
-              acc[1] = fma(aj, d3, acc[1]);
-              acc[2] = fma(aj, d2, acc[2]);
-              acc[3] = fma(aj, d1, acc[3]);
-              acc[4] = fma(aj, E, acc[4]);
-              acc[5] = fma(aj, u1, acc[5]);
-              acc[6] = fma(aj, u2, acc[6]);
-              acc[7] = fma(aj, u3, acc[7]);
-            }
-          }
-          const double c1 = exp_fast<false>(-beta * beta, exptab);   // C_o = c1^(o^2)
-          const double c2 = c1 * c1, c4 = c2 * c2, c8 = c4 * c4, c9 = c8 * c1, c16 = c8 * c8;
-          acc[0] *= c16; acc[1] *= c9; acc[2] *= c4; acc[3] *= c1; acc[5] *= c1; acc[6] *= c4; acc[7] *= c9;
+      for (int o = 1; o < 32; o <<= 1) {
+        if (o > maxd) break;   // warp-uniform
+        const double tV = __shfl_up_sync(FULL, V, o), tVd = __shfl_up_sync(FULL, Vd, o);
+        const double tVdd = __shfl_up_sync(FULL, Vdd, o), tQ = __shfl_up_sync(FULL, Q, o);
+        const bool take = reach >= o;
+        V += take ? tV : 0.0;
+        Vd += take ? tVd : 0.0;
+        Vdd += take ? tVdd : 0.0;
+        Q += take ? tQ : 0.0;
+      }
+      int n = __popc(lrun);
+      int len = reach + 1;
+      if (open_left) { V += cV; Vd += cVd; Vdd += cVdd; Q += cQ; n += cn; len += clen; }
+      // what the next row inherits (lane 31's run when it stays open)
+      {
+        const bool open31 = __shfl_sync(FULL, (int)(in && !tail), 31) != 0;
+        const unsigned lr31 = __shfl_sync(FULL, lrun, 31);
+        const bool left31 = __shfl_sync(FULL, (int)open_left, 31) != 0;
+        const double kk = __shfl_sync(FULL, K, lr31 ? 31 - __clz(lr31) : 31);
+        const double nV = __shfl_sync(FULL, V, 31), nVd = __shfl_sync(FULL, Vd, 31);
+        const double nVdd = __shfl_sync(FULL, Vdd, 31), nQ = __shfl_sync(FULL, Q, 31);
+        const int nn = __shfl_sync(FULL, n, 31), nlen = __shfl_sync(FULL, len, 31);
+        if (open31) {
+          if (lr31 && !(left31 && cHasK)) { cK = kk; cHasK = true; }
+          else if (!left31) cHasK = false;
+          cV = nV; cVd = nVd; cVdd = nVdd; cQ = nQ; cn = nn; clen = nlen;
         } else {
-          // narrow kernels (h < dz / 4.2, a degenerate pixel): every Gaussian by its own exponential
-          for (int64_t c0 = r0; c0 < r1; c0 += 32) {
-            const int64_t k = c0 + lane;
-            double zs = 0.0, a = 0.0;
-            if (k < r1) {
-              const double2 zv = scr[k];
-              a = zv.y >= 0.0 ? zv.y * norm : 0.0;
-              zs = zv.x * sinvh;
-            }
-            const int cnt = (int)min((int64_t)32, r1 - c0);
-            for (int j = 0; j < cnt; ++j) {
-              const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
-#pragma unroll
-              for (int i = 0; i < KDE_NPL; ++i) {
-                const double q = fma((double)(KDE_NPL * lane + i), beta, -zj);
-                acc[i] = fma(aj, exp_fast<true>(-q * q, exptab), acc[i]);
-              }
-            }
-          }
-        }
-        // ---- prior at the lane's nodes: p_los(z_g | row) by the table's linear interpolation, times c_g R(z_g) ----
-        const LosT* lrow = reinterpret_cast<const LosT*>(p.los) + (size_t)prow * (size_t)p.n_z;
-        double part = 0.0;
-#pragma unroll
-        for (int i = 0; i < KDE_NPL; ++i) {
-          const int g = KDE_NPL * lane + i;
-          if (g < G) {
-            const double zg = fmin(g * dzg, p.los_zmax);
-            const double tz = zg / dzl;
-            int b = (int)floor(tz);
-            b = b > p.n_z - 2 ? p.n_z - 2 : b;
-            const double fz = tz - (double)b;
-            const double q0 = (double)lrow[b], q1 = (double)lrow[b + 1];
-            part = fma(acc[i], (q0 + fz * (q1 - q0)) * s_rg[i * 32 + lane], part);
-          }
-        }
-        const double I = wsum(part);
-        if (I > 0.0) {
-          esum += I;
-          ++np;
-          nu += n;
+          cV = 0.0; cVd = 0.0; cVdd = 0.0; cQ = 0.0; cn = 0; clen = 0; cHasK = false;
         }
       }
-      r0 = r1;
+      // the pixels that end in this row
+      bool pass = tail && n >= 2 && V > 0.0 && V * V >= p.neff_min * Q;
+      double sd = 0.0, h = 0.0;
+      if (pass) {
+        const double mo = Vd / V;
+        const double var = fma(-Vd, mo, Vdd) / V;
+        pass = var > 0.0;
+        sd = pass ? sqrt(var) : 0.0;
+        h = 1.06 * sd * pow((double)n, -0.2);   // Eq. D1
+      }
+      unsigned pm = __ballot_sync(FULL, pass);
+      while (pm) {
+        const int tl = __ffs(pm) - 1;
+        pm &= pm - 1;
+        const int n_p = __shfl_sync(FULL, n, tl), len_p = __shfl_sync(FULL, len, tl);
+        const int32_t prow = __shfl_sync(FULL, r, tl);
+        double h_p = __shfl_sync(FULL, h, tl);
+        const int64_t r1 = c0 + tl + 1, r0 = r1 - len_p;
+        if (p.bw_rule == 1) {                            // Eq. D2
+          const double sd_p = __shfl_sync(FULL, sd, tl);
+          const double iqr = live_quantile(scr, r0, r1, n_p, 0.75, lane) - live_quantile(scr, r0, r1, n_p, 0.25, lane);
+          const double spread = iqr / 1.34 < sd_p ? iqr / 1.34 : sd_p;
+          h_p = 0.9 * spread * pow((double)n_p, -0.2);
+          if (!(h_p > 0.0)) continue;
+        }
+        const double part = kde_pixel<LosT>(scr, r0, r1, h_p, prow, p, dzg, s_w, s_b, exptab, lane);
+        if (__any_sync(FULL, part > 0.0)) {
+          esum += part;
+          ++np;
+          nu += n_p;
+        }
+      }
     }
+    esum = wsum(esum);
     if (lane == 0) {
       p.logL[o] = (s1 > s0 && esum > 0.0) ? shift + log(esum) - log((double)(s1 - s0)) : -CUDART_INF;
       if (p.npass) p.npass[o] = np;
@@ -435,7 +496,7 @@ int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst,
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
   p.n_grid = n_grid; p.neff_min = neff_min; p.bw_rule = bw_rule; p.logL = logL; p.npass = npass; p.nused = nused;
   p.scr = (double2*)scratch; p.scr_stride = scr_stride;
-  const size_t smem = sizeof(MathTables) + sizeof(double) * KDE_WARPS * 32 * KDE_NPL;
+  const size_t smem = sizeof(MathTables) + sizeof(NodeW) * KDE_WARPS * 32 * KDE_NPL + (sizeof(int) + sizeof(double)) * 32 * KDE_NPL;
   const int64_t blocks = n_blocks;
 #define GWC_KDE_LAUNCH(NodeT, LosT)                                                                              \
   do {                                                                                                           \
