@@ -29,7 +29,7 @@ namespace {
 constexpr int KDE_THREADS = 256;
 constexpr int KDE_WARPS = KDE_THREADS / 32;
 constexpr int KDE_NPL = 8;            // grid nodes per lane: G <= 256
-constexpr double KDE_BETA_MAX = 3.0;  // fast path of the KDE pass: grid step <= 3 h sqrt(2)
+constexpr double KDE_BETA_MAX = 1.5;  // fast path of the KDE pass: grid step <= 1.5 h sqrt(2)
 constexpr double C_KMS_KDE = 299792.458;
 
 struct KdeParams {
@@ -172,10 +172,14 @@ __device__ double live_quantile(const double2* scr, int64_t r0, int64_t r1, int6
   return x0 + f * (x1 - x0);
 }
 
+// Grid node i (< KDE_NPL) of a lane in the prior stage: half-warp lane l16 = lane & 15 owns the 16 consecutive nodes
+// 16 l16 .. 16 l16 + 15, of which the lower half-warp keeps the first eight and the upper one the last eight.
+__device__ __forceinline__ int kde_node(int lane, int i) { return 16 * (lane & 15) + KDE_NPL * (lane >> 4) + i; }
+
 // The KDE of one pixel on the grid times the prior, Eq. 5-6: returns this lane's share of
-// I_j = sum_g c_g R(z_g) p_los(z_g | row) sum_k v_k N(z_g; z_k, h)  (lanes own KDE_NPL consecutive nodes each;
-// the caller adds the lanes' shares of all pixels and reduces once per event).  s_w: per-node prior weights of this
-// theta, [i][lane] pairs (w0, w1) = c_g R(z_g) (1 - f_g, f_g) for the two LOS nodes around z_g, and the index b_g.
+// I_j = sum_g c_g R(z_g) p_los(z_g | row) sum_k v_k N(z_g; z_k, h)  (the caller adds the lanes' shares of all pixels
+// and reduces once per event).  s_w: per-node prior weights of this theta, [i][lane] pairs (w0, w1) =
+// c_g R(z_g) (1 - f_g, f_g) for the two LOS nodes around z_g, g = kde_node(lane, i); s_b: the LOS bin b_g.
 struct NodeW { double w0, w1; };
 template <typename LosT>
 __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int64_t r0, int64_t r1, double h,
@@ -191,21 +195,24 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
   const double invh = 1.0 / h;
   const double norm = invh * 0.39894228040143267794;   // 1 / (h sqrt(2 pi))
   const double sinvh = invh * 0.70710678118654752440;  // so that the exponent is -(q')^2
-  double acc[KDE_NPL];
-#pragma unroll
-  for (int i = 0; i < KDE_NPL; ++i) acc[i] = 0.0;
   const double beta = dzg * sinvh;   // grid step in units of h sqrt(2)
+  const int l16 = lane & 15, up = lane >> 4;
+  double mine[KDE_NPL];   // f_j at this lane's eight nodes
   if (beta <= KDE_BETA_MAX) {
-    // Fast path (the grid resolves the kernel: h >= dz / 4.2).  A lane owns KDE_NPL CONSECUTIVE nodes
-    // g = 8 lane + s.  With q_c = (8 lane + 4) beta - z_k / (h sqrt 2) the exponent at node s is
-    //   -(q_c + o beta)^2 = -q_c^2 - 2 o beta q_c - o^2 beta^2,   o = s - 4,
+    // Fast path (the grid resolves the kernel: h >= dz / 2.1).  The two half-warps take alternate samples; inside a
+    // half-warp lane l16 covers the 16 CONSECUTIVE nodes g = 16 l16 + s.  With q_c = (16 l16 + 8) beta - z_k / (h sqrt 2)
+    // the exponent at node s is
+    //   -(q_c + o beta)^2 = -q_c^2 - 2 o beta q_c - o^2 beta^2,   o = s - 8,
     // so N(z_g; z_k, h) = E P^o C_o with E = exp(-q_c^2), P = exp(-2 beta q_c) and the per-pixel constants
     // C_o = exp(-o^2 beta^2), which leave the sum over samples: two exponentials and a reciprocal per
-    // (sample, lane) instead of eight exponentials, the other nodes by multiplication (every intermediate is a
-    // Gaussian value <= 1).  q_c is clamped to +-(12.5 + 4 beta): beyond it every node of the lane is below
-    // e^-156 of the sample's own peak, and inside the clamp all arguments stay within the range of exp_fast.
-    const double qL = (double)(KDE_NPL * lane + 4) * beta;
-    const int hiQc = __double2hiint(12.5 + 4.0 * beta);   // the clamp compares high words (2^-20 below the limit)
+    // (sample, lane) for 16 Gaussians, the other nodes by multiplication (every intermediate E P^o is a Gaussian
+    // value <= 1).  q_c is clamped to +-(12.5 + 8 beta): beyond it every node of the lane is below e^-156 of the
+    // sample's own peak, and inside the clamp all arguments stay within the range of exp_fast.
+    double acc[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc[i] = 0.0;
+    const double qL = (double)(16 * l16 + 8) * beta;
+    const int hiQc = __double2hiint(12.5 + 8.0 * beta);   // the clamp compares high words (2^-20 below the limit)
     const double g2 = -2.0 * beta;
     for (int64_t c0 = r0; c0 < r1; c0 += 32) {
       const int64_t k = c0 + lane;
@@ -216,8 +223,7 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
         zs = zv.x * sinvh;
       }
       const int cnt = (int)min((int64_t)32, r1 - c0);
-#pragma unroll 2
-      for (int j = 0; j < cnt; ++j) {
+      for (int j = up; j - up < cnt; j += 2) {   // (a slot past the end holds a = 0)
         const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
         double qc = qL - zj;
         {
@@ -229,23 +235,48 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
         const double P = exp_fast<false>(g2 * qc, exptab);
         const double Pi = rcp_fast(P);
         const double P2 = P * P, Pi2 = Pi * Pi;
-        const double u1 = E * P, u2 = E * P2, u3 = u1 * P2;
-        const double d1 = E * Pi, d2 = E * Pi2, d3 = d1 * Pi2, d4 = d2 * Pi2;
-        acc[0] = fma(aj, d4, acc[0]);
-        acc[1] = fma(aj, d3, acc[1]);
-        acc[2] = fma(aj, d2, acc[2]);
-        acc[3] = fma(aj, d1, acc[3]);
-        acc[4] = fma(aj, E, acc[4]);
-        acc[5] = fma(aj, u1, acc[5]);
-        acc[6] = fma(aj, u2, acc[6]);
-        acc[7] = fma(aj, u3, acc[7]);
+        const double u1 = E * P, u2 = E * P2, u3 = u1 * P2, u4 = u2 * P2, u5 = u3 * P2, u6 = u4 * P2, u7 = u5 * P2;
+        const double d1 = E * Pi, d2 = E * Pi2, d3 = d1 * Pi2, d4 = d2 * Pi2, d5 = d3 * Pi2, d6 = d4 * Pi2,
+                     d7 = d5 * Pi2, d8 = d6 * Pi2;
+        acc[0] = fma(aj, d8, acc[0]);
+        acc[1] = fma(aj, d7, acc[1]);
+        acc[2] = fma(aj, d6, acc[2]);
+        acc[3] = fma(aj, d5, acc[3]);
+        acc[4] = fma(aj, d4, acc[4]);
+        acc[5] = fma(aj, d3, acc[5]);
+        acc[6] = fma(aj, d2, acc[6]);
+        acc[7] = fma(aj, d1, acc[7]);
+        acc[8] = fma(aj, E, acc[8]);
+        acc[9] = fma(aj, u1, acc[9]);
+        acc[10] = fma(aj, u2, acc[10]);
+        acc[11] = fma(aj, u3, acc[11]);
+        acc[12] = fma(aj, u4, acc[12]);
+        acc[13] = fma(aj, u5, acc[13]);
+        acc[14] = fma(aj, u6, acc[14]);
+        acc[15] = fma(aj, u7, acc[15]);
       }
     }
-    const double c1 = exp_fast<false>(-beta * beta, exptab);   // C_o = c1^(o^2)
-    const double c2 = c1 * c1, c4 = c2 * c2, c8 = c4 * c4, c9 = c8 * c1, c16 = c8 * c8;
-    acc[0] *= c16; acc[1] *= c9; acc[2] *= c4; acc[3] *= c1; acc[5] *= c1; acc[6] *= c4; acc[7] *= c9;
+    // the halves exchange what the other one keeps; C_o = c1^(o^2), c1 = exp(-beta^2) to full accuracy (its 64th
+    // power is taken)
+    const double c1 = exp(-beta * beta), cs = c1 * c1;
+    double C[9];
+    C[0] = 1.0;
+    double t = c1;
+#pragma unroll
+    for (int o = 1; o <= 8; ++o) {
+      C[o] = C[o - 1] * t;   // c1^(o^2): ratios c1^(2o-1)
+      t *= cs;
+    }
+#pragma unroll
+    for (int i = 0; i < KDE_NPL; ++i) {
+      const double send = up ? acc[i] : acc[KDE_NPL + i];
+      const double keep = up ? acc[KDE_NPL + i] : acc[i];
+      mine[i] = (keep + __shfl_xor_sync(FULL, send, 16)) * (up ? C[i] : C[KDE_NPL - i]);
+    }
   } else {
-    // narrow kernels (h < dz / 4.2, a degenerate pixel): every Gaussian by its own exponential
+    // narrow kernels (h < dz / 2.1, a degenerate pixel): every Gaussian by its own exponential
+#pragma unroll
+    for (int i = 0; i < KDE_NPL; ++i) mine[i] = 0.0;
     for (int64_t c0 = r0; c0 < r1; c0 += 32) {
       const int64_t k = c0 + lane;
       double zs = 0.0, a = 0.0;
@@ -259,8 +290,8 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
         const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
 #pragma unroll
         for (int i = 0; i < KDE_NPL; ++i) {
-          const double q = fma((double)(KDE_NPL * lane + i), beta, -zj);
-          acc[i] = fma(aj, exp_fast<true>(-q * q, exptab), acc[i]);
+          const double q = fma((double)kde_node(lane, i), beta, -zj);
+          mine[i] = fma(aj, exp_fast<true>(-q * q, exptab), mine[i]);
         }
       }
     }
@@ -271,7 +302,7 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
   for (int i = 0; i < KDE_NPL; ++i) {
     const NodeW w = s_w[i * 32 + lane];
     const int b = s_b[i * 32 + lane];
-    part = fma(acc[i], fma((double)lrow[b + 1], w.w1, (double)lrow[b] * w.w0), part);
+    part = fma(mine[i], fma((double)lrow[b + 1], w.w1, (double)lrow[b] * w.w0), part);
   }
   return part;
 }
@@ -294,8 +325,8 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
   const double dzg = p.los_zmax / (G - 1);
   const double dzl = p.los_zmax / (p.n_z - 1);
   const int64_t n_units = p.n_theta * p.n_events;
-  if (tid < 32 * KDE_NPL) {   // LOS bin and fraction of grid node g = 8 l + i, stored at [i][l]
-    const int g = tid, l = g / KDE_NPL, i = g % KDE_NPL;
+  if (tid < 32 * KDE_NPL) {   // LOS bin and fraction of grid node g = kde_node(l, i), stored at [i][l]
+    const int l = tid & 31, i = tid >> 5, g = kde_node(l, i);
     const double zg = fmin(g * dzg, p.los_zmax);
     const double tz = zg / dzl;
     int b = (int)floor(tz);
@@ -345,7 +376,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
 #pragma unroll
       for (int i = 0; i < KDE_NPL; ++i) {
-        const int g = KDE_NPL * lane + i;   // a lane owns 8 consecutive nodes; stored [i][lane]: conflict-free
+        const int g = kde_node(lane, i);   // stored [i][lane]: conflict-free
         const double x = 1.0 + g * dzg;
         const double psi = psi0 * pow(x, gam) / (1.0 + pow(x / (1.0 + zp), gam + kap));
         const double c = (g == 0 || g == G - 1) ? 0.5 * dzg : dzg;
