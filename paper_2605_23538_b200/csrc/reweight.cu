@@ -216,28 +216,58 @@ __device__ __forceinline__ int pop_lowest(unsigned& mask) {
 }
 
 // ---- per-pixel effective-sample cut (Eq. 8; R25) -------------------------------------
-// A pixel is a maximal run of consecutive samples of the segment with the same sample_row.  The warp's block
-// holds positions pos = k * 32 + lane; PixShape is the run structure of the block (the same for every theta).
+// A pixel is a maximal run of consecutive samples of the segment with the same sample_row.  In pixel-cut mode a lane
+// owns the SPT = 2 CONSECUTIVE positions 2 lane, 2 lane + 1 of the warp's block, so that one segmented scan over the
+// 32 lanes serves the 64 samples.  PixShape is the run structure of the block (the same for every theta).
 struct PixShape {
-  int d[SPT];        // lanes back to the head of this position's run inside row k (>= 64: the run began earlier)
-  bool tail[SPT];    // last sample of its run
-  bool lead[SPT];    // inside the run that was already open where this warp's range begins
-  int maxd[SPT];     // largest reach of the row (d, or the lane index where the run began earlier): scan steps needed
-  bool last_open;    // the block's last position is inside a run that continues in the next block
+  bool h1;              // position 1 starts a run
+  bool cont0;           // position 0 continues the run of the previous lane (or of the previous block)
+  bool t0, t1;          // last sample of its run
+  bool left0, left1;    // the run of position k began before the block
+  bool lead0, lead1;    // ... before this warp's range of the segment
+  int reach;            // lanes back to the nearest lane (this one included) that holds a run start, else to lane 0
+  int nsteps;           // scan steps the block needs (warp-uniform)
+  unsigned m0a, m1a;    // lanes whose position 0 / position 1 lies in the run of position 0, up to it (live counts)
+  unsigned m0b, m1b;    // ... in the run of position 1
+  bool last_open;       // the block's last position is inside a run that continues in the next block
 };
 
-// Segmented inclusive scan of (W, Q, n) over the 32 lanes of one row; lanes add from `o` lanes back while that
-// lane is still inside their run.
-__device__ __forceinline__ void seg_scan(double& W, double& Q, int d, int maxd) {
+__device__ __forceinline__ void pix_shape(PixShape& ps, bool in0, bool in1, bool head0, bool head1, bool tail0,
+                                          bool tail1, bool lead_open, int lane) {
   const unsigned FULL = 0xffffffffu;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    if (o > maxd) break;  // warp-uniform
-    const double tW = __shfl_up_sync(FULL, W, o), tQ = __shfl_up_sync(FULL, Q, o);
-    const bool take = d >= 64 ? (int)(threadIdx.x & 31) >= o : d >= o;
-    W += take ? tW : 0.0;
-    Q += take ? tQ : 0.0;
+  const unsigned hall = __ballot_sync(FULL, head0 | head1), h1all = __ballot_sync(FULL, head1);
+  const unsigned lt = (1u << lane) - 1u;
+  const unsigned hprev = hall & lt;           // lanes before this one that hold a run start
+  ps.h1 = head1;
+  ps.cont0 = in0 && !head0;
+  ps.t0 = tail0;
+  ps.t1 = tail1;
+  ps.left0 = !head0 && hprev == 0;
+  ps.left1 = ps.left0 && !head1;
+  ps.lead0 = lead_open && ps.left0;
+  ps.lead1 = lead_open && ps.left1;
+  const unsigned hm = hall & (lt | (1u << lane));
+  ps.reach = hm ? lane - (31 - __clz(hm)) : lane;   // (no start so far: the run reaches back to lane 0)
+  const int maxd = __reduce_max_sync(FULL, in0 ? ps.reach : 0);
+  ps.nsteps = maxd == 0 ? 0 : 32 - __clz(maxd);
+  // lanes of the run of position 0 (up to it): from the run's first position f
+  const unsigned upto = lt | (1u << lane);    // lanes <= this one
+  if (head0) {
+    ps.m0a = 1u << lane;
+    ps.m1a = 0u;
+  } else if (hprev == 0) {
+    ps.m0a = upto;
+    ps.m1a = lt;
+  } else {
+    const int lp = 31 - __clz(hprev);                       // nearest earlier lane with a run start
+    const bool odd = (h1all >> lp) & 1u;                    // its last start is its position 1
+    const unsigned from = ~((1u << lp) - 1u);               // lanes >= lp
+    ps.m0a = upto & (odd ? from & ~(1u << lp) : from);
+    ps.m1a = lt & from;
   }
+  ps.m0b = head1 ? 0u : ps.m0a;
+  ps.m1b = head1 ? (1u << lane) : (ps.m1a | (1u << lane));
+  ps.last_open = __shfl_sync(FULL, (int)(in1 && !tail1), 31) != 0;
 }
 
 // From the per-sample weights of one theta to what the passing pixels add to this lane's sums.
@@ -248,55 +278,52 @@ __device__ __forceinline__ void pix_reduce(const PixShape& ps, const double* w, 
                                            double* carryWQ, int* carryN, double* leadWQ, int* leadN, int lane,
                                            double& cW, double& cQ, int& cn, int& cp) {
   const unsigned FULL = 0xffffffffu;
-  double W[SPT], Q[SPT];
-  int n[SPT];
+  const double q0 = w[0] * w[0];
+  // the lane's part of the run that is open at its end, then the inclusive segmented scan of it over the lanes
+  double XW = ps.h1 ? w[1] : w[0] + w[1];
+  double XQ = ps.h1 ? w[1] * w[1] : fma(w[1], w[1], q0);
 #pragma unroll
-  for (int k = 0; k < SPT; ++k) {
-    W[k] = w[k];
-    Q[k] = w[k] * w[k];
-    seg_scan(W[k], Q[k], ps.d[k], ps.maxd[k]);
-    // live samples of the run inside this row: no scan needed, a ballot and a population count over the run's lanes
-    const unsigned lm = __ballot_sync(FULL, live[k]);
-    const int first = ps.d[k] >= 64 ? 0 : lane - ps.d[k];
-    n[k] = __popc(lm & (0xffffffffu >> (31 - lane)) & (0xffffffffu << first));
-  }
-  // runs that began before the row: add what the previous row (or the previous block) accumulated for them
-  double inW = carryWQ[0], inQ = carryWQ[1];
-  int inN = *carryN;
-#pragma unroll
-  for (int k = 0; k < SPT; ++k) {
-    const bool open_left = ps.d[k] >= 64;
-    W[k] += open_left ? inW : 0.0;
-    Q[k] += open_left ? inQ : 0.0;
-    n[k] += open_left ? inN : 0;
-    inW = __shfl_sync(FULL, W[k], 31);
-    inQ = __shfl_sync(FULL, Q[k], 31);
-    inN = __shfl_sync(FULL, n[k], 31);
-  }
-  __syncwarp();
-  if (lane == 0) {  // what the next block inherits
-    carryWQ[0] = ps.last_open ? inW : 0.0;
-    carryWQ[1] = ps.last_open ? inQ : 0.0;
-    *carryN = ps.last_open ? inN : 0;
-  }
-  __syncwarp();
-  cW = 0.0;
-  cQ = 0.0;
-  cn = 0;
-  cp = 0;
-#pragma unroll
-  for (int k = 0; k < SPT; ++k) {
-    if (ps.tail[k] && ps.lead[k]) {  // began in an earlier warp's range: the segment-end stitch decides (one lane at most)
-      leadWQ[0] = W[k];
-      leadWQ[1] = Q[k];
-      *leadN = n[k];
+  for (int st = 0; st < 5; ++st) {
+    if (st >= ps.nsteps) break;  // warp-uniform
+    const int o = 1 << st;
+    const double tW = __shfl_up_sync(FULL, XW, o), tQ = __shfl_up_sync(FULL, XQ, o);
+    if (ps.reach >= o) {
+      XW += tW;
+      XQ += tQ;
     }
-    const bool pass = ps.tail[k] && !ps.lead[k] && W[k] > 0.0 && W[k] * W[k] >= neff_min * Q[k];
-    cW += pass ? W[k] : 0.0;
-    cQ += pass ? Q[k] : 0.0;
-    cn += pass ? n[k] : 0;
-    cp += pass ? 1 : 0;
   }
+  // what the run of position 0 collected before this lane: the previous lane's scan value, plus the open run of
+  // the previous block when it reaches this far
+  double CW = __shfl_up_sync(FULL, XW, 1), CQ = __shfl_up_sync(FULL, XQ, 1);
+  if (lane == 0) { CW = 0.0; CQ = 0.0; }
+  const double inW = carryWQ[0], inQ = carryWQ[1];
+  const int inN = *carryN;
+  CW += ps.left0 ? inW : 0.0;
+  CQ += ps.left0 ? inQ : 0.0;
+  const double W0 = ps.cont0 ? CW + w[0] : w[0], Q0 = ps.cont0 ? CQ + q0 : q0;
+  const double W1 = ps.h1 ? w[1] : W0 + w[1], Q1 = ps.h1 ? w[1] * w[1] : fma(w[1], w[1], Q0);
+  const unsigned b0 = __ballot_sync(FULL, live[0]), b1 = __ballot_sync(FULL, live[1]);
+  const int n0 = __popc(b0 & ps.m0a) + __popc(b1 & ps.m1a) + (ps.left0 ? inN : 0);
+  const int n1 = __popc(b0 & ps.m0b) + __popc(b1 & ps.m1b) + (ps.left1 ? inN : 0);
+  // what the next block inherits
+  const double oW = __shfl_sync(FULL, W1, 31), oQ = __shfl_sync(FULL, Q1, 31);
+  const int oN = __shfl_sync(FULL, n1, 31);
+  __syncwarp();
+  if (lane == 0) {
+    carryWQ[0] = ps.last_open ? oW : 0.0;
+    carryWQ[1] = ps.last_open ? oQ : 0.0;
+    *carryN = ps.last_open ? oN : 0;
+  }
+  __syncwarp();
+  // began in an earlier warp's range: the segment-end stitch decides (one position of the block at most)
+  if (ps.t0 && ps.lead0) { leadWQ[0] = W0; leadWQ[1] = Q0; *leadN = n0; }
+  if (ps.t1 && ps.lead1) { leadWQ[0] = W1; leadWQ[1] = Q1; *leadN = n1; }
+  const bool p0 = ps.t0 && !ps.lead0 && W0 > 0.0 && W0 * W0 >= neff_min * Q0;
+  const bool p1 = ps.t1 && !ps.lead1 && W1 > 0.0 && W1 * W1 >= neff_min * Q1;
+  cW = (p0 ? W0 : 0.0) + (p1 ? W1 : 0.0);
+  cQ = (p0 ? Q0 : 0.0) + (p1 ? Q1 : 0.0);
+  cn = (p0 ? n0 : 0) + (p1 ? n1 : 0);
+  cp = (p0 ? 1 : 0) + (p1 ? 1 : 0);
 }
 
 // One sample's theta-independent values, held in registers while the warp loops over the tile's theta points.
@@ -442,25 +469,24 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         Sample<RowT> sm[SPT];
         PixShape ps;
         double dmin = CUDART_INF;  // smallest d_L of the warp's samples: a whole-warp range test per theta
+        if (PIX) {
+          // run structure of the block: run starts and ends at this lane's two consecutive positions
+          static_assert(!PIX || SPT == 2, "pixel-cut mode: two consecutive samples per lane");
+          const int64_t g0 = c0 + 2 * lane;
+          const bool in0 = g0 < w_hi, in1 = g0 + 1 < w_hi;
+          const int32_t r0 = in0 ? p.row[g0] : 0, r1 = in1 ? p.row[g0 + 1] : 0;
+          const bool head0 = in0 && (g0 == s0 || p.row[g0 - 1] != r0);
+          const bool head1 = in1 && r1 != r0;
+          // (ranges end on block boundaries or on the segment's last sample, which is a tail)
+          const bool tail0 = in0 && (g0 + 1 >= s1 || p.row[g0 + 1] != r0);
+          const bool tail1 = in1 && (g0 + 2 >= s1 || p.row[g0 + 2] != r1);
+          pix_shape(ps, in0, in1, head0, head1, tail0, tail1, lead_open, lane);
+          lead_open = lead_open && __ballot_sync(FULL, head0 | head1) == 0;
+        }
 #pragma unroll
         for (int k = 0; k < SPT; ++k) {
-          const int64_t g = c0 + k * 32 + lane;
+          const int64_t g = PIX ? c0 + SPT * lane + k : c0 + k * 32 + lane;
           const bool in = g < w_hi;  // slots past the end are dead
-          if (PIX) {
-            // run structure of the row: heads, distance to the head, tails
-            const int32_t r = in ? p.row[g] : 0;
-            const bool head = in && (g == s0 || p.row[g - 1] != r);
-            const bool tail = in && (g + 1 >= s1 || p.row[g + 1] != r);
-            const unsigned hall = __ballot_sync(FULL, head);
-            const unsigned hm = hall & (0xffffffffu >> (31 - lane));
-            ps.d[k] = hm ? lane - (31 - __clz(hm)) : 64;
-            ps.tail[k] = tail;
-            ps.lead[k] = lead_open && hm == 0;
-            ps.maxd[k] = __reduce_max_sync(FULL, in ? (hm ? ps.d[k] : lane) : 0);
-            // (ranges end on block boundaries or on the segment's last sample, which is a tail)
-            if (k == SPT - 1) ps.last_open = __shfl_sync(FULL, (int)(in && !tail), 31) != 0;
-            lead_open = lead_open && hall == 0;
-          }
           sm[k].A = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
           sm[k].m2z = in ? p.m2z[g] : 1.0;
           sm[k].C = make_double2(in ? p.L1[g] : 0.0, in ? p.Q[g] : 0.0);
