@@ -18,7 +18,9 @@ _SRC = os.path.join(_HERE, "gwc_oracle.c")
 _LIB = os.path.join(_HERE, "libgwc_oracle.so")
 
 NPAR = 12
+NPAR_MULTIPEAK = 16
 TABLE, EXACT = 0, 1
+MASS_MODELS = {"plpeak": 0, "multipeak": 1}
 
 
 def build(force: bool = False) -> str:
@@ -73,6 +75,8 @@ def lib():
             "orc_pack_events": (i64, [i64, i64, vp, vp, vp, vp, vp, vp, vp]),
             "orc_cap_pixels": (i64, [i64, i64, i64, vp, vp, vp, i64, C.c_uint64, vp]),
             "orc_num_threads": (C.c_int, []), "orc_set_num_threads": (None, [C.c_int]),
+            "orc_set_mass_model": (None, [C.c_int]), "orc_npar": (C.c_int, []),
+            "orc_mp_smooth": (d, [d, d, d]), "orc_mp_C": (d, [d, vp]), "orc_mp_N1": (d, [vp]),
         }
         for name, (res, args) in sig.items():
             f = getattr(L, name)
@@ -93,8 +97,29 @@ def _theta(theta):
     th = _f64(theta)
     if th.ndim == 1:
         th = th[None, :]
-    assert th.shape[1] == NPAR
+    assert th.shape[1] == lib().orc_npar()
     return th
+
+
+class mass_model:
+    """``with oracle.mass_model("multipeak"): ...`` -- theta rows have 16 columns inside the block (the 12 of the
+    power-law+peak row, then delta_m, mu_g,low, sigma_g,low, lambda_g,low; R33-R36)."""
+
+    def __init__(self, name):
+        self.model = MASS_MODELS[name]
+
+    def __enter__(self):
+        lib().orc_set_mass_model(self.model)
+        return self
+
+    def __exit__(self, *exc):
+        lib().orc_set_mass_model(0)
+        return False
+
+
+def mp_smooth(m, mmin, dm): return lib().orc_mp_smooth(m, mmin, dm)
+def mp_C(m1, th): th = _f64(th); return lib().orc_mp_C(m1, _p(th))
+def mp_N1(th): th = _f64(th); return lib().orc_mp_N1(_p(th))
 
 
 # ---- scalar pieces (used by the pins) -------------------------------------------------------

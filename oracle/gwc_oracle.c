@@ -37,9 +37,15 @@
 #include <omp.h>
 #endif
 
-#define ORC_NPAR 12
-/* theta row: H0, Om, alpha, beta, mmin, mmax, mu, sigma, lambda, gamma, kappa, zp */
-enum { P_H0 = 0, P_OM, P_ALPHA, P_BETA, P_MMIN, P_MMAX, P_MU, P_SIGMA, P_LAMBDA, P_GAMMA, P_KAPPA, P_ZP };
+/* theta row, power law + peak (model 0): H0, Om, alpha, beta, mmin, mmax, mu, sigma, lambda, gamma, kappa, zp.
+ * MULTIPEAK (model 1; App. A, Table III :263-274; R33-R36) appends delta_m, mu_g,low,
+ * sigma_g,low, lambda_g,low; there mu, sigma are the HIGH peak and lambda is lambda_g, the Gaussian fraction. */
+enum { P_H0 = 0, P_OM, P_ALPHA, P_BETA, P_MMIN, P_MMAX, P_MU, P_SIGMA, P_LAMBDA, P_GAMMA, P_KAPPA, P_ZP,
+       P_DM, P_MULOW, P_SIGLOW, P_LAMLOW };
+static int g_model = 0;   /* set once before a run by the test that wants MULTIPEAK; never changed during one */
+void orc_set_mass_model(int model) { g_model = model == 1 ? 1 : 0; }
+int orc_npar(void) { return g_model == 1 ? 16 : 12; }
+#define ORC_NPAR (orc_npar())
 
 static const double C_KMS = 299792.458; /* km/s, exact */
 
@@ -191,6 +197,11 @@ int orc_theta_valid(const double* th) {
   if (!(th[P_MMIN] > 0.0 && th[P_MMIN] < th[P_MMAX])) return 0;
   if (!(th[P_LAMBDA] >= 0.0 && th[P_LAMBDA] <= 1.0)) return 0;
   if (!(th[P_ZP] > -1.0)) return 0;
+  if (g_model == 1) {
+    if (!(th[P_DM] >= 0.0 && th[P_MMIN] + th[P_DM] < th[P_MMAX])) return 0;
+    if (!(th[P_SIGLOW] > 0.0)) return 0;
+    if (!(th[P_LAMLOW] >= 0.0 && th[P_LAMLOW] <= 1.0)) return 0;
+  }
   return 1;
 }
 
@@ -207,17 +218,106 @@ double orc_norm_g(const double* th) {
 }
 
 /* per-theta constants of the population laws, computed once per theta */
-typedef struct { double n_pl, n_g, psi0; } orc_pop;
+typedef struct {
+  double n_pl, n_g, psi0;
+  double n_gl;   /* MULTIPEAK: normalisation of the low Gaussian on [mmin, mmax] */
+  double N1;     /* MULTIPEAK: int_mmin^mmax mix(m) S(m) dm */
+  double Cwin;   /* MULTIPEAK: int over the smoothing window [mmin, mmin + delta_m] of m^beta S(m) dm */
+} orc_pop;
+
+/* ---- MULTIPEAK with low-mass smoothing (readings R33-R36; the formula is not in the paper) ----------------
+ *   S(m) = 0 (m <= mmin), 1 (m >= mmin + dm), else 1 / (1 + exp(dm/m' + dm/(m' - dm))), m' = m - mmin;
+ *          a smoothing factor below e^-600 counts as 0 (R35)
+ *   mix(m) = (1-lam) P(m) + lam lam_low G(m; mu_low, s_low) + lam (1-lam_low) G(m; mu_high, s_high),
+ *            P = power law m^-alpha, G = Gaussian, each truncated to and normalised on [mmin, mmax]
+ *   p(m1) = mix(m1) S(m1) / N1,   N1 = int mix S
+ *   p(m2 | m1) = m2^beta S(m2) / C(m1),   C(m1) = int_mmin^m1 m^beta S(m) dm                                */
+double orc_mp_smooth(double m, double mmin, double dm) {
+  double mp = m - mmin;
+  if (!(mp >= 0.0)) return 0.0;
+  if (mp >= dm) return 1.0;
+  if (mp == 0.0) return 0.0;
+  double e = dm / mp + dm / (mp - dm);
+  if (e > 600.0) return 0.0;
+  return 1.0 / (1.0 + exp(e));
+}
+
+static double gl_panels(double (*f)(double, const void*), const void* ctx, double a, double b, int np) {
+  gl_init();
+  double h = (b - a) / np, total = 0.0;
+  for (int p = 0; p < np; ++p) {
+    double lo = a + p * h, s = 0.0;
+    for (int i = 0; i < GL_N; ++i) s += gl_w[i] * f(lo + 0.5 * h * (gl_x[i] + 1.0), ctx);
+    total += 0.5 * h * s;
+  }
+  return total;
+}
+
+typedef struct { const double* th; double n_pl, n_gl, n_gh; } mp_ctx;
+
+static double gauss_norm(double mu, double s, double lo, double hi) {
+  return 1.0 / (0.5 * (erf((hi - mu) / (s * M_SQRT2)) - erf((lo - mu) / (s * M_SQRT2))));
+}
+
+/* the mixture before smoothing */
+static double mp_mix(double m, const void* vc) {
+  const mp_ctx* c = (const mp_ctx*)vc;
+  const double* th = c->th;
+  double lam = th[P_LAMBDA], ll = th[P_LAMLOW];
+  double v = (1.0 - lam) * c->n_pl * pow(m, -th[P_ALPHA]);
+  if (lam > 0.0) {
+    double xl = (m - th[P_MULOW]) / th[P_SIGLOW], xh = (m - th[P_MU]) / th[P_SIGMA];
+    if (ll > 0.0) v += lam * ll * c->n_gl * exp(-0.5 * xl * xl) / (th[P_SIGLOW] * sqrt(2.0 * M_PI));
+    if (ll < 1.0) v += lam * (1.0 - ll) * c->n_gh * exp(-0.5 * xh * xh) / (th[P_SIGMA] * sqrt(2.0 * M_PI));
+  }
+  return v;
+}
+static double mp_mix_s(double m, const void* vc) {
+  const mp_ctx* c = (const mp_ctx*)vc;
+  return mp_mix(m, vc) * orc_mp_smooth(m, c->th[P_MMIN], c->th[P_DM]);
+}
+static double mp_pow_s(double m, const void* vc) {
+  const double* th = (const double*)vc;
+  return pow(m, th[P_BETA]) * orc_mp_smooth(m, th[P_MMIN], th[P_DM]);
+}
+#define MP_WIN_PANELS 16
+
+/* C(m1) = int_mmin^m1 m^beta S(m) dm: quadrature inside the smoothing window, elementary above it */
+static double mp_C(double m1, const double* th, const orc_pop* P) {
+  double lo = th[P_MMIN], top = th[P_MMIN] + th[P_DM], b = th[P_BETA];
+  if (!(m1 > lo)) return 0.0;
+  if (m1 < top) return gl_panels(mp_pow_s, th, lo, m1, MP_WIN_PANELS);
+  double above = (b == -1.0) ? log(m1 / top) : (pow(m1, b + 1.0) - pow(top, b + 1.0)) / (b + 1.0);
+  return P->Cwin + above;
+}
 
 static void pop_init(const double* th, orc_pop* P) {
   P->n_pl = orc_norm_pl(th);
   P->n_g = orc_norm_g(th);
   P->psi0 = 1.0 + pow(1.0 + th[P_ZP], -(th[P_GAMMA] + th[P_KAPPA]));
+  P->n_gl = P->N1 = P->Cwin = 0.0;
+  if (g_model == 1) {
+    double lo = th[P_MMIN], hi = th[P_MMAX], top = lo + th[P_DM];
+    P->n_gl = gauss_norm(th[P_MULOW], th[P_SIGLOW], lo, hi);
+    mp_ctx c = {th, P->n_pl, P->n_gl, P->n_g};
+    /* N1: the window in MP_WIN_PANELS panels, the rest in panels no wider than the narrower peak */
+    double w = th[P_SIGLOW] < th[P_SIGMA] ? th[P_SIGLOW] : th[P_SIGMA];
+    double np = ceil((hi - top) / w);
+    if (np > 20000.0) np = 20000.0;
+    if (np < 1.0) np = 1.0;
+    P->N1 = (th[P_DM] > 0.0 ? gl_panels(mp_mix_s, &c, lo, top, MP_WIN_PANELS) : 0.0) +
+            gl_panels(mp_mix_s, &c, top, hi, (int)np);
+    P->Cwin = th[P_DM] > 0.0 ? gl_panels(mp_pow_s, th, lo, top, MP_WIN_PANELS) : 0.0;
+  }
 }
 
 /* p(m1|theta): truncated power law + truncated Gaussian peak on (mmin, mmax] */
 static double p1_c(double m1, const double* th, const orc_pop* P) {
   if (!(m1 > th[P_MMIN] && m1 <= th[P_MMAX])) return 0.0;
+  if (g_model == 1) {
+    mp_ctx c = {th, P->n_pl, P->n_gl, P->n_g};
+    return mp_mix(m1, &c) * orc_mp_smooth(m1, th[P_MMIN], th[P_DM]) / P->N1;
+  }
   double lam = th[P_LAMBDA], mu = th[P_MU], s = th[P_SIGMA];
   double pl = (1.0 - lam) * P->n_pl * pow(m1, -th[P_ALPHA]);
   double g = 0.0;
@@ -235,11 +335,34 @@ double orc_p1(double m1, const double* th) {
 }
 
 /* p(m2|m1,theta) = (beta+1) m2^beta / (m1^(beta+1) - mmin^(beta+1)) on [mmin, m1] */
-double orc_p2(double m2, double m1, const double* th) {
+static double p2_c(double m2, double m1, const double* th, const orc_pop* P) {
   double b = th[P_BETA], lo = th[P_MMIN];
   if (!(m2 >= lo && m2 <= m1 && m1 > lo)) return 0.0;
+  if (g_model == 1) {
+    double s = orc_mp_smooth(m2, lo, th[P_DM]);
+    if (!(s > 0.0)) return 0.0;
+    return pow(m2, b) * s / mp_C(m1, th, P);
+  }
   if (b == -1.0) return 1.0 / (m2 * log(m1 / lo));
   return (b + 1.0) * pow(m2, b) / (pow(m1, b + 1.0) - pow(lo, b + 1.0));
+}
+
+double orc_p2(double m2, double m1, const double* th) {
+  orc_pop P;
+  pop_init(th, &P);
+  return p2_c(m2, m1, th, &P);
+}
+
+/* exposed for the pins: C(m1) and N1 of the MULTIPEAK model */
+double orc_mp_C(double m1, const double* th) {
+  orc_pop P;
+  pop_init(th, &P);
+  return mp_C(m1, th, &P);
+}
+double orc_mp_N1(const double* th) {
+  orc_pop P;
+  pop_init(th, &P);
+  return P.N1;
 }
 
 /* Madau-Dickinson psi(z), psi(0) = 1 (App. A; Table III :271-273) */
@@ -325,7 +448,7 @@ double orc_log_weight(const double* th, int mode, const orc_cosmo_tab* ct, doubl
   /* support: mmin < m1 <= mmax, mmin <= m2 <= m1 (m2 <= m1 <=> m2z <= m1z; reading R15) */
   if (!(m1 > th[P_MMIN] && m1 <= th[P_MMAX] && m2 >= th[P_MMIN] && m2z <= m1z)) return -INFINITY;
   double p1 = p1_c(m1, th, &ct->pop);
-  double p2 = orc_p2(m2 <= m1 ? m2 : m1, m1, th);
+  double p2 = p2_c(m2 <= m1 ? m2 : m1, m1, th, &ct->pop);
   double R = psi_c(z, th, &ct->pop) / x;
   double plos = orc_los_lerp(L, row, z);
   if (!(plos > 0.0) || !(p1 > 0.0) || !(p2 > 0.0)) return -INFINITY;
@@ -586,7 +709,7 @@ static double kde_sample(const double* th, int mode, const orc_cosmo_tab* ct, do
   double m1 = m1z / x, m2 = m2z / x;
   if (!(m1 > th[P_MMIN] && m1 <= th[P_MMAX] && m2 >= th[P_MMIN] && m2z <= m1z)) return -INFINITY;
   double p1 = p1_c(m1, th, &ct->pop);
-  double p2 = orc_p2(m2 <= m1 ? m2 : m1, m1, th);
+  double p2 = p2_c(m2 <= m1 ? m2 : m1, m1, th, &ct->pop);
   if (!(p1 > 0.0) || !(p2 > 0.0)) return -INFINITY;
   double J = x * x * (C_KMS / H0) * (u / x + x / orc_E(z, Om));
   *z_out = z;

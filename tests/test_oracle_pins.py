@@ -823,3 +823,163 @@ def test_norm_pl_alpha_one_branch(theta0):
         th2 = th.copy(); th2[2] = 1.0 + eps
         assert O.norm_pl(th2) == pytest.approx(O.norm_pl(th), rel=1e-5)
         assert O.p1(20.0, th2) == pytest.approx(O.p1(20.0, th), rel=1e-5)
+
+
+# ---------------------------------------------------------------- MULTIPEAK with low-mass smoothing (NEXT row 3a)
+# App. A, Table III :263-274; the formula is not in the paper: readings R33-R36 of DESIGN.md.
+def _th_mp(**mod):
+    for line in open(os.path.join(GOLD, "table3_multipeak.txt")):
+        if line.strip() and not line.startswith("#"):
+            th = np.array([float(x) for x in line.split()])
+    names = dict(H0=0, Om=1, alpha=2, beta=3, mmin=4, mmax=5, mu=6, sigma=7, lam=8, dm=12, mul=13, sigl=14, laml=15)
+    for k, v in mod.items():
+        th[names[k]] = v
+    return th
+
+
+def test_mp_smoothing_closed_forms():
+    """S(m) = 1/(1 + exp(dm/m' + dm/(m' - dm))): 0 at mmin, 1 from mmin + dm on, 1/2 at the middle of the window,
+    S(mmin + x) + S(mmin + dm - x) = 1 (the exponent is odd about the middle), increasing; below e^-600 it is 0 (R35)."""
+    lo, dm = 4.6, 4.8
+    assert O.mp_smooth(lo, lo, dm) == 0.0 and O.mp_smooth(lo - 1.0, lo, dm) == 0.0
+    assert O.mp_smooth(lo + dm, lo, dm) == 1.0 and O.mp_smooth(50.0, lo, dm) == 1.0
+    assert O.mp_smooth(lo + 0.5 * dm, lo, dm) == pytest.approx(0.5, abs=1e-15)
+    xs = np.linspace(0.02, 0.98, 49) * dm
+    s = np.array([O.mp_smooth(lo + x, lo, dm) for x in xs])
+    assert np.all(np.diff(s) > 0)
+    np.testing.assert_allclose(s + s[::-1], 1.0, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(s, special.expit(-(dm / xs + dm / (xs - dm))), rtol=1e-13)
+    # the e^-600 rule: the exponent at m' = dm/601 is 601 - 1/(1 - 1/601) = 599.998.., at dm/603 it is 601.998..
+    assert O.mp_smooth(lo + dm / 603.0, lo, dm) == 0.0
+    assert 0.0 < O.mp_smooth(lo + dm / 601.0, lo, dm) < 1e-259
+    # dm = 0: a step at mmin, the lower edge included (R15)
+    assert O.mp_smooth(lo, lo, 0.0) == 1.0 and O.mp_smooth(lo - 1e-9, lo, 0.0) == 0.0
+
+
+@pytest.mark.parametrize("mod", [{}, dict(dm=0.0), dict(laml=0.0), dict(laml=1.0), dict(lam=0.0), dict(lam=1.0, dm=9.0),
+                                 dict(alpha=1.5, mul=7.0, sigl=2.0, dm=2.0, beta=-0.5)])
+def test_mp_p1_normalised(mod):
+    th = _th_mp(**mod)
+    lo, hi, top = th[4], th[5], th[4] + th[12]
+    with O.mass_model("multipeak"):
+        val, _ = integrate.quad(lambda m: O.p1(m, th), lo, hi, points=sorted({lo + 0.5 * th[12], top, th[13], th[6]}),
+                                epsabs=0, epsrel=1e-12, limit=800)
+        assert O.p1(lo, th) == 0.0 and O.p1(hi, th) > 0.0 and O.p1(hi + 1e-9, th) == 0.0
+    assert val == pytest.approx(1.0, abs=1e-10)
+
+
+@pytest.mark.parametrize("beta", [1.0, 0.0, -0.5, 4.0, -1.0, -2.5])
+def test_mp_p2_normalised(beta):
+    th = _th_mp(beta=beta)
+    lo, top = th[4], th[4] + th[12]
+    with O.mass_model("multipeak"):
+        for m1 in (5.3, 6.5, 7.0, 9.0, top, 12.0, 80.0):
+            val, _ = integrate.quad(lambda m: O.p2(m, m1, th), lo, m1, points=sorted({min(m1, lo + 0.5 * th[12]), min(m1, top)}),
+                                    epsabs=0, epsrel=1e-12, limit=400)
+            assert val == pytest.approx(1.0, abs=2e-10), (beta, m1)
+        assert O.p2(lo, 30.0, th) == 0.0 and O.p2(30.0, 30.0, th) > 0 and O.p2(30.0001, 30.0, th) == 0.0
+
+
+def test_mp_C_against_scipy_quad():
+    th = _th_mp()
+    lo, dm, b = th[4], th[12], th[3]
+    f = lambda m: m ** b * special.expit(-(dm / (m - lo) + dm / (m - lo - dm))) if m < lo + dm else m ** b
+    with O.mass_model("multipeak"):
+        for m1 in (5.2, 6.0, 7.0, 8.5, 9.4, 9.5, 20.0, 86.3):
+            ref, _ = integrate.quad(f, lo, m1, points=sorted({min(m1, 7.0), min(m1, lo + dm)}), epsabs=0, epsrel=1e-13,
+                                    limit=400)
+            assert O.mp_C(m1, th) == pytest.approx(ref, rel=2e-11), m1
+
+
+def test_mp_reduces_to_power_law_plus_peak(theta0):
+    """delta_m = 0 with one peak switched off is the (pinned) power-law+peak model: lambda_low = 1 keeps the LOW peak,
+    lambda_low = 0 the HIGH one; in between p(m1) is linear in lambda_low; p(m2|m1) is the plain conditional power law."""
+    th = _th_mp(dm=0.0)
+    ms = (4.6000001, 5.0, 9.7, 12.0, 30.7, 60.0, 86.3)
+
+    def plpeak(mu, sig):
+        t = theta0.copy()
+        t[:12] = th[:12]
+        t[6], t[7] = mu, sig
+        return np.array([O.p1(m, t) for m in ms]), np.array([O.p2(0.7 * m + 0.3 * 4.6, m, t) for m in ms])
+
+    def multipeak(laml):
+        t = th.copy()
+        t[15] = laml
+        with O.mass_model("multipeak"):
+            return np.array([O.p1(m, t) for m in ms]), np.array([O.p2(0.7 * m + 0.3 * 4.6, m, t) for m in ms])
+
+    lo1, lo2 = plpeak(th[13], th[14])
+    hi1, hi2 = plpeak(th[6], th[7])
+    a1, a2 = multipeak(1.0)
+    b1, b2 = multipeak(0.0)
+    np.testing.assert_allclose(a1, lo1, rtol=1e-12)
+    np.testing.assert_allclose(b1, hi1, rtol=1e-12)
+    np.testing.assert_allclose(a2, lo2, rtol=1e-13)
+    np.testing.assert_allclose(b2, hi2, rtol=1e-13)
+    c1, _ = multipeak(0.8)
+    np.testing.assert_allclose(c1, 0.8 * lo1 + 0.2 * hi1, rtol=1e-12)
+    assert abs(lo1[2] / hi1[2] - 1) > 0.5      # the two peaks really differ at 9.7 Msun
+    # the whole event term agrees too (same support rules at delta_m = 0)
+    ev, tab, zmax = _toy_event()
+    ev = dict(ev, m1z=ev["m1z"] * 0.45, m2z=ev["m2z"] * 0.35)
+    t12 = theta0.copy()
+    t12[:12] = th[:12]
+    t12[6], t12[7] = th[13], th[14]
+    L0, n0, k0 = O.event_loglik(t12, ev, tab, zmax)
+    t16 = th.copy()
+    t16[15] = 1.0
+    with O.mass_model("multipeak"):
+        L1, n1, k1 = O.event_loglik(t16, ev, tab, zmax)
+    assert np.array_equal(k0, k1) and k0.min() > 0
+    np.testing.assert_allclose(L1, L0, rtol=0, atol=1e-11)
+
+
+def test_mp_smoothing_shapes_p1_and_p2():
+    """With everything else equal, switching delta_m on multiplies p(m1) by S(m1) N1(0)/N1(dm) and p(m2|m1) by
+    S(m2) C0(m1)/C(m1): ratios at two masses isolate S, which the closed forms above pin."""
+    th, th0 = _th_mp(), _th_mp(dm=0.0)
+    lo, dm = th[4], th[12]
+    with O.mass_model("multipeak"):
+        ma, mb = 6.2, 8.1
+        r = (O.p1(ma, th) / O.p1(ma, th0)) / (O.p1(mb, th) / O.p1(mb, th0))
+        assert r == pytest.approx(O.mp_smooth(ma, lo, dm) / O.mp_smooth(mb, lo, dm), rel=1e-13)
+        r2 = (O.p2(ma, 20.0, th) / O.p2(ma, 20.0, th0)) / (O.p2(mb, 20.0, th) / O.p2(mb, 20.0, th0))
+        assert r2 == pytest.approx(O.mp_smooth(ma, lo, dm) / O.mp_smooth(mb, lo, dm), rel=1e-13)
+        assert O.p1(20.0, th) / O.p1(20.0, th0) == pytest.approx(1.0 / O.mp_N1(th), rel=1e-12)   # N1(dm = 0) = 1
+        assert O.mp_N1(th0) == pytest.approx(1.0, abs=1e-12)
+
+
+def test_mp_selection_constant_weights():
+    """As test_selection_constant_weights, under MULTIPEAK and with masses inside and above the smoothing window:
+    injections drawn from the model itself have equal weights (Eq. 4)."""
+    th = _th_mp()
+    rng = np.random.default_rng(10)
+    zmax, nz = 1.5, 256
+    zb = np.linspace(0, zmax, nz)
+    allsky = 0.3 + zb ** 2 * np.exp(-2 * zb)
+    n = 2000
+    with O.mass_model("multipeak"):
+        zf = np.linspace(0, zmax * (1 - 1e-9), 20001)
+        dens = np.array([O.psi(z, th) for z in zf]) / (1 + zf) * np.interp(zf, zb, allsky)
+        cdf = np.concatenate([[0], np.cumsum(0.5 * (dens[1:] + dens[:-1]) * np.diff(zf))])
+        z = np.interp(rng.uniform(0, 1, n), cdf / cdf[-1], zf)
+        m1 = rng.uniform(5.5, 40, n)
+        m2 = 5.2 + (m1 - 5.2) * rng.uniform(0, 1, n)
+        H0, Om = th[0], th[1]
+        dl = np.array([O.dL(zz, H0, Om) for zz in z])
+        h = 1e-6
+        ddl = np.array([(O.dL(zz + h, H0, Om) - O.dL(zz - h, H0, Om)) / (2 * h) for zz in z])
+        lp = np.log(np.interp(z, zf, dens)) + np.log([O.p1(a, th) * O.p2(b, a, th) for a, b in zip(m1, m2)]) \
+            - 2 * np.log1p(z) - np.log(ddl)
+        inj = dict(dL=dl, m1z=m1 * (1 + z), m2z=m2 * (1 + z), log_pdraw=lp, n_draw=7.0 * n)
+        logxi, neff = O.selection_logxi(th, inj, allsky, zmax, mode=O.EXACT)
+    assert logxi[0] == pytest.approx(math.log(1 / 7.0), abs=2e-6)
+    assert neff[0] == pytest.approx(n, rel=1e-8)
+
+
+def test_mp_theta_domain():
+    with O.mass_model("multipeak"):
+        assert O.theta_valid(_th_mp())
+        for bad in (dict(dm=-0.1), dict(dm=90.0), dict(sigl=0.0), dict(laml=1.2), dict(laml=-0.1)):
+            assert not O.theta_valid(_th_mp(**bad)), bad
