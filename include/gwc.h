@@ -61,6 +61,11 @@ extern "C" {
 #endif
 
 #define GWC_NPAR 12 /* theta row: H0, Om, alpha, beta, mmin, mmax, mu, sigma, lambda, gamma, kappa, zp */
+/* MULTIPEAK theta row (gwc_set_mass_model): the 12 columns above, in which (mu, sigma) are the HIGH Gaussian peak and
+ * lambda is lambda_g, the fraction in the two peaks; then delta_m, mu_g,low, sigma_g,low, lambda_g,low (the share of
+ * lambda_g in the low peak).  Table III. */
+#define GWC_NPAR_MULTIPEAK 16
+#define GWC_NPAR_MAX 16
 
 typedef enum {
   GWC_OK = 0,
@@ -79,6 +84,12 @@ typedef enum { GWC_F64 = 0, GWC_F32 = 1 } gwc_prec;
 /* bandwidth rule of the KDE numerator: Scott, Eq. D1 (the paper's default) | Silverman, Eq. D2 (:300) */
 typedef enum { GWC_BW_SCOTT = 0, GWC_BW_SILVERMAN = 1 } gwc_bw_rule;
 
+/* Mass model (App. A; Table III, :263-274).  GWC_MASS_PLPEAK: truncated power law + one Gaussian peak,
+ * conditional power law in m2 (R2, R3).  GWC_MASS_MULTIPEAK: power law + two Gaussian peaks, the primary
+ * and the secondary law both multiplied by the low-mass smoothing S(m | mmin, delta_m) and normalised numerically per
+ * theta (R33-R36; the formula is not printed in the paper). */
+typedef enum { GWC_MASS_PLPEAK = 0, GWC_MASS_MULTIPEAK = 1 } gwc_mass_model;
+
 typedef struct gwc_ctx gwc_ctx;
 
 /* Create a context on CUDA device `device`; `cuda_stream` is a cudaStream_t (NULL = default stream). */
@@ -92,6 +103,15 @@ const char* gwc_last_error(const gwc_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 int64_t gwc_launch_count(const gwc_ctx* ctx);
 
+/* Select the mass model of this context (default GWC_MASS_PLPEAK).  From then on every d_theta / h_theta argument has
+ * rows of gwc_theta_len(model) doubles.  Tables of an earlier gwc_build_cosmo are dropped (GWC_ERR_NOT_BUILT until the
+ * next build).  Additional theta-domain rules under MULTIPEAK: 0 <= delta_m, mmin + delta_m < mmax, sigma_g,low > 0,
+ * 0 <= lambda_g,low <= 1.  Supported by gwc_build_cosmo, gwc_event_loglik, gwc_event_loglik_pixcut,
+ * gwc_event_loglik_kde, gwc_selection_logxi, gwc_total_loglik, gwc_total_loglik_kde and gwc_total_loglik_host. */
+gwc_status gwc_set_mass_model(gwc_ctx* ctx, gwc_mass_model model);
+/* Doubles per theta row of a mass model: GWC_NPAR or GWC_NPAR_MULTIPEAK (0 for an unknown model). */
+int32_t gwc_theta_len(gwc_mass_model model);
+
 /*
  * A1 + A2.  For each theta: D(z) = int_0^z dz'/E(z') by cumulative Gauss-Legendre
  * quadrature on a uniform z grid (Eq. 1), u(z) = (1+z) D(z) = d_L H0/c, monotone
@@ -101,7 +121,10 @@ int64_t gwc_launch_count(const gwc_ctx* ctx);
  * table_prec = GWC_F32 selects 32-bit storage (8 bytes per node instead of 16): z_m as an unsigned 32-bit
  * fixed-point fraction of z_max (absolute step z_max/(2^32-1)), the slope as a binary32 in the same units
  * (R22).
- *   d_theta [n_theta][GWC_NPAR] f64, row-major.   z_max > 0.   n_nodes in [2, 8193] (1025 typical).
+ *   d_theta [n_theta][gwc_theta_len(model)] f64, row-major.   z_max > 0.   n_nodes in [2, 8193] (1025 typical).
+ * Under GWC_MASS_MULTIPEAK the same call also builds, per theta, the normalisation N1 of p(m1) and a 513-node
+ * cubic-Hermite table of the normaliser of p(m2 | m1) over the smoothing window [mmin, mmin + delta_m] (above the
+ * window it is elementary), by 4 x 8-point Gauss-Legendre quadrature per table interval (R36).
  */
 gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double z_max, int32_t n_nodes,
                            gwc_prec table_prec);

@@ -41,6 +41,9 @@ struct gwc_ctx {
   int* d_flag = nullptr;
   unsigned int* d_counter = nullptr;
   // A1/A2 state
+  int model = 0;            // gwc_mass_model: theta rows have npar doubles, constant rows nconst_of(model)
+  int npar = GWC_NPAR;
+  Buf ftab;                 // MULTIPEAK: [n_theta][MF_PITCH] Node64, F(m1) over the smoothing window
   Buf tab, tconst;
   Buf theta_snap, tvalid;   // the theta rows the tables were built from; per-theta validity (1.0 | NaN)
   const double* built_theta = nullptr;
@@ -146,7 +149,7 @@ gwc_status check_built(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, dou
     return fail(ctx, GWC_ERR_NOT_BUILT, "cosmology table built with a smaller z_max than the LOS table's");
   if (ctx->fresh_build) return GWC_OK;
   return count(ctx, launch_verify_theta(d_theta, (const double*)ctx->theta_snap.p, (const double*)ctx->tconst.p,
-                                        n_theta, (double*)ctx->tvalid.p, ctx->d_flag, ctx->stream),
+                                        n_theta, ctx->model, (double*)ctx->tvalid.p, ctx->d_flag, ctx->stream),
                "verify_theta");
 }
 
@@ -186,7 +189,8 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   GWC_TRY(ensure(ctx, ctx->part_n, (size_t)n_theta * n_seg * sizeof(int32_t)));
   if (pixcut) GWC_TRY(ensure(ctx, ctx->part_np, (size_t)n_theta * n_seg * sizeof(int32_t)));
   // theta tile: as many tables as shared memory holds, balanced over the tiles
-  int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut);
+  const bool mp = ctx->model == GWC_MASS_MULTIPEAK;
+  int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut, mp);
   if (T < 1) return fail(ctx, GWC_ERR_SHAPE, "n_nodes / n_z too large for shared memory");
   if ((int64_t)T > n_theta) T = (int)n_theta;
   const int n_tiles = (int)((n_theta + T - 1) / T);
@@ -202,6 +206,8 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
                 "make_groups"));
   ReweightParams p;
   memset(&p, 0, sizeof(p));
+  p.model = ctx->model;
+  p.ftab = (const Node64*)ctx->ftab.p;
   p.tab = ctx->tab.p;
   p.tconst = (const double*)ctx->tconst.p;
   p.n_theta = (int)n_theta;
@@ -232,8 +238,9 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.pixcut = pixcut ? 1 : 0;
   // events shorter on average than 2048 samples leave warps of a 16-warp CTA without a block: let them share it
   // batches of a few theta points (the sampler's one-point-per-call pattern): no discarded pipeline step
-  p.odd = (!pixcut && n_theta <= 9 && (n_theta & 1)) ? 1 : 0;
-  p.teams = (!inj && !pixcut && !p.odd && n_seg > 0 && n / n_seg < 2048) ? 1 : 0;
+  // (MULTIPEAK has the plain and the pixel-cut kernel only)
+  p.odd = (!mp && !pixcut && n_theta <= 9 && (n_theta & 1)) ? 1 : 0;
+  p.teams = (!mp && !inj && !pixcut && !p.odd && n_seg > 0 && n / n_seg < 2048) ? 1 : 0;
   p.neff_min = neff_min;
   p.unit_counter = ctx->d_counter;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -309,7 +316,7 @@ void gwc_destroy(gwc_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
   cudaStreamSynchronize(ctx->stream);
-  Buf* bufs[] = {&ctx->tab, &ctx->tconst, &ctx->theta_snap, &ctx->tvalid, &ctx->seg_off, &ctx->prep[0].dLc, &ctx->prep[0].L1, &ctx->prep[0].Q,
+  Buf* bufs[] = {&ctx->ftab, &ctx->tab, &ctx->tconst, &ctx->theta_snap, &ctx->tvalid, &ctx->seg_off, &ctx->prep[0].dLc, &ctx->prep[0].L1, &ctx->prep[0].Q,
                  &ctx->prep[0].P, &ctx->prep[0].seg_shift, &ctx->prep[1].dLc, &ctx->prep[1].L1, &ctx->prep[1].Q,
                  &ctx->prep[1].P, &ctx->prep[1].seg_shift,
                  &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->kde_scr, &ctx->kde_len, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
@@ -349,6 +356,20 @@ const char* gwc_last_error(const gwc_ctx* ctx) { return ctx ? ctx->err.c_str() :
 
 int64_t gwc_launch_count(const gwc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+gwc_status gwc_set_mass_model(gwc_ctx* ctx, gwc_mass_model model) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (model != GWC_MASS_PLPEAK && model != GWC_MASS_MULTIPEAK) return fail(ctx, GWC_ERR_INVALID_ARG, "unknown mass model");
+  ctx->model = (int)model;
+  ctx->npar = gwc_theta_len(model);
+  ctx->built_theta = nullptr;   // tables and constants of the other model are of no use
+  ctx->built_n = 0;
+  return GWC_OK;
+}
+
+int32_t gwc_theta_len(gwc_mass_model model) {
+  return model == GWC_MASS_PLPEAK ? GWC_NPAR : model == GWC_MASS_MULTIPEAK ? GWC_NPAR_MULTIPEAK : 0;
+}
+
 gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double z_max, int32_t n_nodes,
                            gwc_prec table_prec) {
   GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
@@ -359,12 +380,13 @@ gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta,
   const size_t node = table_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32);
   ctx->built_theta = nullptr;
   GWC_TRY(ensure(ctx, ctx->tab, (size_t)n_theta * Mp * node));
-  GWC_TRY(ensure(ctx, ctx->tconst, (size_t)n_theta * NCONST * sizeof(double)));
-  GWC_TRY(ensure(ctx, ctx->theta_snap, (size_t)n_theta * GWC_NPAR * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->tconst, (size_t)n_theta * nconst_of(ctx->model) * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->theta_snap, (size_t)n_theta * ctx->npar * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->tvalid, (size_t)n_theta * sizeof(double)));
-  GWC_TRY(count(ctx, launch_cosmo_build(d_theta, n_theta, z_max, n_nodes, Mp, table_prec, ctx->tab.p,
-                                        (double*)ctx->tconst.p, (double*)ctx->theta_snap.p, (double*)ctx->tvalid.p,
-                                        ctx->d_flag, ctx->stream),
+  if (ctx->model == GWC_MASS_MULTIPEAK) GWC_TRY(ensure(ctx, ctx->ftab, (size_t)n_theta * MF_PITCH * sizeof(Node64)));
+  GWC_TRY(count(ctx, launch_cosmo_build(d_theta, n_theta, ctx->model, z_max, n_nodes, Mp, table_prec, ctx->tab.p,
+                                        (double*)ctx->tconst.p, (Node64*)ctx->ftab.p, (double*)ctx->theta_snap.p,
+                                        (double*)ctx->tvalid.p, ctx->d_flag, ctx->stream),
                 "cosmo_build"));
   ctx->built_theta = d_theta;
   ctx->built_n = n_theta;
@@ -378,7 +400,7 @@ gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta,
 gwc_status gwc_export_cosmo(gwc_ctx* ctx, double* d_z, double* d_dz, double* d_umax) {
   if (!ctx) return GWC_ERR_INVALID_ARG;
   if (!ctx->built_theta) return fail(ctx, GWC_ERR_NOT_BUILT, "no cosmology table built");
-  return count(ctx, launch_export_cosmo(ctx->tab.p, (const double*)ctx->tconst.p, ctx->built_n, ctx->M, ctx->Mp,
+  return count(ctx, launch_export_cosmo(ctx->tab.p, (const double*)ctx->tconst.p, nconst_of(ctx->model), ctx->built_n, ctx->M, ctx->Mp,
                                         ctx->tab_prec, ctx->z_max, d_z, d_dz, d_umax, ctx->stream),
                "export_cosmo");
 }
@@ -528,7 +550,7 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
     cudaEventRecord(e0, s);
   }
   // the population parameters come from the copy of theta the tables were built from, never from a changed array
-  const gwc_status st_kde = count(ctx, launch_kde((const double*)ctx->theta_snap.p, ctx->tab.p, (const double*)ctx->tconst.p, (const double*)ctx->tvalid.p, n_theta, ctx->M, ctx->Mp,
+  const gwc_status st_kde = count(ctx, launch_kde(ctx->model, (const Node64*)ctx->ftab.p, (const double*)ctx->theta_snap.p, ctx->tab.p, (const double*)ctx->tconst.p, (const double*)ctx->tvalid.p, n_theta, ctx->M, ctx->Mp,
                                 ctx->tab_prec, ctx->z_max / NODE32_QMAX, ev->n_events, ev->ev_sample_off, ev->dL,
                                 ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->prep[0].seg_shift.p,
                                 los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, bw_rule,
@@ -639,7 +661,7 @@ gwc_status gwc_total_loglik_host(gwc_ctx* ctx, const double* h_theta, int64_t n_
   };
   const size_t ns = (size_t)h_ev->n_samples, ni = (size_t)h_inj->n_found;
   const size_t los_el = h_los->prec == GWC_F64 ? 8 : 4;
-  GWC_TRY(upload(h.theta, h_theta, (size_t)n_theta * GWC_NPAR * 8));
+  GWC_TRY(upload(h.theta, h_theta, (size_t)n_theta * ctx->npar * 8));
   GWC_TRY(upload(h.ev_off, h_ev->ev_sample_off, (size_t)(h_ev->n_events + 1) * 8));
   GWC_TRY(upload(h.ev_dL, h_ev->dL, ns * 8));
   GWC_TRY(upload(h.ev_m1z, h_ev->m1z, ns * 8));

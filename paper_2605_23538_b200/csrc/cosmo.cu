@@ -43,9 +43,15 @@ __device__ __forceinline__ void store_node(Node32* t, double z, double d, double
   t->d = __double2float_rn(d * inv_q);
 }
 
-__device__ bool theta_valid(const double* th) {
-  for (int i = 0; i < GWC_NPAR; ++i)
+__device__ bool theta_valid(const double* th, int model) {
+  const int npar = model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR;
+  for (int i = 0; i < npar; ++i)
     if (!isfinite(th[i])) return false;
+  if (model == 1) {   // MULTIPEAK (R35): delta_m, mu_low, sigma_low, lambda_low = th[12..15]
+    if (!(th[12] >= 0.0 && th[4] + th[12] < th[5])) return false;
+    if (!(th[14] > 0.0)) return false;
+    if (!(th[15] >= 0.0 && th[15] <= 1.0)) return false;
+  }
   if (!(th[0] > 0.0)) return false;
   if (!(th[1] > 0.0 && th[1] <= 1.0)) return false;
   if (!(th[7] > 0.0)) return false;
@@ -57,10 +63,34 @@ __device__ bool theta_valid(const double* th) {
   return true;
 }
 
+// 8-point Gauss-Legendre on [-1, 1]
+__constant__ double GL8_X[8] = {-0.96028985649753623168, -0.79666647741362673959, -0.52553240991632898582,
+                                -0.18343464249564980494, 0.18343464249564980494,  0.52553240991632898582,
+                                0.79666647741362673959,  0.96028985649753623168};
+__constant__ double GL8_W[8] = {0.10122853629037625915, 0.22238103445337447054, 0.31370664587788728734,
+                                0.36268378337836198297, 0.36268378337836198297, 0.31370664587788728734,
+                                0.22238103445337447054, 0.10122853629037625915};
+
+// MULTIPEAK smoothing (R34) at m' = m - mmin inside (0, dm): S and 1 - S, each without cancellation
+__device__ __forceinline__ void mp_smooth(double mp, double dm, double& S, double& oneMinusS) {
+  const double e = dm / mp + dm / (mp - dm);
+  S = 1.0 / (1.0 + exp(e));          // exp overflows to +inf near mmin: S = 0
+  oneMinusS = 1.0 / (1.0 + exp(-e));
+}
+
+struct MpMix {   // the MULTIPEAK mixture before smoothing, components normalised on [mmin, mmax]
+  double a_pl, alpha, a_gl, mul, isl, a_gh, muh, ish;
+  __device__ double operator()(double m) const {
+    const double yl = (m - mul) * isl, yh = (m - muh) * ish;
+    return a_pl * pow(m, -alpha) + a_gl * exp(-0.5 * yl * yl) + a_gh * exp(-0.5 * yh * yh);
+  }
+};
+
 template <typename NodeT>
-__global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* __restrict__ theta, double z_max,
-                                                                  int M, int Mp, NodeT* __restrict__ tab,
+__global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* __restrict__ theta, int model,
+                                                                  double z_max, int M, int Mp, NodeT* __restrict__ tab,
                                                                   double* __restrict__ tconst,
+                                                                  Node64* __restrict__ ftab,
                                                                   double* __restrict__ theta_snap,
                                                                   double* __restrict__ tvalid, int* flag) {
   __shared__ double Dg[QUAD_K + 1];
@@ -68,16 +98,19 @@ __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* _
   __shared__ double part[CB_THREADS];
   __shared__ double s_umax;
   const int t = blockIdx.x, tid = threadIdx.x;
-  const double* th = theta + (size_t)t * GWC_NPAR;
+  const int npar = model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR, ncst = nconst_of(model);
+  const double* th = theta + (size_t)t * npar;
   NodeT* row = tab + (size_t)t * Mp;
-  double* tc = tconst + (size_t)t * NCONST;
-  const bool valid = theta_valid(th);
+  double* tc = tconst + (size_t)t * ncst;
+  const bool valid = theta_valid(th, model);
   // the copy of theta the tables belong to (the dependent calls compare the caller's array with it)
-  if (tid < GWC_NPAR) theta_snap[(size_t)t * GWC_NPAR + tid] = th[tid];
+  if (tid < npar) theta_snap[(size_t)t * npar + tid] = th[tid];
   if (tid == 0) tvalid[t] = valid ? 1.0 : CUDART_NAN;
   if (!valid) {
     for (int m = tid; m < Mp; m += CB_THREADS) store_node(row + m, 0.0, 0.0, 0.0);
-    if (tid < NCONST) tc[tid] = (tid == C_VALID) ? CUDART_NAN : 0.0;
+    if (model == 1)
+      for (int m = tid; m < MF_PITCH; m += CB_THREADS) ftab[(size_t)t * MF_PITCH + m] = Node64{0.0, 0.0};
+    if (tid < ncst) tc[tid] = (tid == C_VALID) ? CUDART_NAN : 0.0;
     if (tid == 0) atomicOr(flag, FLAG_DOMAIN);
     return;
   }
@@ -152,16 +185,112 @@ __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* _
     }
     store_node(row + m, z, d, NODE32_QMAX / z_max);
   }
-  // 4. constants
+  // 4. MULTIPEAK (R33-R36): N1 = int mix S = 1 - int_window mix (1 - S), and the table of
+  //    |F|(m1) = |beta+1| C(m1) / (S(m1) m1^(beta+1)), C(m1) = int_mmin^m1 m^beta S(m) dm, on MF_NODES uniform nodes of
+  //    the window [mmin, mmin + delta_m] with the analytic slopes F' = (beta+1)/m - F (S'/S + (beta+1)/m),
+  //    S'/S = (1 - S) delta_m (1/m'^2 + 1/(m' - delta_m)^2).  Every table interval by 4 panels of 8-point
+  //    Gauss-Legendre.  (The first two intervals, where S < e^-255, are inaccurate in relative terms: the integrand
+  //    is an essential singularity there; samples that low carry no weight.)
+  __shared__ double cI[MF_NODES], dI[MF_NODES];
+  __shared__ double s_n1, s_ctop;
+  const double alpha = th[2], beta = th[3], mmin = th[4], mmax = th[5], mu = th[6], sigma = th[7], lam = th[8];
+  const double n_pl = (1.0 - alpha) / (pow(mmax, 1.0 - alpha) - pow(mmin, 1.0 - alpha));
+  const double rs2 = 1.0 / (sigma * 1.41421356237309504880);
+  const double n_g = 1.0 / (0.5 * (erf((mmax - mu) * rs2) - erf((mmin - mu) * rs2)));
+  double n_gl = 0.0;
+  if (model == 1) {
+    const double dm = th[12], mul = th[13], sigl = th[14], laml = th[15];
+    const double rsl = 1.0 / (sigl * 1.41421356237309504880);
+    n_gl = 1.0 / (0.5 * (erf((mmax - mul) * rsl) - erf((mmin - mul) * rsl)));
+    MpMix mix;
+    mix.a_pl = (1.0 - lam) * n_pl;
+    mix.alpha = alpha;
+    mix.a_gl = lam * laml * n_gl / (sigl * 2.50662827463100050242);
+    mix.mul = mul;
+    mix.isl = 1.0 / sigl;
+    mix.a_gh = lam * (1.0 - laml) * n_g / (sigma * 2.50662827463100050242);
+    mix.muh = mu;
+    mix.ish = 1.0 / sigma;
+    const double hF = dm / (MF_NODES - 1);
+    for (int k = tid; k < MF_NODES - 1; k += CB_THREADS) {
+      double sc = 0.0, sd = 0.0;
+      const double w = 0.25 * hF;
+      for (int sub = 0; sub < 4; ++sub) {
+        const double a = (k * 4 + sub) * w;
+        for (int i = 0; i < 8; ++i) {
+          const double mp = a + 0.5 * w * (GL8_X[i] + 1.0);
+          double S, nS;
+          mp_smooth(mp, dm, S, nS);
+          const double m = mmin + mp;
+          sc = fma(GL8_W[i], pow(m, beta) * S, sc);
+          sd = fma(GL8_W[i], mix(m) * nS, sd);
+        }
+      }
+      cI[k] = 0.5 * w * sc;
+      dI[k] = 0.5 * w * sd;
+    }
+    __syncthreads();
+    if (tid == 0) {   // cumulative C at the nodes (ascending, compensated), total deficit
+      double s = 0.0, comp = 0.0, d = 0.0;
+      for (int k = 0; k < MF_NODES - 1; ++k) {
+        const double v = dm > 0.0 ? cI[k] : 0.0;
+        d += dm > 0.0 ? dI[k] : 0.0;
+        const double tsum = s + v;
+        comp += (s - tsum) + v;
+        s = tsum;
+        cI[k] = s + comp;   // C at node k + 1
+      }
+      s_ctop = s + comp;
+      s_n1 = 1.0 - d;
+    }
+    __syncthreads();
+    const double sgn = (beta + 1.0 > 0.0) ? 1.0 : -1.0;
+    Node64* fr = ftab + (size_t)t * MF_PITCH;
+    for (int k = tid; k < MF_PITCH; k += CB_THREADS) {
+      double F = 0.0, dF = 0.0;
+      if (k >= 1 && dm > 0.0) {
+        const int kk = k < MF_NODES - 1 ? k : MF_NODES - 1;
+        const double mp = kk * hF, m = mmin + mp, C = cI[kk - 1];
+        double S = 1.0, nS = 0.0, q = 0.0;   // q = S'/S
+        if (kk < MF_NODES - 1) {
+          mp_smooth(mp, dm, S, nS);
+          q = nS * dm * (1.0 / (mp * mp) + 1.0 / ((mp - dm) * (mp - dm)));
+        }
+        const double Fs = S > 0.0 ? (beta + 1.0) * C / (S * pow(m, beta + 1.0)) : 0.0;
+        const double dFs = S > 0.0 ? (beta + 1.0) / m - Fs * (q + (beta + 1.0) / m) : 0.0;
+        F = sgn * Fs;
+        dF = (k <= MF_NODES - 1) ? sgn * dFs * hF : 0.0;
+        if (!(isfinite(F) && isfinite(dF))) { F = 0.0; dF = 0.0; }
+      }
+      fr[k] = Node64{F, dF};
+    }
+  }
+  // 5. constants
   if (tid == 0) {
-    const double H0 = th[0], alpha = th[2], beta = th[3], mmin = th[4], mmax = th[5], mu = th[6], sigma = th[7],
-                 lam = th[8], gam = th[9], kap = th[10], zp = th[11];
+    const double H0 = th[0], gam = th[9], kap = th[10], zp = th[11];
     const double h = H0 / C_KMS;
-    const double n_pl = (1.0 - alpha) / (pow(mmax, 1.0 - alpha) - pow(mmin, 1.0 - alpha));
-    const double rs2 = 1.0 / (sigma * 1.41421356237309504880);
-    const double n_g = 1.0 / (0.5 * (erf((mmax - mu) * rs2) - erf((mmin - mu) * rs2)));
     const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
-    const double common = fabs(beta + 1.0) * psi0 * h;
+    double common = fabs(beta + 1.0) * psi0 * h;
+    double lam_hi = lam;   // coefficient of the (high) Gaussian peak
+    double e1c = (beta + 1.0) * log(mmin);
+    if (model == 1) {
+      const double dm = th[12], mul = th[13], sigl = th[14], laml = th[15], top = mmin + dm;
+      common /= s_n1;
+      lam_hi = lam * (1.0 - laml);
+      e1c = log(pow(top, beta + 1.0) - (beta + 1.0) * s_ctop);
+      const double lam_lo = lam * laml;
+      tc[C_CG2] = (lam_lo > 0.0) ? log(lam_lo * n_gl / (sigl * 2.50662827463100050242) * common) : -CUDART_INF;
+      tc[C_INVSIG2] = 1.0 / sigl;
+      tc[C_NMUSIG2] = -mul / sigl;
+      tc[C_DM] = dm;
+      tc[C_FIDX] = dm > 0.0 ? (MF_NODES - 1) / dm : 0.0;
+      tc[C_N1] = s_n1;
+      tc[C_CTOP] = s_ctop;
+      tc[C_NGL] = n_gl;
+      for (int i = C_COUNT_MP; i < NCONST_MP; ++i) tc[i] = 0.0;
+    } else {
+      for (int i = C_COUNT; i < NCONST; ++i) tc[i] = 0.0;
+    }
     tc[C_H] = h;
     tc[C_UMAX] = umax;
     tc[C_INVDU] = (M - 1) / umax;
@@ -171,18 +300,17 @@ __global__ void __launch_bounds__(CB_THREADS) cosmo_build_kernel(const double* _
     tc[C_GM1] = gam - 1.0;
     tc[C_NALPHA] = -alpha;
     tc[C_CPL] = (lam < 1.0) ? log((1.0 - lam) * n_pl * common) : -CUDART_INF;
-    tc[C_CG] = (lam > 0.0) ? log(lam * n_g / (sigma * 2.50662827463100050242) * common) : -CUDART_INF;
+    tc[C_CG] = (lam_hi > 0.0) ? log(lam_hi * n_g / (sigma * 2.50662827463100050242) * common) : -CUDART_INF;
     tc[C_INVSIG] = 1.0 / sigma;
     tc[C_NMUSIG] = -mu / sigma;
     tc[C_NBP1] = -(beta + 1.0);
-    tc[C_E1C] = (beta + 1.0) * log(mmin);
+    tc[C_E1C] = e1c;
     tc[C_SGN] = (beta + 1.0 > 0.0) ? 1.0 : -1.0;
     tc[C_GK] = gam + kap;
     tc[C_E2C] = -(gam + kap) * log1p(zp);
     tc[C_OM] = Om;
     tc[C_OL] = OL;
     tc[C_VALID] = 1.0;
-    for (int i = C_COUNT; i < NCONST; ++i) tc[i] = 0.0;
   }
 }
 
@@ -192,8 +320,8 @@ __device__ __forceinline__ double node_z(const Node32& n, double z_max) { return
 __device__ __forceinline__ double node_d(const Node32& n, double z_max) { return (double)n.d * (z_max / NODE32_QMAX); }
 
 template <typename NodeT>
-__global__ void export_cosmo_kernel(const NodeT* __restrict__ tab, const double* __restrict__ tconst, int64_t n_theta,
-                                    int M, int Mp, double z_max, double* z, double* dz, double* umax) {
+__global__ void export_cosmo_kernel(const NodeT* __restrict__ tab, const double* __restrict__ tconst, int ncst,
+                                    int64_t n_theta, int M, int Mp, double z_max, double* z, double* dz, double* umax) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n_theta * M) return;
   int64_t t = i / M;
@@ -201,57 +329,61 @@ __global__ void export_cosmo_kernel(const NodeT* __restrict__ tab, const double*
   NodeT nd = tab[t * Mp + m];
   if (z) z[i] = node_z(nd, z_max);
   if (dz) dz[i] = node_d(nd, z_max);
-  if (umax && m == 0) umax[t] = tconst[t * NCONST + C_UMAX];
+  if (umax && m == 0) umax[t] = tconst[t * ncst + C_UMAX];
 }
 
 }  // namespace
 
-int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int M, int Mp, gwc_prec prec, void* d_tab,
-                       double* d_tconst, double* d_theta_snap, double* d_tvalid, int* d_flag, cudaStream_t s) {
+int launch_cosmo_build(const double* d_theta, int64_t n_theta, int model, double z_max, int M, int Mp, gwc_prec prec,
+                       void* d_tab, double* d_tconst, Node64* d_ftab, double* d_theta_snap, double* d_tvalid,
+                       int* d_flag, cudaStream_t s) {
   if (n_theta <= 0) return 0;
   if (prec == GWC_F64)
-    cosmo_build_kernel<Node64><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, z_max, M, Mp, (Node64*)d_tab,
-                                                                         d_tconst, d_theta_snap, d_tvalid, d_flag);
+    cosmo_build_kernel<Node64><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, model, z_max, M, Mp, (Node64*)d_tab,
+                                                                         d_tconst, d_ftab, d_theta_snap, d_tvalid,
+                                                                         d_flag);
   else
-    cosmo_build_kernel<Node32><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, z_max, M, Mp, (Node32*)d_tab,
-                                                                         d_tconst, d_theta_snap, d_tvalid, d_flag);
+    cosmo_build_kernel<Node32><<<(unsigned)n_theta, CB_THREADS, 0, s>>>(d_theta, model, z_max, M, Mp, (Node32*)d_tab,
+                                                                         d_tconst, d_ftab, d_theta_snap, d_tvalid,
+                                                                         d_flag);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
 namespace {
 // one thread per theta: bitwise comparison of the caller's row with the copy the tables were built from
 __global__ void verify_theta_kernel(const double* __restrict__ theta, const double* __restrict__ snap,
-                                    const double* __restrict__ tconst, int64_t n_theta, double* __restrict__ tvalid,
-                                    int* flag) {
+                                    const double* __restrict__ tconst, int64_t n_theta, int npar, int ncst,
+                                    double* __restrict__ tvalid, int* flag) {
   const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (t >= n_theta) return;
   bool same = true;
-  for (int i = 0; i < GWC_NPAR; ++i)
-    same = same && __double_as_longlong(theta[t * GWC_NPAR + i]) == __double_as_longlong(snap[t * GWC_NPAR + i]);
-  tvalid[t] = same ? tconst[t * NCONST + C_VALID] : CUDART_NAN;
+  for (int i = 0; i < npar; ++i)
+    same = same && __double_as_longlong(theta[t * npar + i]) == __double_as_longlong(snap[t * npar + i]);
+  tvalid[t] = same ? tconst[t * ncst + C_VALID] : CUDART_NAN;
   if (!same) atomicOr(flag, FLAG_STALE);
 }
 }  // namespace
 
 int launch_verify_theta(const double* d_theta, const double* d_theta_snap, const double* d_tconst, int64_t n_theta,
-                        double* d_tvalid, int* d_flag, cudaStream_t s) {
+                        int model, double* d_tvalid, int* d_flag, cudaStream_t s) {
   if (n_theta <= 0) return 0;
-  verify_theta_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(d_theta, d_theta_snap, d_tconst, n_theta,
-                                                                        d_tvalid, d_flag);
+  verify_theta_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(
+      d_theta, d_theta_snap, d_tconst, n_theta, model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR, nconst_of(model), d_tvalid,
+      d_flag);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-int launch_export_cosmo(const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp, gwc_prec prec,
-                        double z_max, double* d_z, double* d_dz, double* d_umax, cudaStream_t s) {
+int launch_export_cosmo(const void* d_tab, const double* d_tconst, int ncst, int64_t n_theta, int M, int Mp,
+                        gwc_prec prec, double z_max, double* d_z, double* d_dz, double* d_umax, cudaStream_t s) {
   int64_t n = n_theta * M;
   if (n <= 0) return 0;
   unsigned blocks = (unsigned)((n + 255) / 256);
   if (prec == GWC_F64)
-    export_cosmo_kernel<Node64><<<blocks, 256, 0, s>>>((const Node64*)d_tab, d_tconst, n_theta, M, Mp, z_max, d_z, d_dz,
-                                                       d_umax);
+    export_cosmo_kernel<Node64><<<blocks, 256, 0, s>>>((const Node64*)d_tab, d_tconst, ncst, n_theta, M, Mp, z_max, d_z,
+                                                       d_dz, d_umax);
   else
-    export_cosmo_kernel<Node32><<<blocks, 256, 0, s>>>((const Node32*)d_tab, d_tconst, n_theta, M, Mp, z_max, d_z, d_dz,
-                                                       d_umax);
+    export_cosmo_kernel<Node32><<<blocks, 256, 0, s>>>((const Node32*)d_tab, d_tconst, ncst, n_theta, M, Mp, z_max, d_z,
+                                                       d_dz, d_umax);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -33,9 +33,25 @@ enum : int {
   C_OM,
   C_OL,        // 1 - Om
   C_VALID,     // 1.0 or NaN (theta-domain violation)
-  C_COUNT
+  C_COUNT,
+  // ---- MULTIPEAK rows only (row length NCONST_MP; R33-R36).  There CPL / CG carry 1/N1, CG / INVSIG /
+  // NMUSIG belong to the HIGH peak, and E1C = ln(top^(beta+1) - (beta+1) C_top), top = mmin + delta_m, so that above
+  // the smoothing window |beta+1| C(m1) / m1^(beta+1) = sign(beta+1) (1 - e1) as in the power-law+peak model.
+  C_CG2 = C_COUNT,  // ln[lambda_g lambda_low n_g,low / (sigma_low sqrt(2 pi)) |beta+1| psi0 h / N1]   (-inf when absent)
+  C_INVSIG2,   // 1/sigma_low
+  C_NMUSIG2,   // -mu_low/sigma_low
+  C_DM,        // delta_m
+  C_FIDX,      // (MF_NODES - 1) / delta_m   (0 when delta_m = 0)
+  C_N1,        // int mix S dm over [mmin, mmax]                       (read by the KDE kernel)
+  C_CTOP,      // C(top) = int over the smoothing window of m^beta S(m) dm   (read by the KDE kernel)
+  C_NGL,       // normalisation of the low Gaussian on [mmin, mmax]    (read by the KDE kernel)
+  C_COUNT_MP
 };
-constexpr int NCONST = 24;  // padded row length (>= C_COUNT), keeps rows 64-byte aligned
+constexpr int NCONST = 24;     // padded row length (>= C_COUNT), keeps rows 64-byte aligned
+constexpr int NCONST_MP = 32;  // row length under MULTIPEAK (>= C_COUNT_MP)
+constexpr int MF_NODES = 513;  // nodes of the per-theta table of F(m1) = |beta+1| C(m1) / (S(m1) m1^(beta+1)) on the window
+constexpr int MF_PITCH = 514;
+__host__ __device__ inline int nconst_of(int model) { return model == 1 ? NCONST_MP : NCONST; }
 
 #ifndef GWC_NTHREADS
 #define GWC_NTHREADS 512
@@ -47,6 +63,7 @@ constexpr int NTHREADS = GWC_NTHREADS;  // threads per CTA of the fused kernel (
 constexpr int NWARPS = NTHREADS / 32;
 constexpr int SPT = GWC_SPT;      // samples per thread per theta (independent chains in flight)
 constexpr int KT_THETA = 340;     // theta points whose constants fit the constant bank (one launch)
+constexpr int KT_THETA_MP = KT_THETA * NCONST / NCONST_MP;   // ... with MULTIPEAK rows (255)
 #ifndef GWC_MAX_T
 #define GWC_MAX_T 16
 #endif
@@ -63,6 +80,8 @@ constexpr double NODE32_QMAX = 4294967295.0;
 __host__ __device__ inline int table_pitch(int M) { return (M + 2) & ~1; }
 
 struct ReweightParams {
+  int model;                // gwc_mass_model
+  const Node64* ftab;       // MULTIPEAK: [n_theta][MF_PITCH] (F, dm/(MF_NODES-1) F') of the smoothing window
   const void* tab;          // [n_theta][Mp] Node64 | Node32
   const double* tconst;     // [n_theta][NCONST]
   int n_theta, M, Mp, T, n_tiles;   // n_theta, n_tiles: of the batch (set per launch by launch_reweight)
@@ -99,14 +118,16 @@ enum : int {
 // clamped exponentials (e^-700) and the squares of the weights lose their meaning (R23)
 constexpr double RANGE_MIN_SUM = 5.148200222412013e-131;   // e^-300
 
-int launch_cosmo_build(const double* d_theta, int64_t n_theta, double z_max, int M, int Mp, gwc_prec prec,
-                       void* d_tab, double* d_tconst, double* d_theta_snap, double* d_tvalid, int* d_flag,
-                       cudaStream_t s);
+// model: gwc_mass_model; theta rows have gwc_theta_len(model) doubles, tconst rows nconst_of(model); d_ftab only under
+// MULTIPEAK
+int launch_cosmo_build(const double* d_theta, int64_t n_theta, int model, double z_max, int M, int Mp, gwc_prec prec,
+                       void* d_tab, double* d_tconst, Node64* d_ftab, double* d_theta_snap, double* d_tvalid,
+                       int* d_flag, cudaStream_t s);
 // compares d_theta with the copy gwc_build_cosmo took: tvalid[t] = tconst[t][C_VALID] or NaN (+ FLAG_STALE)
 int launch_verify_theta(const double* d_theta, const double* d_theta_snap, const double* d_tconst, int64_t n_theta,
-                        double* d_tvalid, int* d_flag, cudaStream_t s);
-int launch_export_cosmo(const void* d_tab, const double* d_tconst, int64_t n_theta, int M, int Mp, gwc_prec prec,
-                        double z_max, double* d_z, double* d_dz, double* d_umax, cudaStream_t s);
+                        int model, double* d_tvalid, int* d_flag, cudaStream_t s);
+int launch_export_cosmo(const void* d_tab, const double* d_tconst, int ncst, int64_t n_theta, int M, int Mp,
+                        gwc_prec prec, double z_max, double* d_z, double* d_dz, double* d_umax, cudaStream_t s);
 // per-sample, theta-independent preparation (+ per-segment shift = max(-ln pi - ln m1z))
 int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const double* dL, const double* m1z,
                         const double* m2z, const double* lprior, const int32_t* row, int64_t n_rows, double* dLc,
@@ -114,8 +135,8 @@ int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const 
 int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
                        cudaStream_t s);
 int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off, cudaStream_t s);
-size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix);
-int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix);
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp);
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp);
 int reweight_configure(int smem_optin);
 int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm, int device,
                     cudaStream_t s);
@@ -133,7 +154,7 @@ int launch_combine_total(const double* logL, const double* logxi, int64_t n_thet
 int launch_allsky(const void* table, gwc_prec prec, int64_t n_rows, int n_z, double* scratch, double* allsky,
                   cudaStream_t s);
 size_t allsky_scratch_doubles(int64_t n_rows, int n_z);
-int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, const double* d_tvalid, int64_t n_theta, int M, int Mp,
+int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const void* d_tab, const double* d_tconst, const double* d_tvalid, int64_t n_theta, int M, int Mp,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,

@@ -33,9 +33,11 @@ constexpr double KDE_BETA_MAX = 1.5;  // fast path of the KDE pass: grid step <=
 constexpr double C_KMS_KDE = 299792.458;
 
 struct KdeParams {
-  const double* theta;      // [n_theta][12]: the copy gwc_build_cosmo took (the tables belong to it)
+  int model;                // gwc_mass_model
+  const Node64* ftab;       // MULTIPEAK: [n_theta][MF_PITCH] table of |F|(m1) over the smoothing window
+  const double* theta;      // [n_theta][npar]: the copy gwc_build_cosmo took (the tables belong to it)
   const void* tab;          // [n_theta][Mp] Node64 | Node32
-  const double* tconst;     // [n_theta][NCONST] (umax, 1/du)
+  const double* tconst;     // [n_theta][nconst_of(model)] (umax, 1/du; MULTIPEAK: N1, C(top), n_g,low)
   const double* tvalid;     // [n_theta] 1.0, or NaN: outside the domain / changed since the build
   int64_t n_theta, n_events;
   int M, Mp;
@@ -70,6 +72,10 @@ struct ThetaK {
   double a_pl, a_g;      // (1 - lambda) n_pl  and  lambda n_g / (sigma sqrt(2 pi))
   double bp1, mminb;     // beta + 1, mmin^(beta+1)
   double Om, OL, cH;     // c / H0
+  // MULTIPEAK (R33-R36): a_pl, a_g (the high peak) and a_gl carry 1/N1
+  bool mp;
+  double a_gl, mul, sigl, dm, fidx, ctop, topb;   // topb = (mmin + dm)^(beta+1)
+  const Node64* ftab;
 };
 
 __device__ __forceinline__ void node_pair(const Node64* t, int m, double& z0, double& d0, double& z1, double& d1,
@@ -110,9 +116,39 @@ __device__ __forceinline__ double sample_v(const ThetaK& K, const NodeT* tab, in
   if (!(m1 > K.mmin && m1 <= K.mmax && m2 >= K.mmin && m2z <= m1z)) return -1.0;
   const double lm1 = log_fast(m1, logtab), lm2 = log_fast(m2 <= m1 ? m2 : m1, logtab);
   const double y = (m1 - K.mu) / K.sigma;
-  const double p1 = K.a_pl * exp_fast<true>(-K.alpha * lm1, exptab) + K.a_g * exp_fast<true>(-0.5 * y * y, exptab);
-  const double p2 = K.bp1 * exp_fast<true>(K.beta * lm2, exptab) / (exp_fast<true>(K.bp1 * lm1, exptab) - K.mminb);
-  if (!(p1 > 0.0) || !(p2 > 0.0)) return -1.0;
+  double p1 = K.a_pl * exp_fast<true>(-K.alpha * lm1, exptab) + K.a_g * exp_fast<true>(-0.5 * y * y, exptab);
+  double p2;
+  if (K.mp) {
+    // p(m1) p(m2 | m1) = [mix(m1) S(m1) / N1] [m2^beta S(m2) / C(m1)]; inside the smoothing window
+    // C(m1) = S(m1) m1^(beta+1) |F|(m1) / |beta+1| from the table (S(m1) cancels), above it elementary
+    const double yl = (m1 - K.mul) / K.sigl;
+    p1 += K.a_gl * exp_fast<true>(-0.5 * yl * yl, exptab);
+    const double m1p = m1 - K.mmin, m2p = m2 - K.mmin;
+    double S2 = 1.0;
+    if (m2p < K.dm) {
+      const double E = K.dm * fma(2.0, m2p, -K.dm) * rcp_fast(m2p * (m2p - K.dm));
+      if (!(E <= 600.0)) return -1.0;   // a smoothing factor below e^-600 is zero (R35)
+      S2 = 1.0 / (1.0 + exp_fast<true>(E, exptab));
+    }
+    const double num2 = exp_fast<true>(K.beta * lm2, exptab) * S2;
+    const double m1b = exp_fast<true>(K.bp1 * lm1, exptab);
+    if (m1p < K.dm) {
+      const double t = m1p * K.fidx;
+      int k = (int)floor(t);
+      k = k < 0 ? 0 : (k > MF_NODES - 2 ? MF_NODES - 2 : k);
+      const double f = t - (double)k;
+      const Node64 a = K.ftab[k], b = K.ftab[k + 1];
+      const double dl = b.z - a.z, sd = a.d + b.d;
+      const double c3 = fma(-2.0, dl, sd), c2 = fma(3.0, dl, -(sd + a.d));
+      const double F = fma(f, fma(f, fma(f, c3, c2), a.d), a.z);
+      p2 = num2 * fabs(K.bp1) / (m1b * F);
+    } else {
+      p2 = num2 / ((m1b - K.topb) / K.bp1 + K.ctop);
+    }
+  } else {
+    p2 = K.bp1 * exp_fast<true>(K.beta * lm2, exptab) / (exp_fast<true>(K.bp1 * lm1, exptab) - K.mminb);
+  }
+  if (!(p1 > 0.0) || !(p2 > 0.0) || !(p2 < CUDART_INF)) return -1.0;
   const double rE = rsqrt_fast(fma(K.Om * x * x, x, K.OL));
   const double J = x * x * K.cH * (u * rx + x * rE);
   z_out = z;
@@ -340,7 +376,8 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
     const int64_t ev = unit / p.n_theta, t = unit - ev * p.n_theta;   // event-major
     const int64_t s0 = p.ev_off[ev], s1 = p.ev_off[ev + 1];
     const size_t o = (size_t)t * (size_t)p.n_events + (size_t)ev;
-    const double* th = p.theta + t * GWC_NPAR;
+    const double* th = p.theta + t * (p.model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR);
+    const double* tcr = p.tconst + t * nconst_of(p.model);
     if (!(p.tvalid[t] == 1.0)) {   // theta outside the domain or changed since the build: NaN (sticky flag set)
       if (lane == 0) {
         p.logL[o] = CUDART_NAN;
@@ -356,8 +393,8 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
                    lam = th[8];
       K.h0c = H0 / C_KMS_KDE;
       K.cH = C_KMS_KDE / H0;
-      K.umax = p.tconst[t * NCONST + C_UMAX];
-      K.invdu = p.tconst[t * NCONST + C_INVDU];
+      K.umax = tcr[C_UMAX];
+      K.invdu = tcr[C_INVDU];
       K.mmin = mmin; K.mmax = mmax; K.alpha = alpha; K.beta = beta; K.mu = mu; K.sigma = sigma;
       const double n_pl = (1.0 - alpha) / (pow(mmax, 1.0 - alpha) - pow(mmin, 1.0 - alpha));
       const double rs2 = 1.0 / (sigma * 1.41421356237309504880);
@@ -368,6 +405,17 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       K.mminb = pow(mmin, beta + 1.0);
       K.Om = th[1];
       K.OL = 1.0 - th[1];
+      K.mp = p.model == 1;
+      K.a_gl = 0.0; K.mul = 0.0; K.sigl = 1.0; K.dm = 0.0; K.fidx = 0.0; K.ctop = 0.0; K.topb = K.mminb; K.ftab = nullptr;
+      if (K.mp) {
+        const double dm = th[12], laml = th[15], iN1 = 1.0 / tcr[C_N1];
+        K.a_pl *= iN1;
+        K.a_g *= (1.0 - laml) * iN1;
+        K.a_gl = lam * laml * tcr[C_NGL] / (th[14] * 2.50662827463100050242) * iN1;
+        K.mul = th[13]; K.sigl = th[14]; K.dm = dm; K.fidx = tcr[C_FIDX]; K.ctop = tcr[C_CTOP];
+        K.topb = pow(mmin + dm, beta + 1.0);
+        K.ftab = p.ftab + (size_t)t * MF_PITCH;
+      }
     }
     // prior weights at this lane's grid nodes: c_g psi(z_g) / (1 + z_g) (trapezoid weight, reading R4) split over the
     // two LOS nodes around z_g (the table's own linear interpolation, R10)
@@ -515,14 +563,14 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
 
 }  // namespace
 
-int launch_kde(const double* d_theta, const void* d_tab, const double* d_tconst, const double* d_tvalid, int64_t n_theta, int M, int Mp,
+int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const void* d_tab, const double* d_tconst, const double* d_tvalid, int64_t n_theta, int M, int Mp,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
                int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
   if (n_theta <= 0 || n_events <= 0) return 0;
   KdeParams p;
-  p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.tvalid = d_tvalid; p.n_theta = n_theta; p.n_events = n_events;
+  p.model = model; p.ftab = d_ftab; p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.tvalid = d_tvalid; p.n_theta = n_theta; p.n_events = n_events;
   p.M = M; p.Mp = Mp; p.tab_zq = tab_zq; p.ev_off = ev_off; p.dL = dL; p.m1z = m1z; p.m2z = m2z; p.lprior = lprior;
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
   p.n_grid = n_grid; p.neff_min = neff_min; p.bw_rule = bw_rule; p.logL = logL; p.npass = npass; p.nused = nused;

@@ -57,12 +57,13 @@ struct BankGuard {
 BankGuard g_bank[MAX_DEVICES];
 
 struct SmemLayout {
-  size_t math, acc, cnt, np, carry, carryn, lead, leadn, allsky, tab, total;
+  size_t math, acc, cnt, np, carry, carryn, lead, leadn, allsky, ftab, tab, total;
 };
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
-__host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z, bool pix) {
+__host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z, bool pix,
+                                                   bool mp) {
   SmemLayout L;
   size_t o = 0;
   L.math = o;   o = align16(o + sizeof(MathTables));
@@ -76,6 +77,7 @@ __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_byt
   L.lead = o;   o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 : 0));
   L.leadn = o;  o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
   L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
+  L.ftab = o;   o = align16(o + (mp ? sizeof(Node64) * (size_t)T * MF_PITCH : 0));   // MULTIPEAK: F(m1) tables
   L.tab = o;    o = align16(o + node_bytes * (size_t)T * Mp);
   L.total = o;
   return L;
@@ -103,6 +105,7 @@ __device__ __forceinline__ double node_scale(const Node32*, double z, double zq)
 template <typename LosT>
 struct Mid {
   double u, z, m1, fz;
+  double m2;   // MULTIPEAK only (unused fields vanish)
   LosT q0, q1;
   bool ok;
 };
@@ -129,7 +132,7 @@ __device__ __forceinline__ double los_load(const double* p) {
 // First half of one (theta, sample) term: u -> z by cubic Hermite on the per-theta table, source-frame masses,
 // support tests, and the loads of the two line-of-sight nodes around z.  `lrow` points at the sample's LOS row
 // (global memory) or at the all-sky table (shared memory).  No branch, no warp-synchronous operation.
-template <typename NodeT, typename LosT, bool GLOBAL>
+template <typename NodeT, typename LosT, bool GLOBAL, bool MP>
 __device__ __forceinline__ void term_head(const double* __restrict__ tc, const NodeT* __restrict__ tab, double2 A,
                                           double m2z, const LosT* __restrict__ lrow, double inv_dz, double los_zmax,
                                           double zq, int bmax, Mid<LosT>& o) {
@@ -159,33 +162,62 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
   o.q0 = los_load<GLOBAL>(lrow + b);
   o.q1 = los_load<GLOBAL>(lrow + b + 1);
   o.u = u; o.z = z; o.m1 = m1; o.ok = ok;
+  if (MP) o.m2 = m2;
 }
 
 // Second half: population, rate, Jacobian and the LOS interpolation.  C = (ln m1z, ln(m2z/m1z)),
 // P = -ln pi - ln m1z - shift.  Returns the weight relative to the segment shift (0 when dead).
-template <typename LosT>
+// MULTIPEAK (R33-R36): a second Gaussian peak in the numerator; the normaliser of p(m2 | m1) inside the
+// smoothing window from the per-theta table `ftab` of |F|(m1) = |beta+1| C(m1) / (S(m1) m1^(beta+1)) (S(m1) of p(m1)
+// cancels against the one in C), above it sign(beta+1) (1 - e1) with the window's integral folded into E1C; and
+// 1 / S(m2) = 1 + exp(dm (2 m' - dm) / (m' (m' - dm))), m' = m2 - mmin, in the denominator.
+template <typename LosT, bool MP>
 __device__ __forceinline__ double term_tail(const double* __restrict__ tc, const double2* __restrict__ logtab,
-                                            const double* __restrict__ exptab, double2 C, double P,
-                                            const Mid<LosT>& h, bool& live) {
+                                            const double* __restrict__ exptab, const Node64* __restrict__ ftab,
+                                            double2 C, double P, const Mid<LosT>& h, bool& live) {
   const double x = 1.0 + h.z;
   const double lx = log_fast(x, logtab);
   const double t1 = C.x - lx;  // ln m1
   const double c = fma(tc[C_GM1], lx, fma(tc[C_BETA], C.y, P));
   // lambda = 1 / lambda = 0: CPL / CG is -inf, the clamped exponential returns e^-700 (~1e-304, nothing)
   const double y = fma(h.m1, tc[C_INVSIG], tc[C_NMUSIG]);
-  const double num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), exptab) +
-                     exp_fast<true>(fma(-0.5 * y, y, c + tc[C_CG]), exptab);
+  double num = exp_fast<true>(fma(tc[C_NALPHA], t1, c + tc[C_CPL]), exptab) +
+               exp_fast<true>(fma(-0.5 * y, y, c + tc[C_CG]), exptab);
   const double e1 = exp_fast<false>(fma(tc[C_NBP1], t1, tc[C_E1C]), exptab);
   const double e2 = exp_fast<false>(fma(tc[C_GK], lx, tc[C_E2C]), exptab);
   const double x2 = x * x;
   const double rE = rsqrt_fast(fma(tc[C_OM] * x2, x, tc[C_OL]));
   double den = fma(x2, rE, h.u);                   // u + x^2/E
-  den *= fma(-tc[C_SGN], e1, tc[C_SGN]);           // sign(beta+1) (1 - e1)
+  double F = fma(-tc[C_SGN], e1, tc[C_SGN]);       // sign(beta+1) (1 - e1)
+  bool ok = h.ok;
+  if (MP) {
+    const double yl = fma(h.m1, tc[C_INVSIG2], tc[C_NMUSIG2]);
+    num += exp_fast<true>(fma(-0.5 * yl, yl, c + tc[C_CG2]), exptab);
+    // m1 inside the smoothing window: cubic Hermite on the table (lanes outside read a clamped interval, unused)
+    const double m1p = h.m1 - tc[C_MMIN];
+    double tm = fma(m1p, tc[C_FIDX], -0.5) + KM[K_MAGIC];
+    const int k = max(0, min(__double2loint(tm), MF_NODES - 2));
+    const double f = fma(m1p, tc[C_FIDX], -(double)k);
+    const double2* q = reinterpret_cast<const double2*>(ftab + k);
+    const double2 a = q[0], b = q[1];
+    const double dl = b.x - a.x, sd = a.y + b.y;
+    const double c3 = fma(-2.0, dl, sd), c2 = fma(3.0, dl, -(sd + a.y));
+    const double Fin = fma(f, fma(f, fma(f, c3, c2), a.y), a.x);
+    F = m1p < tc[C_DM] ? Fin : F;
+    // 1 / S(m2)
+    const double m2p = h.m2 - tc[C_MMIN];
+    const bool win2 = m2p < tc[C_DM];
+    const double E = tc[C_DM] * fma(2.0, m2p, -tc[C_DM]) * rcp_fast(m2p * (m2p - tc[C_DM]));
+    ok = ok & !(win2 & !(E <= 600.0));   // a smoothing factor below e^-600 is zero (R35); also m2 = mmin and NaN
+    const double f2 = exp_fast<true>(win2 ? E : -700.0, exptab);
+    den *= 1.0 + f2;
+  }
+  den *= F;
   den *= 1.0 + e2;
   const double q0 = widen(h.q0), q1 = widen(h.q1);
   const double plos = fma(h.fz, q1 - q0, q0);
   const double w = num * plos * rcp_fast(den);
-  const bool ok = h.ok & (plos > 0.0) & lt(w, CUDART_INF);  // also rejects NaN from a vanishing denominator
+  ok = ok & (plos > 0.0) & lt(w, CUDART_INF);  // also rejects NaN from a vanishing denominator
   live = ok;
   return ok ? w : 0.0;
 }
@@ -340,8 +372,9 @@ struct Sample {
 // ODD: a theta list that ends on an odd count takes a tail-only path instead of a discarded pipeline step (chosen by
 // the host for batches of a few theta points, the sampler's one-point-per-call pattern: 0.79 -> 0.51 ms for one
 // theta on the O5 catalogue; compiled into the batch kernel the branch costs it 1.7 %).
-template <typename NodeT, typename LosT, bool INJ, bool PIX, bool TEAMS, bool ODD>
+template <typename NodeT, typename LosT, bool INJ, bool PIX, bool TEAMS, bool ODD, bool MP>
 __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightParams p) {
+  constexpr int NC = MP ? NCONST_MP : NCONST;   // row length of the constant bank
   // ASYNC: no barrier between segments.  The sums of consecutive segments go to alternating buffers; the last warp to
   // finish a segment combines it (fixed warp order) while the others are already on the next one, and the blocks are
   // dealt round-robin across segment boundaries, so the warps' loads even out over the group.
@@ -350,7 +383,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
   typedef typename std::conditional<INJ, double, LosT>::type RowT;  // the all-sky table is f64
-  const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z, PIX);
+  const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z, PIX, MP);
   MathTables& mt = *reinterpret_cast<MathTables*>(smem + L.math);
   double* s_acc = reinterpret_cast<double*>(smem + L.acc);
   int* s_cnt = reinterpret_cast<int*>(smem + L.cnt);
@@ -363,6 +396,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   __shared__ int s_hashead[NWARPS];  // pixel-cut mode: the warp's range of the current segment contains a pixel start
   double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
   NodeT* s_tab = reinterpret_cast<NodeT*>(smem + L.tab);
+  Node64* s_ftab = reinterpret_cast<Node64*>(smem + L.ftab);
 
   const unsigned FULL = 0xffffffffu;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -396,6 +430,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       uint4* dst = reinterpret_cast<uint4*>(s_tab);
       const int n16 = (int)(((size_t)nt * Mp * sizeof(NodeT)) / 16);
       for (int i = tid; i < n16; i += NTHREADS) dst[i] = src[i];
+      if (MP) {
+        const uint4* fsrc = reinterpret_cast<const uint4*>(p.ftab + (size_t)(p.t_begin + t0) * MF_PITCH);
+        uint4* fdst = reinterpret_cast<uint4*>(s_ftab);
+        for (int i = tid; i < nt * MF_PITCH; i += NTHREADS) fdst[i] = fsrc[i];
+      }
       cur_tile = tile;
     }
     for (int i = tid; i < NWARPS * T * 2 * NBUF; i += NTHREADS) s_acc[i] = 0.0;
@@ -503,7 +542,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) dmin = fmin(dmin, __shfl_xor_sync(FULL, dmin, o));
         // theta points of the tile for which at least one sample of this warp lies inside the table
-        const double* tcl = KT + (t0 + min(lane, nt - 1)) * NCONST;
+        const double* tcl = KT + (t0 + min(lane, nt - 1)) * NC;
         unsigned todo = __ballot_sync(FULL, lane < nt && dmin * tcl[C_H] < tcl[C_UMAX]);
         if (PIX) todo = 0xffffffffu >> (32 - nt);  // every theta sees every block: open runs are carried through
         // Software pipeline over the theta points: the first half of the next point (table look-up, LOS loads)
@@ -513,7 +552,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           Mid<RowT> cur[SPT], nxt[SPT];
 #pragma unroll
           for (int k = 0; k < SPT; ++k)
-            term_head<NodeT, RowT, !INJ>(KT + (t0 + ja) * NCONST, s_tab + (size_t)ja * Mp, sm[k].A, sm[k].m2z, sm[k].lrow,
+            term_head<NodeT, RowT, !INJ, MP>(KT + (t0 + ja) * NC, s_tab + (size_t)ja * Mp, sm[k].A, sm[k].m2z, sm[k].lrow,
                                          inv_dz, los_zmax, zq, bmax, cur[k]);
           for (;;) {
             const int jb = pop_lowest(todo);
@@ -521,11 +560,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               // the list ends on an odd count: only the second half of the last point is left (warp-uniform)
               double a0 = 0.0, a1 = 0.0;
               int cnt = 0;
-              const double* tct = KT + (t0 + ja) * NCONST;
+              const double* tct = KT + (t0 + ja) * NC;
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
                 bool live;
-                const double w = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, cur[k], live);
+                const double w = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], live);
                 a0 += w;
                 a1 = fma(w, w, a1);
                 cnt += live ? 1 : 0;
@@ -542,17 +581,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
             double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
             int cnt = 0, cntb = 0, npa = 0, npb = 0;  // (cntb, npa, npb: pixel-cut mode)
             {
-              const double* tch = KT + (t0 + jh) * NCONST;
-              const double* tct = KT + (t0 + ja) * NCONST;
+              const double* tch = KT + (t0 + jh) * NC;
+              const double* tct = KT + (t0 + ja) * NC;
 #pragma unroll
               for (int k = 0; k < SPT; ++k)
-                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
+                term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, nxt[k]);
               double wv[SPT];
               bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, cur[k], lv[k]);
+                wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], lv[k]);
                 if (!PIX) {
                   a0 += wv[k];
                   a1 = fma(wv[k], wv[k], a1);
@@ -569,17 +608,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               // a branch here would let the compiler sink the loads of the first step behind it)
               const bool second = jb >= 0;
               const int jh2 = jc >= 0 ? jc : jh;
-              const double* tch = KT + (t0 + jh2) * NCONST;
-              const double* tct = KT + (t0 + jh) * NCONST;
+              const double* tch = KT + (t0 + jh2) * NC;
+              const double* tct = KT + (t0 + jh) * NC;
 #pragma unroll
               for (int k = 0; k < SPT; ++k)
-                term_head<NodeT, RowT, !INJ>(tch, s_tab + (size_t)jh2 * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
+                term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh2 * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, cur[k]);
               double wv[SPT];
               bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                wv[k] = term_tail<RowT>(tct, logtab, exptab, sm[k].C, sm[k].P, nxt[k], lv[k]);
+                wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + jh * MF_PITCH, sm[k].C, sm[k].P, nxt[k], lv[k]);
                 lv[k] = lv[k] & second;
                 wv[k] = lv[k] ? wv[k] : 0.0;
                 if (!PIX) {
@@ -743,55 +782,78 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   }
 }
 
-template <typename NodeT, typename LosT, bool INJ, bool PIX = false, bool TEAMS = false, bool ODD = false>
+template <typename NodeT, typename LosT, bool INJ, bool PIX = false, bool TEAMS = false, bool ODD = false,
+          bool MP = false>
 int launch_one(const ReweightParams& p, int n_blocks, size_t smem, cudaStream_t s) {
-  reweight_kernel<NodeT, LosT, INJ, PIX, TEAMS, ODD><<<n_blocks, NTHREADS, smem, s>>>(p);
+  reweight_kernel<NodeT, LosT, INJ, PIX, TEAMS, ODD, MP><<<n_blocks, NTHREADS, smem, s>>>(p);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-template <typename NodeT, typename LosT, bool INJ, bool PIX = false, bool TEAMS = false, bool ODD = false>
+template <typename NodeT, typename LosT, bool INJ, bool PIX = false, bool TEAMS = false, bool ODD = false,
+          bool MP = false>
 int configure_one(int smem_optin) {
-  return cudaFuncSetAttribute(reweight_kernel<NodeT, LosT, INJ, PIX, TEAMS, ODD>,
+  return cudaFuncSetAttribute(reweight_kernel<NodeT, LosT, INJ, PIX, TEAMS, ODD, MP>,
                               cudaFuncAttributeMaxDynamicSharedMemorySize,
                               smem_optin) == cudaSuccess ? 0 : -1;
 }
 
-}  // namespace
-
-size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix) {
-  return smem_layout(T, Mp, tab_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32), inj, n_z, pix).total;
+// the variants of one (NodeT, LosT) pair of event kernels; MULTIPEAK has the plain and the pixel-cut kernel
+template <typename NodeT, typename LosT>
+int configure_events(int smem_optin) {
+  int rc = 0;
+  rc |= configure_one<NodeT, LosT, false>(smem_optin);
+  rc |= configure_one<NodeT, LosT, false, true>(smem_optin);
+  rc |= configure_one<NodeT, LosT, false, false, true>(smem_optin);
+  rc |= configure_one<NodeT, LosT, false, false, false, true>(smem_optin);
+  rc |= configure_one<NodeT, LosT, false, false, false, false, true>(smem_optin);
+  rc |= configure_one<NodeT, LosT, false, true, false, false, true>(smem_optin);
+  return rc;
 }
 
-int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix) {
+template <typename NodeT, typename LosT>
+int launch_events(const ReweightParams& p, int n_blocks, size_t smem, cudaStream_t s) {
+  if (p.model == 1)
+    return p.pixcut ? launch_one<NodeT, LosT, false, true, false, false, true>(p, n_blocks, smem, s)
+                    : launch_one<NodeT, LosT, false, false, false, false, true>(p, n_blocks, smem, s);
+  if (p.pixcut) return launch_one<NodeT, LosT, false, true>(p, n_blocks, smem, s);
+  if (p.odd) return launch_one<NodeT, LosT, false, false, false, true>(p, n_blocks, smem, s);
+  if (p.teams) return launch_one<NodeT, LosT, false, false, true>(p, n_blocks, smem, s);
+  return launch_one<NodeT, LosT, false>(p, n_blocks, smem, s);
+}
+
+template <typename NodeT>
+int launch_inj(const ReweightParams& p, int n_blocks, size_t smem, cudaStream_t s) {
+  if (p.model == 1) return launch_one<NodeT, double, true, false, false, false, true>(p, n_blocks, smem, s);
+  if (p.odd) return launch_one<NodeT, double, true, false, false, true>(p, n_blocks, smem, s);
+  return launch_one<NodeT, double, true>(p, n_blocks, smem, s);
+}
+
+}  // namespace
+
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp) {
+  return smem_layout(T, Mp, tab_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32), inj, n_z, pix, mp).total;
+}
+
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp) {
   int best = 0;
   for (int T = 1; T <= MAX_T; ++T)
-    if (reweight_smem_bytes(T, Mp, tab_prec, inj, n_z, pix) + SMEM_RESERVE <= (size_t)smem_optin) best = T;
+    if (reweight_smem_bytes(T, Mp, tab_prec, inj, n_z, pix, mp) + SMEM_RESERVE <= (size_t)smem_optin) best = T;
   return best;
 }
 
 int reweight_configure(int smem_optin) {
   smem_optin -= SMEM_RESERVE;  // room for the kernel's static shared memory
   int rc = 0;
-  rc |= configure_one<Node64, double, false>(smem_optin);
-  rc |= configure_one<Node64, float, false>(smem_optin);
-  rc |= configure_one<Node32, double, false>(smem_optin);
-  rc |= configure_one<Node32, float, false>(smem_optin);
-  rc |= configure_one<Node64, double, false, true>(smem_optin);
-  rc |= configure_one<Node64, float, false, true>(smem_optin);
-  rc |= configure_one<Node32, double, false, true>(smem_optin);
-  rc |= configure_one<Node32, float, false, true>(smem_optin);
-  rc |= configure_one<Node64, double, false, false, true>(smem_optin);
-  rc |= configure_one<Node64, float, false, false, true>(smem_optin);
-  rc |= configure_one<Node32, double, false, false, true>(smem_optin);
-  rc |= configure_one<Node32, float, false, false, true>(smem_optin);
-  rc |= configure_one<Node64, double, false, false, false, true>(smem_optin);
-  rc |= configure_one<Node64, float, false, false, false, true>(smem_optin);
-  rc |= configure_one<Node32, double, false, false, false, true>(smem_optin);
-  rc |= configure_one<Node32, float, false, false, false, true>(smem_optin);
+  rc |= configure_events<Node64, double>(smem_optin);
+  rc |= configure_events<Node64, float>(smem_optin);
+  rc |= configure_events<Node32, double>(smem_optin);
+  rc |= configure_events<Node32, float>(smem_optin);
   rc |= configure_one<Node64, double, true, false, false, true>(smem_optin);
   rc |= configure_one<Node32, double, true, false, false, true>(smem_optin);
   rc |= configure_one<Node64, double, true>(smem_optin);
   rc |= configure_one<Node32, double, true>(smem_optin);
+  rc |= configure_one<Node64, double, true, false, false, false, true>(smem_optin);
+  rc |= configure_one<Node32, double, true, false, false, false, true>(smem_optin);
   return rc;
 }
 
@@ -799,8 +861,10 @@ int reweight_configure(int smem_optin) {
 // first copies its points' constants into the constant bank (stream-ordered) and resets the work counter.
 int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm, int device,
                     cudaStream_t s) {
-  const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z, p0.pixcut != 0);
-  const int cap = (KT_THETA / p0.T) * p0.T;
+  const bool mp = p0.model == 1;
+  const int nc = nconst_of(p0.model);
+  const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z, p0.pixcut != 0, mp);
+  const int cap = ((mp ? KT_THETA_MP : KT_THETA) / p0.T) * p0.T;
   int launched = 0;
   if (device < 0 || device >= MAX_DEVICES) return -1;
   BankGuard& bank = g_bank[device];
@@ -814,44 +878,19 @@ int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_pr
     const int64_t n_items = (int64_t)p.n_groups * p.n_tiles;
     const int n_blocks = (int)(n_items < n_sm ? n_items : n_sm);
     if (bank.used && bank.last_stream != s && cudaStreamWaitEvent(s, bank.last, 0) != cudaSuccess) return -1;
-    if (cudaMemcpyToSymbolAsync(KT, p0.tconst + (size_t)tb * NCONST, sizeof(double) * NCONST * (size_t)p.n_theta, 0,
+    if (cudaMemcpyToSymbolAsync(KT, p0.tconst + (size_t)tb * nc, sizeof(double) * nc * (size_t)p.n_theta, 0,
                                 cudaMemcpyDeviceToDevice, s) != cudaSuccess)
       return -1;
     if (cudaMemsetAsync(p.unit_counter, 0, sizeof(unsigned int), s) != cudaSuccess) return -1;
     int rc;
-    if (inj && p.odd) {
-      rc = tab_prec == GWC_F64 ? launch_one<Node64, double, true, false, false, true>(p, n_blocks, smem, s)
-                               : launch_one<Node32, double, true, false, false, true>(p, n_blocks, smem, s);
-    } else if (inj) {
-      rc = tab_prec == GWC_F64 ? launch_one<Node64, double, true>(p, n_blocks, smem, s)
-                               : launch_one<Node32, double, true>(p, n_blocks, smem, s);
-    } else if (p.pixcut) {
-      if (tab_prec == GWC_F64)
-        rc = los_prec == GWC_F64 ? launch_one<Node64, double, false, true>(p, n_blocks, smem, s)
-                                 : launch_one<Node64, float, false, true>(p, n_blocks, smem, s);
-      else
-        rc = los_prec == GWC_F64 ? launch_one<Node32, double, false, true>(p, n_blocks, smem, s)
-                                 : launch_one<Node32, float, false, true>(p, n_blocks, smem, s);
-    } else if (p.odd) {
-      if (tab_prec == GWC_F64)
-        rc = los_prec == GWC_F64 ? launch_one<Node64, double, false, false, false, true>(p, n_blocks, smem, s)
-                                 : launch_one<Node64, float, false, false, false, true>(p, n_blocks, smem, s);
-      else
-        rc = los_prec == GWC_F64 ? launch_one<Node32, double, false, false, false, true>(p, n_blocks, smem, s)
-                                 : launch_one<Node32, float, false, false, false, true>(p, n_blocks, smem, s);
-    } else if (p.teams) {
-      if (tab_prec == GWC_F64)
-        rc = los_prec == GWC_F64 ? launch_one<Node64, double, false, false, true>(p, n_blocks, smem, s)
-                                 : launch_one<Node64, float, false, false, true>(p, n_blocks, smem, s);
-      else
-        rc = los_prec == GWC_F64 ? launch_one<Node32, double, false, false, true>(p, n_blocks, smem, s)
-                                 : launch_one<Node32, float, false, false, true>(p, n_blocks, smem, s);
+    if (inj) {
+      rc = tab_prec == GWC_F64 ? launch_inj<Node64>(p, n_blocks, smem, s) : launch_inj<Node32>(p, n_blocks, smem, s);
     } else if (tab_prec == GWC_F64) {
-      rc = los_prec == GWC_F64 ? launch_one<Node64, double, false>(p, n_blocks, smem, s)
-                               : launch_one<Node64, float, false>(p, n_blocks, smem, s);
+      rc = los_prec == GWC_F64 ? launch_events<Node64, double>(p, n_blocks, smem, s)
+                               : launch_events<Node64, float>(p, n_blocks, smem, s);
     } else {
-      rc = los_prec == GWC_F64 ? launch_one<Node32, double, false>(p, n_blocks, smem, s)
-                               : launch_one<Node32, float, false>(p, n_blocks, smem, s);
+      rc = los_prec == GWC_F64 ? launch_events<Node32, double>(p, n_blocks, smem, s)
+                               : launch_events<Node32, float>(p, n_blocks, smem, s);
     }
     if (rc < 0) return -1;
     launched += rc;

@@ -17,12 +17,15 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgwc.so")
 
 NPAR = 12
+NPAR_MULTIPEAK = 16
+MASS_MODELS = {"plpeak": 0, "multipeak": 1}
 F64, F32 = 0, 1
 OK, ERR_INVALID_ARG, ERR_SHAPE, ERR_DOMAIN, ERR_NOT_BUILT, ERR_NOMEM, ERR_CUDA, ERR_RANGE = range(8)
 _STATUS = ["GWC_OK", "GWC_ERR_INVALID_ARG", "GWC_ERR_SHAPE", "GWC_ERR_DOMAIN", "GWC_ERR_NOT_BUILT", "GWC_ERR_NOMEM",
            "GWC_ERR_CUDA", "GWC_ERR_RANGE"]
 
-EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_launch_count", "gwc_build_cosmo",
+EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_launch_count", "gwc_set_mass_model",
+           "gwc_theta_len", "gwc_build_cosmo",
            "gwc_export_cosmo", "gwc_pack_events", "gwc_cap_pixels", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",
            "gwc_selection_logxi",
            "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_cache_catalogue", "gwc_set_timing", "gwc_get_timing",
@@ -73,6 +76,8 @@ def load():
         "gwc_check": (ci, [vp]),
         "gwc_last_error": (C.c_char_p, [vp]),
         "gwc_launch_count": (i64, [vp]),
+        "gwc_set_mass_model": (ci, [vp, ci]),
+        "gwc_theta_len": (i32, [ci]),
         "gwc_build_cosmo": (ci, [vp, vp, i64, dbl, i32, ci]),
         "gwc_export_cosmo": (ci, [vp, vp, vp, vp]),
         "gwc_pack_events": (ci, [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]),
@@ -181,6 +186,13 @@ class Context:
 
     def gwc_launch_count(self) -> int:
         return int(self._lib.gwc_launch_count(self._h))
+
+    def gwc_set_mass_model(self, model: str):
+        """"plpeak" (12-column theta rows) or "multipeak" (16 columns; include/gwc.h)."""
+        self._ck(self._lib.gwc_set_mass_model(self._h, MASS_MODELS[model]))
+
+    def gwc_theta_len(self, model: str) -> int:
+        return int(self._lib.gwc_theta_len(MASS_MODELS[model]))
 
     def gwc_build_cosmo(self, theta: torch.Tensor, z_max: float, n_nodes: int = 1025, table_prec: int = F64):
         self._ck(self._lib.gwc_build_cosmo(self._h, _ptr(theta, torch.float64), theta.shape[0], float(z_max), n_nodes,

@@ -224,6 +224,30 @@ def make_theta(spec: Spec, seed: int, device, n_theta: Optional[int] = None, str
     return th
 
 
+# Table III of the paper as a MULTIPEAK theta row (include/gwc.h: the 12 power-law+peak columns with
+# the HIGH peak in mu / sigma and lambda_g in lambda, then delta_m, mu_g,low, sigma_g,low, lambda_g,low)
+THETA_TABLE3_MULTIPEAK = (67.4, 0.315, 2.9, 1.0, 4.6, 86.3, 30.7, 6.3, 0.4, 3.3, 2.9, 2.5, 4.8, 9.7, 0.7, 0.8)
+_MP_BOX = {12: (0.5, 8.0), 13: (7.0, 12.0), 14: (0.4, 2.5), 15: (0.0, 1.0)}   # delta_m, mu_low, sigma_low, lambda_low
+
+
+def make_theta_multipeak(spec: Spec, seed: int, device, n_theta: Optional[int] = None, stream: int = 950,
+                         mmin: float = 4.6) -> torch.Tensor:
+    """A MULTIPEAK theta batch: the config's box on the first 12 columns (make_theta), Table III's values for what the
+    box leaves fixed (mmin lowered to `mmin` so that the synthetic catalogues, drawn from a population that starts at
+    5 Msun, put samples inside the smoothing window), the four extra columns uniform in _MP_BOX.  Row 0 is Table III."""
+    n = spec.n_theta if n_theta is None else n_theta
+    th = torch.tensor(THETA_TABLE3_MULTIPEAK, dtype=torch.float64, device=device).repeat(n, 1)
+    box = make_theta(spec, seed, device, n)
+    for name in spec.theta_box:
+        j = _PAR_INDEX[name]
+        th[:, j] = box[:, j]
+    th[:, 4] = mmin
+    for j, (lo, hi) in sorted(_MP_BOX.items()):
+        th[:, j] = lo + (hi - lo) * uniform(seed, stream + j, n, device)
+    th[0] = torch.tensor(THETA_TABLE3_MULTIPEAK, dtype=torch.float64, device=device)
+    return th
+
+
 def make_los(spec: Spec, seed: int, device, rows_chunk: int = 1024) -> torch.Tensor:
     """LOS table [rows][n_z] f64: Schechter-weighted Gaussian galaxies + uncatalogued volume term."""
     fid = _Fiducial(spec.z_max, device)
