@@ -75,6 +75,7 @@ def lib():
             "orc_pack_events": (i64, [i64, i64, vp, vp, vp, vp, vp, vp, vp]),
             "orc_cap_pixels": (i64, [i64, i64, i64, vp, vp, vp, i64, C.c_uint64, vp]),
             "orc_num_threads": (C.c_int, []), "orc_set_num_threads": (None, [C.c_int]),
+            "orc_biweight_midvariance": (d, [vp, i64, vp]),
             "orc_set_mass_model": (None, [C.c_int]), "orc_npar": (C.c_int, []),
             "orc_mp_smooth": (d, [d, d, d]), "orc_mp_C": (d, [d, vp]), "orc_mp_N1": (d, [vp]),
         }
@@ -232,6 +233,16 @@ def event_loglik_pixcut(theta, ev, los_table, los_z_max, neff_min, *, mode=TABLE
     return logL, neff, nlive, npass
 
 
+BW_RULES = {"scott": 0, "silverman": 1, "biweight": 2, "biweight_scott": 3}
+
+
+def biweight_midvariance(x):
+    """Eq. D3-D4 of a sample; NaN when the MAD is zero."""
+    x = _f64(x)
+    work = np.empty(2 * max(x.size, 1))
+    return lib().orc_biweight_midvariance(_p(x), x.size, _p(work))
+
+
 def _events_struct(ev):
     off = np.ascontiguousarray(ev["ev_sample_off"], dtype=np.int64)
     dl, m1, m2 = _f64(ev["dL"]), _f64(ev["m1z"]), _f64(ev["m2z"])
@@ -255,7 +266,7 @@ def event_loglik_kde(theta, ev, los_table, los_z_max, *, n_grid=256, neff_min=0.
     nused = np.empty((nt, ne), dtype=np.int64)
     zm = float(los_z_max if z_max is None else z_max)
     rc = lib().orc_event_loglik_kde(_p(th), nt, C.addressof(es), C.addressof(ls), mode, zm, n_nodes, table_prec,
-                                    int(n_grid), float(neff_min), {"scott": 0, "silverman": 1}[bandwidth], _p(logL),
+                                    int(n_grid), float(neff_min), BW_RULES[bandwidth], _p(logL),
                                     _p(npass), _p(nused))
     assert rc == 0
     if want_nused:

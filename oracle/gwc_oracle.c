@@ -751,8 +751,35 @@ static double quantile_sorted(const double* x, int64_t n, double q) {
   return x[lo] + f * (x[lo + 1] - x[lo]);
 }
 
+/* Biweight midvariance, Eq. D3-D4, of x[0..n-1]; `work` holds 2n doubles.
+ *   Q = median, MAD = median |x_i - Q|, u_i = (x_i - Q) / (9 MAD),
+ *   D3 = n sum_{|u_i|<1} (x_i - Q)^2 (1 - u_i^2)^4 / (sum_{|u_i|<1} (1 - u_i^2)(1 - 5 u_i^2))^2.
+ * Returns NaN when MAD = 0 or the denominator vanishes (no scale: the pixel has no bandwidth, reading R37). */
+double orc_biweight_midvariance(const double* x, int64_t n, double* work) {
+  if (n < 1) return NAN;
+  for (int64_t i = 0; i < n; ++i) work[i] = x[i];
+  qsort(work, (size_t)n, sizeof(double), dbl_cmp);
+  double Q = quantile_sorted(work, n, 0.5);
+  for (int64_t i = 0; i < n; ++i) work[n + i] = fabs(x[i] - Q);
+  qsort(work + n, (size_t)n, sizeof(double), dbl_cmp);
+  double mad = quantile_sorted(work + n, n, 0.5);
+  if (!(mad > 0.0)) return NAN;
+  long double num = 0.0L, den = 0.0L;
+  for (int64_t i = 0; i < n; ++i) {
+    double d = x[i] - Q, u = d / (9.0 * mad);
+    if (!(fabs(u) < 1.0)) continue;
+    double a = 1.0 - u * u;
+    num += (long double)(d * d) * (a * a) * (a * a);
+    den += (long double)a * (1.0 - 5.0 * u * u);
+  }
+  if (den == 0.0L) return NAN;
+  return (double)((long double)n * num / (den * den));
+}
+
 /* bw_rule: 0 = Scott, Eq. D1; 1 = Silverman, Eq. D2:
- * h = 0.9 min(sigma, IQR / 1.34) n^(-1/5) with the IQR of the pixel's live z_k (plain quantiles, reading R32). */
+ * h = 0.9 min(sigma, IQR / 1.34) n^(-1/5) with the IQR of the pixel's live z_k (plain quantiles, reading R32);
+ * 2 = biweight midvariance as printed, h = D3 (reading R37); 3 = the same robust scale in Scott's
+ * rule, h = 1.06 sqrt(D3) n^(-1/5) (R37).  D3 is taken over the pixel's live z_k, unweighted like the IQR. */
 int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events* ev, const orc_los* L, int mode,
                          double z_max, int M, int table_prec, int n_grid, double neff_min, int bw_rule, double* logL,
                          int64_t* npass, int64_t* nused) {
@@ -771,6 +798,8 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
     double* zz = (double*)malloc(sizeof(double) * nb);
     double* lI = (double*)malloc(sizeof(double) * nb);   /* log I_j of the passing pixels of one event */
     double* Rg = (double*)malloc(sizeof(double) * (size_t)n_grid);
+    double* wk = (double*)malloc(sizeof(double) * 3 * nb);   /* biweight: the live z_k and two sorted copies */
+    if (!wk) { free(lv); lv = NULL; }
     if (!orc_theta_valid(th) || !lv || !zz || !lI || !Rg) {
       for (int64_t i = 0; i < ev->n_events; ++i) {
         logL[t * ev->n_events + i] = NAN;
@@ -778,12 +807,12 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
         if (nused) nused[t * ev->n_events + i] = 0;
       }
       if (!lv || !zz || !lI || !Rg) err = 1;
-      free(lv); free(zz); free(lI); free(Rg);
+      free(lv); free(zz); free(lI); free(Rg); free(wk);
       continue;
     }
     orc_cosmo_tab ct;
     double* buf = NULL;
-    if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lv); free(zz); free(lI); free(Rg); continue; }
+    if (prep_cosmo(th, mode, z_max, M, &ct, &buf)) { err = 1; free(lv); free(zz); free(lI); free(Rg); free(wk); continue; }
     if (mode == 0 && table_prec == 1) orc_round_table_32(buf, M, z_max);
     for (int g = 0; g < n_grid; ++g) {            /* rate term on the grid: R(z) = psi(z) / (1+z), reading R4 */
       double zg = g * dzg;
@@ -834,6 +863,13 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
               if (iqr / 1.34 < spread) spread = iqr / 1.34;
               h = 0.9 * spread * pow((double)n, -0.2);
               if (!(h > 0.0)) { r0 = r1; continue; }                          /* IQR = 0: no bandwidth, no contribution */
+            } else if (bw_rule == 2 || bw_rule == 3) {                        /* Eq. D3-D4 */
+              int64_t c = 0;
+              for (int64_t k = r0; k < r1; ++k)
+                if (lv[k - a] > -INFINITY) wk[c++] = zz[k - a];
+              double zeta2 = orc_biweight_midvariance(wk, c, wk + c);
+              h = bw_rule == 2 ? zeta2 : 1.06 * sqrt(zeta2) * pow((double)n, -0.2);
+              if (!(h > 0.0) || !isfinite(h)) { r0 = r1; continue; }          /* no scale: no contribution */
             }
             double norm = 1.0 / (h * sqrt(2.0 * M_PI));
             long double I = 0.0L;
@@ -862,7 +898,7 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
       if (nused) nused[t * ev->n_events + i] = nu;
     }
     free(buf);
-    free(lv); free(zz); free(lI); free(Rg);
+    free(lv); free(zz); free(lI); free(Rg); free(wk);
   }
   return err;
 }

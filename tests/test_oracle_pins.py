@@ -983,3 +983,73 @@ def test_mp_theta_domain():
         assert O.theta_valid(_th_mp())
         for bad in (dict(dm=-0.1), dict(dm=90.0), dict(sigl=0.0), dict(laml=1.2), dict(laml=-0.1)):
             assert not O.theta_valid(_th_mp(**bad)), bad
+
+
+# ---------------------------------------------------------------- biweight midvariance bandwidth (Eq. D3-D4)
+def _biweight_numpy(x):
+    """Eq. D3-D4 with numpy's median for Q and the MAD."""
+    Q = np.median(x)
+    mad = np.median(np.abs(x - Q))
+    u = (x - Q) / (9 * mad)
+    I = np.abs(u) < 1
+    return x.size * np.sum(((x - Q) ** 2 * (1 - u ** 2) ** 4)[I]) / np.sum(((1 - u ** 2) * (1 - 5 * u ** 2))[I]) ** 2
+
+
+def test_biweight_midvariance_properties():
+    """What the statistic is known for (ref. [54]): on a large normal sample it equals the variance; a few
+    gross outliers ("more than nine MADs from the centre": zero weight) leave it alone while they wreck the sample
+    variance; it is shift-invariant and scales with the square; a sample with MAD = 0 has no scale."""
+    rng = np.random.default_rng(3)
+    x = 0.4 + 0.05 * rng.standard_normal(40000)
+    z2 = O.biweight_midvariance(x)
+    assert z2 == pytest.approx(0.05 ** 2, rel=0.02)
+    assert z2 == pytest.approx(_biweight_numpy(x), rel=1e-12)
+    xo = np.concatenate([x, 0.4 + 0.05 * 60 * np.ones(400)])          # 1 % of points at 60 sigma
+    assert np.var(xo) > 30 * 0.05 ** 2
+    assert O.biweight_midvariance(xo) == pytest.approx(z2, rel=0.03)
+    assert O.biweight_midvariance(3.0 * x - 7.0) == pytest.approx(9.0 * z2, rel=1e-11)
+    assert O.biweight_midvariance(rng.permutation(x)) == pytest.approx(z2, rel=1e-13)
+    # small samples, even and odd counts: numpy's median conventions
+    for n in (2, 3, 4, 7, 10):
+        y = rng.standard_normal(n)
+        assert O.biweight_midvariance(y) == pytest.approx(_biweight_numpy(y), rel=1e-12), n
+    assert math.isnan(O.biweight_midvariance(np.array([1.0, 1.0, 1.0, 2.0])))    # MAD = 0
+    # the indicator: a point beyond 9 MAD contributes nothing, wherever it is
+    y = np.array([-1.0, -0.5, 0.0, 0.5, 1.0, 50.0])
+    y2 = y.copy()
+    y2[-1] = 500.0
+    assert O.biweight_midvariance(y) == O.biweight_midvariance(y2)
+
+
+@pytest.mark.parametrize("rule", ["biweight_scott", "biweight"])
+def test_kde_biweight_bandwidth_through_quadratic_prior(theta0, rule):
+    """The z^2 prior exposes h of every pixel (as for Scott and Silverman): rule 3 is 1.06 sqrt(D3) n^(-1/5), rule 2 is
+    D3 itself, the formula as the paper prints it (reading R37).  The toy's redshifts spread widely so that even
+    h = D3 (a variance) is resolved by the 256-node grid; outliers make D3 differ from the plain variance."""
+    ev = _kde_event(n=260, seed=4, rows=5)
+    rng = np.random.default_rng(6)
+    if rule == "biweight":
+        ev["dL"] = ev["dL"] * np.exp(0.3 * rng.standard_normal(260))
+    far = rng.choice(260, 10, replace=False)
+    ev["dL"][far] *= 1.8 if rule == "biweight" else 1.6
+    zmax, nz = 3.0, 8192
+    zb = np.linspace(0, zmax, nz)
+    tab = np.tile(zb ** 2, (5, 1))
+    th = _theta_unit_rate(theta0)
+    z, lv = O.kde_samples(th, ev, 5, zmax)
+    Lk, npass = O.event_loglik_kde(th, ev, tab, zmax, n_grid=1024, bandwidth=rule)
+    Ls, _ = O.event_loglik_kde(th, ev, tab, zmax, n_grid=1024, bandwidth="scott")
+    off = ev["ev_sample_off"]
+    for i, runs in enumerate(_pixel_runs(ev)):
+        tot = 0.0
+        for r0, r1 in runs:
+            live = np.isfinite(lv[r0:r1])
+            v, zz = np.exp(lv[r0:r1][live]), z[r0:r1][live]
+            z2 = _biweight_numpy(zz)
+            h = z2 if rule == "biweight" else 1.06 * math.sqrt(z2) * zz.size ** (-0.2)
+            assert h > 2 * zmax / 1023 and zz.min() - 5.5 * h > 0 and zz.max() + 5.5 * h < zmax, (h, zz.min())
+            tot += np.sum(v * (zz ** 2 + h * h))
+        assert npass[0, i] == len(runs)
+        want = math.log(tot / (off[i + 1] - off[i]))
+        assert Lk[0, i] == pytest.approx(want, abs=2e-6)
+        assert abs(Ls[0, i] - Lk[0, i]) > 1e-4            # and it is not Scott's bandwidth
