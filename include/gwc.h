@@ -81,8 +81,10 @@ typedef enum {
 #define GWC_MAX_NZ_SELECTION 4096 /* largest los->n_z of the selection term (the all-sky table sits in shared memory) */
 
 typedef enum { GWC_F64 = 0, GWC_F32 = 1 } gwc_prec;
-/* bandwidth rule of the KDE numerator: Scott, Eq. D1 (the paper's default) | Silverman, Eq. D2 (:300) */
-typedef enum { GWC_BW_SCOTT = 0, GWC_BW_SILVERMAN = 1 } gwc_bw_rule;
+/* bandwidth rule of the KDE numerator: Scott, Eq. D1 (the paper's default) | Silverman, Eq. D2 (:300) |
+ * the biweight midvariance of Eq. D3-D4 (:303-309) taken as printed, h = D3 | the same robust scale in Scott's rule,
+ * h = 1.06 sqrt(D3) n^(-1/5) (R37).  D3 and the IQR are over the pixel's live redshifts, unweighted. */
+typedef enum { GWC_BW_SCOTT = 0, GWC_BW_SILVERMAN = 1, GWC_BW_BIWEIGHT = 2, GWC_BW_BIWEIGHT_SCOTT = 3 } gwc_bw_rule;
 
 /* Mass model (App. A; Table III, :263-274).  GWC_MASS_PLPEAK: truncated power law + one Gaussian peak,
  * conditional power law in m2 (R2, R3).  GWC_MASS_MULTIPEAK: power law + two Gaussian peaks, the primary

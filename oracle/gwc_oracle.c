@@ -879,7 +879,9 @@ int orc_event_loglik_kde(const double* theta, int64_t n_theta, const orc_events*
               for (int64_t k = r0; k < r1; ++k) {
                 if (lv[k - a] == -INFINITY) continue;
                 double q = (zg - zz[k - a]) / h;
-                f += exp(lv[k - a] - m) * norm * exp(-0.5 * q * q);
+                double g2 = 0.5 * q * q;
+                if (g2 > 700.0) continue;      /* a kernel value below e^-700 is zero (reading R38) */
+                f += exp(lv[k - a] - m) * norm * exp(-g2);
               }
               double zl = zg < L->z_max ? zg : L->z_max;                     /* last node: the table's last value */
               double prior = orc_los_lerp(L, row, zl) * Rg[g];

@@ -520,7 +520,7 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   if (!ev || !d_logL) return fail(ctx, GWC_ERR_INVALID_ARG, "ev or d_logL is NULL");
   if (!(neff_min >= 0.0)) return fail(ctx, GWC_ERR_INVALID_ARG, "neff_min must be >= 0");
   if (n_grid < 2 || n_grid > 256) return fail(ctx, GWC_ERR_SHAPE, "n_grid must be in [2, 256]");
-  if (bw_rule != GWC_BW_SCOTT && bw_rule != GWC_BW_SILVERMAN) return fail(ctx, GWC_ERR_INVALID_ARG, "unknown bw_rule");
+  if (bw_rule < GWC_BW_SCOTT || bw_rule > GWC_BW_BIWEIGHT_SCOTT) return fail(ctx, GWC_ERR_INVALID_ARG, "unknown bw_rule");
   GWC_TRY(check_los(ctx, los, true, false));
   if (ev->n_events < 0 || ev->n_samples < 0 || ev->n_events > 0x7fffffffLL)
     return fail(ctx, GWC_ERR_SHAPE, "event / sample counts out of range");

@@ -15,7 +15,7 @@
 // for which the lanes turn into grid nodes (node g = lane + 32 i, i < 8): the (z_k, v_k) of 32 samples at a time are handed round by
 // shuffles and every lane adds v_k N(z_g; z_k, h) into its 8 node sums.  The prior p_los R c_g at the lane's nodes is
 // then applied once per pixel.  Everything is FP64; the Gaussian uses math64.cuh's 7-instruction exp (the hot
-// instruction: G exponentials per (theta, sample)), the per-sample weight plain libdevice functions.  All sums run in
+// instruction), the per-sample weight the same exp / ln / rcp / rsqrt as the fused kernel.  All sums run in
 // a fixed order (samples in order inside a lane, butterfly across lanes, pixels in order): bitwise reproducible.
 #include <math_constants.h>
 
@@ -52,7 +52,7 @@ struct KdeParams {
   double los_zmax;
   int n_grid;
   double neff_min;
-  int bw_rule;              // 0 = Scott (Eq. D1), 1 = Silverman (Eq. D2)
+  int bw_rule;              // gwc_bw_rule: Scott (D1), Silverman (D2), biweight as printed (D3), biweight in Scott's rule
   double2* scr;             // [resident warps][scr_stride]: (z_k, v_k) of the event a warp is working on (v < 0: dead)
   int64_t scr_stride;       // >= the longest event
   double* logL;             // [n_theta][n_events]
@@ -156,10 +156,20 @@ __device__ __forceinline__ double sample_v(const ThetaK& K, const NodeT* tab, in
   return v >= 0.0 ? v : -1.0;   // (NaN from a degenerate theta: dead)
 }
 
-// ---- order statistics of a pixel's live redshifts (Silverman's rule, Eq. D2) --------------------------------------
-// k-th smallest (0-based) of the live z of scr[r0..r1): bisection on the bit pattern (positive doubles order like
-// their bits), one counting pass per bit; exact, every lane returns the same value.
-__device__ double kth_live_z(const double2* scr, int64_t r0, int64_t r1, int64_t k, int lane) {
+// ---- order statistics of a pixel's live redshifts (Silverman's rule, Eq. D2; biweight midvariance, Eq. D3-D4) -------
+// The value a sample enters the selection with: its redshift, or its absolute deviation from a centre (for the MAD).
+struct KeyZ {
+  __device__ __forceinline__ double operator()(double z) const { return z; }
+};
+struct KeyAbsDev {
+  double centre;
+  __device__ __forceinline__ double operator()(double z) const { return fabs(z - centre); }
+};
+
+// k-th smallest (0-based) key of the live samples of scr[r0..r1): bisection on the bit pattern (non-negative doubles
+// order like their bits), one counting pass per bit; exact, every lane returns the same value.
+template <typename Key>
+__device__ double kth_live(const double2* scr, int64_t r0, int64_t r1, int64_t k, Key key, int lane) {
   unsigned long long prefix = 0;
   for (int bit = 62; bit >= 0; --bit) {
     const unsigned long long cand = prefix | (1ull << bit);
@@ -168,7 +178,7 @@ __device__ double kth_live_z(const double2* scr, int64_t r0, int64_t r1, int64_t
       const int64_t i = c0 + lane;
       if (i < r1) {
         const double2 zv = scr[i];
-        cnt += (zv.y >= 0.0 && (unsigned long long)__double_as_longlong(zv.x) < cand) ? 1 : 0;
+        cnt += (zv.y >= 0.0 && (unsigned long long)__double_as_longlong(key(zv.x)) < cand) ? 1 : 0;
       }
     }
     cnt = __reduce_add_sync(0xffffffffu, cnt);
@@ -177,8 +187,9 @@ __device__ double kth_live_z(const double2* scr, int64_t r0, int64_t r1, int64_t
   return __longlong_as_double((long long)prefix);
 }
 
-// the order statistic after x = the k-th one: x again when it is repeated, else the smallest live z above it
-__device__ double next_live_z(const double2* scr, int64_t r0, int64_t r1, int64_t k, double x, int lane) {
+// the order statistic after x = the k-th one: x again when it is repeated, else the smallest live key above it
+template <typename Key>
+__device__ double next_live(const double2* scr, int64_t r0, int64_t r1, int64_t k, double x, Key key, int lane) {
   int le = 0;
   double up = CUDART_INF;
   for (int64_t c0 = r0; c0 < r1; c0 += 32) {
@@ -186,8 +197,9 @@ __device__ double next_live_z(const double2* scr, int64_t r0, int64_t r1, int64_
     if (i < r1) {
       const double2 zv = scr[i];
       if (zv.y >= 0.0) {
-        le += zv.x <= x ? 1 : 0;
-        up = zv.x > x ? fmin(up, zv.x) : up;
+        const double v = key(zv.x);
+        le += v <= x ? 1 : 0;
+        up = v > x ? fmin(up, v) : up;
       }
     }
   }
@@ -197,15 +209,43 @@ __device__ double next_live_z(const double2* scr, int64_t r0, int64_t r1, int64_
   return (int64_t)le >= k + 2 ? x : up;
 }
 
-// q-quantile of the n live z by linear interpolation between the order statistics at q (n - 1)
-__device__ double live_quantile(const double2* scr, int64_t r0, int64_t r1, int64_t n, double q, int lane) {
+// q-quantile of the n live keys by linear interpolation between the order statistics at q (n - 1)
+template <typename Key>
+__device__ double live_quantile(const double2* scr, int64_t r0, int64_t r1, int64_t n, double q, Key key, int lane) {
   const double pos = q * (double)(n - 1);
   const int64_t lo = (int64_t)floor(pos);
-  if (lo >= n - 1) return kth_live_z(scr, r0, r1, n - 1, lane);
+  if (lo >= n - 1) return kth_live(scr, r0, r1, n - 1, key, lane);
   const double f = pos - (double)lo;
-  const double x0 = kth_live_z(scr, r0, r1, lo, lane);
-  const double x1 = next_live_z(scr, r0, r1, lo, x0, lane);
-  return x0 + f * (x1 - x0);
+  const double x0 = kth_live(scr, r0, r1, lo, key, lane);
+  const double x1 = next_live(scr, r0, r1, lo, x0, key, lane);
+  return __dadd_rn(x0, __dmul_rn(f, x1 - x0));   // (no contraction: the same bits as the plain statement)
+}
+
+// Biweight midvariance of the n live redshifts of a pixel, Eq. D3-D4 (R37); NaN when the
+// MAD or the denominator is zero.
+__device__ double live_biweight(const double2* scr, int64_t r0, int64_t r1, int64_t n, int lane) {
+  const double Q = live_quantile(scr, r0, r1, n, 0.5, KeyZ(), lane);
+  KeyAbsDev dev;
+  dev.centre = Q;
+  const double mad = live_quantile(scr, r0, r1, n, 0.5, dev, lane);
+  if (!(mad > 0.0)) return CUDART_NAN;
+  const double s9 = 9.0 * mad;
+  double num = 0.0, den = 0.0;
+  for (int64_t c0 = r0; c0 < r1; c0 += 32) {
+    const int64_t i = c0 + lane;
+    if (i < r1) {
+      const double2 zv = scr[i];
+      const double d = zv.x - Q, u = d / s9;
+      if (zv.y >= 0.0 && fabs(u) < 1.0) {
+        const double a = 1.0 - u * u, a2 = a * a;
+        num += d * d * a2 * a2;
+        den += a * (1.0 - 5.0 * u * u);
+      }
+    }
+  }
+  num = wsum(num);
+  den = wsum(den);
+  return den != 0.0 ? (double)n * num / (den * den) : CUDART_NAN;
 }
 
 // Grid node i (< KDE_NPL) of a lane in the prior stage: half-warp lane l16 = lane & 15 owns the 16 consecutive nodes
@@ -327,7 +367,8 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
 #pragma unroll
         for (int i = 0; i < KDE_NPL; ++i) {
           const double q = fma((double)kde_node(lane, i), beta, -zj);
-          mine[i] = fma(aj, exp_fast<true>(-q * q, exptab), mine[i]);
+          const double g2 = q * q;   // a kernel value below e^-700 is zero (R38)
+          mine[i] = fma(g2 > 700.0 ? 0.0 : aj, exp_fast<true>(-g2, exptab), mine[i]);
         }
       }
     }
@@ -538,10 +579,15 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         const int64_t r1 = c0 + tl + 1, r0 = r1 - len_p;
         if (p.bw_rule == 1) {                            // Eq. D2
           const double sd_p = __shfl_sync(FULL, sd, tl);
-          const double iqr = live_quantile(scr, r0, r1, n_p, 0.75, lane) - live_quantile(scr, r0, r1, n_p, 0.25, lane);
+          const double iqr = live_quantile(scr, r0, r1, n_p, 0.75, KeyZ(), lane) -
+                             live_quantile(scr, r0, r1, n_p, 0.25, KeyZ(), lane);
           const double spread = iqr / 1.34 < sd_p ? iqr / 1.34 : sd_p;
           h_p = 0.9 * spread * pow((double)n_p, -0.2);
           if (!(h_p > 0.0)) continue;
+        } else if (p.bw_rule >= 2) {                     // Eq. D3-D4: as printed (2) or inside Scott's rule (3)
+          const double zeta2 = live_biweight(scr, r0, r1, n_p, lane);
+          h_p = p.bw_rule == 2 ? zeta2 : 1.06 * sqrt(zeta2) * pow((double)n_p, -0.2);
+          if (!(h_p > 0.0) || !isfinite(h_p)) continue;
         }
         const double part = kde_pixel<LosT>(scr, r0, r1, h_p, prow, p, dzg, s_w, s_b, exptab, lane);
         if (__any_sync(FULL, part > 0.0)) {

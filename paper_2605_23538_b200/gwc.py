@@ -32,7 +32,7 @@ EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_laun
            "gwc_probe_fp64", "gwc_math_selftest"]
 
 
-BW_RULES = {"scott": 0, "silverman": 1}
+BW_RULES = {"scott": 0, "silverman": 1, "biweight": 2, "biweight_scott": 3}
 
 
 class GwcError(RuntimeError):

@@ -167,7 +167,7 @@ def test_multipeak_kde(ctx):
     zmax = W.spec.z_max
     thd, ev, lo = th.to(DEV), to_dev(W.ev, DEV), W.los.to(DEV)
     ctx.gwc_build_cosmo(thd, zmax)
-    for bw in ("scott", "silverman"):
+    for bw in ("scott", "silverman", "biweight_scott"):
         gL, gP, gU = ctx.gwc_event_loglik_kde(thd, ev, lo, zmax, 128, 2.0, bw)
         ctx.gwc_check()
         with oracle.mass_model("multipeak"):

@@ -555,7 +555,34 @@ def test_kde_silverman_bandwidth(ctx):
     th = Wt.theta.to(DEV)
     ctx.gwc_build_cosmo(th, Wt.spec.z_max, 1025, 0)
     with pytest.raises(KeyError):
-        ctx.gwc_event_loglik_kde(th, to_dev(Wt.ev, DEV), Wt.los.to(DEV), Wt.spec.z_max, 256, 0.0, "biweight")
+        ctx.gwc_event_loglik_kde(th, to_dev(Wt.ev, DEV), Wt.los.to(DEV), Wt.spec.z_max, 256, 0.0, "epanechnikov")
+
+
+@pytest.mark.parametrize("rule", ["biweight", "biweight_scott"])
+def test_kde_biweight_bandwidth(ctx, rule):
+    """Eq. D3-D4 on the GPU (R37): median and MAD by exact selection on the live redshifts and on their
+    absolute deviations, then the two sums; rule "biweight" takes h = D3 as printed (narrow kernels: the direct
+    path of the KDE pass), "biweight_scott" puts sqrt(D3) into Scott's rule.  Pixels of 2 samples to hundreds,
+    duplicated redshifts (MAD = 0: no bandwidth) included."""
+    W = workload("o4", n_theta=12, n_events=8, los_rows=400, n_inj=500)
+    ev = dict(W.ev)
+    dl = ev["dL"].clone()
+    dl[40:52] = dl[40]            # a run of identical samples inside one event
+    ev["dL"] = dl
+    ev["m1z"] = ev["m1z"].clone()
+    ev["m1z"][40:52] = ev["m1z"][40]
+    ev["m2z"] = ev["m2z"].clone()
+    ev["m2z"][40:52] = ev["m2z"][40]
+    for nmin in (0.0, 2.0):
+        g, o = _kde_both(ctx, W, W.theta, ev=ev, neff_min=nmin, bandwidth=rule)
+        _kde_compare(g, o, "%s nmin=%g" % (rule, nmin))
+        assert (o[1] > 0).any()
+    gs, _ = _kde_both(ctx, W, W.theta, ev=ev, neff_min=0.0, bandwidth="scott")
+    fin = np.isfinite(g[0]) & np.isfinite(gs[0])
+    assert fin.any() and np.abs(g[0][fin] - gs[0][fin]).max() > 1e-3
+    Wt = workload("tiny")
+    g, o = _kde_both(ctx, Wt, Wt.theta, neff_min=2.0, bandwidth=rule)
+    _kde_compare(g, o, rule + " tiny")
 
 
 def test_catalogue_cache_and_small_batches(ctx):
