@@ -108,6 +108,9 @@ gwc_status ensure(gwc_ctx* ctx, Buf& b, size_t bytes) {
     return cuda_fail(ctx, e, "cudaMalloc");
   }
   b.cap = want;
+#ifdef GWC_CHECKED
+  cudaMemsetAsync(b.p, 0xff, want, ctx->stream);   // poison (NaN / -1): a read of scratch never written shows in the results
+#endif
   return GWC_OK;
 }
 
@@ -243,6 +246,8 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.teams = (!mp && !inj && !pixcut && !p.odd && n_seg > 0 && n / n_seg < 2048) ? 1 : 0;
   p.neff_min = neff_min;
   p.unit_counter = ctx->d_counter;
+  p.flag = ctx->d_flag;
+  p.n_samples = n;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (ctx->timing) {
     e0 = get_event(ctx);
@@ -339,6 +344,12 @@ gwc_status gwc_check(gwc_ctx* ctx) {
   GWC_CUDA(cudaMemcpy(&flag, ctx->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
   if (flag) {
     GWC_CUDA(cudaMemset(ctx->d_flag, 0, sizeof(int)));
+    if (flag & FLAG_CHK_ANY) {
+      char msg[160];
+      snprintf(msg, sizeof(msg), "GWC_CHECKED: a device-side bounds / hand-off check failed (flag bits 0x%x, see gwc_internal.h)",
+               flag & FLAG_CHK_ANY);
+      return fail(ctx, GWC_ERR_CUDA, msg);
+    }
     if (flag & FLAG_STALE)
       return fail(ctx, GWC_ERR_NOT_BUILT,
                   "d_theta changed after gwc_build_cosmo: the outputs of the changed points are NaN (rebuild first)");
@@ -555,7 +566,7 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
                                 ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->prep[0].seg_shift.p,
                                 los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, bw_rule,
                                 d_logL,
-                                d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, s),
+                                d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, ctx->d_flag, s),
                 "kde");
   if (ctx->timing) {
     cudaEventRecord(e1, s);

@@ -105,6 +105,8 @@ struct ReweightParams {
   int pixcut;               // 1: per-pixel effective-sample cut (Eq. 8), threshold neff_min
   double neff_min;
   unsigned int* unit_counter;
+  int* flag;                // sticky device flag word (written by -DGWC_CHECKED builds only)
+  int64_t n_samples;        // length of the sample arrays (checked builds)
 };
 
 // kernels / launchers (each returns the number of kernels it launched, or -1 on a launch error)
@@ -112,8 +114,29 @@ struct ReweightParams {
 enum : int {
   FLAG_DOMAIN = 1,   // a theta point outside the model's domain (gwc_build_cosmo)
   FLAG_STALE = 4,    // d_theta differs from the copy taken by gwc_build_cosmo
-  FLAG_RANGE = 8     // every live weight of a segment lies below e^-300 of the segment's reference
+  FLAG_RANGE = 8,    // every live weight of a segment lies below e^-300 of the segment's reference
+  // -DGWC_CHECKED builds only (tests/sanitizer_cases.py): a device-side check failed
+  FLAG_CHK_TABLE = 1 << 8,     // index into a z(u) table outside [0, Mp - 2]
+  FLAG_CHK_LOS = 1 << 9,       // LOS node index outside [0, n_z - 2], or a row outside the table
+  FLAG_CHK_SAMPLE = 1 << 10,   // sample index outside [0, n_samples)
+  FLAG_CHK_ACC = 1 << 11,      // accumulator slot outside the warp's own (warp, theta) range
+  FLAG_CHK_HANDOFF = 1 << 12,  // barrier-free segment hand-off: a sum buffer reused before it was combined and cleared,
+                               // a wrong arrival count, or segments combined out of order
+  FLAG_CHK_MATH = 1 << 13,     // exp / log table index out of range
+  FLAG_CHK_FTAB = 1 << 14,     // MULTIPEAK F-table index outside [0, MF_NODES - 2]
+  FLAG_CHK_KDE = 1 << 15,      // KDE kernel: scratch slot outside the warp's slice, grid node or LOS bin out of range
+  FLAG_CHK_ANY = 0xff << 8
 };
+#ifdef GWC_CHECKED
+#define GWC_DEV_CHECK(flagp, cond, bit)              \
+  do {                                               \
+    if (!(cond)) atomicOr((flagp), (int)(bit));      \
+  } while (0)
+#else
+#define GWC_DEV_CHECK(flagp, cond, bit) \
+  do {                                  \
+  } while (0)
+#endif
 // smallest linear-domain segment sum (relative to the segment's reference) that is still trusted: below it the
 // clamped exponentials (e^-700) and the squares of the weights lose their meaning (R23)
 constexpr double RANGE_MIN_SUM = 5.148200222412013e-131;   // e^-300
@@ -158,7 +181,8 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
-               int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s);
+               int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks,
+               int* d_flag, cudaStream_t s);
 int kde_grid_blocks(int64_t n_theta, int64_t n_events, int n_sm);
 size_t kde_scratch_bytes(int n_blocks, int64_t max_event_len);
 int launch_max_segment(const int64_t* seg_off, int64_t n_seg, int64_t* d_out, cudaStream_t s);

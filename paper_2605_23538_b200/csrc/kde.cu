@@ -58,6 +58,7 @@ struct KdeParams {
   double* logL;             // [n_theta][n_events]
   int64_t* npass;           // [n_theta][n_events] or NULL
   int64_t* nused;           // [n_theta][n_events] or NULL: live samples of the contributing pixels
+  int* flag;                // sticky device flag word (written by -DGWC_CHECKED builds only)
 };
 
 __device__ __forceinline__ double wsum(double v) {
@@ -379,6 +380,7 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
   for (int i = 0; i < KDE_NPL; ++i) {
     const NodeW w = s_w[i * 32 + lane];
     const int b = s_b[i * 32 + lane];
+    GWC_DEV_CHECK(p.flag, b >= 0 && b <= p.n_z - 2 && prow >= 0 && (int64_t)prow < p.n_rows, FLAG_CHK_KDE);
     part = fma(mine[i], fma((double)lrow[b + 1], w.w1, (double)lrow[b] * w.w0), part);
   }
   return part;
@@ -491,6 +493,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
                                        : (isfinite(lp) ? exp_fast<true>(-lp - shift, exptab) : CUDART_NAN);
         const double v = sample_v(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], scale, p.row[k], p.n_rows, p.los_zmax,
                                   logtab, exptab, z);
+        GWC_DEV_CHECK(p.flag, k - s0 >= 0 && k - s0 < p.scr_stride, FLAG_CHK_KDE);
         scr[k] = make_double2(z, v);
       }
     }
@@ -613,9 +616,11 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
-               int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks, cudaStream_t s) {
+               int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks,
+               int* d_flag, cudaStream_t s) {
   if (n_theta <= 0 || n_events <= 0) return 0;
   KdeParams p;
+  p.flag = d_flag;
   p.model = model; p.ftab = d_ftab; p.theta = d_theta; p.tab = d_tab; p.tconst = d_tconst; p.tvalid = d_tvalid; p.n_theta = n_theta; p.n_events = n_events;
   p.M = M; p.Mp = Mp; p.tab_zq = tab_zq; p.ev_off = ev_off; p.dL = dL; p.m1z = m1z; p.m2z = m2z; p.lprior = lprior;
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;

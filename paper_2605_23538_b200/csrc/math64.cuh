@@ -6,7 +6,8 @@
 // shared-memory and integer pipes.  Polynomial coefficients live in constant memory so that the
 // FP64 instructions read them as c[bank][offset] operands (a 64-bit literal would cost two register
 // moves per use).  Accuracy (tests/test_gpu_parity.py::test_math_functions, against torch's fp64):
-// relative error <= ~4e-16 for rcp/rsqrt, <= ~3e-15 for exp, absolute <= ~4e-16 for log on [1, 2^k).
+// relative error <= ~4e-16 for rcp/rsqrt, <= 1.6e-13 for exp (cubic on a 256-entry table), absolute <= 1.8e-13 for log
+// (quartic on a 128-entry table): the accuracy budget of DESIGN.md section 5, 5000 times inside the 1e-9 parity bar.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

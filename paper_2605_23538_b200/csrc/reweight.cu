@@ -135,7 +135,7 @@ __device__ __forceinline__ double los_load(const double* p) {
 template <typename NodeT, typename LosT, bool GLOBAL, bool MP>
 __device__ __forceinline__ void term_head(const double* __restrict__ tc, const NodeT* __restrict__ tab, double2 A,
                                           double m2z, const LosT* __restrict__ lrow, double inv_dz, double los_zmax,
-                                          double zq, int bmax, Mid<LosT>& o) {
+                                          double zq, int bmax, Mid<LosT>& o, int* chk, int Mp) {
   const double u0 = A.x * tc[C_H];
   bool ok = u0 < tc[C_UMAX];  // false for NaN (samples marked dead by the preparation kernel)
   const double u = ok ? u0 : 0.0;
@@ -145,6 +145,7 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
   tm -= KM[K_MAGIC];
   const double f = fma(u, tc[C_INVDU], -tm);
   double z0, d0, z1, d1;
+  GWC_DEV_CHECK(chk, m >= 0 && m <= Mp - 2, FLAG_CHK_TABLE);
   load_nodes(tab, m, z0, d0, z1, d1);
   const double dl = z1 - z0;
   const double sd = d0 + d1;
@@ -159,6 +160,7 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
   const int b = min(__double2loint(tb), bmax);
   tb -= KM[K_MAGIC];
   o.fz = fma(z, inv_dz, -tb);
+  GWC_DEV_CHECK(chk, b >= 0 && b <= bmax, FLAG_CHK_LOS);
   o.q0 = los_load<GLOBAL>(lrow + b);
   o.q1 = los_load<GLOBAL>(lrow + b + 1);
   o.u = u; o.z = z; o.m1 = m1; o.ok = ok;
@@ -174,7 +176,7 @@ __device__ __forceinline__ void term_head(const double* __restrict__ tc, const N
 template <typename LosT, bool MP>
 __device__ __forceinline__ double term_tail(const double* __restrict__ tc, const double2* __restrict__ logtab,
                                             const double* __restrict__ exptab, const Node64* __restrict__ ftab,
-                                            double2 C, double P, const Mid<LosT>& h, bool& live) {
+                                            double2 C, double P, const Mid<LosT>& h, bool& live, int* chk) {
   const double x = 1.0 + h.z;
   const double lx = log_fast(x, logtab);
   const double t1 = C.x - lx;  // ln m1
@@ -198,6 +200,7 @@ __device__ __forceinline__ double term_tail(const double* __restrict__ tc, const
     double tm = fma(m1p, tc[C_FIDX], -0.5) + KM[K_MAGIC];
     const int k = max(0, min(__double2loint(tm), MF_NODES - 2));
     const double f = fma(m1p, tc[C_FIDX], -(double)k);
+    GWC_DEV_CHECK(chk, k >= 0 && k <= MF_NODES - 2, FLAG_CHK_FTAB);
     const double2* q = reinterpret_cast<const double2*>(ftab + k);
     const double2 a = q[0], b = q[1];
     const double dl = b.x - a.x, sd = a.y + b.y;
@@ -491,6 +494,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         }
         __threadfence_block();  // the cleared buffer is seen after the release
       }
+#ifdef GWC_CHECKED
+      if (ASYNC && lane < nt) {   // this warp's slots of the buffer must be clear before it adds to them
+        GWC_DEV_CHECK(p.flag, *(volatile double*)&acc_b[(warp * T + lane) * 2] == 0.0 &&
+                                  *(volatile double*)&acc_b[(warp * T + lane) * 2 + 1] == 0.0 &&
+                                  *(volatile int*)&cnt_b[warp * T + lane] == 0,
+                      FLAG_CHK_HANDOFF);
+      }
+#endif
       // The segment's samples in blocks of BLK, dealt to the warps round-robin; no barrier until the segment ends.
       // Pixel-cut mode: each warp takes one contiguous range of whole blocks instead, so that the run a block
       // leaves open is continued by the same warp's next block; the pixels that cross from one warp's range
@@ -526,6 +537,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         for (int k = 0; k < SPT; ++k) {
           const int64_t g = PIX ? c0 + SPT * lane + k : c0 + k * 32 + lane;
           const bool in = g < w_hi;  // slots past the end are dead
+          GWC_DEV_CHECK(p.flag, !in || (g >= 0 && g < p.n_samples), FLAG_CHK_SAMPLE);
           sm[k].A = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
           sm[k].m2z = in ? p.m2z[g] : 1.0;
           sm[k].C = make_double2(in ? p.L1[g] : 0.0, in ? p.Q[g] : 0.0);
@@ -535,6 +547,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           } else {
             int32_t r = in ? p.row[g] : 0;
             r = ((unsigned)r < (unsigned)p.n_rows) ? r : 0;  // out-of-range rows are dead (dLc = NaN)
+            GWC_DEV_CHECK(p.flag, r >= 0 && (int64_t)r < p.n_rows, FLAG_CHK_LOS);
             sm[k].lrow = reinterpret_cast<const RowT*>(p.los) + (size_t)r * (size_t)p.n_z;
           }
           dmin = fmin(dmin, sm[k].A.x);  // fmin drops the NaN of dead samples
@@ -553,7 +566,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
 #pragma unroll
           for (int k = 0; k < SPT; ++k)
             term_head<NodeT, RowT, !INJ, MP>(KT + (t0 + ja) * NC, s_tab + (size_t)ja * Mp, sm[k].A, sm[k].m2z, sm[k].lrow,
-                                         inv_dz, los_zmax, zq, bmax, cur[k]);
+                                         inv_dz, los_zmax, zq, bmax, cur[k], p.flag, Mp);
           for (;;) {
             const int jb = pop_lowest(todo);
             if (ODD && jb < 0) {
@@ -564,7 +577,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
                 bool live;
-                const double w = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], live);
+                const double w = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], live, p.flag);
                 a0 += w;
                 a1 = fma(w, w, a1);
                 cnt += live ? 1 : 0;
@@ -586,12 +599,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
 #pragma unroll
               for (int k = 0; k < SPT; ++k)
                 term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
-                                             los_zmax, zq, bmax, nxt[k]);
+                                             los_zmax, zq, bmax, nxt[k], p.flag, Mp);
               double wv[SPT];
               bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], lv[k]);
+                wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], lv[k], p.flag);
                 if (!PIX) {
                   a0 += wv[k];
                   a1 = fma(wv[k], wv[k], a1);
@@ -613,12 +626,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
 #pragma unroll
               for (int k = 0; k < SPT; ++k)
                 term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh2 * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
-                                             los_zmax, zq, bmax, cur[k]);
+                                             los_zmax, zq, bmax, cur[k], p.flag, Mp);
               double wv[SPT];
               bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + jh * MF_PITCH, sm[k].C, sm[k].P, nxt[k], lv[k]);
+                wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + jh * MF_PITCH, sm[k].C, sm[k].P, nxt[k], lv[k], p.flag);
                 lv[k] = lv[k] & second;
                 wv[k] = lv[k] ? wv[k] : 0.0;
                 if (!PIX) {
@@ -641,6 +654,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               if ((lane & 7) == 0) {
                 const int j = (lane & 16) ? jb : ja;
                 if (j >= 0) {
+                  GWC_DEV_CHECK(p.flag, j < nt, FLAG_CHK_ACC);
                   acc_b[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
                   if ((lane & 8) == 0) {
                     cnt_b[warp * T + j] += (lane & 16) ? cntb : cnt;
@@ -658,6 +672,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               if ((lane & 7) == 0) {
                 const int j = (lane & 16) ? jb : ja;
                 if (j >= 0) {
+                  GWC_DEV_CHECK(p.flag, j < nt, FLAG_CHK_ACC);
                   acc_b[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
                   if ((lane & 8) == 0) cnt_b[warp * T + j] += (lane & 16) ? (cnt >> 16) : (cnt & 0xffff);
                 }
@@ -693,6 +708,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         last = __shfl_sync(FULL, last, 0);
         if (last) {  // every warp has arrived: this one combines the segment, in warp order, and clears the buffer
           __threadfence_block();
+          GWC_DEV_CHECK(p.flag, *(volatile int*)&s_arrive[buf] == NWARPS && *(volatile int*)&s_done == sidx,
+                        FLAG_CHK_HANDOFF);
           if (lane < nt) {
             double a = 0.0, b = 0.0;
             int c = 0;

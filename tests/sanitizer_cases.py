@@ -1,14 +1,19 @@
 """Small-case driver for every kernel variant of the library ("Race detection"): the tiny config
 and ragged mini-catalogues, each result checked against the oracle.  compute-sanitizer is closed on the GPU pool this
-repo is measured on, so the evidence asked of memcheck / racecheck is gathered the other way:
-the library built with -DGWC_CHECKED (device-side bounds checks on every table / row / accumulator index and the
-invariants of the barrier-free segment hand-off; a violation raises GWC_ERR_CUDA through gwc_check) runs these cases,
+repo is measured on (its refusal is kept in profiles/r02_sanitizer.md), so the evidence asked of
+memcheck / racecheck / initcheck is gathered the other way: the library built with -DGWC_CHECKED (device-side bounds
+checks on every table / row / sample / accumulator index, the invariants of the barrier-free segment hand-off -- a sum
+buffer must be clear when a warp starts adding to it, the arrival count must be NWARPS and segments must be combined in
+order -- and scratch memory poisoned with 0xff on allocation; a violation raises GWC_ERR_CUDA through gwc_check) runs
+these cases,
 
     GWC_NVCC_FLAGS=-DGWC_CHECKED python -m paper_2605_23538_b200.build --force && python tests/sanitizer_cases.py
 
 Not collected by pytest (no test_ prefix).  Cases: events (plain kernel, barrier-free segment hand-off), teams (short
 segments share the CTA), odd (tail-only last step), pix (per-pixel N_eff cut), inj (selection term), t32 (32-bit
-tables, f32 LOS rows), kde (every bandwidth rule), pack (A0 + cap + all-sky), host (gwc_total_loglik_host).
+tables, f32 LOS rows), kde (every bandwidth rule), pack (A0 + cap + all-sky), host (gwc_total_loglik_host), mp (the
+MULTIPEAK variants of the fused kernel and of the KDE kernel), repeat (the plain and the TEAMS kernel 20 times over:
+bit-identical results, the check a race would fail).
 """
 from __future__ import annotations
 
@@ -146,8 +151,49 @@ def case_host(ctx):
     assert_close_log(a.numpy(), o, RTOL_F64, "host call")
 
 
+def case_mp(ctx):
+    ctx.gwc_set_mass_model("multipeak")
+    try:
+        W = _ragged(9, True)
+        th = synth.make_theta_multipeak(W.spec, synth.DEFAULT_SEED, "cpu", 9)
+        ev = dict(W.ev)
+        ev["m1z"], ev["m2z"] = ev["m1z"] * 0.2, ev["m2z"] * 0.2   # into the smoothing window
+        zmax = W.spec.z_max
+        thd, evd, lo = th.to(DEV), to_dev(ev, DEV), W.los.to(DEV)
+        ctx.gwc_build_cosmo(thd, zmax, 1025, 0)
+        gL, _, gK = ctx.gwc_event_loglik(thd, evd, lo, zmax)
+        qL, _, qK, qP = ctx.gwc_event_loglik_pixcut(thd, evd, lo, zmax, 2.0)
+        kL, kP, kU = ctx.gwc_event_loglik_kde(thd, evd, lo, zmax, 64, 2.0, "scott")
+        ctx.gwc_check()
+        with oracle.mass_model("multipeak"):
+            oL, _, oK = oracle.event_loglik(_np(th), synth.to_numpy(ev), _np(W.los), zmax)
+            pL, _, pK, pP = oracle.event_loglik_pixcut(_np(th), synth.to_numpy(ev), _np(W.los), zmax, 2.0)
+            rL, rP = oracle.event_loglik_kde(_np(th), synth.to_numpy(ev), _np(W.los), zmax, n_grid=64, neff_min=2.0)
+        assert np.array_equal(_np(gK), oK) and np.array_equal(_np(qP), pP) and np.array_equal(_np(kP), rP)
+        assert_close_log(_np(gL), oL, RTOL_F64, "MULTIPEAK events")
+        assert_close_log(_np(qL), pL, RTOL_F64, "MULTIPEAK pixcut")
+        assert_close_log(_np(kL), rL, RTOL_F64, "MULTIPEAK KDE")
+    finally:
+        ctx.gwc_set_mass_model("plpeak")
+
+
+def case_repeat(ctx):
+    for W in (_ragged(12, True), _ragged(12, False)):
+        zmax = W.spec.z_max
+        th, ev, lo = W.theta.to(DEV), to_dev(W.ev, DEV), W.los.to(DEV)
+        ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+        first = None
+        for _ in range(20):
+            logL, neff, nlive = ctx.gwc_event_loglik(th, ev, lo, zmax)
+            ctx.gwc_check()
+            got = (logL.clone(), neff.clone(), nlive.clone())
+            if first is None:
+                first = got
+            assert all(torch.equal(a.view(torch.int64), b.view(torch.int64)) for a, b in zip(first, got))
+
+
 CASES = {"events": case_events, "teams": case_teams, "odd": case_odd, "pix": case_pix, "inj": case_inj,
-         "t32": case_t32, "kde": case_kde, "pack": case_pack, "host": case_host}
+         "t32": case_t32, "kde": case_kde, "pack": case_pack, "host": case_host, "mp": case_mp, "repeat": case_repeat}
 
 
 def main(argv):
