@@ -32,6 +32,14 @@ struct PrepSet {
   bool valid = false;
 };
 
+// Pixel-aligned padded copy of a prepared sample set (pixel-cut mode; pack.cu): every pixel starts at an even position
+// and has an even length.  Valid as long as the PrepSet it was made from is.
+struct PadSet {
+  Buf dLc, m1z, m2z, L1, Q, P, row, seg_off, seg_pads;
+  int64_t n_pad = 0;
+  bool valid = false;
+};
+
 struct gwc_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
@@ -57,6 +65,7 @@ struct gwc_ctx {
   HostCopy hc;
   // theta-independent preparation of the events [0] and the injections [1] (kept between calls when caching is on)
   PrepSet prep[2];
+  PadSet pad;               // of prep[0]
   bool cache_prep = false;
   // timing
   bool timing = false;
@@ -164,6 +173,7 @@ gwc_status prepare_samples(gwc_ctx* ctx, PrepSet& ps, int64_t n, int64_t n_seg, 
       ps.k_row == row && ps.k_off == d_seg_off && ps.k_n == n && ps.k_nseg == n_seg && ps.k_nrows == n_rows)
     return GWC_OK;
   ps.valid = false;
+  if (&ps == &ctx->prep[0]) ctx->pad.valid = false;
   const size_t nd = (size_t)(n > 0 ? n : 1) * sizeof(double);
   GWC_TRY(ensure(ctx, ps.dLc, nd));
   GWC_TRY(ensure(ctx, ps.L1, nd));
@@ -180,6 +190,39 @@ gwc_status prepare_samples(gwc_ctx* ctx, PrepSet& ps, int64_t n, int64_t n_seg, 
   return GWC_OK;
 }
 
+// pixel-cut mode: the pixel-aligned padded copy of the prepared events (one host synchronisation for its length)
+gwc_status prepare_padded(gwc_ctx* ctx, const PrepSet& ps, int64_t n, int64_t n_seg, const int64_t* d_seg_off,
+                          const double* m1z, const double* m2z, const int32_t* row) {
+  PadSet& pd = ctx->pad;
+  if (ctx->cache_prep && pd.valid) return GWC_OK;
+  pd.valid = false;
+  cudaStream_t s = ctx->stream;
+  GWC_TRY(ensure(ctx, pd.seg_off, (size_t)(n_seg + 1) * sizeof(int64_t)));
+  GWC_TRY(ensure(ctx, pd.seg_pads, (size_t)(n_seg > 0 ? n_seg : 1) * sizeof(int64_t)));
+  GWC_TRY(count(ctx, launch_pixpad_count(d_seg_off, n_seg, row, (int64_t*)pd.seg_pads.p, (int64_t*)pd.seg_off.p, s),
+                "pixpad_count"));
+  int64_t n_pad = 0;
+  GWC_CUDA(cudaMemcpyAsync(&n_pad, (const int64_t*)pd.seg_off.p + n_seg, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+  GWC_CUDA(cudaStreamSynchronize(s));
+  if (n_pad < n || n_pad > 2 * n) return fail(ctx, GWC_ERR_SHAPE, "ev_sample_off is not ascending from 0 to n_samples");
+  const size_t nd = (size_t)(n_pad > 0 ? n_pad : 1) * sizeof(double);
+  GWC_TRY(ensure(ctx, pd.dLc, nd));
+  GWC_TRY(ensure(ctx, pd.m1z, nd));
+  GWC_TRY(ensure(ctx, pd.m2z, nd));
+  GWC_TRY(ensure(ctx, pd.L1, nd));
+  GWC_TRY(ensure(ctx, pd.Q, nd));
+  GWC_TRY(ensure(ctx, pd.P, nd));
+  GWC_TRY(ensure(ctx, pd.row, (size_t)(n_pad > 0 ? n_pad : 1) * sizeof(int32_t)));
+  GWC_TRY(count(ctx, launch_pixpad_scatter(d_seg_off, n_seg, (const int64_t*)pd.seg_off.p, (const double*)ps.dLc.p, m1z,
+                                           m2z, (const double*)ps.L1.p, (const double*)ps.Q.p, (const double*)ps.P.p,
+                                           row, (double*)pd.dLc.p, (double*)pd.m1z.p, (double*)pd.m2z.p,
+                                           (double*)pd.L1.p, (double*)pd.Q.p, (double*)pd.P.p, (int32_t*)pd.row.p, s),
+                "pixpad_scatter"));
+  pd.n_pad = n_pad;
+  pd.valid = true;
+  return GWC_OK;
+}
+
 // shared launch sequence of A3 (events) and A5 (injections): prep -> groups -> fused kernel
 gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg, const int64_t* d_seg_off,
                         const double* dL, const double* m1z, const double* m2z, const double* lprior,
@@ -188,6 +231,18 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   cudaStream_t s = ctx->stream;
   PrepSet& ps = ctx->prep[inj ? 1 : 0];
   GWC_TRY(prepare_samples(ctx, ps, n, n_seg, d_seg_off, dL, m1z, m2z, lprior, row, n_rows));
+  // what the fused kernel reads: the prepared arrays, or in pixel-cut mode their pixel-aligned padded copy
+  const double *k_dLc = (const double*)ps.dLc.p, *k_m1z = m1z, *k_m2z = m2z, *k_L1 = (const double*)ps.L1.p,
+               *k_Q = (const double*)ps.Q.p, *k_P = (const double*)ps.P.p;
+  if (pixcut) {
+    GWC_TRY(prepare_padded(ctx, ps, n, n_seg, d_seg_off, m1z, m2z, row));
+    const PadSet& pd = ctx->pad;
+    k_dLc = (const double*)pd.dLc.p; k_m1z = (const double*)pd.m1z.p; k_m2z = (const double*)pd.m2z.p;
+    k_L1 = (const double*)pd.L1.p; k_Q = (const double*)pd.Q.p; k_P = (const double*)pd.P.p;
+    row = (const int32_t*)pd.row.p;
+    d_seg_off = (const int64_t*)pd.seg_off.p;
+    n = pd.n_pad;
+  }
   GWC_TRY(ensure(ctx, ctx->part_w, (size_t)n_theta * n_seg * 2 * sizeof(double)));
   GWC_TRY(ensure(ctx, ctx->part_n, (size_t)n_theta * n_seg * sizeof(int32_t)));
   if (pixcut) GWC_TRY(ensure(ctx, ctx->part_np, (size_t)n_theta * n_seg * sizeof(int32_t)));
@@ -196,8 +251,14 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut, mp);
   if (T < 1) return fail(ctx, GWC_ERR_SHAPE, "n_nodes / n_z too large for shared memory");
   if ((int64_t)T > n_theta) T = (int)n_theta;
-  const int n_tiles = (int)((n_theta + T - 1) / T);
+  int n_tiles = (int)((n_theta + T - 1) / T);
   T = (int)((n_theta + n_tiles - 1) / n_tiles);
+  // the kernel takes the theta points of a tile two at a time: an odd tile pays for one point more than it holds
+  if (T > 2 && (T & 1) && n_theta > T) {
+    const int Tmax = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut, mp);
+    T = T + 1 <= Tmax ? T + 1 : T - 1;
+    n_tiles = (int)((n_theta + T - 1) / T);
+  }
   // segment groups: enough work items to balance the SMs, small enough that a group's LOS rows stay in L2
   int64_t target = (int64_t)((double)n * n_tiles / ((double)ctx->n_sm * 16.0));
   if (target > 65536) target = 65536;
@@ -218,12 +279,12 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.Mp = ctx->Mp;
   p.T = T;
   p.n_tiles = n_tiles;
-  p.dLc = (const double*)ps.dLc.p;
-  p.m1z = m1z;
-  p.m2z = m2z;
-  p.L1 = (const double*)ps.L1.p;
-  p.Q = (const double*)ps.Q.p;
-  p.P = (const double*)ps.P.p;
+  p.dLc = k_dLc;
+  p.m1z = k_m1z;
+  p.m2z = k_m2z;
+  p.L1 = k_L1;
+  p.Q = k_Q;
+  p.P = k_P;
   p.row = row;
   p.seg_off = d_seg_off;
   p.group_off = (const int32_t*)ctx->group_off.p;
@@ -324,6 +385,8 @@ void gwc_destroy(gwc_ctx* ctx) {
   Buf* bufs[] = {&ctx->ftab, &ctx->tab, &ctx->tconst, &ctx->theta_snap, &ctx->tvalid, &ctx->seg_off, &ctx->prep[0].dLc, &ctx->prep[0].L1, &ctx->prep[0].Q,
                  &ctx->prep[0].P, &ctx->prep[0].seg_shift, &ctx->prep[1].dLc, &ctx->prep[1].L1, &ctx->prep[1].Q,
                  &ctx->prep[1].P, &ctx->prep[1].seg_shift,
+                 &ctx->pad.dLc, &ctx->pad.m1z, &ctx->pad.m2z, &ctx->pad.L1, &ctx->pad.Q, &ctx->pad.P, &ctx->pad.row,
+                 &ctx->pad.seg_off, &ctx->pad.seg_pads,
                  &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->kde_scr, &ctx->kde_len, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
                  &ctx->logxi, &ctx->probe, &ctx->hc.theta, &ctx->hc.ev_off, &ctx->hc.ev_dL, &ctx->hc.ev_m1z,
                  &ctx->hc.ev_m2z, &ctx->hc.ev_lp, &ctx->hc.ev_row, &ctx->hc.inj_dL, &ctx->hc.inj_m1z,
@@ -713,6 +776,7 @@ gwc_status gwc_total_loglik_host(gwc_ctx* ctx, const double* h_theta, int64_t n_
   // (gwc_cache_catalogue) must not match them
   ctx->prep[0].valid = false;
   ctx->prep[1].valid = false;
+  ctx->pad.valid = false;
   const gwc_status st_run = gwc_total_loglik(ctx, (const double*)h.theta.p, n_theta, &ev, &inj, &los, n_nodes,
                                              table_prec, (double*)h.out.p);
   ctx->prep[0].valid = false;
@@ -731,6 +795,7 @@ gwc_status gwc_cache_catalogue(gwc_ctx* ctx, int on) {
   ctx->cache_prep = on != 0;
   ctx->prep[0].valid = false;
   ctx->prep[1].valid = false;
+  ctx->pad.valid = false;
   return GWC_OK;
 }
 

@@ -195,6 +195,15 @@ int launch_pack(int64_t n_samples, int64_t n_events, const int32_t* d_event_id, 
                 int64_t* d_ev_sample_off, int64_t* d_ev_pix_off, int32_t* d_ev_pix_rows, int64_t* d_pix_sample_off,
                 int64_t* d_n_pixrefs, int* d_flag, void* scratch, size_t scratch_bytes, cudaStream_t s);
 
+// pixel-aligned padded copy of the prepared samples (pixel-cut mode): pads per segment and the padded offsets, then
+// the scatter; seg_off_pad [n_seg + 1], seg_pads [n_seg]
+int launch_pixpad_count(const int64_t* d_seg_off, int64_t n_seg, const int32_t* d_row, int64_t* d_seg_pads,
+                        int64_t* d_seg_off_pad, cudaStream_t s);
+int launch_pixpad_scatter(const int64_t* d_seg_off, int64_t n_seg, const int64_t* d_seg_off_pad, const double* dLc,
+                          const double* m1z, const double* m2z, const double* L1, const double* Q, const double* P,
+                          const int32_t* row, double* o_dLc, double* o_m1z, double* o_m2z, double* o_L1, double* o_Q,
+                          double* o_P, int32_t* o_row, cudaStream_t s);
+
 size_t cap_scratch_bytes(int64_t n_samples);
 int launch_cap_pixels(int64_t n, int64_t n_events, int64_t n_pix, const int64_t* d_perm_in, int64_t* d_ev_sample_off,
                       int64_t* d_pix_sample_off, int64_t cap, uint64_t seed, int64_t* d_perm_out, int64_t* d_n_kept,

@@ -4,8 +4,10 @@
 // then event offsets, the distinct rows of each event and the start of each (event, row) run.
 // The sort itself is the CUB library radix sort (a library primitive on a one-time, non-hot step);
 // everything else is plain kernels.
+#include <cub/block/block_scan.cuh>
 #include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
+#include <math_constants.h>
 
 #include "gwc_internal.h"
 
@@ -227,6 +229,135 @@ int launch_cap_pixels(int64_t n, int64_t n_events, int64_t n_pix, const int64_t*
   cap_offsets_kernel<<<(unsigned)((n_events + 1 + 255) / 256), 256, 0, s>>>(n, n_events, d_ev_sample_off, newpos, d_n_kept);
   cap_offsets_kernel<<<(unsigned)((n_pix + 1 + 255) / 256), 256, 0, s>>>(n, n_pix, d_pix_sample_off, newpos, d_n_kept);
   return cudaGetLastError() == cudaSuccess ? 14 : -1;  // 5 kernels + the library's radix and scan passes (approximate)
+}
+
+}  // namespace gwc
+
+// ---- pixel-aligned layout of the prepared samples (pixel-cut mode of the fused kernel) ---------------------------------
+// The fused kernel's lanes own two consecutive samples.  In the copy made here every pixel (a maximal run of equal
+// sample_row inside a segment, R25) starts at an even position and has an even length: a run of odd length
+// is followed by one dead slot (dLc = NaN, same row).  Then a lane never straddles two pixels, which is what makes
+// the per-(theta, pixel) sums of Eq. 8 a plain segmented scan over lanes (reweight.cu).  theta-independent: built
+// once per catalogue call (kept between calls with gwc_cache_catalogue).  One CTA per segment walks its samples in
+// order, 256 at a time: run start of every sample by a max-scan of the head positions, pad flag at odd-length tails,
+// running count of pads = the sample's shift.
+namespace gwc {
+namespace {
+
+constexpr int PAD_THREADS = 256;
+struct PadSrc {
+  const double *dLc, *m1z, *m2z, *L1, *Q, *P;
+  const int32_t* row;
+};
+struct PadDst {
+  double *dLc, *m1z, *m2z, *L1, *Q, *P;
+  int32_t* row;
+};
+
+template <bool SCATTER>
+__global__ void __launch_bounds__(PAD_THREADS) pixpad_kernel(const int64_t* __restrict__ seg_off,
+                                                              const int32_t* __restrict__ row,
+                                                              int64_t* __restrict__ seg_pads,          // !SCATTER: out
+                                                              const int64_t* __restrict__ seg_off_pad,  // SCATTER: in
+                                                              PadSrc src, PadDst dst) {
+  typedef cub::BlockScan<long long, PAD_THREADS> Scan;
+  __shared__ typename Scan::TempStorage tmp;
+  __shared__ long long s_head, s_pads;
+  const int seg = blockIdx.x, tid = threadIdx.x;
+  const int64_t s0 = seg_off[seg], s1 = seg_off[seg + 1];
+  if (tid == 0) {
+    s_head = s0;
+    s_pads = 0;
+  }
+  __syncthreads();
+  const int64_t base_out = SCATTER ? seg_off_pad[seg] : 0;
+  for (int64_t base = s0; base < s1; base += PAD_THREADS) {
+    const int64_t k = base + tid;
+    const bool in = k < s1;
+    const int32_t r = in ? row[k] : 0;
+    const bool head = in && (k == s0 || row[k - 1] != r);
+    const bool tail = in && (k + 1 == s1 || row[k + 1] != r);
+    long long start;   // first sample of the run that holds k
+    Scan(tmp).InclusiveScan(head ? (long long)k : -1LL, start, cub::Max());
+    __syncthreads();
+    const long long carry_head = s_head, carry_pads = s_pads;
+    start = start > carry_head ? start : carry_head;
+    const bool pad = tail && (((k - start) & 1) == 0);   // odd length
+    long long shift, total;
+    Scan(tmp).ExclusiveSum(pad ? 1LL : 0LL, shift, total);
+    __syncthreads();
+    if (SCATTER && in) {
+      const int64_t o = base_out + (k - s0) + carry_pads + shift;
+      dst.dLc[o] = src.dLc[k];
+      dst.m1z[o] = src.m1z[k];
+      dst.m2z[o] = src.m2z[k];
+      dst.L1[o] = src.L1[k];
+      dst.Q[o] = src.Q[k];
+      dst.P[o] = src.P[k];
+      dst.row[o] = r;
+      if (pad) {
+        dst.dLc[o + 1] = CUDART_NAN;
+        dst.m1z[o + 1] = 1.0;
+        dst.m2z[o + 1] = 1.0;
+        dst.L1[o + 1] = 0.0;
+        dst.Q[o + 1] = 0.0;
+        dst.P[o + 1] = 0.0;
+        dst.row[o + 1] = r;
+      }
+    }
+    if (tid == PAD_THREADS - 1) {   // (slots past the end repeat the last run start)
+      s_head = start;
+      s_pads = carry_pads + total;
+    }
+    __syncthreads();
+  }
+  if (!SCATTER && tid == 0) seg_pads[seg] = s_pads;
+}
+
+// seg_off_pad[i] = seg_off[i] + pads of the segments before i (single CTA, in order)
+__global__ void __launch_bounds__(PAD_THREADS) pixpad_offsets_kernel(const int64_t* __restrict__ seg_off,
+                                                                      const int64_t* __restrict__ seg_pads,
+                                                                      int64_t n_seg, int64_t* __restrict__ seg_off_pad) {
+  typedef cub::BlockScan<long long, PAD_THREADS> Scan;
+  __shared__ typename Scan::TempStorage tmp;
+  __shared__ long long s_carry;
+  const int tid = threadIdx.x;
+  if (tid == 0) s_carry = 0;
+  __syncthreads();
+  for (int64_t base = 0; base <= n_seg; base += PAD_THREADS) {
+    const int64_t i = base + tid;
+    long long excl, total;
+    Scan(tmp).ExclusiveSum(i < n_seg ? (long long)seg_pads[i] : 0LL, excl, total);
+    __syncthreads();
+    const long long carry = s_carry;
+    if (i <= n_seg) seg_off_pad[i] = seg_off[i] + carry + excl;
+    __syncthreads();
+    if (tid == 0) s_carry = carry + total;
+    __syncthreads();
+  }
+}
+
+}  // namespace
+
+int launch_pixpad_count(const int64_t* d_seg_off, int64_t n_seg, const int32_t* d_row, int64_t* d_seg_pads,
+                        int64_t* d_seg_off_pad, cudaStream_t s) {
+  if (n_seg <= 0) return 0;
+  PadSrc src = {};
+  PadDst dst = {};
+  pixpad_kernel<false><<<(unsigned)n_seg, PAD_THREADS, 0, s>>>(d_seg_off, d_row, d_seg_pads, nullptr, src, dst);
+  pixpad_offsets_kernel<<<1, PAD_THREADS, 0, s>>>(d_seg_off, d_seg_pads, n_seg, d_seg_off_pad);
+  return cudaGetLastError() == cudaSuccess ? 2 : -1;
+}
+
+int launch_pixpad_scatter(const int64_t* d_seg_off, int64_t n_seg, const int64_t* d_seg_off_pad, const double* dLc,
+                          const double* m1z, const double* m2z, const double* L1, const double* Q, const double* P,
+                          const int32_t* row, double* o_dLc, double* o_m1z, double* o_m2z, double* o_L1, double* o_Q,
+                          double* o_P, int32_t* o_row, cudaStream_t s) {
+  if (n_seg <= 0) return 0;
+  PadSrc src = {dLc, m1z, m2z, L1, Q, P, row};
+  PadDst dst = {o_dLc, o_m1z, o_m2z, o_L1, o_Q, o_P, o_row};
+  pixpad_kernel<true><<<(unsigned)n_seg, PAD_THREADS, 0, s>>>(d_seg_off, row, nullptr, d_seg_off_pad, src, dst);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
 }  // namespace gwc

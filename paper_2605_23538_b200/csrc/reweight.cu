@@ -67,15 +67,15 @@ __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_byt
   SmemLayout L;
   size_t o = 0;
   L.math = o;   o = align16(o + sizeof(MathTables));
-  // (two sets of sums unless pixel-cut mode: a warp may start the next segment while the slowest finish this one)
-  L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2 * (pix ? 1 : 2));
-  L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T * (pix ? 1 : 2));
+  // (two sets of everything: a warp may start the next segment while the slowest finish this one)
+  L.acc = o;    o = align16(o + sizeof(double) * NWARPS * T * 2 * 2);
+  L.cnt = o;    o = align16(o + sizeof(int) * NWARPS * T * 2);
   // pixel-cut mode only: passing pixels; the run a block leaves open (W, Q, n); the run open at the range start
-  L.np = o;     o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
-  L.carry = o;  o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 : 0));
-  L.carryn = o; o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
-  L.lead = o;   o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 : 0));
-  L.leadn = o;  o = align16(o + (pix ? sizeof(int) * NWARPS * T : 0));
+  L.np = o;     o = align16(o + (pix ? sizeof(int) * NWARPS * T * 2 : 0));
+  L.carry = o;  o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 * 2 : 0));
+  L.carryn = o; o = align16(o + (pix ? sizeof(int) * NWARPS * T * 2 : 0));
+  L.lead = o;   o = align16(o + (pix ? sizeof(double) * NWARPS * T * 2 * 2 : 0));
+  L.leadn = o;  o = align16(o + (pix ? sizeof(int) * NWARPS * T * 2 : 0));
   L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
   L.ftab = o;   o = align16(o + (mp ? sizeof(Node64) * (size_t)T * MF_PITCH : 0));   // MULTIPEAK: F(m1) tables
   L.tab = o;    o = align16(o + node_bytes * (size_t)T * Mp);
@@ -251,114 +251,110 @@ __device__ __forceinline__ int pop_lowest(unsigned& mask) {
 }
 
 // ---- per-pixel effective-sample cut (Eq. 8; R25) -------------------------------------
-// A pixel is a maximal run of consecutive samples of the segment with the same sample_row.  In pixel-cut mode a lane
-// owns the SPT = 2 CONSECUTIVE positions 2 lane, 2 lane + 1 of the warp's block, so that one segmented scan over the
-// 32 lanes serves the 64 samples.  PixShape is the run structure of the block (the same for every theta).
+// A pixel is a maximal run of consecutive samples of the segment with the same sample_row.  Pixel-cut mode works on
+// the pixel-aligned copy of the samples (pack.cu: every run starts at an even position and has an even length, odd
+// runs end on a dead slot) and a lane owns the SPT = 2 CONSECUTIVE positions 2 lane, 2 lane + 1 of the warp's block:
+// a lane belongs to exactly one run, and the per-(theta, pixel) sums are one segmented scan over the 32 lanes.
+// PixShape is the run structure of the block (the same for every theta).
 struct PixShape {
-  bool h1;              // position 1 starts a run
-  bool cont0;           // position 0 continues the run of the previous lane (or of the previous block)
-  bool t0, t1;          // last sample of its run
-  bool left0, left1;    // the run of position k began before the block
-  bool lead0, lead1;    // ... before this warp's range of the segment
-  int reach;            // lanes back to the nearest lane (this one included) that holds a run start, else to lane 0
+  bool tail;            // the lane's run ends on this lane
+  bool lead;            // ... and it began before this warp's range of the segment: the segment-end stitch decides
+  bool left;            // the lane's run began before the block
+  int reach;            // lanes back to the first lane of the run inside the block
   int nsteps;           // scan steps the block needs (warp-uniform)
-  unsigned m0a, m1a;    // lanes whose position 0 / position 1 lies in the run of position 0, up to it (live counts)
-  unsigned m0b, m1b;    // ... in the run of position 1
-  bool last_open;       // the block's last position is inside a run that continues in the next block
+  unsigned runm;        // lanes of the run up to this one (live counts)
+  bool blk_left;        // lane 0's run is open to the left: the carry of the previous block enters (warp-uniform)
+  bool last_open;       // lane 31's run continues in the next block (warp-uniform)
+  bool interior;        // the whole block lies inside one run that began earlier and goes on (warp-uniform)
+  bool has_head;        // a run starts in the block (warp-uniform)
 };
 
-__device__ __forceinline__ void pix_shape(PixShape& ps, bool in0, bool in1, bool head0, bool head1, bool tail0,
-                                          bool tail1, bool lead_open, int lane) {
+__device__ __forceinline__ void pix_shape(PixShape& ps, bool in, bool head, bool tail, bool lead_open, int lane) {
   const unsigned FULL = 0xffffffffu;
-  const unsigned hall = __ballot_sync(FULL, head0 | head1), h1all = __ballot_sync(FULL, head1);
-  const unsigned lt = (1u << lane) - 1u;
-  const unsigned hprev = hall & lt;           // lanes before this one that hold a run start
-  ps.h1 = head1;
-  ps.cont0 = in0 && !head0;
-  ps.t0 = tail0;
-  ps.t1 = tail1;
-  ps.left0 = !head0 && hprev == 0;
-  ps.left1 = ps.left0 && !head1;
-  ps.lead0 = lead_open && ps.left0;
-  ps.lead1 = lead_open && ps.left1;
-  const unsigned hm = hall & (lt | (1u << lane));
-  ps.reach = hm ? lane - (31 - __clz(hm)) : lane;   // (no start so far: the run reaches back to lane 0)
-  const int maxd = __reduce_max_sync(FULL, in0 ? ps.reach : 0);
+  const unsigned hall = __ballot_sync(FULL, head), inall = __ballot_sync(FULL, in);
+  const unsigned le = 0xffffffffu >> (31 - lane);   // lanes <= this one
+  const unsigned hm = hall & le;
+  ps.left = hm == 0;
+  const int first = ps.left ? 0 : 31 - __clz(hm);
+  ps.reach = lane - first;
+  ps.runm = le & (0xffffffffu << first);
+  ps.tail = tail;
+  ps.lead = lead_open && ps.left;
+  const int maxd = __reduce_max_sync(FULL, in ? ps.reach : 0);
   ps.nsteps = maxd == 0 ? 0 : 32 - __clz(maxd);
-  // lanes of the run of position 0 (up to it): from the run's first position f
-  const unsigned upto = lt | (1u << lane);    // lanes <= this one
-  if (head0) {
-    ps.m0a = 1u << lane;
-    ps.m1a = 0u;
-  } else if (hprev == 0) {
-    ps.m0a = upto;
-    ps.m1a = lt;
-  } else {
-    const int lp = 31 - __clz(hprev);                       // nearest earlier lane with a run start
-    const bool odd = (h1all >> lp) & 1u;                    // its last start is its position 1
-    const unsigned from = ~((1u << lp) - 1u);               // lanes >= lp
-    ps.m0a = upto & (odd ? from & ~(1u << lp) : from);
-    ps.m1a = lt & from;
-  }
-  ps.m0b = head1 ? 0u : ps.m0a;
-  ps.m1b = head1 ? (1u << lane) : (ps.m1a | (1u << lane));
-  ps.last_open = __shfl_sync(FULL, (int)(in1 && !tail1), 31) != 0;
+  ps.blk_left = (inall & 1u) && !(hall & 1u);
+  ps.last_open = (__ballot_sync(FULL, in && !tail) >> 31) != 0;
+  ps.interior = hall == 0 && inall == FULL && ps.last_open;
+  ps.has_head = hall != 0;
 }
 
-// From the per-sample weights of one theta to what the passing pixels add to this lane's sums.
+// From the per-sample weights of TWO theta points (a, b: two independent chains, so that the shuffle latencies of one
+// hide behind the other) to what the passing pixels add to this lane's sums.  No branch: the scan always takes its
+// five steps (a lane whose run does not reach that far adds nothing).
 //   in : w[k], live[k]; carry = (W, Q, n) of the run left open by the previous block (slot of this warp and theta)
-//        leadWQ / leadN: where the run that was open at the start of the warp's range is put when it ends here
-//   out: cW, cQ, cn (weights, squared weights, live samples of the passing pixels that end on this lane), cp = how many
-__device__ __forceinline__ void pix_reduce(const PixShape& ps, const double* w, const bool* live, double neff_min,
-                                           double* carryWQ, int* carryN, double* leadWQ, int* leadN, int lane,
-                                           double& cW, double& cQ, int& cn, int& cp) {
+//        lead: where the run that was open at the start of the warp's range is put when it ends here
+//        second = false: b is a repeated point (odd theta count), its slots are left alone
+//   out: cW, cQ, cn (weights, squared weights, live samples of the passing pixel that ends on this lane), cp = 0 | 1
+struct PixSlot {
+  double* carryWQ;
+  int* carryN;
+  double* leadWQ;
+  int* leadN;
+};
+__device__ __forceinline__ void pix_reduce2(const PixShape& ps, const double* wa, const bool* la, const double* wb,
+                                            const bool* lb, bool second, double neff_min, PixSlot sa, PixSlot sb,
+                                            int lane, double& aW, double& aQ, int& an, int& ap, double& bW, double& bQ,
+                                            int& bn, int& bp) {
   const unsigned FULL = 0xffffffffu;
-  const double q0 = w[0] * w[0];
-  // the lane's part of the run that is open at its end, then the inclusive segmented scan of it over the lanes
-  double XW = ps.h1 ? w[1] : w[0] + w[1];
-  double XQ = ps.h1 ? w[1] * w[1] : fma(w[1], w[1], q0);
+  double XA = wa[0] + wa[1], QA = fma(wa[1], wa[1], wa[0] * wa[0]);
+  double XB = wb[0] + wb[1], QB = fma(wb[1], wb[1], wb[0] * wb[0]);
+  __syncwarp();        // the carry slots were written by other lanes (previous block of this warp)
+  // the run open at the block's start continues on lane 0 (the slots hold zeros when there is none)
+  const int inNA = ps.left ? *sa.carryN : 0, inNB = ps.left ? *sb.carryN : 0;
+  if (lane == 0) {
+    XA += sa.carryWQ[0];
+    QA += sa.carryWQ[1];
+    XB += sb.carryWQ[0];
+    QB += sb.carryWQ[1];
+  }
+  // inclusive segmented scan over the lanes
 #pragma unroll
-  for (int st = 0; st < 5; ++st) {
-    if (st >= ps.nsteps) break;  // warp-uniform
-    const int o = 1 << st;
-    const double tW = __shfl_up_sync(FULL, XW, o), tQ = __shfl_up_sync(FULL, XQ, o);
+  for (int o = 1; o < 32; o <<= 1) {
+    const double tA = __shfl_up_sync(FULL, XA, o), uA = __shfl_up_sync(FULL, QA, o);
+    const double tB = __shfl_up_sync(FULL, XB, o), uB = __shfl_up_sync(FULL, QB, o);
     if (ps.reach >= o) {
-      XW += tW;
-      XQ += tQ;
+      XA += tA;
+      QA += uA;
+      XB += tB;
+      QB += uB;
     }
   }
-  // what the run of position 0 collected before this lane: the previous lane's scan value, plus the open run of
-  // the previous block when it reaches this far
-  double CW = __shfl_up_sync(FULL, XW, 1), CQ = __shfl_up_sync(FULL, XQ, 1);
-  if (lane == 0) { CW = 0.0; CQ = 0.0; }
-  const double inW = carryWQ[0], inQ = carryWQ[1];
-  const int inN = *carryN;
-  CW += ps.left0 ? inW : 0.0;
-  CQ += ps.left0 ? inQ : 0.0;
-  const double W0 = ps.cont0 ? CW + w[0] : w[0], Q0 = ps.cont0 ? CQ + q0 : q0;
-  const double W1 = ps.h1 ? w[1] : W0 + w[1], Q1 = ps.h1 ? w[1] * w[1] : fma(w[1], w[1], Q0);
-  const unsigned b0 = __ballot_sync(FULL, live[0]), b1 = __ballot_sync(FULL, live[1]);
-  const int n0 = __popc(b0 & ps.m0a) + __popc(b1 & ps.m1a) + (ps.left0 ? inN : 0);
-  const int n1 = __popc(b0 & ps.m0b) + __popc(b1 & ps.m1b) + (ps.left1 ? inN : 0);
-  // what the next block inherits
-  const double oW = __shfl_sync(FULL, W1, 31), oQ = __shfl_sync(FULL, Q1, 31);
-  const int oN = __shfl_sync(FULL, n1, 31);
+  const unsigned a0 = __ballot_sync(FULL, la[0]), a1 = __ballot_sync(FULL, la[1]);
+  const unsigned b0 = __ballot_sync(FULL, lb[0]), b1 = __ballot_sync(FULL, lb[1]);
+  const int nA = __popc(a0 & ps.runm) + __popc(a1 & ps.runm) + inNA;
+  const int nB = __popc(b0 & ps.runm) + __popc(b1 & ps.runm) + inNB;
+  // what the next block inherits: lane 31 holds the sums of the run that stays open
   __syncwarp();
-  if (lane == 0) {
-    carryWQ[0] = ps.last_open ? oW : 0.0;
-    carryWQ[1] = ps.last_open ? oQ : 0.0;
-    *carryN = ps.last_open ? oN : 0;
+  if (lane == 31) {
+    sa.carryWQ[0] = ps.last_open ? XA : 0.0;
+    sa.carryWQ[1] = ps.last_open ? QA : 0.0;
+    *sa.carryN = ps.last_open ? nA : 0;
+    if (second) {
+      sb.carryWQ[0] = ps.last_open ? XB : 0.0;
+      sb.carryWQ[1] = ps.last_open ? QB : 0.0;
+      *sb.carryN = ps.last_open ? nB : 0;
+    }
   }
-  __syncwarp();
-  // began in an earlier warp's range: the segment-end stitch decides (one position of the block at most)
-  if (ps.t0 && ps.lead0) { leadWQ[0] = W0; leadWQ[1] = Q0; *leadN = n0; }
-  if (ps.t1 && ps.lead1) { leadWQ[0] = W1; leadWQ[1] = Q1; *leadN = n1; }
-  const bool p0 = ps.t0 && !ps.lead0 && W0 > 0.0 && W0 * W0 >= neff_min * Q0;
-  const bool p1 = ps.t1 && !ps.lead1 && W1 > 0.0 && W1 * W1 >= neff_min * Q1;
-  cW = (p0 ? W0 : 0.0) + (p1 ? W1 : 0.0);
-  cQ = (p0 ? Q0 : 0.0) + (p1 ? Q1 : 0.0);
-  cn = (p0 ? n0 : 0) + (p1 ? n1 : 0);
-  cp = (p0 ? 1 : 0) + (p1 ? 1 : 0);
+  // began in an earlier warp's range: the segment-end stitch decides (one lane of the block at most)
+  if (ps.tail && ps.lead) {
+    sa.leadWQ[0] = XA; sa.leadWQ[1] = QA; *sa.leadN = nA;
+    if (second) { sb.leadWQ[0] = XB; sb.leadWQ[1] = QB; *sb.leadN = nB; }
+  }
+  const bool own = ps.tail && !ps.lead;
+  const bool pa = own && XA > 0.0 && XA * XA >= neff_min * QA;
+  const bool pb = own && second && XB > 0.0 && XB * XB >= neff_min * QB;
+  aW = pa ? XA : 0.0; aQ = pa ? QA : 0.0; an = pa ? nA : 0; ap = pa ? 1 : 0;
+  bW = pb ? XB : 0.0; bQ = pb ? QB : 0.0; bn = pb ? nB : 0; bp = pb ? 1 : 0;
 }
 
 // One sample's theta-independent values, held in registers while the warp loops over the tile's theta points.
@@ -381,8 +377,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   // ASYNC: no barrier between segments.  The sums of consecutive segments go to alternating buffers; the last warp to
   // finish a segment combines it (fixed warp order) while the others are already on the next one, and the blocks are
   // dealt round-robin across segment boundaries, so the warps' loads even out over the group.
-  constexpr bool ASYNC = !PIX && !TEAMS;
-  constexpr int NBUF = PIX ? 1 : 2;
+  // (Pixel-cut mode keeps contiguous ranges per warp; what evens out there is the cost of its blocks, which differs
+  // between blocks inside one pixel and blocks full of pixel ends.)
+  constexpr bool ASYNC = !TEAMS;
+  constexpr int NBUF = 2;
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
   typedef typename std::conditional<INJ, double, LosT>::type RowT;  // the all-sky table is f64
@@ -396,7 +394,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   double* s_lead = reinterpret_cast<double*>(smem + L.lead);
   int* s_leadn = reinterpret_cast<int*>(smem + L.leadn);
   __shared__ int s_arrive[2], s_done;  // ASYNC: warps that finished a segment (per buffer), segments combined so far
-  __shared__ int s_hashead[NWARPS];  // pixel-cut mode: the warp's range of the current segment contains a pixel start
+  __shared__ int s_hashead[2][NWARPS];  // pixel-cut mode: the warp's range of the segment contains a pixel start
   double* s_allsky = reinterpret_cast<double*>(smem + L.allsky);
   NodeT* s_tab = reinterpret_cast<NodeT*>(smem + L.tab);
   Node64* s_ftab = reinterpret_cast<Node64*>(smem + L.ftab);
@@ -449,11 +447,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     }
     int rot = 0;  // ASYNC: the warp that takes the first block of the current segment
     if (PIX) {
-      for (int i = tid; i < NWARPS * T * 2; i += NTHREADS) {
+      for (int i = tid; i < NWARPS * T * 2 * NBUF; i += NTHREADS) {
         s_carry[i] = 0.0;
         s_lead[i] = 0.0;
       }
-      for (int i = tid; i < NWARPS * T; i += NTHREADS) {
+      for (int i = tid; i < NWARPS * T * NBUF; i += NTHREADS) {
         s_np[i] = 0;
         s_carryn[i] = 0;
         s_leadn[i] = 0;
@@ -488,10 +486,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       const int buf = ASYNC ? (sidx & 1) : 0;
       double* acc_b = s_acc + buf * (NWARPS * T * 2);
       int* cnt_b = s_cnt + buf * (NWARPS * T);
+      // pixel-cut mode: this segment's set of the per-(warp, theta) pixel state
+      int* np_b = s_np + buf * (NWARPS * T);
+      double* carry_b = s_carry + buf * (NWARPS * T * 2);
+      int* carryn_b = s_carryn + buf * (NWARPS * T);
+      double* lead_b = s_lead + buf * (NWARPS * T * 2);
+      int* leadn_b = s_leadn + buf * (NWARPS * T);
       if (ASYNC && sidx >= 2) {
         // this buffer last held segment sidx-2: wait until it has been combined and cleared
-        while (*(volatile int*)&s_done < sidx - 1) {
-        }
+        while (*(volatile int*)&s_done < sidx - 1) __nanosleep(PIX ? 400 : 100);   // (no issue slots burnt while waiting)
         __threadfence_block();  // the cleared buffer is seen after the release
       }
 #ifdef GWC_CHECKED
@@ -510,9 +513,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       if (ASYNC) rot = (rot + (int)((s1 - s0 + BLK - 1) / BLK)) & (NWARPS - 1);
       bool lead_open = true;  // no pixel start seen yet in this warp's range
       if (PIX) {
+        // (the ranges are dealt to the warps rotated by one per segment, so that the range that is one block longer
+        // than the others does not always fall on the same warp)
         const int64_t nb = (s1 - s0 + BLK - 1) / BLK;
-        w_lo = s0 + nb * warp / NWARPS * BLK;
-        w_hi = min(s1, s0 + nb * (warp + 1) / NWARPS * BLK);
+        const int rw = (warp + sidx) & (NWARPS - 1);   // this warp's range of the segment
+        w_lo = s0 + nb * rw / NWARPS * BLK;
+        w_hi = min(s1, s0 + nb * (rw + 1) / NWARPS * BLK);
         w_step = BLK;
       }
       for (int64_t c0 = w_lo; c0 < w_hi; c0 += w_step) {
@@ -520,18 +526,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         PixShape ps;
         double dmin = CUDART_INF;  // smallest d_L of the warp's samples: a whole-warp range test per theta
         if (PIX) {
-          // run structure of the block: run starts and ends at this lane's two consecutive positions
+          // run structure of the block (pixel-aligned copy: the lane's two positions lie in one run)
           static_assert(!PIX || SPT == 2, "pixel-cut mode: two consecutive samples per lane");
           const int64_t g0 = c0 + 2 * lane;
-          const bool in0 = g0 < w_hi, in1 = g0 + 1 < w_hi;
-          const int32_t r0 = in0 ? p.row[g0] : 0, r1 = in1 ? p.row[g0 + 1] : 0;
-          const bool head0 = in0 && (g0 == s0 || p.row[g0 - 1] != r0);
-          const bool head1 = in1 && r1 != r0;
+          const bool in = g0 < w_hi;
+          const int32_t r0 = in ? p.row[g0] : 0;
+          const bool head = in && (g0 == s0 || p.row[g0 - 1] != r0);
           // (ranges end on block boundaries or on the segment's last sample, which is a tail)
-          const bool tail0 = in0 && (g0 + 1 >= s1 || p.row[g0 + 1] != r0);
-          const bool tail1 = in1 && (g0 + 2 >= s1 || p.row[g0 + 2] != r1);
-          pix_shape(ps, in0, in1, head0, head1, tail0, tail1, lead_open, lane);
-          lead_open = lead_open && __ballot_sync(FULL, head0 | head1) == 0;
+          const bool tail = in && (g0 + 2 >= s1 || p.row[g0 + 2] != r0);
+          pix_shape(ps, in, head, tail, lead_open, lane);
+          // (no short-circuit: a vote under a branch makes ptxas treat the whole loop as divergent, and the per-theta
+          // constants then come through vector loads instead of uniform ones)
+          lead_open = lead_open & !ps.has_head;
         }
 #pragma unroll
         for (int k = 0; k < SPT; ++k) {
@@ -557,9 +563,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         // theta points of the tile for which at least one sample of this warp lies inside the table
         const double* tcl = KT + (t0 + min(lane, nt - 1)) * NC;
         unsigned todo = __ballot_sync(FULL, lane < nt && dmin * tcl[C_H] < tcl[C_UMAX]);
-        if (PIX) todo = 0xffffffffu >> (32 - nt);  // every theta sees every block: open runs are carried through
+        // every theta sees every block: open runs are carried through (a ballot: the compiler then knows the list is
+        // warp-uniform and reads the constants of its points through uniform loads)
+        if (PIX) todo = __ballot_sync(FULL, lane < nt);
         // Software pipeline over the theta points: the first half of the next point (table look-up, LOS loads)
         // is issued together with the second half of the current one, so its latencies hide behind FP64 work.
+        // (pixel-cut mode: a block that lies inside one pixel is summed like a block of the uncut estimator; the two
+        // forms of the loop are separate instantiations, so that no branch sits inside the pipeline)
+        auto theta_loop = [&](auto interior_c) {
+        constexpr bool plain = !PIX || decltype(interior_c)::value;
         int ja = pop_lowest(todo);
         if (ja >= 0) {
           Mid<RowT> cur[SPT], nxt[SPT];
@@ -593,6 +605,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
             const int jh = jb >= 0 ? jb : ja;  // (a redundant look-up when the list ends on an odd count)
             double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
             int cnt = 0, cntb = 0, npa = 0, npb = 0;  // (cntb, npa, npb: pixel-cut mode)
+            double wa[SPT];   // (pixel-cut mode: the first point's weights wait for the second's)
+            bool la[SPT];
             {
               const double* tch = KT + (t0 + jh) * NC;
               const double* tct = KT + (t0 + ja) * NC;
@@ -600,20 +614,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               for (int k = 0; k < SPT; ++k)
                 term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, nxt[k], p.flag, Mp);
-              double wv[SPT];
-              bool lv[SPT];
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
-                wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], lv[k], p.flag);
-                if (!PIX) {
-                  a0 += wv[k];
-                  a1 = fma(wv[k], wv[k], a1);
-                  cnt += lv[k] ? 1 : 0;
+                wa[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + ja * MF_PITCH, sm[k].C, sm[k].P, cur[k], la[k], p.flag);
+                if (plain) {
+                  a0 += wa[k];
+                  a1 = fma(wa[k], wa[k], a1);
+                  cnt += la[k] ? 1 : 0;
                 }
               }
-              if (PIX)
-                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + ja) * 2, s_carryn + warp * T + ja,
-                           s_lead + (warp * T + ja) * 2, s_leadn + warp * T + ja, lane, a0, a1, cnt, npa);
             }
             const int jc = pop_lowest(todo);
             {
@@ -634,22 +643,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
                 wv[k] = term_tail<RowT, MP>(tct, logtab, exptab, s_ftab + jh * MF_PITCH, sm[k].C, sm[k].P, nxt[k], lv[k], p.flag);
                 lv[k] = lv[k] & second;
                 wv[k] = lv[k] ? wv[k] : 0.0;
-                if (!PIX) {
+                if (plain) {
                   b0 += wv[k];
                   b1 = fma(wv[k], wv[k], b1);
                   cnt += lv[k] ? 0x10000 : 0;
                 }
               }
-              if (PIX && second)  // warp-uniform
-                pix_reduce(ps, wv, lv, p.neff_min, s_carry + (warp * T + jh) * 2, s_carryn + warp * T + jh,
-                           s_lead + (warp * T + jh) * 2, s_leadn + warp * T + jh, lane, b0, b1, cntb, npb);
+              if (!plain) {
+                const PixSlot sa = {carry_b + (warp * T + ja) * 2, carryn_b + warp * T + ja, lead_b + (warp * T + ja) * 2,
+                                    leadn_b + warp * T + ja};
+                const PixSlot sb = {carry_b + (warp * T + jh) * 2, carryn_b + warp * T + jh, lead_b + (warp * T + jh) * 2,
+                                    leadn_b + warp * T + jh};
+                pix_reduce2(ps, wa, la, wv, lv, second, p.neff_min, sa, sb, lane, a0, a1, cnt, npa, b0, b1, cntb, npb);
+              }
             }
-            if (PIX) {
-              // pixel-cut mode: the live counts of whole pixels do not fit the 16-bit packing; four reductions
+            if (!plain) {
+              // pixel-cut mode: the live counts of whole pixels do not fit the 16-bit packing; three reductions
               cnt = __reduce_add_sync(FULL, cnt);
               cntb = __reduce_add_sync(FULL, cntb);
-              npa = __reduce_add_sync(FULL, npa);
-              npb = __reduce_add_sync(FULL, npb);
+              npa = __reduce_add_sync(FULL, npa | (npb << 16));   // (at most 32 pixels end in a block)
+              npb = npa >> 16;
+              npa &= 0xffff;
               const double k = warp_sum4(a0, a1, b0, b1, lane);
               if ((lane & 7) == 0) {
                 const int j = (lane & 16) ? jb : ja;
@@ -658,7 +672,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
                   acc_b[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
                   if ((lane & 8) == 0) {
                     cnt_b[warp * T + j] += (lane & 16) ? cntb : cnt;
-                    s_np[warp * T + j] += (lane & 16) ? npb : npa;
+                    np_b[warp * T + j] += (lane & 16) ? npb : npa;
                   }
                 }
               }
@@ -668,13 +682,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
             }
             cnt = __reduce_add_sync(FULL, cnt);
             if (cnt) {  // warp-uniform
+              // (pixel-cut mode, a block inside one pixel: the sums go on the run that stays open)
+              double* sum_b = PIX ? carry_b : acc_b;
+              int* n_b = PIX ? carryn_b : cnt_b;
               const double k = warp_sum4(a0, a1, b0, b1, lane);
               if ((lane & 7) == 0) {
                 const int j = (lane & 16) ? jb : ja;
                 if (j >= 0) {
                   GWC_DEV_CHECK(p.flag, j < nt, FLAG_CHK_ACC);
-                  acc_b[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
-                  if ((lane & 8) == 0) cnt_b[warp * T + j] += (lane & 16) ? (cnt >> 16) : (cnt & 0xffff);
+                  sum_b[(warp * T + j) * 2 + ((lane >> 3) & 1)] += k;
+                  if ((lane & 8) == 0) n_b[warp * T + j] += (lane & 16) ? (cnt >> 16) : (cnt & 0xffff);
                 }
               }
             }
@@ -682,6 +699,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
             ja = jc;
           }
         }
+        };
+        if (PIX && ps.interior) theta_loop(std::true_type{});   // warp-uniform, the same for every theta
+        else theta_loop(std::false_type{});
       }
       if (PIX) {
         // What this warp's range leaves for the stitch: the run open at its start (lead), whether a pixel starts
@@ -689,14 +709,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         // is one open run and belongs to the lead.
         __syncwarp();
         if (lead_open && lane < nt) {
-          s_lead[(warp * T + lane) * 2] += s_carry[(warp * T + lane) * 2];
-          s_lead[(warp * T + lane) * 2 + 1] += s_carry[(warp * T + lane) * 2 + 1];
-          s_leadn[warp * T + lane] += s_carryn[warp * T + lane];
-          s_carry[(warp * T + lane) * 2] = 0.0;
-          s_carry[(warp * T + lane) * 2 + 1] = 0.0;
-          s_carryn[warp * T + lane] = 0;
+          lead_b[(warp * T + lane) * 2] += carry_b[(warp * T + lane) * 2];
+          lead_b[(warp * T + lane) * 2 + 1] += carry_b[(warp * T + lane) * 2 + 1];
+          leadn_b[warp * T + lane] += carryn_b[warp * T + lane];
+          carry_b[(warp * T + lane) * 2] = 0.0;
+          carry_b[(warp * T + lane) * 2 + 1] = 0.0;
+          carryn_b[warp * T + lane] = 0;
         }
-        if (lane == 0) s_hashead[warp] = lead_open ? 0 : 1;
+        if (lane == 0) s_hashead[buf][warp] = lead_open ? 0 : 1;
       }
       if (ASYNC) {
         __syncwarp();
@@ -712,7 +732,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
                         FLAG_CHK_HANDOFF);
           if (lane < nt) {
             double a = 0.0, b = 0.0;
-            int c = 0;
+            int c = 0, np = 0;
             for (int w = 0; w < NWARPS; ++w) {
               a += *(volatile double*)&acc_b[(w * T + lane) * 2];
               b += *(volatile double*)&acc_b[(w * T + lane) * 2 + 1];
@@ -720,11 +740,50 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               acc_b[(w * T + lane) * 2] = 0.0;
               acc_b[(w * T + lane) * 2 + 1] = 0.0;
               cnt_b[w * T + lane] = 0;
+              if (PIX) {
+                np += *(volatile int*)&np_b[w * T + lane];
+                np_b[w * T + lane] = 0;
+              }
+            }
+            if (PIX) {
+              // pixels that cross warp ranges: walk the ranges in order, close the open run wherever a pixel starts
+              double oW = 0.0, oQ = 0.0;
+              int oN = 0;
+              for (int r = 0; r <= NWARPS; ++r) {
+                const int w = r < NWARPS ? ((r - sidx) & (NWARPS - 1)) : NWARPS;   // the warp that had range r
+                if (w < NWARPS) {
+                  oW += *(volatile double*)&lead_b[(w * T + lane) * 2];
+                  oQ += *(volatile double*)&lead_b[(w * T + lane) * 2 + 1];
+                  oN += *(volatile int*)&leadn_b[w * T + lane];
+                }
+                if (w == NWARPS || *(volatile int*)&s_hashead[buf][w]) {
+                  if (oW > 0.0 && oW * oW >= p.neff_min * oQ) {
+                    a += oW;
+                    b += oQ;
+                    c += oN;
+                    np += 1;
+                  }
+                  if (w < NWARPS) {
+                    oW = *(volatile double*)&carry_b[(w * T + lane) * 2];
+                    oQ = *(volatile double*)&carry_b[(w * T + lane) * 2 + 1];
+                    oN = *(volatile int*)&carryn_b[w * T + lane];
+                  }
+                }
+                if (w < NWARPS) {
+                  lead_b[(w * T + lane) * 2] = 0.0;
+                  lead_b[(w * T + lane) * 2 + 1] = 0.0;
+                  leadn_b[w * T + lane] = 0;
+                  carry_b[(w * T + lane) * 2] = 0.0;
+                  carry_b[(w * T + lane) * 2 + 1] = 0.0;
+                  carryn_b[w * T + lane] = 0;
+                }
+              }
             }
             const size_t o = (size_t)(p.t_begin + t0 + lane) * (size_t)p.n_seg + (size_t)seg;
             p.out_w[2 * o] = a;
             p.out_w[2 * o + 1] = b;
             p.out_n[o] = c;
+            if (PIX) p.out_np[o] = np;
           }
           __syncwarp();
           if (lane == 0) {
@@ -741,7 +800,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       if ((tid & 31) < nt && (tid >> 5) < nteam) {  // (acc_b = s_acc here: one buffer)
         const int team = tid >> 5, j = tid & 31;  // one thread per (segment of this round, theta)
         double a = 0.0, b = 0.0;
-        int c = 0, np = 0;
+        int c = 0;
         for (int w = team * tsz; w < (team + 1) * tsz; ++w) {
           a += s_acc[(w * T + j) * 2];
           b += s_acc[(w * T + j) * 2 + 1];
@@ -749,49 +808,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           s_acc[(w * T + j) * 2] = 0.0;
           s_acc[(w * T + j) * 2 + 1] = 0.0;
           s_cnt[w * T + j] = 0;
-          if (PIX) {
-            np += s_np[w * T + j];
-            s_np[w * T + j] = 0;
-          }
-        }
-        if (PIX) {
-          // pixels that cross warp ranges: walk the ranges in order, close the open run wherever a pixel starts
-          double oW = 0.0, oQ = 0.0;
-          int oN = 0;
-          for (int w = 0; w <= NWARPS; ++w) {
-            if (w < NWARPS) {
-              oW += s_lead[(w * T + j) * 2];
-              oQ += s_lead[(w * T + j) * 2 + 1];
-              oN += s_leadn[w * T + j];
-            }
-            if (w == NWARPS || s_hashead[w]) {
-              if (oW > 0.0 && oW * oW >= p.neff_min * oQ) {
-                a += oW;
-                b += oQ;
-                c += oN;
-                np += 1;
-              }
-              if (w < NWARPS) {
-                oW = s_carry[(w * T + j) * 2];
-                oQ = s_carry[(w * T + j) * 2 + 1];
-                oN = s_carryn[w * T + j];
-              }
-            }
-            if (w < NWARPS) {
-              s_lead[(w * T + j) * 2] = 0.0;
-              s_lead[(w * T + j) * 2 + 1] = 0.0;
-              s_leadn[w * T + j] = 0;
-              s_carry[(w * T + j) * 2] = 0.0;
-              s_carry[(w * T + j) * 2 + 1] = 0.0;
-              s_carryn[w * T + j] = 0;
-            }
-          }
         }
         const size_t o = (size_t)(p.t_begin + t0 + j) * (size_t)p.n_seg + (size_t)(seg0 + team);
         p.out_w[2 * o] = a;
         p.out_w[2 * o + 1] = b;
         p.out_n[o] = c;
-        if (PIX) p.out_np[o] = np;
       }
       __syncthreads();  // the reset above precedes the next segment's accumulation
       seg0 += nteam;
