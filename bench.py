@@ -33,9 +33,21 @@ from paper_2605_23538_b200 import synth  # noqa: E402
 
 METRIC = "(theta*event*sample) terms/s, whole hot path (events + injections)"
 UNIT = "terms/s"
-# Algorithmic FP64-pipe instructions per term of THIS formulation (counted from SASS)
+# FP64-pipe instructions per term of THIS formulation.  NECESSARY (what a live / a dead term needs: DESIGN.md section 7,
+# counted from the SASS of the main loop) is what `roofline.frac` uses; EXECUTED is what the shipped event kernel runs
+# per term, live or dead, MEASURED by ncu (sass__thread_inst_executed_true_per_opcode: DFMA + DADD + DMUL + DSETP over
+# the terms of one 340-theta launch of the O5 catalogue; profiles/r02a_reweight_events_ncu_full.md).  Re-measure
+# after any edit of the kernel: the profile names the command.
 FP64_INSTR_LIVE = 104.0
 FP64_INSTR_DEAD = 28.0
+FP64_INSTR_EXECUTED = 108.26
+FP64_COUNT_SOURCE = "necessary: static SASS count of the main loop (DESIGN.md 7); executed: ncu op counters, profiles/r02a_reweight_events_ncu_full.md"
+# the KDE kernel: FP64 thread instructions per Gaussian evaluation, everything included (per-sample weights, per-pixel
+# statistics, prior), measured the same way (profiles/r02d_kde_kernel_ncu_full.md)
+KDE_FP64_INSTR_PER_EVAL = 4.95
+# DRAM bytes of one 340-theta launch of the event kernel on the O5 catalogue (ncu dram__bytes_read.sum +
+# dram__bytes_write.sum, same capture)
+O5_DRAM_BYTES_PER_340_THETA = 7.301e9 + 0.078e9
 # B200 FP64 issue peak derived from the unit counts: 148 SMs x 64 FP64 lanes x 1.965 GHz
 FP64_PEAK_INSTR = 148 * 64 * 1.965e9
 
@@ -107,6 +119,16 @@ def _bench_spec(name: str, theta_scale: float):
     if theta_scale != 1.0:
         spec = synth.scaled(spec, n_theta=max(1, int(round(spec.n_theta * theta_scale))))
     return spec
+
+
+def _hbm_peak():
+    """Measured HBM copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the profiling
+    guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json (hbm_gbs)"
+    except Exception:
+        return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
 def _pin(t):
@@ -276,15 +298,21 @@ def run_gwc(args):
     achieved = instr * 2.0 / (ms_ev_kernel * 1e-3) / 1e12          # FP64 issue slots x 2 flop
     peak = FP64_PEAK_INSTR * 2.0 / 1e12
     probe_ms, probe_n = ctx.gwc_probe_fp64(1 << 13)
-    # DRAM bytes of the event kernel from the ncu --set full capture (profiles/r01c): 7.26e9 per 340-theta launch
-    # of the O5 catalogue; kernel_ms covers the ceil(n_theta / 340) launches of one step, so the traffic does too
-    traffic = 7.26e9 * n_theta / 340.0 if spec.name == "o5" else None
+    # DRAM bytes of the event kernel: an ncu figure (a capture, not this run), only for the workload it was taken on;
+    # kernel_ms covers the ceil(n_theta / 340) launches of one step, so the traffic is scaled to them
+    traffic = O5_DRAM_BYTES_PER_340_THETA * n_theta / 340.0 if spec.name == "o5" and args.table_prec == "f64" else None
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": traffic, "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01c "
-                "(bytes per step's event-kernel launches; HBM does not bind)" if traffic else None, "kernel": "reweight_kernel<events>", "kernel_ms": ms_ev_kernel,
+                "traffic": traffic, "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of one 340-theta "
+                "launch, profiles/r02a_reweight_events_ncu_full.md, scaled to the step's launches (HBM does not bind)"
+                if traffic else None, "kernel": "reweight_kernel<events>", "kernel_ms": ms_ev_kernel,
                 "kernel_share_of_step": ms_ev_kernel / (ms / args.steps),
                 "inj_kernel_ms": ms_inj_kernel,
                 "fp64_instr_per_live_term": FP64_INSTR_LIVE, "fp64_instr_per_dead_term": FP64_INSTR_DEAD,
+                # the instructions the kernel executes per term (ncu-measured), against the same peak: the FP64 pipe's
+                # utilisation as the run itself sees it
+                "fp64_instr_executed_per_term": FP64_INSTR_EXECUTED,
+                "frac_executed": terms_ev * FP64_INSTR_EXECUTED / (ms_ev_kernel * 1e-3) / FP64_PEAK_INSTR,
+                "fp64_count_source": FP64_COUNT_SOURCE,
                 # the same time against the budget BASELINE.md froze before any code (180 live / 30 dead): context only
                 "frac_at_survey_budget_180_30": terms_ev * (live_frac_ev * 180.0 + (1.0 - live_frac_ev) * 30.0)
                 / (ms_ev_kernel * 1e-3) / FP64_PEAK_INSTR,
@@ -327,11 +355,14 @@ def run_gwc(args):
         ctx.gwc_set_timing(False)
         ms_kde = tk["ms_ev"] / max(tk["n_ev"], 1)
         evals = float(nused.sum().item()) * 256.0
-        # 10 FP64 instructions per Gaussian evaluation (offset, square, 7-instruction exp, accumulate): DESIGN.md 11
         kde = {"n_theta": int(th_k.shape[0]), "n_grid": 256, "neff_min": 2.0, "kernel_ms": ms_kde,
                "event_terms_per_s": th_k.shape[0] * n_samples / (ms_kde * 1e-3),
                "gaussian_evals_per_s": evals / (ms_kde * 1e-3),
-               "roofline_frac_fp64": evals * 10.0 / (ms_kde * 1e-3) / FP64_PEAK_INSTR}
+               "fp64_instr_per_eval": KDE_FP64_INSTR_PER_EVAL,
+               "fp64_count_source": "ncu op counters over the Gaussian evaluations of the launch, profiles/r02d_kde_kernel_ncu_full.md",
+               "roofline_frac_fp64": evals * KDE_FP64_INSTR_PER_EVAL / (ms_kde * 1e-3) / FP64_PEAK_INSTR,
+               # (round 1 counted 10 instructions per evaluation for the kernel of that round: the same time on that scale)
+               "roofline_frac_fp64_at_r01_count_10": evals * 10.0 / (ms_kde * 1e-3) / FP64_PEAK_INSTR}
         del nused
     # ---- NEXT row 4, reported beside the headline: one theta per call (the sampler's pattern), catalogue cache on ----
     lat = None
@@ -350,10 +381,20 @@ def run_gwc(args):
             l1.record()
             torch.cuda.synchronize()
             wall = (time.perf_counter() - t0) / args.latency_calls * 1e3
-            lat = {"n_theta": 1, "calls": args.latency_calls, "device_ms_per_call": l0.elapsed_time(l1) / args.latency_calls,
-                   "wall_ms_per_call": wall, "catalogue_cache": True}
+            # what one call must stream (HBM-bound at one theta): the prepared samples (d_L, m1z, m2z, ln m1z, ln q, P: 48 B
+            # + 4 B row per event sample) and the two LOS nodes of every event sample (2 x 4 B, f32 table)
+            los_b = 2 * W.los.element_size()
+            lat_bytes = n_samples * (52 + los_b) + n_inj * 48
+            hbm, hbm_src = _hbm_peak()
+            dev_ms = l0.elapsed_time(l1) / args.latency_calls
+            lat = {"n_theta": 1, "calls": args.latency_calls, "device_ms_per_call": dev_ms,
+                   "wall_ms_per_call": wall, "catalogue_cache": True,
+                   "roofline": {"bound": "hbm", "bytes_per_call": lat_bytes, "achieved": lat_bytes / (dev_ms * 1e-3) / 1e9,
+                                "peak": hbm, "unit": "GB/s", "frac": lat_bytes / (dev_ms * 1e-3) / 1e9 / hbm,
+                                "peak_source": hbm_src}}
         finally:
             ctx.gwc_cache_catalogue(False)
+    a0 = a0_report(ctx, W, spec, args.seed) if args.a0 else None
     cpu = cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
     stress = stress_report(ctx, W, theta, zmax, allsky, args.n_nodes) if spec.name == "stress" else None
     line = {
@@ -385,9 +426,52 @@ def run_gwc(args):
         line["kde"] = kde
     if lat is not None:
         line["latency"] = lat
+    if a0 is not None:
+        line["a0_pack"] = a0
     print(json.dumps(line))
     if dist:
         td.destroy_process_group()
+
+
+def a0_report(ctx, W, spec, seed):
+    """A0 at full size (untimed region of the bench): gwc_pack_events + gwc_cap_pixels(2500) on the UNSORTED sample
+    list of the workload (the synthetic samples come sorted; a seeded permutation unsorts them).  Checked at full size
+    by what defines the answer (a permutation; keys ascending; equal keys in input order = the stable sort is unique);
+    the bit-for-bit comparison with the oracle is tests/test_gpu_full_size.py::test_pack_full_size.  The paper re-fills its padded tensor on every likelihood
+    call ("Fill Arrays": 5.38 ms per call at 2000 events on an H100); here it is one-time."""
+    dev = W.ev["dL"].device
+    off = W.ev["ev_sample_off"]
+    n_ev = int(off.numel()) - 1
+    n = int(off[-1])
+    eid = torch.repeat_interleave(torch.arange(n_ev, dtype=torch.int32, device=dev), (off[1:] - off[:-1]))
+    g = torch.Generator(device=dev).manual_seed(seed + 4242)
+    shuf = torch.randperm(n, generator=g, device=dev)
+    eid_u, row_u = eid[shuf].contiguous(), W.ev["sample_row"][shuf].contiguous()
+    del eid, shuf
+    ctx.gwc_pack_events(eid_u, row_u, n_ev)   # warm-up (scratch allocation)
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    torch.cuda.synchronize()
+    e0.record()
+    packed = ctx.gwc_pack_events(eid_u, row_u, n_ev)
+    e1.record()
+    kept, eso, pso = ctx.gwc_cap_pixels(packed, 2500, seed)
+    e2.record()
+    torch.cuda.synchronize()
+    ms_pack, ms_cap = e0.elapsed_time(e1), e1.elapsed_time(e2)
+    perm = packed["perm"]
+    key = (eid_u[perm].to(torch.int64) << 32) | row_u[perm].to(torch.int64)
+    ok_perm = bool(torch.equal(torch.sort(perm)[0], torch.arange(n, device=dev)))
+    ok_sorted = bool((key[1:] >= key[:-1]).all())
+    ok_stable = bool(((key[1:] != key[:-1]) | (perm[1:] > perm[:-1])).all())
+    ok_off = bool(torch.equal(packed["ev_sample_off"], off))
+    del key
+    # bytes the packing must move at the least: the two 4-byte keys in, the 8-byte permutation out
+    return {"n_samples": n, "n_events": n_ev, "n_pixrefs": int(packed["n_pixrefs"]), "pack_ms": ms_pack,
+            "cap2500_ms": ms_cap, "samples_kept_cap2500": int(kept.numel()),
+            "pack_samples_per_s": n / (ms_pack * 1e-3), "pack_GBps_algorithmic_16B_per_sample": n * 16 / (ms_pack * 1e-3) / 1e9,
+            "full_size_checks": {"permutation": ok_perm, "keys_ascending": ok_sorted, "stable": ok_stable,
+                                 "event_offsets": ok_off},
+            "paper_fill_arrays_ms_per_call_H100_2000_events": 5.38}
 
 
 def stress_report(ctx, W, theta, zmax, allsky, n_nodes):
@@ -523,6 +607,8 @@ def main():
     ap.add_argument("--leg", default="all", choices=["all", "events", "pixcut", "kde", "inj"],
                     help="run one leg alone and print its kernel time (profiling runs)")
     ap.add_argument("--kde-bandwidth", default="scott")
+    ap.add_argument("--no-a0", dest="a0", action="store_false",
+                    help="skip the A0 line (gwc_pack_events + gwc_cap_pixels on the unsorted sample list)")
     ap.add_argument("--pixcut", type=float, default=2.0,
                     help="also time the event term with the per-pixel N_eff cut at this threshold (< 0: skip)")
     args = ap.parse_args()

@@ -204,3 +204,74 @@ def test_o4_kde_theta_subset(ctx):
     fin = same & np.isfinite(oL)
     err = np.abs(gL[fin] - oL[fin]) / np.maximum(np.abs(oL[fin]), 1.0)
     assert err.max() <= RTOL_F64, err.max()
+
+
+def test_pack_full_size(ctx):
+    """A0 at O5 size (2.5e7 samples, 5000 events) on the UNSORTED sample list: gwc_pack_events is checked by what
+    defines its answer (a permutation; (event, row) keys ascending; equal keys in input order: the stable sort is
+    unique; the event offsets of the generator), gwc_cap_pixels(500) by its invariants (min(n, cap) kept per pixel,
+    kept samples in packed order); and both bit for bit against the oracle on a seeded sub-list of 2e5 samples."""
+    spec = synth.CONFIGS["o5"]
+    W = synth.make_workload(synth.scaled(spec, n_inj=1000, los_rows=spec.los_rows), seed=synth.DEFAULT_SEED, device=DEV,
+                            keep_f64_los=False)
+    off = W.ev["ev_sample_off"]
+    n_ev, n = int(off.numel()) - 1, int(off[-1])
+    assert n == 25_000_000
+    eid = torch.repeat_interleave(torch.arange(n_ev, dtype=torch.int32, device=DEV), off[1:] - off[:-1])
+    g = torch.Generator(device=DEV).manual_seed(99)
+    shuf = torch.randperm(n, generator=g, device=DEV)
+    eid_u, row_u = eid[shuf].contiguous(), W.ev["sample_row"][shuf].contiguous()
+    del eid, shuf
+    packed = ctx.gwc_pack_events(eid_u, row_u, n_ev)
+    perm = packed["perm"]
+    assert torch.equal(torch.sort(perm)[0], torch.arange(n, device=DEV))
+    key = (eid_u[perm].to(torch.int64) << 32) | row_u[perm].to(torch.int64)
+    assert bool((key[1:] >= key[:-1]).all())
+    assert bool(((key[1:] != key[:-1]) | (perm[1:] > perm[:-1])).all())
+    assert torch.equal(packed["ev_sample_off"], off)
+    heads = torch.cat([torch.ones(1, dtype=torch.bool, device=DEV), key[1:] != key[:-1]])
+    assert torch.equal(packed["pix_sample_off"][:-1], torch.nonzero(heads).flatten())
+    assert int(packed["pix_sample_off"][-1]) == n and packed["n_pixrefs"] == int(heads.sum())
+    # the cap: every pixel keeps min(n, cap), in packed order
+    cap = 500            # (the fiducial 2500 of PAPER.md:196 never binds on this catalogue: its largest pixel holds ~1900)
+    kept, eso, pso = ctx.gwc_cap_pixels(packed, cap, 7)
+    sizes = packed["pix_sample_off"][1:] - packed["pix_sample_off"][:-1]
+    assert torch.equal(pso[1:] - pso[:-1], torch.clamp(sizes, max=cap))
+    assert int(eso[-1]) == kept.numel() == int(torch.clamp(sizes, max=cap).sum())
+    assert (sizes > cap).any(), "the O5 catalogue has pixels above the cap"
+    pos = torch.empty(n, dtype=torch.int64, device=DEV)
+    pos[perm] = torch.arange(n, device=DEV)
+    assert bool((pos[kept][1:] > pos[kept][:-1]).all())          # a subsequence of the packed order
+    # the oracle on a sub-list
+    m = 200_000
+    sub = ctx.gwc_pack_events(eid_u[:m].contiguous(), row_u[:m].contiguous(), n_ev)
+    ref = oracle.pack_events(_np(eid_u[:m]), _np(row_u[:m]), n_ev)
+    for k in ("perm", "ev_sample_off", "ev_pix_off", "ev_pix_rows", "pix_sample_off"):
+        assert np.array_equal(_np(sub[k]), ref[k]), k
+    skept, seso, spso = ctx.gwc_cap_pixels(sub, 3, 7)
+    okept, oeso, opso = oracle.cap_pixels(ref["perm"], ref["ev_sample_off"], ref["pix_sample_off"], 3, 7)
+    assert np.array_equal(_np(skept), okept) and np.array_equal(_np(seso), oeso) and np.array_equal(_np(spso), opso)
+
+
+def test_production_multipeak_sampled():
+    """The production batch under the MULTIPEAK mass model (NEXT row 3a), every second event scaled into the smoothing
+    window: sampled against the oracle like the other full-size tests (4 theta x all events, all theta x 6 events)."""
+    from paper_2605_23538_b200 import gwc
+    c = gwc.Context(0)
+    try:
+        c.gwc_set_mass_model("multipeak")
+        W, _ = _device_workload("production")
+        spec = W.spec
+        theta = synth.make_theta_multipeak(spec, synth.DEFAULT_SEED, DEV)
+        off = W.ev["ev_sample_off"]
+        eid = torch.repeat_interleave(torch.arange(off.numel() - 1, device=DEV), off[1:] - off[:-1])
+        f = torch.where(eid % 2 == 1, 0.2, 1.0).to(torch.float64)
+        W.ev["m1z"], W.ev["m2z"] = W.ev["m1z"] * f, W.ev["m2z"] * f
+        gi = torch.where(torch.arange(W.inj["m1z"].numel(), device=DEV) % 2 == 1, 0.2, 1.0).to(torch.float64)
+        W.inj["m1z"], W.inj["m2z"] = W.inj["m1z"] * gi, W.inj["m2z"] * gi
+        g = _run_gpu(c, W, theta, W.los, 0)
+        with oracle.mass_model("multipeak"):
+            r = _check_sampled(W, theta, W.los, g, 0, n_th=4, n_ev=6)
+        print("production, MULTIPEAK: worst rel err on log L_i %.2e" % r["worst"])
+    finally:
+        c.close()
