@@ -91,7 +91,7 @@ __device__ __forceinline__ void node_pair(const Node32* t, int m, double& z0, do
 // z_k and v_k of one sample relative to e^shift (v < 0: dead): DESIGN.md section 3 without p_los and the rate term.
 // `scale` = exp(-l_pi - shift) (for the default prior exp(-shift) / d_L^2, no logarithm at all).  Powers and the
 // Gaussian go through math64.cuh's exp / ln (2e-13), like the fused kernel.
-template <typename NodeT>
+template <typename NodeT, bool MP>
 __device__ __forceinline__ double sample_v(const ThetaK& K, const NodeT* tab, int M, double zq, double dL, double m1z,
                                            double m2z, double scale, int32_t row, int64_t n_rows, double los_zmax,
                                            const double2* logtab, const double* exptab, double& z_out) {
@@ -119,7 +119,7 @@ __device__ __forceinline__ double sample_v(const ThetaK& K, const NodeT* tab, in
   const double y = (m1 - K.mu) / K.sigma;
   double p1 = K.a_pl * exp_fast<true>(-K.alpha * lm1, exptab) + K.a_g * exp_fast<true>(-0.5 * y * y, exptab);
   double p2;
-  if (K.mp) {
+  if (MP) {
     // p(m1) p(m2 | m1) = [mix(m1) S(m1) / N1] [m2^beta S(m2) / C(m1)]; inside the smoothing window
     // C(m1) = S(m1) m1^(beta+1) |F|(m1) / |beta+1| from the table (S(m1) cancels), above it elementary
     const double yl = (m1 - K.mul) / K.sigl;
@@ -269,7 +269,7 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
 #pragma unroll
   for (int i = 0; i < KDE_NPL; i += 2) asm volatile("prefetch.global.L1 [%0];" ::"l"(lrow + s_b[i * 32 + lane]));
   asm volatile("prefetch.global.L1 [%0];" ::"l"(lrow + s_b[(KDE_NPL - 1) * 32 + lane] + 1));
-  const double invh = 1.0 / h;
+  const double invh = rcp_fast(h);
   const double norm = invh * 0.39894228040143267794;   // 1 / (h sqrt(2 pi))
   const double sinvh = invh * 0.70710678118654752440;  // so that the exponent is -(q')^2
   const double beta = dzg * sinvh;   // grid step in units of h sqrt(2)
@@ -333,9 +333,8 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
         acc[15] = fma(aj, u7, acc[15]);
       }
     }
-    // the halves exchange what the other one keeps; C_o = c1^(o^2), c1 = exp(-beta^2) to full accuracy (its 64th
-    // power is taken)
-    const double c1 = exp(-beta * beta), cs = c1 * c1;
+    // the halves exchange what the other one keeps; C_o = c1^(o^2), c1 = exp(-beta^2)
+    const double c1 = exp_fast<false>(-beta * beta, exptab), cs = c1 * c1;   // (2e-13; its 64th power: 1e-11)
     double C[9];
     C[0] = 1.0;
     double t = c1;
@@ -386,7 +385,7 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
   return part;
 }
 
-template <typename NodeT, typename LosT>
+template <typename NodeT, typename LosT, bool MP>
 __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) {
   extern __shared__ __align__(16) unsigned char kde_smem[];
   MathTables& mt = *reinterpret_cast<MathTables*>(kde_smem);
@@ -448,9 +447,9 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       K.mminb = pow(mmin, beta + 1.0);
       K.Om = th[1];
       K.OL = 1.0 - th[1];
-      K.mp = p.model == 1;
+      K.mp = MP;
       K.a_gl = 0.0; K.mul = 0.0; K.sigl = 1.0; K.dm = 0.0; K.fidx = 0.0; K.ctop = 0.0; K.topb = K.mminb; K.ftab = nullptr;
-      if (K.mp) {
+      if (MP) {
         const double dm = th[12], laml = th[15], iN1 = 1.0 / tcr[C_N1];
         K.a_pl *= iN1;
         K.a_g *= (1.0 - laml) * iN1;
@@ -491,7 +490,7 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
         const double lp = p.lprior ? p.lprior[k] : 0.0;
         const double scale = !p.lprior ? eshift / (d * d)
                                        : (isfinite(lp) ? exp_fast<true>(-lp - shift, exptab) : CUDART_NAN);
-        const double v = sample_v(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], scale, p.row[k], p.n_rows, p.los_zmax,
+        const double v = sample_v<NodeT, MP>(K, tab, p.M, p.tab_zq, d, p.m1z[k], p.m2z[k], scale, p.row[k], p.n_rows, p.los_zmax,
                                   logtab, exptab, z);
         GWC_DEV_CHECK(p.flag, k - s0 >= 0 && k - s0 < p.scr_stride, FLAG_CHK_KDE);
         scr[k] = make_double2(z, v);
@@ -566,11 +565,12 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
       bool pass = tail && n >= 2 && V > 0.0 && V * V >= p.neff_min * Q;
       double sd = 0.0, h = 0.0;
       if (pass) {
-        const double mo = Vd / V;
-        const double var = fma(-Vd, mo, Vdd) / V;
+        const double rV = rcp_fast(V);
+        const double mo = Vd * rV;
+        const double var = fma(-Vd, mo, Vdd) * rV;
         pass = var > 0.0;
         sd = pass ? sqrt(var) : 0.0;
-        h = 1.06 * sd * pow((double)n, -0.2);   // Eq. D1
+        h = 1.06 * sd * exp_fast<false>(-0.2 * log_fast((double)n, logtab), exptab);   // Eq. D1: n^(-1/5) = e^(-ln n / 5)
       }
       unsigned pm = __ballot_sync(FULL, pass);
       while (pm) {
@@ -628,12 +628,17 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
   p.scr = (double2*)scratch; p.scr_stride = scr_stride;
   const size_t smem = sizeof(MathTables) + sizeof(NodeW) * KDE_WARPS * 32 * KDE_NPL + (sizeof(int) + sizeof(double)) * 32 * KDE_NPL;
   const int64_t blocks = n_blocks;
-#define GWC_KDE_LAUNCH(NodeT, LosT)                                                                              \
-  do {                                                                                                           \
-    if (cudaFuncSetAttribute(kde_kernel<NodeT, LosT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != \
-        cudaSuccess)                                                                                             \
-      return -1;                                                                                                 \
-    kde_kernel<NodeT, LosT><<<(unsigned)blocks, KDE_THREADS, smem, s>>>(p);                                      \
+#define GWC_KDE_LAUNCH1(NodeT, LosT, MP)                                                                              \
+  do {                                                                                                                \
+    if (cudaFuncSetAttribute(kde_kernel<NodeT, LosT, MP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != \
+        cudaSuccess)                                                                                                  \
+      return -1;                                                                                                      \
+    kde_kernel<NodeT, LosT, MP><<<(unsigned)blocks, KDE_THREADS, smem, s>>>(p);                                      \
+  } while (0)
+#define GWC_KDE_LAUNCH(NodeT, LosT)                   \
+  do {                                                \
+    if (model == 1) GWC_KDE_LAUNCH1(NodeT, LosT, true); \
+    else GWC_KDE_LAUNCH1(NodeT, LosT, false);           \
   } while (0)
   if (tab_prec == GWC_F64) {
     if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node64, double); else GWC_KDE_LAUNCH(Node64, float);
@@ -641,6 +646,7 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
     if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node32, double); else GWC_KDE_LAUNCH(Node32, float);
   }
 #undef GWC_KDE_LAUNCH
+#undef GWC_KDE_LAUNCH1
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
