@@ -36,18 +36,18 @@ UNIT = "terms/s"
 # FP64-pipe instructions per term of THIS formulation.  NECESSARY (what a live / a dead term needs: DESIGN.md section 7,
 # counted from the SASS of the main loop) is what `roofline.frac` uses; EXECUTED is what the shipped event kernel runs
 # per term, live or dead, MEASURED by ncu (sass__thread_inst_executed_true_per_opcode: DFMA + DADD + DMUL + DSETP over
-# the terms of one 340-theta launch of the O5 catalogue; profiles/r02a_reweight_events_ncu_full.md).  Re-measure
+# the terms of one 340-theta launch of the O5 catalogue; profiles/r02e_reweight_events_ncu_full.md).  Re-measure
 # after any edit of the kernel: the profile names the command.
 FP64_INSTR_LIVE = 104.0
 FP64_INSTR_DEAD = 28.0
 FP64_INSTR_EXECUTED = 108.26
-FP64_COUNT_SOURCE = "necessary: static SASS count of the main loop (DESIGN.md 7); executed: ncu op counters, profiles/r02a_reweight_events_ncu_full.md"
+FP64_COUNT_SOURCE = "necessary: static SASS count of the main loop (DESIGN.md 7); executed: ncu op counters, profiles/r02e_reweight_events_ncu_full.md"
 # the KDE kernel: FP64 thread instructions per Gaussian evaluation, everything included (per-sample weights, per-pixel
-# statistics, prior), measured the same way (profiles/r02d_kde_kernel_ncu_full.md)
-KDE_FP64_INSTR_PER_EVAL = 4.95
+# statistics, prior), measured the same way (profiles/r02e_kde_ncu_full.md)
+KDE_FP64_INSTR_PER_EVAL = 4.87
 # DRAM bytes of one 340-theta launch of the event kernel on the O5 catalogue (ncu dram__bytes_read.sum +
 # dram__bytes_write.sum, same capture)
-O5_DRAM_BYTES_PER_340_THETA = 7.301e9 + 0.078e9
+O5_DRAM_BYTES_PER_340_THETA = 7.247e9 + 0.068e9
 # B200 FP64 issue peak derived from the unit counts: 148 SMs x 64 FP64 lanes x 1.965 GHz
 FP64_PEAK_INSTR = 148 * 64 * 1.965e9
 
@@ -208,10 +208,15 @@ def run_gwc(args):
     t_gen = time.time()
     W = synth.make_workload(spec, seed=args.seed, device=dev, keep_f64_los=False)
     # every rank owns a full-size theta batch of its own (weak scaling over theta)
-    theta = synth.make_theta(spec, args.seed + 7919 * rank, dev)
+    mp = args.mass_model == "multipeak"
+    theta = (synth.make_theta_multipeak if mp else synth.make_theta)(spec, args.seed + 7919 * rank, dev)
     torch.cuda.synchronize()
     t_gen = time.time() - t_gen
     ctx = gwc.Context(local)
+    if mp:
+        # MULTIPEAK with delta_m smoothing (NEXT row 3a): 16-column theta rows; mmin = 4.6 keeps the catalogue's masses
+        # (drawn from a population that starts at 5 Msun) inside the support
+        ctx.gwc_set_mass_model("multipeak")
     zmax = spec.z_max
     prec = gwc.F32 if args.table_prec == "f32" else gwc.F64
     allsky = ctx.gwc_los_allsky(W.los, zmax)
@@ -294,7 +299,9 @@ def run_gwc(args):
     # ---- roofline of the dominant kernel (event re-weighting), timed live with CUDA events on its stream ----
     ms_ev_kernel = tm["ms_ev"] / max(tm["n_ev"], 1)
     ms_inj_kernel = tm["ms_inj"] / max(tm["n_inj"], 1)
-    instr = terms_ev * (live_frac_ev * FP64_INSTR_LIVE + (1.0 - live_frac_ev) * FP64_INSTR_DEAD)
+    # (MULTIPEAK: + 42 FP64 instructions per live term, static count of the added code, R36)
+    instr_live = FP64_INSTR_LIVE + (42.0 if mp else 0.0)
+    instr = terms_ev * (live_frac_ev * instr_live + (1.0 - live_frac_ev) * FP64_INSTR_DEAD)
     achieved = instr * 2.0 / (ms_ev_kernel * 1e-3) / 1e12          # FP64 issue slots x 2 flop
     peak = FP64_PEAK_INSTR * 2.0 / 1e12
     probe_ms, probe_n = ctx.gwc_probe_fp64(1 << 13)
@@ -303,15 +310,15 @@ def run_gwc(args):
     traffic = O5_DRAM_BYTES_PER_340_THETA * n_theta / 340.0 if spec.name == "o5" and args.table_prec == "f64" else None
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of one 340-theta "
-                "launch, profiles/r02a_reweight_events_ncu_full.md, scaled to the step's launches (HBM does not bind)"
+                "launch, profiles/r02e_reweight_events_ncu_full.md, scaled to the step's launches (HBM does not bind)"
                 if traffic else None, "kernel": "reweight_kernel<events>", "kernel_ms": ms_ev_kernel,
                 "kernel_share_of_step": ms_ev_kernel / (ms / args.steps),
                 "inj_kernel_ms": ms_inj_kernel,
-                "fp64_instr_per_live_term": FP64_INSTR_LIVE, "fp64_instr_per_dead_term": FP64_INSTR_DEAD,
+                "fp64_instr_per_live_term": instr_live, "fp64_instr_per_dead_term": FP64_INSTR_DEAD,
                 # the instructions the kernel executes per term (ncu-measured), against the same peak: the FP64 pipe's
                 # utilisation as the run itself sees it
-                "fp64_instr_executed_per_term": FP64_INSTR_EXECUTED,
-                "frac_executed": terms_ev * FP64_INSTR_EXECUTED / (ms_ev_kernel * 1e-3) / FP64_PEAK_INSTR,
+                "fp64_instr_executed_per_term": None if mp else FP64_INSTR_EXECUTED,
+                "frac_executed": None if mp else terms_ev * FP64_INSTR_EXECUTED / (ms_ev_kernel * 1e-3) / FP64_PEAK_INSTR,
                 "fp64_count_source": FP64_COUNT_SOURCE,
                 # the same time against the budget BASELINE.md froze before any code (180 live / 30 dead): context only
                 "frac_at_survey_budget_180_30": terms_ev * (live_frac_ev * 180.0 + (1.0 - live_frac_ev) * 30.0)
@@ -359,7 +366,7 @@ def run_gwc(args):
                "event_terms_per_s": th_k.shape[0] * n_samples / (ms_kde * 1e-3),
                "gaussian_evals_per_s": evals / (ms_kde * 1e-3),
                "fp64_instr_per_eval": KDE_FP64_INSTR_PER_EVAL,
-               "fp64_count_source": "ncu op counters over the Gaussian evaluations of the launch, profiles/r02d_kde_kernel_ncu_full.md",
+               "fp64_count_source": "ncu op counters over the Gaussian evaluations of the launch, profiles/r02e_kde_ncu_full.md",
                "roofline_frac_fp64": evals * KDE_FP64_INSTR_PER_EVAL / (ms_kde * 1e-3) / FP64_PEAK_INSTR,
                # (round 1 counted 10 instructions per evaluation for the kernel of that round: the same time on that scale)
                "roofline_frac_fp64_at_r01_count_10": evals * 10.0 / (ms_kde * 1e-3) / FP64_PEAK_INSTR}
@@ -395,13 +402,14 @@ def run_gwc(args):
         finally:
             ctx.gwc_cache_catalogue(False)
     a0 = a0_report(ctx, W, spec, args.seed) if args.a0 else None
-    cpu = cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
+    cpu = (cpu_baseline(spec, args.seed, W=W, theta=theta, budget_s=args.cpu_seconds, mass_model=args.mass_model)
+           if args.cpu_seconds > 0 else None)
     stress = stress_report(ctx, W, theta, zmax, allsky, args.n_nodes) if spec.name == "stress" else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": spec.name, "n_theta": n_theta, "n_events": spec.n_events, "n_samples": n_samples,
+        "config": {"workload": spec.name, "mass_model": args.mass_model, "n_theta": n_theta, "n_events": spec.n_events, "n_samples": n_samples,
                    "n_injections": n_inj, "los_rows": spec.los_rows, "n_z": spec.n_z, "los_dtype": spec.los_dtype,
                    "cosmo_table": "%s x %d nodes" % (args.table_prec, args.n_nodes), "seed": args.seed,
                    "parallelism": "theta-sharded x%d, catalogue replicated" % world,
@@ -503,10 +511,15 @@ def stress_report(ctx, W, theta, zmax, allsky, n_nodes):
 
 
 # ---------------------------------------------------------------------------------------------
-def cpu_baseline(spec, seed, W=None, theta=None, budget_s=15.0):
+def cpu_baseline(spec, seed, W=None, theta=None, budget_s=15.0, mass_model="plpeak"):
     """The oracle as it stands, on the host cores, on a bounded sample of the workload:
     the first theta points x the first events (all their samples) + the same theta x a slice of injections."""
     import oracle
+    with oracle.mass_model(mass_model):
+        return _cpu_baseline(oracle, spec, seed, W, theta, budget_s)
+
+
+def _cpu_baseline(oracle, spec, seed, W, theta, budget_s):
     if W is None:
         small = synth.scaled(spec, n_events=min(spec.n_events, 64), n_inj=min(spec.n_inj, 50_000),
                              los_rows=min(spec.los_rows, 4096))
@@ -607,6 +620,8 @@ def main():
     ap.add_argument("--leg", default="all", choices=["all", "events", "pixcut", "kde", "inj"],
                     help="run one leg alone and print its kernel time (profiling runs)")
     ap.add_argument("--kde-bandwidth", default="scott")
+    ap.add_argument("--mass-model", default="plpeak", choices=["plpeak", "multipeak"],
+                    help="multipeak: the MULTIPEAK mass model with delta_m smoothing (16-column theta rows)")
     ap.add_argument("--no-a0", dest="a0", action="store_false",
                     help="skip the A0 line (gwc_pack_events + gwc_cap_pixels on the unsorted sample list)")
     ap.add_argument("--pixcut", type=float, default=2.0,
