@@ -62,6 +62,7 @@ struct gwc_ctx {
   double z_max = 0.0;
   // per-call scratch
   Buf seg_off, group_off, part_w, part_n, part_np, kde_scr, kde_len, allsky_scr, pack_scr, logL, logxi, probe;
+  Buf kde_cnt, kde_coff, kde_cstart, kde_cend, kde_cev, kde_thk, kde_gw, kde_pe, kde_pnp, kde_pnu;   // KDE chunks, partials
   HostCopy hc;
   // theta-independent preparation of the events [0] and the injections [1] (kept between calls when caching is on)
   PrepSet prep[2];
@@ -387,6 +388,8 @@ void gwc_destroy(gwc_ctx* ctx) {
                  &ctx->prep[1].P, &ctx->prep[1].seg_shift,
                  &ctx->pad.dLc, &ctx->pad.m1z, &ctx->pad.m2z, &ctx->pad.L1, &ctx->pad.Q, &ctx->pad.P, &ctx->pad.row,
                  &ctx->pad.seg_off, &ctx->pad.seg_pads,
+                 &ctx->kde_cnt, &ctx->kde_coff, &ctx->kde_cstart, &ctx->kde_cend, &ctx->kde_cev, &ctx->kde_thk, &ctx->kde_gw,
+                 &ctx->kde_pe, &ctx->kde_pnp, &ctx->kde_pnu,
                  &ctx->group_off, &ctx->part_w, &ctx->part_n, &ctx->part_np, &ctx->kde_scr, &ctx->kde_len, &ctx->allsky_scr, &ctx->pack_scr, &ctx->logL,
                  &ctx->logxi, &ctx->probe, &ctx->hc.theta, &ctx->hc.ev_off, &ctx->hc.ev_dL, &ctx->hc.ev_m1z,
                  &ctx->hc.ev_m2z, &ctx->hc.ev_lp, &ctx->hc.ev_row, &ctx->hc.inj_dL, &ctx->hc.inj_m1z,
@@ -608,15 +611,34 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   const int64_t n = ev->n_samples, n_seg = ev->n_events;
   GWC_TRY(prepare_samples(ctx, ctx->prep[0], n, n_seg, ev->ev_sample_off, ev->dL, ev->m1z, ev->m2z, ev->log_pe_prior,
                           ev->sample_row, los->n_rows));
-  // scratch of the kernel: one slice of (z, v) pairs per resident warp, as long as the longest event
-  GWC_TRY(ensure(ctx, ctx->kde_len, sizeof(int64_t)));
-  GWC_TRY(count(ctx, launch_max_segment(ev->ev_sample_off, ev->n_events, (int64_t*)ctx->kde_len.p, s), "max_segment"));
-  int64_t max_len = 0;
+  // work units are (chunk, theta): the chunk table of the catalogue (runs of whole pixels of about 1024 samples), then
+  // one host synchronisation for its size and the longest chunk (the scratch slice of a warp)
+  const int64_t nc_max = kde_chunk_bound(n, n_seg);
+  GWC_TRY(ensure(ctx, ctx->kde_len, 2 * sizeof(int64_t)));
+  GWC_TRY(ensure(ctx, ctx->kde_cnt, (size_t)n_seg * sizeof(int64_t)));
+  GWC_TRY(ensure(ctx, ctx->kde_coff, (size_t)(n_seg + 1) * sizeof(int64_t)));
+  GWC_TRY(ensure(ctx, ctx->kde_cstart, (size_t)nc_max * sizeof(int64_t)));
+  GWC_TRY(ensure(ctx, ctx->kde_cend, (size_t)nc_max * sizeof(int64_t)));
+  GWC_TRY(ensure(ctx, ctx->kde_cev, (size_t)nc_max * sizeof(int32_t)));
+  GWC_CUDA(cudaMemsetAsync(ctx->kde_len.p, 0, 2 * sizeof(int64_t), s));
+  GWC_TRY(count(ctx, launch_kde_chunks(ev->ev_sample_off, n_seg, ev->sample_row, (int64_t*)ctx->kde_cnt.p,
+                                       (int64_t*)ctx->kde_coff.p, (int64_t*)ctx->kde_cstart.p, (int64_t*)ctx->kde_cend.p,
+                                       (int32_t*)ctx->kde_cev.p, (int64_t*)ctx->kde_len.p, s),
+                "kde_chunks"));
+  int64_t max_len = 0, n_chunks = 0;
   GWC_CUDA(cudaMemcpyAsync(&max_len, ctx->kde_len.p, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+  GWC_CUDA(cudaMemcpyAsync(&n_chunks, (const int64_t*)ctx->kde_coff.p + n_seg, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
   GWC_CUDA(cudaStreamSynchronize(s));
-  if (max_len < 0 || max_len > ev->n_samples) return fail(ctx, GWC_ERR_SHAPE, "ev_sample_off is not ascending");
-  const int n_blocks = kde_grid_blocks(n_theta, ev->n_events, ctx->n_sm);
+  if (max_len < 0 || max_len > n || n_chunks < 0 || n_chunks > nc_max)
+    return fail(ctx, GWC_ERR_SHAPE, "ev_sample_off is not ascending");
+  const int n_blocks = kde_grid_blocks(n_theta, n_chunks, ctx->n_sm);
   GWC_TRY(ensure(ctx, ctx->kde_scr, kde_scratch_bytes(n_blocks, max_len)));
+  GWC_TRY(ensure(ctx, ctx->kde_thk, kde_theta_bytes(n_theta)));
+  GWC_TRY(ensure(ctx, ctx->kde_gw, kde_weight_bytes(n_theta)));
+  const size_t n_part = (size_t)n_theta * (size_t)(n_chunks > 0 ? n_chunks : 1);
+  GWC_TRY(ensure(ctx, ctx->kde_pe, n_part * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->kde_pnp, n_part * sizeof(int32_t)));
+  GWC_TRY(ensure(ctx, ctx->kde_pnu, n_part * sizeof(int64_t)));
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (ctx->timing) {   // (taken after the last step that can fail before the launch: nothing leaks on an error return)
     e0 = get_event(ctx);
@@ -629,7 +651,11 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
                                 ev->m1z, ev->m2z, ev->log_pe_prior, ev->sample_row, (const double*)ctx->prep[0].seg_shift.p,
                                 los->table, los->prec, los->n_rows, los->n_z, los->z_max, n_grid, neff_min, bw_rule,
                                 d_logL,
-                                d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, ctx->d_flag, s),
+                                d_npass, d_nused, ctx->kde_scr.p, max_len > 0 ? max_len : 1, n_blocks, n_chunks,
+                                (const int64_t*)ctx->kde_coff.p, (const int64_t*)ctx->kde_cstart.p,
+                                (const int64_t*)ctx->kde_cend.p, (const int32_t*)ctx->kde_cev.p, ctx->kde_thk.p,
+                                ctx->kde_gw.p, (double*)ctx->kde_pe.p, (int32_t*)ctx->kde_pnp.p, (int64_t*)ctx->kde_pnu.p,
+                                ctx->d_flag, s),
                 "kde");
   if (ctx->timing) {
     cudaEventRecord(e1, s);

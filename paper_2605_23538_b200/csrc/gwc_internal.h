@@ -182,9 +182,18 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
                int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks,
-               int* d_flag, cudaStream_t s);
-int kde_grid_blocks(int64_t n_theta, int64_t n_events, int n_sm);
-size_t kde_scratch_bytes(int n_blocks, int64_t max_event_len);
+               int64_t n_chunks, const int64_t* d_chunk_off, const int64_t* d_start, const int64_t* d_end,
+               const int32_t* d_event, void* d_thk, void* d_gw, double* d_part_e, int32_t* d_part_np,
+               int64_t* d_part_nu, int* d_flag, cudaStream_t s);
+// KDE work units are (chunk, theta): the chunk table of a catalogue (runs of whole pixels, about 1024 samples)
+int64_t kde_chunk_bound(int64_t n_samples, int64_t n_events);
+int launch_kde_chunks(const int64_t* ev_off, int64_t n_events, const int32_t* row, int64_t* d_cnt,
+                      int64_t* d_chunk_off, int64_t* d_start, int64_t* d_end, int32_t* d_event, int64_t* d_max_len,
+                      cudaStream_t s);
+size_t kde_theta_bytes(int64_t n_theta);
+size_t kde_weight_bytes(int64_t n_theta);
+int kde_grid_blocks(int64_t n_theta, int64_t n_chunks, int n_sm);
+size_t kde_scratch_bytes(int n_blocks, int64_t max_chunk_len);
 int launch_max_segment(const int64_t* seg_off, int64_t n_seg, int64_t* d_out, cudaStream_t s);
 int launch_probe_fp64(int64_t iters, int n_blocks, double* d_sink, cudaStream_t s, double* n_instr);
 int launch_math_selftest(int which, int64_t n, const double* d_in, double* d_out, cudaStream_t s);

@@ -59,6 +59,18 @@ struct KdeParams {
   int64_t* npass;           // [n_theta][n_events] or NULL
   int64_t* nused;           // [n_theta][n_events] or NULL: live samples of the contributing pixels
   int* flag;                // sticky device flag word (written by -DGWC_CHECKED builds only)
+  // Work units are (chunk, theta): a chunk is a run of whole pixels of one event, about KDE_CHUNK samples long
+  // (theta-independent; kde_chunk_* kernels).  Chunks keep the (z, v) scratch slice of a warp small enough to stay in
+  // L2 and split the long events of a ragged catalogue over many warps.
+  const struct ThetaK* thk; // [n_theta] per-theta values (kde_theta_prep_kernel)
+  const struct NodeW* gw;   // [n_theta][32 * KDE_NPL] prior weights at the grid nodes
+  int64_t n_chunks;
+  const int64_t *chunk_start, *chunk_end;   // [n_chunks]
+  const int32_t* chunk_event;               // [n_chunks]
+  const int64_t* chunk_off;                 // [n_events + 1] chunks of each event
+  double* part_e;           // [n_theta][n_chunks] sum of I_j over the chunk's contributing pixels, relative to e^shift
+  int32_t* part_np;         // [n_theta][n_chunks] contributing pixels
+  int64_t* part_nu;         // [n_theta][n_chunks] their live samples
 };
 
 __device__ __forceinline__ double wsum(double v) {
@@ -385,14 +397,137 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
   return part;
 }
 
+#ifndef GWC_KDE_CHUNK
+#define GWC_KDE_CHUNK 1024
+#endif
+constexpr int KDE_CHUNK = GWC_KDE_CHUNK;   // target samples per chunk (a pixel is never split)
+
+// ---- chunks: runs of whole pixels of one event, cut at the first pixel start at or after every KDE_CHUNK samples ----
+__global__ void kde_chunk_count_kernel(const int64_t* __restrict__ ev_off, int64_t n_events, int64_t* __restrict__ cnt) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n_events) cnt[i] = (ev_off[i + 1] - ev_off[i] + KDE_CHUNK - 1) / KDE_CHUNK;
+}
+// exclusive scan in order (single CTA); off[n] = total
+__global__ void kde_chunk_scan_kernel(const int64_t* __restrict__ cnt, int64_t n, int64_t* __restrict__ off) {
+  __shared__ long long part[256];
+  __shared__ long long carry;
+  const int tid = threadIdx.x;
+  if (tid == 0) carry = 0;
+  __syncthreads();
+  for (int64_t base = 0; base <= n; base += 256) {
+    const int64_t i = base + tid;
+    part[tid] = i < n ? cnt[i] : 0;
+    __syncthreads();
+    if (tid == 0) {
+      long long run = carry;
+      for (int j = 0; j < 256; ++j) {
+        const long long v = part[j];
+        part[j] = run;
+        run += v;
+      }
+      carry = run;
+    }
+    __syncthreads();
+    if (i <= n) off[i] = part[tid];
+    __syncthreads();
+  }
+}
+// first pixel start at or after position k of the event [s0, s1) (s1 when there is none)
+__device__ __forceinline__ int64_t next_pixel_start(const int32_t* __restrict__ row, int64_t s0, int64_t s1, int64_t k) {
+  if (k <= s0) return s0;
+  while (k < s1 && row[k] == row[k - 1]) ++k;
+  return k < s1 ? k : s1;
+}
+__global__ void kde_chunk_bounds_kernel(const int64_t* __restrict__ ev_off, int64_t n_events,
+                                        const int64_t* __restrict__ chunk_off, const int32_t* __restrict__ row,
+                                        int64_t* __restrict__ c_start, int64_t* __restrict__ c_end,
+                                        int32_t* __restrict__ c_event, int64_t* __restrict__ max_len) {
+  const int64_t ev = blockIdx.x;
+  const int64_t s0 = ev_off[ev], s1 = ev_off[ev + 1];
+  const int64_t c0 = chunk_off[ev], nc = chunk_off[ev + 1] - c0;
+  long long mx = 0;
+  for (int64_t c = threadIdx.x; c < nc; c += blockDim.x) {
+    const int64_t a = next_pixel_start(row, s0, s1, s0 + c * KDE_CHUNK);
+    const int64_t b = c + 1 < nc ? next_pixel_start(row, s0, s1, s0 + (c + 1) * KDE_CHUNK) : s1;
+    c_start[c0 + c] = a;
+    c_end[c0 + c] = b;
+    c_event[c0 + c] = (int32_t)ev;
+    mx = b - a > mx ? b - a : mx;
+  }
+  if (mx > 0) atomicMax(reinterpret_cast<long long*>(max_len), mx);
+}
+
+// ---- per-theta values and prior weights, once per call (one warp per theta) ----
+template <bool MP>
+__global__ void __launch_bounds__(32) kde_theta_prep_kernel(const KdeParams p, ThetaK* __restrict__ thk,
+                                                            NodeW* __restrict__ gw) {
+  const int64_t t = blockIdx.x;
+  const int lane = threadIdx.x;
+  const int G = p.n_grid;
+  const double dzg = p.los_zmax / (G - 1);
+  const double dzl = p.los_zmax / (p.n_z - 1);
+  const double* th = p.theta + t * (MP ? GWC_NPAR_MULTIPEAK : GWC_NPAR);
+  const double* tcr = p.tconst + t * nconst_of(MP ? 1 : 0);
+  ThetaK K;
+  {
+    const double H0 = th[0], alpha = th[2], beta = th[3], mmin = th[4], mmax = th[5], mu = th[6], sigma = th[7],
+                 lam = th[8];
+    K.h0c = H0 / C_KMS_KDE;
+    K.cH = C_KMS_KDE / H0;
+    K.umax = tcr[C_UMAX];
+    K.invdu = tcr[C_INVDU];
+    K.mmin = mmin; K.mmax = mmax; K.alpha = alpha; K.beta = beta; K.mu = mu; K.sigma = sigma;
+    const double n_pl = (1.0 - alpha) / (pow(mmax, 1.0 - alpha) - pow(mmin, 1.0 - alpha));
+    const double rs2 = 1.0 / (sigma * 1.41421356237309504880);
+    const double n_g = 1.0 / (0.5 * (erf((mmax - mu) * rs2) - erf((mmin - mu) * rs2)));
+    K.a_pl = (1.0 - lam) * n_pl;
+    K.a_g = lam * n_g / (sigma * 2.50662827463100050242);
+    K.bp1 = beta + 1.0;
+    K.mminb = pow(mmin, beta + 1.0);
+    K.Om = th[1];
+    K.OL = 1.0 - th[1];
+    K.mp = MP;
+    K.a_gl = 0.0; K.mul = 0.0; K.sigl = 1.0; K.dm = 0.0; K.fidx = 0.0; K.ctop = 0.0; K.topb = K.mminb; K.ftab = nullptr;
+    if (MP) {
+      const double dm = th[12], laml = th[15], iN1 = 1.0 / tcr[C_N1];
+      K.a_pl *= iN1;
+      K.a_g *= (1.0 - laml) * iN1;
+      K.a_gl = lam * laml * tcr[C_NGL] / (th[14] * 2.50662827463100050242) * iN1;
+      K.mul = th[13]; K.sigl = th[14]; K.dm = dm; K.fidx = tcr[C_FIDX]; K.ctop = tcr[C_CTOP];
+      K.topb = pow(mmin + dm, beta + 1.0);
+      K.ftab = p.ftab + (size_t)t * MF_PITCH;
+    }
+  }
+  if (lane == 0) thk[t] = K;
+  // prior weights at the grid nodes: c_g psi(z_g) / (1 + z_g) (trapezoid weight, reading R4) split over the two LOS
+  // nodes around z_g (the table's own linear interpolation, R10); stored [i][lane] for node kde_node(lane, i)
+  const double gam = th[9], kap = th[10], zp = th[11];
+  const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
+#pragma unroll 1
+  for (int i = 0; i < KDE_NPL; ++i) {
+    const int g = kde_node(lane, i);
+    const double zg = fmin(g * dzg, p.los_zmax);
+    const double tz = zg / dzl;
+    int b = (int)floor(tz);
+    b = b > p.n_z - 2 ? p.n_z - 2 : b;
+    const double fz = tz - (double)b;
+    const double x = 1.0 + g * dzg;
+    const double psi = psi0 * pow(x, gam) / (1.0 + pow(x / (1.0 + zp), gam + kap));
+    const double c = (g == 0 || g == G - 1) ? 0.5 * dzg : dzg;
+    const double w = g < G ? c * psi / x : 0.0;
+    NodeW nw;
+    nw.w0 = w * (1.0 - fz);
+    nw.w1 = w * fz;
+    gw[(size_t)t * (32 * KDE_NPL) + i * 32 + lane] = nw;
+  }
+}
+
 template <typename NodeT, typename LosT, bool MP>
 __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) {
   extern __shared__ __align__(16) unsigned char kde_smem[];
   MathTables& mt = *reinterpret_cast<MathTables*>(kde_smem);
-  // prior weights at the grid nodes, one set per warp (they depend on theta), and the LOS bin of every grid node
-  NodeW* s_w = reinterpret_cast<NodeW*>(kde_smem + sizeof(MathTables)) + (threadIdx.x >> 5) * (32 * KDE_NPL);
-  int* s_b = reinterpret_cast<int*>(kde_smem + sizeof(MathTables) + sizeof(NodeW) * KDE_WARPS * 32 * KDE_NPL);
-  double* s_fz = reinterpret_cast<double*>(s_b + 32 * KDE_NPL);
+  // the LOS bin of every grid node
+  int* s_b = reinterpret_cast<int*>(kde_smem + sizeof(MathTables));
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   init_math_tables(mt, tid, KDE_THREADS);
   __syncthreads();
@@ -402,80 +537,31 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
   const int G = p.n_grid;
   const double dzg = p.los_zmax / (G - 1);
   const double dzl = p.los_zmax / (p.n_z - 1);
-  const int64_t n_units = p.n_theta * p.n_events;
-  if (tid < 32 * KDE_NPL) {   // LOS bin and fraction of grid node g = kde_node(l, i), stored at [i][l]
+  const int64_t n_units = p.n_theta * p.n_chunks;
+  if (tid < 32 * KDE_NPL) {   // LOS bin of grid node g = kde_node(l, i), stored at [i][l]
     const int l = tid & 31, i = tid >> 5, g = kde_node(l, i);
     const double zg = fmin(g * dzg, p.los_zmax);
-    const double tz = zg / dzl;
-    int b = (int)floor(tz);
+    int b = (int)floor(zg / dzl);
     b = b > p.n_z - 2 ? p.n_z - 2 : b;
     s_b[i * 32 + l] = b;
-    s_fz[i * 32 + l] = tz - (double)b;
   }
   __syncthreads();
 
   for (int64_t unit = (int64_t)blockIdx.x * KDE_WARPS + warp; unit < n_units; unit += (int64_t)gridDim.x * KDE_WARPS) {
-    const int64_t ev = unit / p.n_theta, t = unit - ev * p.n_theta;   // event-major
-    const int64_t s0 = p.ev_off[ev], s1 = p.ev_off[ev + 1];
-    const size_t o = (size_t)t * (size_t)p.n_events + (size_t)ev;
-    const double* th = p.theta + t * (p.model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR);
-    const double* tcr = p.tconst + t * nconst_of(p.model);
-    if (!(p.tvalid[t] == 1.0)) {   // theta outside the domain or changed since the build: NaN (sticky flag set)
+    const int64_t chunk = unit / p.n_theta, t = unit - chunk * p.n_theta;   // chunk-major: a CTA's warps share samples
+    const int64_t ev = p.chunk_event[chunk];
+    const int64_t s0 = p.chunk_start[chunk], s1 = p.chunk_end[chunk];
+    const size_t o = (size_t)t * (size_t)p.n_chunks + (size_t)chunk;
+    if (!(p.tvalid[t] == 1.0) || s1 <= s0) {   // (an invalid theta gets its NaN in the combine)
       if (lane == 0) {
-        p.logL[o] = CUDART_NAN;
-        if (p.npass) p.npass[o] = 0;
-        if (p.nused) p.nused[o] = 0;
+        p.part_e[o] = 0.0;
+        p.part_np[o] = 0;
+        p.part_nu[o] = 0;
       }
       continue;
     }
-    // ---- per-theta values (every lane computes them: no divergence, no broadcast) ----
-    ThetaK K;
-    {
-      const double H0 = th[0], alpha = th[2], beta = th[3], mmin = th[4], mmax = th[5], mu = th[6], sigma = th[7],
-                   lam = th[8];
-      K.h0c = H0 / C_KMS_KDE;
-      K.cH = C_KMS_KDE / H0;
-      K.umax = tcr[C_UMAX];
-      K.invdu = tcr[C_INVDU];
-      K.mmin = mmin; K.mmax = mmax; K.alpha = alpha; K.beta = beta; K.mu = mu; K.sigma = sigma;
-      const double n_pl = (1.0 - alpha) / (pow(mmax, 1.0 - alpha) - pow(mmin, 1.0 - alpha));
-      const double rs2 = 1.0 / (sigma * 1.41421356237309504880);
-      const double n_g = 1.0 / (0.5 * (erf((mmax - mu) * rs2) - erf((mmin - mu) * rs2)));
-      K.a_pl = (1.0 - lam) * n_pl;
-      K.a_g = lam * n_g / (sigma * 2.50662827463100050242);
-      K.bp1 = beta + 1.0;
-      K.mminb = pow(mmin, beta + 1.0);
-      K.Om = th[1];
-      K.OL = 1.0 - th[1];
-      K.mp = MP;
-      K.a_gl = 0.0; K.mul = 0.0; K.sigl = 1.0; K.dm = 0.0; K.fidx = 0.0; K.ctop = 0.0; K.topb = K.mminb; K.ftab = nullptr;
-      if (MP) {
-        const double dm = th[12], laml = th[15], iN1 = 1.0 / tcr[C_N1];
-        K.a_pl *= iN1;
-        K.a_g *= (1.0 - laml) * iN1;
-        K.a_gl = lam * laml * tcr[C_NGL] / (th[14] * 2.50662827463100050242) * iN1;
-        K.mul = th[13]; K.sigl = th[14]; K.dm = dm; K.fidx = tcr[C_FIDX]; K.ctop = tcr[C_CTOP];
-        K.topb = pow(mmin + dm, beta + 1.0);
-        K.ftab = p.ftab + (size_t)t * MF_PITCH;
-      }
-    }
-    // prior weights at this lane's grid nodes: c_g psi(z_g) / (1 + z_g) (trapezoid weight, reading R4) split over the
-    // two LOS nodes around z_g (the table's own linear interpolation, R10)
-    {
-      const double gam = th[9], kap = th[10], zp = th[11];
-      const double psi0 = 1.0 + pow(1.0 + zp, -(gam + kap));
-#pragma unroll
-      for (int i = 0; i < KDE_NPL; ++i) {
-        const int g = kde_node(lane, i);   // stored [i][lane]: conflict-free
-        const double x = 1.0 + g * dzg;
-        const double psi = psi0 * pow(x, gam) / (1.0 + pow(x / (1.0 + zp), gam + kap));
-        const double c = (g == 0 || g == G - 1) ? 0.5 * dzg : dzg;
-        const double w = g < G ? c * psi / x : 0.0;
-        const double fz = s_fz[i * 32 + lane];
-        s_w[i * 32 + lane].w0 = w * (1.0 - fz);
-        s_w[i * 32 + lane].w1 = w * fz;
-      }
-    }
+    const ThetaK K = p.thk[t];
+    const NodeW* s_w = p.gw + (size_t)t * (32 * KDE_NPL);
     __syncwarp();
     const NodeT* tab = reinterpret_cast<const NodeT*>(p.tab) + (size_t)t * p.Mp;
     const double shift = p.seg_shift[ev];
@@ -602,22 +688,68 @@ __global__ void __launch_bounds__(KDE_THREADS, 2) kde_kernel(const KdeParams p) 
     }
     esum = wsum(esum);
     if (lane == 0) {
-      p.logL[o] = (s1 > s0 && esum > 0.0) ? shift + log(esum) - log((double)(s1 - s0)) : -CUDART_INF;
-      if (p.npass) p.npass[o] = np;
-      if (p.nused) p.nused[o] = nu;
+      p.part_e[o] = esum;
+      p.part_np[o] = np;
+      p.part_nu[o] = nu;
     }
     __syncwarp();   // the scratch slice is rewritten by the next unit
   }
 }
 
+// log L_i = shift + ln(sum over the event's chunks, in order) - ln S_i; npass, nused summed the same way
+__global__ void kde_combine_kernel(const KdeParams p) {
+  const int64_t o = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (o >= p.n_theta * p.n_events) return;
+  const int64_t t = o / p.n_events, ev = o - t * p.n_events;
+  const int64_t S = p.ev_off[ev + 1] - p.ev_off[ev];
+  if (!(p.tvalid[t] == 1.0)) {   // theta outside the domain or changed since the build: NaN (sticky flag set)
+    p.logL[o] = CUDART_NAN;
+    if (p.npass) p.npass[o] = 0;
+    if (p.nused) p.nused[o] = 0;
+    return;
+  }
+  double e = 0.0;
+  int64_t np = 0, nu = 0;
+  for (int64_t c = p.chunk_off[ev]; c < p.chunk_off[ev + 1]; ++c) {
+    const size_t q = (size_t)t * (size_t)p.n_chunks + (size_t)c;
+    e += p.part_e[q];
+    np += p.part_np[q];
+    nu += p.part_nu[q];
+  }
+  p.logL[o] = (S > 0 && e > 0.0) ? p.seg_shift[ev] + log(e) - log((double)S) : -CUDART_INF;
+  if (p.npass) p.npass[o] = np;
+  if (p.nused) p.nused[o] = nu;
+}
+
 }  // namespace
+
+// upper bound of the number of chunks of a catalogue (what the chunk arrays are sized for)
+int64_t kde_chunk_bound(int64_t n_samples, int64_t n_events) { return n_samples / KDE_CHUNK + n_events + 1; }
+
+// chunk table of a catalogue: d_cnt [n_events] scratch, d_chunk_off [n_events + 1] (its last entry = number of
+// chunks), start / end / event [kde_chunk_bound], *d_max_len = longest chunk (must hold 0 before the call)
+int launch_kde_chunks(const int64_t* ev_off, int64_t n_events, const int32_t* row, int64_t* d_cnt,
+                      int64_t* d_chunk_off, int64_t* d_start, int64_t* d_end, int32_t* d_event, int64_t* d_max_len,
+                      cudaStream_t s) {
+  if (n_events <= 0) return 0;
+  kde_chunk_count_kernel<<<(unsigned)((n_events + 255) / 256), 256, 0, s>>>(ev_off, n_events, d_cnt);
+  kde_chunk_scan_kernel<<<1, 256, 0, s>>>(d_cnt, n_events, d_chunk_off);
+  kde_chunk_bounds_kernel<<<(unsigned)n_events, 64, 0, s>>>(ev_off, n_events, d_chunk_off, row, d_start, d_end, d_event,
+                                                            d_max_len);
+  return cudaGetLastError() == cudaSuccess ? 3 : -1;
+}
+
+size_t kde_theta_bytes(int64_t n_theta) { return (size_t)n_theta * sizeof(ThetaK); }
+size_t kde_weight_bytes(int64_t n_theta) { return (size_t)n_theta * 32 * KDE_NPL * sizeof(NodeW); }
 
 int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const void* d_tab, const double* d_tconst, const double* d_tvalid, int64_t n_theta, int M, int Mp,
                gwc_prec tab_prec, double tab_zq, int64_t n_events, const int64_t* ev_off, const double* dL,
                const double* m1z, const double* m2z, const double* lprior, const int32_t* row, const double* seg_shift,
                const void* los, gwc_prec los_prec, int64_t n_rows, int n_z, double los_zmax, int n_grid, double neff_min,
                int bw_rule, double* logL, int64_t* npass, int64_t* nused, void* scratch, int64_t scr_stride, int n_blocks,
-               int* d_flag, cudaStream_t s) {
+               int64_t n_chunks, const int64_t* d_chunk_off, const int64_t* d_start, const int64_t* d_end,
+               const int32_t* d_event, void* d_thk, void* d_gw, double* d_part_e, int32_t* d_part_np,
+               int64_t* d_part_nu, int* d_flag, cudaStream_t s) {
   if (n_theta <= 0 || n_events <= 0) return 0;
   KdeParams p;
   p.flag = d_flag;
@@ -626,8 +758,14 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
   p.row = row; p.seg_shift = seg_shift; p.los = los; p.n_rows = n_rows; p.n_z = n_z; p.los_zmax = los_zmax;
   p.n_grid = n_grid; p.neff_min = neff_min; p.bw_rule = bw_rule; p.logL = logL; p.npass = npass; p.nused = nused;
   p.scr = (double2*)scratch; p.scr_stride = scr_stride;
-  const size_t smem = sizeof(MathTables) + sizeof(NodeW) * KDE_WARPS * 32 * KDE_NPL + (sizeof(int) + sizeof(double)) * 32 * KDE_NPL;
+  p.thk = (const ThetaK*)d_thk; p.gw = (const NodeW*)d_gw; p.n_chunks = n_chunks; p.chunk_start = d_start;
+  p.chunk_end = d_end; p.chunk_event = d_event; p.chunk_off = d_chunk_off; p.part_e = d_part_e; p.part_np = d_part_np;
+  p.part_nu = d_part_nu;
+  if (model == 1) kde_theta_prep_kernel<true><<<(unsigned)n_theta, 32, 0, s>>>(p, (ThetaK*)d_thk, (NodeW*)d_gw);
+  else kde_theta_prep_kernel<false><<<(unsigned)n_theta, 32, 0, s>>>(p, (ThetaK*)d_thk, (NodeW*)d_gw);
+  const size_t smem = sizeof(MathTables) + sizeof(int) * 32 * KDE_NPL;
   const int64_t blocks = n_blocks;
+  if (n_chunks > 0) {
 #define GWC_KDE_LAUNCH1(NodeT, LosT, MP)                                                                              \
   do {                                                                                                                \
     if (cudaFuncSetAttribute(kde_kernel<NodeT, LosT, MP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != \
@@ -640,26 +778,29 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
     if (model == 1) GWC_KDE_LAUNCH1(NodeT, LosT, true); \
     else GWC_KDE_LAUNCH1(NodeT, LosT, false);           \
   } while (0)
-  if (tab_prec == GWC_F64) {
-    if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node64, double); else GWC_KDE_LAUNCH(Node64, float);
-  } else {
-    if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node32, double); else GWC_KDE_LAUNCH(Node32, float);
-  }
+    if (tab_prec == GWC_F64) {
+      if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node64, double); else GWC_KDE_LAUNCH(Node64, float);
+    } else {
+      if (los_prec == GWC_F64) GWC_KDE_LAUNCH(Node32, double); else GWC_KDE_LAUNCH(Node32, float);
+    }
 #undef GWC_KDE_LAUNCH
 #undef GWC_KDE_LAUNCH1
-  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+  }
+  const int64_t n_out = n_theta * n_events;
+  kde_combine_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, s>>>(p);
+  return cudaGetLastError() == cudaSuccess ? (n_chunks > 0 ? 3 : 2) : -1;
 }
 
-// grid of the KDE kernel (persistent, two CTAs of 8 warps per SM) and the scratch it needs: one slice of
-// `max_event_len` (z, v) pairs per resident warp
-int kde_grid_blocks(int64_t n_theta, int64_t n_events, int n_sm) {
-  const int64_t units = n_theta * n_events;
+// grid of the KDE kernel (persistent, two CTAs of 8 warps per SM) and the scratch it needs: one slice of the longest
+// chunk's (z, v) pairs per resident warp
+int kde_grid_blocks(int64_t n_theta, int64_t n_chunks, int n_sm) {
+  const int64_t units = n_theta * n_chunks;
   int64_t blocks = (units + KDE_WARPS - 1) / KDE_WARPS;
   if (blocks > (int64_t)n_sm * 2) blocks = (int64_t)n_sm * 2;
   return (int)(blocks < 1 ? 1 : blocks);
 }
-size_t kde_scratch_bytes(int n_blocks, int64_t max_event_len) {
-  return (size_t)n_blocks * KDE_WARPS * (size_t)(max_event_len > 0 ? max_event_len : 1) * sizeof(double2);
+size_t kde_scratch_bytes(int n_blocks, int64_t max_chunk_len) {
+  return (size_t)n_blocks * KDE_WARPS * (size_t)(max_chunk_len > 0 ? max_chunk_len : 1) * sizeof(double2);
 }
 
 }  // namespace gwc
