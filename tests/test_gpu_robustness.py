@@ -318,3 +318,79 @@ def test_nz_limit_checked_before_any_work(ctx):
     oL, _, oK = oracle.event_loglik(_np(W.theta), synth.to_numpy(W.ev), _np(los), 1.5)
     assert np.array_equal(_np(nlive), oK)
     assert_close_log(_np(logL), oL, RTOL_F64, "log L_i, n_z = 4097")
+
+
+def _structured_events(pattern, rows0=5):
+    """One event per entry of `pattern`; an entry is the list of its pixel sizes (runs of equal sample_row)."""
+    g = torch.Generator().manual_seed(17)
+    dl, m1, m2, row, off = [], [], [], [], [0]
+    for e, sizes in enumerate(pattern):
+        n = int(sum(sizes))
+        dl.append(900.0 * torch.exp(0.25 * torch.randn(n, generator=g, dtype=torch.float64)))
+        a = 42.0 * (1 + 0.07 * torch.randn(n, generator=g, dtype=torch.float64))
+        b = 31.0 * (1 + 0.07 * torch.randn(n, generator=g, dtype=torch.float64))
+        m1.append(torch.maximum(a, b))
+        m2.append(torch.minimum(a, b))
+        row.append(torch.repeat_interleave(torch.arange(len(sizes)) + rows0 + e, torch.tensor(sizes, dtype=torch.int64)))
+        off.append(off[-1] + n)
+    cat = lambda xs, dt: (torch.cat(xs).to(dt) if xs else torch.zeros(0, dtype=dt))
+    return {"ev_sample_off": torch.tensor(off, dtype=torch.int64), "dL": cat(dl, torch.float64), "m1z": cat(m1, torch.float64),
+            "m2z": cat(m2, torch.float64), "sample_row": cat(row, torch.int32), "log_pe_prior": None}
+
+
+def test_pixcut_and_kde_on_structured_pixel_patterns(ctx):
+    """The pixel-aligned padded copy (pixel-cut mode) and the chunk table (KDE) on run patterns chosen to hit their
+    corners: only odd runs (every pixel padded), only single samples, one pixel longer than several 64-sample blocks
+    and than a KDE chunk, runs that end exactly on block boundaries, an empty event in the middle, a one-sample
+    event, pixels of 63 / 64 / 65 / 127 / 129 samples."""
+    import oracle
+    from paper_2605_23538_b200 import synth
+    from util import RTOL_F64, assert_close_log
+    W = workload("o4", n_theta=6, n_events=2, los_rows=400, n_inj=100)
+    pattern = [[1, 3, 5, 7, 9, 11, 13], [1] * 40, [2600, 3, 1], [64, 64, 128, 2], [], [1], [63, 64, 65, 127, 129, 1, 2],
+               [2] * 33 + [1], [1100, 1100, 7]]
+    ev = _structured_events(pattern)
+    zmax = W.spec.z_max
+    th, evd, lo = W.theta.to(DEV), to_dev(ev, DEV), W.los.to(DEV)
+    ev_np = {k: (v.numpy() if isinstance(v, torch.Tensor) else v) for k, v in ev.items()}
+    ctx.gwc_build_cosmo(th, zmax)
+    for thr in (0.0, 2.0, 5.0):
+        gL, gN, gK, gP = ctx.gwc_event_loglik_pixcut(th, evd, lo, zmax, thr)
+        ctx.gwc_check()
+        oL, oN, oK, oP = oracle.event_loglik_pixcut(W.theta.numpy(), ev_np, W.los.numpy(), zmax, thr)
+        assert np.array_equal(gP.cpu().numpy(), oP) and np.array_equal(gK.cpu().numpy(), oK), thr
+        assert_close_log(gL.cpu().numpy(), oL, RTOL_F64, "pixel cut, structured patterns, threshold %g" % thr)
+    for bw in ("scott", "silverman"):
+        kL, kP, kU = ctx.gwc_event_loglik_kde(th, evd, lo, zmax, 256, 2.0, bw)
+        ctx.gwc_check()
+        rL, rP, rU = oracle.event_loglik_kde(W.theta.numpy(), ev_np, W.los.numpy(), zmax, n_grid=256, neff_min=2.0,
+                                             bandwidth=bw, want_nused=True)
+        assert np.array_equal(kP.cpu().numpy(), rP) and np.array_equal(kU.cpu().numpy(), rU), bw
+        assert_close_log(kL.cpu().numpy(), rL, RTOL_F64, "KDE, structured patterns, %s" % bw)
+    assert np.isneginf(gL.cpu().numpy()[:, 4]).all() and np.isneginf(kL.cpu().numpy()[:, 4]).all()   # the empty event
+
+
+def test_pixcut_with_cache_on_between_plain_and_cut_calls(ctx):
+    """gwc_cache_catalogue keeps the prepared samples AND their padded copy: plain, cut, plain, cut on one catalogue,
+    then another catalogue in other arrays: every result equals the uncached one bit for bit."""
+    Wa = workload("o4", n_theta=8, n_events=6, los_rows=400, n_inj=500)
+    Wb = workload("o4", n_theta=8, n_events=5, los_rows=400, n_inj=500, seed=3)
+    zmax = Wa.spec.z_max
+    ref = {}
+    for name, W in (("a", Wa), ("b", Wb)):
+        th, ev, lo = W.theta.to(DEV), to_dev(W.ev, DEV), W.los.to(DEV)
+        ctx.gwc_build_cosmo(th, zmax)
+        ref[name] = (th, ev, lo, ctx.gwc_event_loglik(th, ev, lo, zmax)[0].clone(),
+                     [x.clone() for x in ctx.gwc_event_loglik_pixcut(th, ev, lo, zmax, 2.0)])
+    ctx.gwc_cache_catalogue(True)
+    try:
+        for name in ("a", "a", "b", "a"):
+            th, ev, lo, plain, cut = ref[name]
+            ctx.gwc_build_cosmo(th, zmax)
+            for _ in range(2):
+                assert torch.equal(ctx.gwc_event_loglik(th, ev, lo, zmax)[0].view(torch.int64), plain.view(torch.int64))
+                got = ctx.gwc_event_loglik_pixcut(th, ev, lo, zmax, 2.0)
+                assert all(torch.equal(g.view(torch.int64), c.view(torch.int64)) for g, c in zip(got, cut))
+        ctx.gwc_check()
+    finally:
+        ctx.gwc_cache_catalogue(False)
