@@ -133,41 +133,58 @@ __global__ void finalize_inj_kernel(const double* __restrict__ part_w, const int
                                     const double* __restrict__ seg_shift, const double* __restrict__ tvalid,
                                     int64_t n_theta, int64_t n_seg, double n_draw, double* __restrict__ logxi,
                                     double* __restrict__ neff, int* __restrict__ flag) {
-  const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (t >= n_theta) return;
+  // one warp per theta: a lane takes the segments lane, lane + 32, .. in order, then a butterfly (a fixed order: the
+  // one-theta calls of a sampler spent a fifth of their time in the serial form of this loop)
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const int64_t t = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  if (t >= n_theta) return;   // (whole warps)
   const double valid = tvalid[t];
   if (valid != valid) {
-    logxi[t] = CUDART_NAN;
-    if (neff) neff[t] = CUDART_NAN;
+    if (lane == 0) {
+      logxi[t] = CUDART_NAN;
+      if (neff) neff[t] = CUDART_NAN;
+    }
     return;
   }
   const double* pw = part_w + 2 * t * n_seg;
   const int32_t* pn = part_n + t * n_seg;
   double smax = -CUDART_INF;
   bool range = false;
-  for (int64_t s = 0; s < n_seg; ++s) {
+  for (int64_t s = lane; s < n_seg; s += 32) {
     if (pw[2 * s] > 0.0) smax = fmax(smax, seg_shift[s]);
     range = range || (pn[s] > 0 && !(pw[2 * s] >= RANGE_MIN_SUM));
   }
-  if (range) {  // a segment whose live weights all lie below e^-300 of its reference (see finalize_events_kernel)
-    logxi[t] = CUDART_NAN;
-    if (neff) neff[t] = CUDART_NAN;
-    atomicOr(flag, FLAG_RANGE);
+  for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(FULL, smax, o));
+  if (__any_sync(FULL, range)) {  // a segment whose live weights all lie below e^-300 of its reference
+    if (lane == 0) {
+      logxi[t] = CUDART_NAN;
+      if (neff) neff[t] = CUDART_NAN;
+      atomicOr(flag, FLAG_RANGE);
+    }
     return;
   }
   if (!(smax > -CUDART_INF)) {
-    logxi[t] = -CUDART_INF;
-    if (neff) neff[t] = 0.0;
+    if (lane == 0) {
+      logxi[t] = -CUDART_INF;
+      if (neff) neff[t] = 0.0;
+    }
     return;
   }
   double a = 0.0, b = 0.0;
-  for (int64_t s = 0; s < n_seg; ++s) {
+  for (int64_t s = lane; s < n_seg; s += 32) {
     const double e = exp(seg_shift[s] - smax);
     a = fma(pw[2 * s], e, a);
     b = fma(pw[2 * s + 1], e * e, b);
   }
-  logxi[t] = (log(a) + smax) - log(n_draw);
-  if (neff) neff[t] = a * a / b;
+  for (int o = 16; o > 0; o >>= 1) {
+    a += __shfl_xor_sync(FULL, a, o);
+    b += __shfl_xor_sync(FULL, b, o);
+  }
+  if (lane == 0) {
+    logxi[t] = (log(a) + smax) - log(n_draw);
+    if (neff) neff[t] = a * a / b;
+  }
 }
 
 constexpr int TOT_THREADS = 128;
@@ -312,7 +329,7 @@ int launch_finalize_inj(const double* part_w, const int32_t* part_n, const doubl
                         int64_t n_theta, int64_t n_seg, double n_draw, double* logxi, double* neff, int* d_flag,
                         cudaStream_t s) {
   if (n_theta <= 0) return 0;
-  finalize_inj_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(part_w, part_n, seg_shift, tvalid, n_theta,
+  finalize_inj_kernel<<<(unsigned)((n_theta * 32 + 127) / 128), 128, 0, s>>>(part_w, part_n, seg_shift, tvalid, n_theta,
                                                                         n_seg, n_draw, logxi, neff, d_flag);
   return ok();
 }
