@@ -521,6 +521,70 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
         w_hi = min(s1, s0 + nb * (rw + 1) / NWARPS * BLK);
         w_step = BLK;
       }
+      if (ODD && nt == 1) {
+        // One theta point (the sampler's one-point-per-call pattern): there is no theta loop to hide the loads
+        // behind, so the pipeline runs across the warp's BLOCKS instead: the samples of the next block are requested
+        // before the second half of the current one is computed.  (warp-uniform branch; the tile is theta t0)
+        auto load_block = [&](int64_t c0, Sample<RowT>* sm) {
+#pragma unroll
+          for (int k = 0; k < SPT; ++k) {
+            const int64_t g = c0 + k * 32 + lane;
+            const bool in = g < w_hi;
+            GWC_DEV_CHECK(p.flag, !in || (g >= 0 && g < p.n_samples), FLAG_CHK_SAMPLE);
+            sm[k].A = make_double2(in ? p.dLc[g] : CUDART_NAN, in ? p.m1z[g] : 1.0);
+            sm[k].m2z = in ? p.m2z[g] : 1.0;
+            sm[k].C = make_double2(in ? p.L1[g] : 0.0, in ? p.Q[g] : 0.0);
+            sm[k].P = in ? p.P[g] : 0.0;
+            if (INJ) {
+              sm[k].lrow = reinterpret_cast<const RowT*>(s_allsky);
+            } else {
+              int32_t r = in ? p.row[g] : 0;
+              r = ((unsigned)r < (unsigned)p.n_rows) ? r : 0;
+              sm[k].lrow = reinterpret_cast<const RowT*>(p.los) + (size_t)r * (size_t)p.n_z;
+            }
+          }
+        };
+        const double* tc1 = KT + t0 * NC;
+        if (w_lo < w_hi) {
+          Sample<RowT> sa[SPT], sb[SPT];
+          Mid<RowT> cur[SPT];
+          load_block(w_lo, sa);
+#pragma unroll
+          for (int k = 0; k < SPT; ++k)
+            term_head<NodeT, RowT, !INJ, MP>(tc1, s_tab, sa[k].A, sa[k].m2z, sa[k].lrow, inv_dz, los_zmax, zq, bmax, cur[k],
+                                             p.flag, Mp);
+          double a0 = 0.0, a1 = 0.0;   // per-lane sums over the warp's blocks of this segment: one reduction at the end
+          int cnt = 0;
+          for (int64_t c0 = w_lo;;) {
+            const int64_t cn = c0 + w_step;
+            const bool more = cn < w_hi;   // warp-uniform
+            if (more) load_block(cn, sb);
+#pragma unroll
+            for (int k = 0; k < SPT; ++k) {
+              bool live;
+              const double w = term_tail<RowT, MP>(tc1, logtab, exptab, s_ftab, sa[k].C, sa[k].P, cur[k], live, p.flag);
+              a0 += w;
+              a1 = fma(w, w, a1);
+              cnt += live ? 1 : 0;
+            }
+            if (!more) break;
+#pragma unroll
+            for (int k = 0; k < SPT; ++k) {
+              term_head<NodeT, RowT, !INJ, MP>(tc1, s_tab, sb[k].A, sb[k].m2z, sb[k].lrow, inv_dz, los_zmax, zq, bmax, cur[k],
+                                               p.flag, Mp);
+              sa[k].C = sb[k].C;
+              sa[k].P = sb[k].P;
+            }
+            c0 = cn;
+          }
+          cnt = __reduce_add_sync(FULL, cnt);
+          if (cnt) {
+            const double k = warp_sum4(a0, a1, 0.0, 0.0, lane);
+            if ((lane & 23) == 0) acc_b[(warp * T) * 2 + ((lane >> 3) & 1)] += k;
+            if (lane == 0) cnt_b[warp * T] += cnt;
+          }
+        }
+      } else
       for (int64_t c0 = w_lo; c0 < w_hi; c0 += w_step) {
         Sample<RowT> sm[SPT];
         PixShape ps;
