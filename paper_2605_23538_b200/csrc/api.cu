@@ -261,7 +261,10 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
     n_tiles = (int)((n_theta + T - 1) / T);
   }
   // segment groups: enough work items to balance the SMs, small enough that a group's LOS rows stay in L2
-  int64_t target = (int64_t)((double)n * n_tiles / ((double)ctx->n_sm * 16.0));
+  // (a launch holds the tiles of at most KT_THETA points: the items that have to balance the SMs are those of ONE launch)
+  const int kt_cap = ((mp ? KT_THETA_MP : KT_THETA) / T) * T;
+  const int tiles_per_launch = n_tiles < kt_cap / T ? n_tiles : kt_cap / T;
+  int64_t target = (int64_t)((double)n * tiles_per_launch / ((double)ctx->n_sm * 16.0));
   if (target > 65536) target = 65536;
   if (target < 4096) target = 4096;
   while ((n / target + 2) * (int64_t)n_tiles > (int64_t)0x7fffffff) target *= 2;
