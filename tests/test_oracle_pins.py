@@ -1053,3 +1053,29 @@ def test_kde_biweight_bandwidth_through_quadratic_prior(theta0, rule):
         want = math.log(tot / (off[i + 1] - off[i]))
         assert Lk[0, i] == pytest.approx(want, abs=2e-6)
         assert abs(Ls[0, i] - Lk[0, i]) > 1e-4            # and it is not Scott's bandwidth
+
+
+def test_kde_kernel_underflow_rule(theta0):
+    """Reading R38: a Gaussian kernel value whose exponent is below -700 is zero.  A two-sample pixel that sits midway
+    between two grid nodes with a bandwidth far below the grid step contributes (and is counted in npass) while the
+    exponent at its nearest node is above -700, and neither contributes nor is counted once it is below; log L_i of
+    the event does not notice either way (the other pixel carries it)."""
+    th = _theta_unit_rate(theta0)
+    H0, Om = th[0], th[1]
+    zmax, G = 1.5, 64
+    dz = zmax / (G - 1)
+    zc = 20.5 * dz                                    # midway between nodes 20 and 21
+    tab = np.ones((2, 256))
+    res = {}
+    for name, g2 in (("above", 640.0), ("below", 770.0)):
+        h = 0.5 * dz / math.sqrt(2.0 * g2)            # exponent (d / h)^2 / 2 = g2 at the nearest nodes, d = dz / 2
+        delta = h / (1.06 * 2 ** -0.2)                # Scott: h = 1.06 sd 2^(-1/5), sd = delta for two equal weights
+        zs = np.array([zc - delta, zc + delta, 0.30, 0.34, 0.38, 0.42])
+        dl = np.array([O.dL(z, H0, Om) for z in zs])
+        ev = dict(ev_sample_off=np.array([0, 6], dtype=np.int64), dL=dl, m1z=np.full(6, 50.0), m2z=np.full(6, 38.0),
+                  sample_row=np.array([0, 0, 1, 1, 1, 1], np.int32), log_pe_prior=np.zeros(6))
+        res[name] = O.event_loglik_kde(th, ev, tab, zmax, n_grid=G, mode=O.EXACT, want_nused=True)
+    (La, Pa, Ua), (Lb, Pb, Ub) = res["above"], res["below"]
+    assert Pa[0, 0] == 2 and Ua[0, 0] == 6            # e^-640 at the nearest nodes: the pixel still counts
+    assert Pb[0, 0] == 1 and Ub[0, 0] == 4            # e^-770: it does not
+    assert La[0, 0] == pytest.approx(Lb[0, 0], abs=1e-12)
