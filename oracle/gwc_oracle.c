@@ -227,7 +227,7 @@ typedef struct {
 
 /* ---- MULTIPEAK with low-mass smoothing (readings R33-R36; the formula is not in the paper) ----------------
  *   S(m) = 0 (m <= mmin), 1 (m >= mmin + dm), else 1 / (1 + exp(dm/m' + dm/(m' - dm))), m' = m - mmin;
- *          a smoothing factor below e^-600 counts as 0 (R35)
+ *          a smoothing factor below e^-250 counts as 0 (R35)
  *   mix(m) = (1-lam) P(m) + lam lam_low G(m; mu_low, s_low) + lam (1-lam_low) G(m; mu_high, s_high),
  *            P = power law m^-alpha, G = Gaussian, each truncated to and normalised on [mmin, mmax]
  *   p(m1) = mix(m1) S(m1) / N1,   N1 = int mix S
@@ -238,7 +238,7 @@ double orc_mp_smooth(double m, double mmin, double dm) {
   if (mp >= dm) return 1.0;
   if (mp == 0.0) return 0.0;
   double e = dm / mp + dm / (mp - dm);
-  if (e > 600.0) return 0.0;
+  if (e > 250.0) return 0.0;
   return 1.0 / (1.0 + exp(e));
 }
 

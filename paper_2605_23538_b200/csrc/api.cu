@@ -269,8 +269,9 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   if (target < 4096) target = 4096;
   while ((n / target + 2) * (int64_t)n_tiles > (int64_t)0x7fffffff) target *= 2;
   const int n_groups = (int)(n > 0 ? (n + target - 1) / target : 1);
-  GWC_TRY(ensure(ctx, ctx->group_off, (size_t)(n_groups + 1) * sizeof(int32_t)));
-  GWC_TRY(count(ctx, launch_make_groups(d_seg_off, n_seg, target, n_groups, (int32_t*)ctx->group_off.p, s),
+  GWC_TRY(ensure(ctx, ctx->group_off, (size_t)(2 * n_groups + 1) * sizeof(int32_t)));   // offsets, then the order
+  int32_t* d_group_order = (int32_t*)ctx->group_off.p + n_groups + 1;
+  GWC_TRY(count(ctx, launch_make_groups(d_seg_off, n_seg, target, n_groups, (int32_t*)ctx->group_off.p, d_group_order, s),
                 "make_groups"));
   ReweightParams p;
   memset(&p, 0, sizeof(p));
@@ -292,6 +293,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.row = row;
   p.seg_off = d_seg_off;
   p.group_off = (const int32_t*)ctx->group_off.p;
+  p.group_order = d_group_order;
   p.n_groups = n_groups;
   p.n_seg = n_seg;
   p.los = los_table;

@@ -140,7 +140,7 @@ __device__ __forceinline__ double sample_v(const ThetaK& K, const NodeT* tab, in
     double S2 = 1.0;
     if (m2p < K.dm) {
       const double E = K.dm * fma(2.0, m2p, -K.dm) * rcp_fast(m2p * (m2p - K.dm));
-      if (!(E <= 600.0)) return -1.0;   // a smoothing factor below e^-600 is zero (R35)
+      if (!(E <= 250.0)) return -1.0;   // a smoothing factor below e^-250 is zero (R35)
       S2 = 1.0 / (1.0 + exp_fast<true>(E, exptab));
     }
     const double num2 = exp_fast<true>(K.beta * lm2, exptab) * S2;

@@ -295,10 +295,41 @@ int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const 
   return ok();
 }
 
+// Heaviest group first (longest-processing-time order of the work items): order[rank] = group, rank = the number of
+// groups with more samples (ties in group order, so equal groups keep the group-major order that keeps a group's LOS
+// rows in L2).  Catalogues whose groups are all within 25 % of the mean are left in catalogue order; a ragged one no
+// longer ends a launch on its heaviest items.
+__global__ void order_groups_kernel(const int64_t* __restrict__ seg_off, const int32_t* __restrict__ group_off,
+                                    int n_groups, int32_t* __restrict__ order) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n_groups) return;
+  const int64_t w = seg_off[group_off[g + 1]] - seg_off[group_off[g]];
+  int rank = 0;
+  int64_t wmax = 0;
+  for (int h = 0; h < n_groups; ++h) {
+    const int64_t wh = seg_off[group_off[h + 1]] - seg_off[group_off[h]];
+    rank += (wh > w || (wh == w && h < g)) ? 1 : 0;
+    wmax = wh > wmax ? wh : wmax;
+  }
+  // (groups that are all about the same size stay in catalogue order)
+  const int64_t n = seg_off[group_off[n_groups]] - seg_off[group_off[0]];
+  const bool ragged = wmax * 4 * n_groups > 5 * n;   // heaviest group > 1.25 x the mean
+  order[ragged ? rank : g] = g;
+}
+__global__ void identity_order_kernel(int n_groups, int32_t* __restrict__ order) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g < n_groups) order[g] = g;
+}
+
+// group_off [n_groups + 1], group_order [n_groups]
 int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
-                       cudaStream_t s) {
+                       int32_t* group_order, cudaStream_t s) {
   make_groups_kernel<<<(n_groups + 1 + 127) / 128, 128, 0, s>>>(seg_off, n_seg, target, n_groups, group_off);
-  return ok();
+  if (n_groups <= 8192)
+    order_groups_kernel<<<(n_groups + 127) / 128, 128, 0, s>>>(seg_off, group_off, n_groups, group_order);
+  else
+    identity_order_kernel<<<(n_groups + 127) / 128, 128, 0, s>>>(n_groups, group_order);
+  return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
 
 int launch_max_segment(const int64_t* seg_off, int64_t n_seg, int64_t* d_out, cudaStream_t s) {

@@ -211,7 +211,7 @@ __device__ __forceinline__ double term_tail(const double* __restrict__ tc, const
     const double m2p = h.m2 - tc[C_MMIN];
     const bool win2 = m2p < tc[C_DM];
     const double E = tc[C_DM] * fma(2.0, m2p, -tc[C_DM]) * rcp_fast(m2p * (m2p - tc[C_DM]));
-    ok = ok & !(win2 & !(E <= 600.0));   // a smoothing factor below e^-600 is zero (R35); also m2 = mmin and NaN
+    ok = ok & !(win2 & !(E <= 250.0));   // a smoothing factor below e^-250 is zero (R35); also m2 = mmin and NaN
     const double f2 = exp_fast<true>(win2 ? E : -700.0, exptab);
     den *= 1.0 + f2;
   }
@@ -420,8 +420,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     __syncthreads();
     const unsigned item = s_item;
     if (item >= n_items) break;
-    const int group = (int)(item / (unsigned)p.n_tiles);
-    const int tile = (int)(item - (unsigned)group * (unsigned)p.n_tiles);
+    const int gslot = (int)(item / (unsigned)p.n_tiles);
+    const int tile = (int)(item - (unsigned)gslot * (unsigned)p.n_tiles);
+    const int group = p.group_order[gslot];   // heaviest group first
     const int t0 = tile * T;  // first theta of the tile, relative to this launch
     const int nt = min(T, p.n_theta - t0);
     if (tile != cur_tile) {

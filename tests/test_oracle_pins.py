@@ -839,7 +839,7 @@ def _th_mp(**mod):
 
 def test_mp_smoothing_closed_forms():
     """S(m) = 1/(1 + exp(dm/m' + dm/(m' - dm))): 0 at mmin, 1 from mmin + dm on, 1/2 at the middle of the window,
-    S(mmin + x) + S(mmin + dm - x) = 1 (the exponent is odd about the middle), increasing; below e^-600 it is 0 (R35)."""
+    S(mmin + x) + S(mmin + dm - x) = 1 (the exponent is odd about the middle), increasing; below e^-250 it is 0 (R35)."""
     lo, dm = 4.6, 4.8
     assert O.mp_smooth(lo, lo, dm) == 0.0 and O.mp_smooth(lo - 1.0, lo, dm) == 0.0
     assert O.mp_smooth(lo + dm, lo, dm) == 1.0 and O.mp_smooth(50.0, lo, dm) == 1.0
@@ -849,9 +849,9 @@ def test_mp_smoothing_closed_forms():
     assert np.all(np.diff(s) > 0)
     np.testing.assert_allclose(s + s[::-1], 1.0, rtol=0, atol=1e-13)
     np.testing.assert_allclose(s, special.expit(-(dm / xs + dm / (xs - dm))), rtol=1e-13)
-    # the e^-600 rule: the exponent at m' = dm/601 is 601 - 1/(1 - 1/601) = 599.998.., at dm/603 it is 601.998..
-    assert O.mp_smooth(lo + dm / 603.0, lo, dm) == 0.0
-    assert 0.0 < O.mp_smooth(lo + dm / 601.0, lo, dm) < 1e-259
+    # the e^-250 rule: the exponent at m' = dm/251 is 251 - 1/(1 - 1/251) = 249.996, at dm/253 it is 251.996
+    assert O.mp_smooth(lo + dm / 253.0, lo, dm) == 0.0
+    assert 0.0 < O.mp_smooth(lo + dm / 251.0, lo, dm) < 1e-108
     # dm = 0: a step at mmin, the lower edge included (R15)
     assert O.mp_smooth(lo, lo, 0.0) == 1.0 and O.mp_smooth(lo - 1e-9, lo, 0.0) == 0.0
 
