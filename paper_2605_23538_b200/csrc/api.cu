@@ -271,7 +271,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   const int n_groups = (int)(n > 0 ? (n + target - 1) / target : 1);
   GWC_TRY(ensure(ctx, ctx->group_off, (size_t)(2 * n_groups + 1) * sizeof(int32_t)));   // offsets, then the order
   int32_t* d_group_order = (int32_t*)ctx->group_off.p + n_groups + 1;
-  GWC_TRY(count(ctx, launch_make_groups(d_seg_off, n_seg, target, n_groups, (int32_t*)ctx->group_off.p, d_group_order, s),
+  GWC_TRY(count(ctx, launch_make_groups(d_seg_off, n_seg, target, n_groups, (int32_t*)ctx->group_off.p, d_group_order, inj, s),
                 "make_groups"));
   ReweightParams p;
   memset(&p, 0, sizeof(p));

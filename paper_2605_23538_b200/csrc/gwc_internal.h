@@ -90,7 +90,6 @@ struct ReweightParams {
   const int32_t* row;       // [n_samples] (events) or nullptr (injections)
   const int64_t* seg_off;   // [n_seg+1] device
   const int32_t* group_off; // [n_groups+1] device: segments of each work group
-  const int32_t* group_order; // [n_groups] device: the groups, heaviest first (the order work items are handed out in)
   int n_groups;
   int64_t n_seg;
   const void* los;          // [n_rows][n_z] (events) | allsky [n_z] f64 (injections)
@@ -108,6 +107,7 @@ struct ReweightParams {
   unsigned int* unit_counter;
   int* flag;                // sticky device flag word (written by -DGWC_CHECKED builds only)
   int64_t n_samples;        // length of the sample arrays (checked builds)
+  const int32_t* group_order; // [n_groups] device: the groups, heaviest first (the order work items are handed out in)
 };
 
 // kernels / launchers (each returns the number of kernels it launched, or -1 on a launch error)
@@ -157,7 +157,7 @@ int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const 
                         const double* m2z, const double* lprior, const int32_t* row, int64_t n_rows, double* dLc,
                         double* L1, double* Q, double* P, double* seg_shift, cudaStream_t s);
 int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
-                       int32_t* group_order, cudaStream_t s);
+                       int32_t* group_order, bool uniform, cudaStream_t s);
 int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off, cudaStream_t s);
 size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp);
 int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp);

@@ -299,15 +299,19 @@ int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const 
 // groups with more samples (ties in group order, so equal groups keep the group-major order that keeps a group's LOS
 // rows in L2).  Catalogues whose groups are all within 25 % of the mean are left in catalogue order; a ragged one no
 // longer ends a launch on its heaviest items.
-__global__ void order_groups_kernel(const int64_t* __restrict__ seg_off, const int32_t* __restrict__ group_off,
-                                    int n_groups, int32_t* __restrict__ order) {
+__global__ void __launch_bounds__(256) order_groups_kernel(const int64_t* __restrict__ seg_off,
+                                                           const int32_t* __restrict__ group_off, int n_groups,
+                                                           int32_t* __restrict__ order) {
+  extern __shared__ int64_t s_w[];   // every group's samples (each CTA loads them all; n_groups <= 8192)
+  for (int h = threadIdx.x; h < n_groups; h += blockDim.x) s_w[h] = seg_off[group_off[h + 1]] - seg_off[group_off[h]];
+  __syncthreads();
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
-  const int64_t w = seg_off[group_off[g + 1]] - seg_off[group_off[g]];
+  const int64_t w = s_w[g];
   int rank = 0;
   int64_t wmax = 0;
   for (int h = 0; h < n_groups; ++h) {
-    const int64_t wh = seg_off[group_off[h + 1]] - seg_off[group_off[h]];
+    const int64_t wh = s_w[h];
     rank += (wh > w || (wh == w && h < g)) ? 1 : 0;
     wmax = wh > wmax ? wh : wmax;
   }
@@ -321,14 +325,17 @@ __global__ void identity_order_kernel(int n_groups, int32_t* __restrict__ order)
   if (g < n_groups) order[g] = g;
 }
 
-// group_off [n_groups + 1], group_order [n_groups]
+// group_off [n_groups + 1], group_order [n_groups]; uniform = segments of equal length (the injections): no ordering
 int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
-                       int32_t* group_order, cudaStream_t s) {
+                       int32_t* group_order, bool uniform, cudaStream_t s) {
   make_groups_kernel<<<(n_groups + 1 + 127) / 128, 128, 0, s>>>(seg_off, n_seg, target, n_groups, group_off);
-  if (n_groups <= 8192)
-    order_groups_kernel<<<(n_groups + 127) / 128, 128, 0, s>>>(seg_off, group_off, n_groups, group_order);
-  else
+  if (!uniform && n_groups <= 8192) {
+    cudaFuncSetAttribute(order_groups_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 8);   // (per device)
+    order_groups_kernel<<<(n_groups + 255) / 256, 256, (size_t)n_groups * sizeof(int64_t), s>>>(seg_off, group_off, n_groups,
+                                                                                             group_order);
+  } else {
     identity_order_kernel<<<(n_groups + 127) / 128, 128, 0, s>>>(n_groups, group_order);
+  }
   return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
 

@@ -422,7 +422,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
     if (item >= n_items) break;
     const int gslot = (int)(item / (unsigned)p.n_tiles);
     const int tile = (int)(item - (unsigned)gslot * (unsigned)p.n_tiles);
+#ifdef GWC_NO_ORDER
+    const int group = gslot;
+#else
     const int group = p.group_order[gslot];   // heaviest group first
+#endif
     const int t0 = tile * T;  // first theta of the tile, relative to this launch
     const int nt = min(T, p.n_theta - t0);
     if (tile != cur_tile) {
