@@ -43,8 +43,8 @@ FP64_INSTR_DEAD = 28.0
 FP64_INSTR_EXECUTED = 108.26
 FP64_COUNT_SOURCE = "necessary: static SASS count of the main loop (DESIGN.md 7); executed: ncu op counters, profiles/r02e_reweight_events_ncu_full.md"
 # the KDE kernel: FP64 thread instructions per Gaussian evaluation, everything included (per-sample weights, per-pixel
-# statistics, prior), measured the same way (profiles/r02e_kde_ncu_full.md)
-KDE_FP64_INSTR_PER_EVAL = 4.87
+# statistics, prior), measured the same way (profiles/r02f_kde_ncu_full.md)
+KDE_FP64_INSTR_PER_EVAL = 4.81
 # DRAM bytes of one 340-theta launch of the event kernel on the O5 catalogue (ncu dram__bytes_read.sum +
 # dram__bytes_write.sum, same capture)
 O5_DRAM_BYTES_PER_340_THETA = 7.247e9 + 0.068e9
@@ -366,7 +366,7 @@ def run_gwc(args):
                "event_terms_per_s": th_k.shape[0] * n_samples / (ms_kde * 1e-3),
                "gaussian_evals_per_s": evals / (ms_kde * 1e-3),
                "fp64_instr_per_eval": KDE_FP64_INSTR_PER_EVAL,
-               "fp64_count_source": "ncu op counters over the Gaussian evaluations of the launch, profiles/r02e_kde_ncu_full.md",
+               "fp64_count_source": "ncu op counters over the Gaussian evaluations of the launch, profiles/r02f_kde_ncu_full.md",
                "roofline_frac_fp64": evals * KDE_FP64_INSTR_PER_EVAL / (ms_kde * 1e-3) / FP64_PEAK_INSTR,
                # (round 1 counted 10 instructions per evaluation for the kernel of that round: the same time on that scale)
                "roofline_frac_fp64_at_r01_count_10": evals * 10.0 / (ms_kde * 1e-3) / FP64_PEAK_INSTR}
