@@ -58,6 +58,7 @@ struct gwc_ctx {
   int64_t built_n = 0;
   bool fresh_build = false;   // inside gwc_total_loglik*: the build was enqueued by this very call, no verification
   int M = 0, Mp = 0;
+  bool tab_shared = false;  // the batch of the last build has one Omega_m: one z(u) table serves every theta
   gwc_prec tab_prec = GWC_F64;
   double z_max = 0.0;
   // per-call scratch
@@ -249,14 +250,15 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   if (pixcut) GWC_TRY(ensure(ctx, ctx->part_np, (size_t)n_theta * n_seg * sizeof(int32_t)));
   // theta tile: as many tables as shared memory holds, balanced over the tiles
   const bool mp = ctx->model == GWC_MASS_MULTIPEAK;
-  int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut, mp);
+  const bool shared_tab = ctx->tab_shared;
+  int T = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut, mp, shared_tab);
   if (T < 1) return fail(ctx, GWC_ERR_SHAPE, "n_nodes / n_z too large for shared memory");
   if ((int64_t)T > n_theta) T = (int)n_theta;
   int n_tiles = (int)((n_theta + T - 1) / T);
   T = (int)((n_theta + n_tiles - 1) / n_tiles);
   // the kernel takes the theta points of a tile two at a time: an odd tile pays for one point more than it holds
   if (T > 2 && (T & 1) && n_theta > T) {
-    const int Tmax = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut, mp);
+    const int Tmax = reweight_max_T(ctx->Mp, ctx->tab_prec, inj, n_z, ctx->smem_optin, pixcut, mp, shared_tab);
     T = T + 1 <= Tmax ? T + 1 : T - 1;
     n_tiles = (int)((n_theta + T - 1) / T);
   }
@@ -294,6 +296,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   p.seg_off = d_seg_off;
   p.group_off = (const int32_t*)ctx->group_off.p;
   p.group_order = d_group_order;
+  p.shared_tab = shared_tab ? 1 : 0;
   p.n_groups = n_groups;
   p.n_seg = n_seg;
   p.los = los_table;
@@ -370,9 +373,9 @@ gwc_status gwc_create(gwc_ctx** out, int device, void* cuda_stream) {
   cudaError_t e = cudaSetDevice(device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
-  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_flag, 2 * sizeof(int));   // [0] sticky flags, [1] A0 packing
+  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_flag, 4 * sizeof(int));   // [0] sticky flags, [1] A0 packing, [2] one-Omega_m answer
   if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_counter, sizeof(unsigned int));
-  if (e == cudaSuccess) e = cudaMemset(ctx->d_flag, 0, 2 * sizeof(int));
+  if (e == cudaSuccess) e = cudaMemset(ctx->d_flag, 0, 4 * sizeof(int));
   if (e == cudaSuccess && reweight_configure(ctx->smem_optin) != 0) e = cudaGetLastError();
   if (e != cudaSuccess) {
     g_create_error = std::string("gwc_create: ") + cudaGetErrorString(e);
@@ -470,6 +473,18 @@ gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta,
                                         (double*)ctx->tconst.p, (Node64*)ctx->ftab.p, (double*)ctx->theta_snap.p,
                                         (double*)ctx->tvalid.p, ctx->d_flag, ctx->stream),
                 "cosmo_build"));
+  // One Omega_m in the whole batch (a population-only batch: configs Tiny and O4): z(u) depends on Omega_m alone, so
+  // one table serves every theta and a tile holds MAX_T points instead of what fits next to T tables.  Asked of the
+  // device (one small kernel and a 4-byte read: the call synchronises) only when it would change the tile.
+  ctx->tab_shared = false;
+  // (and only for batches of at least four tiles: the synchronisation costs a small batch more than the tile gains)
+  if (n_theta >= 4 * reweight_max_T(Mp, table_prec, false, 2, ctx->smem_optin, false, ctx->model == GWC_MASS_MULTIPEAK, false)) {
+    int same = 0;
+    GWC_TRY(count(ctx, launch_omega_same(d_theta, n_theta, ctx->model, ctx->d_flag + 2, ctx->stream), "omega_same"));
+    GWC_CUDA(cudaMemcpyAsync(&same, ctx->d_flag + 2, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    GWC_CUDA(cudaStreamSynchronize(ctx->stream));
+    ctx->tab_shared = same != 0;
+  }
   ctx->built_theta = d_theta;
   ctx->built_n = n_theta;
   ctx->M = n_nodes;

@@ -108,6 +108,7 @@ struct ReweightParams {
   int* flag;                // sticky device flag word (written by -DGWC_CHECKED builds only)
   int64_t n_samples;        // length of the sample arrays (checked builds)
   const int32_t* group_order; // [n_groups] device: the groups, heaviest first (the order work items are handed out in)
+  int shared_tab;           // 1: the batch has a single Omega_m, the tile stages ONE z(u) table (of its first theta)
 };
 
 // kernels / launchers (each returns the number of kernels it launched, or -1 on a launch error)
@@ -159,8 +160,10 @@ int launch_prep_samples(int64_t n, int64_t n_seg, const int64_t* seg_off, const 
 int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, int n_groups, int32_t* group_off,
                        int32_t* group_order, bool uniform, cudaStream_t s);
 int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off, cudaStream_t s);
-size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp);
-int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp);
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp, bool shared_tab);
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp, bool shared_tab);
+// *d_same = 1 when every theta row has the same Omega_m bits (one z(u) table serves the batch), else 0
+int launch_omega_same(const double* d_theta, int64_t n_theta, int model, int* d_same, cudaStream_t s);
 int reweight_configure(int smem_optin);
 int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm, int device,
                     cudaStream_t s);

@@ -62,7 +62,8 @@ struct SmemLayout {
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
-__host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_bytes, bool inj, int n_z, bool pix,
+// tabs: z(u) tables per tile (T, or 1 when the whole batch has one Omega_m and so one table)
+__host__ __device__ inline SmemLayout smem_layout(int T, int tabs, int Mp, size_t node_bytes, bool inj, int n_z, bool pix,
                                                    bool mp) {
   SmemLayout L;
   size_t o = 0;
@@ -78,7 +79,7 @@ __host__ __device__ inline SmemLayout smem_layout(int T, int Mp, size_t node_byt
   L.leadn = o;  o = align16(o + (pix ? sizeof(int) * NWARPS * T * 2 : 0));
   L.allsky = o; o = align16(o + (inj ? sizeof(double) * n_z : 0));
   L.ftab = o;   o = align16(o + (mp ? sizeof(Node64) * (size_t)T * MF_PITCH : 0));   // MULTIPEAK: F(m1) tables
-  L.tab = o;    o = align16(o + node_bytes * (size_t)T * Mp);
+  L.tab = o;    o = align16(o + node_bytes * (size_t)tabs * Mp);
   L.total = o;
   return L;
 }
@@ -384,7 +385,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   extern __shared__ __align__(16) unsigned char smem[];
   __shared__ unsigned s_item;
   typedef typename std::conditional<INJ, double, LosT>::type RowT;  // the all-sky table is f64
-  const SmemLayout L = smem_layout(p.T, p.Mp, sizeof(NodeT), INJ, p.n_z, PIX, MP);
+  const SmemLayout L = smem_layout(p.T, p.shared_tab ? 1 : p.T, p.Mp, sizeof(NodeT), INJ, p.n_z, PIX, MP);
   MathTables& mt = *reinterpret_cast<MathTables*>(smem + L.math);
   double* s_acc = reinterpret_cast<double*>(smem + L.acc);
   int* s_cnt = reinterpret_cast<int*>(smem + L.cnt);
@@ -402,6 +403,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
   const unsigned FULL = 0xffffffffu;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int T = p.T, Mp = p.Mp;
+  const int tstride = p.shared_tab ? 0 : Mp;   // one Omega_m in the batch: every theta of the tile reads the same table
   init_math_tables(mt, tid, NTHREADS);
   const double2* logtab = mt.logtab + (lane & (LOG_REP - 1));  // this lane's copies: conflict-free look-ups
   const double* exptab = mt.exptab + (lane & (EXP_REP - 1));
@@ -434,7 +436,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
       const uint4* src =
           reinterpret_cast<const uint4*>(reinterpret_cast<const NodeT*>(p.tab) + (size_t)(p.t_begin + t0) * Mp);
       uint4* dst = reinterpret_cast<uint4*>(s_tab);
-      const int n16 = (int)(((size_t)nt * Mp * sizeof(NodeT)) / 16);
+      const int n16 = (int)(((size_t)(p.shared_tab ? 1 : nt) * Mp * sizeof(NodeT)) / 16);
       for (int i = tid; i < n16; i += NTHREADS) dst[i] = src[i];
       if (MP) {
         const uint4* fsrc = reinterpret_cast<const uint4*>(p.ftab + (size_t)(p.t_begin + t0) * MF_PITCH);
@@ -646,7 +648,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
           Mid<RowT> cur[SPT], nxt[SPT];
 #pragma unroll
           for (int k = 0; k < SPT; ++k)
-            term_head<NodeT, RowT, !INJ, MP>(KT + (t0 + ja) * NC, s_tab + (size_t)ja * Mp, sm[k].A, sm[k].m2z, sm[k].lrow,
+            term_head<NodeT, RowT, !INJ, MP>(KT + (t0 + ja) * NC, s_tab + (size_t)ja * tstride, sm[k].A, sm[k].m2z, sm[k].lrow,
                                          inv_dz, los_zmax, zq, bmax, cur[k], p.flag, Mp);
           for (;;) {
             const int jb = pop_lowest(todo);
@@ -681,7 +683,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               const double* tct = KT + (t0 + ja) * NC;
 #pragma unroll
               for (int k = 0; k < SPT; ++k)
-                term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
+                term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh * tstride, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, nxt[k], p.flag, Mp);
 #pragma unroll
               for (int k = 0; k < SPT; ++k) {
@@ -703,7 +705,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) reweight_kernel(const ReweightPar
               const double* tct = KT + (t0 + jh) * NC;
 #pragma unroll
               for (int k = 0; k < SPT; ++k)
-                term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh2 * Mp, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
+                term_head<NodeT, RowT, !INJ, MP>(tch, s_tab + (size_t)jh2 * tstride, sm[k].A, sm[k].m2z, sm[k].lrow, inv_dz,
                                              los_zmax, zq, bmax, cur[k], p.flag, Mp);
               double wv[SPT];
               bool lv[SPT];
@@ -937,14 +939,15 @@ int launch_inj(const ReweightParams& p, int n_blocks, size_t smem, cudaStream_t 
 
 }  // namespace
 
-size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp) {
-  return smem_layout(T, Mp, tab_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32), inj, n_z, pix, mp).total;
+size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp, bool shared_tab) {
+  return smem_layout(T, shared_tab ? 1 : T, Mp, tab_prec == GWC_F64 ? sizeof(Node64) : sizeof(Node32), inj, n_z, pix, mp)
+      .total;
 }
 
-int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp) {
+int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp, bool shared_tab) {
   int best = 0;
   for (int T = 1; T <= MAX_T; ++T)
-    if (reweight_smem_bytes(T, Mp, tab_prec, inj, n_z, pix, mp) + SMEM_RESERVE <= (size_t)smem_optin) best = T;
+    if (reweight_smem_bytes(T, Mp, tab_prec, inj, n_z, pix, mp, shared_tab) + SMEM_RESERVE <= (size_t)smem_optin) best = T;
   return best;
 }
 
@@ -970,7 +973,7 @@ int launch_reweight(const ReweightParams& p0, gwc_prec tab_prec, gwc_prec los_pr
                     cudaStream_t s) {
   const bool mp = p0.model == 1;
   const int nc = nconst_of(p0.model);
-  const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z, p0.pixcut != 0, mp);
+  const size_t smem = reweight_smem_bytes(p0.T, p0.Mp, tab_prec, inj, p0.n_z, p0.pixcut != 0, mp, p0.shared_tab != 0);
   const int cap = ((mp ? KT_THETA_MP : KT_THETA) / p0.T) * p0.T;
   int launched = 0;
   if (device < 0 || device >= MAX_DEVICES) return -1;
