@@ -394,3 +394,30 @@ def test_pixcut_with_cache_on_between_plain_and_cut_calls(ctx):
         ctx.gwc_check()
     finally:
         ctx.gwc_cache_catalogue(False)
+
+
+def test_single_omega_batches_share_one_table(ctx):
+    """A batch of 48 theta with one Omega_m stages one z(u) table per tile (16 theta per tile); the same batch with the
+    Omega_m of its last point changed must not.  Both against the oracle, events, injections and the pixel cut."""
+    import oracle
+    from util import RTOL_F64, assert_close_log
+    W = workload("o4", n_theta=48, n_events=6, los_rows=400, n_inj=3000)
+    zmax = W.spec.z_max
+    assert bool((W.theta[:, 1] == W.theta[0, 1]).all())
+    ev, inj, lo = to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(lo, zmax)
+    ev_np, inj_np = synth.to_numpy(W.ev), synth.to_numpy(W.inj)
+    for change in (False, True):
+        th = W.theta.clone()
+        if change:
+            th[47, 1] = 0.27
+        thd = th.to(DEV)
+        total = ctx.gwc_total_loglik(thd, ev, inj, lo, zmax, allsky)
+        ctx.gwc_build_cosmo(thd, zmax)
+        gL, gN, gK, gP = ctx.gwc_event_loglik_pixcut(thd, ev, lo, zmax, 2.0)
+        ctx.gwc_check()
+        o = oracle.total_loglik(th.numpy(), ev_np, inj_np, W.los.numpy(), zmax)
+        assert_close_log(total.cpu().numpy(), o, RTOL_F64, "log L(theta), single Omega_m %s" % (not change))
+        oL, oN, oK, oP = oracle.event_loglik_pixcut(th.numpy(), ev_np, W.los.numpy(), zmax, 2.0)
+        assert np.array_equal(gP.cpu().numpy(), oP) and np.array_equal(gK.cpu().numpy(), oK)
+        assert_close_log(gL.cpu().numpy(), oL, RTOL_F64, "pixel cut, single Omega_m %s" % (not change))
