@@ -267,7 +267,7 @@ gwc_status run_reweight(gwc_ctx* ctx, int64_t n_theta, int64_t n, int64_t n_seg,
   const int kt_cap = ((mp ? KT_THETA_MP : KT_THETA) / T) * T;
   const int tiles_per_launch = n_tiles < kt_cap / T ? n_tiles : kt_cap / T;
   int64_t target = (int64_t)((double)n * tiles_per_launch / ((double)ctx->n_sm * 16.0));
-  if (target > 65536) target = 65536;
+  if (target > 131072) target = 131072;   // (O5 event kernel: 1003 ms at 65536, 998 at 131072 / 262144, 1029 at 524288)
   if (target < 4096) target = 4096;
   while ((n / target + 2) * (int64_t)n_tiles > (int64_t)0x7fffffff) target *= 2;
   const int n_groups = (int)(n > 0 ? (n + target - 1) / target : 1);
