@@ -127,6 +127,9 @@ int32_t gwc_theta_len(gwc_mass_model model);
  * Under GWC_MASS_MULTIPEAK the same call also builds, per theta, the normalisation N1 of p(m1) and a 513-node
  * cubic-Hermite table of the normaliser of p(m2 | m1) over the smoothing window [mmin, mmin + delta_m] (above the
  * window it is elementary), by 4 x 8-point Gauss-Legendre quadrature per table interval (R36).
+ * For batches of 40 theta points or more the call also asks the device whether every row has the same Omega_m (then
+ * one z(u) table serves the whole batch and a tile of the fused kernel holds 16 points instead of 10) and reads the
+ * 4-byte answer: it SYNCHRONISES the stream in that case; smaller batches stay asynchronous.
  */
 gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double z_max, int32_t n_nodes,
                            gwc_prec table_prec);
@@ -215,6 +218,9 @@ gwc_status gwc_event_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
  * neff_min = 0 gives gwc_event_loglik's results.  Same preconditions and errors as gwc_event_loglik;
  * neff_min < 0 or NaN -> GWC_ERR_INVALID_ARG.
  *   d_logL [n_theta][n_events] f64;  d_neff f64, d_nlive i64, d_npass i64: same shape or NULL.
+ * The kernel works on a pixel-aligned copy of the samples kept in the context (every pixel on an even slot, odd
+ * pixels padded by one dead slot: at most twice the samples, typically a few per cent more); building it
+ * SYNCHRONISES the stream once (its length), unless gwc_cache_catalogue is on and the copy is still valid.
  */
 gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                                    const gwc_los* los, double neff_min, double* d_logL, double* d_neff,
@@ -227,7 +233,8 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
  *   v_k = p(m1, m2 | theta) / (J pi_PE)  (Eq. 7 without the redshift prior),  n_j = its live samples,
  *   h_j = 1.06 sigma_j n_j^(-1/5) with sigma_j the v-weighted standard deviation of the z_k (bw_rule = GWC_BW_SCOTT),
  *         or 0.9 min(sigma_j, IQR_j / 1.34) n_j^(-1/5) with the interquartile range of the live z_k, plain quantiles
- *         by linear interpolation (GWC_BW_SILVERMAN; R32),
+ *         by linear interpolation (GWC_BW_SILVERMAN; R32), or from the biweight midvariance D3 of the live z_k
+ *         (Eq. D3-D4): h_j = D3 as printed (GWC_BW_BIWEIGHT) or 1.06 sqrt(D3) n_j^(-1/5) (GWC_BW_BIWEIGHT_SCOTT; R37),
  *   I_j = trapezoid over the n_grid-node uniform grid on [0, los->z_max] of
  *         [sum_k v_k N(z; z_k, h_j)] p_los(z | row_j) psi(z) / (1+z),
  *   log L_i = log( (1/S_i) sum_j I_j )  over the pixels with n_j >= 2, sigma_j > 0 and N_eff,j >= neff_min.
@@ -235,7 +242,9 @@ gwc_status gwc_event_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t 
  * neff_min < 0 or NaN -> GWC_ERR_INVALID_ARG.
  *   d_logL [n_theta][n_events] f64;  d_npass, d_nused same shape i64 or NULL (pixels that contributed, and their
  *   live samples: n_grid * d_nused Gaussian evaluations were needed).
- * Synchronises the stream once (the longest event sizes a scratch buffer).
+ * A Gaussian kernel value below e^-700 counts as zero (R38).  Work is split into chunks of whole pixels of about 1024
+ * samples (a table built on the device per call).  Synchronises the stream once (the number of chunks and the
+ * longest chunk size the scratch buffers).
  */
 gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                                 const gwc_los* los, int32_t n_grid, double neff_min, int32_t bw_rule, double* d_logL,
