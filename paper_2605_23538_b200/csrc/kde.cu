@@ -312,7 +312,7 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
         zs = zv.x * sinvh;
       }
       const int cnt = (int)min((int64_t)32, r1 - c0);
-      for (int j = up; j - up < cnt; j += 2) {   // (a slot past the end holds a = 0)
+      auto step = [&](int j) {
         const double zj = __shfl_sync(FULL, zs, j), aj = __shfl_sync(FULL, a, j);
         double qc = qL - zj;
         {
@@ -343,6 +343,11 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
         acc[13] = fma(aj, u5, acc[13]);
         acc[14] = fma(aj, u6, acc[14]);
         acc[15] = fma(aj, u7, acc[15]);
+      };
+      // two samples per half-warp and step (two independent chains); a slot past the end holds a = 0
+      for (int j = up; j - up < cnt; j += 4) {
+        step(j);
+        step((j + 2) & 31);
       }
     }
     // the halves exchange what the other one keeps; C_o = c1^(o^2), c1 = exp(-beta^2)
