@@ -272,6 +272,17 @@ gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
                             double* d_logL_total);
 
 /*
+ * gwc_total_loglik with the per-pixel effective-sample cut of Eq. 8 on the event term: the direct
+ * Monte-Carlo sum over the samples of the pixels that pass N_eff,j >= neff_min (gwc_event_loglik_pixcut), the same
+ * selection term, the same total.  neff_min = 0 gives gwc_total_loglik's result.  Same arguments and errors as
+ * gwc_total_loglik; synchronises the stream once (the padded copy of gwc_event_loglik_pixcut), twice for batches of
+ * 40 theta points or more (gwc_build_cosmo).
+ */
+gwc_status gwc_total_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                                   const gwc_injections* inj, const gwc_los* los, int32_t n_nodes,
+                                   gwc_prec table_prec, double neff_min, double* d_logL_total);
+
+/*
  * The paper's likelihood in one call: Eq. 5 with the KDE numerator (gwc_event_loglik_kde: n_grid, neff_min), the
  * per-pixel cut of Eq. 8 and the selection term of Eq. 4:  build_cosmo(z_max = los->z_max, n_nodes, table_prec),
  * the KDE event term, gwc_selection_logxi, gwc_combine_total.  Same arguments, errors and NaN / -inf rules as

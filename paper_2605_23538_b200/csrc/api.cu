@@ -736,6 +736,25 @@ gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta
   return gwc_combine_total(ctx, (const double*)ctx->logL.p, (const double*)ctx->logxi.p, n_theta, E, d_logL_total);
 }
 
+gwc_status gwc_total_loglik_pixcut(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
+                                   const gwc_injections* inj, const gwc_los* los, int32_t n_nodes,
+                                   gwc_prec table_prec, double neff_min, double* d_logL_total) {
+  GWC_TRY(check_theta_args(ctx, d_theta, n_theta));
+  if (!ev || !inj || !d_logL_total) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL argument");
+  GWC_TRY(check_los(ctx, los, true, true));
+  if (los->n_z > GWC_MAX_NZ_SELECTION)
+    return fail(ctx, GWC_ERR_SHAPE, "los->n_z > 4096 is not supported by the selection term");
+  GWC_TRY(gwc_build_cosmo(ctx, d_theta, n_theta, los->z_max, n_nodes, table_prec));
+  const int64_t E = ev->n_events;
+  GWC_TRY(ensure(ctx, ctx->logL, (size_t)n_theta * (size_t)(E > 0 ? E : 1) * sizeof(double)));
+  GWC_TRY(ensure(ctx, ctx->logxi, (size_t)n_theta * sizeof(double)));
+  FreshBuild fresh(ctx);
+  GWC_TRY(gwc_event_loglik_pixcut(ctx, d_theta, n_theta, ev, los, neff_min, (double*)ctx->logL.p, nullptr, nullptr,
+                                  nullptr));
+  GWC_TRY(gwc_selection_logxi(ctx, d_theta, n_theta, inj, los, (double*)ctx->logxi.p, nullptr));
+  return gwc_combine_total(ctx, (const double*)ctx->logL.p, (const double*)ctx->logxi.p, n_theta, E, d_logL_total);
+}
+
 gwc_status gwc_total_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                                 const gwc_injections* inj, const gwc_los* los, int32_t n_nodes, gwc_prec table_prec,
                                 int32_t n_grid, double neff_min, int32_t bw_rule, double* d_logL_total) {

@@ -28,7 +28,7 @@ EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_laun
            "gwc_theta_len", "gwc_build_cosmo",
            "gwc_export_cosmo", "gwc_pack_events", "gwc_cap_pixels", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",
            "gwc_selection_logxi",
-           "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_cache_catalogue", "gwc_set_timing", "gwc_get_timing",
+           "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_pixcut", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_cache_catalogue", "gwc_set_timing", "gwc_get_timing",
            "gwc_probe_fp64", "gwc_math_selftest"]
 
 
@@ -89,6 +89,7 @@ def load():
         "gwc_selection_logxi": (ci, [vp, vp, i64, C.POINTER(Injections), C.POINTER(Los), vp, vp]),
         "gwc_combine_total": (ci, [vp, vp, vp, i64, i64, vp]),
         "gwc_total_loglik": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci, vp]),
+        "gwc_total_loglik_pixcut": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci, dbl, vp]),
         "gwc_total_loglik_kde": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci, i32,
                                       dbl, i32, vp]),
         "gwc_total_loglik_host": (ci, [vp, vp, i64, C.POINTER(Events), C.POINTER(Injections), C.POINTER(Los), i32, ci,
@@ -299,6 +300,15 @@ class Context:
         es, js, los = make_events(ev), make_injections(inj), make_los(table, z_max, allsky)
         self._ck(self._lib.gwc_total_loglik(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(js),
                                             C.byref(los), n_nodes, table_prec, out.data_ptr()))
+        return out
+
+    def gwc_total_loglik_pixcut(self, theta, ev, inj, table, z_max, allsky, neff_min=2.0, n_nodes=1025, table_prec=F64):
+        """gwc_total_loglik with the per-pixel N_eff cut of Eq. 8 on the event term."""
+        nt = theta.shape[0]
+        out = torch.empty(nt, dtype=torch.float64, device=self.device)
+        es, js, los = make_events(ev), make_injections(inj), make_los(table, z_max, allsky)
+        self._ck(self._lib.gwc_total_loglik_pixcut(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(js),
+                                                   C.byref(los), n_nodes, table_prec, float(neff_min), out.data_ptr()))
         return out
 
     def gwc_total_loglik_kde(self, theta, ev, inj, table, z_max, allsky, n_grid=256, neff_min=2.0, n_nodes=1025,

@@ -622,3 +622,24 @@ def test_catalogue_cache_and_small_batches(ctx):
         ctx.gwc_cache_catalogue(False)
     got = _np(ctx.gwc_total_loglik(W.theta[:5].to(DEV), ev, inj, los, zmax, allsky))
     assert np.array_equal(got, ref[5], equal_nan=True)
+
+
+def test_total_loglik_pixcut(ctx):
+    """gwc_total_loglik_pixcut = the composed calls, bit for bit, and the oracle's pieces at the FP64 bar; threshold 0
+    agrees with gwc_total_loglik to rounding."""
+    W = workload("o4", n_theta=14, n_events=7, los_rows=400, n_inj=5000)
+    zmax = W.spec.z_max
+    th, ev, inj, los = W.theta.to(DEV), to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    tot = ctx.gwc_total_loglik_pixcut(th, ev, inj, los, zmax, allsky, 2.0)
+    ctx.gwc_build_cosmo(th, zmax)
+    gL = ctx.gwc_event_loglik_pixcut(th, ev, los, zmax, 2.0)[0]
+    gX, _ = ctx.gwc_selection_logxi(th, inj, allsky, los.shape[1], zmax)
+    assert np.array_equal(_np(ctx.gwc_combine_total(gL, gX)), _np(tot), equal_nan=True)
+    ctx.gwc_check()
+    oL = oracle.event_loglik_pixcut(_np(W.theta), synth.to_numpy(W.ev), _np(W.los), zmax, 2.0)[0]
+    oX, _ = oracle.selection_logxi(_np(W.theta), synth.to_numpy(W.inj), oracle.los_allsky(_np(W.los), zmax), zmax)
+    assert_close_log(_np(tot), oracle.total_from_parts(oL, oX), RTOL_F64, "log L(theta) with the pixel cut")
+    t0 = ctx.gwc_total_loglik_pixcut(th, ev, inj, los, zmax, allsky, 0.0)
+    t1 = ctx.gwc_total_loglik(th, ev, inj, los, zmax, allsky)
+    assert_close_log(_np(t0), _np(t1), 1e-13, "threshold 0 against the uncut total")
