@@ -255,6 +255,8 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
  * los->allsky and log_pdraw in place of the PE prior; optional N_eff of the injection sum.
  *   d_logxi [n_theta];  d_neff_inj [n_theta] or NULL.
  * los->n_z <= GWC_MAX_NZ_SELECTION (4096) else GWC_ERR_SHAPE (here and, before any work, in gwc_total_loglik*).
+ * Calls of 2e8 (theta x injection) terms and up work on a copy of the injections in order of d_L kept in the context
+ * (whole warps then leave a theta's table together; the sum does not depend on the order beyond rounding).
  */
 gwc_status gwc_selection_logxi(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_injections* inj,
                                const gwc_los* los, double* d_logxi, double* d_neff_inj);

@@ -217,6 +217,11 @@ int launch_pixpad_scatter(const int64_t* d_seg_off, int64_t n_seg, const int64_t
                           const int32_t* row, double* o_dLc, double* o_m1z, double* o_m2z, double* o_L1, double* o_Q,
                           double* o_P, int32_t* o_row, cudaStream_t s);
 
+// injections in order of d_L (selection term): sorted copies of the four arrays
+size_t injsort_scratch_bytes(int64_t n);
+int launch_injsort(int64_t n, const double* dL, const double* m1z, const double* m2z, const double* lp, double* o_dL,
+                   double* o_m1z, double* o_m2z, double* o_lp, void* scratch, size_t scratch_bytes, cudaStream_t s);
+
 size_t cap_scratch_bytes(int64_t n_samples);
 int launch_cap_pixels(int64_t n, int64_t n_events, int64_t n_pix, const int64_t* d_perm_in, int64_t* d_ev_sample_off,
                       int64_t* d_pix_sample_off, int64_t cap, uint64_t seed, int64_t* d_perm_out, int64_t* d_n_kept,

@@ -361,3 +361,54 @@ int launch_pixpad_scatter(const int64_t* d_seg_off, int64_t n_seg, const int64_t
 }
 
 }  // namespace gwc
+
+// ---- injections in order of d_L (selection term) ----------------------------------------------------------------------
+// The selection sum does not depend on the order of the injections (beyond rounding), and in order of d_L whole
+// warps fall outside a theta's table together and skip it: one radix sort of the d_L bit patterns (positive doubles
+// order like their bits; invalid values end up anywhere, they are dead) and a gather of the four arrays, once per
+// injection set (kept between calls with gwc_cache_catalogue).
+namespace gwc {
+namespace {
+__global__ void injsort_keys_kernel(int64_t n, const double* __restrict__ dL, uint64_t* __restrict__ keys,
+                                    int64_t* __restrict__ idx) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  keys[k] = (uint64_t)__double_as_longlong(dL[k]);
+  idx[k] = k;
+}
+__global__ void injsort_gather_kernel(int64_t n, const int64_t* __restrict__ perm, const double* __restrict__ a,
+                                      const double* __restrict__ b, const double* __restrict__ c,
+                                      const double* __restrict__ d, double* __restrict__ oa, double* __restrict__ ob,
+                                      double* __restrict__ oc, double* __restrict__ od) {
+  const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const int64_t j = perm[k];
+  oa[k] = a[j];
+  ob[k] = b[j];
+  oc[k] = c[j];
+  od[k] = d[j];
+}
+}  // namespace
+
+size_t injsort_scratch_bytes(int64_t n) {
+  const size_t m = (size_t)(n > 0 ? n : 1);
+  return 4 * a256(8 * m) + a256(cub_temp_bytes((int64_t)m)) + 256;
+}
+
+int launch_injsort(int64_t n, const double* dL, const double* m1z, const double* m2z, const double* lp, double* o_dL,
+                   double* o_m1z, double* o_m2z, double* o_lp, void* scratch, size_t scratch_bytes, cudaStream_t s) {
+  if (n <= 0) return 0;
+  unsigned char* base = (unsigned char*)scratch;
+  uint64_t* keys = (uint64_t*)base;          base += a256(8 * (size_t)n);
+  uint64_t* keys_sorted = (uint64_t*)base;   base += a256(8 * (size_t)n);
+  int64_t* idx = (int64_t*)base;             base += a256(8 * (size_t)n);
+  int64_t* perm = (int64_t*)base;            base += a256(8 * (size_t)n);
+  size_t temp = scratch_bytes - (size_t)(base - (unsigned char*)scratch);
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  injsort_keys_kernel<<<blocks, 256, 0, s>>>(n, dL, keys, idx);
+  if (cub::DeviceRadixSort::SortPairs(base, temp, keys, keys_sorted, idx, perm, n, 0, 64, s) != cudaSuccess) return -1;
+  injsort_gather_kernel<<<blocks, 256, 0, s>>>(n, perm, dL, m1z, m2z, lp, o_dL, o_m1z, o_m2z, o_lp);
+  return cudaGetLastError() == cudaSuccess ? 3 : -1;
+}
+
+}  // namespace gwc

@@ -421,3 +421,34 @@ def test_single_omega_batches_share_one_table(ctx):
         oL, oN, oK, oP = oracle.event_loglik_pixcut(th.numpy(), ev_np, W.los.numpy(), zmax, 2.0)
         assert np.array_equal(gP.cpu().numpy(), oP) and np.array_equal(gK.cpu().numpy(), oK)
         assert_close_log(gL.cpu().numpy(), oL, RTOL_F64, "pixel cut, single Omega_m %s" % (not change))
+
+
+def test_selection_with_injections_sorted_inside_the_library(ctx):
+    """Calls of 2e8 (theta x injection) terms and up run the selection term on a copy of the injections in order of
+    d_L (pack.cu).  Against the oracle (which sums in the caller's order) at the FP64 bar; with the catalogue cache on,
+    a second injection set of the same shape in other arrays must not meet the first one's sorted copy; invalid
+    injections (NaN, negative d_L) stay dead wherever the sort puts them."""
+    import oracle
+    from util import RTOL_F64, assert_close_log
+    W = workload("production", n_theta=1024, n_events=2, los_rows=300, n_inj=200_000)
+    zmax = W.spec.z_max
+    th, lo = W.theta.to(DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(lo, zmax)
+    sky_np = oracle.los_allsky(W.los.numpy(), zmax)
+    inj_a = {k: (v.clone() if isinstance(v, torch.Tensor) else v) for k, v in W.inj.items()}
+    inj_a["dL"][5], inj_a["dL"][77], inj_a["m1z"][123] = float("nan"), -3.0, float("inf")
+    inj_b = {k: (v.flip(0).contiguous() * (1.02 if k == "dL" else 1.0) if isinstance(v, torch.Tensor) else v)
+             for k, v in W.inj.items()}
+    ctx.gwc_build_cosmo(th, zmax)
+    ctx.gwc_cache_catalogue(True)
+    try:
+        for inj in (inj_a, inj_b, inj_a):
+            d = to_dev(inj, DEV)
+            for _ in range(2):
+                gX, gN = ctx.gwc_selection_logxi(th, d, allsky, lo.shape[1], zmax)
+            ctx.gwc_check()
+            oX, oN = oracle.selection_logxi(W.theta.numpy(), synth.to_numpy(inj), sky_np, zmax)
+            assert_close_log(gX.cpu().numpy(), oX, RTOL_F64, "log xi on sorted injections")
+            np.testing.assert_allclose(gN.cpu().numpy(), oN, rtol=1e-7)
+    finally:
+        ctx.gwc_cache_catalogue(False)
