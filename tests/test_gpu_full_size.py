@@ -275,3 +275,35 @@ def test_production_multipeak_sampled():
         print("production, MULTIPEAK: worst rel err on log L_i %.2e" % r["worst"])
     finally:
         c.close()
+
+
+@pytest.mark.parametrize("name,bw", [("production", "scott"), ("stress", "silverman")])
+def test_full_size_kde_sampled(ctx, name, bw):
+    """NEXT row 1 at full size, in the configuration bench.py times (the whole catalogue, units = (chunk, theta)): the
+    KDE numerator for 4 theta on every event of the production batch / the stress catalogue (its 20 events of 32768
+    samples are split into ~32 chunks each), compared with the oracle on a seeded subset of 10 events, the largest
+    and the smallest included (256 Gaussians per (theta, sample) on the CPU)."""
+    W, theta = _device_workload(name)
+    los = W.los
+    tsel = _pick(theta.shape[0], 4, 23)
+    th = theta[torch.as_tensor(tsel, device=theta.device)].contiguous()
+    zmax = W.spec.z_max
+    ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+    gL, gP, gU = [_np(x) for x in ctx.gwc_event_loglik_kde(th, W.ev, los, zmax, 256, 2.0, bw)]
+    ctx.gwc_check()
+    ev_np = synth.to_numpy(W.ev)
+    S = np.diff(ev_np["ev_sample_off"])
+    esel = _pick(S.size, 10, 29, must=(int(np.argmax(S)), int(np.argmin(S))))
+    sub = _sub_events(ev_np, esel)
+    oL, oP, oU = oracle.event_loglik_kde(_np(th), sub, _np(los), zmax, n_grid=256, neff_min=2.0, bandwidth=bw,
+                                         want_nused=True)
+    g_L, g_P, g_U = gL[:, esel], gP[:, esel], gU[:, esel]
+    same = g_P == oP
+    print("%s KDE (%s): %d (theta, event) pairs, %d with a different pixel count" % (name, bw, same.size, int((~same).sum())))
+    assert (~same).sum() <= max(1, int(0.05 * same.size))      # (R25: N_eff = 2 decisions on the last bit)
+    assert np.array_equal(g_U[same], oU[same])
+    assert np.array_equal(np.isneginf(g_L[same]), np.isneginf(oL[same]))
+    fin = same & np.isfinite(oL)
+    assert fin.any()
+    err = np.abs(g_L[fin] - oL[fin]) / np.maximum(np.abs(oL[fin]), 1.0)
+    assert err.max() <= RTOL_F64, err.max()
