@@ -452,3 +452,49 @@ def test_selection_with_injections_sorted_inside_the_library(ctx):
             np.testing.assert_allclose(gN.cpu().numpy(), oN, rtol=1e-7)
     finally:
         ctx.gwc_cache_catalogue(False)
+
+
+def test_two_contexts_pixcut_and_kde_concurrently(ctx):
+    """Two contexts on two streams from two host threads, one running the pixel-cut event term (constant bank, padded
+    copy), the other the KDE numerator (chunk table, scratch): the bits of the serial results."""
+    from paper_2605_23538_b200 import gwc
+    Wa = workload("o4", n_theta=400, n_events=30, los_rows=2000, n_inj=1000)
+    Wb = workload("production", n_theta=12, n_events=20, los_rows=2000, n_inj=1000, seed=5)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    ca, cb = gwc.Context(0, stream=sa), gwc.Context(0, stream=sb)
+    try:
+        A = (Wa.theta.to(DEV), to_dev(Wa.ev, DEV), Wa.los.to(DEV))
+        B = (Wb.theta.to(DEV), to_dev(Wb.ev, DEV), Wb.los.to(DEV))
+        torch.cuda.synchronize()
+        ctx.gwc_build_cosmo(A[0], Wa.spec.z_max)
+        ra = [x.clone() for x in ctx.gwc_event_loglik_pixcut(A[0], A[1], A[2], Wa.spec.z_max, 2.0)]
+        ctx.gwc_build_cosmo(B[0], Wb.spec.z_max)
+        rb = [x.clone() for x in ctx.gwc_event_loglik_kde(B[0], B[1], B[2], Wb.spec.z_max, 256, 2.0)]
+        torch.cuda.synchronize()
+        out = {"a": [], "b": []}
+
+        def run_a():
+            with torch.cuda.stream(sa):
+                for _ in range(5):
+                    ca.gwc_build_cosmo(A[0], Wa.spec.z_max)
+                    out["a"].append(ca.gwc_event_loglik_pixcut(A[0], A[1], A[2], Wa.spec.z_max, 2.0))
+            sa.synchronize()
+
+        def run_b():
+            with torch.cuda.stream(sb):
+                for _ in range(5):
+                    cb.gwc_build_cosmo(B[0], Wb.spec.z_max)
+                    out["b"].append(cb.gwc_event_loglik_kde(B[0], B[1], B[2], Wb.spec.z_max, 256, 2.0))
+            sb.synchronize()
+
+        ta, tb = threading.Thread(target=run_a), threading.Thread(target=run_b)
+        ta.start(); tb.start(); ta.join(); tb.join()
+        torch.cuda.synchronize()
+        ca.gwc_check(); cb.gwc_check()
+        eq = lambda x, y: torch.equal(torch.nan_to_num(x.double(), nan=1.0, neginf=-1e300), torch.nan_to_num(y.double(), nan=1.0, neginf=-1e300))
+        for r in out["a"]:
+            assert all(eq(x, y) for x, y in zip(r, ra))
+        for r in out["b"]:
+            assert all(eq(x, y) for x, y in zip(r, rb))
+    finally:
+        ca.close(); cb.close()
