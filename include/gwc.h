@@ -199,6 +199,35 @@ gwc_status gwc_cap_pixels(gwc_ctx* ctx, int64_t n_samples, int64_t n_events, int
 gwc_status gwc_los_allsky(gwc_ctx* ctx, const gwc_los* los, double* d_allsky /* [n_z] */);
 
 /*
+ * gwc_los_allsky for callers that must not allocate device memory.  Who they are: a program that has given all of the
+ * GPU's memory to its own pool or arena (a cudaMalloc made behind its back fails, or eats memory the pool counts on);
+ * a sampling or serving loop with other streams busy (cudaMalloc / cudaFree take a device-wide lock and can wait for
+ * the device, stalling every stream); and, because of either, code that may not even call gwc_create (which
+ * allocates).  So this call takes NO context, and neither it nor anything under it calls cudaMalloc, cudaFree or an
+ * allocating library routine: the partial sums that gwc_los_allsky keeps in context scratch live in a fixed array
+ * inside the library image (4 MiB of device memory, held by every GPU that loads libgwc.so until the process exits).
+ *   in : los->table [n_rows][n_z] (device, f64 or f32 per los->prec), los->n_rows, los->n_z, los->z_max > 0;
+ *        los->allsky is not read.   out: d_allsky [n_z] f64 (device, caller-owned).   cuda_stream: a cudaStream_t of
+ *        the calling thread's CURRENT device (NULL = default stream); the table and d_allsky must be on that device.
+ * Result: bit-identical to gwc_los_allsky (same kernels, same fixed summation order).  Asynchronous on cuda_stream.
+ * Limit: ceil(n_rows / GWC_ALLSKY_STATIC_ROWS_PER_PART) * n_z <= GWC_ALLSKY_STATIC_MAX_DOUBLES (the O5-scale table,
+ *   200000 rows x 1000 nodes, needs 391000 and fits); a larger table is refused with GWC_ERR_SHAPE before anything is
+ *   enqueued, d_allsky untouched.  Other argument errors as gwc_los_allsky.  The text of the last non-OK status of
+ *   the calling thread comes from gwc_los_allsky_static_error() (there is no context to hold it).
+ * Set-up: the FIRST call on each device asks the runtime for the array's address on that device (one
+ *   cudaGetSymbolAddress, which may also make the runtime load the library's device code).  Make that first call
+ *   during start-up, before any stream capture and before the phase in which allocation is forbidden.
+ * Sharing: all calls on one GPU use the same array, from every thread and stream.  Nothing in it needs to be zero at
+ *   entry (each call overwrites exactly the part it then reads), so calls one after the other on one stream, or
+ *   ordered by events, are safe; two calls that can RUN AT THE SAME TIME on one GPU (different streams, no ordering
+ *   between them) race on it and give wrong sums.  Serialise them.
+ */
+#define GWC_ALLSKY_STATIC_ROWS_PER_PART 512
+#define GWC_ALLSKY_STATIC_MAX_DOUBLES (1 << 19)
+gwc_status gwc_los_allsky_static(const gwc_los* los, double* d_allsky /* [n_z] */, void* cuda_stream);
+const char* gwc_los_allsky_static_error(void);
+
+/*
  * A3 + A4.  log L_i(theta) = log( (1/S_i) sum_k w_ik ) for every (theta, event); optional
  * N_eff,i (Eq. 8) and the number of live samples.  Needs gwc_build_cosmo(d_theta, n_theta) first
  * (same pointer and count) else GWC_ERR_NOT_BUILT; needs los->z_max <= the z_max of that build.

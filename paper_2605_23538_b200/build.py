@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libgwc.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "cosmo.cu", "reweight.cu", "reduce.cu", "pack.cu", "kde.cu"]
+SOURCES = ["api.cu", "cosmo.cu", "reweight.cu", "reduce.cu", "pack.cu", "kde.cu", "noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "gwc_internal.h"), os.path.join(CSRC, "math64.cuh"), os.path.join(INCLUDE, "gwc.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
               "--fmad=true", "-Xptxas", "-v"]

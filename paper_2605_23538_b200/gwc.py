@@ -29,7 +29,9 @@ EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_laun
            "gwc_export_cosmo", "gwc_pack_events", "gwc_cap_pixels", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",
            "gwc_selection_logxi",
            "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_pixcut", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_cache_catalogue", "gwc_set_timing", "gwc_get_timing",
-           "gwc_probe_fp64", "gwc_math_selftest"]
+           "gwc_probe_fp64", "gwc_math_selftest", "gwc_los_allsky_static", "gwc_los_allsky_static_error"]
+ALLSKY_STATIC_ROWS_PER_PART = 512
+ALLSKY_STATIC_MAX_DOUBLES = 1 << 19
 
 
 BW_RULES = {"scott": 0, "silverman": 1, "biweight": 2, "biweight_scott": 3}
@@ -99,6 +101,8 @@ def load():
         "gwc_get_timing": (ci, [vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64), C.POINTER(dbl)]),
         "gwc_probe_fp64": (ci, [vp, i64, C.POINTER(dbl), C.POINTER(dbl)]),
         "gwc_math_selftest": (ci, [vp, ci, i64, vp, vp]),
+        "gwc_los_allsky_static": (ci, [C.POINTER(Los), vp, vp]),
+        "gwc_los_allsky_static_error": (C.c_char_p, []),
     }
     for name, (res, args) in sig.items():
         f = getattr(L, name)
@@ -240,6 +244,29 @@ class Context:
         los = make_los(table, z_max)
         self._ck(self._lib.gwc_los_allsky(self._h, C.byref(los), out.data_ptr()))
         return out
+
+    @staticmethod
+    def gwc_los_allsky_static(table: torch.Tensor, z_max: float, out: torch.Tensor) -> torch.Tensor:
+        """gwc_los_allsky without any device allocation, for programs whose memory pool owns the whole GPU or whose
+        other streams must not be stalled by cudaMalloc (include/gwc.h).  Needs no Context: the caller brings `out`
+        ([n_z] float64 on the table's device) and the partial sums go to a fixed 4 MiB array inside libgwc.so, which
+        limits the table to ceil(n_rows / 512) * n_z <= 2**19 (GwcError GWC_ERR_SHAPE beyond).  Runs on torch's
+        current stream of the table's device; the first call on a device does a one-time set-up, so make it at
+        start-up.  Calls that overlap on one GPU race on the shared array."""
+        lib = load()
+        if out.dim() != 1 or out.shape[0] != table.shape[1] or out.device != table.device:
+            raise ValueError("out must be [n_z] on the table's device")
+        los = make_los(table, z_max)
+        with torch.cuda.device(table.device):
+            st = lib.gwc_los_allsky_static(C.byref(los), _ptr(out, torch.float64),
+                                           C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        if st != OK:
+            raise GwcError(st, lib.gwc_los_allsky_static_error().decode())
+        return out
+
+    @staticmethod
+    def gwc_los_allsky_static_error() -> str:
+        return load().gwc_los_allsky_static_error().decode()
 
     def gwc_event_loglik(self, theta, ev, table, z_max, want_neff=True, want_nlive=True):
         nt, ne = theta.shape[0], ev["ev_sample_off"].numel() - 1
