@@ -36,7 +36,9 @@
  *    event is a few nats.  When a log_pe_prior / log_pdraw of enormous spread breaks this (every live weight more
  *    than 300 nats below the reference), the outputs of that (theta, event) are NaN and gwc_check() returns
  *    GWC_ERR_RANGE; nothing is clamped silently.  (Single weights more than 700 nats below the reference count as
- *    e^-700 of it, far below the rounding of the sum.  gwc_event_loglik_pixcut decides per pixel: a pixel whose
+ *    e^-700 of it, far below the rounding of the sum.  A block of injections in that state is simply left out when
+ *    even an upper bound of its sum lies 60 nats under the largest block of that theta: it cannot change log xi;
+ *    only a block that could matter makes log xi NaN.  gwc_event_loglik_pixcut decides per pixel: a pixel whose
  *    own weights all lie more than 300 nats below its event's reference may be counted wrongly in d_npass /
  *    d_nlive while contributing nothing to log L_i.)
  *  - theta and the tables: gwc_build_cosmo keeps, next to the tables, a copy of the theta rows it was given.  The
@@ -127,7 +129,8 @@ int32_t gwc_theta_len(gwc_mass_model model);
  * Under GWC_MASS_MULTIPEAK the same call also builds, per theta, the normalisation N1 of p(m1) and a 513-node
  * cubic-Hermite table of the normaliser of p(m2 | m1) over the smoothing window [mmin, mmin + delta_m] (above the
  * window it is elementary), by 4 x 8-point Gauss-Legendre quadrature per table interval (R36).
- * For batches of 40 theta points or more the call also asks the device whether every row has the same Omega_m (then
+ * For batches of 40 theta points or more the call also asks the device whether every row has the same Omega_m and is
+ * inside the model's domain (then
  * one z(u) table serves the whole batch and a tile of the fused kernel holds 16 points instead of 10) and reads the
  * 4-byte answer: it SYNCHRONISES the stream in that case; smaller batches stay asynchronous.
  */

@@ -653,14 +653,15 @@ gwc_status gwc_event_loglik_kde(gwc_ctx* ctx, const double* d_theta, int64_t n_t
   GWC_CUDA(cudaMemsetAsync(ctx->kde_len.p, 0, 2 * sizeof(int64_t), s));
   GWC_TRY(count(ctx, launch_kde_chunks(ev->ev_sample_off, n_seg, ev->sample_row, (int64_t*)ctx->kde_cnt.p,
                                        (int64_t*)ctx->kde_coff.p, (int64_t*)ctx->kde_cstart.p, (int64_t*)ctx->kde_cend.p,
-                                       (int32_t*)ctx->kde_cev.p, (int64_t*)ctx->kde_len.p, s),
+                                       (int32_t*)ctx->kde_cev.p, (int64_t*)ctx->kde_len.p, n, s),
                 "kde_chunks"));
-  int64_t max_len = 0, n_chunks = 0;
-  GWC_CUDA(cudaMemcpyAsync(&max_len, ctx->kde_len.p, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+  int64_t len_bad[2] = {0, 0}, n_chunks = 0;
+  GWC_CUDA(cudaMemcpyAsync(len_bad, ctx->kde_len.p, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, s));
   GWC_CUDA(cudaMemcpyAsync(&n_chunks, (const int64_t*)ctx->kde_coff.p + n_seg, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
   GWC_CUDA(cudaStreamSynchronize(s));
-  if (max_len < 0 || max_len > n || n_chunks < 0 || n_chunks > nc_max)
-    return fail(ctx, GWC_ERR_SHAPE, "ev_sample_off is not ascending");
+  const int64_t max_len = len_bad[0];
+  if (len_bad[1] != 0 || max_len < 0 || max_len > n || n_chunks < 0 || n_chunks > nc_max)
+    return fail(ctx, GWC_ERR_SHAPE, "ev_sample_off is not ascending inside [0, n_samples]");
   const int n_blocks = kde_grid_blocks(n_theta, n_chunks, ctx->n_sm);
   GWC_TRY(ensure(ctx, ctx->kde_scr, kde_scratch_bytes(n_blocks, max_len)));
   GWC_TRY(ensure(ctx, ctx->kde_thk, kde_theta_bytes(n_theta)));

@@ -365,10 +365,14 @@ __global__ void verify_theta_kernel(const double* __restrict__ theta, const doub
 }  // namespace
 
 namespace {
-__global__ void omega_same_kernel(const double* __restrict__ theta, int64_t n_theta, int npar, int* __restrict__ same) {
+// One table can serve the batch only if every row is inside the model's domain as well: cosmo_build_kernel writes an
+// all-zero table for a row outside it, and a tile stages the table of its FIRST theta for all of its points.
+__global__ void omega_same_kernel(const double* __restrict__ theta, int64_t n_theta, int npar, int model,
+                                  int* __restrict__ same) {
   const long long ref = __double_as_longlong(theta[1]);
   bool ok = true;
-  for (int64_t t = threadIdx.x; t < n_theta; t += blockDim.x) ok = ok && __double_as_longlong(theta[t * npar + 1]) == ref;
+  for (int64_t t = threadIdx.x; t < n_theta; t += blockDim.x)
+    ok = ok && __double_as_longlong(theta[t * npar + 1]) == ref && theta_valid(theta + t * npar, model);
   const int all = __syncthreads_and(ok ? 1 : 0);
   if (threadIdx.x == 0) *same = all;
 }
@@ -376,7 +380,7 @@ __global__ void omega_same_kernel(const double* __restrict__ theta, int64_t n_th
 
 int launch_omega_same(const double* d_theta, int64_t n_theta, int model, int* d_same, cudaStream_t s) {
   if (n_theta <= 0) return 0;
-  omega_same_kernel<<<1, 256, 0, s>>>(d_theta, n_theta, model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR, d_same);
+  omega_same_kernel<<<1, 256, 0, s>>>(d_theta, n_theta, model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR, model, d_same);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

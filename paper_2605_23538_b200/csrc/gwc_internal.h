@@ -162,7 +162,8 @@ int launch_make_groups(const int64_t* seg_off, int64_t n_seg, int64_t target, in
 int launch_uniform_segments(int64_t n, int64_t seg, int64_t n_seg, int64_t* seg_off, cudaStream_t s);
 size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, bool pix, bool mp, bool shared_tab);
 int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp, bool shared_tab);
-// *d_same = 1 when every theta row has the same Omega_m bits (one z(u) table serves the batch), else 0
+// *d_same = 1 when every theta row has the same Omega_m bits and lies inside the model's domain (one z(u) table
+// serves the batch), else 0
 int launch_omega_same(const double* d_theta, int64_t n_theta, int model, int* d_same, cudaStream_t s);
 int reweight_configure(int smem_optin);
 int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm, int device,
@@ -193,7 +194,7 @@ int launch_kde(int model, const Node64* d_ftab, const double* d_theta, const voi
 int64_t kde_chunk_bound(int64_t n_samples, int64_t n_events);
 int launch_kde_chunks(const int64_t* ev_off, int64_t n_events, const int32_t* row, int64_t* d_cnt,
                       int64_t* d_chunk_off, int64_t* d_start, int64_t* d_end, int32_t* d_event, int64_t* d_max_len,
-                      cudaStream_t s);
+                      int64_t n_samples, cudaStream_t s);
 size_t kde_theta_bytes(int64_t n_theta);
 size_t kde_weight_bytes(int64_t n_theta);
 int kde_grid_blocks(int64_t n_theta, int64_t n_chunks, int n_sm);

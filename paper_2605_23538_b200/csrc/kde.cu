@@ -408,9 +408,17 @@ __device__ __forceinline__ double kde_pixel(const double2* __restrict__ scr, int
 constexpr int KDE_CHUNK = GWC_KDE_CHUNK;   // target samples per chunk (a pixel is never split)
 
 // ---- chunks: runs of whole pixels of one event, cut at the first pixel start at or after every KDE_CHUNK samples ----
-__global__ void kde_chunk_count_kernel(const int64_t* __restrict__ ev_off, int64_t n_events, int64_t* __restrict__ cnt) {
+// An event whose offsets do not ascend inside [0, n_samples] gets no chunk (nothing of it is read or written later) and
+// raises *bad, which the host turns into GWC_ERR_SHAPE: with every event inside the sample list and disjoint from its
+// neighbours the chunk count stays below kde_chunk_bound, the size of the chunk tables.
+__global__ void kde_chunk_count_kernel(const int64_t* __restrict__ ev_off, int64_t n_events, int64_t n_samples,
+                                       int64_t* __restrict__ cnt, int64_t* __restrict__ bad) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (i < n_events) cnt[i] = (ev_off[i + 1] - ev_off[i] + KDE_CHUNK - 1) / KDE_CHUNK;
+  if (i >= n_events) return;
+  const int64_t s0 = ev_off[i], s1 = ev_off[i + 1];
+  const bool ok = s0 >= 0 && s0 <= s1 && s1 <= n_samples;
+  cnt[i] = ok ? (s1 - s0 + KDE_CHUNK - 1) / KDE_CHUNK : 0;
+  if (!ok) *bad = 1;
 }
 // exclusive scan in order (single CTA); off[n] = total
 __global__ void kde_chunk_scan_kernel(const int64_t* __restrict__ cnt, int64_t n, int64_t* __restrict__ off) {
@@ -446,12 +454,13 @@ __device__ __forceinline__ int64_t next_pixel_start(const int32_t* __restrict__ 
 __global__ void kde_chunk_bounds_kernel(const int64_t* __restrict__ ev_off, int64_t n_events,
                                         const int64_t* __restrict__ chunk_off, const int32_t* __restrict__ row,
                                         int64_t* __restrict__ c_start, int64_t* __restrict__ c_end,
-                                        int32_t* __restrict__ c_event, int64_t* __restrict__ max_len) {
+                                        int32_t* __restrict__ c_event, int64_t* __restrict__ max_len,
+                                        int64_t nc_max) {
   const int64_t ev = blockIdx.x;
   const int64_t s0 = ev_off[ev], s1 = ev_off[ev + 1];
   const int64_t c0 = chunk_off[ev], nc = chunk_off[ev + 1] - c0;
   long long mx = 0;
-  for (int64_t c = threadIdx.x; c < nc; c += blockDim.x) {
+  for (int64_t c = threadIdx.x; c < nc && c0 + c < nc_max; c += blockDim.x) {
     const int64_t a = next_pixel_start(row, s0, s1, s0 + c * KDE_CHUNK);
     const int64_t b = c + 1 < nc ? next_pixel_start(row, s0, s1, s0 + (c + 1) * KDE_CHUNK) : s1;
     c_start[c0 + c] = a;
@@ -732,15 +741,17 @@ __global__ void kde_combine_kernel(const KdeParams p) {
 int64_t kde_chunk_bound(int64_t n_samples, int64_t n_events) { return n_samples / KDE_CHUNK + n_events + 1; }
 
 // chunk table of a catalogue: d_cnt [n_events] scratch, d_chunk_off [n_events + 1] (its last entry = number of
-// chunks), start / end / event [kde_chunk_bound], *d_max_len = longest chunk (must hold 0 before the call)
+// chunks), start / end / event [kde_chunk_bound], d_max_len[0] = longest chunk, d_max_len[1] = 1 when an event's
+// offsets do not ascend inside [0, n_samples] (both must hold 0 before the call)
 int launch_kde_chunks(const int64_t* ev_off, int64_t n_events, const int32_t* row, int64_t* d_cnt,
                       int64_t* d_chunk_off, int64_t* d_start, int64_t* d_end, int32_t* d_event, int64_t* d_max_len,
-                      cudaStream_t s) {
+                      int64_t n_samples, cudaStream_t s) {
   if (n_events <= 0) return 0;
-  kde_chunk_count_kernel<<<(unsigned)((n_events + 255) / 256), 256, 0, s>>>(ev_off, n_events, d_cnt);
+  kde_chunk_count_kernel<<<(unsigned)((n_events + 255) / 256), 256, 0, s>>>(ev_off, n_events, n_samples, d_cnt,
+                                                                            d_max_len + 1);
   kde_chunk_scan_kernel<<<1, 256, 0, s>>>(d_cnt, n_events, d_chunk_off);
   kde_chunk_bounds_kernel<<<(unsigned)n_events, 64, 0, s>>>(ev_off, n_events, d_chunk_off, row, d_start, d_end, d_event,
-                                                            d_max_len);
+                                                            d_max_len, kde_chunk_bound(n_samples, n_events));
   return cudaGetLastError() == cudaSuccess ? 3 : -1;
 }
 

@@ -149,14 +149,31 @@ __global__ void finalize_inj_kernel(const double* __restrict__ part_w, const int
   }
   const double* pw = part_w + 2 * t * n_seg;
   const int32_t* pn = part_n + t * n_seg;
-  double smax = -CUDART_INF;
-  bool range = false;
+  // A segment whose live weights all lie below e^-300 of its own reference has left the range of its linear-domain
+  // sums (gwc.h, "Range").  Its computed sum is still an UPPER bound of its true sum (weights are clamped from below,
+  // never raised above their value), so shift + ln(sum) bounds what it can add to xi.  When that bound lies 60 nats
+  // (e^-60 = 9e-27) under the largest in-range segment, the segment is left out: it cannot move log xi or N_eff
+  // in the last bit, however many such segments there are.  Otherwise, or with no segment in range, the theta's
+  // outputs are NaN and FLAG_RANGE is raised.
+  constexpr double NEGLIGIBLE = 60.0;
+  double smax = -CUDART_INF;   // largest shift of the in-range segments
+  double lin = -CUDART_INF;    // largest ln(segment sum) + shift of the in-range segments
+  double lout = -CUDART_INF;   // largest bound of an out-of-range live segment
   for (int64_t s = lane; s < n_seg; s += 32) {
-    if (pw[2 * s] > 0.0) smax = fmax(smax, seg_shift[s]);
-    range = range || (pn[s] > 0 && !(pw[2 * s] >= RANGE_MIN_SUM));
+    const double w = pw[2 * s];
+    if (w >= RANGE_MIN_SUM) {
+      smax = fmax(smax, seg_shift[s]);
+      lin = fmax(lin, seg_shift[s] + log(w));
+    } else if (pn[s] > 0) {
+      lout = fmax(lout, seg_shift[s] + (w > 0.0 ? log(w) : -690.0));
+    }
   }
-  for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(FULL, smax, o));
-  if (__any_sync(FULL, range)) {  // a segment whose live weights all lie below e^-300 of its reference
+  for (int o = 16; o > 0; o >>= 1) {
+    smax = fmax(smax, __shfl_xor_sync(FULL, smax, o));
+    lin = fmax(lin, __shfl_xor_sync(FULL, lin, o));
+    lout = fmax(lout, __shfl_xor_sync(FULL, lout, o));
+  }
+  if (lout > -CUDART_INF && !(lout <= lin - NEGLIGIBLE)) {  // (lin = -inf: no segment in range)
     if (lane == 0) {
       logxi[t] = CUDART_NAN;
       if (neff) neff[t] = CUDART_NAN;
@@ -173,6 +190,7 @@ __global__ void finalize_inj_kernel(const double* __restrict__ part_w, const int
   }
   double a = 0.0, b = 0.0;
   for (int64_t s = lane; s < n_seg; s += 32) {
+    if (!(pw[2 * s] >= RANGE_MIN_SUM)) continue;   // no live injection, or left out as negligible (above)
     const double e = exp(seg_shift[s] - smax);
     a = fma(pw[2 * s], e, a);
     b = fma(pw[2 * s + 1], e * e, b);

@@ -169,6 +169,15 @@ class Context:
         if st != OK:
             raise GwcError(st, self._lib.gwc_last_error(None).decode() or "gwc_create failed")
         self._h = h
+        self._npar = NPAR   # row width of theta under the selected mass model (gwc_set_mass_model)
+
+    def _theta(self, theta: torch.Tensor):
+        """Device pointer of a theta batch after checking its row width against the selected mass model (the C entry
+        points take no width: a [n, 12] array under MULTIPEAK would be read past its end)."""
+        if theta.dim() != 2 or theta.shape[1] != self._npar:
+            raise ValueError("theta must be [n_theta, %d] under the selected mass model, got %s"
+                             % (self._npar, tuple(theta.shape)))
+        return _ptr(theta, torch.float64)
 
     def close(self):
         if getattr(self, "_h", None):
@@ -195,12 +204,13 @@ class Context:
     def gwc_set_mass_model(self, model: str):
         """"plpeak" (12-column theta rows) or "multipeak" (16 columns; include/gwc.h)."""
         self._ck(self._lib.gwc_set_mass_model(self._h, MASS_MODELS[model]))
+        self._npar = int(self._lib.gwc_theta_len(MASS_MODELS[model]))
 
     def gwc_theta_len(self, model: str) -> int:
         return int(self._lib.gwc_theta_len(MASS_MODELS[model]))
 
     def gwc_build_cosmo(self, theta: torch.Tensor, z_max: float, n_nodes: int = 1025, table_prec: int = F64):
-        self._ck(self._lib.gwc_build_cosmo(self._h, _ptr(theta, torch.float64), theta.shape[0], float(z_max), n_nodes,
+        self._ck(self._lib.gwc_build_cosmo(self._h, self._theta(theta), theta.shape[0], float(z_max), n_nodes,
                                            table_prec))
 
     def gwc_export_cosmo(self, n_theta: int, n_nodes: int):
@@ -274,7 +284,7 @@ class Context:
         neff = torch.empty_like(logL) if want_neff else None
         nlive = torch.empty((nt, ne), dtype=torch.int64, device=self.device) if want_nlive else None
         es, los = make_events(ev), make_los(table, z_max)
-        self._ck(self._lib.gwc_event_loglik(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(los),
+        self._ck(self._lib.gwc_event_loglik(self._h, self._theta(theta), nt, C.byref(es), C.byref(los),
                                             logL.data_ptr(), _ptr(neff), _ptr(nlive)))
         return logL, neff, nlive
 
@@ -286,7 +296,7 @@ class Context:
         nlive = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
         npass = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
         es, los = make_events(ev), make_los(table, z_max)
-        self._ck(self._lib.gwc_event_loglik_pixcut(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(los),
+        self._ck(self._lib.gwc_event_loglik_pixcut(self._h, self._theta(theta), nt, C.byref(es), C.byref(los),
                                                    float(neff_min), logL.data_ptr(), neff.data_ptr(),
                                                    nlive.data_ptr(), npass.data_ptr()))
         return logL, neff, nlive, npass
@@ -298,7 +308,7 @@ class Context:
         npass = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
         nused = torch.empty((nt, ne), dtype=torch.int64, device=self.device)
         es, los = make_events(ev), make_los(table, z_max)
-        self._ck(self._lib.gwc_event_loglik_kde(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(los),
+        self._ck(self._lib.gwc_event_loglik_kde(self._h, self._theta(theta), nt, C.byref(es), C.byref(los),
                                                 int(n_grid), float(neff_min), BW_RULES[bandwidth], logL.data_ptr(),
                                                 npass.data_ptr(), nused.data_ptr()))
         return logL, npass, nused
@@ -309,7 +319,7 @@ class Context:
         neff = torch.empty_like(logxi) if want_neff else None
         js = make_injections(inj)
         los = Los(1, n_z, float(z_max), F64, None, _ptr(allsky, torch.float64))
-        self._ck(self._lib.gwc_selection_logxi(self._h, _ptr(theta, torch.float64), nt, C.byref(js), C.byref(los),
+        self._ck(self._lib.gwc_selection_logxi(self._h, self._theta(theta), nt, C.byref(js), C.byref(los),
                                                logxi.data_ptr(), _ptr(neff)))
         return logxi, neff
 
@@ -325,7 +335,7 @@ class Context:
         if out is None:
             out = torch.empty(nt, dtype=torch.float64, device=self.device)
         es, js, los = make_events(ev), make_injections(inj), make_los(table, z_max, allsky)
-        self._ck(self._lib.gwc_total_loglik(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(js),
+        self._ck(self._lib.gwc_total_loglik(self._h, self._theta(theta), nt, C.byref(es), C.byref(js),
                                             C.byref(los), n_nodes, table_prec, out.data_ptr()))
         return out
 
@@ -334,7 +344,7 @@ class Context:
         nt = theta.shape[0]
         out = torch.empty(nt, dtype=torch.float64, device=self.device)
         es, js, los = make_events(ev), make_injections(inj), make_los(table, z_max, allsky)
-        self._ck(self._lib.gwc_total_loglik_pixcut(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(js),
+        self._ck(self._lib.gwc_total_loglik_pixcut(self._h, self._theta(theta), nt, C.byref(es), C.byref(js),
                                                    C.byref(los), n_nodes, table_prec, float(neff_min), out.data_ptr()))
         return out
 
@@ -344,7 +354,7 @@ class Context:
         nt = theta.shape[0]
         out = torch.empty(nt, dtype=torch.float64, device=self.device)
         es, js, los = make_events(ev), make_injections(inj), make_los(table, z_max, allsky)
-        self._ck(self._lib.gwc_total_loglik_kde(self._h, _ptr(theta, torch.float64), nt, C.byref(es), C.byref(js),
+        self._ck(self._lib.gwc_total_loglik_kde(self._h, self._theta(theta), nt, C.byref(es), C.byref(js),
                                                 C.byref(los), n_nodes, table_prec, int(n_grid), float(neff_min),
                                                 BW_RULES[bandwidth], out.data_ptr()))
         return out
@@ -352,6 +362,8 @@ class Context:
     def gwc_total_loglik_host(self, theta, ev, inj, table, z_max, allsky=None, n_nodes=1025, table_prec=F64, out=None):
         """All tensors on the HOST (pinned memory makes the copies faster).  Returns (out, h2d_bytes, d2h_bytes)."""
         nt = theta.shape[0]
+        if theta.dim() != 2 or theta.shape[1] != self._npar:
+            raise ValueError("theta must be [n_theta, %d] under the selected mass model" % self._npar)
         if out is None:
             out = torch.empty(nt, dtype=torch.float64)
         es, js = make_events(ev, cuda=False), make_injections(inj, cuda=False)

@@ -189,8 +189,15 @@ def test_multipeak_host_call_and_model_switch(ctx):
     thd, ev, lo = th.to(DEV), to_dev(W.ev, DEV), W.los.to(DEV)
     ctx.gwc_build_cosmo(thd, zmax)
     ctx.gwc_set_mass_model("plpeak")
-    with pytest.raises(gwc.GwcError) as e:
+    with pytest.raises(ValueError):          # the binding checks the row width against the selected model
+        ctx.gwc_event_loglik(thd, ev, lo, zmax)
+    with pytest.raises(ValueError):
+        ctx.gwc_build_cosmo(thd, zmax)
+    ctx.gwc_set_mass_model("multipeak")
+    with pytest.raises(gwc.GwcError) as e:   # the tables built before the switch are gone
         ctx.gwc_event_loglik(thd, ev, lo, zmax)
     assert e.value.status == gwc.ERR_NOT_BUILT
-    ctx.gwc_set_mass_model("multipeak")
+    ctx.gwc_build_cosmo(thd, zmax)
+    ctx.gwc_event_loglik(thd, ev, lo, zmax)
+    ctx.gwc_check()
     assert ctx.gwc_theta_len("multipeak") == 16 and ctx.gwc_theta_len("plpeak") == 12

@@ -155,6 +155,46 @@ def test_wide_log_pe_prior_range_rule(ctx):
     assert e.value.status == gwc.ERR_RANGE and torch.isnan(logxi).all()
 
 
+def test_selection_block_out_of_range_but_negligible(ctx):
+    """gwc.h "Range", selection term: a block of 8192 injections whose live weights all lie far below the block's own
+    reference makes log xi NaN only if it could matter.  Block 1 of three: its first injection sets the reference
+    and is dead for every theta (m1 > mmax); the others carry a draw density e^+600 larger, i.e. weights e^-600 of
+    the other blocks'.  (a) The block's upper bound lies hundreds of nats under the other blocks: log xi and N_eff
+    match the oracle (which sums everything exactly), GWC_OK.  (b) The same block with ordinary draw densities and
+    only the reference sample 1000 nats up: it carries a third of xi, so NaN + GWC_ERR_RANGE as before."""
+    from paper_2605_23538_b200 import gwc
+    W = workload("production", n_theta=12, n_events=2, los_rows=300, n_inj=3 * 8192)
+    zmax = W.spec.z_max
+    th, los = W.theta.to(DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(los, zmax)
+    sky_np = oracle.los_allsky(_np(W.los), zmax)
+    a, b = 8192, 2 * 8192
+    for negligible in (True, False):
+        inj_cpu = {k: (v.clone() if isinstance(v, torch.Tensor) else v) for k, v in W.inj.items()}
+        lp = inj_cpu["log_pdraw"].clone()
+        if negligible:
+            lp[a + 1:b] += 600.0            # weights e^-600 of the other blocks'
+            lp[a] -= 100.0                  # the dead reference sample: 700 nats above the block's live weights
+        else:
+            lp[a] -= 1000.0
+        inj_cpu["m1z"][a] = 1e5
+        inj_cpu["m2z"][a] = 9e4
+        inj_cpu["log_pdraw"] = lp.contiguous()
+        ctx.gwc_build_cosmo(th, zmax, 1025, 0)
+        gX, gN = ctx.gwc_selection_logxi(th, to_dev(inj_cpu, DEV), allsky, los.shape[1], zmax)
+        if negligible:
+            ctx.gwc_check()
+            oX, oN = oracle.selection_logxi(_np(W.theta), synth.to_numpy(inj_cpu), sky_np, zmax)
+            assert np.isfinite(oX).all()
+            assert_close_log(_np(gX), oX, RTOL_F64, "log xi with a negligible out-of-range block")
+            np.testing.assert_allclose(_np(gN), oN, rtol=1e-7)
+        else:
+            with pytest.raises(gwc.GwcError) as e:
+                ctx.gwc_check()
+            assert e.value.status == gwc.ERR_RANGE and torch.isnan(gX).all() and torch.isnan(gN).all()
+            ctx.gwc_check()
+
+
 def test_two_contexts_two_streams(ctx):
     """Two contexts on two streams of one device, driven from two host threads at once (the per-theta
     constants of all contexts share the device's constant bank).  Results must equal the serial ones bit for bit."""
@@ -423,6 +463,48 @@ def test_single_omega_batches_share_one_table(ctx):
         assert_close_log(gL.cpu().numpy(), oL, RTOL_F64, "pixel cut, single Omega_m %s" % (not change))
 
 
+def test_single_omega_batch_with_points_outside_the_domain(ctx):
+    """48 theta with one Omega_m, rows 0 and 16 outside the domain (sigma < 0; Omega_m itself valid and equal): they are
+    the first points of their 16-point tiles, whose all-zero z(u) table must not be staged for the valid points beside
+    them.  Only those two rows are NaN; every other row matches the oracle: events, pixel cut, injections, total."""
+    import oracle
+    from paper_2605_23538_b200 import gwc
+    from util import RTOL_F64, assert_close_log
+    W = workload("o4", n_theta=48, n_events=6, los_rows=400, n_inj=3000)
+    zmax = W.spec.z_max
+    assert bool((W.theta[:, 1] == W.theta[0, 1]).all())
+    th = W.theta.clone()
+    bad = [0, 16]
+    th[bad, 7] = -1.0
+    good = [t for t in range(48) if t not in bad]
+    ev, inj, lo = to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(lo, zmax)
+    ev_np, inj_np = synth.to_numpy(W.ev), synth.to_numpy(W.inj)
+    thd = th.to(DEV)
+    total = ctx.gwc_total_loglik(thd, ev, inj, lo, zmax, allsky).cpu().numpy()
+    ctx.gwc_build_cosmo(thd, zmax)
+    gL, _, gK = ctx.gwc_event_loglik(thd, ev, lo, zmax)
+    pL, _, pK, pP = ctx.gwc_event_loglik_pixcut(thd, ev, lo, zmax, 2.0)
+    gX, _ = ctx.gwc_selection_logxi(thd, inj, allsky, lo.shape[1], zmax)
+    with pytest.raises(gwc.GwcError) as e:
+        ctx.gwc_check()
+    assert e.value.status == gwc.ERR_DOMAIN
+    ctx.gwc_check()
+    gL, pL, gX = gL.cpu().numpy(), pL.cpu().numpy(), gX.cpu().numpy()
+    assert np.isnan(total[bad]).all() and np.isnan(gL[bad]).all() and np.isnan(pL[bad]).all() and np.isnan(gX[bad]).all()
+    tg = th[good].numpy()     # the oracle sees the valid rows only
+    los_np = W.los.numpy()
+    assert_close_log(total[good], oracle.total_loglik(tg, ev_np, inj_np, los_np, zmax), RTOL_F64, "log L(theta) beside invalid rows")
+    oL, _, oK = oracle.event_loglik(tg, ev_np, los_np, zmax)
+    assert_close_log(gL[good], oL, RTOL_F64, "log L_i beside invalid rows")
+    assert np.array_equal(gK.cpu().numpy()[good], oK)
+    qL, _, qK, qP = oracle.event_loglik_pixcut(tg, ev_np, los_np, zmax, 2.0)
+    assert_close_log(pL[good], qL, RTOL_F64, "pixel cut beside invalid rows")
+    assert np.array_equal(pK.cpu().numpy()[good], qK) and np.array_equal(pP.cpu().numpy()[good], qP)
+    oX, _ = oracle.selection_logxi(tg, inj_np, oracle.los_allsky(los_np, zmax), zmax)
+    assert_close_log(gX[good], oX, RTOL_F64, "log xi beside invalid rows")
+
+
 def test_selection_with_injections_sorted_inside_the_library(ctx):
     """Calls of 2e8 (theta x injection) terms and up run the selection term on a copy of the injections in order of
     d_L (pack.cu).  Against the oracle (which sums in the caller's order) at the FP64 bar; with the catalogue cache on,
@@ -496,5 +578,66 @@ def test_two_contexts_pixcut_and_kde_concurrently(ctx):
             assert all(eq(x, y) for x, y in zip(r, ra))
         for r in out["b"]:
             assert all(eq(x, y) for x, y in zip(r, rb))
+    finally:
+        ca.close(); cb.close()
+
+
+def test_two_contexts_share_the_constant_bank_across_streams(ctx):
+    """Both contexts run the fused re-weighting kernel, which reads the per-theta constants from the device's ONE
+    constant bank: two streams, two host threads, different theta batches of different sizes (700 and 400 points: three
+    and two launches of at most 340 points each, so the bank is rewritten inside every call and between the contexts'
+    launches).  A copy into the bank that overtook a kernel still reading it would change that kernel's results: every
+    repetition must give the bits of the serial run.  One context does the event term, the other alternates the
+    selection term and the event term."""
+    from paper_2605_23538_b200 import gwc
+    Wa = workload("production", n_theta=700, n_events=12, los_rows=1000, n_inj=30_000, seed=3)
+    Wb = workload("production", n_theta=400, n_events=8, los_rows=1000, n_inj=40_000, seed=4)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    ca, cb = gwc.Context(0, stream=sa), gwc.Context(0, stream=sb)
+    try:
+        A = (Wa.theta.to(DEV), to_dev(Wa.ev, DEV), Wa.los.to(DEV), to_dev(Wa.inj, DEV))
+        B = (Wb.theta.to(DEV), to_dev(Wb.ev, DEV), Wb.los.to(DEV), to_dev(Wb.inj, DEV))
+        za, zb = Wa.spec.z_max, Wb.spec.z_max
+        sky_b = ctx.gwc_los_allsky(B[2], zb)
+        nzb = B[2].shape[1]
+        ctx.gwc_build_cosmo(A[0], za)
+        ra = [x.clone() for x in ctx.gwc_event_loglik(A[0], A[1], A[2], za)]
+        ctx.gwc_build_cosmo(B[0], zb)
+        rb_x = [x.clone() for x in ctx.gwc_selection_logxi(B[0], B[3], sky_b, nzb, zb)]
+        rb_e = [x.clone() for x in ctx.gwc_event_loglik(B[0], B[1], B[2], zb)]
+        ctx.gwc_check()
+        torch.cuda.synchronize()
+        out = {"a": [], "bx": [], "be": []}
+        go = threading.Barrier(2)
+
+        def run_a():
+            go.wait()
+            with torch.cuda.stream(sa):
+                for _ in range(6):
+                    ca.gwc_build_cosmo(A[0], za)
+                    out["a"].append(ca.gwc_event_loglik(A[0], A[1], A[2], za))
+            sa.synchronize()
+
+        def run_b():
+            go.wait()
+            with torch.cuda.stream(sb):
+                for _ in range(6):
+                    cb.gwc_build_cosmo(B[0], zb)
+                    out["bx"].append(cb.gwc_selection_logxi(B[0], B[3], sky_b, nzb, zb))
+                    out["be"].append(cb.gwc_event_loglik(B[0], B[1], B[2], zb))
+            sb.synchronize()
+
+        ta, tb = threading.Thread(target=run_a), threading.Thread(target=run_b)
+        ta.start(); tb.start(); ta.join(); tb.join()
+        torch.cuda.synchronize()
+        ca.gwc_check(); cb.gwc_check()
+        eq = lambda x, y: torch.equal(torch.nan_to_num(x.double(), nan=1.0, neginf=-1e300), torch.nan_to_num(y.double(), nan=1.0, neginf=-1e300))
+        assert len(out["a"]) == 6 and len(out["bx"]) == 6 and len(out["be"]) == 6
+        for r in out["a"]:
+            assert all(eq(x, y) for x, y in zip(r, ra))
+        for r in out["bx"]:
+            assert all(eq(x, y) for x, y in zip(r, rb_x))
+        for r in out["be"]:
+            assert all(eq(x, y) for x, y in zip(r, rb_e))
     finally:
         ca.close(); cb.close()
