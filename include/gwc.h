@@ -298,6 +298,28 @@ gwc_status gwc_combine_total(gwc_ctx* ctx, const double* d_logL, const double* d
                              int64_t n_events, double* d_total);
 
 /*
+ * A6 for a catalogue split over R ranks (SURVEY.md 8e-2; the sampler's one-theta-per-call pattern, PAPER.md:129, :166,
+ * leaves nothing to split but the events and the injections).  Rank r owns a block of events and a block of the found
+ * injections and computes, with the ordinary calls on its block,
+ *   S_r[t]  = sum over ITS events of log L_i(theta_t)       (gwc_combine_total with a zero log xi; 0 without events),
+ *   x_r[t]  = log xi_r(theta_t), N_r[t] = N_eff,r            (gwc_selection_logxi with the GLOBAL n_draw),
+ * the ranks exchange these (an all-gather of 3 x n_theta doubles per rank), and every rank combines them here in
+ * rank order, so that all ranks hold the same bits (Eq. 3-4):
+ *   xi = sum_r xi_r,   N_eff,inj = (sum_r xi_r)^2 / sum_r (xi_r^2 / N_r),   log L = sum_r S_r - n_events_total log xi.
+ *   d_sum_logL_parts, d_logxi_parts, d_neff_inj_parts: [n_parts][n_theta] f64 (the last may be NULL when d_neff_inj is);
+ *   d_total, d_logxi, d_neff_inj: [n_theta] f64, each may be NULL.   n_parts in [1, 65536].
+ * A NaN in any piece of a theta makes its outputs NaN; -inf stays -inf.  The _host form takes HOST pointers, needs
+ * no context and no GPU (the same function compiled for the host): for ranks that gathered through host memory.
+ */
+gwc_status gwc_combine_sharded(gwc_ctx* ctx, int32_t n_parts, int64_t n_theta, int64_t n_events_total,
+                               const double* d_sum_logL_parts, const double* d_logxi_parts,
+                               const double* d_neff_inj_parts, double* d_total, double* d_logxi, double* d_neff_inj);
+gwc_status gwc_combine_sharded_host(int32_t n_parts, int64_t n_theta, int64_t n_events_total,
+                                    const double* h_sum_logL_parts, const double* h_logxi_parts,
+                                    const double* h_neff_inj_parts, double* h_total, double* h_logxi,
+                                    double* h_neff_inj);
+
+/*
  * The whole hot path A1..A6 for one theta batch: build_cosmo(z_max = los->z_max, n_nodes, table_prec),
  * event_loglik, selection_logxi, combine.   d_logL_total [n_theta] f64.
  */

@@ -757,6 +757,30 @@ gwc_status gwc_combine_total(gwc_ctx* ctx, const double* d_logL, const double* d
   return count(ctx, launch_combine_total(d_logL, d_logxi, n_theta, n_events, d_total, ctx->stream), "combine_total");
 }
 
+gwc_status gwc_combine_sharded(gwc_ctx* ctx, int32_t n_parts, int64_t n_theta, int64_t n_events_total,
+                               const double* d_sum_logL_parts, const double* d_logxi_parts,
+                               const double* d_neff_inj_parts, double* d_total, double* d_logxi, double* d_neff_inj) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (!d_sum_logL_parts || !d_logxi_parts) return fail(ctx, GWC_ERR_INVALID_ARG, "NULL pointer");
+  if (d_neff_inj && !d_neff_inj_parts) return fail(ctx, GWC_ERR_INVALID_ARG, "d_neff_inj needs d_neff_inj_parts");
+  if (n_parts < 1 || n_parts > 65536 || n_theta < 1 || n_events_total < 0)
+    return fail(ctx, GWC_ERR_SHAPE, "sizes out of range");
+  return count(ctx, launch_combine_sharded(d_sum_logL_parts, d_logxi_parts, d_neff_inj_parts, n_parts, n_theta,
+                                           n_events_total, d_total, d_logxi, d_neff_inj, ctx->stream),
+               "combine_sharded");
+}
+
+gwc_status gwc_combine_sharded_host(int32_t n_parts, int64_t n_theta, int64_t n_events_total,
+                                    const double* h_sum_logL_parts, const double* h_logxi_parts,
+                                    const double* h_neff_inj_parts, double* h_total, double* h_logxi,
+                                    double* h_neff_inj) {
+  if (!h_sum_logL_parts || !h_logxi_parts || (h_neff_inj && !h_neff_inj_parts)) return GWC_ERR_INVALID_ARG;
+  if (n_parts < 1 || n_parts > 65536 || n_theta < 1 || n_events_total < 0) return GWC_ERR_SHAPE;
+  combine_sharded_host(h_sum_logL_parts, h_logxi_parts, h_neff_inj_parts, n_parts, n_theta, n_events_total, h_total,
+                       h_logxi, h_neff_inj);
+  return GWC_OK;
+}
+
 gwc_status gwc_total_loglik(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, const gwc_events* ev,
                             const gwc_injections* inj, const gwc_los* los, int32_t n_nodes, gwc_prec table_prec,
                             double* d_logL_total) {

@@ -179,6 +179,13 @@ int launch_widen_i32(const int32_t* in, const double* tvalid, int64_t n_theta, i
                      cudaStream_t s);
 int launch_combine_total(const double* logL, const double* logxi, int64_t n_theta, int64_t n_events, double* total,
                          cudaStream_t s);
+// event / injection sharding: pieces [n_parts][n_theta] of R ranks -> total, log xi, N_eff,inj [n_theta] (rank order);
+// the kernel and the host loop run the same function
+int launch_combine_sharded(const double* sum_parts, const double* logxi_parts, const double* neff_parts, int n_parts,
+                           int64_t n_theta, int64_t n_events_total, double* total, double* logxi, double* neff,
+                           cudaStream_t s);
+void combine_sharded_host(const double* sum_parts, const double* logxi_parts, const double* neff_parts, int n_parts,
+                          int64_t n_theta, int64_t n_events_total, double* total, double* logxi, double* neff);
 int launch_allsky(const void* table, gwc_prec prec, int64_t n_rows, int n_z, double* scratch, double* allsky,
                   cudaStream_t s);
 size_t allsky_scratch_doubles(int64_t n_rows, int n_z);

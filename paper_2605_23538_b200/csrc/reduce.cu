@@ -231,6 +231,58 @@ __global__ void __launch_bounds__(TOT_THREADS) combine_total_kernel(const double
   }
 }
 
+// ---- event / injection sharding: the pieces of R ranks -> log L(theta), in rank order ----
+// One theta.  S_r = sum of log L_i over rank r's events, x_r = log xi_r and N_r = N_eff,r over rank r's injections
+// (computed with the GLOBAL n_draw, so xi = sum_r xi_r; with S1_r = xi_r and S2_r = xi_r^2 / N_r the effective
+// number of the whole set is (sum S1)^2 / sum S2).  NaN in any piece -> NaN; -inf stays -inf, never NaN.
+__host__ __device__ inline void combine_sharded_one(const double* sum_parts, const double* logxi_parts,
+                                                    const double* neff_parts, int n_parts, int64_t stride,
+                                                    double n_events_total, double* total, double* logxi, double* neff) {
+  const double INF = 1.0 / 0.0;
+  double S = 0.0, m = -INF;
+  bool nan = false;
+  for (int r = 0; r < n_parts; ++r) {
+    const double sr = sum_parts[r * stride], xr = logxi_parts[r * stride];
+    nan = nan || sr != sr || xr != xr;
+    S += sr;
+    m = xr > m ? xr : m;
+  }
+  double lx, ne;
+  if (nan) {
+    lx = ne = S = INF - INF;
+  } else if (!(m > -INF)) {
+    lx = -INF;
+    ne = 0.0;
+  } else {
+    double s1 = 0.0, s2 = 0.0;
+    for (int r = 0; r < n_parts; ++r) {
+      const double e = exp(logxi_parts[r * stride] - m);   // xi_r relative to the largest piece (0 for -inf)
+      const double nr = neff_parts ? neff_parts[r * stride] : 0.0;
+      s1 += e;
+      if (nr > 0.0) s2 += e * e / nr;
+    }
+    lx = m + log(s1);
+    ne = s2 > 0.0 ? s1 * s1 / s2 : 0.0;
+  }
+  double tot;
+  if (nan) tot = INF - INF;
+  else if (S == -INF || lx == -INF) tot = -INF;
+  else tot = S - n_events_total * lx;
+  if (total) *total = tot;
+  if (logxi) *logxi = lx;
+  if (neff) *neff = ne;
+}
+__global__ void combine_sharded_kernel(const double* __restrict__ sum_parts, const double* __restrict__ logxi_parts,
+                                       const double* __restrict__ neff_parts, int n_parts, int64_t n_theta,
+                                       double n_events_total, double* __restrict__ total, double* __restrict__ logxi,
+                                       double* __restrict__ neff) {
+  const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (t >= n_theta) return;
+  combine_sharded_one(sum_parts + t, logxi_parts + t, neff_parts ? neff_parts + t : nullptr, n_parts, n_theta,
+                      n_events_total, total ? total + t : nullptr, logxi ? logxi + t : nullptr,
+                      neff ? neff + t : nullptr);
+}
+
 constexpr int AS_ROWS = 512;  // rows per partial block of the all-sky mean
 template <typename LosT>
 __global__ void allsky_partial_kernel(const LosT* __restrict__ table, int64_t n_rows, int n_z,
@@ -403,6 +455,23 @@ int launch_combine_total(const double* logL, const double* logxi, int64_t n_thet
   if (n_theta <= 0) return 0;
   combine_total_kernel<<<(unsigned)n_theta, TOT_THREADS, 0, s>>>(logL, logxi, n_events, total);
   return ok();
+}
+
+int launch_combine_sharded(const double* sum_parts, const double* logxi_parts, const double* neff_parts, int n_parts,
+                           int64_t n_theta, int64_t n_events_total, double* total, double* logxi, double* neff,
+                           cudaStream_t s) {
+  if (n_theta <= 0) return 0;
+  combine_sharded_kernel<<<(unsigned)((n_theta + 127) / 128), 128, 0, s>>>(sum_parts, logxi_parts, neff_parts, n_parts,
+                                                                          n_theta, (double)n_events_total, total, logxi,
+                                                                          neff);
+  return ok();
+}
+void combine_sharded_host(const double* sum_parts, const double* logxi_parts, const double* neff_parts, int n_parts,
+                          int64_t n_theta, int64_t n_events_total, double* total, double* logxi, double* neff) {
+  for (int64_t t = 0; t < n_theta; ++t)
+    combine_sharded_one(sum_parts + t, logxi_parts + t, neff_parts ? neff_parts + t : nullptr, n_parts, n_theta,
+                        (double)n_events_total, total ? total + t : nullptr, logxi ? logxi + t : nullptr,
+                        neff ? neff + t : nullptr);
 }
 
 size_t allsky_scratch_doubles(int64_t n_rows, int n_z) {

@@ -29,7 +29,8 @@ EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_laun
            "gwc_export_cosmo", "gwc_pack_events", "gwc_cap_pixels", "gwc_los_allsky", "gwc_event_loglik", "gwc_event_loglik_pixcut", "gwc_event_loglik_kde",
            "gwc_selection_logxi",
            "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_pixcut", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_cache_catalogue", "gwc_set_timing", "gwc_get_timing",
-           "gwc_probe_fp64", "gwc_math_selftest", "gwc_los_allsky_static", "gwc_los_allsky_static_error"]
+           "gwc_probe_fp64", "gwc_math_selftest", "gwc_los_allsky_static", "gwc_los_allsky_static_error",
+           "gwc_combine_sharded", "gwc_combine_sharded_host"]
 ALLSKY_STATIC_ROWS_PER_PART = 512
 ALLSKY_STATIC_MAX_DOUBLES = 1 << 19
 
@@ -101,6 +102,8 @@ def load():
         "gwc_get_timing": (ci, [vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64), C.POINTER(dbl)]),
         "gwc_probe_fp64": (ci, [vp, i64, C.POINTER(dbl), C.POINTER(dbl)]),
         "gwc_math_selftest": (ci, [vp, ci, i64, vp, vp]),
+        "gwc_combine_sharded": (ci, [vp, i32, i64, i64, vp, vp, vp, vp, vp, vp]),
+        "gwc_combine_sharded_host": (ci, [i32, i64, i64, vp, vp, vp, vp, vp, vp]),
         "gwc_los_allsky_static": (ci, [C.POINTER(Los), vp, vp]),
         "gwc_los_allsky_static_error": (C.c_char_p, []),
     }
@@ -329,6 +332,33 @@ class Context:
         self._ck(self._lib.gwc_combine_total(self._h, _ptr(logL, torch.float64), _ptr(logxi, torch.float64), nt, ne,
                                              out.data_ptr()))
         return out
+
+    def gwc_combine_sharded(self, sum_logL_parts, logxi_parts, neff_inj_parts, n_events_total: int):
+        """Pieces [n_parts, n_theta] of an event / injection-sharded evaluation (device tensors, rank order) ->
+        (total, logxi, neff_inj), each [n_theta]."""
+        R, nt = sum_logL_parts.shape
+        if tuple(logxi_parts.shape) != (R, nt) or tuple(neff_inj_parts.shape) != (R, nt):
+            raise ValueError("the three piece arrays must have the same [n_parts, n_theta] shape")
+        out = [torch.empty(nt, dtype=torch.float64, device=self.device) for _ in range(3)]
+        self._ck(self._lib.gwc_combine_sharded(self._h, R, nt, int(n_events_total), _ptr(sum_logL_parts, torch.float64),
+                                               _ptr(logxi_parts, torch.float64), _ptr(neff_inj_parts, torch.float64),
+                                               out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr()))
+        return tuple(out)
+
+    @staticmethod
+    def gwc_combine_sharded_host(sum_logL_parts, logxi_parts, neff_inj_parts, n_events_total: int):
+        """gwc_combine_sharded on HOST tensors; needs no context and no GPU."""
+        R, nt = sum_logL_parts.shape
+        if tuple(logxi_parts.shape) != (R, nt) or tuple(neff_inj_parts.shape) != (R, nt):
+            raise ValueError("the three piece arrays must have the same [n_parts, n_theta] shape")
+        out = [torch.empty(nt, dtype=torch.float64) for _ in range(3)]
+        st = load().gwc_combine_sharded_host(R, nt, int(n_events_total), _ptr(sum_logL_parts, torch.float64, False),
+                                             _ptr(logxi_parts, torch.float64, False),
+                                             _ptr(neff_inj_parts, torch.float64, False), out[0].data_ptr(),
+                                             out[1].data_ptr(), out[2].data_ptr())
+        if st != OK:
+            raise GwcError(st, "gwc_combine_sharded_host: bad arguments")
+        return tuple(out)
 
     def gwc_total_loglik(self, theta, ev, inj, table, z_max, allsky, n_nodes=1025, table_prec=F64, out=None):
         nt = theta.shape[0]

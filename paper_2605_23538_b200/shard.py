@@ -1,9 +1,12 @@
-"""theta-sharding over ranks: host logic only, no arithmetic of the method.
+"""Sharding over ranks: host logic only -- index ranges and `torch.distributed` exchanges.  The
+arithmetic of the method stays behind the C ABI: the cross-rank combine of an event / injection-sharded evaluation is
+`gwc_combine_sharded` (device tensors) or `gwc_combine_sharded_host` (host tensors) of libgwc.so.
 
-log L(theta) of one hyper-parameter point needs nothing from any other point, so N GPUs split a batch of
-theta and replicate the catalogue; there is no collective on the data path.  The only communication is
-the gather of the `[n_theta]` results and the max-over-ranks of a device time, both through
-`torch.distributed` (NCCL on GPUs; the CPU tests use gloo).
+theta-sharding: log L(theta) of one hyper-parameter point needs nothing from any other point, so N GPUs split a batch
+of theta and replicate the catalogue; there is no collective on the data path, only the gather of the `[n_theta]`
+results and the max-over-ranks of a device time (NCCL on GPUs; the CPU tests use gloo).
+Event / injection sharding: for the sampler's one-theta-per-call pattern and for catalogues that outgrow one GPU; one
+all-gather of 3 x n_theta doubles per rank, then the combine.
 """
 from __future__ import annotations
 
@@ -51,8 +54,8 @@ def max_over_ranks(value: float, device, group: Optional[dist.ProcessGroup] = No
 # ---- event / injection sharding (SURVEY.md 8e-2): for catalogues that outgrow one GPU or very small theta batches --
 # Each rank owns a contiguous block of events (balanced by samples) and a contiguous block of the found injections,
 # evaluates every theta on them with the ordinary calls (gwc_event_loglik, gwc_selection_logxi with the GLOBAL
-# n_draw), and the ranks exchange two small arrays: an all-reduce of sum_i log L_i  [n_theta]  and an all-gather of
-# (log xi_r, N_eff,r)  [world][n_theta][2], combined in rank order so that every rank gets the same bits.
+# n_draw), and the ranks exchange one small array: an all-gather of (sum_i log L_i, log xi_r, N_eff,r)
+# [world][3][n_theta], combined in rank order by gwc_combine_sharded so that every rank gets the same bits.
 def event_range(ev_sample_off: torch.Tensor, rank: int, world: int) -> Tuple[int, int]:
     """[lo, hi) of the events owned by `rank`: contiguous blocks cut where the cumulative sample count crosses
     k * n_samples / world (every event belongs to exactly one rank; a rank may own none)."""
@@ -70,32 +73,51 @@ def event_range(ev_sample_off: torch.Tensor, rank: int, world: int) -> Tuple[int
     return lo, lo + int((owner == rank).sum())
 
 
+def event_shard(ev: dict, lo: int, hi: int) -> dict:
+    """The sub-catalogue of events [lo, hi): sample arrays sliced, offsets rebased to 0; sample_row keeps the GLOBAL
+    rows of the line-of-sight table, which every rank holds in full.  Indexing only."""
+    off = ev["ev_sample_off"]
+    a, b = int(off[lo]), int(off[hi])
+    sub = {"ev_sample_off": (off[lo:hi + 1] - off[lo]).contiguous()}
+    for k in ("dL", "m1z", "m2z", "sample_row", "log_pe_prior"):
+        v = ev.get(k)
+        sub[k] = None if v is None else v[a:b].contiguous()
+    return sub
+
+
+def injection_shard(inj: dict, rank: int, world: int) -> dict:
+    """Rank `rank`'s contiguous block of the found injections (balanced like theta_range), with the GLOBAL n_draw, so
+    that the xi of the whole set is the sum of the ranks' xi_r."""
+    a, b = theta_range(inj["dL"].numel() if hasattr(inj["dL"], "numel") else len(inj["dL"]), rank, world)
+    sub = {k: inj[k][a:b] for k in ("dL", "m1z", "m2z", "log_pdraw")}
+    sub = {k: (v.contiguous() if hasattr(v, "contiguous") else v) for k, v in sub.items()}
+    sub["n_draw"] = inj["n_draw"]
+    return sub
+
+
 def combine_event_sharded(sum_logL_local: torch.Tensor, logxi_local: torch.Tensor, neff_inj_local: torch.Tensor,
-                          n_events_total: int, group: Optional[dist.ProcessGroup] = None):
+                          n_events_total: int, group: Optional[dist.ProcessGroup] = None, ctx=None):
     """log L(theta) = sum over ALL events of log L_i - n_events_total * log xi from per-rank pieces.
     sum_logL_local [n_theta]: sum of log L_i over this rank's events (0 for a rank without events).
     logxi_local, neff_inj_local [n_theta]: selection term over this rank's injections, computed with the global
-    n_draw, so that xi = sum_r xi_r; N_eff = (sum_r S1_r)^2 / sum_r S2_r with S1_r = xi_r, S2_r = xi_r^2 / N_eff,r.
-    Returns (total, logxi, neff_inj), identical on every rank (fixed rank order)."""
+    n_draw.  The pieces of all ranks are gathered (one all-gather of [3][n_theta]) and combined in rank order by
+    libgwc.so: on the device through `ctx` (a gwc.Context) when the tensors are CUDA tensors, else by the host form.
+    Returns (total, logxi, neff_inj), identical on every rank."""
     world = dist.get_world_size(group)
-    s = sum_logL_local.clone()
-    parts = [torch.empty_like(s) for _ in range(world)]
-    dist.all_gather(parts, s, group=group)                   # gathered, then summed in rank order: same bits everywhere
-    sum_logL = torch.stack(parts, 0).sum(0) if world > 1 else s
-    pair = torch.stack([logxi_local, neff_inj_local], -1).contiguous()
-    pairs = [torch.empty_like(pair) for _ in range(world)]
-    dist.all_gather(pairs, pair, group=group)
-    lx = torch.stack([p[..., 0] for p in pairs], 0)          # [world][n_theta]
-    ne = torch.stack([p[..., 1] for p in pairs], 0)
-    m = lx.max(0).values
-    m_safe = torch.where(torch.isfinite(m), m, torch.zeros_like(m))
-    s1 = torch.exp(lx - m_safe)                              # xi_r relative to e^m  (0 for -inf)
-    s2 = torch.where(ne > 0, s1 * s1 / ne.clamp_min(1e-300), torch.zeros_like(s1))
-    S1, S2 = s1.sum(0), s2.sum(0)
-    logxi = torch.where(S1 > 0, m_safe + torch.log(S1.clamp_min(1e-300)), torch.full_like(m, float("-inf")))
-    neff = torch.where(S2 > 0, S1 * S1 / S2.clamp_min(1e-300), torch.zeros_like(S1))
-    total = sum_logL - float(n_events_total) * logxi
-    total = torch.where(torch.isneginf(sum_logL) | torch.isneginf(logxi), torch.full_like(total, float("-inf")), total)
-    nan = torch.isnan(sum_logL) | torch.isnan(lx).any(0)
-    total = torch.where(nan, torch.full_like(total, float("nan")), total)
-    return total, logxi, neff
+    trio = torch.stack([sum_logL_local, logxi_local, neff_inj_local], 0).to(torch.float64).contiguous()
+    parts = [torch.empty_like(trio) for _ in range(world)]
+    dist.all_gather(parts, trio, group=group)
+    return combine_parts(parts, n_events_total, ctx)
+
+
+def combine_parts(parts, n_events_total: int, ctx=None):
+    """The combine step alone: `parts` is the rank-ordered list of [3][n_theta] tensors (sum log L_i, log xi_r,
+    N_eff,r)."""
+    from . import gwc
+    allp = torch.stack(list(parts), 0)                       # [world][3][n_theta]
+    pieces = [allp[:, k].contiguous() for k in range(3)]
+    if allp.is_cuda:
+        if ctx is None:
+            raise ValueError("CUDA tensors need the gwc.Context to combine on")
+        return ctx.gwc_combine_sharded(pieces[0], pieces[1], pieces[2], n_events_total)
+    return gwc.Context.gwc_combine_sharded_host(pieces[0], pieces[1], pieces[2], n_events_total)

@@ -138,3 +138,43 @@ def test_world2_gloo_event_sharding_matches_single_process(tmp_path):
     np.testing.assert_allclose(got[0][0][fin], ref[fin], rtol=1e-12)
     np.testing.assert_allclose(got[0][1], lx, rtol=0, atol=1e-12)
     np.testing.assert_allclose(got[0][2], ne, rtol=1e-10)
+
+
+def test_combine_sharded_host_closed_forms():
+    """gwc_combine_sharded_host (the function the device kernel also runs) against what the definitions fix:
+    one part is the identity; R equal parts give log xi + ln R and R x N_eff; parts of very different size are summed
+    without overflow; a part without live injections (-inf, N_eff 0) adds nothing; -inf and NaN propagate as gwc.h
+    states; the total is sum_r S_r - n_events log xi."""
+    from paper_2605_23538_b200 import gwc
+    f = gwc.Context.gwc_combine_sharded_host
+    T = lambda rows: torch.tensor(rows, dtype=torch.float64)
+    # one part: identity
+    tot, lx, ne = f(T([[-12.5, 3.0]]), T([[-2.0, 700.0]]), T([[40.0, 7.0]]), 5)
+    assert lx.tolist() == [-2.0, 700.0] and ne.tolist() == [40.0, 7.0]
+    assert tot.tolist() == [-12.5 - 5 * -2.0, 3.0 - 5 * 700.0]
+    # R equal parts
+    R = 4
+    tot, lx, ne = f(T([[1.0]] * R), T([[-3.0]] * R), T([[10.0]] * R), 2)
+    np.testing.assert_allclose(lx.numpy(), [-3.0 + np.log(R)], rtol=1e-15)
+    np.testing.assert_allclose(ne.numpy(), [R * 10.0], rtol=1e-15)
+    np.testing.assert_allclose(tot.numpy(), [R * 1.0 - 2 * (-3.0 + np.log(R))], rtol=1e-15)
+    # very different sizes (no overflow of exp), against numpy's logaddexp; N_eff by the definition in linear terms
+    x = np.array([-900.0, -905.0, 650.0 - 1550.0])
+    n = np.array([3.0, 8.0, 2.0])
+    tot, lx, ne = f(T(x[:, None].tolist()), T(x[:, None].tolist()), T(n[:, None].tolist()), 0)
+    np.testing.assert_allclose(lx.numpy(), [np.logaddexp.reduce(x)], rtol=1e-15)
+    w = np.exp(x - x.max())
+    np.testing.assert_allclose(ne.numpy(), [w.sum() ** 2 / (w ** 2 / n).sum()], rtol=1e-14)
+    np.testing.assert_allclose(tot.numpy(), [x.sum()], rtol=1e-15)
+    # a rank without live injections, a rank without events
+    tot, lx, ne = f(T([[0.0], [-7.0]]), T([[-np.inf], [-4.0]]), T([[0.0], [9.0]]), 3)
+    assert lx.tolist() == [-4.0] and ne.tolist() == [9.0] and tot.tolist() == [-7.0 + 12.0]
+    # -inf stays -inf (never NaN): no live injection anywhere; an event with no live sample
+    tot, lx, ne = f(T([[1.0], [2.0]]), T([[-np.inf], [-np.inf]]), T([[0.0], [0.0]]), 3)
+    assert lx.tolist() == [-np.inf] and ne.tolist() == [0.0] and tot.tolist() == [-np.inf]
+    tot, lx, ne = f(T([[-np.inf], [2.0]]), T([[-1.0], [-1.0]]), T([[5.0], [5.0]]), 3)
+    assert tot.tolist() == [-np.inf] and np.isfinite(lx.numpy()).all()
+    # NaN in any piece of a theta: that theta's outputs are NaN, its neighbour's are not
+    tot, lx, ne = f(T([[1.0, 1.0], [2.0, 2.0]]), T([[-1.0, np.nan], [-1.0, -1.0]]), T([[5.0, 5.0], [5.0, 5.0]]), 3)
+    tot, lx, ne = tot.numpy(), lx.numpy(), ne.numpy()
+    assert np.isnan(tot[1]) and np.isnan(lx[1]) and np.isnan(ne[1]) and np.isfinite(tot[0]) and np.isfinite(lx[0])
