@@ -42,6 +42,65 @@ FP64_INSTR_LIVE = 104.0
 FP64_INSTR_DEAD = 28.0
 FP64_INSTR_EXECUTED = 108.26
 FP64_COUNT_SOURCE = "necessary: static SASS count of the main loop (DESIGN.md 7); executed: ncu op counters, profiles/r02e_reweight_events_ncu_full.md"
+# The counts above belong to ONE build of the fused kernel: profiles/fp64_counts.json records the SHA-256 of that
+# build's SASS (the reweight_kernel functions of libgwc.so, `cuobjdump -sass`).  The bench line carries
+# "count_stale": true when the library it ran hashes differently (the kernel was edited and the counts were not
+# re-measured), null when cuobjdump is not there to tell.
+FP64_COUNTS_FILE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "fp64_counts.json")
+
+
+def reweight_sass_sha256(lib_path):
+    """SHA-256 over the SASS instruction text of every reweight_kernel instantiation in `lib_path`, or None."""
+    import hashlib
+    import re
+    import subprocess
+    try:
+        out = subprocess.run(["cuobjdump", "-sass", lib_path], capture_output=True, text=True, timeout=300).stdout
+    except Exception:
+        return None
+    h, keep, n = hashlib.sha256(), False, 0
+    for line in out.splitlines():
+        if "Function :" in line:
+            keep = "reweight_kernel" in line
+            if keep:
+                h.update(line.split("Function :")[1].strip().encode())
+                n += 1
+            continue
+        if keep:
+            m = re.match(r"\s*/\*[0-9a-f]{4,}\*/\s+(.*?);", line)      # address, instruction text (no encoding words)
+            if m:
+                h.update(m.group(1).encode())
+    return h.hexdigest() if n else None
+
+
+def _load_counts():
+    """The tracked counts replace the constants above when the file is there (same numbers today: the file is what a
+    re-measurement updates, together with the hash of the build it was made on)."""
+    global FP64_INSTR_LIVE, FP64_INSTR_DEAD, FP64_INSTR_EXECUTED, FP64_COUNT_SOURCE
+    import json as _json
+    try:
+        rec = _json.load(open(FP64_COUNTS_FILE))
+        FP64_INSTR_LIVE = float(rec["fp64_instr_per_live_term_necessary"])
+        FP64_INSTR_DEAD = float(rec["fp64_instr_per_dead_term_necessary"])
+        FP64_INSTR_EXECUTED = float(rec["fp64_instr_executed_per_term"]["events_o5"])
+        FP64_COUNT_SOURCE = rec.get("source", FP64_COUNT_SOURCE)
+        return rec
+    except Exception:
+        return None
+
+
+FP64_COUNTS = _load_counts()
+
+
+def fp64_count_state(lib_path):
+    import json as _json
+    try:
+        rec = _json.load(open(FP64_COUNTS_FILE))
+    except Exception:
+        return {"count_stale": None, "counts_file": None}
+    sha = reweight_sass_sha256(lib_path)
+    return {"count_stale": None if sha is None else sha != rec.get("reweight_sass_sha256"),
+            "counts_file": "profiles/fp64_counts.json", "reweight_sass_sha256": sha}
 # the KDE kernel: FP64 thread instructions per Gaussian evaluation, everything included (per-sample weights, per-pixel
 # statistics, prior), measured the same way (profiles/r02f_kde_ncu_full.md)
 KDE_FP64_INSTR_PER_EVAL = 4.81
@@ -146,8 +205,11 @@ def run_leg(args):
     dev = torch.device("cuda", 0)
     spec = _bench_spec(args.workload, args.theta_scale)
     W = synth.make_workload(spec, seed=args.seed, device=dev, keep_f64_los=False)
-    theta = synth.make_theta(spec, args.seed, dev)
+    mp = args.mass_model == "multipeak"
+    theta = (synth.make_theta_multipeak if mp else synth.make_theta)(spec, args.seed, dev)
     ctx = gwc.Context(0)
+    if mp:
+        ctx.gwc_set_mass_model("multipeak")
     zmax = spec.z_max
     prec = gwc.F32 if args.table_prec == "f32" else gwc.F64
     if args.leg == "kde":
@@ -187,7 +249,8 @@ def run_leg(args):
         extra["live_fraction"] = float(r.sum().item()) / units
     else:
         extra["mean_passing_pixels_per_event"] = float(r.double().mean())
-    print(json.dumps(dict({"leg": args.leg, "workload": spec.name, "n_theta": n_theta, "kernel_ms": ms,
+    print(json.dumps(dict({"leg": args.leg, "workload": spec.name, "mass_model": args.mass_model, "n_theta": n_theta,
+                           "kernel_ms": ms,
                            "terms_per_s": units / (ms * 1e-3)}, **extra)))
     ctx.close()
 
@@ -274,7 +337,9 @@ def run_gwc(args):
     h_inj = {k: _pin(v.cpu()) if isinstance(v, torch.Tensor) else v for k, v in W.inj.items()}
     h_los = _pin(W.los.cpu())
     h_out = _pin(torch.empty(n_theta, dtype=torch.float64))
-    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    # (default: as many as the device-resident figure on the small configs, 2 on o5 where a step takes 1.2 s)
+    e2e_cap = args.e2e_steps if args.e2e_steps > 0 else (2 if spec.name == "o5" else args.steps)
+    e2e_steps = max(1, min(args.steps, e2e_cap))
     up = down = 0
     _, up, down = ctx.gwc_total_loglik_host(h_theta, h_ev, h_inj, h_los, zmax, None, args.n_nodes, prec, out=h_out)
     barrier()
@@ -301,10 +366,39 @@ def run_gwc(args):
     ms_inj_kernel = tm["ms_inj"] / max(tm["n_inj"], 1)
     # (MULTIPEAK: + 42 FP64 instructions per live term, static count of the added code, R36)
     instr_live = FP64_INSTR_LIVE + (42.0 if mp else 0.0)
+    # executed FP64 instructions per term, ncu-measured on the workload they are quoted for (profiles/fp64_counts.json)
+    ex = (FP64_COUNTS or {}).get("fp64_instr_executed_per_term", {})
+    if mp:
+        executed = ex.get("events_production_multipeak") if spec.name == "production" else None
+    else:
+        executed = FP64_INSTR_EXECUTED
     instr = terms_ev * (live_frac_ev * instr_live + (1.0 - live_frac_ev) * FP64_INSTR_DEAD)
     achieved = instr * 2.0 / (ms_ev_kernel * 1e-3) / 1e12          # FP64 issue slots x 2 flop
-    peak = FP64_PEAK_INSTR * 2.0 / 1e12
-    probe_ms, probe_n = ctx.gwc_probe_fp64(1 << 13)
+    peak_derived = FP64_PEAK_INSTR * 2.0 / 1e12
+    # the denominator: the dependent-free DFMA probe of this very run (BASELINE.md section 3 asks for a measured FP64
+    # figure; MEASURED_PEAKS.json has none), the best of three; the derived unit-count figure is reported beside it
+    probe = [ctx.gwc_probe_fp64(1 << 13) for _ in range(3)]
+    peak = max(n * 2.0 / (t * 1e-3) / 1e12 for t, n in probe)
+    peak_instr = peak * 1e12 / 2.0
+    # the injection instantiation (the step's second kernel): same formulation, same counts, its own live fraction
+    # (counted by running the injections through the event entry point as 8192-sample pseudo-events on the all-sky row)
+    ctx.gwc_build_cosmo(theta, zmax, args.n_nodes, prec)
+    pseudo_off = torch.arange(0, n_inj + 8192, 8192, dtype=torch.int64, device=dev).clamp_(max=n_inj)
+    pseudo = {"ev_sample_off": pseudo_off, "dL": W.inj["dL"], "m1z": W.inj["m1z"], "m2z": W.inj["m2z"],
+              "log_pe_prior": W.inj["log_pdraw"], "sample_row": torch.zeros(n_inj, dtype=torch.int32, device=dev)}
+    _, _, nlive_inj = ctx.gwc_event_loglik(theta, pseudo, allsky.view(1, -1).contiguous(), zmax, want_neff=False)
+    live_frac_inj = float(nlive_inj.sum().item()) / max(terms_inj, 1.0)
+    del nlive_inj
+    instr_inj = terms_inj * (live_frac_inj * instr_live + (1.0 - live_frac_inj) * FP64_INSTR_DEAD)
+    achieved_inj = instr_inj * 2.0 / (ms_inj_kernel * 1e-3) / 1e12
+    roofline_inj = {"bound": "alu", "kernel": "reweight_kernel<injections>", "kernel_ms": ms_inj_kernel,
+                    "kernel_share_of_step": ms_inj_kernel / (ms / args.steps), "achieved": achieved_inj, "peak": peak,
+                    "unit": "TFLOP/s", "frac": achieved_inj / peak, "frac_vs_derived_peak": achieved_inj / peak_derived,
+                    "live_fraction_injections": live_frac_inj,
+                    "fp64_instr_executed_per_term": None if mp else ex.get("injections_o5"),
+                    "frac_executed": None if mp or not ex.get("injections_o5") else
+                    terms_inj * ex["injections_o5"] / (ms_inj_kernel * 1e-3) / peak_instr,
+                    "note": "same necessary FP64 count per live / dead term as the event instantiation"}
     # DRAM bytes of the event kernel: an ncu figure (a capture, not this run), only for the workload it was taken on;
     # kernel_ms covers the ceil(n_theta / 340) launches of one step, so the traffic is scaled to them
     traffic = O5_DRAM_BYTES_PER_340_THETA * n_theta / 340.0 if spec.name == "o5" and args.table_prec == "f64" else None
@@ -317,15 +411,21 @@ def run_gwc(args):
                 "fp64_instr_per_live_term": instr_live, "fp64_instr_per_dead_term": FP64_INSTR_DEAD,
                 # the instructions the kernel executes per term (ncu-measured), against the same peak: the FP64 pipe's
                 # utilisation as the run itself sees it
-                "fp64_instr_executed_per_term": None if mp else FP64_INSTR_EXECUTED,
-                "frac_executed": None if mp else terms_ev * FP64_INSTR_EXECUTED / (ms_ev_kernel * 1e-3) / FP64_PEAK_INSTR,
+                "fp64_instr_executed_per_term": executed,
+                "frac_executed": None if executed is None else terms_ev * executed / (ms_ev_kernel * 1e-3) / peak_instr,
+                "frac_vs_derived_peak": achieved / peak_derived,
+                "frac_executed_vs_derived_peak": None if executed is None else terms_ev * executed / (ms_ev_kernel * 1e-3)
+                / FP64_PEAK_INSTR,
                 "fp64_count_source": FP64_COUNT_SOURCE,
                 # the same time against the budget BASELINE.md froze before any code (180 live / 30 dead): context only
                 "frac_at_survey_budget_180_30": terms_ev * (live_frac_ev * 180.0 + (1.0 - live_frac_ev) * 30.0)
                 / (ms_ev_kernel * 1e-3) / FP64_PEAK_INSTR,
                 "live_fraction_events": live_frac_ev,
-                "peak_source": "derived: 148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md section 7)",
-                "peak_measured_dfma_probe": probe_n * 2.0 / (probe_ms * 1e-3) / 1e12}
+                "peak_source": "measured in this run: dependent-free DFMA probe on all SMs (gwc_probe_fp64, best of 3)",
+                "peak_derived": peak_derived,
+                "peak_derived_source": "148 SM x 64 FP64 lanes x 1.965 GHz x 2 (DESIGN.md section 7)",
+                "peak_measured_dfma_probe": peak}
+    roofline.update(fp64_count_state(gwc.LIB_PATH))
     # ---- NEXT row 2, reported beside the headline: the event term with the per-pixel N_eff cut (Eq. 8) ----
     pix = None
     if args.pixcut >= 0:
@@ -424,6 +524,7 @@ def run_gwc(args):
                 "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps, "matches_device_path": same},
         "gpu_launches": int(launches),
         "roofline": roofline,
+        "roofline_inj": roofline_inj,
         "cpu_baseline": cpu,
     }
     if stress is not None:
@@ -612,7 +713,7 @@ def main():
     ap.add_argument("--n-nodes", type=int, default=1025)
     ap.add_argument("--seed", type=int, default=synth.DEFAULT_SEED)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle timing budget (0 = skip)")
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=0, help="0 = --steps, but 2 on o5")
     ap.add_argument("--latency-calls", type=int, default=50,
                     help="also time this many one-theta calls with the catalogue cache on (0: skip)")
     ap.add_argument("--kde-theta", type=int, default=16,

@@ -100,8 +100,8 @@ typedef struct gwc_ctx gwc_ctx;
 gwc_status gwc_create(gwc_ctx** ctx, int device, void* cuda_stream);
 void gwc_destroy(gwc_ctx* ctx);
 /* Synchronise the stream and report sticky device errors, then clear them: GWC_ERR_NOT_BUILT (theta changed since
- * the build), GWC_ERR_DOMAIN (a theta point outside the model's domain), GWC_ERR_RANGE (see "Range" above), in
- * that order of precedence; GWC_ERR_CUDA. */
+ * the build), GWC_ERR_INVALID_ARG (a broken GWC_OMEGA_SINGLE promise, gwc_set_omega_hint), GWC_ERR_DOMAIN (a theta
+ * point outside the model's domain), GWC_ERR_RANGE (see "Range" above), in that order of precedence; GWC_ERR_CUDA. */
 gwc_status gwc_check(gwc_ctx* ctx);
 const char* gwc_last_error(const gwc_ctx* ctx);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
@@ -136,6 +136,19 @@ int32_t gwc_theta_len(gwc_mass_model model);
  */
 gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta, double z_max, int32_t n_nodes,
                            gwc_prec table_prec);
+/*
+ * What the caller knows about Omega_m in its theta batches, so that gwc_build_cosmo need not ask the device (and
+ * synchronise) for batches of 40 points and more.  Applies to every later build of this context.
+ *   GWC_OMEGA_DETECT (default): as described above, one synchronisation per large batch.
+ *   GWC_OMEGA_VARIES: never share a table; no question, no synchronisation.  Always correct (a batch that does have a
+ *     single Omega_m merely runs with 10 points per tile instead of 16).
+ *   GWC_OMEGA_SINGLE: the caller promises that every batch has one Omega_m and no point outside the model's domain
+ *     (a population-only analysis with a fixed cosmology): the table is shared without synchronising.  The promise is
+ *     checked on the device all the same: a batch that breaks it raises a sticky flag, gwc_check() returns
+ *     GWC_ERR_INVALID_ARG, and the outputs computed from that build must be discarded.
+ */
+typedef enum { GWC_OMEGA_DETECT = 0, GWC_OMEGA_VARIES = 1, GWC_OMEGA_SINGLE = 2 } gwc_omega_hint;
+gwc_status gwc_set_omega_hint(gwc_ctx* ctx, gwc_omega_hint hint);
 /* Copy the tables of the last gwc_build_cosmo out (widened to f64): d_z, d_dz [n_theta][n_nodes]
  * (dz = du * z'(u_m)), d_umax [n_theta].  Any pointer may be NULL. */
 gwc_status gwc_export_cosmo(gwc_ctx* ctx, double* d_z, double* d_dz, double* d_umax);

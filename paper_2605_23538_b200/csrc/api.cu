@@ -67,6 +67,7 @@ struct gwc_ctx {
   bool fresh_build = false;   // inside gwc_total_loglik*: the build was enqueued by this very call, no verification
   int M = 0, Mp = 0;
   bool tab_shared = false;  // the batch of the last build has one Omega_m: one z(u) table serves every theta
+  int omega_hint = GWC_OMEGA_DETECT;   // gwc_set_omega_hint
   gwc_prec tab_prec = GWC_F64;
   double z_max = 0.0;
   // per-call scratch
@@ -437,6 +438,10 @@ gwc_status gwc_check(gwc_ctx* ctx) {
     if (flag & FLAG_STALE)
       return fail(ctx, GWC_ERR_NOT_BUILT,
                   "d_theta changed after gwc_build_cosmo: the outputs of the changed points are NaN (rebuild first)");
+    if (flag & FLAG_OMEGA)
+      return fail(ctx, GWC_ERR_INVALID_ARG,
+                  "GWC_OMEGA_SINGLE was promised but a theta batch has several Omega_m or a point outside the domain: "
+                  "discard the outputs computed from that build");
     if (flag & FLAG_DOMAIN)
       return fail(ctx, GWC_ERR_DOMAIN, "a theta point is outside the model's domain (its outputs are NaN)");
     if (flag & FLAG_RANGE)
@@ -458,6 +463,14 @@ gwc_status gwc_set_mass_model(gwc_ctx* ctx, gwc_mass_model model) {
   ctx->npar = gwc_theta_len(model);
   ctx->built_theta = nullptr;   // tables and constants of the other model are of no use
   ctx->built_n = 0;
+  return GWC_OK;
+}
+
+gwc_status gwc_set_omega_hint(gwc_ctx* ctx, gwc_omega_hint hint) {
+  if (!ctx) return GWC_ERR_INVALID_ARG;
+  if (hint != GWC_OMEGA_DETECT && hint != GWC_OMEGA_VARIES && hint != GWC_OMEGA_SINGLE)
+    return fail(ctx, GWC_ERR_INVALID_ARG, "unknown Omega_m hint");
+  ctx->omega_hint = (int)hint;
   return GWC_OK;
 }
 
@@ -488,7 +501,12 @@ gwc_status gwc_build_cosmo(gwc_ctx* ctx, const double* d_theta, int64_t n_theta,
   // device (one small kernel and a 4-byte read: the call synchronises) only when it would change the tile.
   ctx->tab_shared = false;
   // (and only for batches of at least four tiles: the synchronisation costs a small batch more than the tile gains)
-  if (n_theta >= 4 * reweight_max_T(Mp, table_prec, false, 2, ctx->smem_optin, false, ctx->model == GWC_MASS_MULTIPEAK, false)) {
+  if (ctx->omega_hint == GWC_OMEGA_SINGLE) {
+    // the caller's promise: shared without waiting; checked on the device, a broken promise raises FLAG_OMEGA
+    GWC_TRY(count(ctx, launch_omega_same(d_theta, n_theta, ctx->model, ctx->d_flag + 2, ctx->stream, ctx->d_flag), "omega_same"));
+    ctx->tab_shared = true;
+  } else if (ctx->omega_hint == GWC_OMEGA_DETECT &&
+             n_theta >= 4 * reweight_max_T(Mp, table_prec, false, 2, ctx->smem_optin, false, ctx->model == GWC_MASS_MULTIPEAK, false)) {
     int same = 0;
     GWC_TRY(count(ctx, launch_omega_same(d_theta, n_theta, ctx->model, ctx->d_flag + 2, ctx->stream), "omega_same"));
     GWC_CUDA(cudaMemcpyAsync(&same, ctx->d_flag + 2, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));

@@ -368,19 +368,23 @@ namespace {
 // One table can serve the batch only if every row is inside the model's domain as well: cosmo_build_kernel writes an
 // all-zero table for a row outside it, and a tile stages the table of its FIRST theta for all of its points.
 __global__ void omega_same_kernel(const double* __restrict__ theta, int64_t n_theta, int npar, int model,
-                                  int* __restrict__ same) {
+                                  int* __restrict__ same, int* __restrict__ flag) {
   const long long ref = __double_as_longlong(theta[1]);
   bool ok = true;
   for (int64_t t = threadIdx.x; t < n_theta; t += blockDim.x)
     ok = ok && __double_as_longlong(theta[t * npar + 1]) == ref && theta_valid(theta + t * npar, model);
   const int all = __syncthreads_and(ok ? 1 : 0);
-  if (threadIdx.x == 0) *same = all;
+  if (threadIdx.x == 0) {
+    *same = all;
+    if (flag && !all) atomicOr(flag, FLAG_OMEGA);
+  }
 }
 }  // namespace
 
-int launch_omega_same(const double* d_theta, int64_t n_theta, int model, int* d_same, cudaStream_t s) {
+int launch_omega_same(const double* d_theta, int64_t n_theta, int model, int* d_same, cudaStream_t s, int* d_flag) {
   if (n_theta <= 0) return 0;
-  omega_same_kernel<<<1, 256, 0, s>>>(d_theta, n_theta, model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR, model, d_same);
+  omega_same_kernel<<<1, 256, 0, s>>>(d_theta, n_theta, model == 1 ? GWC_NPAR_MULTIPEAK : GWC_NPAR, model, d_same,
+                                      d_flag);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -117,6 +117,7 @@ enum : int {
   FLAG_DOMAIN = 1,   // a theta point outside the model's domain (gwc_build_cosmo)
   FLAG_STALE = 4,    // d_theta differs from the copy taken by gwc_build_cosmo
   FLAG_RANGE = 8,    // every live weight of a segment lies below e^-300 of the segment's reference
+  FLAG_OMEGA = 16,   // GWC_OMEGA_SINGLE was promised (gwc_set_omega_hint) and the batch has several Omega_m or an invalid row
   // -DGWC_CHECKED builds only (tests/sanitizer_cases.py): a device-side check failed
   FLAG_CHK_TABLE = 1 << 8,     // index into a z(u) table outside [0, Mp - 2]
   FLAG_CHK_LOS = 1 << 9,       // LOS node index outside [0, n_z - 2], or a row outside the table
@@ -164,7 +165,9 @@ size_t reweight_smem_bytes(int T, int Mp, gwc_prec tab_prec, bool inj, int n_z, 
 int reweight_max_T(int Mp, gwc_prec tab_prec, bool inj, int n_z, int smem_optin, bool pix, bool mp, bool shared_tab);
 // *d_same = 1 when every theta row has the same Omega_m bits and lies inside the model's domain (one z(u) table
 // serves the batch), else 0
-int launch_omega_same(const double* d_theta, int64_t n_theta, int model, int* d_same, cudaStream_t s);
+// d_flag != nullptr: a 0 answer also raises FLAG_OMEGA there (the caller's promise is checked, nobody waits for it)
+int launch_omega_same(const double* d_theta, int64_t n_theta, int model, int* d_same, cudaStream_t s,
+                      int* d_flag = nullptr);
 int reweight_configure(int smem_optin);
 int launch_reweight(const ReweightParams& p, gwc_prec tab_prec, gwc_prec los_prec, bool inj, int n_sm, int device,
                     cudaStream_t s);

@@ -8,15 +8,22 @@
 //   I_j  = trapezoid over the G-node grid on [0, z_max] of f_j(z) p_los(z | row_j) psi(z)/(1+z)
 //   L_i  = (1/S_i) sum_j I_j   over the pixels with n_j >= 2, sigma_j > 0, N_eff,j >= neff_min (Eq. 8)
 //
-// Mapping.  One warp per (theta, event), event-major so that the warps of a CTA share the event's samples in L1.
-// The warp first computes (z_k, v_k) of the whole event, 32 samples at a time with every lane busy, into its slice
-// of a scratch buffer (L1/L2-resident), then walks the event pixel by pixel.  Per pixel it makes three passes over
-// the stored pairs, lanes = samples: moments (sum v, sum v z, sum v^2, n), centred second moment, and the KDE itself,
-// for which the lanes turn into grid nodes (node g = lane + 32 i, i < 8): the (z_k, v_k) of 32 samples at a time are handed round by
-// shuffles and every lane adds v_k N(z_g; z_k, h) into its 8 node sums.  The prior p_los R c_g at the lane's nodes is
-// then applied once per pixel.  Everything is FP64; the Gaussian uses math64.cuh's 7-instruction exp (the hot
-// instruction), the per-sample weight the same exp / ln / rcp / rsqrt as the fused kernel.  All sums run in
-// a fixed order (samples in order inside a lane, butterfly across lanes, pixels in order): bitwise reproducible.
+// Mapping (round 2).  Work units are (chunk, theta), chunk-major, handed to the resident warps
+// of a persistent grid: a chunk is a run of whole pixels of one event of about KDE_CHUNK = 1024 samples (the table is
+// theta-independent, built per call by the kde_chunk_* kernels), so long events spread over many warps and a warp's
+// scratch slice stays L2-resident.  Per-theta values and the prior weights on the grid are computed once per call by
+// kde_theta_prep_kernel.  A warp first computes (z_k, v_k) of its chunk, 32 samples at a time with every lane busy,
+// into its scratch slice; then it takes the chunk 32 samples at a time whatever the pixel boundaries: segmented warp
+// scans give sum v, sum v d, sum v d^2, sum v^2 (d = z minus the pixel's first live redshift: the shifted one-pass
+// variance) at every pixel's last sample, a run left open by one row is carried to the next, and the pixels that pass
+// (n >= 2, variance > 0, N_eff) go through the KDE one after the other.  The KDE pass factorises the Gaussian on the
+// uniform grid: a half-warp lane covers 16 consecutive nodes around a centre c, and with q_c = (z_c - z_k)/(h sqrt 2),
+// beta = dz/(h sqrt 2) the value at node c + o is E P^o C_o, E = exp(-q_c^2), P = exp(-2 beta q_c),
+// C_o = exp(-o^2 beta^2): two exponentials and one reciprocal per (sample, lane) give 16 Gaussians; the two half-warps
+// take alternate samples, two samples per step.  Pixels whose bandwidth is below half a grid step take a direct path
+// (one exponential per node).  The per-chunk partial sums (relative to e^shift of the event) are combined in chunk
+// order by kde_combine_kernel.  Everything is FP64, with math64.cuh's exp / ln / rcp / rsqrt; all sums run in a fixed
+// order (bitwise reproducible).  Measured: 4.81 FP64 instructions per Gaussian evaluation (profiles/r02f).
 #include <math_constants.h>
 
 #include "gwc_internal.h"

@@ -30,7 +30,8 @@ EXPORTS = ["gwc_create", "gwc_destroy", "gwc_check", "gwc_last_error", "gwc_laun
            "gwc_selection_logxi",
            "gwc_combine_total", "gwc_total_loglik", "gwc_total_loglik_pixcut", "gwc_total_loglik_kde", "gwc_total_loglik_host", "gwc_cache_catalogue", "gwc_set_timing", "gwc_get_timing",
            "gwc_probe_fp64", "gwc_math_selftest", "gwc_los_allsky_static", "gwc_los_allsky_static_error",
-           "gwc_combine_sharded", "gwc_combine_sharded_host"]
+           "gwc_combine_sharded", "gwc_combine_sharded_host", "gwc_set_omega_hint"]
+OMEGA_HINTS = {"detect": 0, "varies": 1, "single": 2}
 ALLSKY_STATIC_ROWS_PER_PART = 512
 ALLSKY_STATIC_MAX_DOUBLES = 1 << 19
 
@@ -81,6 +82,7 @@ def load():
         "gwc_launch_count": (i64, [vp]),
         "gwc_set_mass_model": (ci, [vp, ci]),
         "gwc_theta_len": (i32, [ci]),
+        "gwc_set_omega_hint": (ci, [vp, ci]),
         "gwc_build_cosmo": (ci, [vp, vp, i64, dbl, i32, ci]),
         "gwc_export_cosmo": (ci, [vp, vp, vp, vp]),
         "gwc_pack_events": (ci, [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]),
@@ -208,6 +210,12 @@ class Context:
         """"plpeak" (12-column theta rows) or "multipeak" (16 columns; include/gwc.h)."""
         self._ck(self._lib.gwc_set_mass_model(self._h, MASS_MODELS[model]))
         self._npar = int(self._lib.gwc_theta_len(MASS_MODELS[model]))
+
+    def gwc_set_omega_hint(self, hint: str):
+        """"detect" (default: gwc_build_cosmo asks the device and synchronises for batches of 40+ points), "varies"
+        (never share a z(u) table, never synchronise) or "single" (the caller promises one Omega_m per batch and no
+        invalid point; checked on the device, a broken promise -> GWC_ERR_INVALID_ARG from gwc_check)."""
+        self._ck(self._lib.gwc_set_omega_hint(self._h, OMEGA_HINTS[hint]))
 
     def gwc_theta_len(self, model: str) -> int:
         return int(self._lib.gwc_theta_len(MASS_MODELS[model]))

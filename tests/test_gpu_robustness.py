@@ -463,6 +463,45 @@ def test_single_omega_batches_share_one_table(ctx):
         assert_close_log(gL.cpu().numpy(), oL, RTOL_F64, "pixel cut, single Omega_m %s" % (not change))
 
 
+def test_omega_hint(ctx):
+    """gwc_set_omega_hint: what the caller knows about Omega_m replaces the device question (and its stream
+    synchronisation) of gwc_build_cosmo.  "varies" and "single" on a single-Omega_m batch (48 points and 7 points)
+    both match the oracle; "single" on a batch that breaks the promise is reported by gwc_check as
+    GWC_ERR_INVALID_ARG; back on "detect" the same batch is right again."""
+    import oracle
+    from paper_2605_23538_b200 import gwc
+    from util import RTOL_F64, assert_close_log
+    W = workload("o4", n_theta=48, n_events=6, los_rows=400, n_inj=3000)
+    zmax = W.spec.z_max
+    ev, inj, lo = to_dev(W.ev, DEV), to_dev(W.inj, DEV), W.los.to(DEV)
+    allsky = ctx.gwc_los_allsky(lo, zmax)
+    ev_np, inj_np, los_np = synth.to_numpy(W.ev), synth.to_numpy(W.inj), W.los.numpy()
+    o = oracle.total_loglik(W.theta.numpy(), ev_np, inj_np, los_np, zmax)
+    try:
+        for hint in ("varies", "single"):
+            ctx.gwc_set_omega_hint(hint)
+            for n in (48, 7):
+                thd = W.theta[:n].contiguous().to(DEV)
+                total = ctx.gwc_total_loglik(thd, ev, inj, lo, zmax, allsky)
+                ctx.gwc_check()
+                assert_close_log(total.cpu().numpy(), o[:n], RTOL_F64, "log L(theta), hint %s, %d points" % (hint, n))
+        th = W.theta.clone()
+        th[47, 1] = 0.27                                    # the promise of one Omega_m is broken
+        thd = th.to(DEV)
+        ctx.gwc_total_loglik(thd, ev, inj, lo, zmax, allsky)
+        with pytest.raises(gwc.GwcError) as e:
+            ctx.gwc_check()
+        assert e.value.status == gwc.ERR_INVALID_ARG and "GWC_OMEGA_SINGLE" in str(e.value)
+        ctx.gwc_check()
+        ctx.gwc_set_omega_hint("detect")
+        total = ctx.gwc_total_loglik(thd, ev, inj, lo, zmax, allsky)
+        ctx.gwc_check()
+        assert_close_log(total.cpu().numpy(), oracle.total_loglik(th.numpy(), ev_np, inj_np, los_np, zmax), RTOL_F64,
+                         "log L(theta), detect, two Omega_m")
+    finally:
+        ctx.gwc_set_omega_hint("detect")
+
+
 def test_single_omega_batch_with_points_outside_the_domain(ctx):
     """48 theta with one Omega_m, rows 0 and 16 outside the domain (sigma < 0; Omega_m itself valid and equal): they are
     the first points of their 16-point tiles, whose all-zero z(u) table must not be staged for the valid points beside
